@@ -1,0 +1,275 @@
+/*
+ * azint_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, double-precision CPU statement of what the 1D azimuthal-integration hot path computes:
+ * bounding-box pixel splitting as a FORWARD scatter ("loops over all the pixels of the detector, adding their
+ * contributions to the appropriate bins", section 4.1), followed by the ratio of the weighted and
+ * unweighted histograms (section 3.3).  The CUDA path reaches the same sums in another
+ * order (gather / sparse matrix), so this file is the definition it is checked against.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call this library.
+ * It shares no code with paper_1412_6367_b200/csrc and includes none of its headers.
+ *
+ * Steps (notation of DESIGN.md section 3, which restates SURVEY.md section 8(c) O1-O7):
+ *   O1  radial extent [r_min, r_max] of the pixel rectangle   (PAPER.md:50 r = sqrt((x-xc)^2+(y-yc)^2)
+ *       "rectangular box circumscribing the actual pixel")
+ *   O2  unit transform u(r): r, 2theta = atan(r/d), q = 4 pi sin(2theta/2)/lambda
+ *   O3  bins: npt equal-width bins on [u0, u1]; default range = extent of all pixels
+ *   O4  split: outermost bins get their fractional overlap, internal bins share the rest evenly
+ *   O5  per-pixel value v = (I - dark) / (flat * solidangle * polarization)
+ *   O6  S[b] += c v,  C[b] += c
+ *   O7  intensity = S / C
+ *
+ * Parity pins (tests/test_oracle_pins.py): hand-worked split, the 2x2 worked example, mpmath brute force of every
+ * coefficient on tiny images, closed-form ranges, conservation of signal and of pixel count, uniform
+ * image, npt = 1 mean, scipy CSR product, Bragg ring positions, the nnz / row-length statistics of
+ * SURVEY.md section 8(a).  Unpinned: behaviour for non-finite inputs and <= 1 ulp bin-edge ties (reported, not asserted).
+ *
+ * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).  No fast-math; IEEE double throughout.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct {
+    double distance_m, pixel_y_m, pixel_x_m, center_y_px, center_x_px, wavelength_m;
+} aio_geometry;
+
+enum { AIO_R_MM = 0, AIO_TTH_DEG = 1, AIO_TTH_RAD = 2, AIO_Q_NM = 3, AIO_Q_A = 4 };
+
+static double max3(double a, double b, double c) { double m = a > b ? a : b; return m > c ? m : c; }
+static double max2(double a, double b) { return a > b ? a : b; }
+static double min2(double a, double b) { return a < b ? a : b; }
+
+/* O2: radial coordinate in the requested unit, r in metres. */
+static double unit_of_r(double r, const aio_geometry *g, int unit)
+{
+    const double pi = 3.14159265358979323846;
+    switch (unit) {
+    case AIO_R_MM:    return 1e3 * r;
+    case AIO_TTH_RAD: return atan(r / g->distance_m);
+    case AIO_TTH_DEG: return atan(r / g->distance_m) * 180.0 / pi;
+    case AIO_Q_NM:    return 1e-9 * (4.0 * pi * sin(atan(r / g->distance_m) / 2.0) / g->wavelength_m);
+    case AIO_Q_A:     return 1e-10 * (4.0 * pi * sin(atan(r / g->distance_m) / 2.0) / g->wavelength_m);
+    }
+    return NAN;
+}
+
+/* O1 + O2 for pixel (i, j): the pixel occupies [j, j+1] x [i, i+1] in pixel units. */
+static void pixel_bounds(const aio_geometry *g, int unit, int i, int j, double *u_min, double *u_max)
+{
+    double x_lo = ((double)j - g->center_x_px) * g->pixel_x_m;
+    double x_hi = ((double)(j + 1) - g->center_x_px) * g->pixel_x_m;
+    double y_lo = ((double)i - g->center_y_px) * g->pixel_y_m;
+    double y_hi = ((double)(i + 1) - g->center_y_px) * g->pixel_y_m;
+    /* nearest point of the rectangle to the beam centre (0 along an axis the centre projects inside of) */
+    double nx = max3(x_lo, -x_hi, 0.0);
+    double ny = max3(y_lo, -y_hi, 0.0);
+    /* farthest corner */
+    double fx = max2(fabs(x_lo), fabs(x_hi));
+    double fy = max2(fabs(y_lo), fabs(y_hi));
+    double r_min = sqrt(nx * nx + ny * ny);
+    double r_max = sqrt(fx * fx + fy * fy);
+    *u_min = unit_of_r(r_min, g, unit);
+    *u_max = unit_of_r(r_max, g, unit);
+}
+
+int aio_pixel_bounds(const aio_geometry *g, int height, int width, int unit, double *u_min, double *u_max)
+{
+    if (!g || height < 1 || width < 1 || unit < 0 || unit > 4) return -1;
+    for (int i = 0; i < height; ++i)
+        for (int j = 0; j < width; ++j)
+            pixel_bounds(g, unit, i, j, &u_min[(int64_t)i * width + j], &u_max[(int64_t)i * width + j]);
+    return 0;
+}
+
+/* O3: automatic range = [min u_min, max u_max] over ALL pixels (independent of any mask). */
+int aio_auto_range(const double *u_min, const double *u_max, int64_t n, double *u0, double *u1)
+{
+    if (n < 1) return -1;
+    double lo = u_min[0], hi = u_max[0];
+    for (int64_t p = 1; p < n; ++p) {
+        if (u_min[p] < lo) lo = u_min[p];
+        if (u_max[p] > hi) hi = u_max[p];
+    }
+    *u0 = lo; *u1 = hi;
+    return 0;
+}
+
+/*
+ * O4 for one pixel.  In bin units f = (u - u0)/delta the pixel covers [f_min, f_max]; bin b is [b, b+1), the last bin
+ * closed.  Writes up to `cap` (bin, coefficient) pairs and returns how many the pixel has (may exceed cap).
+ *   whole pixel in one bin        -> coefficient 1                         ("no pixel splitting")
+ *   left / right outermost bins   -> (b_min+1-f_min)/w and (f_max-b_max)/w ("calculated first")
+ *   internal bins                 -> 1/w each                              ("evenly distributed")
+ * all of which is  overlap([f_min,f_max], [b,b+1]) / (f_max - f_min).
+ */
+int aio_split(double u_min, double u_max, double u0, double u1, int npt, int *bins, double *coefs, int cap)
+{
+    double delta = (u1 - u0) / (double)npt;
+    double f_min = (u_min - u0) / delta;
+    double f_max = (u_max - u0) / delta;
+    double w = f_max - f_min;
+    int n = 0;
+    if (!(f_max > 0.0) || !(f_min < (double)npt)) return 0;       /* entirely outside the range */
+    if (!(w > 0.0)) {                                               /* degenerate zero-width pixel */
+        int b = (int)floor(f_min);
+        if (b > npt - 1) b = npt - 1;
+        if (b < 0) b = 0;
+        if (cap > 0) { bins[0] = b; coefs[0] = 1.0; }
+        return 1;
+    }
+    double a = max2(f_min, 0.0);
+    double z = min2(f_max, (double)npt);
+    int b_first = (int)floor(a);
+    int b_last = (int)floor(z);
+    if (b_last > npt - 1) b_last = npt - 1;
+    for (int b = b_first; b <= b_last; ++b) {
+        double ov = min2(z, (double)(b + 1)) - max2(a, (double)b);
+        if (ov > 0.0) {
+            if (n < cap) { bins[n] = b; coefs[n] = ov / w; }
+            ++n;
+        }
+    }
+    return n;
+}
+
+#define AIO_MAX_SPLIT 4096
+
+/* O5: corrected value and validity of one pixel. */
+static int pixel_value(int64_t p, const double *image, const double *dark, const double *flat,
+                       const double *solidangle, const double *polarization, const uint8_t *mask, double *v)
+{
+    if (mask && mask[p]) return 0;
+    double den = 1.0;
+    if (flat) den *= flat[p];
+    if (solidangle) den *= solidangle[p];
+    if (polarization) den *= polarization[p];
+    double num = image[p] - (dark ? dark[p] : 0.0);
+    if (den == 0.0 || !isfinite(den) || !isfinite(num)) return 0;
+    *v = num / den;
+    return 1;
+}
+
+/*
+ * O4-O7 as a forward scatter over precomputed pixel bounds (one frame).  This is also the routine bench.py times as the
+ * CPU baseline ("per-frame integrate"): bounds are geometry-only and computed once per detector, as in the paper.
+ * nthreads > 1 uses the paper's own multi-thread scheme: image rows split across threads, one private pair of
+ * histograms per thread, merged at the end (section 3.4.1).  nthreads = 1 is the parity reference.
+ */
+int aio_integrate1d_bounds(const double *u_min, const double *u_max, int64_t npix, int npt, double u0, double u1,
+                           const double *image, const double *dark, const double *flat, const double *solidangle,
+                           const double *polarization, const uint8_t *mask, double empty_value, int nthreads,
+                           double *radial, double *intensity, double *sum_signal, double *count)
+{
+    if (npix < 1 || npt < 1 || !(u1 > u0) || !image) return -1;
+    if (nthreads < 1) nthreads = 1;
+    double delta = (u1 - u0) / (double)npt;
+    double *S = (double *)calloc((size_t)nthreads * npt, sizeof(double));
+    double *C = (double *)calloc((size_t)nthreads * npt, sizeof(double));
+    if (!S || !C) { free(S); free(C); return -2; }
+#ifdef _OPENMP
+#pragma omp parallel num_threads(nthreads)
+#endif
+    {
+        int t = 0, nt = 1;
+#ifdef _OPENMP
+        t = omp_get_thread_num(); nt = omp_get_num_threads();
+#endif
+        double *St = S + (size_t)t * npt, *Ct = C + (size_t)t * npt;
+        int64_t lo = npix * t / nt, hi = npix * (t + 1) / nt;
+        int bins[AIO_MAX_SPLIT]; double coefs[AIO_MAX_SPLIT];
+        for (int64_t p = lo; p < hi; ++p) {
+            double v;
+            if (!pixel_value(p, image, dark, flat, solidangle, polarization, mask, &v)) continue;
+            int n = aio_split(u_min[p], u_max[p], u0, u1, npt, bins, coefs, AIO_MAX_SPLIT);
+            if (n > AIO_MAX_SPLIT) n = AIO_MAX_SPLIT;
+            for (int k = 0; k < n; ++k) {
+                St[bins[k]] += coefs[k] * v;      /* weighted histogram   */
+                Ct[bins[k]] += coefs[k];          /* unweighted histogram */
+            }
+        }
+    }
+    for (int t = 1; t < nthreads; ++t)
+        for (int b = 0; b < npt; ++b) { S[b] += S[(size_t)t * npt + b]; C[b] += C[(size_t)t * npt + b]; }
+    for (int b = 0; b < npt; ++b) {
+        if (radial) radial[b] = u0 + ((double)b + 0.5) * delta;
+        sum_signal[b] = S[b];
+        count[b] = C[b];
+        intensity[b] = C[b] > 0.0 ? S[b] / C[b] : empty_value;
+    }
+    free(S); free(C);
+    return 0;
+}
+
+/* O1-O7 from the geometry (single thread). range_or_null = {u0, u1} or NULL for the automatic range. */
+int aio_integrate1d(const aio_geometry *g, int height, int width, int npt, int unit, const double *range_or_null,
+                    const double *image, const double *dark, const double *flat, const double *solidangle,
+                    const double *polarization, const uint8_t *mask, double empty_value,
+                    double *radial, double *intensity, double *sum_signal, double *count, double *range_out)
+{
+    int64_t n = (int64_t)height * width;
+    double *u_min = (double *)malloc((size_t)n * sizeof(double));
+    double *u_max = (double *)malloc((size_t)n * sizeof(double));
+    if (!u_min || !u_max) { free(u_min); free(u_max); return -2; }
+    int rc = aio_pixel_bounds(g, height, width, unit, u_min, u_max);
+    double u0, u1;
+    if (rc == 0) {
+        if (range_or_null) { u0 = range_or_null[0]; u1 = range_or_null[1]; }
+        else rc = aio_auto_range(u_min, u_max, n, &u0, &u1);
+    }
+    if (rc == 0) {
+        if (range_out) { range_out[0] = u0; range_out[1] = u1; }
+        rc = aio_integrate1d_bounds(u_min, u_max, n, npt, u0, u1, image, dark, flat, solidangle, polarization, mask,
+                                    empty_value, 1, radial, intensity, sum_signal, count);
+    }
+    free(u_min); free(u_max);
+    return rc;
+}
+
+/*
+ * The matrix of the "scatter to gather" transformation in scipy-compatible CSR form
+ * (data / indices / indptr): the triplets of O4 taken in pixel order and counting-sorted by bin, so
+ * that column indices ascend within a row.  Two calls: indices == NULL returns nnz and fills indptr only.
+ */
+int64_t aio_csr(const double *u_min, const double *u_max, int64_t npix, int npt, double u0, double u1,
+                int64_t *indptr, int32_t *indices, double *data)
+{
+    int bins[AIO_MAX_SPLIT]; double coefs[AIO_MAX_SPLIT];
+    int64_t *len = (int64_t *)calloc((size_t)npt + 1, sizeof(int64_t));
+    if (!len) return -2;
+    for (int64_t p = 0; p < npix; ++p) {
+        int n = aio_split(u_min[p], u_max[p], u0, u1, npt, bins, coefs, AIO_MAX_SPLIT);
+        if (n > AIO_MAX_SPLIT) { free(len); return -3; }
+        for (int k = 0; k < n; ++k) len[bins[k]]++;
+    }
+    indptr[0] = 0;
+    for (int b = 0; b < npt; ++b) indptr[b + 1] = indptr[b] + len[b];
+    int64_t nnz = indptr[npt];
+    if (indices && data) {
+        for (int b = 0; b < npt; ++b) len[b] = indptr[b];      /* running cursors */
+        for (int64_t p = 0; p < npix; ++p) {
+            int n = aio_split(u_min[p], u_max[p], u0, u1, npt, bins, coefs, AIO_MAX_SPLIT);
+            for (int k = 0; k < n; ++k) {
+                int64_t pos = len[bins[k]]++;
+                indices[pos] = (int32_t)p;
+                data[pos] = coefs[k];
+            }
+        }
+    }
+    free(len);
+    return nnz;
+}
+
+int aio_num_threads_available(void)
+{
+#ifdef _OPENMP
+    return omp_get_num_procs();
+#else
+    return 1;
+#endif
+}
