@@ -1,0 +1,143 @@
+/*
+ * azint.h -- C ABI of libazint: the 1D azimuthal-integration hot path of arxiv 1412.6367 (pyFAI) on one B200.
+ *
+ * What the library computes (citations are PAPER.md lines; DESIGN.md section 3 holds the exact definition O1-O7):
+ *   - per-pixel radial bounds of the pixel's bounding box in r, 2theta or q   (PAPER.md:32-41 section 3, :50, :120)
+ *   - the bounding-box pixel-splitting matrix "bin <- (pixel, weight)" in CSR form: data / indices / indptr,
+ *     scipy.sparse.csr_matrix compatible                                      (PAPER.md:122 section 4.1, :159-180)
+ *   - per frame: cast + dark / flat / solid-angle / polarisation / mask correction in one pass over the pixels
+ *     (PAPER.md:240), the sparse matrix x dense vector product with compensated accumulation and the
+ *     three outputs weighted histogram, unweighted histogram and their ratio
+ *
+ * Conventions
+ *   - Every function returns AI_OK (0) or a negative ai_status; nothing throws or aborts across this boundary.
+ *   - "DEVICE pointer" = CUDA global memory on the current device; "HOST pointer" = ordinary host memory.
+ *     The caller owns every buffer it passes in; the library never frees, keeps or modifies them beyond the
+ *     documented outputs.  The library owns the context, the matrix and its scratch buffers.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).  ai_integrate1d* only ENQUEUE work on that
+ *     stream and return without synchronising.  ai_build_csr synchronises the stream (it reads nnz back to size the
+ *     matrix).  One context must not be used from two streams at once (it owns per-call scratch).
+ *   - Image layout: height x width, row-major, linear pixel index p = i*width + j (i = slow / y, j = fast / x).  Pixel
+ *     (i, j) covers [j, j+1] x [i, i+1] in pixel units; the beam centre is given in the same units.
+ *   - Frames and correction arrays need only their natural alignment (4 bytes for 32-bit, 2 bytes for 16-bit types).
+ */
+#ifndef AZINT_H
+#define AZINT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ai_ctx ai_ctx; /* opaque, library-owned */
+
+typedef enum {
+    AI_OK = 0,
+    AI_EINVAL = -1,    /* bad shape, npt < 1, non-positive distance / pixel / wavelength, NULL required pointer, u1 <= u0 */
+    AI_ENOTBUILT = -2, /* integrate or get_csr before ai_build_csr */
+    AI_ECUDA = -3,     /* a CUDA call failed; text kept for ai_last_error */
+    AI_ENOMEM = -4,    /* host or device allocation failed */
+    AI_EUNSUPPORTED = -5 /* e.g. a matrix with more than 2^31-1 entries or a LUT that would exceed device memory */
+} ai_status;
+
+/* radial unit u(r): r in mm; 2theta = atan(r/d) in degrees or radians;
+ * q = 4 pi sin(2theta / 2) / lambda in nm^-1 or A^-1 */
+typedef enum { AI_R_MM = 0, AI_TTH_DEG = 1, AI_TTH_RAD = 2, AI_Q_NM = 3, AI_Q_A = 4 } ai_unit;
+
+/* dtype of the raw frame: "16 or 32 bits (int or uint)" or float32 */
+typedef enum { AI_F32 = 0, AI_I32 = 1, AI_U16 = 2, AI_I16 = 3, AI_U32 = 4 } ai_dtype;
+
+/* execution layout of the matrix.
+ *   AI_LAYOUT_TILED  B200 design: the CSR re-ordered by image tile, tiles staged in shared memory
+ *   AI_LAYOUT_CSR    the canonical CSR applied row by row, one thread block per bin
+ *   AI_LAYOUT_LUT    padded look-up table, one thread per bin                              */
+typedef enum { AI_LAYOUT_TILED = 0, AI_LAYOUT_CSR = 1, AI_LAYOUT_LUT = 2 } ai_layout;
+
+/* accumulator arithmetic: fp32 with Kahan compensation, plain fp32, or fp64 */
+typedef enum { AI_ACC_F32_KAHAN = 0, AI_ACC_F32_PLAIN = 1, AI_ACC_F64 = 2 } ai_accum;
+
+/* planar detector orthogonal to the beam; lengths in metres, centre in pixels */
+typedef struct {
+    double distance_m;
+    double pixel_y_m, pixel_x_m;
+    double center_y_px, center_x_px;
+    double wavelength_m;
+} ai_geometry;
+
+/* Create a context (host work only, no device allocation yet).
+ *   out             receives the context; destroy with ai_destroy
+ *   g               geometry; distance, pixel sizes > 0; wavelength > 0 (only used by the q units)
+ *   height, width   detector shape in pixels, >= 1
+ *   npt             number of radial bins, >= 1
+ *   range_or_null   HOST pointer to {u0, u1} in `unit`, u1 > u0; NULL = [min u_min, max u_max] over all pixels
+ * Errors: AI_EINVAL, AI_ENOMEM. */
+int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt, ai_unit unit,
+             const double *range_or_null);
+
+/* Build the matrix on the device: bounds -> range -> count -> exclusive scan -> ordered fill (PAPER.md:120-122 for
+ * the coefficients, :150 scan, :180 CSR), then the tiled execution layout.  Idempotent.  Synchronises `cuda_stream`.
+ * Errors: AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED. */
+int ai_build_csr(ai_ctx *ctx, void *cuda_stream);
+
+/* Borrow the canonical CSR (DEVICE pointers, valid until ai_destroy): indptr[npt+1], indices[nnz] ascending within
+ * each row, data[nnz] float32.  Any output pointer may be NULL.  u0/u1 = the range in use.
+ * Errors: AI_ENOTBUILT. */
+int ai_get_csr(const ai_ctx *ctx, const int32_t **indptr, const int32_t **indices, const float **data,
+               int64_t *nnz, double *u0, double *u1);
+
+/* Choose execution layout, accumulator and the intensity written to bins with count == 0 (default: TILED, KAHAN, 0).
+ * AI_LAYOUT_LUT builds the padded table on first use (inside the next integrate call's stream).
+ * Errors: AI_EINVAL. */
+int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_value);
+
+/* Integrate one frame.  All pointers are DEVICE pointers.
+ *   image                      height*width elements of `dtype`
+ *   dark, flat, solidangle,
+ *   polarization               float32[height*width] or NULL (absent = 0 for dark, 1 for the others)
+ *   mask                       uint8[height*width] or NULL; mask != 0 => pixel ignored
+ *   radial                     float32[npt] bin centres u0 + (b + 1/2) delta, may be NULL
+ *   intensity, sum_signal,
+ *   count                      float32[npt] each, required:  sum_signal_b = sum_k c_k v_k, count_b = sum_k c_k valid_k,
+ *                              intensity_b = sum_signal_b / count_b (empty_value where count_b == 0), with
+ *                              v = (I - dark) / (flat * solidangle * polarization); a pixel is invalid if masked or if
+ *                              its denominator is 0 / non-finite or its numerator non-finite.
+ * Enqueues on `cuda_stream`; does not synchronise.  Errors: AI_EINVAL, AI_ENOTBUILT, AI_ECUDA. */
+int ai_integrate1d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *dark, const float *flat,
+                   const float *solidangle, const float *polarization, const uint8_t *mask, float *radial,
+                   float *intensity, float *sum_signal, float *count, void *cuda_stream);
+
+/* Integrate `nframes` frames that share one matrix and one set of correction arrays (a detector streaming frames,
+ * PAPER.md:11); the matrix is read once per group of frames.  All pointers are DEVICE pointers.
+ *   frames                     frame f starts at element f * frame_stride_elems (>= height*width)
+ *   intensity, sum_signal,
+ *   count                      float32[nframes][npt], row-major
+ * Enqueues on `cuda_stream`; does not synchronise.  Errors as ai_integrate1d. */
+int ai_integrate1d_batch(ai_ctx *ctx, const void *frames, ai_dtype dtype, int nframes, int64_t frame_stride_elems,
+                         const float *dark, const float *flat, const float *solidangle, const float *polarization,
+                         const uint8_t *mask, float *intensity, float *sum_signal, float *count, void *cuda_stream);
+
+/* End-to-end variant: `image_host` and the three outputs are HOST pointers (pinned memory makes the copies
+ * asynchronous); correction arrays and mask stay DEVICE pointers (they are per-detector constants, uploaded once, as in
+ * PAPER.md:240-254 where only the image crosses the bus per frame).  Copies the frame host->device, integrates, copies
+ * the 3*npt results device->host and synchronises `cuda_stream` before returning.
+ * Errors as ai_integrate1d. */
+int ai_integrate1d_host(ai_ctx *ctx, const void *image_host, ai_dtype dtype, const float *dark, const float *flat,
+                        const float *solidangle, const float *polarization, const uint8_t *mask,
+                        float *intensity_host, float *sum_signal_host, float *count_host, void *cuda_stream);
+
+/* Number of kernels the last ai_integrate1d* call launched (for accounting in benchmarks). */
+int ai_last_launch_count(const ai_ctx *ctx);
+
+/* Release the context, the matrix and all scratch memory.  NULL is allowed. */
+void ai_destroy(ai_ctx *ctx);
+
+/* Static description of a status code. */
+const char *ai_strerror(int code);
+/* Text of the last error on this context ("" if none); valid until the next call on the context. */
+const char *ai_last_error(const ai_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AZINT_H */

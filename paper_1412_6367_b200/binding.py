@@ -1,0 +1,234 @@
+"""Thin ctypes binding of include/azint.h -- argument marshalling only.
+
+Functions carry the C names (ai_setup, ai_build_csr, ai_get_csr, ai_set_options, ai_integrate1d,
+ai_integrate1d_batch, ai_integrate1d_host, ai_destroy); `Integrator` bundles a context with them.  PyTorch supplies
+device memory and streams, nothing else.  The library is loaded from this directory (built by
+`python -m paper_1412_6367_b200.build`); if it is missing the import of `lib()` fails loudly -- there is no fallback.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libazint.so")
+
+# enums of include/azint.h
+AI_R_MM, AI_TTH_DEG, AI_TTH_RAD, AI_Q_NM, AI_Q_A = range(5)
+AI_F32, AI_I32, AI_U16, AI_I16, AI_U32 = range(5)
+AI_LAYOUT_TILED, AI_LAYOUT_CSR, AI_LAYOUT_LUT = range(3)
+AI_ACC_F32_KAHAN, AI_ACC_F32_PLAIN, AI_ACC_F64 = range(3)
+AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
+
+EXPORTS = ["ai_setup", "ai_build_csr", "ai_get_csr", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
+           "ai_integrate1d_host", "ai_last_launch_count", "ai_destroy", "ai_strerror", "ai_last_error"]
+
+
+class ai_geometry(C.Structure):
+    _fields_ = [(n, C.c_double) for n in
+                ("distance_m", "pixel_y_m", "pixel_x_m", "center_y_px", "center_x_px", "wavelength_m")]
+
+
+class AzintError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__(f"libazint status {code}: {text}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libazint.so (once).  Raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_1412_6367_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, dp, fp = C.c_void_p, C.POINTER(C.c_double), C.c_void_p
+    L.ai_setup.argtypes = [C.POINTER(vp), C.POINTER(ai_geometry), C.c_int, C.c_int, C.c_int, C.c_int, dp]
+    L.ai_build_csr.argtypes = [vp, vp]
+    L.ai_get_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int64), dp, dp]
+    L.ai_set_options.argtypes = [vp, C.c_int, C.c_int, C.c_float]
+    L.ai_integrate1d.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
+    L.ai_integrate1d_batch.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
+    L.ai_integrate1d_host.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, vp]
+    L.ai_last_launch_count.argtypes = [vp]
+    L.ai_destroy.argtypes = [vp]
+    L.ai_destroy.restype = None
+    L.ai_strerror.argtypes = [C.c_int]
+    L.ai_strerror.restype = C.c_char_p
+    L.ai_last_error.argtypes = [vp]
+    L.ai_last_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc, ctx=None):
+    if rc != AI_OK:
+        L = lib()
+        text = L.ai_strerror(rc).decode()
+        if ctx:
+            extra = L.ai_last_error(ctx).decode()
+            if extra:
+                text += ": " + extra
+        raise AzintError(rc, text)
+
+
+def _ptr(t):
+    """Device (torch tensor) or host (numpy array) address, or None."""
+    if t is None:
+        return None
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+_DTYPES = {"float32": AI_F32, "int32": AI_I32, "uint16": AI_U16, "int16": AI_I16, "uint32": AI_U32}
+
+
+def dtype_code(t) -> int:
+    name = str(t.dtype).replace("torch.", "")
+    if name not in _DTYPES:
+        raise AzintError(AI_EINVAL, f"unsupported frame dtype {name}")
+    return _DTYPES[name]
+
+
+# ---- functions named after the C entry points -------------------------------------------------------------------------
+def ai_setup(distance_m, pixel_y_m, pixel_x_m, center_y_px, center_x_px, wavelength_m, height, width, npt, unit,
+             radial_range=None):
+    g = ai_geometry(distance_m, pixel_y_m, pixel_x_m, center_y_px, center_x_px, wavelength_m)
+    ctx = C.c_void_p()
+    rng = None if radial_range is None else (C.c_double * 2)(*radial_range)
+    _check(lib().ai_setup(C.byref(ctx), C.byref(g), height, width, npt, unit, rng))
+    return ctx
+
+
+def ai_build_csr(ctx, stream=None):
+    _check(lib().ai_build_csr(ctx, _stream(stream)), ctx)
+
+
+def ai_get_csr(ctx):
+    """(indptr_ptr, indices_ptr, data_ptr, nnz, u0, u1): borrowed DEVICE addresses."""
+    a, b, c = C.c_void_p(), C.c_void_p(), C.c_void_p()
+    nnz, u0, u1 = C.c_int64(), C.c_double(), C.c_double()
+    _check(lib().ai_get_csr(ctx, C.byref(a), C.byref(b), C.byref(c), C.byref(nnz), C.byref(u0), C.byref(u1)), ctx)
+    return a.value, b.value, c.value, nnz.value, u0.value, u1.value
+
+
+def ai_set_options(ctx, layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN, empty_value=0.0):
+    _check(lib().ai_set_options(ctx, layout, accum, empty_value), ctx)
+
+
+def ai_integrate1d(ctx, image, dark, flat, solidangle, polarization, mask, radial, intensity, sum_signal, count,
+                   stream=None, dtype=None):
+    _check(lib().ai_integrate1d(ctx, _ptr(image), dtype_code(image) if dtype is None else dtype, _ptr(dark),
+                                _ptr(flat), _ptr(solidangle), _ptr(polarization), _ptr(mask), _ptr(radial),
+                                _ptr(intensity), _ptr(sum_signal), _ptr(count), _stream(stream)), ctx)
+
+
+def ai_integrate1d_batch(ctx, frames, nframes, frame_stride_elems, dark, flat, solidangle, polarization, mask,
+                         intensity, sum_signal, count, stream=None, dtype=None):
+    _check(lib().ai_integrate1d_batch(ctx, _ptr(frames), dtype_code(frames) if dtype is None else dtype, nframes,
+                                      frame_stride_elems, _ptr(dark), _ptr(flat), _ptr(solidangle),
+                                      _ptr(polarization), _ptr(mask), _ptr(intensity), _ptr(sum_signal), _ptr(count),
+                                      _stream(stream)), ctx)
+
+
+def ai_integrate1d_host(ctx, image_host, dark, flat, solidangle, polarization, mask, intensity_host, sum_signal_host,
+                        count_host, stream=None, dtype=None):
+    _check(lib().ai_integrate1d_host(ctx, _ptr(image_host), dtype_code(image_host) if dtype is None else dtype,
+                                     _ptr(dark), _ptr(flat), _ptr(solidangle), _ptr(polarization), _ptr(mask),
+                                     _ptr(intensity_host), _ptr(sum_signal_host), _ptr(count_host), _stream(stream)),
+           ctx)
+
+
+def ai_last_launch_count(ctx) -> int:
+    return int(lib().ai_last_launch_count(ctx))
+
+
+def ai_destroy(ctx):
+    lib().ai_destroy(ctx)
+
+
+# ---- convenience holder (still marshalling only) ------------------------------------------------------------------------
+class Integrator:
+    """A context for one detector geometry: setup + build at construction, integrate per frame.
+
+    cfg: object with height, width, pixel_m, distance_m, wavelength_m, center_x_px, center_y_px, unit, npt
+    (e.g. workloads.Config).  Outputs are torch float32 CUDA tensors allocated here for convenience."""
+
+    def __init__(self, cfg, radial_range=None, device="cuda:0", layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN,
+                 empty_value=0.0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1412_6367_b200 needs a CUDA device (no CPU fallback)")
+        self.torch = torch
+        self.device = torch.device(device)
+        self.cfg = cfg
+        self.npt = cfg.npt
+        self.ctx = ai_setup(cfg.distance_m, cfg.pixel_m, cfg.pixel_m, cfg.center_y_px, cfg.center_x_px,
+                            cfg.wavelength_m, cfg.height, cfg.width, cfg.npt, cfg.unit, radial_range)
+        with torch.cuda.device(self.device):
+            ai_build_csr(self.ctx)
+        ai_set_options(self.ctx, layout, accum, empty_value)
+
+    def set_options(self, layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN, empty_value=0.0):
+        ai_set_options(self.ctx, layout, accum, empty_value)
+
+    def csr(self):
+        """Canonical CSR as torch tensors copied out of the borrowed device arrays (indptr, indices, data), + range."""
+        torch = self.torch
+        a, b, c, nnz, u0, u1 = ai_get_csr(self.ctx)
+
+        def view(ptr, n, dt):
+            import numpy as np
+            host = np.empty(n, dtype=dt)
+            if n:
+                rc = torch.cuda.cudart().cudaMemcpy(host.ctypes.data, ptr, host.nbytes, 2)   # 2 = DeviceToHost
+                if int(rc) != 0:
+                    raise AzintError(AI_ECUDA, f"cudaMemcpy failed: {rc}")
+            return host
+        import numpy as np
+        return view(a, self.npt + 1, np.int32), view(b, nnz, np.int32), view(c, nnz, np.float32), (u0, u1)
+
+    def outputs(self, nframes=None):
+        shape = (self.npt,) if nframes is None else (nframes, self.npt)
+        t = self.torch
+        return tuple(t.empty(shape, dtype=t.float32, device=self.device) for _ in range(3))
+
+    def integrate1d(self, image, dark=None, flat=None, solidangle=None, polarization=None, mask=None, out=None,
+                    radial=None):
+        """Returns (intensity, sum_signal, count) device tensors; enqueues on the current stream."""
+        intensity, sum_signal, count = out if out is not None else self.outputs()
+        ai_integrate1d(self.ctx, image, dark, flat, solidangle, polarization, mask, radial, intensity, sum_signal,
+                       count)
+        return intensity, sum_signal, count
+
+    def integrate1d_batch(self, frames, dark=None, flat=None, solidangle=None, polarization=None, mask=None,
+                          out=None):
+        nframes = frames.shape[0]
+        intensity, sum_signal, count = out if out is not None else self.outputs(nframes)
+        ai_integrate1d_batch(self.ctx, frames, nframes, frames.stride(0), dark, flat, solidangle, polarization, mask,
+                             intensity, sum_signal, count)
+        return intensity, sum_signal, count
+
+    def close(self):
+        if self.ctx is not None:
+            ai_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,193 @@
+// C ABI entry points of libazint (include/azint.h): argument checks, context life cycle, dispatch to the kernels.
+#include <math.h>
+#include <stdarg.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "ctx.h"
+
+int ai_fail(ai_ctx *ctx, int code, const char *fmt, ...)
+{
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+extern "C" {
+
+const char *ai_strerror(int code)
+{
+    switch (code) {
+    case AI_OK: return "ok";
+    case AI_EINVAL: return "invalid argument";
+    case AI_ENOTBUILT: return "matrix not built (call ai_build_csr first)";
+    case AI_ECUDA: return "CUDA error";
+    case AI_ENOMEM: return "out of memory";
+    case AI_EUNSUPPORTED: return "unsupported size";
+    }
+    return "unknown status";
+}
+
+const char *ai_last_error(const ai_ctx *ctx) { return ctx ? ctx->err : ""; }
+
+int ai_last_launch_count(const ai_ctx *ctx) { return ctx ? ctx->last_launches : 0; }
+
+int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt, ai_unit unit,
+             const double *range_or_null)
+{
+    if (!out) return AI_EINVAL;
+    *out = nullptr;
+    if (!g || height < 1 || width < 1 || npt < 1) return AI_EINVAL;
+    if ((int)unit < AI_R_MM || (int)unit > AI_Q_A) return AI_EINVAL;
+    if (!(g->distance_m > 0.0) || !(g->pixel_x_m > 0.0) || !(g->pixel_y_m > 0.0) || !(g->wavelength_m > 0.0)) return AI_EINVAL;
+    if (!isfinite(g->distance_m) || !isfinite(g->pixel_x_m) || !isfinite(g->pixel_y_m) || !isfinite(g->wavelength_m) ||
+        !isfinite(g->center_x_px) || !isfinite(g->center_y_px))
+        return AI_EINVAL;
+    if ((int64_t)height * width > 0x7fffffffLL) return AI_EUNSUPPORTED;     // pixel indices are int32
+    if (range_or_null && !(range_or_null[1] > range_or_null[0] && isfinite(range_or_null[0]) && isfinite(range_or_null[1])))
+        return AI_EINVAL;
+    ai_ctx *ctx = new (std::nothrow) ai_ctx();
+    if (!ctx) return AI_ENOMEM;
+    ctx->geo = *g;
+    ctx->height = height;
+    ctx->width = width;
+    ctx->npt = npt;
+    ctx->unit = unit;
+    if (range_or_null) {
+        ctx->user_range = true;
+        ctx->range_host[0] = range_or_null[0];
+        ctx->range_host[1] = range_or_null[1];
+    }
+    *out = ctx;
+    return AI_OK;
+}
+
+int ai_build_csr(ai_ctx *ctx, void *cuda_stream)
+{
+    if (!ctx) return AI_EINVAL;
+    if (ctx->built) return AI_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    AI_CUDA(ctx, cudaGetDevice(&ctx->device));
+    AI_CUDA(ctx, cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device));
+    PixelSpans spans;
+    int rc = ai_build_canonical(ctx, &spans, st);
+    if (rc == AI_OK) rc = ai_build_tiled(ctx, spans, st);
+    ai_free_spans(&spans);
+    if (rc != AI_OK) return rc;
+    AI_CUDA(ctx, cudaMalloc(&ctx->out_dev, 3 * (size_t)ctx->npt * sizeof(float)));
+    ctx->built = true;
+    return AI_OK;
+}
+
+int ai_get_csr(const ai_ctx *ctx, const int32_t **indptr, const int32_t **indices, const float **data, int64_t *nnz,
+               double *u0, double *u1)
+{
+    if (!ctx) return AI_EINVAL;
+    if (!ctx->built) return AI_ENOTBUILT;
+    if (indptr) *indptr = ctx->indptr;
+    if (indices) *indices = ctx->indices;
+    if (data) *data = ctx->data;
+    if (nnz) *nnz = ctx->nnz;
+    if (u0) *u0 = ctx->range_host[0];
+    if (u1) *u1 = ctx->range_host[1];
+    return AI_OK;
+}
+
+int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_value)
+{
+    if (!ctx) return AI_EINVAL;
+    if ((int)layout < AI_LAYOUT_TILED || (int)layout > AI_LAYOUT_LUT) return ai_fail(ctx, AI_EINVAL, "bad layout %d", (int)layout);
+    if ((int)accum < AI_ACC_F32_KAHAN || (int)accum > AI_ACC_F64) return ai_fail(ctx, AI_EINVAL, "bad accum %d", (int)accum);
+    ctx->layout = layout;
+    ctx->accum = accum;
+    ctx->empty_value = empty_value;
+    return AI_OK;
+}
+
+static int integrate(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
+{
+    if (!ctx) return AI_EINVAL;
+    if (!ctx->built) return ai_fail(ctx, AI_ENOTBUILT, "ai_build_csr has not been called");
+    if (!a.image || !a.intensity || !a.sum_signal || !a.count) return ai_fail(ctx, AI_EINVAL, "NULL image or output");
+    if ((int)a.dtype < AI_F32 || (int)a.dtype > AI_U32) return ai_fail(ctx, AI_EINVAL, "bad dtype %d", (int)a.dtype);
+    if (a.nframes < 1) return ai_fail(ctx, AI_EINVAL, "nframes < 1");
+    if (a.frame_stride < (int64_t)ctx->height * ctx->width) return ai_fail(ctx, AI_EINVAL, "frame stride < height*width");
+    switch (ctx->layout) {
+    case AI_LAYOUT_TILED: return ai_launch_tiled(ctx, a, st);
+    case AI_LAYOUT_CSR: return ai_launch_csr(ctx, a, st);
+    case AI_LAYOUT_LUT: return ai_launch_lut(ctx, a, st);
+    }
+    return AI_EINVAL;
+}
+
+int ai_integrate1d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *dark, const float *flat,
+                   const float *solidangle, const float *polarization, const uint8_t *mask, float *radial,
+                   float *intensity, float *sum_signal, float *count, void *cuda_stream)
+{
+    if (!ctx) return AI_EINVAL;
+    FrameArgs a{image, dtype, dark, flat, solidangle, polarization, mask, radial, intensity, sum_signal, count, 1,
+                (int64_t)ctx->height * ctx->width};
+    return integrate(ctx, a, (cudaStream_t)cuda_stream);
+}
+
+int ai_integrate1d_batch(ai_ctx *ctx, const void *frames, ai_dtype dtype, int nframes, int64_t frame_stride_elems,
+                         const float *dark, const float *flat, const float *solidangle, const float *polarization,
+                         const uint8_t *mask, float *intensity, float *sum_signal, float *count, void *cuda_stream)
+{
+    if (!ctx) return AI_EINVAL;
+    FrameArgs a{frames, dtype, dark, flat, solidangle, polarization, mask, nullptr, intensity, sum_signal, count,
+                nframes, frame_stride_elems};
+    return integrate(ctx, a, (cudaStream_t)cuda_stream);
+}
+
+int ai_integrate1d_host(ai_ctx *ctx, const void *image_host, ai_dtype dtype, const float *dark, const float *flat,
+                        const float *solidangle, const float *polarization, const uint8_t *mask,
+                        float *intensity_host, float *sum_signal_host, float *count_host, void *cuda_stream)
+{
+    if (!ctx) return AI_EINVAL;
+    if (!ctx->built) return ai_fail(ctx, AI_ENOTBUILT, "ai_build_csr has not been called");
+    if (!image_host || !intensity_host || !sum_signal_host || !count_host) return ai_fail(ctx, AI_EINVAL, "NULL image or output");
+    if ((int)dtype < AI_F32 || (int)dtype > AI_U32) return ai_fail(ctx, AI_EINVAL, "bad dtype %d", (int)dtype);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t esz = (dtype == AI_U16 || dtype == AI_I16) ? 2 : 4;
+    const size_t bytes = (size_t)ctx->height * ctx->width * esz;
+    if (ctx->staging_bytes < bytes) {
+        if (ctx->staging) AI_CUDA(ctx, cudaFree(ctx->staging));
+        ctx->staging = nullptr;
+        ctx->staging_bytes = 0;
+        AI_CUDA(ctx, cudaMalloc(&ctx->staging, bytes));
+        ctx->staging_bytes = bytes;
+    }
+    const size_t nb = (size_t)ctx->npt * sizeof(float);
+    AI_CUDA(ctx, cudaMemcpyAsync(ctx->staging, image_host, bytes, cudaMemcpyHostToDevice, st));
+    FrameArgs a{ctx->staging, dtype, dark, flat, solidangle, polarization, mask, nullptr, ctx->out_dev,
+                ctx->out_dev + ctx->npt, ctx->out_dev + 2 * ctx->npt, 1, (int64_t)ctx->height * ctx->width};
+    int rc = integrate(ctx, a, st);
+    if (rc != AI_OK) return rc;
+    // the three outputs are adjacent on the device; three copies because the host buffers are the caller's
+    AI_CUDA(ctx, cudaMemcpyAsync(intensity_host, ctx->out_dev, nb, cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaMemcpyAsync(sum_signal_host, ctx->out_dev + ctx->npt, nb, cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaMemcpyAsync(count_host, ctx->out_dev + 2 * ctx->npt, nb, cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    return AI_OK;
+}
+
+void ai_destroy(ai_ctx *ctx)
+{
+    if (!ctx) return;
+    cudaFree(ctx->indptr); cudaFree(ctx->indices); cudaFree(ctx->data); cudaFree(ctx->row_csum); cudaFree(ctx->d_range);
+    cudaFree(ctx->lut_coef); cudaFree(ctx->lut_idx);
+    TiledLayout &tl = ctx->tl;
+    cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_csum);
+    cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
+    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev);
+    delete ctx;
+}
+
+}  // extern "C"

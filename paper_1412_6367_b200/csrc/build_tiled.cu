@@ -1,0 +1,238 @@
+// Tiled execution layout (SURVEY.md section 8(a) B6 "derived layouts"): the same bounding-box
+// coefficients as the canonical CSR, re-ordered so that all entries whose pixel lies in one
+// kTileH x kTileW image tile are contiguous, grouped by bin into (tile, bin) segments, pixel index stored as a 16-bit
+// offset inside the tile.  Built from the same per-pixel spans with the same ordered fill as the canonical CSR.
+#include "build_common.cuh"
+#include "ctx.h"
+
+namespace {
+
+__device__ __forceinline__ bool tile_pixel(int t, int k, int tiles_x, int height, int width, int64_t *p)
+{
+    int ty = t / tiles_x, tx = t - ty * tiles_x;
+    int y = ty * kTileH + k / kTileW, x = tx * kTileW + k % kTileW;
+    *p = (int64_t)y * width + x;
+    return y < height && x < width;
+}
+
+// range of bins touched by each tile
+__global__ void __launch_bounds__(256) tile_range_kernel(int tiles_x, int height, int width,
+                                                         const int *__restrict__ first_a, const int *__restrict__ nb_a,
+                                                         int *__restrict__ tile_bmin, int *__restrict__ tile_nbins)
+{
+    const int t = blockIdx.x;
+    int lo = 0x7fffffff, hi = -1;
+    for (int k = threadIdx.x; k < kTilePix; k += blockDim.x) {
+        int64_t p;
+        if (tile_pixel(t, k, tiles_x, height, width, &p)) {
+            int nb = nb_a[p], first = first_a[p];
+            if (nb > 0) { lo = min(lo, first); hi = max(hi, first + nb - 1); }
+        }
+    }
+    __shared__ int s_lo[8], s_hi[8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if ((threadIdx.x & 31) == 0) { s_lo[threadIdx.x >> 5] = lo; s_hi[threadIdx.x >> 5] = hi; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) { lo = min(lo, s_lo[w]); hi = max(hi, s_hi[w]); }
+        tile_bmin[t] = hi >= 0 ? lo : 0;
+        tile_nbins[t] = hi >= 0 ? hi - lo + 1 : 0;
+    }
+}
+
+// exclusive scan of ceil(len / pad) * pad over n elements, one block; out[n] = total
+__global__ void __launch_bounds__(1024) scan_pad_kernel(int n, const int *__restrict__ len, int pad,
+                                                        int *__restrict__ out, long long *__restrict__ total)
+{
+    __shared__ long long warp_sum[32];
+    __shared__ long long carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int base = 0; base < n; base += blockDim.x) {
+        int i = base + threadIdx.x;
+        long long v = i < n ? (long long)((len[i] + pad - 1) / pad) * pad : 0;
+        long long x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            long long y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_sum[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            long long w = warp_sum[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                long long y = __shfl_up_sync(0xffffffffu, w, o);
+                if (lane >= o) w += y;
+            }
+            warp_sum[lane] = w;
+        }
+        __syncthreads();
+        long long before = carry + (wid > 0 ? warp_sum[wid - 1] : 0) + (x - v);
+        if (i < n) out[i] = (int)before;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry = before + v;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        *total = carry;
+        out[n] = (int)carry;
+    }
+}
+
+// number of entries of every (tile, bin) segment
+__global__ void __launch_bounds__(256) tile_count_kernel(int tiles_x, int height, int width,
+                                                         const int *__restrict__ first_a, const int *__restrict__ nb_a,
+                                                         const int *__restrict__ tile_bmin,
+                                                         const int *__restrict__ tile_seg_ptr, int *__restrict__ seg_len)
+{
+    const int t = blockIdx.x;
+    const int bmin = tile_bmin[t], s0 = tile_seg_ptr[t];
+    for (int k = threadIdx.x; k < kTilePix; k += blockDim.x) {
+        int64_t p;
+        if (tile_pixel(t, k, tiles_x, height, width, &p)) {
+            int nb = nb_a[p], first = first_a[p];
+            for (int b = first; b < first + nb; ++b) atomicAdd(&seg_len[s0 + b - bmin], 1);
+        }
+    }
+}
+
+struct TileChunk {
+    int t, tiles_x, height, width, bmin, s0;
+    const int *seg_ptr;
+    int *seg_cur;
+    float *tcoef;
+    uint16_t *tidx;
+    __device__ int npix() const { return kTilePix; }
+    __device__ bool pixel(int k, int64_t *p) const { return tile_pixel(t, k, tiles_x, height, width, p); }
+    __device__ int base(int b) const { return seg_ptr[s0 + b - bmin]; }
+    __device__ volatile int *cursor(int b) const { return seg_cur + s0 + b - bmin; }
+    __device__ void emit(int64_t pos, int k, int64_t, float coef) const { tcoef[pos] = coef; tidx[pos] = (uint16_t)k; }
+};
+
+__global__ void __launch_bounds__(128) fill_tiles_kernel(int ntiles, int tiles_x, int height, int width, int npt,
+                                                         const double *__restrict__ fmin_a,
+                                                         const double *__restrict__ fmax_a,
+                                                         const int *__restrict__ first_a, const int *__restrict__ nb_a,
+                                                         const int *__restrict__ tile_bmin,
+                                                         const int *__restrict__ tile_seg_ptr,
+                                                         const int *__restrict__ seg_ptr, int *seg_cur,
+                                                         float *__restrict__ tcoef, uint16_t *__restrict__ tidx)
+{
+    int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (t >= ntiles) return;
+    TileChunk ch{t, tiles_x, height, width, tile_bmin[t], tile_seg_ptr[t], seg_ptr, seg_cur, tcoef, tidx};
+    marching_fill(ch, fmin_a, fmax_a, first_a, nb_a, npt);
+}
+
+// per-segment coefficient sum (fp64, fixed order): the segment's `count` contribution when all its pixels are valid
+__global__ void __launch_bounds__(256) seg_sum_kernel(int nseg, const int *__restrict__ seg_ptr,
+                                                      const float *__restrict__ tcoef, double *__restrict__ seg_csum)
+{
+    int s = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (s >= nseg) return;
+    double a = 0.0;
+    for (int k = seg_ptr[s] + (threadIdx.x & 31); k < seg_ptr[s + 1]; k += 32) a += (double)tcoef[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    if ((threadIdx.x & 31) == 0) seg_csum[s] = a;
+}
+
+// number of tiles touching each bin (= number of partial slots of the bin)
+__global__ void __launch_bounds__(128) bin_tiles_count_kernel(int npt, int ntiles, const int *__restrict__ tile_bmin,
+                                                              const int *__restrict__ tile_nbins, int *__restrict__ nslot)
+{
+    int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= npt) return;
+    int c = 0;
+    for (int t = 0; t < ntiles; ++t) {
+        int lo = tile_bmin[t];
+        c += (b >= lo && b < lo + tile_nbins[t]) ? 1 : 0;
+    }
+    nslot[b] = c;
+}
+
+// slot of every segment in the bin-major partial buffer: bin b's slots are ordered by ascending tile
+__global__ void __launch_bounds__(128) bin_tiles_assign_kernel(int npt, int ntiles, const int *__restrict__ tile_bmin,
+                                                               const int *__restrict__ tile_nbins,
+                                                               const int *__restrict__ tile_seg_ptr,
+                                                               const int *__restrict__ bin_slot_ptr,
+                                                               int *__restrict__ seg_slot)
+{
+    int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= npt) return;
+    int slot = bin_slot_ptr[b];
+    for (int t = 0; t < ntiles; ++t) {
+        int lo = tile_bmin[t];
+        if (b >= lo && b < lo + tile_nbins[t]) seg_slot[tile_seg_ptr[t] + b - lo] = slot++;
+    }
+}
+
+}  // namespace
+
+int ai_build_tiled(ai_ctx *ctx, const PixelSpans &sp, cudaStream_t st)
+{
+    TiledLayout &tl = ctx->tl;
+    const int H = ctx->height, W = ctx->width, npt = ctx->npt;
+    tl.tiles_y = (H + kTileH - 1) / kTileH;
+    tl.tiles_x = (W + kTileW - 1) / kTileW;
+    tl.ntiles = tl.tiles_y * tl.tiles_x;
+    int *tile_bmin = nullptr, *tile_nbins = nullptr, *seg_len = nullptr, *seg_cur = nullptr, *nslot = nullptr;
+    long long *d_total = nullptr, h_total = 0;
+    AI_CUDA(ctx, cudaMalloc(&tile_bmin, tl.ntiles * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&tile_nbins, tl.ntiles * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&tl.tile_seg_ptr, (tl.ntiles + 1) * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&d_total, sizeof(long long)));
+    tile_range_kernel<<<tl.ntiles, 256, 0, st>>>(tl.tiles_x, H, W, sp.first, sp.nb, tile_bmin, tile_nbins);
+    scan_pad_kernel<<<1, 1024, 0, st>>>(tl.ntiles, tile_nbins, 1, tl.tile_seg_ptr, d_total);
+    AI_CUDA(ctx, cudaGetLastError());
+    AI_CUDA(ctx, cudaMemcpyAsync(&h_total, d_total, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    if (h_total > 0x7fffffffLL) return ai_fail(ctx, AI_EUNSUPPORTED, "too many (tile, bin) segments: %lld", h_total);
+    tl.nseg = (int)h_total;
+    tl.nslot = tl.nseg;
+    const size_t nseg_alloc = tl.nseg > 0 ? tl.nseg : 1;
+
+    AI_CUDA(ctx, cudaMalloc(&seg_len, nseg_alloc * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&seg_cur, nseg_alloc * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&tl.seg_ptr, (nseg_alloc + 1) * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&tl.seg_slot, nseg_alloc * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&tl.seg_csum, nseg_alloc * sizeof(double)));
+    AI_CUDA(ctx, cudaMemsetAsync(seg_len, 0, nseg_alloc * sizeof(int), st));
+    AI_CUDA(ctx, cudaMemsetAsync(seg_cur, 0, nseg_alloc * sizeof(int), st));
+    tile_count_kernel<<<tl.ntiles, 256, 0, st>>>(tl.tiles_x, H, W, sp.first, sp.nb, tile_bmin, tl.tile_seg_ptr, seg_len);
+    scan_pad_kernel<<<1, 1024, 0, st>>>(tl.nseg, seg_len, kSegPad, tl.seg_ptr, d_total);
+    AI_CUDA(ctx, cudaGetLastError());
+    AI_CUDA(ctx, cudaMemcpyAsync(&h_total, d_total, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    if (h_total > 0x7fffffffLL) return ai_fail(ctx, AI_EUNSUPPORTED, "tiled layout has %lld entries", h_total);
+    tl.tnnz = h_total;
+    const size_t nnz_alloc = tl.tnnz > 0 ? (size_t)tl.tnnz : 1;
+
+    AI_CUDA(ctx, cudaMalloc(&tl.tcoef, nnz_alloc * sizeof(float)));
+    AI_CUDA(ctx, cudaMalloc(&tl.tidx, nnz_alloc * sizeof(uint16_t)));
+    AI_CUDA(ctx, cudaMemsetAsync(tl.tcoef, 0, nnz_alloc * sizeof(float), st));       // padding: coefficient 0,
+    AI_CUDA(ctx, cudaMemsetAsync(tl.tidx, 0, nnz_alloc * sizeof(uint16_t), st));     // pixel 0 of the tile
+    fill_tiles_kernel<<<(tl.ntiles + 3) / 4, 128, 0, st>>>(tl.ntiles, tl.tiles_x, H, W, npt, sp.fmin, sp.fmax, sp.first,
+                                                           sp.nb, tile_bmin, tl.tile_seg_ptr, tl.seg_ptr, seg_cur,
+                                                           tl.tcoef, tl.tidx);
+    if (tl.nseg > 0)
+        seg_sum_kernel<<<(tl.nseg + 7) / 8, 256, 0, st>>>(tl.nseg, tl.seg_ptr, tl.tcoef, tl.seg_csum);
+
+    AI_CUDA(ctx, cudaMalloc(&nslot, (size_t)npt * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&tl.bin_slot_ptr, ((size_t)npt + 1) * sizeof(int)));
+    bin_tiles_count_kernel<<<(npt + 127) / 128, 128, 0, st>>>(npt, tl.ntiles, tile_bmin, tile_nbins, nslot);
+    scan_pad_kernel<<<1, 1024, 0, st>>>(npt, nslot, 1, tl.bin_slot_ptr, d_total);
+    bin_tiles_assign_kernel<<<(npt + 127) / 128, 128, 0, st>>>(npt, tl.ntiles, tile_bmin, tile_nbins, tl.tile_seg_ptr,
+                                                               tl.bin_slot_ptr, tl.seg_slot);
+    AI_CUDA(ctx, cudaGetLastError());
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    cudaFree(tile_bmin); cudaFree(tile_nbins); cudaFree(seg_len); cudaFree(seg_cur); cudaFree(nslot); cudaFree(d_total);
+    return AI_OK;
+}
