@@ -86,6 +86,10 @@ int ai_build_csr(ai_ctx *ctx, void *cuda_stream);
 int ai_get_csr(const ai_ctx *ctx, const int32_t **indptr, const int32_t **indices, const float **data,
                int64_t *nnz, double *u0, double *u1);
 
+/* Copy the canonical CSR into HOST buffers of indptr[npt+1], indices[nnz], data[nnz] elements (sizes from ai_get_csr);
+ * any pointer may be NULL.  Synchronous.  Errors: AI_ENOTBUILT, AI_ECUDA. */
+int ai_copy_csr_to_host(const ai_ctx *ctx, int32_t *indptr_host, int32_t *indices_host, float *data_host);
+
 /* Choose execution layout, accumulator and the intensity written to bins with count == 0 (default: TILED, KAHAN, 0).
  * AI_LAYOUT_LUT builds the padded table on first use (inside the next integrate call's stream).
  * Errors: AI_EINVAL. */
@@ -128,6 +132,13 @@ int ai_integrate1d_host(ai_ctx *ctx, const void *image_host, ai_dtype dtype, con
 
 /* Number of kernels the last ai_integrate1d* call launched (for accounting in benchmarks). */
 int ai_last_launch_count(const ai_ctx *ctx);
+
+/* Measurement hook: when enabled, every ai_integrate1d* call records CUDA events on its stream around its dominant
+ * kernel (TILED: stage 1, the SpMV; CSR / LUT: the single kernel).  ai_profile_last synchronises on the last of those
+ * events and returns the device time of that kernel launch in milliseconds through *kernel_ms.
+ * Errors: AI_EINVAL (NULL, or nothing recorded yet), AI_ECUDA. */
+int ai_profile_enable(ai_ctx *ctx, int on);
+int ai_profile_last(ai_ctx *ctx, float *kernel_ms);
 
 /* Release the context, the matrix and all scratch memory.  NULL is allowed. */
 void ai_destroy(ai_ctx *ctx);

@@ -20,7 +20,7 @@ AI_LAYOUT_TILED, AI_LAYOUT_CSR, AI_LAYOUT_LUT = range(3)
 AI_ACC_F32_KAHAN, AI_ACC_F32_PLAIN, AI_ACC_F64 = range(3)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ai_setup", "ai_build_csr", "ai_get_csr", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
+EXPORTS = ["ai_setup", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
            "ai_integrate1d_host", "ai_last_launch_count", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
@@ -51,6 +51,7 @@ def lib():
     L.ai_setup.argtypes = [C.POINTER(vp), C.POINTER(ai_geometry), C.c_int, C.c_int, C.c_int, C.c_int, dp]
     L.ai_build_csr.argtypes = [vp, vp]
     L.ai_get_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int64), dp, dp]
+    L.ai_copy_csr_to_host.argtypes = [vp, vp, vp, vp]
     L.ai_set_options.argtypes = [vp, C.c_int, C.c_int, C.c_float]
     L.ai_integrate1d.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
     L.ai_integrate1d_batch.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
@@ -125,6 +126,10 @@ def ai_get_csr(ctx):
     return a.value, b.value, c.value, nnz.value, u0.value, u1.value
 
 
+def ai_copy_csr_to_host(ctx, indptr_host=None, indices_host=None, data_host=None):
+    _check(lib().ai_copy_csr_to_host(ctx, _ptr(indptr_host), _ptr(indices_host), _ptr(data_host)), ctx)
+
+
 def ai_set_options(ctx, layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN, empty_value=0.0):
     _check(lib().ai_set_options(ctx, layout, accum, empty_value), ctx)
 
@@ -186,20 +191,14 @@ class Integrator:
         ai_set_options(self.ctx, layout, accum, empty_value)
 
     def csr(self):
-        """Canonical CSR as torch tensors copied out of the borrowed device arrays (indptr, indices, data), + range."""
-        torch = self.torch
-        a, b, c, nnz, u0, u1 = ai_get_csr(self.ctx)
-
-        def view(ptr, n, dt):
-            import numpy as np
-            host = np.empty(n, dtype=dt)
-            if n:
-                rc = torch.cuda.cudart().cudaMemcpy(host.ctypes.data, ptr, host.nbytes, 2)   # 2 = DeviceToHost
-                if int(rc) != 0:
-                    raise AzintError(AI_ECUDA, f"cudaMemcpy failed: {rc}")
-            return host
+        """Canonical CSR copied to host numpy arrays (indptr, indices, data) + the range in use."""
         import numpy as np
-        return view(a, self.npt + 1, np.int32), view(b, nnz, np.int32), view(c, nnz, np.float32), (u0, u1)
+        _, _, _, nnz, u0, u1 = ai_get_csr(self.ctx)
+        indptr = np.empty(self.npt + 1, dtype=np.int32)
+        indices = np.empty(nnz, dtype=np.int32)
+        data = np.empty(nnz, dtype=np.float32)
+        ai_copy_csr_to_host(self.ctx, indptr, indices, data)
+        return indptr, indices, data, (u0, u1)
 
     def outputs(self, nframes=None):
         shape = (self.npt,) if nframes is None else (nframes, self.npt)

@@ -99,6 +99,20 @@ int ai_get_csr(const ai_ctx *ctx, const int32_t **indptr, const int32_t **indice
     return AI_OK;
 }
 
+int ai_copy_csr_to_host(const ai_ctx *ctx, int32_t *indptr_host, int32_t *indices_host, float *data_host)
+{
+    if (!ctx) return AI_EINVAL;
+    if (!ctx->built) return AI_ENOTBUILT;
+    ai_ctx *c = const_cast<ai_ctx *>(ctx);      // only the error text is written
+    if (indptr_host)
+        AI_CUDA(c, cudaMemcpy(indptr_host, ctx->indptr, ((size_t)ctx->npt + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    if (indices_host && ctx->nnz)
+        AI_CUDA(c, cudaMemcpy(indices_host, ctx->indices, (size_t)ctx->nnz * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    if (data_host && ctx->nnz)
+        AI_CUDA(c, cudaMemcpy(data_host, ctx->data, (size_t)ctx->nnz * sizeof(float), cudaMemcpyDeviceToHost));
+    return AI_OK;
+}
+
 int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_value)
 {
     if (!ctx) return AI_EINVAL;

@@ -62,7 +62,18 @@ struct ai_ctx {
     void *staging = nullptr;        // device copy of a host frame (ai_integrate1d_host)
     size_t staging_bytes = 0;
     float *out_dev = nullptr;       // [3*npt] device outputs of ai_integrate1d_host
+
+    // measurement hook (ai_profile_enable): events around the dominant kernel of the last call
+    bool profile = false, profile_valid = false;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
 };
+
+// events around the dominant kernel when profiling is on (no-ops otherwise)
+inline void ai_prof_begin(ai_ctx *ctx, cudaStream_t st) { if (ctx->profile) cudaEventRecord(ctx->ev0, st); }
+inline void ai_prof_end(ai_ctx *ctx, cudaStream_t st)
+{
+    if (ctx->profile) { cudaEventRecord(ctx->ev1, st); ctx->profile_valid = true; }
+}
 
 // error plumbing -------------------------------------------------------------------------------------------------
 int ai_fail(ai_ctx *ctx, int code, const char *fmt, ...);

@@ -25,7 +25,7 @@ def _declared_functions():
 
 def test_library_exports_every_declared_symbol(B):
     names = _declared_functions()
-    assert {"ai_setup", "ai_build_csr", "ai_get_csr", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
+    assert {"ai_setup", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
             "ai_integrate1d_host", "ai_destroy", "ai_strerror", "ai_last_error"} <= set(names)
     L = B.lib()
     for n in names:
