@@ -21,7 +21,7 @@ AI_ACC_F32_KAHAN, AI_ACC_F32_PLAIN, AI_ACC_F64 = range(3)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["ai_setup", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
-           "ai_integrate1d_host", "ai_last_launch_count", "ai_destroy", "ai_strerror", "ai_last_error"]
+           "ai_integrate1d_host", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
 class ai_geometry(C.Structure):
@@ -57,6 +57,8 @@ def lib():
     L.ai_integrate1d_batch.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_integrate1d_host.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_last_launch_count.argtypes = [vp]
+    L.ai_profile_enable.argtypes = [vp, C.c_int]
+    L.ai_profile_last.argtypes = [vp, C.POINTER(C.c_float)]
     L.ai_destroy.argtypes = [vp]
     L.ai_destroy.restype = None
     L.ai_strerror.argtypes = [C.c_int]
@@ -159,6 +161,17 @@ def ai_integrate1d_host(ctx, image_host, dark, flat, solidangle, polarization, m
 
 def ai_last_launch_count(ctx) -> int:
     return int(lib().ai_last_launch_count(ctx))
+
+
+def ai_profile_enable(ctx, on=True):
+    _check(lib().ai_profile_enable(ctx, 1 if on else 0), ctx)
+
+
+def ai_profile_last(ctx) -> float:
+    """Device time (ms) of the dominant kernel of the last profiled call."""
+    ms = C.c_float()
+    _check(lib().ai_profile_last(ctx, C.byref(ms)), ctx)
+    return float(ms.value)
 
 
 def ai_destroy(ctx):

@@ -38,6 +38,27 @@ const char *ai_last_error(const ai_ctx *ctx) { return ctx ? ctx->err : ""; }
 
 int ai_last_launch_count(const ai_ctx *ctx) { return ctx ? ctx->last_launches : 0; }
 
+int ai_profile_enable(ai_ctx *ctx, int on)
+{
+    if (!ctx) return AI_EINVAL;
+    if (on && !ctx->ev0) {
+        AI_CUDA(ctx, cudaEventCreate(&ctx->ev0));
+        AI_CUDA(ctx, cudaEventCreate(&ctx->ev1));
+    }
+    ctx->profile = on != 0;
+    ctx->profile_valid = false;
+    return AI_OK;
+}
+
+int ai_profile_last(ai_ctx *ctx, float *kernel_ms)
+{
+    if (!ctx || !kernel_ms) return AI_EINVAL;
+    if (!ctx->profile_valid) return ai_fail(ctx, AI_EINVAL, "no profiled call yet");
+    AI_CUDA(ctx, cudaEventSynchronize(ctx->ev1));
+    AI_CUDA(ctx, cudaEventElapsedTime(kernel_ms, ctx->ev0, ctx->ev1));
+    return AI_OK;
+}
+
 int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt, ai_unit unit,
              const double *range_or_null)
 {
@@ -201,6 +222,8 @@ void ai_destroy(ai_ctx *ctx)
     cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_csum);
     cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
     cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev);
+    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;
 }
 

@@ -99,9 +99,11 @@ int launch_csr_typed(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 {
     Corrections cor{a.dark, a.flat, a.solidangle, a.polarization, a.mask};
     dim3 grid(ctx->npt, a.nframes);
+    ai_prof_begin(ctx, st);
     csr_row_kernel<DT, ACC><<<grid, kRowThreads, 0, st>>>(ctx->indptr, ctx->indices, ctx->data, ctx->npt, a.image,
                                                          a.frame_stride, cor, ctx->d_range, ctx->empty_value, a.radial,
                                                          a.intensity, a.sum_signal, a.count);
+    ai_prof_end(ctx, st);
     AI_CUDA(ctx, cudaGetLastError());
     ctx->last_launches = 1;
     return AI_OK;
@@ -112,9 +114,11 @@ int launch_lut_typed(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 {
     Corrections cor{a.dark, a.flat, a.solidangle, a.polarization, a.mask};
     dim3 grid((ctx->npt + 127) / 128, a.nframes);
+    ai_prof_begin(ctx, st);
     lut_kernel<DT, ACC><<<grid, 128, 0, st>>>(ctx->lut_coef, ctx->lut_idx, ctx->lut_width, ctx->npt, a.image,
                                              a.frame_stride, cor, ctx->d_range, ctx->empty_value, a.radial,
                                              a.intensity, a.sum_signal, a.count);
+    ai_prof_end(ctx, st);
     AI_CUDA(ctx, cudaGetLastError());
     ctx->last_launches = 1;
     return AI_OK;

@@ -180,8 +180,10 @@ int launch_typed(ai_ctx *ctx, const FrameArgs &a, const TiledView &tv, const Cor
                  cudaStream_t st)
 {
     dim3 g1(ctx->tl.ntiles, a.nframes);
+    ai_prof_begin(ctx, st);
     tiled_stage1_kernel<DT, ACC><<<g1, kS1Threads, 0, st>>>(tv, a.image, a.frame_stride, cor, ctx->height, ctx->width,
                                                            vec_ok, ctx->partials);
+    ai_prof_end(ctx, st);
     dim3 g2((ctx->npt + 7) / 8, a.nframes);
     tiled_stage2_kernel<ACC><<<g2, 256, 0, st>>>(tv.bin_slot_ptr, tv.nslot, ctx->npt, ctx->partials, ctx->d_range,
                                                  ctx->empty_value, a.radial, a.intensity, a.sum_signal, a.count);
