@@ -137,7 +137,7 @@ int ai_copy_csr_to_host(const ai_ctx *ctx, int32_t *indptr_host, int32_t *indice
 int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_value)
 {
     if (!ctx) return AI_EINVAL;
-    if ((int)layout < AI_LAYOUT_TILED || (int)layout > AI_LAYOUT_LUT) return ai_fail(ctx, AI_EINVAL, "bad layout %d", (int)layout);
+    if ((int)layout < AI_LAYOUT_TILED || (int)layout > AI_LAYOUT_TILED_DIRECT) return ai_fail(ctx, AI_EINVAL, "bad layout %d", (int)layout);
     if ((int)accum < AI_ACC_F32_KAHAN || (int)accum > AI_ACC_F64) return ai_fail(ctx, AI_EINVAL, "bad accum %d", (int)accum);
     ctx->layout = layout;
     ctx->accum = accum;
@@ -154,7 +154,8 @@ static int integrate(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
     if (a.nframes < 1) return ai_fail(ctx, AI_EINVAL, "nframes < 1");
     if (a.frame_stride < (int64_t)ctx->height * ctx->width) return ai_fail(ctx, AI_EINVAL, "frame stride < height*width");
     switch (ctx->layout) {
-    case AI_LAYOUT_TILED: return ai_launch_tiled(ctx, a, st);
+    case AI_LAYOUT_TILED:
+    case AI_LAYOUT_TILED_DIRECT: return ai_launch_tiled(ctx, a, st);
     case AI_LAYOUT_CSR: return ai_launch_csr(ctx, a, st);
     case AI_LAYOUT_LUT: return ai_launch_lut(ctx, a, st);
     }
@@ -219,7 +220,8 @@ void ai_destroy(ai_ctx *ctx)
     cudaFree(ctx->indptr); cudaFree(ctx->indices); cudaFree(ctx->data); cudaFree(ctx->row_csum); cudaFree(ctx->d_range);
     cudaFree(ctx->lut_coef); cudaFree(ctx->lut_idx);
     TiledLayout &tl = ctx->tl;
-    cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_csum);
+    cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_meta); cudaFree(tl.seg_csum);
+    cudaFree(tl.tile_desc); cudaFree(tl.tile_order);
     cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
     cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);

@@ -2,6 +2,9 @@
 // coefficients as the canonical CSR, re-ordered so that all entries whose pixel lies in one
 // kTileH x kTileW image tile are contiguous, grouped by bin into (tile, bin) segments, pixel index stored as a 16-bit
 // offset inside the tile.  Built from the same per-pixel spans with the same ordered fill as the canonical CSR.
+#include <algorithm>
+#include <vector>
+
 #include "build_common.cuh"
 #include "ctx.h"
 
@@ -174,6 +177,38 @@ __global__ void __launch_bounds__(128) bin_tiles_assign_kernel(int npt, int ntil
     }
 }
 
+// padded segment lengths: every segment a multiple of kSegPad entries (128-bit coefficient loads), every tile a
+// multiple of 8 entries so that the tile's slice of the 16-bit index array starts on a 16-byte boundary (bulk copies)
+__global__ void __launch_bounds__(128) pad_segments_kernel(int ntiles, const int *__restrict__ tile_seg_ptr,
+                                                           int *__restrict__ seg_len)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntiles) return;
+    const int s0 = tile_seg_ptr[t], s1 = tile_seg_ptr[t + 1];
+    int total = 0;
+    for (int s = s0; s < s1; ++s) {
+        int p = (seg_len[s] + kSegPad - 1) / kSegPad * kSegPad;
+        seg_len[s] = p;
+        total += p;
+    }
+    if (s1 > s0 && (total & 7)) seg_len[s1 - 1] += 8 - (total & 7);
+}
+
+// {first entry, padded end, partial slot, coefficient sum as float bits} of every segment: one 128-bit load
+__global__ void __launch_bounds__(256) seg_meta_kernel(int ntiles, const int *__restrict__ tile_seg_ptr,
+                                                       const int *__restrict__ seg_ptr, const int *__restrict__ seg_slot,
+                                                       const double *__restrict__ seg_csum,
+                                                       int4 *__restrict__ seg_meta, int4 *__restrict__ tile_desc)
+{
+    const int t = blockIdx.x;
+    if (t >= ntiles) return;
+    const int s0 = tile_seg_ptr[t], s1 = tile_seg_ptr[t + 1];
+    for (int s = s0 + threadIdx.x; s < s1; s += blockDim.x)
+        seg_meta[s] = make_int4(seg_ptr[s], seg_ptr[s + 1], seg_slot[s], __float_as_int((float)seg_csum[s]));
+    // {first entry, number of entries, first segment, number of segments} of the tile
+    if (threadIdx.x == 0) tile_desc[t] = make_int4(seg_ptr[s0], seg_ptr[s1] - seg_ptr[s0], s0, s1 - s0);
+}
+
 }  // namespace
 
 int ai_build_tiled(ai_ctx *ctx, const PixelSpans &sp, cudaStream_t st)
@@ -207,7 +242,8 @@ int ai_build_tiled(ai_ctx *ctx, const PixelSpans &sp, cudaStream_t st)
     AI_CUDA(ctx, cudaMemsetAsync(seg_len, 0, nseg_alloc * sizeof(int), st));
     AI_CUDA(ctx, cudaMemsetAsync(seg_cur, 0, nseg_alloc * sizeof(int), st));
     tile_count_kernel<<<tl.ntiles, 256, 0, st>>>(tl.tiles_x, H, W, sp.first, sp.nb, tile_bmin, tl.tile_seg_ptr, seg_len);
-    scan_pad_kernel<<<1, 1024, 0, st>>>(tl.nseg, seg_len, kSegPad, tl.seg_ptr, d_total);
+    pad_segments_kernel<<<(tl.ntiles + 127) / 128, 128, 0, st>>>(tl.ntiles, tl.tile_seg_ptr, seg_len);
+    scan_pad_kernel<<<1, 1024, 0, st>>>(tl.nseg, seg_len, 1, tl.seg_ptr, d_total);
     AI_CUDA(ctx, cudaGetLastError());
     AI_CUDA(ctx, cudaMemcpyAsync(&h_total, d_total, sizeof(long long), cudaMemcpyDeviceToHost, st));
     AI_CUDA(ctx, cudaStreamSynchronize(st));
@@ -231,7 +267,30 @@ int ai_build_tiled(ai_ctx *ctx, const PixelSpans &sp, cudaStream_t st)
     scan_pad_kernel<<<1, 1024, 0, st>>>(npt, nslot, 1, tl.bin_slot_ptr, d_total);
     bin_tiles_assign_kernel<<<(npt + 127) / 128, 128, 0, st>>>(npt, tl.ntiles, tile_bmin, tile_nbins, tl.tile_seg_ptr,
                                                                tl.bin_slot_ptr, tl.seg_slot);
+    AI_CUDA(ctx, cudaMalloc(&tl.seg_meta, nseg_alloc * sizeof(int4)));
+    AI_CUDA(ctx, cudaMalloc(&tl.tile_desc, (size_t)tl.ntiles * sizeof(int4)));
+    AI_CUDA(ctx, cudaMalloc(&tl.tile_order, (size_t)tl.ntiles * sizeof(int)));
+    seg_meta_kernel<<<tl.ntiles, 256, 0, st>>>(tl.ntiles, tl.tile_seg_ptr, tl.seg_ptr, tl.seg_slot, tl.seg_csum,
+                                               tl.seg_meta, tl.tile_desc);
     AI_CUDA(ctx, cudaGetLastError());
+    // longest-processing-time-first order of the tiles (host sort of ntiles integers, one-time)
+    std::vector<int4> desc(tl.ntiles);
+    AI_CUDA(ctx, cudaMemcpyAsync(desc.data(), tl.tile_desc, (size_t)tl.ntiles * sizeof(int4), cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    std::vector<int> order(tl.ntiles);
+    for (int t = 0; t < tl.ntiles; ++t) order[t] = t;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return desc[a].y > desc[b].y; });
+    tl.max_tile_entries = 0;
+    tl.max_tile_segs = 0;
+    for (const int4 &d : desc) {
+        tl.max_tile_entries = std::max(tl.max_tile_entries, d.y);
+        tl.max_tile_segs = std::max(tl.max_tile_segs, d.w);
+    }
+    // tile_desc is kept in the same longest-first order as tile_order (the pipelined kernel indexes both by rank)
+    std::vector<int4> desc_lpt(tl.ntiles);
+    for (int r = 0; r < tl.ntiles; ++r) desc_lpt[r] = desc[order[r]];
+    AI_CUDA(ctx, cudaMemcpyAsync(tl.tile_order, order.data(), (size_t)tl.ntiles * sizeof(int), cudaMemcpyHostToDevice, st));
+    AI_CUDA(ctx, cudaMemcpyAsync(tl.tile_desc, desc_lpt.data(), (size_t)tl.ntiles * sizeof(int4), cudaMemcpyHostToDevice, st));
     AI_CUDA(ctx, cudaStreamSynchronize(st));
     cudaFree(tile_bmin); cudaFree(tile_nbins); cudaFree(seg_len); cudaFree(seg_cur); cudaFree(nslot); cudaFree(d_total);
     return AI_OK;

@@ -19,6 +19,10 @@ struct TiledLayout {
     int *tile_seg_ptr = nullptr;   // [ntiles+1] first segment of each tile
     int *seg_ptr = nullptr;        // [nseg+1]   first entry of each segment (multiple of kSegPad)
     int *seg_slot = nullptr;       // [nseg]     slot of the segment's partial in the bin-major partial buffer
+    int4 *seg_meta = nullptr;      // [nseg]     {first entry, padded end, partial slot, float bits of the coefficient sum}
+    int4 *tile_desc = nullptr;     // [ntiles]   {first entry, number of entries, first segment, number of segments}
+    int *tile_order = nullptr;     // [ntiles]   tiles by descending number of entries (longest first scheduling)
+    int max_tile_entries = 0, max_tile_segs = 0;
     double *seg_csum = nullptr;    // [nseg]     sum of the segment's coefficients (count when every pixel is valid)
     float *tcoef = nullptr;        // [tnnz]     coefficient
     uint16_t *tidx = nullptr;      // [tnnz]     pixel index inside the tile (ly * kTileW + lx)

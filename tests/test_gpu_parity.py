@@ -10,7 +10,7 @@ from parity import assert_profile, compare_csr, rel_err
 
 pytestmark = pytest.mark.gpu
 
-LAYOUTS = {"tiled": 0, "csr": 1, "lut": 2}
+LAYOUTS = {"tiled": 0, "csr": 1, "lut": 2, "direct": 3}
 ACCUMS = {"kahan": 0, "plain": 1, "f64": 2}
 
 
@@ -115,7 +115,7 @@ def test_csr_with_explicit_range(torch, B, oracle, workloads):
 # ----------------------------------------------------------------------------------------------------------------------
 # H1-H5: one frame, every layout and accumulator
 # ----------------------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("layout", ["tiled", "csr", "lut"])
+@pytest.mark.parametrize("layout", ["tiled", "direct", "csr", "lut"])
 @pytest.mark.parametrize("accum", ["kahan", "f64"])
 @pytest.mark.parametrize("name", ["cfg1", "cfg1b", "cfg2"])
 def test_profile_parity(torch, B, oracle, workloads, name, layout, accum):
@@ -130,7 +130,7 @@ def test_profile_parity(torch, B, oracle, workloads, name, layout, accum):
     integ.close()
 
 
-@pytest.mark.parametrize("layout", ["tiled", "csr"])
+@pytest.mark.parametrize("layout", ["tiled", "direct", "csr"])
 def test_profile_parity_full_corrections_cfg3(torch, B, oracle, workloads, layout):
     cfg = workloads.CONFIGS["cfg3"]
     fr = workloads.make_frame(cfg)
@@ -148,7 +148,7 @@ def test_profile_parity_cfg5_layouts_and_accumulators(torch, B, oracle, workload
     want = _oracle_profile(oracle, cfg, fr)
     integ = B.Integrator(cfg)
     report = {}
-    for layout in ("tiled", "csr", "lut"):
+    for layout in ("tiled", "direct", "csr", "lut"):
         for accum in ("kahan", "f64", "plain"):
             integ.set_options(LAYOUTS[layout], ACCUMS[accum])
             got = _run(torch, integ, fr)
@@ -191,7 +191,7 @@ def test_raw_dtypes(torch, B, oracle, workloads, dtype, layout):
 # ragged shapes, unaligned buffers, masks, empty bins, non-finite data
 # ----------------------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("idx", range(6))
-@pytest.mark.parametrize("layout", ["tiled", "csr", "lut"])
+@pytest.mark.parametrize("layout", ["tiled", "direct", "csr", "lut"])
 def test_ragged_and_degenerate_shapes(torch, B, oracle, workloads, idx, layout):
     cfg = _ragged_cases(workloads)[idx]
     rng = np.random.default_rng(100 + idx)
@@ -225,7 +225,7 @@ def test_unaligned_buffers_take_the_scalar_path(torch, B, oracle, workloads):
     integ.close()
 
 
-@pytest.mark.parametrize("layout", ["tiled", "csr", "lut"])
+@pytest.mark.parametrize("layout", ["tiled", "direct", "csr", "lut"])
 def test_all_masked_and_non_finite_pixels(torch, B, oracle, workloads, layout):
     cfg = workloads.CONFIGS["cfg1b"]
     fr = workloads.make_frame(cfg)
