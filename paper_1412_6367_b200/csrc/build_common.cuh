@@ -56,6 +56,7 @@ __device__ __forceinline__ void split_span(double f_lo, double f_hi, int npt, in
 //   bool pixel(int k, int64_t *p)     global pixel index of slot k (false: slot outside the image)
 //   int  base(int b)                  start of bin b's destination range
 //   volatile int *cursor(int b)       running offset of this chunk inside that range
+//   int64_t place(int b, int64_t pos) final position of the entry whose position in ascending pixel order is pos
 //   void emit(int64_t pos, int k, int64_t p, float coef)
 template <class Chunk>
 __device__ __forceinline__ void marching_fill(Chunk &ch, const double *__restrict__ fmin_a,
@@ -95,7 +96,8 @@ __device__ __forceinline__ void marching_fill(Chunk &ch, const double *__restric
                 bool covers = nb > 0 && b >= first && b < first + nb;
                 unsigned m = __ballot_sync(0xffffffffu, covers);
                 int s = __shfl_sync(0xffffffffu, start, bb);
-                if (covers) ch.emit((int64_t)s + __popc(m & lt), k, p, (float)split_coefficient(f_lo, f_hi, b, npt));
+                if (covers)
+                    ch.emit(ch.place(b, (int64_t)s + __popc(m & lt)), k, p, (float)split_coefficient(f_lo, f_hi, b, npt));
                 if (lane == bb) mine = __popc(m);
             }
             if (cur) *cur = *cur + mine;

@@ -208,6 +208,7 @@ struct LineChunk {
     __device__ bool pixel(int k, int64_t *p) const { *p = (int64_t)line * width + k; return true; }
     __device__ int base(int b) const { return indptr[b]; }
     __device__ volatile int *cursor(int b) const { return cnt_line + b; }
+    __device__ int64_t place(int, int64_t pos) const { return pos; }      // canonical CSR: ascending pixel order
     __device__ void emit(int64_t pos, int, int64_t p, float coef) const { indices[pos] = (int32_t)p; data[pos] = coef; }
 };
 

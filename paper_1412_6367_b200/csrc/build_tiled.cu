@@ -1,7 +1,9 @@
 // Tiled execution layout (SURVEY.md section 8(a) B6 "derived layouts"): the same bounding-box
 // coefficients as the canonical CSR, re-ordered so that all entries whose pixel lies in one
-// kTileH x kTileW image tile are contiguous, grouped by bin into (tile, bin) segments, pixel index stored as a 16-bit
-// offset inside the tile.  Built from the same per-pixel spans with the same ordered fill as the canonical CSR.
+// tile_h x kTileW image tile are contiguous, grouped by bin into (tile, bin) segments, pixel stored as its 16-bit
+// position inside the tile's shared-memory buffer (ai_tile_pos).  Built from the same per-pixel spans with the same
+// ordered fill as the canonical CSR.  tile_h is the largest of 64, 32, 16, 8 for which the pipelined kernel's
+// shared-memory plan fits (ai_pipe_plan).
 #include <algorithm>
 #include <vector>
 
@@ -10,24 +12,24 @@
 
 namespace {
 
-__device__ __forceinline__ bool tile_pixel(int t, int k, int tiles_x, int height, int width, int64_t *p)
+__device__ __forceinline__ bool tile_pixel(int t, int k, int tiles_x, int th, int height, int width, int64_t *p)
 {
     int ty = t / tiles_x, tx = t - ty * tiles_x;
-    int y = ty * kTileH + k / kTileW, x = tx * kTileW + k % kTileW;
+    int y = ty * th + k / kTileW, x = tx * kTileW + k % kTileW;
     *p = (int64_t)y * width + x;
     return y < height && x < width;
 }
 
 // range of bins touched by each tile
-__global__ void __launch_bounds__(256) tile_range_kernel(int tiles_x, int height, int width,
+__global__ void __launch_bounds__(256) tile_range_kernel(int tiles_x, int th, int height, int width,
                                                          const int *__restrict__ first_a, const int *__restrict__ nb_a,
                                                          int *__restrict__ tile_bmin, int *__restrict__ tile_nbins)
 {
     const int t = blockIdx.x;
     int lo = 0x7fffffff, hi = -1;
-    for (int k = threadIdx.x; k < kTilePix; k += blockDim.x) {
+    for (int k = threadIdx.x; k < th * kTileW; k += blockDim.x) {
         int64_t p;
-        if (tile_pixel(t, k, tiles_x, height, width, &p)) {
+        if (tile_pixel(t, k, tiles_x, th, height, width, &p)) {
             int nb = nb_a[p], first = first_a[p];
             if (nb > 0) { lo = min(lo, first); hi = max(hi, first + nb - 1); }
         }
@@ -90,16 +92,16 @@ __global__ void __launch_bounds__(1024) scan_pad_kernel(int n, const int *__rest
 }
 
 // number of entries of every (tile, bin) segment
-__global__ void __launch_bounds__(256) tile_count_kernel(int tiles_x, int height, int width,
+__global__ void __launch_bounds__(256) tile_count_kernel(int tiles_x, int th, int height, int width,
                                                          const int *__restrict__ first_a, const int *__restrict__ nb_a,
                                                          const int *__restrict__ tile_bmin,
                                                          const int *__restrict__ tile_seg_ptr, int *__restrict__ seg_len)
 {
     const int t = blockIdx.x;
     const int bmin = tile_bmin[t], s0 = tile_seg_ptr[t];
-    for (int k = threadIdx.x; k < kTilePix; k += blockDim.x) {
+    for (int k = threadIdx.x; k < th * kTileW; k += blockDim.x) {
         int64_t p;
-        if (tile_pixel(t, k, tiles_x, height, width, &p)) {
+        if (tile_pixel(t, k, tiles_x, th, height, width, &p)) {
             int nb = nb_a[p], first = first_a[p];
             for (int b = first; b < first + nb; ++b) atomicAdd(&seg_len[s0 + b - bmin], 1);
         }
@@ -107,19 +109,34 @@ __global__ void __launch_bounds__(256) tile_count_kernel(int tiles_x, int height
 }
 
 struct TileChunk {
-    int t, tiles_x, height, width, bmin, s0;
+    int t, tiles_x, th, height, width, bmin, s0;
     const int *seg_ptr;
     int *seg_cur;
     float *tcoef;
     uint16_t *tidx;
-    __device__ int npix() const { return kTilePix; }
-    __device__ bool pixel(int k, int64_t *p) const { return tile_pixel(t, k, tiles_x, height, width, p); }
+    __device__ int npix() const { return th * kTileW; }
+    __device__ bool pixel(int k, int64_t *p) const { return tile_pixel(t, k, tiles_x, th, height, width, p); }
     __device__ int base(int b) const { return seg_ptr[s0 + b - bmin]; }
     __device__ volatile int *cursor(int b) const { return seg_cur + s0 + b - bmin; }
-    __device__ void emit(int64_t pos, int k, int64_t, float coef) const { tcoef[pos] = coef; tidx[pos] = (uint16_t)k; }
+    // Entries of a segment are consumed in windows of 32 by kTileLanes = 8 lanes, lane l reading entries 4l .. 4l+3
+    // of the window with one 128-bit load.  Pixel-order entry j of a window is stored at (j % la) * 4 + j / la (la =
+    // lanes the window occupies), so that in each of a lane's four gathers the lanes read CONSECUTIVE pixels of the
+    // segment -- neighbours along the ring, which ai_tile_pos puts in different banks.
+    __device__ int64_t place(int b, int64_t pos) const
+    {
+        const int base = seg_ptr[s0 + b - bmin], plen = seg_ptr[s0 + b - bmin + 1] - base;
+        const int r = (int)(pos - base), w = r >> 5, j = r & 31;
+        const int la = min(8, (plen - 32 * w) / 4);
+        return (int64_t)base + 32 * w + (j % la) * 4 + j / la;
+    }
+    __device__ void emit(int64_t pos, int k, int64_t, float coef) const
+    {
+        tcoef[pos] = coef;
+        tidx[pos] = (uint16_t)(ai_tile_pos(k / kTileW, k % kTileW) * 4);      // byte offset in the tile buffer
+    }
 };
 
-__global__ void __launch_bounds__(128) fill_tiles_kernel(int ntiles, int tiles_x, int height, int width, int npt,
+__global__ void __launch_bounds__(128) fill_tiles_kernel(int ntiles, int tiles_x, int th, int height, int width, int npt,
                                                          const double *__restrict__ fmin_a,
                                                          const double *__restrict__ fmax_a,
                                                          const int *__restrict__ first_a, const int *__restrict__ nb_a,
@@ -130,7 +147,7 @@ __global__ void __launch_bounds__(128) fill_tiles_kernel(int ntiles, int tiles_x
 {
     int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (t >= ntiles) return;
-    TileChunk ch{t, tiles_x, height, width, tile_bmin[t], tile_seg_ptr[t], seg_ptr, seg_cur, tcoef, tidx};
+    TileChunk ch{t, tiles_x, th, height, width, tile_bmin[t], tile_seg_ptr[t], seg_ptr, seg_cur, tcoef, tidx};
     marching_fill(ch, fmin_a, fmax_a, first_a, nb_a, npt);
 }
 
@@ -180,7 +197,7 @@ __global__ void __launch_bounds__(128) bin_tiles_assign_kernel(int npt, int ntil
 // padded segment lengths: every segment a multiple of kSegPad entries (128-bit coefficient loads), every tile a
 // multiple of 8 entries so that the tile's slice of the 16-bit index array starts on a 16-byte boundary (bulk copies)
 __global__ void __launch_bounds__(128) pad_segments_kernel(int ntiles, const int *__restrict__ tile_seg_ptr,
-                                                           int *__restrict__ seg_len)
+                                                           int *__restrict__ seg_len, int *__restrict__ tile_entries)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ntiles) return;
@@ -191,10 +208,16 @@ __global__ void __launch_bounds__(128) pad_segments_kernel(int ntiles, const int
         seg_len[s] = p;
         total += p;
     }
-    if (s1 > s0 && (total & 7)) seg_len[s1 - 1] += 8 - (total & 7);
+    if (s1 > s0 && (total & 7)) {
+        seg_len[s1 - 1] += 8 - (total & 7);
+        total += 8 - (total & 7);
+    }
+    tile_entries[t] = total;
 }
 
-// {first entry, padded end, partial slot, coefficient sum as float bits} of every segment: one 128-bit load
+// {first entry, padded end, partial slot, coefficient sum as float bits} of every segment: one 128-bit load.  The
+// records of a tile are written in order of descending segment length (rank by counting, ties by bin), so that the
+// lane groups of one warp, which take consecutive records, work on segments of similar length.
 __global__ void __launch_bounds__(256) seg_meta_kernel(int ntiles, const int *__restrict__ tile_seg_ptr,
                                                        const int *__restrict__ seg_ptr, const int *__restrict__ seg_slot,
                                                        const double *__restrict__ seg_csum,
@@ -203,46 +226,100 @@ __global__ void __launch_bounds__(256) seg_meta_kernel(int ntiles, const int *__
     const int t = blockIdx.x;
     if (t >= ntiles) return;
     const int s0 = tile_seg_ptr[t], s1 = tile_seg_ptr[t + 1];
-    for (int s = s0 + threadIdx.x; s < s1; s += blockDim.x)
-        seg_meta[s] = make_int4(seg_ptr[s], seg_ptr[s + 1], seg_slot[s], __float_as_int((float)seg_csum[s]));
+    for (int s = s0 + threadIdx.x; s < s1; s += blockDim.x) {
+        const int len = seg_ptr[s + 1] - seg_ptr[s];
+        int rank = 0;
+        for (int o = s0; o < s1; ++o) {
+            const int lo = seg_ptr[o + 1] - seg_ptr[o];
+            rank += (lo > len || (lo == len && o < s)) ? 1 : 0;
+        }
+        seg_meta[s0 + rank] = make_int4(seg_ptr[s], seg_ptr[s + 1], seg_slot[s], __float_as_int((float)seg_csum[s]));
+    }
     // {first entry, number of entries, first segment, number of segments} of the tile
     if (threadIdx.x == 0) tile_desc[t] = make_int4(seg_ptr[s0], seg_ptr[s1] - seg_ptr[s0], s0, s1 - s0);
 }
 
 }  // namespace
 
-int ai_build_tiled(ai_ctx *ctx, const PixelSpans &sp, cudaStream_t st)
+static void free_tiled(TiledLayout &tl)
+{
+    cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_meta); cudaFree(tl.seg_csum);
+    cudaFree(tl.tile_desc); cudaFree(tl.tile_order); cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
+    tl = TiledLayout{};
+}
+
+// Segment structure for one tile height: tile_seg_ptr, padded seg_len, the largest tile.  Returns AI_OK and sets *fits.
+static int plan_tiles(ai_ctx *ctx, const PixelSpans &sp, int th, cudaStream_t st, int **tile_bmin, int **tile_nbins,
+                      int **seg_len, bool *fits)
 {
     TiledLayout &tl = ctx->tl;
-    const int H = ctx->height, W = ctx->width, npt = ctx->npt;
-    tl.tiles_y = (H + kTileH - 1) / kTileH;
+    const int H = ctx->height, W = ctx->width;
+    tl.tile_h = th;
+    tl.tiles_y = (H + th - 1) / th;
     tl.tiles_x = (W + kTileW - 1) / kTileW;
     tl.ntiles = tl.tiles_y * tl.tiles_x;
-    int *tile_bmin = nullptr, *tile_nbins = nullptr, *seg_len = nullptr, *seg_cur = nullptr, *nslot = nullptr;
     long long *d_total = nullptr, h_total = 0;
-    AI_CUDA(ctx, cudaMalloc(&tile_bmin, tl.ntiles * sizeof(int)));
-    AI_CUDA(ctx, cudaMalloc(&tile_nbins, tl.ntiles * sizeof(int)));
+    int *tile_entries = nullptr;
+    AI_CUDA(ctx, cudaMalloc(tile_bmin, tl.ntiles * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(tile_nbins, tl.ntiles * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&tile_entries, tl.ntiles * sizeof(int)));
     AI_CUDA(ctx, cudaMalloc(&tl.tile_seg_ptr, (tl.ntiles + 1) * sizeof(int)));
     AI_CUDA(ctx, cudaMalloc(&d_total, sizeof(long long)));
-    tile_range_kernel<<<tl.ntiles, 256, 0, st>>>(tl.tiles_x, H, W, sp.first, sp.nb, tile_bmin, tile_nbins);
-    scan_pad_kernel<<<1, 1024, 0, st>>>(tl.ntiles, tile_nbins, 1, tl.tile_seg_ptr, d_total);
+    tile_range_kernel<<<tl.ntiles, 256, 0, st>>>(tl.tiles_x, th, H, W, sp.first, sp.nb, *tile_bmin, *tile_nbins);
+    scan_pad_kernel<<<1, 1024, 0, st>>>(tl.ntiles, *tile_nbins, 1, tl.tile_seg_ptr, d_total);
     AI_CUDA(ctx, cudaGetLastError());
     AI_CUDA(ctx, cudaMemcpyAsync(&h_total, d_total, sizeof(long long), cudaMemcpyDeviceToHost, st));
     AI_CUDA(ctx, cudaStreamSynchronize(st));
+    cudaFree(d_total);
     if (h_total > 0x7fffffffLL) return ai_fail(ctx, AI_EUNSUPPORTED, "too many (tile, bin) segments: %lld", h_total);
     tl.nseg = (int)h_total;
     tl.nslot = tl.nseg;
     const size_t nseg_alloc = tl.nseg > 0 ? tl.nseg : 1;
+    AI_CUDA(ctx, cudaMalloc(seg_len, nseg_alloc * sizeof(int)));
+    AI_CUDA(ctx, cudaMemsetAsync(*seg_len, 0, nseg_alloc * sizeof(int), st));
+    tile_count_kernel<<<tl.ntiles, 256, 0, st>>>(tl.tiles_x, th, H, W, sp.first, sp.nb, *tile_bmin, tl.tile_seg_ptr,
+                                                 *seg_len);
+    pad_segments_kernel<<<(tl.ntiles + 127) / 128, 128, 0, st>>>(tl.ntiles, tl.tile_seg_ptr, *seg_len, tile_entries);
+    AI_CUDA(ctx, cudaGetLastError());
+    std::vector<int> h_entries(tl.ntiles), h_nbins(tl.ntiles);
+    AI_CUDA(ctx, cudaMemcpyAsync(h_entries.data(), tile_entries, tl.ntiles * sizeof(int), cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaMemcpyAsync(h_nbins.data(), *tile_nbins, tl.ntiles * sizeof(int), cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    cudaFree(tile_entries);
+    tl.max_tile_entries = 0;
+    tl.max_tile_segs = 0;
+    for (int t = 0; t < tl.ntiles; ++t) {
+        tl.max_tile_entries = std::max(tl.max_tile_entries, h_entries[t]);
+        tl.max_tile_segs = std::max(tl.max_tile_segs, h_nbins[t]);
+    }
+    *fits = ai_pipe_plan(tl.max_tile_entries, tl.max_tile_segs, th, false).fits;
+    return AI_OK;
+}
 
-    AI_CUDA(ctx, cudaMalloc(&seg_len, nseg_alloc * sizeof(int)));
+int ai_build_tiled(ai_ctx *ctx, const PixelSpans &sp, cudaStream_t st)
+{
+    TiledLayout &tl = ctx->tl;
+    const int H = ctx->height, W = ctx->width, npt = ctx->npt;
+    int *tile_bmin = nullptr, *tile_nbins = nullptr, *seg_len = nullptr, *seg_cur = nullptr, *nslot = nullptr;
+    long long *d_total = nullptr, h_total = 0;
+    // largest tile height whose slices fit the pipelined kernel (8 is taken regardless: the direct kernel serves it)
+    for (int th = kTileHMax;; th /= 2) {
+        bool fits = false;
+        int rc = plan_tiles(ctx, sp, th, st, &tile_bmin, &tile_nbins, &seg_len, &fits);
+        if (rc != AI_OK) return rc;
+        if (fits || th == 8) break;
+        cudaFree(tile_bmin); cudaFree(tile_nbins); cudaFree(seg_len);
+        tile_bmin = tile_nbins = seg_len = nullptr;
+        free_tiled(tl);
+    }
+    const int th = tl.tile_h;
+    const size_t nseg_alloc = tl.nseg > 0 ? tl.nseg : 1;
+    AI_CUDA(ctx, cudaMalloc(&d_total, sizeof(long long)));
     AI_CUDA(ctx, cudaMalloc(&seg_cur, nseg_alloc * sizeof(int)));
     AI_CUDA(ctx, cudaMalloc(&tl.seg_ptr, (nseg_alloc + 1) * sizeof(int)));
     AI_CUDA(ctx, cudaMalloc(&tl.seg_slot, nseg_alloc * sizeof(int)));
     AI_CUDA(ctx, cudaMalloc(&tl.seg_csum, nseg_alloc * sizeof(double)));
-    AI_CUDA(ctx, cudaMemsetAsync(seg_len, 0, nseg_alloc * sizeof(int), st));
     AI_CUDA(ctx, cudaMemsetAsync(seg_cur, 0, nseg_alloc * sizeof(int), st));
-    tile_count_kernel<<<tl.ntiles, 256, 0, st>>>(tl.tiles_x, H, W, sp.first, sp.nb, tile_bmin, tl.tile_seg_ptr, seg_len);
-    pad_segments_kernel<<<(tl.ntiles + 127) / 128, 128, 0, st>>>(tl.ntiles, tl.tile_seg_ptr, seg_len);
     scan_pad_kernel<<<1, 1024, 0, st>>>(tl.nseg, seg_len, 1, tl.seg_ptr, d_total);
     AI_CUDA(ctx, cudaGetLastError());
     AI_CUDA(ctx, cudaMemcpyAsync(&h_total, d_total, sizeof(long long), cudaMemcpyDeviceToHost, st));
@@ -255,9 +332,9 @@ int ai_build_tiled(ai_ctx *ctx, const PixelSpans &sp, cudaStream_t st)
     AI_CUDA(ctx, cudaMalloc(&tl.tidx, nnz_alloc * sizeof(uint16_t)));
     AI_CUDA(ctx, cudaMemsetAsync(tl.tcoef, 0, nnz_alloc * sizeof(float), st));       // padding: coefficient 0,
     AI_CUDA(ctx, cudaMemsetAsync(tl.tidx, 0, nnz_alloc * sizeof(uint16_t), st));     // pixel 0 of the tile
-    fill_tiles_kernel<<<(tl.ntiles + 3) / 4, 128, 0, st>>>(tl.ntiles, tl.tiles_x, H, W, npt, sp.fmin, sp.fmax, sp.first,
-                                                           sp.nb, tile_bmin, tl.tile_seg_ptr, tl.seg_ptr, seg_cur,
-                                                           tl.tcoef, tl.tidx);
+    fill_tiles_kernel<<<(tl.ntiles + 3) / 4, 128, 0, st>>>(tl.ntiles, tl.tiles_x, th, H, W, npt, sp.fmin, sp.fmax,
+                                                           sp.first, sp.nb, tile_bmin, tl.tile_seg_ptr, tl.seg_ptr,
+                                                           seg_cur, tl.tcoef, tl.tidx);
     if (tl.nseg > 0)
         seg_sum_kernel<<<(tl.nseg + 7) / 8, 256, 0, st>>>(tl.nseg, tl.seg_ptr, tl.tcoef, tl.seg_csum);
 
@@ -280,12 +357,6 @@ int ai_build_tiled(ai_ctx *ctx, const PixelSpans &sp, cudaStream_t st)
     std::vector<int> order(tl.ntiles);
     for (int t = 0; t < tl.ntiles; ++t) order[t] = t;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return desc[a].y > desc[b].y; });
-    tl.max_tile_entries = 0;
-    tl.max_tile_segs = 0;
-    for (const int4 &d : desc) {
-        tl.max_tile_entries = std::max(tl.max_tile_entries, d.y);
-        tl.max_tile_segs = std::max(tl.max_tile_segs, d.w);
-    }
     // tile_desc is kept in the same longest-first order as tile_order (the pipelined kernel indexes both by rank)
     std::vector<int4> desc_lpt(tl.ntiles);
     for (int r = 0; r < tl.ntiles; ++r) desc_lpt[r] = desc[order[r]];

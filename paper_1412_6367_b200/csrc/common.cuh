@@ -111,6 +111,7 @@ template <> struct Accum<AI_ACC_F32_KAHAN> {
         c = __fsub_rn(__fadd_rn(c, c2), e);
         s = t;
     }
+    __device__ __forceinline__ void absorb(const Accum &o) { merge(o.s, o.c); }
     __device__ __forceinline__ void warp_reduce()
     {
 #pragma unroll
@@ -128,6 +129,7 @@ template <> struct Accum<AI_ACC_F32_PLAIN> {
     float s = 0.0f;
     __device__ __forceinline__ void add(float coef, float v) { s = __fmaf_rn(coef, v, s); }
     __device__ __forceinline__ void add1(float x) { s = __fadd_rn(s, x); }
+    __device__ __forceinline__ void absorb(const Accum &o) { s = __fadd_rn(s, o.s); }
     __device__ __forceinline__ void warp_reduce()
     {
 #pragma unroll
@@ -141,6 +143,7 @@ template <> struct Accum<AI_ACC_F64> {
     double s = 0.0;
     __device__ __forceinline__ void add(float coef, float v) { s = fma((double)coef, (double)v, s); }
     __device__ __forceinline__ void add1(float x) { s += (double)x; }
+    __device__ __forceinline__ void absorb(const Accum &o) { s += o.s; }
     __device__ __forceinline__ void warp_reduce()
     {
 #pragma unroll

@@ -6,26 +6,76 @@
 
 #include "../../include/azint.h"
 
-// Tile of the detector staged in shared memory by the TILED layout.
-constexpr int kTileH = 64;
+// Tile of the detector staged in shared memory by the TILED layout: kTileW pixels wide and
+// tile_h rows high, tile_h chosen at build time (64, 32, 16 or 8) so that two tiles' slices of the matrix plus the
+// image ring fit the shared memory of one SM.
 constexpr int kTileW = 64;
-constexpr int kTilePix = kTileH * kTileW;
+constexpr int kTileHMax = 64;
+constexpr int kTilePixMax = kTileHMax * kTileW;
 constexpr int kSegPad = 4;   // segments are padded to a multiple of 4 entries (one 128-bit coefficient load)
 
+// Position of pixel (ly, lx) of a tile inside its shared-memory buffer.  Rows are rotated by one 16-byte chunk per
+// row, so pixels above each other (a ring crossing the tile vertically) fall in different banks while every aligned
+// group of 4 pixels stays contiguous for 128-bit stores.  The matrix stores these positions, not ly * kTileW + lx.
+__host__ __device__ inline int ai_tile_pos(int ly, int lx)
+{
+    return (ly * kTileW) | ((((lx >> 2) + ly) & (kTileW / 4 - 1)) << 2) | (lx & 3);
+}
+
+// Shared-memory plan of the pipelined stage-1 kernel (integrate_pipe.cu), needed by the builder to pick tile_h.
+// Every image stage belongs to one stager warp, so there are at most kPipeMaxImgStages of them; the matrix ring is
+// double-buffered for single frames and single-buffered for batches (one slice serves many frames there).
+constexpr int kPipeSmemBudget = 227 * 1024;
+constexpr int kPipeHeaderBytes = 512;
+constexpr int kPipeMaxImgStages = 7;
+constexpr int kPipeMinImgStages = 3;
+struct PipePlan {
+    int coef_bytes, idx_bytes, meta_bytes, mat_stage_bytes, mat_stages, img_stage_bytes, img_stages;
+    size_t smem;
+    bool fits;
+};
+inline int ai_align128(int x) { return (x + 127) & ~127; }
+inline PipePlan ai_pipe_plan(int max_tile_entries, int max_tile_segs, int tile_h, bool batch)
+{
+    PipePlan p{};
+    p.coef_bytes = ai_align128(max_tile_entries * 4);
+    p.idx_bytes = ai_align128(max_tile_entries * 2);
+    p.meta_bytes = ai_align128(max_tile_segs * 16);
+    p.mat_stage_bytes = p.coef_bytes + p.idx_bytes + p.meta_bytes;
+    p.img_stage_bytes = tile_h * kTileW * 4;
+    // Single frame: bulk copies need about 100 KB in flight per SM to stream at full rate (measured, DESIGN.md
+    // section 5.3), i.e. two slices loading while a third is consumed; fall back to two stages for large slices.
+    // Batch: one slice serves many frames, all the room goes to image stages.
+    const int img_cap = batch ? kPipeMaxImgStages : 4;
+    for (p.mat_stages = batch ? 1 : 3; p.mat_stages >= (batch ? 1 : 2); --p.mat_stages) {
+        const int room = kPipeSmemBudget - kPipeHeaderBytes - p.mat_stages * p.mat_stage_bytes;
+        p.img_stages = room > 0 ? room / p.img_stage_bytes : 0;
+        if (p.img_stages > img_cap) p.img_stages = img_cap;
+        if (p.img_stages >= kPipeMinImgStages) break;
+    }
+    if (p.mat_stages < 1) p.mat_stages = 1;
+    p.fits = p.img_stages >= kPipeMinImgStages;
+    p.smem = (size_t)kPipeHeaderBytes + (size_t)p.mat_stages * p.mat_stage_bytes + (size_t)p.img_stages * p.img_stage_bytes;
+    return p;
+}
+
 struct TiledLayout {
+    int tile_h = 0;                // rows per tile
     int tiles_y = 0, tiles_x = 0, ntiles = 0;
     int nseg = 0;                  // number of (tile, bin) segments
     int64_t tnnz = 0;              // padded number of entries
     int *tile_seg_ptr = nullptr;   // [ntiles+1] first segment of each tile
-    int *seg_ptr = nullptr;        // [nseg+1]   first entry of each segment (multiple of kSegPad)
+    int *seg_ptr = nullptr;        // [nseg+1]   first entry of each segment (multiple of kSegPad), segments in bin order
     int *seg_slot = nullptr;       // [nseg]     slot of the segment's partial in the bin-major partial buffer
-    int4 *seg_meta = nullptr;      // [nseg]     {first entry, padded end, partial slot, float bits of the coefficient sum}
+    int4 *seg_meta = nullptr;      // [nseg]     {first entry, padded end, partial slot, float bits of the coefficient
+                                   //            sum}; within a tile ordered by descending length (lanes of a warp work
+                                   //            on segments of similar length)
     int4 *tile_desc = nullptr;     // [ntiles]   {first entry, number of entries, first segment, number of segments}
     int *tile_order = nullptr;     // [ntiles]   tiles by descending number of entries (longest first scheduling)
     int max_tile_entries = 0, max_tile_segs = 0;
     double *seg_csum = nullptr;    // [nseg]     sum of the segment's coefficients (count when every pixel is valid)
     float *tcoef = nullptr;        // [tnnz]     coefficient
-    uint16_t *tidx = nullptr;      // [tnnz]     pixel index inside the tile (ly * kTileW + lx)
+    uint16_t *tidx = nullptr;      // [tnnz]     ai_tile_pos of the pixel inside the tile
     int *bin_slot_ptr = nullptr;   // [npt+1]    partial slots of bin b are [bin_slot_ptr[b], bin_slot_ptr[b+1])
     int nslot = 0;                 // == nseg
 };

@@ -23,7 +23,7 @@ struct TiledView {
     const int4 *seg_meta;
     const float *tcoef;
     const uint16_t *tidx;
-    int tiles_x, nslot;
+    int tiles_x, tile_h, nslot;
 };
 
 constexpr int kS1Threads = 128;                       // 12 blocks per SM: one wave holds 1776 tiles
@@ -42,7 +42,7 @@ __device__ __forceinline__ void process_segments(const TiledView &tv, const floa
     while (__any_sync(AI_FULL_MASK, s < s_end)) {
         const int s_next = s + kGroups;
         const int4 m_next = s_next < s_end ? __ldg(tv.seg_meta + s_next) : make_int4(0, 0, 0, 0);
-        Accum<ACC> S, C;
+        Accum2<ACC> S2, C2;
         const int end = m.y;
         int k = m.x + gl * 4;
         // software pipeline: loads for step i+1 are issued before step i is consumed
@@ -58,11 +58,12 @@ __device__ __forceinline__ void process_segments(const TiledView &tv, const floa
                 cb = __ldg(reinterpret_cast<const float4 *>(tv.tcoef + k2));
                 ib = __ldg(reinterpret_cast<const ushort4 *>(tv.tidx + k2));
             }
-            consume4<ACC, TRACK>(tile, ca, ia, S, C);
+            consume4<ACC, TRACK>(tile, ca, ia, S2, C2);
             ca = cb;
             ia = ib;
             k = k2;
         }
+        Accum<ACC> S = S2.total(), C = C2.total();
         group_reduce<ACC>(S);
         if constexpr (TRACK) group_reduce<ACC>(C);
         if (gl == 0 && s < s_end) store_partial<ACC>(part_f, m.z, S, C, TRACK, (double)__int_as_float(m.w));
@@ -77,12 +78,13 @@ __global__ void __launch_bounds__(kS1Threads, kS1MinBlocks) tiled_stage1_kernel(
                                                                                 int height, int width, int vec_ok,
                                                                                 void *partials)
 {
-    __shared__ __align__(16) float tile[kTilePix];
+    __shared__ __align__(16) float tile[kTilePixMax];
     using T = typename RawType<DT>::T;
     const int t = blockIdx.x, f = blockIdx.y;
     const int ty = t / tv.tiles_x, tx = t - ty * tv.tiles_x;
     const void *img = reinterpret_cast<const T *>(frames) + (int64_t)f * frame_stride;
-    const bool bad = stage_tile<DT, kS1Threads>(tile, img, cor, ty, tx, height, width, vec_ok, threadIdx.x);
+    const bool bad = stage_tile<DT, kS1Threads, 8, 2>(tile, img, cor, ty, tx, tv.tile_h, height, width, vec_ok, threadIdx.x,
+                                                [] {});
     // some pixel of the tile is invalid -> count must be accumulated too; else it is the static coefficient sum
     const bool track = __syncthreads_or(bad) != 0;
     void *part_f = reinterpret_cast<char *>(partials) + (int64_t)f * tv.nslot * 16;
@@ -144,7 +146,7 @@ template <int DT, int ACC>
 int launch_simple(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st)
 {
     const TiledLayout &tl = ctx->tl;
-    TiledView tv{tl.tile_seg_ptr, tl.seg_meta, tl.tcoef, tl.tidx, tl.tiles_x, tl.nslot};
+    TiledView tv{tl.tile_seg_ptr, tl.seg_meta, tl.tcoef, tl.tidx, tl.tiles_x, tl.tile_h, tl.nslot};
     Corrections cor{a.dark, a.flat, a.solidangle, a.polarization, a.mask};
     dim3 g1(tl.ntiles, a.nframes);
     ai_prof_begin(ctx, st);

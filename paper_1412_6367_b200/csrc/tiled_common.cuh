@@ -1,11 +1,22 @@
 // Pieces shared by the two TILED stage-1 kernels (integrate_tiled.cu: one block per tile; integrate_pipe.cu: persistent,
-// warp-specialised, bulk-copy pipelined): tile staging with fused cast + corrections, the per-lane
-// accumulate step, the merge inside a group of lanes (PAPER.md:186-188 compensated sums) and the partial record.
+// warp-specialised, bulk-copy pipelined): the per-lane accumulators (PAPER.md:186-188 compensated sums), the merge
+// inside a group of lanes, the partial record, and tile staging with fused cast + corrections.
 #pragma once
 #include "common.cuh"
 
 constexpr int kLanes = 8;            // lanes cooperating on one (tile, bin) segment
 constexpr int kStep = kLanes * 4;    // entries consumed per group per 128-bit coefficient load
+
+// two interleaved accumulators per lane (even / odd entries): halves the dependent chain of the Kahan recurrence
+template <int ACC> struct Accum2 {
+    Accum<ACC> a, b;
+    __device__ __forceinline__ Accum<ACC> total() const
+    {
+        Accum<ACC> r = a;
+        r.absorb(b);
+        return r;
+    }
+};
 
 template <int ACC>
 __device__ __forceinline__ void group_reduce(Accum<ACC> &a)
@@ -40,91 +51,132 @@ __device__ __forceinline__ void store_partial(void *partials, int64_t slot, cons
     }
 }
 
-// four matrix entries against the staged tile; TRACK: the tile holds invalid (NaN) pixels, so count is accumulated too
-template <int ACC, bool TRACK>
-__device__ __forceinline__ void consume4(const float *tile, const float4 &c4, const ushort4 &i4, Accum<ACC> &S,
-                                         Accum<ACC> &C)
+// value of the pixel whose position in the tile buffer is stored as a byte offset
+__device__ __forceinline__ float tile_at(const float *tile, unsigned off)
 {
-    const float c[4] = {c4.x, c4.y, c4.z, c4.w};
-    const float v[4] = {tile[i4.x], tile[i4.y], tile[i4.z], tile[i4.w]};
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        if constexpr (TRACK) {
-            bool ok = v[e] == v[e];
-            S.add(c[e], ok ? v[e] : 0.0f);
-            C.add1(ok ? c[e] : 0.0f);
-        } else {
-            S.add(c[e], v[e]);
-        }
-    }
+    return *reinterpret_cast<const float *>(reinterpret_cast<const char *>(tile) + off);
+}
+__device__ __forceinline__ float4 gather4(const float *tile, const ushort4 &x)
+{
+    return make_float4(tile_at(tile, x.x), tile_at(tile, x.y), tile_at(tile, x.z), tile_at(tile, x.w));
 }
 
-// H1 + H2: load tile (ty, tx) of one frame, cast, correct, park in shared memory; NT threads cooperate, `tid` in [0, NT).
+// four matrix entries against four gathered pixel values; TRACK: the tile holds invalid (NaN) pixels, so count is
+// accumulated too
+template <int ACC, bool TRACK>
+__device__ __forceinline__ void accumulate4(const float4 &c4, const float4 &v, Accum2<ACC> &S, Accum2<ACC> &C)
+{
+    if constexpr (TRACK) {
+        const bool k0 = v.x == v.x, k1 = v.y == v.y, k2 = v.z == v.z, k3 = v.w == v.w;
+        S.a.add(c4.x, k0 ? v.x : 0.0f);
+        S.b.add(c4.y, k1 ? v.y : 0.0f);
+        S.a.add(c4.z, k2 ? v.z : 0.0f);
+        S.b.add(c4.w, k3 ? v.w : 0.0f);
+        C.a.add1(k0 ? c4.x : 0.0f);
+        C.b.add1(k1 ? c4.y : 0.0f);
+        C.a.add1(k2 ? c4.z : 0.0f);
+        C.b.add1(k3 ? c4.w : 0.0f);
+    } else {
+        S.a.add(c4.x, v.x);
+        S.b.add(c4.y, v.y);
+        S.a.add(c4.z, v.z);
+        S.b.add(c4.w, v.w);
+    }
+}
+template <int ACC, bool TRACK>
+__device__ __forceinline__ void consume4(const float *tile, const float4 &c4, const ushort4 &i4, Accum2<ACC> &S,
+                                         Accum2<ACC> &C)
+{
+    accumulate4<ACC, TRACK>(c4, gather4(tile, i4), S, C);
+}
+
+// ---- H1 + H2: tile staging ---------------------------------------------------------------------------------------------
+// Loads tile (ty, tx) of one frame, casts, corrects, and parks it in shared memory at ai_tile_pos; NT threads cooperate
+// (`tid` in [0, NT)).  All loads of a batch are issued before the first is used, so a thread keeps BATCH 128-bit loads
+// per array in flight; `acquire()` is called once, after the first batch's loads were issued and before the first
+// store (the pipelined kernel waits for its shared-memory stage there, so the wait overlaps the load latency).
 // Returns true if this thread met an invalid pixel (masked, zero / non-finite denominator, non-finite value).
-template <int DT, int NT>
+template <int DT, int NT, int BP, int BC, class Acquire>   // BP / BC: batch size without / with correction arrays
 __device__ __forceinline__ bool stage_tile(float *tile, const void *img, const Corrections &cor, int ty, int tx,
-                                           int height, int width, int vec_ok, int tid)
+                                           int th, int height, int width, int vec_ok, int tid, Acquire acquire)
 {
     const bool has_den = cor.flat || cor.solidangle || cor.polarization;
     const bool plain = !cor.dark && !has_den && !cor.mask;
-    bool bad = false;
+    const int nchunk = th * (kTileW / 4);
+    const int y0 = ty * th, x0 = tx * kTileW;
+    bool bad = false, acquired = false;
     if (vec_ok && plain) {
-        // no correction arrays: all of the thread's 128-bit loads are in flight together
-        constexpr int kPer = kTilePix / 4 / NT;
-        float4 v[kPer];
+        constexpr int B = BP;
+        for (int q0 = tid; q0 < nchunk; q0 += NT * B) {
+            float4 v[B];
 #pragma unroll
-        for (int i = 0; i < kPer; ++i) {
-            int q = tid + i * NT;
-            int y = ty * kTileH + q / (kTileW / 4), x = tx * kTileW + (q % (kTileW / 4)) * 4;
-            v[i] = (y < height && x < width) ? load_raw4<DT>(img, (int64_t)y * width + x) : make_float4(0, 0, 0, 0);
-        }
-#pragma unroll
-        for (int i = 0; i < kPer; ++i) {
-            if constexpr (DT == AI_F32) {
-                bool b = !finite_f(v[i].x) || !finite_f(v[i].y) || !finite_f(v[i].z) || !finite_f(v[i].w);
-                if (b) {
-                    v[i].x = finite_f(v[i].x) ? v[i].x : quiet_nan();
-                    v[i].y = finite_f(v[i].y) ? v[i].y : quiet_nan();
-                    v[i].z = finite_f(v[i].z) ? v[i].z : quiet_nan();
-                    v[i].w = finite_f(v[i].w) ? v[i].w : quiet_nan();
-                    bad = true;
-                }
+            for (int i = 0; i < B; ++i) {
+                const int q = q0 + i * NT, y = y0 + (q >> 4), x = x0 + (q & 15) * 4;
+                v[i] = (q < nchunk && y < height && x < width) ? load_raw4<DT>(img, (int64_t)y * width + x)
+                                                               : make_float4(0, 0, 0, 0);
             }
-            reinterpret_cast<float4 *>(tile)[tid + i * NT] = v[i];
+            if (!acquired) { acquire(); acquired = true; }
+#pragma unroll
+            for (int i = 0; i < B; ++i) {
+                const int q = q0 + i * NT;
+                if constexpr (DT == AI_F32) {
+                    if (!finite_f(v[i].x) || !finite_f(v[i].y) || !finite_f(v[i].z) || !finite_f(v[i].w)) {
+                        v[i].x = finite_f(v[i].x) ? v[i].x : quiet_nan();
+                        v[i].y = finite_f(v[i].y) ? v[i].y : quiet_nan();
+                        v[i].z = finite_f(v[i].z) ? v[i].z : quiet_nan();
+                        v[i].w = finite_f(v[i].w) ? v[i].w : quiet_nan();
+                        bad = true;
+                    }
+                }
+                if (q < nchunk) *reinterpret_cast<float4 *>(tile + ai_tile_pos(q >> 4, (q & 15) * 4)) = v[i];
+            }
         }
     } else if (vec_ok) {
-        for (int q = tid; q < kTilePix / 4; q += NT) {
-            int ly = q / (kTileW / 4), lx = (q % (kTileW / 4)) * 4;
-            int y = ty * kTileH + ly, x = tx * kTileW + lx;
-            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (y < height && x < width) {
-                int64_t p = (int64_t)y * width + x;
-                float4 raw = load_raw4<DT>(img, p);
-                float4 dk = cor.dark ? __ldg(reinterpret_cast<const float4 *>(cor.dark + p)) : make_float4(0, 0, 0, 0);
-                float4 fl = cor.flat ? __ldg(reinterpret_cast<const float4 *>(cor.flat + p)) : make_float4(1, 1, 1, 1);
-                float4 sa = cor.solidangle ? __ldg(reinterpret_cast<const float4 *>(cor.solidangle + p))
-                                           : make_float4(1, 1, 1, 1);
-                float4 po = cor.polarization ? __ldg(reinterpret_cast<const float4 *>(cor.polarization + p))
-                                             : make_float4(1, 1, 1, 1);
-                uchar4 mk = cor.mask ? __ldg(reinterpret_cast<const uchar4 *>(cor.mask + p)) : make_uchar4(0, 0, 0, 0);
-                v.x = correct_value(raw.x, dk.x, fl.x, sa.x, po.x, mk.x != 0, has_den);
-                v.y = correct_value(raw.y, dk.y, fl.y, sa.y, po.y, mk.y != 0, has_den);
-                v.z = correct_value(raw.z, dk.z, fl.z, sa.z, po.z, mk.z != 0, has_den);
-                v.w = correct_value(raw.w, dk.w, fl.w, sa.w, po.w, mk.w != 0, has_den);
-                bad = bad || v.x != v.x || v.y != v.y || v.z != v.z || v.w != v.w;
+        constexpr int B = BC;
+        const float4 one4 = make_float4(1, 1, 1, 1), zero4 = make_float4(0, 0, 0, 0);
+        for (int q0 = tid; q0 < nchunk; q0 += NT * B) {
+            float4 raw[B], dk[B], fl[B], sa[B], po[B];
+            uchar4 mk[B];
+            bool in[B];
+#pragma unroll
+            for (int i = 0; i < B; ++i) {
+                const int q = q0 + i * NT, y = y0 + (q >> 4), x = x0 + (q & 15) * 4;
+                const int64_t p = (int64_t)y * width + x;
+                in[i] = q < nchunk && y < height && x < width;
+                raw[i] = in[i] ? load_raw4<DT>(img, p) : zero4;
+                dk[i] = (in[i] && cor.dark) ? __ldg(reinterpret_cast<const float4 *>(cor.dark + p)) : zero4;
+                fl[i] = (in[i] && cor.flat) ? __ldg(reinterpret_cast<const float4 *>(cor.flat + p)) : one4;
+                sa[i] = (in[i] && cor.solidangle) ? __ldg(reinterpret_cast<const float4 *>(cor.solidangle + p)) : one4;
+                po[i] = (in[i] && cor.polarization) ? __ldg(reinterpret_cast<const float4 *>(cor.polarization + p)) : one4;
+                mk[i] = (in[i] && cor.mask) ? __ldg(reinterpret_cast<const uchar4 *>(cor.mask + p)) : make_uchar4(0, 0, 0, 0);
             }
-            reinterpret_cast<float4 *>(tile)[q] = v;
+            if (!acquired) { acquire(); acquired = true; }
+#pragma unroll
+            for (int i = 0; i < B; ++i) {
+                const int q = q0 + i * NT;
+                float4 v = zero4;
+                if (in[i]) {
+                    v.x = correct_value(raw[i].x, dk[i].x, fl[i].x, sa[i].x, po[i].x, mk[i].x != 0, has_den);
+                    v.y = correct_value(raw[i].y, dk[i].y, fl[i].y, sa[i].y, po[i].y, mk[i].y != 0, has_den);
+                    v.z = correct_value(raw[i].z, dk[i].z, fl[i].z, sa[i].z, po[i].z, mk[i].z != 0, has_den);
+                    v.w = correct_value(raw[i].w, dk[i].w, fl[i].w, sa[i].w, po[i].w, mk[i].w != 0, has_den);
+                    bad = bad || v.x != v.x || v.y != v.y || v.z != v.z || v.w != v.w;
+                }
+                if (q < nchunk) *reinterpret_cast<float4 *>(tile + ai_tile_pos(q >> 4, (q & 15) * 4)) = v;
+            }
         }
     } else {
-        for (int k = tid; k < kTilePix; k += NT) {
-            int y = ty * kTileH + k / kTileW, x = tx * kTileW + k % kTileW;
+        acquire();
+        for (int k = tid; k < th * kTileW; k += NT) {
+            const int ly = k / kTileW, lx = k % kTileW, y = y0 + ly, x = x0 + lx;
             float v = 0.f;
             if (y < height && x < width) {
                 v = corrected_pixel<DT>(img, (int64_t)y * width + x, cor);
                 bad = bad || v != v;
             }
-            tile[k] = v;
+            tile[ai_tile_pos(ly, lx)] = v;
         }
     }
+    if (!acquired) acquire();
     return bad;
 }
