@@ -85,6 +85,8 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
         ctx->range_host[0] = range_or_null[0];
         ctx->range_host[1] = range_or_null[1];
     }
+    const char *e = getenv("AZINT_NO_TMA");
+    ctx->no_tma = e && e[0] == '1';
     *out = ctx;
     return AI_OK;
 }
@@ -221,7 +223,7 @@ void ai_destroy(ai_ctx *ctx)
     cudaFree(ctx->lut_coef); cudaFree(ctx->lut_idx);
     TiledLayout &tl = ctx->tl;
     cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_meta); cudaFree(tl.seg_csum);
-    cudaFree(tl.tile_desc); cudaFree(tl.tile_order);
+    cudaFree(tl.tile_desc); cudaFree(tl.tile_order); cudaFree(tl.blob); cudaFree(tl.blob_desc);
     cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
     cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);

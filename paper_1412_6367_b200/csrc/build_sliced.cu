@@ -1,0 +1,279 @@
+// Sliced execution layout (SURVEY.md section 8(a) B6 "derived layouts"): the entries of the tiled
+// layout (build_tiled.cu: same coefficients as the canonical CSR) cut into slices of at most
+// kSliceMax entries and packed, 32 slices of similar length at a time, into blocks that one warp consumes with one
+// lane per slice.  A tile's blocks form one blob moved to shared memory by a single bulk copy (ctx.h).
+//
+// Order of the slices of a tile: all full slices (kSliceMax entries) in (bin, position) order, then the last, shorter
+// slice of every segment by descending length, bins ascending among equals.  Adjacent lanes of a block that belong to
+// the same segment form a run; a run yields one partial sum per frame.
+#include <algorithm>
+#include <vector>
+
+#include "ctx.h"
+
+namespace {
+
+struct SegLens {                 // padded segment lengths either as an array or as differences of seg_ptr
+    const int *len, *ptr;
+    __device__ int operator()(int s) const { return len ? len[s] : ptr[s + 1] - ptr[s]; }
+};
+
+// steps (groups of 4 entries) of the slice at sorted position i of a tile with nfull full slices and cnt[r] last
+// slices of r steps
+__device__ __forceinline__ int slice_steps_at(int i, int nfull, const int *cnt)
+{
+    if (i < nfull) return kSliceSteps;
+    i -= nfull;
+    for (int r = kSliceSteps - 1; r >= 1; --r) {
+        if (i < cnt[r]) return r;
+        i -= cnt[r];
+    }
+    return 0;
+}
+
+__device__ __forceinline__ void tile_slice_counts(const SegLens &L, int s0, int s1, int *nfull, int *cnt)
+{
+    *nfull = 0;
+    for (int r = 0; r < kSliceSteps; ++r) cnt[r] = 0;
+    for (int s = s0; s < s1; ++s) {
+        const int n = L(s);
+        *nfull += n / kSliceMax;
+        const int r = (n % kSliceMax) / 4;
+        if (r) cnt[r]++;
+    }
+}
+
+// per tile: number of slices, number of blocks, bytes of the blob
+__global__ void __launch_bounds__(64) slice_plan_kernel(int ntiles, const int *__restrict__ tile_seg_ptr, SegLens L,
+                                                        int *__restrict__ tile_nslices, int *__restrict__ tile_nblk,
+                                                        int *__restrict__ tile_blob_bytes)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntiles) return;
+    int nfull, cnt[kSliceSteps];
+    tile_slice_counts(L, tile_seg_ptr[t], tile_seg_ptr[t + 1], &nfull, cnt);
+    int S = nfull;
+    for (int r = 1; r < kSliceSteps; ++r) S += cnt[r];
+    const int nblk = (S + 31) / 32;
+    int bytes = (4 * (1 + nblk) + 15) / 16 * 16;
+    for (int b = 0; b < nblk; ++b) bytes += slice_steps_at(32 * b, nfull, cnt) * kBlkStepBytes + kBlkMetaBytes;
+    tile_nslices[t] = S;
+    tile_nblk[t] = nblk;
+    tile_blob_bytes[t] = bytes;
+}
+
+// per tile (one thread): which (segment, window of 32 entries) every slice is, the runs, the blob header
+__global__ void __launch_bounds__(64) slice_assign_kernel(int ntiles, const int *__restrict__ tile_seg_ptr, SegLens L,
+                                                          const int *__restrict__ tile_slice_ptr,
+                                                          const long long *__restrict__ tile_blob_off,
+                                                          int *__restrict__ slice_seg, int *__restrict__ slice_win,
+                                                          int *__restrict__ slice_run, int *__restrict__ seg_nruns,
+                                                          unsigned char *__restrict__ blob)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntiles) return;
+    const int s0 = tile_seg_ptr[t], s1 = tile_seg_ptr[t + 1];
+    int nfull, cnt[kSliceSteps], part_pos[kSliceSteps];
+    tile_slice_counts(L, s0, s1, &nfull, cnt);
+    int S = nfull;
+    for (int r = kSliceSteps - 1; r >= 1; --r) { part_pos[r] = S; S += cnt[r]; }
+    const int g0 = tile_slice_ptr[t];
+    int full_pos = 0;
+    for (int s = s0; s < s1; ++s) {
+        const int n = L(s), nf = n / kSliceMax, r = (n % kSliceMax) / 4;
+        for (int k = 0; k < nf; ++k, ++full_pos) { slice_seg[g0 + full_pos] = s; slice_win[g0 + full_pos] = k; }
+        if (r) { const int i = part_pos[r]++; slice_seg[g0 + i] = s; slice_win[g0 + i] = nf; }
+        seg_nruns[s] = 0;
+    }
+    // runs: adjacent lanes of one block with the same segment; run index counted per segment in slice order
+    int run = 0;
+    for (int i = 0; i < S; ++i) {
+        const int s = slice_seg[g0 + i];
+        const bool head = (i & 31) == 0 || slice_seg[g0 + i - 1] != s;
+        if (head) run = seg_nruns[s]++;
+        slice_run[g0 + i] = run | (head ? (int)0x80000000 : 0);
+    }
+    // lanes of the run after this one (backwards), longest run of every block -> reduction rounds
+    unsigned *hdr = reinterpret_cast<unsigned *>(blob + tile_blob_off[t]);
+    const int nblk = (S + 31) / 32;
+    hdr[0] = (unsigned)nblk;
+    int off = (4 * (1 + nblk) + 15) / 16 * 16;
+    for (int b = 0; b < nblk; ++b) {
+        const int lo = 32 * b, hi = min(S, lo + 32);
+        int rem = 0, maxrun = 1;
+        for (int i = hi - 1; i >= lo; --i) {
+            const bool last = i == hi - 1 || (slice_run[g0 + i + 1] < 0);
+            rem = last ? 0 : rem + 1;
+            maxrun = max(maxrun, rem + 1);
+            slice_run[g0 + i] |= rem << 24;
+        }
+        int rounds = 0;
+        while ((1 << rounds) < maxrun) ++rounds;
+        const int nsteps = slice_steps_at(lo, nfull, cnt);
+        hdr[1 + b] = ((unsigned)(off / 16) << 8) | ((unsigned)rounds << 4) | (unsigned)nsteps;
+        off += nsteps * kBlkStepBytes + kBlkMetaBytes;
+    }
+}
+
+// one thread block per tile: copy the entries of every slice into its lane of its block, write the lane records
+__global__ void __launch_bounds__(256) slice_fill_kernel(const int *__restrict__ tile_slice_ptr,
+                                                         const long long *__restrict__ tile_blob_off,
+                                                         const int *__restrict__ slice_seg,
+                                                         const int *__restrict__ slice_win,
+                                                         const int *__restrict__ slice_run,
+                                                         const int *__restrict__ seg_ptr, const int *__restrict__ seg_slot,
+                                                         const float *__restrict__ tcoef,
+                                                         const uint16_t *__restrict__ tidx, unsigned char *__restrict__ blob)
+{
+    const int t = blockIdx.x;
+    const int g0 = tile_slice_ptr[t], S = tile_slice_ptr[t + 1] - g0;
+    unsigned char *tb = blob + tile_blob_off[t];
+    const unsigned *hdr = reinterpret_cast<const unsigned *>(tb);
+    for (int w = threadIdx.x; w < S * kSliceSteps; w += blockDim.x) {
+        const int i = w / kSliceSteps, step = w % kSliceSteps, b = i >> 5, lane = i & 31;
+        const unsigned h = hdr[1 + b];
+        const int nsteps = h & 15;
+        unsigned char *blk = tb + (size_t)(h >> 8) * 16;
+        const int s = slice_seg[g0 + i], win = slice_win[g0 + i];
+        const int base = seg_ptr[s] + kSliceMax * win;
+        const int len = min(kSliceMax, seg_ptr[s + 1] - base);
+        if (step * 4 < len) {      // the rest of the block stays zero: coefficient 0 at pixel 0 of the tile
+            const float4 c = *reinterpret_cast<const float4 *>(tcoef + base + step * 4);
+            const ushort4 x = *reinterpret_cast<const ushort4 *>(tidx + base + step * 4);
+            reinterpret_cast<float4 *>(blk)[step * 32 + lane] = c;
+            reinterpret_cast<ushort4 *>(blk + (size_t)nsteps * 512)[step * 32 + lane] = x;
+        }
+        if (step == 0) {
+            const int r = slice_run[g0 + i];
+            int2 m = make_int2(r & 0x1f000000, 0);
+            if (r < 0) {
+                const int rem = (r >> 24) & 31;
+                double sum = 0.0;      // coefficient sum of the run, fixed order: `count` when every pixel is valid
+                for (int j = 0; j <= rem; ++j) {
+                    const int bj = seg_ptr[s] + kSliceMax * slice_win[g0 + i + j];
+                    const int lj = min(kSliceMax, seg_ptr[s + 1] - bj);
+                    for (int e = 0; e < lj; ++e) sum += (double)tcoef[bj + e];
+                }
+                m.x |= (int)0x80000000 | (seg_slot[s] + (r & kMetaSlotMask));
+                m.y = __float_as_int((float)sum);
+            }
+            reinterpret_cast<int2 *>(blk + (size_t)nsteps * kBlkStepBytes)[lane] = m;
+        }
+    }
+}
+
+}  // namespace
+
+// Largest blob over all tiles for the segment lengths `seg_len` (padded): decides whether a tile height fits the
+// shared-memory ring of the pipelined kernel.
+int ai_slice_max_blob(ai_ctx *ctx, int ntiles, const int *tile_seg_ptr, const int *seg_len, cudaStream_t st,
+                      int *max_blob)
+{
+    int *d = nullptr;
+    AI_CUDA(ctx, cudaMalloc(&d, (size_t)3 * ntiles * sizeof(int)));
+    slice_plan_kernel<<<(ntiles + 63) / 64, 64, 0, st>>>(ntiles, tile_seg_ptr, SegLens{seg_len, nullptr}, d, d + ntiles,
+                                                         d + 2 * ntiles);
+    std::vector<int> h(ntiles);
+    cudaError_t e = cudaMemcpyAsync(h.data(), d + 2 * ntiles, (size_t)ntiles * sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d);
+    AI_CUDA(ctx, e);
+    *max_blob = 0;
+    for (int t = 0; t < ntiles; ++t) *max_blob = std::max(*max_blob, h[t]);
+    return AI_OK;
+}
+
+// Scratch of the sliced build, alive between its two phases.
+struct SliceScratch {
+    int *tile_counts = nullptr;       // [3][ntiles] slices, blocks, blob bytes
+    int *tile_slice_ptr = nullptr;    // [ntiles+1]
+    long long *tile_blob_off = nullptr;
+    int *slice_seg = nullptr, *slice_win = nullptr, *slice_run = nullptr;
+    std::vector<int> h_nblk, h_bytes;
+    std::vector<long long> h_off;
+    void release()
+    {
+        cudaFree(tile_counts); cudaFree(tile_slice_ptr); cudaFree(tile_blob_off);
+        cudaFree(slice_seg); cudaFree(slice_win); cudaFree(slice_run);
+        tile_counts = tile_slice_ptr = slice_seg = slice_win = slice_run = nullptr;
+        tile_blob_off = nullptr;
+    }
+};
+
+// Phase 1 (needs seg_ptr): slices, runs, blob headers; fills seg_nruns[nseg] so that the caller can assign partial slots.
+int ai_build_sliced_plan(ai_ctx *ctx, SliceScratch *sc, int *seg_nruns, cudaStream_t st)
+{
+    TiledLayout &tl = ctx->tl;
+    const int nt = tl.ntiles;
+    AI_CUDA(ctx, cudaMalloc(&sc->tile_counts, (size_t)3 * nt * sizeof(int)));
+    const SegLens L{nullptr, tl.seg_ptr};
+    slice_plan_kernel<<<(nt + 63) / 64, 64, 0, st>>>(nt, tl.tile_seg_ptr, L, sc->tile_counts, sc->tile_counts + nt,
+                                                     sc->tile_counts + 2 * nt);
+    AI_CUDA(ctx, cudaGetLastError());
+    std::vector<int> h(3 * (size_t)nt);
+    AI_CUDA(ctx, cudaMemcpyAsync(h.data(), sc->tile_counts, h.size() * sizeof(int), cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    std::vector<int> slice_ptr(nt + 1, 0);
+    sc->h_off.assign(nt, 0);
+    sc->h_nblk.assign(h.begin() + nt, h.begin() + 2 * nt);
+    sc->h_bytes.assign(h.begin() + 2 * nt, h.end());
+    long long off = 0, nslices = 0;
+    tl.max_blob_bytes = 0;
+    for (int t = 0; t < nt; ++t) {
+        slice_ptr[t] = (int)nslices;
+        nslices += h[t];
+        sc->h_off[t] = off;
+        off += sc->h_bytes[t];
+        tl.max_blob_bytes = std::max(tl.max_blob_bytes, sc->h_bytes[t]);
+    }
+    slice_ptr[nt] = (int)nslices;
+    if (nslices > 0x7fffffffLL || off / 16 > 0x7fffffffLL) return ai_fail(ctx, AI_EUNSUPPORTED, "sliced layout too large");
+    tl.blob_bytes = off;
+    const size_t ns = nslices > 0 ? (size_t)nslices : 1;
+    AI_CUDA(ctx, cudaMalloc(&sc->tile_slice_ptr, ((size_t)nt + 1) * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&sc->tile_blob_off, (size_t)nt * sizeof(long long)));
+    AI_CUDA(ctx, cudaMalloc(&sc->slice_seg, ns * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&sc->slice_win, ns * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&sc->slice_run, ns * sizeof(int)));
+    AI_CUDA(ctx, cudaMalloc(&tl.blob, (size_t)(off > 0 ? off : 16)));
+    AI_CUDA(ctx, cudaMemsetAsync(tl.blob, 0, (size_t)(off > 0 ? off : 16), st));
+    AI_CUDA(ctx, cudaMemcpyAsync(sc->tile_slice_ptr, slice_ptr.data(), ((size_t)nt + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
+    AI_CUDA(ctx, cudaMemcpyAsync(sc->tile_blob_off, sc->h_off.data(), (size_t)nt * sizeof(long long), cudaMemcpyHostToDevice, st));
+    slice_assign_kernel<<<(nt + 63) / 64, 64, 0, st>>>(nt, tl.tile_seg_ptr, L, sc->tile_slice_ptr, sc->tile_blob_off,
+                                                       sc->slice_seg, sc->slice_win, sc->slice_run, seg_nruns, tl.blob);
+    AI_CUDA(ctx, cudaGetLastError());
+    AI_CUDA(ctx, cudaStreamSynchronize(st));      // slice_ptr (host vector) was the source of an async copy
+    return AI_OK;
+}
+
+// Phase 2 (needs seg_slot): the blocks themselves and the longest-first schedule.
+int ai_build_sliced_fill(ai_ctx *ctx, SliceScratch *sc, cudaStream_t st)
+{
+    TiledLayout &tl = ctx->tl;
+    const int nt = tl.ntiles;
+    slice_fill_kernel<<<nt, 256, 0, st>>>(sc->tile_slice_ptr, sc->tile_blob_off, sc->slice_seg, sc->slice_win,
+                                          sc->slice_run, tl.seg_ptr, tl.seg_slot, tl.tcoef, tl.tidx, tl.blob);
+    AI_CUDA(ctx, cudaGetLastError());
+    // longest-processing-time-first order of the tiles (host sort of ntiles integers, one-time)
+    std::vector<int> order(nt);
+    for (int t = 0; t < nt; ++t) order[t] = t;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return sc->h_bytes[a] > sc->h_bytes[b]; });
+    std::vector<int4> desc(nt);
+    for (int r = 0; r < nt; ++r) {
+        const int t = order[r];
+        desc[r] = make_int4((int)(sc->h_off[t] / 16), sc->h_bytes[t], t, sc->h_nblk[t]);
+    }
+    AI_CUDA(ctx, cudaMalloc(&tl.blob_desc, (size_t)nt * sizeof(int4)));
+    AI_CUDA(ctx, cudaMemcpyAsync(tl.blob_desc, desc.data(), (size_t)nt * sizeof(int4), cudaMemcpyHostToDevice, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    sc->release();
+    return AI_OK;
+}
+
+SliceScratch *ai_slice_scratch_new() { return new SliceScratch(); }
+void ai_slice_scratch_delete(SliceScratch *sc)
+{
+    if (!sc) return;
+    sc->release();
+    delete sc;
+}

@@ -10,6 +10,13 @@
 #include "build_common.cuh"
 #include "ctx.h"
 
+struct SliceScratch;
+int ai_slice_max_blob(ai_ctx *ctx, int ntiles, const int *tile_seg_ptr, const int *seg_len, cudaStream_t st, int *max_blob);
+int ai_build_sliced_plan(ai_ctx *ctx, SliceScratch *sc, int *seg_nruns, cudaStream_t st);
+int ai_build_sliced_fill(ai_ctx *ctx, SliceScratch *sc, cudaStream_t st);
+SliceScratch *ai_slice_scratch_new();
+void ai_slice_scratch_delete(SliceScratch *sc);
+
 namespace {
 
 __device__ __forceinline__ bool tile_pixel(int t, int k, int tiles_x, int th, int height, int width, int64_t *p)
@@ -132,7 +139,7 @@ struct TileChunk {
     __device__ void emit(int64_t pos, int k, int64_t, float coef) const
     {
         tcoef[pos] = coef;
-        tidx[pos] = (uint16_t)(ai_tile_pos(k / kTileW, k % kTileW) * 4);      // byte offset in the tile buffer
+        tidx[pos] = (uint16_t)(ai_tile_pos(k / kTileW, k % kTileW, th) * 4);      // byte offset in the tile buffer
     }
 };
 
@@ -164,24 +171,28 @@ __global__ void __launch_bounds__(256) seg_sum_kernel(int nseg, const int *__res
     if ((threadIdx.x & 31) == 0) seg_csum[s] = a;
 }
 
-// number of tiles touching each bin (= number of partial slots of the bin)
+// number of partial slots of each bin: the runs (build_sliced.cu) of its segments over all tiles
 __global__ void __launch_bounds__(128) bin_tiles_count_kernel(int npt, int ntiles, const int *__restrict__ tile_bmin,
-                                                              const int *__restrict__ tile_nbins, int *__restrict__ nslot)
+                                                              const int *__restrict__ tile_nbins,
+                                                              const int *__restrict__ tile_seg_ptr,
+                                                              const int *__restrict__ seg_nruns, int *__restrict__ nslot)
 {
     int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= npt) return;
     int c = 0;
     for (int t = 0; t < ntiles; ++t) {
         int lo = tile_bmin[t];
-        c += (b >= lo && b < lo + tile_nbins[t]) ? 1 : 0;
+        if (b >= lo && b < lo + tile_nbins[t]) c += seg_nruns[tile_seg_ptr[t] + b - lo];
     }
     nslot[b] = c;
 }
 
-// slot of every segment in the bin-major partial buffer: bin b's slots are ordered by ascending tile
+// first slot of every segment in the bin-major partial buffer: bin b's slots are ordered by ascending tile, the runs
+// of one segment are adjacent
 __global__ void __launch_bounds__(128) bin_tiles_assign_kernel(int npt, int ntiles, const int *__restrict__ tile_bmin,
                                                                const int *__restrict__ tile_nbins,
                                                                const int *__restrict__ tile_seg_ptr,
+                                                               const int *__restrict__ seg_nruns,
                                                                const int *__restrict__ bin_slot_ptr,
                                                                int *__restrict__ seg_slot)
 {
@@ -190,7 +201,11 @@ __global__ void __launch_bounds__(128) bin_tiles_assign_kernel(int npt, int ntil
     int slot = bin_slot_ptr[b];
     for (int t = 0; t < ntiles; ++t) {
         int lo = tile_bmin[t];
-        if (b >= lo && b < lo + tile_nbins[t]) seg_slot[tile_seg_ptr[t] + b - lo] = slot++;
+        if (b >= lo && b < lo + tile_nbins[t]) {
+            const int s = tile_seg_ptr[t] + b - lo;
+            seg_slot[s] = slot;
+            slot += seg_nruns[s];
+        }
     }
 }
 
@@ -245,6 +260,7 @@ static void free_tiled(TiledLayout &tl)
 {
     cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_meta); cudaFree(tl.seg_csum);
     cudaFree(tl.tile_desc); cudaFree(tl.tile_order); cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
+    cudaFree(tl.blob); cudaFree(tl.blob_desc);
     tl = TiledLayout{};
 }
 
@@ -273,7 +289,6 @@ static int plan_tiles(ai_ctx *ctx, const PixelSpans &sp, int th, cudaStream_t st
     cudaFree(d_total);
     if (h_total > 0x7fffffffLL) return ai_fail(ctx, AI_EUNSUPPORTED, "too many (tile, bin) segments: %lld", h_total);
     tl.nseg = (int)h_total;
-    tl.nslot = tl.nseg;
     const size_t nseg_alloc = tl.nseg > 0 ? tl.nseg : 1;
     AI_CUDA(ctx, cudaMalloc(seg_len, nseg_alloc * sizeof(int)));
     AI_CUDA(ctx, cudaMemsetAsync(*seg_len, 0, nseg_alloc * sizeof(int), st));
@@ -292,7 +307,10 @@ static int plan_tiles(ai_ctx *ctx, const PixelSpans &sp, int th, cudaStream_t st
         tl.max_tile_entries = std::max(tl.max_tile_entries, h_entries[t]);
         tl.max_tile_segs = std::max(tl.max_tile_segs, h_nbins[t]);
     }
-    *fits = ai_pipe_plan(tl.max_tile_entries, tl.max_tile_segs, th, false).fits;
+    int max_blob = 0;
+    int rc = ai_slice_max_blob(ctx, tl.ntiles, tl.tile_seg_ptr, *seg_len, st, &max_blob);
+    if (rc != AI_OK) return rc;
+    *fits = ai_pipe_plan(max_blob, th, false).fits;
     return AI_OK;
 }
 
@@ -338,12 +356,28 @@ int ai_build_tiled(ai_ctx *ctx, const PixelSpans &sp, cudaStream_t st)
     if (tl.nseg > 0)
         seg_sum_kernel<<<(tl.nseg + 7) / 8, 256, 0, st>>>(tl.nseg, tl.seg_ptr, tl.tcoef, tl.seg_csum);
 
+    // slices and runs of the sliced layout: one partial slot per run, bin-major
+    int *seg_nruns = nullptr;
+    AI_CUDA(ctx, cudaMalloc(&seg_nruns, nseg_alloc * sizeof(int)));
+    AI_CUDA(ctx, cudaMemsetAsync(seg_nruns, 0, nseg_alloc * sizeof(int), st));
+    SliceScratch *sc = ai_slice_scratch_new();
+    int rc = ai_build_sliced_plan(ctx, sc, seg_nruns, st);
+    if (rc != AI_OK) { ai_slice_scratch_delete(sc); return rc; }
     AI_CUDA(ctx, cudaMalloc(&nslot, (size_t)npt * sizeof(int)));
     AI_CUDA(ctx, cudaMalloc(&tl.bin_slot_ptr, ((size_t)npt + 1) * sizeof(int)));
-    bin_tiles_count_kernel<<<(npt + 127) / 128, 128, 0, st>>>(npt, tl.ntiles, tile_bmin, tile_nbins, nslot);
+    bin_tiles_count_kernel<<<(npt + 127) / 128, 128, 0, st>>>(npt, tl.ntiles, tile_bmin, tile_nbins, tl.tile_seg_ptr,
+                                                              seg_nruns, nslot);
     scan_pad_kernel<<<1, 1024, 0, st>>>(npt, nslot, 1, tl.bin_slot_ptr, d_total);
     bin_tiles_assign_kernel<<<(npt + 127) / 128, 128, 0, st>>>(npt, tl.ntiles, tile_bmin, tile_nbins, tl.tile_seg_ptr,
-                                                               tl.bin_slot_ptr, tl.seg_slot);
+                                                               seg_nruns, tl.bin_slot_ptr, tl.seg_slot);
+    AI_CUDA(ctx, cudaMemcpyAsync(&h_total, d_total, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    if (h_total > kMetaSlotMask) { ai_slice_scratch_delete(sc); return ai_fail(ctx, AI_EUNSUPPORTED, "%lld partial slots", h_total); }
+    tl.nslot = (int)h_total;
+    rc = ai_build_sliced_fill(ctx, sc, st);
+    ai_slice_scratch_delete(sc);
+    cudaFree(seg_nruns);
+    if (rc != AI_OK) return rc;
     AI_CUDA(ctx, cudaMalloc(&tl.seg_meta, nseg_alloc * sizeof(int4)));
     AI_CUDA(ctx, cudaMalloc(&tl.tile_desc, (size_t)tl.ntiles * sizeof(int4)));
     AI_CUDA(ctx, cudaMalloc(&tl.tile_order, (size_t)tl.ntiles * sizeof(int)));

@@ -112,6 +112,11 @@ template <> struct Accum<AI_ACC_F32_KAHAN> {
         s = t;
     }
     __device__ __forceinline__ void absorb(const Accum &o) { merge(o.s, o.c); }
+    __device__ __forceinline__ void shfl_down(int d)
+    {
+        s = __shfl_down_sync(AI_FULL_MASK, s, d);
+        c = __shfl_down_sync(AI_FULL_MASK, c, d);
+    }
     __device__ __forceinline__ void warp_reduce()
     {
 #pragma unroll
@@ -130,6 +135,7 @@ template <> struct Accum<AI_ACC_F32_PLAIN> {
     __device__ __forceinline__ void add(float coef, float v) { s = __fmaf_rn(coef, v, s); }
     __device__ __forceinline__ void add1(float x) { s = __fadd_rn(s, x); }
     __device__ __forceinline__ void absorb(const Accum &o) { s = __fadd_rn(s, o.s); }
+    __device__ __forceinline__ void shfl_down(int d) { s = __shfl_down_sync(AI_FULL_MASK, s, d); }
     __device__ __forceinline__ void warp_reduce()
     {
 #pragma unroll
@@ -144,6 +150,7 @@ template <> struct Accum<AI_ACC_F64> {
     __device__ __forceinline__ void add(float coef, float v) { s = fma((double)coef, (double)v, s); }
     __device__ __forceinline__ void add1(float x) { s += (double)x; }
     __device__ __forceinline__ void absorb(const Accum &o) { s += o.s; }
+    __device__ __forceinline__ void shfl_down(int d) { s = __shfl_down_sync(AI_FULL_MASK, s, d); }
     __device__ __forceinline__ void warp_reduce()
     {
 #pragma unroll

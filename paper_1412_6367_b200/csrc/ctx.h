@@ -14,46 +14,57 @@ constexpr int kTileHMax = 64;
 constexpr int kTilePixMax = kTileHMax * kTileW;
 constexpr int kSegPad = 4;   // segments are padded to a multiple of 4 entries (one 128-bit coefficient load)
 
-// Position of pixel (ly, lx) of a tile inside its shared-memory buffer.  Rows are rotated by one 16-byte chunk per
-// row, so pixels above each other (a ring crossing the tile vertically) fall in different banks while every aligned
-// group of 4 pixels stays contiguous for 128-bit stores.  The matrix stores these positions, not ly * kTileW + lx.
-__host__ __device__ inline int ai_tile_pos(int ly, int lx)
+// Position (in floats) of pixel (ly, lx) of a tile inside its shared-memory buffer.  The buffer is the image of two TMA
+// boxes of 32 pixels x tile_h rows loaded with the 128-byte swizzle: left half first, each row 128 bytes, the 16-byte
+// chunk index of a row XORed with (row & 7).  Pixels above each other (a ring crossing the tile vertically) fall in
+// different banks over 8 rows; every aligned group of 4 pixels stays contiguous for 128-bit stores.  The matrix
+// stores these positions (as byte offsets), so the register-staged path writes the same arrangement.
+__host__ __device__ inline int ai_tile_pos(int ly, int lx, int th)
 {
-    return (ly * kTileW) | ((((lx >> 2) + ly) & (kTileW / 4 - 1)) << 2) | (lx & 3);
+    return (lx >> 5) * th * 32 + ly * 32 + (((((lx >> 2) & 7) ^ (ly & 7))) << 2) + (lx & 3);
 }
 
+// ---- sliced execution layout of a tile's part of the matrix --------------------------------
+// Every (tile, bin) segment is cut into slices of at most kSliceMax entries; one lane of a warp owns one slice and
+// walks it four entries (one 128-bit coefficient load) per step.  32 slices of similar length form a block:
+//   coef  [nsteps][32] float4     idx [nsteps][32] ushort4 (byte offsets into the tile buffer)     meta [32] int2
+// A tile's blocks plus a header (number of blocks, then per block  byte offset / 16 << 8 | rounds << 4 | nsteps)
+// are one contiguous 16-byte aligned blob, moved to shared memory by one bulk copy.
+constexpr int kSliceMax = 32;
+constexpr int kSliceSteps = kSliceMax / 4;
+constexpr int kBlkStepBytes = 32 * 16 + 32 * 8;     // one step of a block: 32 float4 + 32 ushort4
+constexpr int kBlkMetaBytes = 32 * 8;
+// meta.x: bit 31 = this lane heads a run (adjacent lanes of one segment), bits 24..28 = lanes of the run after this
+// one, bits 0..23 = partial slot of the run (head only); meta.y = float bits of the run's coefficient sum (head only)
+constexpr int kMetaSlotMask = 0xffffff;
+
 // Shared-memory plan of the pipelined stage-1 kernel (integrate_pipe.cu), needed by the builder to pick tile_h.
-// Every image stage belongs to one stager warp, so there are at most kPipeMaxImgStages of them; the matrix ring is
-// double-buffered for single frames and single-buffered for batches (one slice serves many frames there).
 constexpr int kPipeSmemBudget = 227 * 1024;
-constexpr int kPipeHeaderBytes = 512;
-constexpr int kPipeMaxImgStages = 7;
+constexpr int kPipeHeaderBytes = 1024;
+constexpr int kPipeMaxMatStages = 4;
+constexpr int kPipeMaxImgStages = 8;
 constexpr int kPipeMinImgStages = 3;
 struct PipePlan {
-    int coef_bytes, idx_bytes, meta_bytes, mat_stage_bytes, mat_stages, img_stage_bytes, img_stages;
+    int mat_stage_bytes, mat_stages, img_stage_bytes, img_stages;
     size_t smem;
     bool fits;
 };
-inline int ai_align128(int x) { return (x + 127) & ~127; }
-inline PipePlan ai_pipe_plan(int max_tile_entries, int max_tile_segs, int tile_h, bool batch)
+inline int ai_align_up(int x, int a) { return (x + a - 1) / a * a; }
+inline PipePlan ai_pipe_plan(int max_blob_bytes, int tile_h, bool batch)
 {
     PipePlan p{};
-    p.coef_bytes = ai_align128(max_tile_entries * 4);
-    p.idx_bytes = ai_align128(max_tile_entries * 2);
-    p.meta_bytes = ai_align128(max_tile_segs * 16);
-    p.mat_stage_bytes = p.coef_bytes + p.idx_bytes + p.meta_bytes;
+    p.mat_stage_bytes = ai_align_up(max_blob_bytes > 16 ? max_blob_bytes : 16, 1024);   // image stages stay 1 KB aligned
     p.img_stage_bytes = tile_h * kTileW * 4;
-    // Single frame: bulk copies need about 100 KB in flight per SM to stream at full rate (measured, DESIGN.md
-    // section 5.3), i.e. two slices loading while a third is consumed; fall back to two stages for large slices.
-    // Batch: one slice serves many frames, all the room goes to image stages.
-    const int img_cap = batch ? kPipeMaxImgStages : 4;
-    for (p.mat_stages = batch ? 1 : 3; p.mat_stages >= (batch ? 1 : 2); --p.mat_stages) {
+    // Single frame: about 100 KB must be in flight per SM to stream at full rate, i.e. two slices loading while a
+    // third is consumed; two stages for large slices.  Batch: one slice serves many frames, the room goes to images.
+    const int img_cap = batch ? kPipeMaxImgStages : 6;
+    for (p.mat_stages = batch ? 2 : 3; p.mat_stages >= 2; --p.mat_stages) {
         const int room = kPipeSmemBudget - kPipeHeaderBytes - p.mat_stages * p.mat_stage_bytes;
         p.img_stages = room > 0 ? room / p.img_stage_bytes : 0;
         if (p.img_stages > img_cap) p.img_stages = img_cap;
         if (p.img_stages >= kPipeMinImgStages) break;
     }
-    if (p.mat_stages < 1) p.mat_stages = 1;
+    if (p.mat_stages < 2) p.mat_stages = 2;
     p.fits = p.img_stages >= kPipeMinImgStages;
     p.smem = (size_t)kPipeHeaderBytes + (size_t)p.mat_stages * p.mat_stage_bytes + (size_t)p.img_stages * p.img_stage_bytes;
     return p;
@@ -73,11 +84,16 @@ struct TiledLayout {
     int4 *tile_desc = nullptr;     // [ntiles]   {first entry, number of entries, first segment, number of segments}
     int *tile_order = nullptr;     // [ntiles]   tiles by descending number of entries (longest first scheduling)
     int max_tile_entries = 0, max_tile_segs = 0;
+    // sliced layout (pipelined kernel)
+    unsigned char *blob = nullptr; // all tiles' blobs, tile t at 16 * blob_desc[rank].x
+    int4 *blob_desc = nullptr;     // [ntiles] longest first: {blob offset / 16, blob bytes, tile id, number of blocks}
+    int64_t blob_bytes = 0;
+    int max_blob_bytes = 0;
     double *seg_csum = nullptr;    // [nseg]     sum of the segment's coefficients (count when every pixel is valid)
     float *tcoef = nullptr;        // [tnnz]     coefficient
     uint16_t *tidx = nullptr;      // [tnnz]     ai_tile_pos of the pixel inside the tile
     int *bin_slot_ptr = nullptr;   // [npt+1]    partial slots of bin b are [bin_slot_ptr[b], bin_slot_ptr[b+1])
-    int nslot = 0;                 // == nseg
+    int nslot = 0;                 // number of partials per frame: one per run of the sliced layout
 };
 
 struct ai_ctx {
@@ -118,6 +134,7 @@ struct ai_ctx {
     float *out_dev = nullptr;       // [3*npt] device outputs of ai_integrate1d_host
 
     // measurement hook (ai_profile_enable): events around the dominant kernel of the last call
+    bool no_tma = false;            // AZINT_NO_TMA=1: stage raw frames through registers even where TMA applies (testing)
     bool profile = false, profile_valid = false;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
 };

@@ -66,7 +66,7 @@ __device__ __forceinline__ void process_segments(const TiledView &tv, const floa
         Accum<ACC> S = S2.total(), C = C2.total();
         group_reduce<ACC>(S);
         if constexpr (TRACK) group_reduce<ACC>(C);
-        if (gl == 0 && s < s_end) store_partial<ACC>(part_f, m.z, S, C, TRACK, (double)__int_as_float(m.w));
+        if (gl == 0 && s < s_end && m.y > m.x) store_partial<ACC>(part_f, m.z, S, C, TRACK, (double)__int_as_float(m.w));
         s = s_next;
         m = m_next;
     }
@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(kS1Threads, kS1MinBlocks) tiled_stage1_kernel(
                                                                                 int height, int width, int vec_ok,
                                                                                 void *partials)
 {
-    __shared__ __align__(16) float tile[kTilePixMax];
+    __shared__ __align__(16) float tile[kTilePixMax];     // ai_tile_pos needs no particular alignment beyond 16 bytes here
     using T = typename RawType<DT>::T;
     const int t = blockIdx.x, f = blockIdx.y;
     const int ty = t / tv.tiles_x, tx = t - ty * tv.tiles_x;
@@ -219,6 +219,9 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
     int rc = ctx->layout == AI_LAYOUT_TILED_DIRECT ? AI_OK : ai_launch_pipe_stage1(ctx, a, vec_ok, st, &handled);
     if (rc != AI_OK) return rc;
     if (!handled) {
+        // this kernel writes one partial per segment, into the first of the segment's slots (one per run of the
+        // sliced layout): the others must read as zero
+        AI_CUDA(ctx, cudaMemsetAsync(ctx->partials, 0, need, st));
         rc = launch_simple_any(ctx, a, vec_ok, st);
         if (rc != AI_OK) return rc;
     }

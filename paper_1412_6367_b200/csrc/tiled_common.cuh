@@ -128,7 +128,7 @@ __device__ __forceinline__ bool stage_tile(float *tile, const void *img, const C
                         bad = true;
                     }
                 }
-                if (q < nchunk) *reinterpret_cast<float4 *>(tile + ai_tile_pos(q >> 4, (q & 15) * 4)) = v[i];
+                if (q < nchunk) *reinterpret_cast<float4 *>(tile + ai_tile_pos(q >> 4, (q & 15) * 4, th)) = v[i];
             }
         }
     } else if (vec_ok) {
@@ -162,7 +162,7 @@ __device__ __forceinline__ bool stage_tile(float *tile, const void *img, const C
                     v.w = correct_value(raw[i].w, dk[i].w, fl[i].w, sa[i].w, po[i].w, mk[i].w != 0, has_den);
                     bad = bad || v.x != v.x || v.y != v.y || v.z != v.z || v.w != v.w;
                 }
-                if (q < nchunk) *reinterpret_cast<float4 *>(tile + ai_tile_pos(q >> 4, (q & 15) * 4)) = v;
+                if (q < nchunk) *reinterpret_cast<float4 *>(tile + ai_tile_pos(q >> 4, (q & 15) * 4, th)) = v;
             }
         }
     } else {
@@ -174,7 +174,7 @@ __device__ __forceinline__ bool stage_tile(float *tile, const void *img, const C
                 v = corrected_pixel<DT>(img, (int64_t)y * width + x, cor);
                 bad = bad || v != v;
             }
-            tile[ai_tile_pos(ly, lx)] = v;
+            tile[ai_tile_pos(ly, lx, th)] = v;
         }
     }
     if (!acquired) acquire();
