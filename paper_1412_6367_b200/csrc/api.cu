@@ -87,6 +87,22 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
     }
     const char *e = getenv("AZINT_NO_TMA");
     ctx->no_tma = e && e[0] == '1';
+    if ((e = getenv("AZINT_TUNE")) != nullptr) {        // experiments only: "th:32,ms:6,is:8,bms:2,bis:8,fl:2"
+        for (const char *q = e; q && *q;) {
+            char key[8] = {0};
+            int val = 0;
+            if (sscanf(q, "%7[a-z]:%d", key, &val) == 2) {
+                if (!strcmp(key, "th")) ctx->tune.tile_h_max = val;
+                else if (!strcmp(key, "ms")) ctx->tune.mat_stages = val;
+                else if (!strcmp(key, "is")) ctx->tune.img_stages = val;
+                else if (!strcmp(key, "bms")) ctx->tune.batch_mat_stages = val;
+                else if (!strcmp(key, "bis")) ctx->tune.batch_img_stages = val;
+                else if (!strcmp(key, "fl")) ctx->tune.inflight = val;
+            }
+            q = strchr(q, ',');
+            if (q) ++q;
+        }
+    }
     *out = ctx;
     return AI_OK;
 }

@@ -261,7 +261,7 @@ int ai_build_sliced_fill(ai_ctx *ctx, SliceScratch *sc, cudaStream_t st)
     std::vector<int4> desc(nt);
     for (int r = 0; r < nt; ++r) {
         const int t = order[r];
-        desc[r] = make_int4((int)(sc->h_off[t] / 16), sc->h_bytes[t], t, sc->h_nblk[t]);
+        desc[r] = make_int4((int)(sc->h_off[t] / 16), sc->h_bytes[t], ((t / tl.tiles_x) << 16) | (t % tl.tiles_x), sc->h_nblk[t]);
     }
     AI_CUDA(ctx, cudaMalloc(&tl.blob_desc, (size_t)nt * sizeof(int4)));
     AI_CUDA(ctx, cudaMemcpyAsync(tl.blob_desc, desc.data(), (size_t)nt * sizeof(int4), cudaMemcpyHostToDevice, st));

@@ -310,7 +310,7 @@ static int plan_tiles(ai_ctx *ctx, const PixelSpans &sp, int th, cudaStream_t st
     int max_blob = 0;
     int rc = ai_slice_max_blob(ctx, tl.ntiles, tl.tile_seg_ptr, *seg_len, st, &max_blob);
     if (rc != AI_OK) return rc;
-    *fits = ai_pipe_plan(max_blob, th, false).fits;
+    *fits = ai_pipe_plan(max_blob, th, false, ctx->tune).fits;
     return AI_OK;
 }
 
@@ -321,7 +321,9 @@ int ai_build_tiled(ai_ctx *ctx, const PixelSpans &sp, cudaStream_t st)
     int *tile_bmin = nullptr, *tile_nbins = nullptr, *seg_len = nullptr, *seg_cur = nullptr, *nslot = nullptr;
     long long *d_total = nullptr, h_total = 0;
     // largest tile height whose slices fit the pipelined kernel (8 is taken regardless: the direct kernel serves it)
-    for (int th = kTileHMax;; th /= 2) {
+    int th0 = kTileHMax;
+    while (th0 > 8 && th0 > ctx->tune.tile_h_max) th0 /= 2;
+    for (int th = th0;; th /= 2) {
         bool fits = false;
         int rc = plan_tiles(ctx, sp, th, st, &tile_bmin, &tile_nbins, &seg_len, &fits);
         if (rc != AI_OK) return rc;

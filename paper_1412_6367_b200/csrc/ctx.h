@@ -41,7 +41,7 @@ constexpr int kMetaSlotMask = 0xffffff;
 // Shared-memory plan of the pipelined stage-1 kernel (integrate_pipe.cu), needed by the builder to pick tile_h.
 constexpr int kPipeSmemBudget = 227 * 1024;
 constexpr int kPipeHeaderBytes = 1024;
-constexpr int kPipeMaxMatStages = 4;
+constexpr int kPipeMaxMatStages = 8;
 constexpr int kPipeMaxImgStages = 8;
 constexpr int kPipeMinImgStages = 3;
 struct PipePlan {
@@ -50,18 +50,27 @@ struct PipePlan {
     bool fits;
 };
 inline int ai_align_up(int x, int a) { return (x + a - 1) / a * a; }
-inline PipePlan ai_pipe_plan(int max_blob_bytes, int tile_h, bool batch)
+// Tunables (defaults chosen by measurement; AZINT_TUNE="th:32,ms:6,is:8,fl:2" overrides them
+// for experiments): largest tile height tried, caps on the matrix / image stages, tiles in flight per block.
+struct PipeTune {
+    int tile_h_max = 64;
+    int mat_stages = 3, img_stages = 6;        // single frame
+    int batch_mat_stages = 2, batch_img_stages = kPipeMaxImgStages;
+    int inflight = 0;                          // 0 = as many as there are stages
+};
+inline PipePlan ai_pipe_plan(int max_blob_bytes, int tile_h, bool batch, const PipeTune &tune = PipeTune())
 {
     PipePlan p{};
     p.mat_stage_bytes = ai_align_up(max_blob_bytes > 16 ? max_blob_bytes : 16, 1024);   // image stages stay 1 KB aligned
     p.img_stage_bytes = tile_h * kTileW * 4;
-    // Single frame: about 100 KB must be in flight per SM to stream at full rate, i.e. two slices loading while a
-    // third is consumed; two stages for large slices.  Batch: one slice serves many frames, the room goes to images.
-    const int img_cap = batch ? kPipeMaxImgStages : 6;
-    for (p.mat_stages = batch ? 2 : 3; p.mat_stages >= 2; --p.mat_stages) {
+    int ms_max = batch ? tune.batch_mat_stages : tune.mat_stages;
+    int is_max = batch ? tune.batch_img_stages : tune.img_stages;
+    ms_max = ms_max < 2 ? 2 : (ms_max > kPipeMaxMatStages ? kPipeMaxMatStages : ms_max);
+    is_max = is_max < kPipeMinImgStages ? kPipeMinImgStages : (is_max > kPipeMaxImgStages ? kPipeMaxImgStages : is_max);
+    for (p.mat_stages = ms_max; p.mat_stages >= 2; --p.mat_stages) {
         const int room = kPipeSmemBudget - kPipeHeaderBytes - p.mat_stages * p.mat_stage_bytes;
         p.img_stages = room > 0 ? room / p.img_stage_bytes : 0;
-        if (p.img_stages > img_cap) p.img_stages = img_cap;
+        if (p.img_stages > is_max) p.img_stages = is_max;
         if (p.img_stages >= kPipeMinImgStages) break;
     }
     if (p.mat_stages < 2) p.mat_stages = 2;
@@ -86,7 +95,7 @@ struct TiledLayout {
     int max_tile_entries = 0, max_tile_segs = 0;
     // sliced layout (pipelined kernel)
     unsigned char *blob = nullptr; // all tiles' blobs, tile t at 16 * blob_desc[rank].x
-    int4 *blob_desc = nullptr;     // [ntiles] longest first: {blob offset / 16, blob bytes, tile id, number of blocks}
+    int4 *blob_desc = nullptr;     // [ntiles] longest first: {blob offset / 16, blob bytes, tile row << 16 | tile column, number of blocks}
     int64_t blob_bytes = 0;
     int max_blob_bytes = 0;
     double *seg_csum = nullptr;    // [nseg]     sum of the segment's coefficients (count when every pixel is valid)
@@ -134,6 +143,7 @@ struct ai_ctx {
     float *out_dev = nullptr;       // [3*npt] device outputs of ai_integrate1d_host
 
     // measurement hook (ai_profile_enable): events around the dominant kernel of the last call
+    PipeTune tune;
     bool no_tma = false;            // AZINT_NO_TMA=1: stage raw frames through registers even where TMA applies (testing)
     bool profile = false, profile_valid = false;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;

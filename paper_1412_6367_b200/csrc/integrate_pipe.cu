@@ -29,11 +29,12 @@ namespace {
 constexpr int kStageWarps = 3;
 constexpr int kConsWarps = 16;
 constexpr int kPipeThreads = 32 * (1 + kStageWarps + kConsWarps);
+static_assert((kConsWarps & (kConsWarps - 1)) == 0, "block dealing assumes a power of two");
 static_assert((2 * kPipeMaxMatStages + 3 * kPipeMaxImgStages) * 8 + kPipeMaxImgStages * 4 <= kPipeHeaderBytes,
               "header too small");
 
 struct PipeParams {
-    const int4 *blob_desc;       // longest first: {blob offset / 16, blob bytes, tile id, number of blocks}
+    const int4 *blob_desc;       // longest first: {blob offset / 16, blob bytes, tile row << 16 | column, blocks}
     const unsigned char *blob;
     int tiles_x, tile_h, ntiles, nslot;
     int mat_stages, img_stages, mat_stage_bytes, img_stage_bytes;
@@ -41,7 +42,7 @@ struct PipeParams {
     int64_t frame_stride;
     int nframes, frames_per_item, nitems;
     Corrections cor;
-    int height, width, vec_ok, use_tma;
+    int height, width, vec_ok, use_tma, inflight;
     void *partials;
 };
 
@@ -55,6 +56,10 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_n(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
 {
@@ -89,11 +94,26 @@ __device__ __forceinline__ void tma_box(void *dst_smem, const CUtensorMap *map, 
 // orders this thread's shared-memory accesses through the generic proxy before later accesses of the async proxy (TMA)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// n-th use of a ring of `stages` buffers -> (stage, parity of the phase that use completes)
-struct Slot {
-    int stage;
-    uint32_t parity;
-    __device__ Slot(int n, int stages) : stage(n % stages), parity((uint32_t)(n / stages) & 1u) {}
+// ---- development aid: per-block event trace (compiled in only with -DAI_PIPE_TRACE) -------
+#ifdef AI_PIPE_TRACE
+__device__ long long *g_trace = nullptr;          // [grid][kTraceItems][16] clock64 stamps
+constexpr int kTraceItems = 16;
+#define AI_TRACE(item, slot)                                                                             \
+    do {                                                                                                 \
+        if (g_trace && (item) < kTraceItems) g_trace[((size_t)blockIdx.x * kTraceItems + (item)) * 16 + (slot)] = clock64(); \
+    } while (0)
+#else
+#define AI_TRACE(item, slot) do { } while (0)
+#endif
+
+// position in a ring of buffers: stage and parity of the phase the current use completes
+struct Ring {
+    int stage = 0;
+    uint32_t parity = 0;
+    __device__ __forceinline__ void next(int stages)
+    {
+        if (++stage == stages) { stage = 0; parity ^= 1u; }
+    }
 };
 
 // n-th item of this block: tiles (longest first) are dealt to the blocks in snake order
@@ -102,27 +122,81 @@ __device__ __forceinline__ int item_at(int n)
     return n * gridDim.x + ((n & 1) ? gridDim.x - 1 - blockIdx.x : blockIdx.x);
 }
 
+// (tile rank, chunk of frames) of successive items of this block, without integer division
+struct ItemWalk {
+    int rank = 0, chunk = 0, prev = 0;
+    __device__ __forceinline__ void to(int w, int ntiles)
+    {
+        rank += w - prev;
+        prev = w;
+        while (rank >= ntiles) { rank -= ntiles; ++chunk; }
+    }
+};
+
+// Descriptors of this block's items, fetched 32 at a time (lane l holds item n0 + l) one window ahead of their use, so
+// that no role ever waits on a dependent global load between two items.  All lanes of the warp call get() together.
+struct DescWindow {
+    int4 cur, nxt;
+    __device__ __forceinline__ static int4 load(const PipeParams &p, int k)
+    {
+        const int w = item_at(k);
+        return w < p.nitems ? __ldg(p.blob_desc + (p.nitems == p.ntiles ? w : w % p.ntiles)) : make_int4(0, 0, 0, 0);
+    }
+    __device__ __forceinline__ void init(const PipeParams &p, int lane)
+    {
+        cur = load(p, lane);
+        nxt = load(p, 32 + lane);
+    }
+    __device__ __forceinline__ int4 get(const PipeParams &p, int n, int lane)
+    {
+        if ((n & 31) == 0 && n > 0) {
+            cur = nxt;
+            nxt = load(p, n + 32 + lane);
+        }
+        int4 d;
+        d.x = __shfl_sync(AI_FULL_MASK, cur.x, n & 31);
+        d.y = __shfl_sync(AI_FULL_MASK, cur.y, n & 31);
+        d.z = __shfl_sync(AI_FULL_MASK, cur.z, n & 31);
+        d.w = __shfl_sync(AI_FULL_MASK, cur.w, n & 31);
+        return d;
+    }
+};
+
 // One block of 32 slices against one staged tile: lane = slice.  All loads of the block are conflict-free 128 / 64-bit
 // shared loads at consecutive addresses; the gathers hit the tile buffer at the stored byte offsets.
+// `lazy` (used with TRACK false): the tile was not screened for non-finite pixels; a non-finite lane sum anywhere in
+// the warp means one may have been gathered, nothing is stored and true is returned -- the caller repeats the block
+// with TRACK, which skips such pixels and accumulates count.  The step loop is kept rolled (two steps per trip, loads
+// one trip ahead): the hot code of all consumer warps must stay inside the instruction cache.
 template <int ACC, bool TRACK>
-__device__ __forceinline__ void consume_block(const float *tile, const unsigned char *blob, unsigned h, void *part_f,
-                                              int lane)
+__device__ __noinline__ bool consume_block(const float *tile, const unsigned char *blob, unsigned h, void *part_f,
+                                           int lane, bool lazy)
 {
     const int nsteps = h & 15, rounds = (h >> 4) & 7;
     const unsigned char *blk = blob + (size_t)(h >> 8) * 16;
     const float4 *cp = reinterpret_cast<const float4 *>(blk) + lane;
     const ushort4 *xp = reinterpret_cast<const ushort4 *>(blk + nsteps * 512) + lane;
     const int2 m = reinterpret_cast<const int2 *>(blk + nsteps * kBlkStepBytes)[lane];
-    Accum2<ACC> S2, C2;
-    if (nsteps == kSliceSteps) {
-#pragma unroll
-        for (int j = 0; j < kSliceSteps; ++j) consume4<ACC, TRACK>(tile, cp[j * 32], xp[j * 32], S2, C2);
-    } else {
-#pragma unroll
-        for (int j = 0; j < kSliceSteps - 1; ++j)
-            if (j < nsteps) consume4<ACC, TRACK>(tile, cp[j * 32], xp[j * 32], S2, C2);
+    const float4 zero4 = make_float4(0, 0, 0, 0);
+    const ushort4 zeroi = make_ushort4(0, 0, 0, 0);
+    AccumQ<ACC> S2, C2;
+    float4 c0 = cp[0], c1 = nsteps > 1 ? cp[32] : zero4;
+    ushort4 x0 = xp[0], x1 = nsteps > 1 ? xp[32] : zeroi;
+#pragma unroll 1
+    for (int j = 2; j < nsteps + 2; j += 2) {
+        float4 n0 = zero4, n1 = zero4;
+        ushort4 y0 = zeroi, y1 = zeroi;
+        if (j < nsteps) { n0 = cp[j * 32]; y0 = xp[j * 32]; }
+        if (j + 1 < nsteps) { n1 = cp[j * 32 + 32]; y1 = xp[j * 32 + 32]; }
+        const float4 v0 = gather4(tile, x0), v1 = gather4(tile, x1);
+        accumulate4<ACC, TRACK>(c0, v0, S2, C2);
+        accumulate4<ACC, TRACK>(c1, v1, S2, C2);
+        c0 = n0; c1 = n1; x0 = y0; x1 = y1;
     }
     Accum<ACC> S = S2.total(), C = C2.total();
+    if constexpr (!TRACK) {
+        if (lazy && __any_sync(AI_FULL_MASK, !finite_f((float)S.s))) return true;
+    }
     // lanes of a run are adjacent: suffix sums by doubling, the head of the run ends with the run's total
     const int rem = (m.x >> 24) & 31;
     for (int r = 0; r < rounds; ++r) {
@@ -136,6 +210,7 @@ __device__ __forceinline__ void consume_block(const float *tile, const unsigned 
         }
     }
     if (m.x < 0) store_partial<ACC>(part_f, m.x & kMetaSlotMask, S, C, TRACK, (double)__int_as_float(m.y));
+    return false;
 }
 
 // TMA mode: the raw 32-bit tile becomes float32 in place; non-finite float pixels become NaN.  Returns true if this
@@ -144,19 +219,36 @@ template <int DT>
 __device__ __forceinline__ bool convert_tile_in_place(float *tile, int nchunk, int tid, int nthreads)
 {
     bool bad = false;
+    if constexpr (DT == AI_F32) {
+        // all loads first (independent), then one test per 128 bits: exponent field all ones <=> Inf or NaN
+        constexpr int U = 6;
+        for (int q0 = tid; q0 < nchunk; q0 += nthreads * U) {
+            uint4 v[U];
+#pragma unroll
+            for (int i = 0; i < U; ++i) {
+                const int q = q0 + i * nthreads;
+                v[i] = q < nchunk ? reinterpret_cast<const uint4 *>(tile)[q] : make_uint4(0, 0, 0, 0);
+            }
+#pragma unroll
+            for (int i = 0; i < U; ++i) {
+                const unsigned e = 0x7f800000u;
+                if ((v[i].x & e) == e || (v[i].y & e) == e || (v[i].z & e) == e || (v[i].w & e) == e) {
+                    float4 *p = reinterpret_cast<float4 *>(tile) + (q0 + i * nthreads);
+                    float4 f = *p;
+                    f.x = finite_f(f.x) ? f.x : quiet_nan();
+                    f.y = finite_f(f.y) ? f.y : quiet_nan();
+                    f.z = finite_f(f.z) ? f.z : quiet_nan();
+                    f.w = finite_f(f.w) ? f.w : quiet_nan();
+                    *p = f;
+                    bad = true;
+                }
+            }
+        }
+        return bad;
+    }
     for (int q = tid; q < nchunk; q += nthreads) {
         float4 *p = reinterpret_cast<float4 *>(tile) + q;
-        if constexpr (DT == AI_F32) {
-            float4 v = *p;
-            if (!finite_f(v.x) || !finite_f(v.y) || !finite_f(v.z) || !finite_f(v.w)) {
-                v.x = finite_f(v.x) ? v.x : quiet_nan();
-                v.y = finite_f(v.y) ? v.y : quiet_nan();
-                v.z = finite_f(v.z) ? v.z : quiet_nan();
-                v.w = finite_f(v.w) ? v.w : quiet_nan();
-                *p = v;
-                bad = true;
-            }
-        } else if constexpr (DT == AI_I32) {
+        if constexpr (DT == AI_I32) {
             const int4 v = *reinterpret_cast<const int4 *>(p);
             *p = make_float4((float)v.x, (float)v.y, (float)v.z, (float)v.w);
         } else if constexpr (DT == AI_U32) {
@@ -181,6 +273,12 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
     unsigned char *mat_base = smem + kPipeHeaderBytes;
     unsigned char *img_base = mat_base + (size_t)p.mat_stages * p.mat_stage_bytes;
     using T = typename RawType<DT>::T;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // float32 frames that arrive by TMA need no staging pass: consumers gather from the raw tile and detect
+    // non-finite pixels lazily (consume_block)
+    const bool direct = DT == AI_F32 && p.use_tma;
+    DescWindow win;
+    win.init(p, lane);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < kPipeMaxMatStages; ++s) {
@@ -196,99 +294,133 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    if (threadIdx.x == 0) AI_TRACE(0, 15);
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    ItemWalk walk;
+    Ring mr, ir;                                     // matrix ring position of item n, image ring position of image ii
     if (warp == 0) {
-        // ===== producer ================================================================================================
-        if (lane != 0) return;
-        int ii = 0;
+        // ===== producer: the warp stays converged (waits are warp-uniform), lane 0 issues the copies ===================
         for (int n = 0;; ++n) {
             const int w = item_at(n);
             if (w >= p.nitems) break;
-            const int4 d = __ldg(p.blob_desc + (w % p.ntiles));
-            const int f0 = (w / p.ntiles) * p.frames_per_item;
+            const int4 d = win.get(p, n, lane);
+            if (d.w == 0) continue;                       // tile without entries: skipped by every role
+            walk.to(w, p.ntiles);
+            const int f0 = walk.chunk * p.frames_per_item;
             const int f1 = min(p.nframes, f0 + p.frames_per_item);
-            const int ty = d.z / p.tiles_x, tx = d.z - ty * p.tiles_x;
-            for (int f = f0; f < f1; ++f, ++ii) {
+            const int ty = d.z >> 16, tx = d.z & 0xffff;
+            if (p.inflight && n >= p.inflight) {         // pace: at most `inflight` blobs outstanding
+                const int k = n - p.inflight;
+                mbar_wait(mat_full + k % p.mat_stages, (uint32_t)(k / p.mat_stages) & 1u);
+            }
+            for (int f = f0; f < f1; ++f) {
                 if (p.use_tma) {
-                    const Slot is(ii, p.img_stages);
-                    mbar_wait(img_empty + is.stage, is.parity ^ 1u);
-                    unsigned char *dst = img_base + (size_t)is.stage * p.img_stage_bytes;
-                    mbar_arrive_expect_tx(raw_full + is.stage, (uint32_t)p.img_stage_bytes);
-                    tma_box(dst, &tmap, tx * kTileW, ty * p.tile_h, f, raw_full + is.stage);
-                    tma_box(dst + p.img_stage_bytes / 2, &tmap, tx * kTileW + 32, ty * p.tile_h, f, raw_full + is.stage);
+                    if (lane == 0) AI_TRACE(n, 0);
+                    mbar_wait(img_empty + ir.stage, ir.parity ^ 1u);
+                    if (lane == 0) {
+                        AI_TRACE(n, 1);
+                        unsigned char *dst = img_base + (size_t)ir.stage * p.img_stage_bytes;
+                        mbar_arrive_expect_tx(raw_full + ir.stage, (uint32_t)p.img_stage_bytes);
+                        tma_box(dst, &tmap, tx * kTileW, ty * p.tile_h, f, raw_full + ir.stage);
+                        tma_box(dst + p.img_stage_bytes / 2, &tmap, tx * kTileW + 32, ty * p.tile_h, f, raw_full + ir.stage);
+                        AI_TRACE(n, 2);
+                    }
+                    ir.next(p.img_stages);
                 }
                 if (f == f0) {
-                    const Slot ms(n, p.mat_stages);
-                    mbar_wait(mat_empty + ms.stage, ms.parity ^ 1u);
-                    mbar_arrive_expect_tx(mat_full + ms.stage, (uint32_t)d.y);
-                    bulk_g2s(mat_base + (size_t)ms.stage * p.mat_stage_bytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y,
-                             mat_full + ms.stage);
+                    mbar_wait(mat_empty + mr.stage, mr.parity ^ 1u);
+                    if (lane == 0) {
+                        AI_TRACE(n, 3);
+                        mbar_arrive_expect_tx(mat_full + mr.stage, (uint32_t)d.y);
+                        bulk_g2s(mat_base + (size_t)mr.stage * p.mat_stage_bytes, p.blob + (size_t)d.x * 16,
+                                 (uint32_t)d.y, mat_full + mr.stage);
+                        AI_TRACE(n, 4);
+                    }
+                    mr.next(p.mat_stages);
                 }
             }
         }
     } else if (warp <= kStageWarps) {
         // ===== stagers: raw tile -> float32, corrected, invalid pixels as NaN ==========================================
+        if (direct) return;
         const int sw = warp - 1, tid = sw * 32 + lane;
         int ii = 0;
         for (int n = 0;; ++n) {
             const int w = item_at(n);
             if (w >= p.nitems) break;
-            const int f0 = (w / p.ntiles) * p.frames_per_item;
+            const int4 d = win.get(p, n, lane);
+            if (d.w == 0) continue;
+            walk.to(w, p.ntiles);
+            const int f0 = walk.chunk * p.frames_per_item;
             const int f1 = min(p.nframes, f0 + p.frames_per_item);
-            const int t = __ldg(p.blob_desc + (w % p.ntiles)).z;
-            const int ty = t / p.tiles_x, tx = t - ty * p.tiles_x;
+            const int ty = d.z >> 16, tx = d.z & 0xffff;
             for (int f = f0; f < f1; ++f, ++ii) {
-                const Slot is(ii, p.img_stages);
-                float *tile = reinterpret_cast<float *>(img_base + (size_t)is.stage * p.img_stage_bytes);
+                float *tile = reinterpret_cast<float *>(img_base + (size_t)ir.stage * p.img_stage_bytes);
                 bool bad;
                 if (p.use_tma) {
-                    mbar_wait(raw_full + is.stage, is.parity);
+                    if (tid == 0) AI_TRACE(ii, 5);
+                    mbar_wait(raw_full + ir.stage, ir.parity);
+                    if (tid == 0) AI_TRACE(ii, 6);
                     bad = convert_tile_in_place<DT>(tile, p.tile_h * (kTileW / 4), tid, kStageWarps * 32);
-                    if (DT != AI_F32 || bad) fence_proxy_async();      // generic-proxy writes before the next TMA write
+                    fence_proxy_async();               // generic-proxy writes before the next TMA write to the stage
                 } else {
                     const void *img = reinterpret_cast<const T *>(p.frames) + (int64_t)f * p.frame_stride;
                     bad = stage_tile<DT, kStageWarps * 32, 8, 3>(tile, img, p.cor, ty, tx, p.tile_h, p.height, p.width,
                                                                   p.vec_ok, tid,
-                                                                  [&] { mbar_wait(img_empty + is.stage, is.parity ^ 1u); });
+                                                                  [&] { mbar_wait(img_empty + ir.stage, ir.parity ^ 1u); });
                 }
-                if (bad) img_flag[is.stage] = ii + 1;           // value-equal writers; read after the barrier
+                if (bad) img_flag[ir.stage] = ii + 1;           // value-equal writers; read after the barrier
                 __syncwarp();
-                if (lane == 0) mbar_arrive(img_ready + is.stage);
+                if (tid == 0) AI_TRACE(ii, 7);
+                if (lane == 0) mbar_arrive(img_ready + ir.stage);
+                ir.next(p.img_stages);
             }
         }
     } else {
         // ===== consumers: gather-reduce, one lane per slice ============================================================
+        // A tile's blocks are dealt round-robin to the warps, continuing across tiles.
         const int cw = warp - 1 - kStageWarps;
-        int ii = 0, dealt = 0;                       // blocks are dealt round-robin to the warps across tiles
+        uint64_t *img_bar = direct ? raw_full : img_ready;
+        int ii = 0, first = cw;
         for (int n = 0;; ++n) {
             const int w = item_at(n);
             if (w >= p.nitems) break;
-            const int4 d = __ldg(p.blob_desc + (w % p.ntiles));
-            const int f0 = (w / p.ntiles) * p.frames_per_item;
+            const int4 d = win.get(p, n, lane);
+            if (d.w == 0) continue;
+            walk.to(w, p.ntiles);
+            const int f0 = walk.chunk * p.frames_per_item;
             const int f1 = min(p.nframes, f0 + p.frames_per_item);
-            const Slot ms(n, p.mat_stages);
-            mbar_wait(mat_full + ms.stage, ms.parity);
-            const unsigned char *blob = mat_base + (size_t)ms.stage * p.mat_stage_bytes;
+            // Every warp waits on and arrives at every barrier, also for items of which it holds no block: no warp
+            // is ever a whole phase away from a barrier (parity waits would alias).
+            const bool mine = first < d.w;
+            if (cw == 0 && lane == 0) AI_TRACE(n, 8);
+            mbar_wait(mat_full + mr.stage, mr.parity);
+            if (cw == 0 && lane == 0) AI_TRACE(n, 9);
+            const unsigned char *blob = mat_base + (size_t)mr.stage * p.mat_stage_bytes;
             const unsigned *hdr = reinterpret_cast<const unsigned *>(blob) + 1;
-            const int first = (cw - dealt % kConsWarps + kConsWarps) % kConsWarps;
             for (int f = f0; f < f1; ++f, ++ii) {
-                const Slot is(ii, p.img_stages);
-                mbar_wait(img_ready + is.stage, is.parity);
-                const float *tile = reinterpret_cast<const float *>(img_base + (size_t)is.stage * p.img_stage_bytes);
-                const bool track = img_flag[is.stage] == ii + 1;
-                void *part_f = reinterpret_cast<char *>(p.partials) + (int64_t)f * p.nslot * 16;
-                if (track) {
-                    for (int b = first; b < d.w; b += kConsWarps) consume_block<ACC, true>(tile, blob, hdr[b], part_f, lane);
-                } else {
-                    for (int b = first; b < d.w; b += kConsWarps) consume_block<ACC, false>(tile, blob, hdr[b], part_f, lane);
+                mbar_wait(img_bar + ir.stage, ir.parity);
+                if (lane == 0 && (cw == 0 || cw == 8)) AI_TRACE(ii, cw ? 12 : 10);
+                if (mine) {
+                    const float *tile = reinterpret_cast<const float *>(img_base + (size_t)ir.stage * p.img_stage_bytes);
+                    void *part_f = reinterpret_cast<char *>(p.partials) + (int64_t)f * p.nslot * 16;
+                    const bool track = !direct && img_flag[ir.stage] == ii + 1;
+                    for (int b = first; b < d.w; b += kConsWarps) {
+                        const unsigned h = hdr[b];
+                        if (track || consume_block<ACC, false>(tile, blob, h, part_f, lane, direct))
+                            consume_block<ACC, true>(tile, blob, h, part_f, lane, false);
+                    }
+                    __syncwarp();
+                    if (lane == 0 && (cw == 0 || cw == 8 || cw == 15)) AI_TRACE(ii, cw == 0 ? 11 : cw == 8 ? 13 : 14);
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(img_empty + is.stage);
+                if (lane == 0) mbar_arrive(img_empty + ir.stage);
+                ir.next(p.img_stages);
             }
-            dealt += d.w;
-            __syncwarp();
-            if (lane == 0) mbar_arrive(mat_empty + ms.stage);
+            if (lane == 0) mbar_arrive(mat_empty + mr.stage);
+            // the warp after the one that took this tile's last block takes the next tile's first
+            first -= d.w & (kConsWarps - 1);
+            if (first < 0) first += kConsWarps;
+            mr.next(p.mat_stages);
         }
     }
 }
@@ -358,6 +490,13 @@ int launch_pipe_dt(ai_ctx *ctx, const CUtensorMap &map, const PipeParams &p, siz
 
 }  // namespace
 
+#ifdef AI_PIPE_TRACE
+extern "C" int ai_debug_set_trace(void *dev_buffer)
+{
+    return (int)cudaMemcpyToSymbol(g_trace, &dev_buffer, sizeof(void *));
+}
+#endif
+
 // Launches the pipelined stage 1 if a tile's blob fits the shared-memory ring (*handled = true); otherwise leaves
 // *handled false and the caller falls back to the one-block-per-tile kernel.
 int ai_launch_pipe_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled)
@@ -365,7 +504,7 @@ int ai_launch_pipe_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStrea
     const TiledLayout &tl = ctx->tl;
     *handled = false;
     if (tl.ntiles < 1 || !tl.blob) return AI_OK;
-    const PipePlan plan = ai_pipe_plan(tl.max_blob_bytes, tl.tile_h, a.nframes >= 16);
+    const PipePlan plan = ai_pipe_plan(tl.max_blob_bytes, tl.tile_h, a.nframes >= 16, ctx->tune);
     if (!plan.fits) return AI_OK;                    // blob too large for the ring: direct kernel
     PipeParams p{};
     p.mat_stages = plan.mat_stages;
@@ -400,6 +539,7 @@ int ai_launch_pipe_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStrea
     p.width = ctx->width;
     p.vec_ok = vec_ok;
     p.partials = ctx->partials;
+    p.inflight = ctx->tune.inflight > 0 && ctx->tune.inflight < plan.mat_stages ? ctx->tune.inflight : 0;
     // TMA for the image: 32-bit pixels, nothing to correct, rows and frames on 16-byte boundaries
     const bool plain = !a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask;
     const bool is32 = a.dtype == AI_F32 || a.dtype == AI_I32 || a.dtype == AI_U32;

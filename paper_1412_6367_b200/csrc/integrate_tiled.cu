@@ -42,7 +42,7 @@ __device__ __forceinline__ void process_segments(const TiledView &tv, const floa
     while (__any_sync(AI_FULL_MASK, s < s_end)) {
         const int s_next = s + kGroups;
         const int4 m_next = s_next < s_end ? __ldg(tv.seg_meta + s_next) : make_int4(0, 0, 0, 0);
-        Accum2<ACC> S2, C2;
+        AccumQ<ACC> S2, C2;
         const int end = m.y;
         int k = m.x + gl * 4;
         // software pipeline: loads for step i+1 are issued before step i is consumed

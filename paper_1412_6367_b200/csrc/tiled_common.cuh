@@ -7,13 +7,16 @@
 constexpr int kLanes = 8;            // lanes cooperating on one (tile, bin) segment
 constexpr int kStep = kLanes * 4;    // entries consumed per group per 128-bit coefficient load
 
-// two interleaved accumulators per lane (even / odd entries): halves the dependent chain of the Kahan recurrence
-template <int ACC> struct Accum2 {
-    Accum<ACC> a, b;
+// four interleaved accumulators per lane, one per entry of a 128-bit coefficient load: the four compensated
+// recurrences of a step are independent, so their latencies overlap
+template <int ACC> struct AccumQ {
+    Accum<ACC> a, b, c, d;
     __device__ __forceinline__ Accum<ACC> total() const
     {
-        Accum<ACC> r = a;
+        Accum<ACC> r = a, q = c;
         r.absorb(b);
+        q.absorb(d);
+        r.absorb(q);
         return r;
     }
 };
@@ -61,31 +64,31 @@ __device__ __forceinline__ float4 gather4(const float *tile, const ushort4 &x)
     return make_float4(tile_at(tile, x.x), tile_at(tile, x.y), tile_at(tile, x.z), tile_at(tile, x.w));
 }
 
-// four matrix entries against four gathered pixel values; TRACK: the tile holds invalid (NaN) pixels, so count is
-// accumulated too
+// four matrix entries against four gathered pixel values; TRACK: the tile holds invalid (non-finite) pixels, so they
+// are skipped and count is accumulated too
 template <int ACC, bool TRACK>
-__device__ __forceinline__ void accumulate4(const float4 &c4, const float4 &v, Accum2<ACC> &S, Accum2<ACC> &C)
+__device__ __forceinline__ void accumulate4(const float4 &c4, const float4 &v, AccumQ<ACC> &S, AccumQ<ACC> &C)
 {
     if constexpr (TRACK) {
-        const bool k0 = v.x == v.x, k1 = v.y == v.y, k2 = v.z == v.z, k3 = v.w == v.w;
+        const bool k0 = finite_f(v.x), k1 = finite_f(v.y), k2 = finite_f(v.z), k3 = finite_f(v.w);
         S.a.add(c4.x, k0 ? v.x : 0.0f);
         S.b.add(c4.y, k1 ? v.y : 0.0f);
-        S.a.add(c4.z, k2 ? v.z : 0.0f);
-        S.b.add(c4.w, k3 ? v.w : 0.0f);
+        S.c.add(c4.z, k2 ? v.z : 0.0f);
+        S.d.add(c4.w, k3 ? v.w : 0.0f);
         C.a.add1(k0 ? c4.x : 0.0f);
         C.b.add1(k1 ? c4.y : 0.0f);
-        C.a.add1(k2 ? c4.z : 0.0f);
-        C.b.add1(k3 ? c4.w : 0.0f);
+        C.c.add1(k2 ? c4.z : 0.0f);
+        C.d.add1(k3 ? c4.w : 0.0f);
     } else {
         S.a.add(c4.x, v.x);
         S.b.add(c4.y, v.y);
-        S.a.add(c4.z, v.z);
-        S.b.add(c4.w, v.w);
+        S.c.add(c4.z, v.z);
+        S.d.add(c4.w, v.w);
     }
 }
 template <int ACC, bool TRACK>
-__device__ __forceinline__ void consume4(const float *tile, const float4 &c4, const ushort4 &i4, Accum2<ACC> &S,
-                                         Accum2<ACC> &C)
+__device__ __forceinline__ void consume4(const float *tile, const float4 &c4, const ushort4 &i4, AccumQ<ACC> &S,
+                                         AccumQ<ACC> &C)
 {
     accumulate4<ACC, TRACK>(c4, gather4(tile, i4), S, C);
 }
