@@ -135,9 +135,12 @@ int ai_integrate1d_host(ai_ctx *ctx, const void *image_host, ai_dtype dtype, con
 /* Number of kernels the last ai_integrate1d* call launched (for accounting in benchmarks). */
 int ai_last_launch_count(const ai_ctx *ctx);
 
-/* Measurement hook: when enabled, every ai_integrate1d* call records CUDA events on its stream around its dominant
- * kernel (TILED: stage 1, the SpMV; CSR / LUT: the single kernel).  ai_profile_last synchronises on the last of those
+/* Measurement hook.  on = 1: every ai_integrate1d* call records CUDA events on its stream around its dominant
+ * kernel (TILED: stage 1, the SpMV; CSR / LUT: the single kernel); ai_profile_last synchronises on the last of those
  * events and returns the device time of that kernel launch in milliseconds through *kernel_ms.
+ * on = 2 (TILED layouts): ai_integrate1d* launches ONLY the dominant kernel -- no events, no second stage, the outputs
+ * are not written -- so that a benchmark can time a train of back-to-back launches of that kernel with its own events.
+ * on = 0: normal operation.
  * Errors: AI_EINVAL (NULL, or nothing recorded yet), AI_ECUDA. */
 int ai_profile_enable(ai_ctx *ctx, int on);
 int ai_profile_last(ai_ctx *ctx, float *kernel_ms);

@@ -164,7 +164,8 @@ def ai_last_launch_count(ctx) -> int:
 
 
 def ai_profile_enable(ctx, on=True):
-    _check(lib().ai_profile_enable(ctx, 1 if on else 0), ctx)
+    """on: False / 0 off, True / 1 events around the dominant kernel, 2 launch only the dominant kernel."""
+    _check(lib().ai_profile_enable(ctx, int(on)), ctx)
 
 
 def ai_profile_last(ctx) -> float:

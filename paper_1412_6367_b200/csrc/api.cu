@@ -41,11 +41,12 @@ int ai_last_launch_count(const ai_ctx *ctx) { return ctx ? ctx->last_launches : 
 int ai_profile_enable(ai_ctx *ctx, int on)
 {
     if (!ctx) return AI_EINVAL;
-    if (on && !ctx->ev0) {
+    if (on == 1 && !ctx->ev0) {
         AI_CUDA(ctx, cudaEventCreate(&ctx->ev0));
         AI_CUDA(ctx, cudaEventCreate(&ctx->ev1));
     }
-    ctx->profile = on != 0;
+    ctx->profile = on == 1;
+    ctx->stage1_only = on == 2;
     ctx->profile_valid = false;
     return AI_OK;
 }
@@ -87,6 +88,8 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
     }
     const char *e = getenv("AZINT_NO_TMA");
     ctx->no_tma = e && e[0] == '1';
+    e = getenv("AZINT_NO_STREAM");
+    ctx->no_stream = e && e[0] == '1';
     if ((e = getenv("AZINT_TUNE")) != nullptr) {        // experiments only: "th:32,ms:6,is:8,bms:2,bis:8,fl:2"
         for (const char *q = e; q && *q;) {
             char key[8] = {0};
@@ -98,6 +101,7 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
                 else if (!strcmp(key, "bms")) ctx->tune.batch_mat_stages = val;
                 else if (!strcmp(key, "bis")) ctx->tune.batch_img_stages = val;
                 else if (!strcmp(key, "fl")) ctx->tune.inflight = val;
+                else if (!strcmp(key, "ss")) ctx->tune.stream_stages = val;
             }
             q = strchr(q, ',');
             if (q) ++q;
@@ -120,6 +124,9 @@ int ai_build_csr(ai_ctx *ctx, void *cuda_stream)
     ai_free_spans(&spans);
     if (rc != AI_OK) return rc;
     AI_CUDA(ctx, cudaMalloc(&ctx->out_dev, 3 * (size_t)ctx->npt * sizeof(float)));
+    AI_CUDA(ctx, cudaMalloc(&ctx->grid_sync, sizeof(unsigned long long)));
+    AI_CUDA(ctx, cudaMemsetAsync(ctx->grid_sync, 0, sizeof(unsigned long long), st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
     ctx->built = true;
     return AI_OK;
 }
@@ -241,7 +248,8 @@ void ai_destroy(ai_ctx *ctx)
     cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_meta); cudaFree(tl.seg_csum);
     cudaFree(tl.tile_desc); cudaFree(tl.tile_order); cudaFree(tl.blob); cudaFree(tl.blob_desc);
     cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
-    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev);
+    free(tl.h_first_desc);
+    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;

@@ -6,6 +6,8 @@
 // Order of the slices of a tile: all full slices (kSliceMax entries) in (bin, position) order, then the last, shorter
 // slice of every segment by descending length, bins ascending among equals.  Adjacent lanes of a block that belong to
 // the same segment form a run; a run yields one partial sum per frame.
+#include <stdlib.h>
+
 #include <algorithm>
 #include <vector>
 
@@ -29,6 +31,13 @@ __device__ __forceinline__ int slice_steps_at(int i, int nfull, const int *cnt)
         i -= cnt[r];
     }
     return 0;
+}
+
+// steps of the block whose first slice sits at sorted position i: the longest of its slices, rounded up to an even
+// number (the stream kernel consumes two steps per trip without tail predicates; the extra step is zero padding)
+__device__ __forceinline__ int block_steps_at(int i, int nfull, const int *cnt)
+{
+    return (slice_steps_at(i, nfull, cnt) + 1) & ~1;
 }
 
 __device__ __forceinline__ void tile_slice_counts(const SegLens &L, int s0, int s1, int *nfull, int *cnt)
@@ -56,7 +65,7 @@ __global__ void __launch_bounds__(64) slice_plan_kernel(int ntiles, const int *_
     for (int r = 1; r < kSliceSteps; ++r) S += cnt[r];
     const int nblk = (S + 31) / 32;
     int bytes = (4 * (1 + nblk) + 15) / 16 * 16;
-    for (int b = 0; b < nblk; ++b) bytes += slice_steps_at(32 * b, nfull, cnt) * kBlkStepBytes + kBlkMetaBytes;
+    for (int b = 0; b < nblk; ++b) bytes += block_steps_at(32 * b, nfull, cnt) * kBlkStepBytes + kBlkMetaBytes;
     tile_nslices[t] = S;
     tile_nblk[t] = nblk;
     tile_blob_bytes[t] = bytes;
@@ -109,7 +118,7 @@ __global__ void __launch_bounds__(64) slice_assign_kernel(int ntiles, const int 
         }
         int rounds = 0;
         while ((1 << rounds) < maxrun) ++rounds;
-        const int nsteps = slice_steps_at(lo, nfull, cnt);
+        const int nsteps = block_steps_at(lo, nfull, cnt);
         hdr[1 + b] = ((unsigned)(off / 16) << 8) | ((unsigned)rounds << 4) | (unsigned)nsteps;
         off += nsteps * kBlkStepBytes + kBlkMetaBytes;
     }
@@ -263,6 +272,9 @@ int ai_build_sliced_fill(ai_ctx *ctx, SliceScratch *sc, cudaStream_t st)
         const int t = order[r];
         desc[r] = make_int4((int)(sc->h_off[t] / 16), sc->h_bytes[t], ((t / tl.tiles_x) << 16) | (t % tl.tiles_x), sc->h_nblk[t]);
     }
+    tl.h_first_desc = static_cast<int4 *>(malloc((size_t)(nt > 0 ? nt : 1) * sizeof(int4)));
+    if (!tl.h_first_desc) return ai_fail(ctx, AI_ENOMEM, "host copy of the tile descriptors");
+    for (int r = 0; r < nt; ++r) tl.h_first_desc[r] = desc[r];
     AI_CUDA(ctx, cudaMalloc(&tl.blob_desc, (size_t)nt * sizeof(int4)));
     AI_CUDA(ctx, cudaMemcpyAsync(tl.blob_desc, desc.data(), (size_t)nt * sizeof(int4), cudaMemcpyHostToDevice, st));
     AI_CUDA(ctx, cudaStreamSynchronize(st));

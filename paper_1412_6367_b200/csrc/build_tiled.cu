@@ -261,6 +261,7 @@ static void free_tiled(TiledLayout &tl)
     cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_meta); cudaFree(tl.seg_csum);
     cudaFree(tl.tile_desc); cudaFree(tl.tile_order); cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
     cudaFree(tl.blob); cudaFree(tl.blob_desc);
+    free(tl.h_first_desc);
     tl = TiledLayout{};
 }
 

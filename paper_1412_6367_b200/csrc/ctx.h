@@ -57,6 +57,7 @@ struct PipeTune {
     int mat_stages = 3, img_stages = 6;        // single frame
     int batch_mat_stages = 2, batch_img_stages = kPipeMaxImgStages;
     int inflight = 0;                          // 0 = as many as there are stages
+    int stream_stages = 0;                     // cap on the (tile + blob) stages of the single-frame kernel, 0 = none
 };
 inline PipePlan ai_pipe_plan(int max_blob_bytes, int tile_h, bool batch, const PipeTune &tune = PipeTune())
 {
@@ -96,6 +97,7 @@ struct TiledLayout {
     // sliced layout (pipelined kernel)
     unsigned char *blob = nullptr; // all tiles' blobs, tile t at 16 * blob_desc[rank].x
     int4 *blob_desc = nullptr;     // [ntiles] longest first: {blob offset / 16, blob bytes, tile row << 16 | tile column, number of blocks}
+    int4 *h_first_desc = nullptr;  // HOST copy of blob_desc (the single-frame kernel takes each block's first tiles by value)
     int64_t blob_bytes = 0;
     int max_blob_bytes = 0;
     double *seg_csum = nullptr;    // [nseg]     sum of the segment's coefficients (count when every pixel is valid)
@@ -141,11 +143,14 @@ struct ai_ctx {
     void *staging = nullptr;        // device copy of a host frame (ai_integrate1d_host)
     size_t staging_bytes = 0;
     float *out_dev = nullptr;       // [3*npt] device outputs of ai_integrate1d_host
+    unsigned long long *grid_sync = nullptr;   // arrival counter of the fused single-frame kernel's grid barrier
 
     // measurement hook (ai_profile_enable): events around the dominant kernel of the last call
     PipeTune tune;
     bool no_tma = false;            // AZINT_NO_TMA=1: stage raw frames through registers even where TMA applies (testing)
+    bool no_stream = false;         // AZINT_NO_STREAM=1: single frames take the general pipelined kernel too (testing)
     bool profile = false, profile_valid = false;
+    bool stage1_only = false;       // ai_profile_enable(ctx, 2): launch only the dominant kernel
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
 };
 

@@ -22,6 +22,7 @@
 // the batched variant that amortises the matrix read across frames.
 #include <cuda.h>
 
+#include "pipe_common.cuh"
 #include "tiled_common.cuh"
 
 namespace {
@@ -46,75 +47,23 @@ struct PipeParams {
     void *partials;
 };
 
-// ---- mbarrier / bulk-copy primitives (PTX, sm_90+) ---------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_n(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t ok;
-    asm volatile("{\n\t.reg .pred p;\n\t"
-                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-                 "selp.u32 %0, 1, 0, p;\n\t}"
-                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    return ok != 0;
-}
-// bounded wait: a protocol bug traps (the launch fails with an error) instead of hanging the device
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    for (uint32_t spin = 0; !mbar_try_wait(bar, parity); ++spin)
-        if (spin > (1u << 22)) __trap();
-}
-__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-// one box of the (x, y, frame) tensor of frames: 32 pixels x tile_h rows, 128-byte swizzle
-__device__ __forceinline__ void tma_box(void *dst_smem, const CUtensorMap *map, int x, int y, int f, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                 ::"r"(smem_u32(dst_smem)), "l"(map), "r"(x), "r"(y), "r"(f), "r"(smem_u32(bar)) : "memory");
-}
-// orders this thread's shared-memory accesses through the generic proxy before later accesses of the async proxy (TMA)
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
 // ---- development aid: per-block event trace (compiled in only with -DAI_PIPE_TRACE) -------
 #ifdef AI_PIPE_TRACE
-__device__ long long *g_trace = nullptr;          // [grid][kTraceItems][16] clock64 stamps
+__device__ long long *g_trace = nullptr;          // [grid][kTraceItems][16] globaltimer stamps (ns)
 constexpr int kTraceItems = 16;
+__device__ __forceinline__ long long trace_now()
+{
+    long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 #define AI_TRACE(item, slot)                                                                             \
     do {                                                                                                 \
-        if (g_trace && (item) < kTraceItems) g_trace[((size_t)blockIdx.x * kTraceItems + (item)) * 16 + (slot)] = clock64(); \
+        if (g_trace && (item) < kTraceItems) g_trace[((size_t)blockIdx.x * kTraceItems + (item)) * 16 + (slot)] = trace_now(); \
     } while (0)
 #else
 #define AI_TRACE(item, slot) do { } while (0)
 #endif
-
-// position in a ring of buffers: stage and parity of the phase the current use completes
-struct Ring {
-    int stage = 0;
-    uint32_t parity = 0;
-    __device__ __forceinline__ void next(int stages)
-    {
-        if (++stage == stages) { stage = 0; parity ^= 1u; }
-    }
-};
 
 // n-th item of this block: tiles (longest first) are dealt to the blocks in snake order
 __device__ __forceinline__ int item_at(int n)
@@ -294,6 +243,9 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    // stage 2 is launched with programmatic stream serialisation: let its blocks be scheduled as SMs free up (they
+    // wait in griddepcontrol.wait until this whole grid has completed)
+    asm volatile("griddepcontrol.launch_dependents;");
     if (threadIdx.x == 0) AI_TRACE(0, 15);
 
     ItemWalk walk;
@@ -342,6 +294,23 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
         }
     } else if (warp <= kStageWarps) {
         // ===== stagers: raw tile -> float32, corrected, invalid pixels as NaN ==========================================
+#ifdef AI_PIPE_TRACE
+        if (direct && warp == 1 && p.frames_per_item == 1) {   // monitor: when did each blob / image tile land?
+            for (int n = 0;; ++n) {
+                const int w = item_at(n);
+                if (w >= p.nitems) break;
+                const int4 d = win.get(p, n, lane);
+                if (d.w == 0) continue;
+                mbar_wait(raw_full + ir.stage, ir.parity);
+                if (lane == 0) AI_TRACE(n, 6);
+                mbar_wait(mat_full + mr.stage, mr.parity);
+                if (lane == 0) AI_TRACE(n, 5);
+                ir.next(p.img_stages);
+                mr.next(p.mat_stages);
+            }
+            return;
+        }
+#endif
         if (direct) return;
         const int sw = warp - 1, tid = sw * 32 + lane;
         int ii = 0;
@@ -444,8 +413,10 @@ EncodeTiledFn encode_tiled_fn()
     return fn;
 }
 
+}  // namespace
+
 // (x, y, frame) view of the frames, boxes of 32 pixels x tile_h rows x 1 frame, 128-byte swizzle, zeros outside
-int make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *map)
+int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *map)
 {
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return ai_fail(ctx, AI_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
@@ -461,6 +432,8 @@ int make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *map
     if (r != CUDA_SUCCESS) return ai_fail(ctx, AI_ECUDA, "cuTensorMapEncodeTiled failed with %d", (int)r);
     return AI_OK;
 }
+
+namespace {
 
 template <int DT, int ACC>
 int launch_pipe(ai_ctx *ctx, const CUtensorMap &map, const PipeParams &p, size_t smem, int grid, cudaStream_t st)
@@ -546,7 +519,7 @@ int ai_launch_pipe_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStrea
     p.use_tma = plain && is32 && vec_ok && (reinterpret_cast<uintptr_t>(a.image) % 16) == 0 && !ctx->no_tma;
     CUtensorMap map{};
     if (p.use_tma) {
-        int rc = make_frame_map(ctx, a, tl.tile_h, &map);
+        int rc = ai_make_frame_map(ctx, a, tl.tile_h, &map);
         if (rc != AI_OK) return rc;
     }
     const int grid = p.nitems < sms ? p.nitems : sms;

@@ -1,0 +1,459 @@
+// TILED stage 1, single-frame fast path: the CSR SpMV of PAPER.md:174-188 for one frame of
+// 32-bit pixels without correction arrays -- the configuration the headline metric is quoted on.
+//
+// Same sliced matrix layout and the same arithmetic as integrate_pipe.cu, with everything that kernel carries for
+// batches, corrections and 16-bit pixels stripped from the critical path:
+//   - one persistent block per SM, 1 producer warp + kStreamCons consumer warps, no stager warps: float frames are
+//     gathered straight from the TMA tile, integer frames are converted at gather time ("casted from
+//     integer to float");
+//   - one ring whose stage holds a tile of the frame AND that tile's blob of the matrix, one full / empty mbarrier pair
+//     per stage: a consumer warp waits once and arrives once per tile;
+//   - the block's tile descriptors sit in shared memory (one LDS per tile and warp); the first kStreamFirst of every
+//     block travel in the kernel parameters, so the first copies are issued before any global load has returned;
+//   - pixel positions of two entries are rebased with one packed 16-bit add: the tile buffers live in the first 64 KB of
+//     the shared window, so a position's low half-word is its whole shared address.
+#include "pipe_common.cuh"
+#include "tiled_common.cuh"
+
+namespace {
+
+constexpr int kStreamCons = 20;                      // consumer warps (21 warps x 72 registers leave room for
+                                                     // a block of stage 2 next to this one: see the launch chain)
+constexpr int kStreamThreads = 32 * (1 + kStreamCons);
+constexpr int kStreamFirst = 3;                      // descriptors per block passed by value
+constexpr int kStreamMaxGrid = 160;
+constexpr int kStreamMaxStages = 4;
+constexpr int kStreamBarBytes = 128;                 // full[4] + empty[4], padded
+
+struct StreamFirstDescs {
+    int4 d[kStreamFirst][kStreamMaxGrid];
+};
+
+struct StreamParams {
+    const int4 *blob_desc;       // longest first: {blob offset / 16, blob bytes, tile row << 16 | column, blocks}
+    const unsigned char *blob;
+    int tile_h, ntiles, nslot;
+    int stages, mat_stage_bytes, img_stage_bytes, hdr_bytes, items_max;
+    void *partials;
+    // H5 fused behind a grid-wide barrier (every block is resident: one per SM, grid <= number of SMs)
+    unsigned long long *grid_sync;     // arrivals of all launches of this context, never reset
+    const int *bin_slot_ptr;
+    const double *range;
+    int npt;
+    float empty;
+    float *radial, *intensity, *sum_signal, *count;
+};
+
+// ---- development aid (-DAI_PIPE_TRACE): per (block, tile, warp) globaltimer stamps ------------------------------------
+#ifdef AI_PIPE_TRACE
+__device__ long long *g_strace = nullptr;          // [grid][16 tiles][32 warps][4]
+__device__ __forceinline__ long long strace_now()
+{
+    long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define AI_STRACE(item, slot, val)                                                                              \
+    do {                                                                                                        \
+        if (g_strace && (threadIdx.x & 31) == 0 && (item) < 16)                                                 \
+            g_strace[((((size_t)blockIdx.x * 16 + (item)) * 32) + (threadIdx.x >> 5)) * 4 + (slot)] = (val);    \
+    } while (0)
+#else
+#define AI_STRACE(item, slot, val) do { } while (0)
+#define strace_now() 0
+#endif
+
+// n-th tile of this block: tiles (longest first) are dealt to the blocks in snake order
+__device__ __forceinline__ int stream_item_at(int n)
+{
+    return n * gridDim.x + ((n & 1) ? gridDim.x - 1 - blockIdx.x : blockIdx.x);
+}
+
+__device__ __forceinline__ float lds_f32(unsigned addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ int lds_s32(unsigned addr)
+{
+    int v;
+    asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+
+// pixel values of the four entries of one step; x holds four 16-bit byte offsets into the tile, rebase = low half-word
+// of the tile's shared address in both halves
+template <int DT>
+__device__ __forceinline__ float4 stream_gather4(const uint2 &x, unsigned rebase)
+{
+    const unsigned p0 = x.x + rebase, p1 = x.y + rebase;
+    if constexpr (DT == AI_F32) {
+        return make_float4(lds_f32(p0 & 0xffffu), lds_f32(p0 >> 16), lds_f32(p1 & 0xffffu), lds_f32(p1 >> 16));
+    } else if constexpr (DT == AI_I32) {
+        return make_float4((float)lds_s32(p0 & 0xffffu), (float)lds_s32(p0 >> 16), (float)lds_s32(p1 & 0xffffu),
+                           (float)lds_s32(p1 >> 16));
+    } else {
+        return make_float4((float)(unsigned)lds_s32(p0 & 0xffffu), (float)(unsigned)lds_s32(p0 >> 16),
+                           (float)(unsigned)lds_s32(p1 & 0xffffu), (float)(unsigned)lds_s32(p1 >> 16));
+    }
+}
+
+// lanes of a run are adjacent: suffix sums by doubling, the head of the run ends with the run's total
+template <int ACC, bool TRACK>
+__device__ __forceinline__ void stream_finish_block(Accum<ACC> &S, Accum<ACC> &C, const int2 &m, int rounds, void *part_f)
+{
+    const int rem = (m.x >> 24) & 31;
+    for (int r = 0; r < rounds; ++r) {
+        const int d = 1 << r;
+        Accum<ACC> S_o = S, C_o = C;
+        S_o.shfl_down(d);
+        if constexpr (TRACK) C_o.shfl_down(d);
+        if (rem >= d) {
+            S.absorb(S_o);
+            if constexpr (TRACK) C.absorb(C_o);
+        }
+    }
+    if (m.x < 0) store_partial<ACC>(part_f, m.x & kMetaSlotMask, S, C, TRACK, (double)__int_as_float(m.y));
+}
+
+// One block of 32 slices against the staged tile: lane = slice, two steps (8 entries) per trip, the loads of the next
+// trip issued before the current one is consumed.  Blocks hold an even number of steps (build_sliced.cu) and the
+// stage has slack behind the blob, so the look-ahead needs no predicate.  Float frames are not screened: a
+// non-finite lane sum anywhere in the warp means a non-finite pixel may have been gathered; nothing is stored and
+// true is returned (the caller repeats the block with stream_block_tracked).
+template <int DT, int ACC>
+__device__ __noinline__ bool stream_block(unsigned rebase, const unsigned char *blob, unsigned h, void *part_f, int lane)
+{
+    const int nsteps = h & 15, rounds = (h >> 4) & 7;
+    const unsigned char *blk = blob + (size_t)(h >> 8) * 16;
+    const float4 *cp = reinterpret_cast<const float4 *>(blk) + lane;
+    const uint2 *xp = reinterpret_cast<const uint2 *>(blk + nsteps * 512) + lane;
+    const int2 m = reinterpret_cast<const int2 *>(blk + nsteps * kBlkStepBytes)[lane];
+    AccumQ<ACC> S2, C2;
+    float4 c0 = cp[0], c1 = cp[32];
+    uint2 x0 = xp[0], x1 = xp[32];
+#pragma unroll 1
+    for (int j = 2; j <= nsteps; j += 2) {
+        const float4 n0 = cp[j * 32], n1 = cp[j * 32 + 32];
+        const uint2 y0 = xp[j * 32], y1 = xp[j * 32 + 32];
+        const float4 v0 = stream_gather4<DT>(x0, rebase), v1 = stream_gather4<DT>(x1, rebase);
+        accumulate4<ACC, false>(c0, v0, S2, C2);
+        accumulate4<ACC, false>(c1, v1, S2, C2);
+        c0 = n0; c1 = n1; x0 = y0; x1 = y1;
+    }
+    Accum<ACC> S = S2.total(), C = C2.total();
+    if constexpr (DT == AI_F32) {
+        if (__any_sync(AI_FULL_MASK, !finite_f((float)S.s))) return true;
+    }
+    stream_finish_block<ACC, false>(S, C, m, rounds, part_f);
+    return false;
+}
+
+// the same block with non-finite pixels skipped and count accumulated (float frames only; rare, kept simple)
+template <int ACC>
+__device__ __noinline__ void stream_block_tracked(unsigned rebase, const unsigned char *blob, unsigned h, void *part_f,
+                                                  int lane)
+{
+    const int nsteps = h & 15, rounds = (h >> 4) & 7;
+    const unsigned char *blk = blob + (size_t)(h >> 8) * 16;
+    const float4 *cp = reinterpret_cast<const float4 *>(blk) + lane;
+    const uint2 *xp = reinterpret_cast<const uint2 *>(blk + nsteps * 512) + lane;
+    const int2 m = reinterpret_cast<const int2 *>(blk + nsteps * kBlkStepBytes)[lane];
+    AccumQ<ACC> S2, C2;
+#pragma unroll 1
+    for (int j = 0; j < nsteps; ++j) {
+        const float4 c = cp[j * 32];
+        const float4 v = stream_gather4<AI_F32>(xp[j * 32], rebase);
+        accumulate4<ACC, true>(c, v, S2, C2);
+    }
+    Accum<ACC> S = S2.total(), C = C2.total();
+    stream_finish_block<ACC, true>(S, C, m, rounds, part_f);
+}
+
+template <int DT, int ACC>
+__global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const __grid_constant__ CUtensorMap tmap,
+                                                                         const __grid_constant__ StreamFirstDescs first,
+                                                                         const StreamParams p)
+{
+    // [tile stages][barriers, tile descriptors][matrix stages]
+    extern __shared__ __align__(1024) unsigned char smem[];
+    unsigned char *img_base = smem;
+    unsigned char *hdr = smem + (size_t)p.stages * p.img_stage_bytes;
+    uint64_t *full = reinterpret_cast<uint64_t *>(hdr);              // tile + blob landed (complete_tx)
+    uint64_t *empty = full + kStreamMaxStages;                        // every consumer warp is done with the stage
+    int4 *desc_s = reinterpret_cast<int4 *>(hdr + kStreamBarBytes);
+    unsigned char *mat_base = hdr + p.hdr_bytes;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    AI_STRACE(15, 0, strace_now());
+
+    // number of tiles of this block
+    int nmine = 0;
+    while (stream_item_at(nmine) < p.ntiles) ++nmine;
+
+    // Launch chain (programmatic dependent launch): this grid may start while the previous kernel of the stream is
+    // still running (stage 2 of the previous frame triggers its dependents at once).  Nothing that kernel may still
+    // read or write is touched before griddepcontrol.wait: until then only the matrix (static since ai_build_csr) is
+    // fetched -- the blobs of the block's first tiles -- together with descriptors, barriers and the tensor map; the
+    // frame is read and the partials are written after it.
+    auto issue_blob = [&](int stage, const int4 &d) {
+        mbar_arrive_expect_tx(full + stage, (uint32_t)(p.img_stage_bytes + d.y));
+        bulk_g2s(mat_base + (size_t)stage * p.mat_stage_bytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y, full + stage);
+    };
+    auto issue_tile = [&](int stage, const int4 &d) {
+        unsigned char *tile = img_base + (size_t)stage * p.img_stage_bytes;
+        const int ty = d.z >> 16, tx = d.z & 0xffff;
+        tma_box(tile, &tmap, tx * kTileW, ty * p.tile_h, 0, full + stage);
+        tma_box(tile + p.img_stage_bytes / 2, &tmap, tx * kTileW + 32, ty * p.tile_h, 0, full + stage);
+    };
+    const int npre = min(min(kStreamFirst, p.stages), nmine);         // tiles whose copies are issued by thread 0 here
+
+    if (threadIdx.x == 0) {
+        // the packed rebase needs every tile buffer inside the first 64 KB of the shared window
+        if (smem_u32(img_base) + (unsigned)(p.stages * p.img_stage_bytes) > 0x10000u) __trap();
+        for (int s = 0; s < kStreamMaxStages; ++s) {
+            mbar_init(full + s, 1);
+            mbar_init(empty + s, kStreamCons);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        // first blobs, from descriptors that came with the launch: in flight before any global load returns
+        int stage = 0;
+        for (int n = 0; n < npre; ++n) {
+            const int4 d = first.d[n][blockIdx.x];
+            if (d.w == 0) continue;
+            issue_blob(stage++, d);
+        }
+    }
+    for (int k = threadIdx.x; k < nmine; k += kStreamThreads)
+        desc_s[k] = k < kStreamFirst ? first.d[k][blockIdx.x] : __ldg(p.blob_desc + stream_item_at(k));
+    // H5 reads the slot ranges of the bins at the very end: pull them into L2 now (static data, 4 bytes per bin)
+    for (int k = threadIdx.x * 32; k <= p.npt; k += kStreamThreads * 32)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(p.bin_slot_ptr + k));
+    // stage 2 is launched with programmatic stream serialisation too: its blocks may be scheduled as SMs free up
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (threadIdx.x == 0) {
+        int stage = 0;
+        for (int n = 0; n < npre; ++n) {
+            const int4 d = first.d[n][blockIdx.x];
+            if (d.w == 0) continue;
+            issue_tile(stage++, d);
+        }
+    }
+    __syncthreads();
+    AI_STRACE(15, 1, strace_now());
+
+    Ring r;
+    if (warp == 0) {
+        // ===== producer ================================================================================================
+        int issued = 0;
+        for (int n = 0; n < nmine; ++n) {
+            const int4 d = desc_s[n];
+            if (d.w == 0) continue;                       // tile without entries: skipped by every role
+            if (n >= npre) {
+                AI_STRACE(n, 0, strace_now());
+                if (issued >= p.stages) mbar_wait(empty + r.stage, r.parity ^ 1u);
+                if (lane == 0) {
+                    issue_blob(r.stage, d);
+                    issue_tile(r.stage, d);
+                }
+                AI_STRACE(n, 1, strace_now());
+            }
+            ++issued;
+            r.next(p.stages);
+        }
+    } else {
+        // ===== consumers: a tile's blocks are dealt round-robin to the warps, continuing across tiles ===================
+        const int cw = warp - 1;
+        int firstb = cw;
+        for (int n = 0; n < nmine; ++n) {
+            const int4 d = desc_s[n];
+            if (d.w == 0) continue;
+            // every warp waits on and arrives at every stage, also when it holds no block of the tile: no warp is
+            // ever a whole phase away from a barrier
+            AI_STRACE(n, 0, strace_now());
+            mbar_wait(full + r.stage, r.parity);
+            AI_STRACE(n, 1, strace_now());
+            if (firstb < d.w) {
+                const unsigned char *blob = mat_base + (size_t)r.stage * p.mat_stage_bytes;
+                const unsigned *bh = reinterpret_cast<const unsigned *>(blob) + 1;
+                const unsigned rebase = (smem_u32(img_base + (size_t)r.stage * p.img_stage_bytes) & 0xffffu) * 0x10001u;
+                for (int b = firstb; b < d.w; b += kStreamCons) {
+                    const unsigned h = bh[b];
+                    if (stream_block<DT, ACC>(rebase, blob, h, p.partials, lane)) {
+                        if constexpr (DT == AI_F32) stream_block_tracked<ACC>(rebase, blob, h, p.partials, lane);
+                    }
+                }
+                __syncwarp();
+                AI_STRACE(n, 2, strace_now());
+                AI_STRACE(n, 3, (long long)((d.w - firstb + kStreamCons - 1) / kStreamCons));
+            }
+            if (lane == 0) mbar_arrive(empty + r.stage);
+            firstb -= d.w % kStreamCons;
+            if (firstb < 0) firstb += kStreamCons;
+            r.next(p.stages);
+        }
+    }
+    AI_STRACE(15, 2, strace_now());
+
+    // ===== H5: the last blocks to finish add up the partials ===========================================================
+    // Every block publishes its partials (block barrier, then one thread: fence + atomic arrival).  A launch adds
+    // exactly gridDim.x arrivals to the context's counter, so old / gridDim.x is the launch's generation and
+    // old % gridDim.x the block's place in the order of arrival.  All but the last `nfin` blocks to arrive leave at once
+    // -- their SMs go to the next kernel of the stream; the last ones wait for the stragglers among themselves (all
+    // blocks of the grid are resident: one per SM), then share the bins: one warp per bin, fixed summation order.
+    volatile int *fin_rank = reinterpret_cast<volatile int *>(empty + kStreamMaxStages);   // spare bytes of the header
+    const int nwarps = kStreamThreads / 32;
+    const int nfin = min((int)gridDim.x, max(1, (p.npt + nwarps - 1) / nwarps));           // one bin per warp if possible
+    unsigned long long target = 0;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned long long old = atomicAdd(p.grid_sync, 1ULL);
+        const int place = (int)(old % gridDim.x);
+        target = (old / gridDim.x + 1ULL) * gridDim.x;
+        if (old + 1 == target) target = 0;                       // the last block to arrive has nothing to wait for
+        *fin_rank = place >= (int)gridDim.x - nfin ? place - ((int)gridDim.x - nfin) : -1;
+    }
+    __syncthreads();
+    const int rank = *fin_rank;
+    if (rank < 0) return;
+    // the slot range of the warp's first bin is fetched while thread 0 waits for the stragglers
+    int b = rank + nfin * warp;
+    int beg = 0, end = 0;
+    if (b < p.npt) { beg = __ldg(p.bin_slot_ptr + b); end = __ldg(p.bin_slot_ptr + b + 1); }
+    if (threadIdx.x == 0 && target) {
+        unsigned spin = 0;
+        while (true) {
+            unsigned long long now;
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(now) : "l"(p.grid_sync) : "memory");
+            if (now >= target) break;
+            if (++spin > (1u << 24)) __trap();               // a lost block traps instead of hanging the device
+        }
+    }
+    __syncthreads();
+    AI_STRACE(15, 3, strace_now());
+    while (b < p.npt) {
+        const int bn = b + nfin * nwarps;
+        int beg_n = 0, end_n = 0;
+        if (bn < p.npt) { beg_n = __ldg(p.bin_slot_ptr + bn); end_n = __ldg(p.bin_slot_ptr + bn + 1); }
+        finish_bin<ACC>(p.partials, beg, end, lane, p.empty, p.intensity + b, p.sum_signal + b, p.count + b);
+        if (lane == 0 && p.radial) {
+            const double u0 = p.range[0], delta = (p.range[1] - p.range[0]) / (double)p.npt;
+            p.radial[b] = (float)(u0 + ((double)b + 0.5) * delta);
+        }
+        b = bn; beg = beg_n; end = end_n;
+    }
+    AI_STRACE(14, 0, strace_now());
+}
+
+template <int DT, int ACC>
+int launch_stream(ai_ctx *ctx, const CUtensorMap &map, const StreamFirstDescs &first, const StreamParams &p, size_t smem,
+                  int grid, cudaStream_t st)
+{
+    static int configured_device = -1;            // per instantiation: opt in to the large dynamic shared memory once
+    if (configured_device != ctx->device) {
+        AI_CUDA(ctx, cudaFuncSetAttribute(tiled_stream_kernel<DT, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          kPipeSmemBudget));
+        configured_device = ctx->device;
+    }
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kStreamThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ai_prof_begin(ctx, st);
+    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, tiled_stream_kernel<DT, ACC>, map, first, p));
+    ai_prof_end(ctx, st);
+    return AI_OK;
+}
+
+template <int DT>
+int launch_stream_dt(ai_ctx *ctx, const CUtensorMap &map, const StreamFirstDescs &first, const StreamParams &p,
+                     size_t smem, int grid, cudaStream_t st)
+{
+    switch (ctx->accum) {
+    case AI_ACC_F32_KAHAN: return launch_stream<DT, AI_ACC_F32_KAHAN>(ctx, map, first, p, smem, grid, st);
+    case AI_ACC_F32_PLAIN: return launch_stream<DT, AI_ACC_F32_PLAIN>(ctx, map, first, p, smem, grid, st);
+    default: return launch_stream<DT, AI_ACC_F64>(ctx, map, first, p, smem, grid, st);
+    }
+}
+
+}  // namespace
+
+#ifdef AI_PIPE_TRACE
+extern "C" int ai_debug_set_stream_trace(void *dev_buffer)
+{
+    return (int)cudaMemcpyToSymbol(g_strace, &dev_buffer, sizeof(void *));
+}
+#endif
+
+// Launches the single-frame fast path when it applies (*handled = true): one frame of 32-bit pixels, no correction
+// arrays, rows on 16-byte boundaries, and at least two (tile + blob) stages fitting the shared memory of an SM.
+// The kernel is the whole hot path of the frame: stage 1 and, behind a grid barrier, H5 (no second launch).
+int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled)
+{
+    const TiledLayout &tl = ctx->tl;
+    *handled = false;
+    if (a.nframes != 1 || tl.ntiles < 1 || !tl.blob || !tl.h_first_desc || !ctx->grid_sync || ctx->no_tma || ctx->no_stream)
+        return AI_OK;
+    const bool plain = !a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask;
+    const bool is32 = a.dtype == AI_F32 || a.dtype == AI_I32 || a.dtype == AI_U32;
+    if (!plain || !is32 || !vec_ok || (reinterpret_cast<uintptr_t>(a.image) % 16) != 0) return AI_OK;
+    const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
+    const int grid = tl.ntiles < sms ? tl.ntiles : sms;
+    if (grid > kStreamMaxGrid) return AI_OK;
+
+    StreamParams p{};
+    p.img_stage_bytes = tl.tile_h * kTileW * 4;
+    p.mat_stage_bytes = ai_align_up(tl.max_blob_bytes + 1024, 1024);      // slack: the look-ahead reads past a blob's end
+    p.items_max = (tl.ntiles + grid - 1) / grid;
+    p.hdr_bytes = ai_align_up(kStreamBarBytes + 16 * p.items_max, 1024);
+    int stages = (kPipeSmemBudget - p.hdr_bytes) / (p.img_stage_bytes + p.mat_stage_bytes);
+    if (stages > kStreamMaxStages) stages = kStreamMaxStages;
+    if (ctx->tune.stream_stages > 0 && stages > ctx->tune.stream_stages) stages = ctx->tune.stream_stages;
+    while (stages * p.img_stage_bytes > 0xf000) --stages;     // tile buffers stay inside the first 64 KB (packed rebase)
+    if (stages < 2) return AI_OK;
+    p.stages = stages;
+    p.blob_desc = tl.blob_desc;
+    p.blob = tl.blob;
+    p.tile_h = tl.tile_h;
+    p.ntiles = tl.ntiles;
+    p.nslot = tl.nslot;
+    p.partials = ctx->partials;
+    p.grid_sync = ctx->grid_sync;
+    p.bin_slot_ptr = tl.bin_slot_ptr;
+    p.range = ctx->d_range;
+    p.npt = ctx->npt;
+    p.empty = ctx->empty_value;
+    p.radial = a.radial;
+    p.intensity = a.intensity;
+    p.sum_signal = a.sum_signal;
+    p.count = a.count;
+    const size_t smem = (size_t)stages * (p.img_stage_bytes + p.mat_stage_bytes) + p.hdr_bytes;
+
+    // descriptors of the first tiles of every block (host copy kept by the builder)
+    StreamFirstDescs first{};
+    for (int n = 0; n < kStreamFirst; ++n)
+        for (int b = 0; b < grid; ++b) {
+            const int w = n * grid + ((n & 1) ? grid - 1 - b : b);
+            first.d[n][b] = w < tl.ntiles ? tl.h_first_desc[w] : make_int4(0, 0, 0, 0);
+        }
+    CUtensorMap map{};
+    int rc = ai_make_frame_map(ctx, a, tl.tile_h, &map);
+    if (rc != AI_OK) return rc;
+    rc = AI_EINVAL;
+    switch (a.dtype) {
+    case AI_F32: rc = launch_stream_dt<AI_F32>(ctx, map, first, p, smem, grid, st); break;
+    case AI_I32: rc = launch_stream_dt<AI_I32>(ctx, map, first, p, smem, grid, st); break;
+    case AI_U32: rc = launch_stream_dt<AI_U32>(ctx, map, first, p, smem, grid, st); break;
+    default: break;
+    }
+    if (rc == AI_OK) *handled = true;
+    return rc;
+}

@@ -15,6 +15,7 @@
 #include "tiled_common.cuh"
 
 int ai_launch_pipe_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);
+int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);
 
 namespace {
 
@@ -94,52 +95,35 @@ __global__ void __launch_bounds__(kS1Threads, kS1MinBlocks) tiled_stage1_kernel(
 }
 
 // ---- H5: fixed-order sum of each bin's partials, ratio, three outputs --------------------------------------------------
+// Launched with programmatic stream serialisation (launch_stage2): the blocks may become resident while stage 1 is
+// still running; everything that does not depend on stage 1 (the slot range of the bin, the radial axis) is done
+// before griddepcontrol.wait, which returns once stage 1 has completed and its partials are visible.
 template <int ACC>
 __global__ void __launch_bounds__(256) tiled_stage2_kernel(const int *__restrict__ bin_slot_ptr, int nslot, int npt,
-                                                           const void *__restrict__ partials,
+                                                           const void *partials,
                                                            const double *__restrict__ range, float empty,
                                                            float *__restrict__ radial, float *__restrict__ intensity,
                                                            float *__restrict__ sum_signal, float *__restrict__ count)
 {
     const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const int f = blockIdx.y, lane = threadIdx.x & 31;
+    int beg = 0, end = 0;
+    if (b < npt) {
+        beg = __ldg(bin_slot_ptr + b);
+        end = __ldg(bin_slot_ptr + b + 1);
+        if (lane == 0 && radial && f == 0) {
+            double u0 = range[0], delta = (range[1] - range[0]) / (double)npt;
+            radial[b] = (float)(u0 + ((double)b + 0.5) * delta);
+        }
+    }
+    // the next stage 1 of the stream (integrate_stream.cu) may start its prologue now; it touches the partials only
+    // after its own griddepcontrol.wait, i.e. after this grid has completed
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (b >= npt) return;
-    const int beg = bin_slot_ptr[b], end = bin_slot_ptr[b + 1];
     const int64_t o = (int64_t)f * npt + b;
-    if constexpr (ACC == AI_ACC_F32_PLAIN) {
-        const float4 *p = reinterpret_cast<const float4 *>(partials) + (int64_t)f * nslot;
-        float S = 0.f, C = 0.f;
-        for (int k = beg + lane; k < end; k += 32) { float4 v = p[k]; S += v.x; C += v.z; }
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            S += __shfl_xor_sync(AI_FULL_MASK, S, d);
-            C += __shfl_xor_sync(AI_FULL_MASK, C, d);
-        }
-        if (lane == 0) write_bin_f32(0, S, C, empty, intensity + o, sum_signal + o, count + o);
-    } else {
-        double S = 0.0, C = 0.0;
-        if constexpr (ACC == AI_ACC_F64) {
-            const double2 *p = reinterpret_cast<const double2 *>(partials) + (int64_t)f * nslot;
-            for (int k = beg + lane; k < end; k += 32) { double2 v = p[k]; S += v.x; C += v.y; }
-        } else {
-            const float4 *p = reinterpret_cast<const float4 *>(partials) + (int64_t)f * nslot;
-            for (int k = beg + lane; k < end; k += 32) {
-                float4 v = p[k];
-                S += (double)v.x + (double)v.y;
-                C += (double)v.z + (double)v.w;
-            }
-        }
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            S += __shfl_xor_sync(AI_FULL_MASK, S, d);
-            C += __shfl_xor_sync(AI_FULL_MASK, C, d);
-        }
-        if (lane == 0) write_bin(0, S, C, empty, intensity + o, sum_signal + o, count + o);
-    }
-    if (lane == 0 && radial && f == 0) {
-        double u0 = range[0], delta = (range[1] - range[0]) / (double)npt;
-        radial[b] = (float)(u0 + ((double)b + 0.5) * delta);
-    }
+    finish_bin<ACC>(reinterpret_cast<const char *>(partials) + (int64_t)f * nslot * 16, beg, end, lane, empty,
+                    intensity + o, sum_signal + o, count + o);
 }
 
 template <int DT, int ACC>
@@ -181,17 +165,27 @@ int launch_simple_any(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t 
 int launch_stage2(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 {
     const TiledLayout &tl = ctx->tl;
-    dim3 g2((ctx->npt + 7) / 8, a.nframes);
+    // programmatic dependent launch: the launch latency of stage 2 overlaps the tail of stage 1
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((ctx->npt + 7) / 8, a.nframes);
+    cfg.blockDim = dim3(256);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
 #define AI_S2(ACC)                                                                                                  \
-    tiled_stage2_kernel<ACC><<<g2, 256, 0, st>>>(tl.bin_slot_ptr, tl.nslot, ctx->npt, ctx->partials, ctx->d_range,  \
-                                                 ctx->empty_value, a.radial, a.intensity, a.sum_signal, a.count)
+    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, tiled_stage2_kernel<ACC>, (const int *)tl.bin_slot_ptr, tl.nslot, ctx->npt, \
+                                    (const void *)ctx->partials, (const double *)ctx->d_range, ctx->empty_value,    \
+                                    a.radial, a.intensity, a.sum_signal, a.count))
     switch (ctx->accum) {
     case AI_ACC_F32_KAHAN: AI_S2(AI_ACC_F32_KAHAN); break;
     case AI_ACC_F32_PLAIN: AI_S2(AI_ACC_F32_PLAIN); break;
     default: AI_S2(AI_ACC_F64); break;
     }
 #undef AI_S2
-    AI_CUDA(ctx, cudaGetLastError());
     return AI_OK;
 }
 
@@ -216,7 +210,16 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
                        aligned(a.dark, 16) && aligned(a.flat, 16) && aligned(a.solidangle, 16) &&
                        aligned(a.polarization, 16) && aligned(a.mask, 4);
     bool handled = false;
-    int rc = ctx->layout == AI_LAYOUT_TILED_DIRECT ? AI_OK : ai_launch_pipe_stage1(ctx, a, vec_ok, st, &handled);
+    int rc = AI_OK;
+    if (ctx->layout != AI_LAYOUT_TILED_DIRECT) {
+        rc = ai_launch_stream_stage1(ctx, a, vec_ok, st, &handled);           // one plain 32-bit frame: whole hot path
+        if (rc != AI_OK) return rc;
+        if (handled) {
+            ctx->last_launches = 1;
+            return AI_OK;
+        }
+        rc = ai_launch_pipe_stage1(ctx, a, vec_ok, st, &handled);
+    }
     if (rc != AI_OK) return rc;
     if (!handled) {
         // this kernel writes one partial per segment, into the first of the segment's slots (one per run of the
@@ -224,6 +227,10 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
         AI_CUDA(ctx, cudaMemsetAsync(ctx->partials, 0, need, st));
         rc = launch_simple_any(ctx, a, vec_ok, st);
         if (rc != AI_OK) return rc;
+    }
+    if (ctx->stage1_only) {
+        ctx->last_launches = 1;
+        return AI_OK;
     }
     rc = launch_stage2(ctx, a, st);
     ctx->last_launches = 2;

@@ -54,6 +54,64 @@ __device__ __forceinline__ void store_partial(void *partials, int64_t slot, cons
     }
 }
 
+// ---- H5: one warp adds the partials [beg, end) of one bin in a fixed order (lane-strided, then a shuffle tree) and
+// writes the three outputs (ratio, unweighted histogram, weighted histogram).  `part_f` = the frame's
+// partial records; loads bypass L1 (the records were written by other SMs).
+constexpr int kFinishUnroll = 4;      // 128-bit loads in flight per lane: 128 partials of a bin per trip
+
+template <int ACC>
+__device__ __forceinline__ void finish_bin(const void *part_f, int beg, int end, int lane, float empty, float *intensity,
+                                           float *sum_signal, float *count)
+{
+    if constexpr (ACC == AI_ACC_F32_PLAIN) {
+        const float4 *p = reinterpret_cast<const float4 *>(part_f);
+        float S = 0.f, C = 0.f;
+        for (int k0 = beg + lane; k0 < end; k0 += 32 * kFinishUnroll) {
+            float4 v[kFinishUnroll];
+#pragma unroll
+            for (int i = 0; i < kFinishUnroll; ++i) v[i] = k0 + 32 * i < end ? __ldcg(p + k0 + 32 * i) : make_float4(0, 0, 0, 0);
+#pragma unroll
+            for (int i = 0; i < kFinishUnroll; ++i) { S += v[i].x; C += v[i].z; }
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            S += __shfl_xor_sync(AI_FULL_MASK, S, d);
+            C += __shfl_xor_sync(AI_FULL_MASK, C, d);
+        }
+        if (lane == 0) write_bin_f32(0, S, C, empty, intensity, sum_signal, count);
+    } else {
+        double S = 0.0, C = 0.0;
+        if constexpr (ACC == AI_ACC_F64) {
+            const double2 *p = reinterpret_cast<const double2 *>(part_f);
+            for (int k0 = beg + lane; k0 < end; k0 += 32 * kFinishUnroll) {
+                double2 v[kFinishUnroll];
+#pragma unroll
+                for (int i = 0; i < kFinishUnroll; ++i) v[i] = k0 + 32 * i < end ? __ldcg(p + k0 + 32 * i) : make_double2(0, 0);
+#pragma unroll
+                for (int i = 0; i < kFinishUnroll; ++i) { S += v[i].x; C += v[i].y; }
+            }
+        } else {
+            const float4 *p = reinterpret_cast<const float4 *>(part_f);
+            for (int k0 = beg + lane; k0 < end; k0 += 32 * kFinishUnroll) {
+                float4 v[kFinishUnroll];
+#pragma unroll
+                for (int i = 0; i < kFinishUnroll; ++i) v[i] = k0 + 32 * i < end ? __ldcg(p + k0 + 32 * i) : make_float4(0, 0, 0, 0);
+#pragma unroll
+                for (int i = 0; i < kFinishUnroll; ++i) {
+                    S += (double)v[i].x + (double)v[i].y;
+                    C += (double)v[i].z + (double)v[i].w;
+                }
+            }
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            S += __shfl_xor_sync(AI_FULL_MASK, S, d);
+            C += __shfl_xor_sync(AI_FULL_MASK, C, d);
+        }
+        if (lane == 0) write_bin(0, S, C, empty, intensity, sum_signal, count);
+    }
+}
+
 // value of the pixel whose position in the tile buffer is stored as a byte offset
 __device__ __forceinline__ float tile_at(const float *tile, unsigned off)
 {

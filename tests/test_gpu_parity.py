@@ -278,6 +278,60 @@ def test_compensation_keeps_small_terms(torch, B, workloads):
 
 
 # ----------------------------------------------------------------------------------------------------------------------
+# the two pipelined stage-1 kernels: single-frame stream kernel (default for plain 32-bit frames) and the general one
+# ----------------------------------------------------------------------------------------------------------------------
+def _run_raw(torch, B, integ, img, dtype):
+    if dtype == "uint32":
+        t, code = torch.from_numpy(img.view(np.int32)).cuda(), B.AI_U32
+    else:
+        t, code = torch.from_numpy(img).cuda(), None
+    i, s, c = integ.outputs()
+    B.ai_integrate1d(integ.ctx, t, None, None, None, None, None, None, i, s, c, dtype=code)
+    torch.cuda.synchronize()
+    return {"intensity": i.cpu().numpy(), "sum_signal": s.cpu().numpy(), "count": c.cpu().numpy()}
+
+
+@pytest.mark.parametrize("path", ["stream", "pipe"])
+@pytest.mark.parametrize("dtype", ["float32", "int32", "uint32"])
+@pytest.mark.parametrize("shape", [(256, 256), (130, 200), (70, 1028)])
+def test_single_frame_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, shape):
+    """AZINT_NO_STREAM=1 (read by ai_setup) sends single plain frames through the general pipelined kernel."""
+    if path == "pipe":
+        monkeypatch.setenv("AZINT_NO_STREAM", "1")
+    h, w = shape
+    cfg = workloads.tiny_config(h, w, center_x=w * 0.41, center_y=h * 0.57, unit=workloads.Q_NM, npt=173,
+                                distance_m=0.02, name=f"single_{h}x{w}")
+    rng = np.random.default_rng(h * 1000 + w)
+    img = rng.poisson(200.0, size=(h, w)).astype(dtype)
+    integ = B.Integrator(cfg)
+    for acc in ("kahan", "f64"):
+        integ.set_options(LAYOUTS["tiled"], ACCUMS[acc])
+        got = _run_raw(torch, B, integ, img, dtype)
+        assert_profile(got, _oracle_profile(oracle, cfg, workloads.Frame(image=img)), what=f"{path}/{dtype}/{shape}/{acc}")
+    integ.close()
+
+
+@pytest.mark.parametrize("path", ["stream", "pipe"])
+def test_non_finite_pixels_in_plain_float_frames(torch, B, oracle, workloads, monkeypatch, path):
+    """No mask, no corrections: NaN / Inf pixels are found lazily (a non-finite lane sum repeats the block with the
+    tracked variant) and behave like masked pixels (oracle O5)."""
+    if path == "pipe":
+        monkeypatch.setenv("AZINT_NO_STREAM", "1")
+    cfg = workloads.CONFIGS["cfg1b"]
+    img = workloads.make_frame(cfg).image.copy()
+    rng = np.random.default_rng(77)
+    bad = rng.integers(0, cfg.npix, size=40)
+    img.ravel()[bad[:20]] = np.nan
+    img.ravel()[bad[20:30]] = np.inf
+    img.ravel()[bad[30:]] = -np.inf
+    img[0, 0] = np.inf                      # pixel 0 of a tile: where padding entries point
+    integ = B.Integrator(cfg, empty_value=-3.0)
+    fr = workloads.Frame(image=img)
+    assert_profile(_run(torch, integ, fr), _oracle_profile(oracle, cfg, fr, empty=-3.0), what=f"non-finite/{path}")
+    integ.close()
+
+
+# ----------------------------------------------------------------------------------------------------------------------
 # H6: batch
 # ----------------------------------------------------------------------------------------------------------------------
 def test_batch_matches_oracle_small(torch, B, oracle, workloads):
