@@ -132,6 +132,12 @@ int ai_integrate1d_host(ai_ctx *ctx, const void *image_host, ai_dtype dtype, con
                         const float *solidangle, const float *polarization, const uint8_t *mask,
                         float *intensity_host, float *sum_signal_host, float *count_host, void *cuda_stream);
 
+/* Sizes of the TILED execution layout, for byte accounting in benchmarks.  info (HOST pointer)
+ * receives 8 values: {tile height in rows, number of tiles, number of (tile, bin) segments, padded number of entries,
+ * total bytes of the sliced matrix (all blobs), largest blob in bytes, partial records per frame, (tile + blob) stages
+ * the single-frame kernel would use (0 = it does not apply)}.  Errors: AI_EINVAL, AI_ENOTBUILT. */
+int ai_get_layout_info(const ai_ctx *ctx, int64_t info[8]);
+
 /* Number of kernels the last ai_integrate1d* call launched (for accounting in benchmarks). */
 int ai_last_launch_count(const ai_ctx *ctx);
 

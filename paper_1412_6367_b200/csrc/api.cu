@@ -38,6 +38,22 @@ const char *ai_last_error(const ai_ctx *ctx) { return ctx ? ctx->err : ""; }
 
 int ai_last_launch_count(const ai_ctx *ctx) { return ctx ? ctx->last_launches : 0; }
 
+int ai_get_layout_info(const ai_ctx *ctx, int64_t info[8])
+{
+    if (!ctx || !info) return AI_EINVAL;
+    if (!ctx->built) return AI_ENOTBUILT;
+    const TiledLayout &tl = ctx->tl;
+    info[0] = tl.tile_h;
+    info[1] = tl.ntiles;
+    info[2] = tl.nseg;
+    info[3] = tl.tnnz;
+    info[4] = tl.blob_bytes;
+    info[5] = tl.max_blob_bytes;
+    info[6] = tl.nslot;
+    info[7] = ai_stream_stages(ctx);
+    return AI_OK;
+}
+
 int ai_profile_enable(ai_ctx *ctx, int on)
 {
     if (!ctx) return AI_EINVAL;
@@ -102,6 +118,7 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
                 else if (!strcmp(key, "bis")) ctx->tune.batch_img_stages = val;
                 else if (!strcmp(key, "fl")) ctx->tune.inflight = val;
                 else if (!strcmp(key, "ss")) ctx->tune.stream_stages = val;
+                else if (!strcmp(key, "pf")) ctx->tune.prefetch_tiles = val;
             }
             q = strchr(q, ',');
             if (q) ++q;

@@ -146,9 +146,22 @@ __global__ void __launch_bounds__(256) slice_fill_kernel(const int *__restrict__
         const int s = slice_seg[g0 + i], win = slice_win[g0 + i];
         const int base = seg_ptr[s] + kSliceMax * win;
         const int len = min(kSliceMax, seg_ptr[s + 1] - base);
+        // Adjacent lanes that hold full slices of the same segment (windows win0, win0 + 1, ... of its entries) share
+        // them interleaved: at step j lane q of m reads the four entries 4 * (j * m + q) ... of the m windows, so that
+        // the lanes of one segment gather neighbouring pixels in the same step (different rows and columns of the tile
+        // -> different shared-memory banks) instead of pixels 32 entries, i.e. a whole number of swizzle periods, apart.
+        int src = base + step * 4;
+        if (len == kSliceMax) {
+            int q = 0, m = 1;
+            while (q < lane && slice_seg[g0 + i - q - 1] == s && slice_win[g0 + i - q - 1] == win - q - 1) ++q;
+            while (lane - q + m < 32 && i - q + m < S && slice_seg[g0 + i - q + m] == s &&
+                   seg_ptr[s + 1] - (seg_ptr[s] + kSliceMax * slice_win[g0 + i - q + m]) >= kSliceMax)
+                ++m;
+            src = seg_ptr[s] + kSliceMax * (win - q) + 4 * (step * m + q);
+        }
         if (step * 4 < len) {      // the rest of the block stays zero: coefficient 0 at pixel 0 of the tile
-            const float4 c = *reinterpret_cast<const float4 *>(tcoef + base + step * 4);
-            const ushort4 x = *reinterpret_cast<const ushort4 *>(tidx + base + step * 4);
+            const float4 c = *reinterpret_cast<const float4 *>(tcoef + src);
+            const ushort4 x = *reinterpret_cast<const ushort4 *>(tidx + src);
             reinterpret_cast<float4 *>(blk)[step * 32 + lane] = c;
             reinterpret_cast<ushort4 *>(blk + (size_t)nsteps * 512)[step * 32 + lane] = x;
         }

@@ -58,6 +58,7 @@ struct PipeTune {
     int batch_mat_stages = 2, batch_img_stages = kPipeMaxImgStages;
     int inflight = 0;                          // 0 = as many as there are stages
     int stream_stages = 0;                     // cap on the (tile + blob) stages of the single-frame kernel, 0 = none
+    int prefetch_tiles = 0;                    // single-frame kernel: tiles per block prefetched into L2 in the prologue
 };
 inline PipePlan ai_pipe_plan(int max_blob_bytes, int tile_h, bool batch, const PipeTune &tune = PipeTune())
 {
@@ -196,3 +197,4 @@ struct FrameArgs {
 int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_csr(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_lut(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
+int ai_stream_stages(const ai_ctx *ctx);      // integrate_stream.cu: (tile + blob) stages of the single-frame kernel, 0 = n/a

@@ -22,8 +22,8 @@ constexpr int kStreamCons = 20;                      // consumer warps (21 warps
 constexpr int kStreamThreads = 32 * (1 + kStreamCons);
 constexpr int kStreamFirst = 3;                      // descriptors per block passed by value
 constexpr int kStreamMaxGrid = 160;
-constexpr int kStreamMaxStages = 4;
-constexpr int kStreamBarBytes = 128;                 // full[4] + empty[4], padded
+constexpr int kStreamMaxStages = 8;
+constexpr int kStreamBarBytes = 256;                 // full[8] + empty[8] + a few words of block-wide state
 
 struct StreamFirstDescs {
     int4 d[kStreamFirst][kStreamMaxGrid];
@@ -34,6 +34,8 @@ struct StreamParams {
     const unsigned char *blob;
     int tile_h, ntiles, nslot;
     int stages, mat_stage_bytes, img_stage_bytes, hdr_bytes, items_max;
+    int prefetch_tiles;          // tiles per block whose data is pulled into L2 before the grid dependency resolves
+    int launch_index;            // launches of this context so far, modulo 8 (development trace only)
     void *partials;
     // H5 fused behind a grid-wide barrier (every block is resident: one per SM, grid <= number of SMs)
     unsigned long long *grid_sync;     // arrivals of all launches of this context, never reset
@@ -47,19 +49,26 @@ struct StreamParams {
 // ---- development aid (-DAI_PIPE_TRACE): per (block, tile, warp) globaltimer stamps ------------------------------------
 #ifdef AI_PIPE_TRACE
 __device__ long long *g_strace = nullptr;          // [grid][16 tiles][32 warps][4]
+__device__ int g_strace_div = 1;                   // trace every g_strace_div-th tile
 __device__ __forceinline__ long long strace_now()
 {
     long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
+#define AI_STRACE_AT(row, slot, val)                                                                            \
+    do {                                                                                                        \
+        if (g_strace && (threadIdx.x & 31) == 0)                                                                \
+            g_strace[(((((size_t)p.launch_index * gridDim.x + blockIdx.x) * 16 + (row)) * 32) + (threadIdx.x >> 5)) * 4 + (slot)] = (val); \
+    } while (0)
+// tiles: every g_strace_div-th one, rows 0..13; rows 14 and 15 hold the kernel-level stamps
 #define AI_STRACE(item, slot, val)                                                                              \
     do {                                                                                                        \
-        if (g_strace && (threadIdx.x & 31) == 0 && (item) < 16)                                                 \
-            g_strace[((((size_t)blockIdx.x * 16 + (item)) * 32) + (threadIdx.x >> 5)) * 4 + (slot)] = (val);    \
+        if ((item) % g_strace_div == 0 && (item) / g_strace_div < 14) AI_STRACE_AT((item) / g_strace_div, slot, val); \
     } while (0)
 #else
 #define AI_STRACE(item, slot, val) do { } while (0)
+#define AI_STRACE_AT(row, slot, val) do { } while (0)
 #define strace_now() 0
 #endif
 
@@ -185,7 +194,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
     int4 *desc_s = reinterpret_cast<int4 *>(hdr + kStreamBarBytes);
     unsigned char *mat_base = hdr + p.hdr_bytes;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    AI_STRACE(15, 0, strace_now());
+    AI_STRACE_AT(15, 0, strace_now());
 
     // number of tiles of this block
     int nmine = 0;
@@ -229,9 +238,29 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
     // H5 reads the slot ranges of the bins at the very end: pull them into L2 now (static data, 4 bytes per bin)
     for (int k = threadIdx.x * 32; k <= p.npt; k += kStreamThreads * 32)
         asm volatile("prefetch.global.L2 [%0];" ::"l"(p.bin_slot_ptr + k));
-    // stage 2 is launched with programmatic stream serialisation too: its blocks may be scheduled as SMs free up
+    // the next kernel of the stream may be scheduled as SMs free up
     asm volatile("griddepcontrol.launch_dependents;");
+    __syncthreads();                                   // descriptors are in shared memory
+    // While the previous kernel of the stream drains, HBM would idle: pull this block's share of the frame and the
+    // rest of its matrix into L2 (prefetches return nothing to the SM, and L2 is the point of coherence: a frame
+    // that the previous kernel is still writing is read, after the wait below, as that kernel left it).
+    if (warp == 0) {
+        const int npf = min(nmine, p.prefetch_tiles);
+        for (int n = lane; n < npf; n += 32) {
+            const int4 d = desc_s[n];
+            if (d.w == 0) continue;
+            const int ty = d.z >> 16, tx = d.z & 0xffff;
+            asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
+                         ::"l"(&tmap), "r"(tx * kTileW), "r"(ty * p.tile_h), "r"(0) : "memory");
+            asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
+                         ::"l"(&tmap), "r"(tx * kTileW + 32), "r"(ty * p.tile_h), "r"(0) : "memory");
+            if (n >= npre)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;"
+                             ::"l"(p.blob + (size_t)d.x * 16), "r"(d.y) : "memory");
+        }
+    }
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    AI_STRACE_AT(14, 1, strace_now());
     if (threadIdx.x == 0) {
         int stage = 0;
         for (int n = 0; n < npre; ++n) {
@@ -241,7 +270,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
         }
     }
     __syncthreads();
-    AI_STRACE(15, 1, strace_now());
+    AI_STRACE_AT(15, 1, strace_now());
 
     Ring r;
     if (warp == 0) {
@@ -294,7 +323,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
             r.next(p.stages);
         }
     }
-    AI_STRACE(15, 2, strace_now());
+    AI_STRACE_AT(15, 2, strace_now());
 
     // ===== H5: the last blocks to finish add up the partials ===========================================================
     // Every block publishes its partials (block barrier, then one thread: fence + atomic arrival).  A launch adds
@@ -318,10 +347,12 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
     __syncthreads();
     const int rank = *fin_rank;
     if (rank < 0) return;
-    // the slot range of the warp's first bin is fetched while thread 0 waits for the stragglers
+    // the slot ranges of the warp's first two bins are fetched while thread 0 waits for the stragglers
+    const int stride = nfin * nwarps;
     int b = rank + nfin * warp;
-    int beg = 0, end = 0;
-    if (b < p.npt) { beg = __ldg(p.bin_slot_ptr + b); end = __ldg(p.bin_slot_ptr + b + 1); }
+    int beg0 = 0, end0 = 0, beg1 = 0, end1 = 0;
+    if (b < p.npt) { beg0 = __ldg(p.bin_slot_ptr + b); end0 = __ldg(p.bin_slot_ptr + b + 1); }
+    if (b + stride < p.npt) { beg1 = __ldg(p.bin_slot_ptr + b + stride); end1 = __ldg(p.bin_slot_ptr + b + stride + 1); }
     if (threadIdx.x == 0 && target) {
         unsigned spin = 0;
         while (true) {
@@ -332,19 +363,23 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
         }
     }
     __syncthreads();
-    AI_STRACE(15, 3, strace_now());
+    AI_STRACE_AT(15, 3, strace_now());
     while (b < p.npt) {
-        const int bn = b + nfin * nwarps;
-        int beg_n = 0, end_n = 0;
-        if (bn < p.npt) { beg_n = __ldg(p.bin_slot_ptr + bn); end_n = __ldg(p.bin_slot_ptr + bn + 1); }
-        finish_bin<ACC>(p.partials, beg, end, lane, p.empty, p.intensity + b, p.sum_signal + b, p.count + b);
+        const bool two = b + stride < p.npt;
+        const int bn = b + 2 * stride;
+        int nb0 = 0, ne0 = 0, nb1 = 0, ne1 = 0;
+        if (bn < p.npt) { nb0 = __ldg(p.bin_slot_ptr + bn); ne0 = __ldg(p.bin_slot_ptr + bn + 1); }
+        if (bn + stride < p.npt) { nb1 = __ldg(p.bin_slot_ptr + bn + stride); ne1 = __ldg(p.bin_slot_ptr + bn + stride + 1); }
+        finish_bins<ACC>(p.partials, b, beg0, end0, two, b + stride, beg1, end1, lane, p.empty, p.intensity, p.sum_signal,
+                         p.count);
         if (lane == 0 && p.radial) {
             const double u0 = p.range[0], delta = (p.range[1] - p.range[0]) / (double)p.npt;
             p.radial[b] = (float)(u0 + ((double)b + 0.5) * delta);
+            if (two) p.radial[b + stride] = (float)(u0 + ((double)(b + stride) + 0.5) * delta);
         }
-        b = bn; beg = beg_n; end = end_n;
+        b = bn; beg0 = nb0; end0 = ne0; beg1 = nb1; end1 = ne1;
     }
-    AI_STRACE(14, 0, strace_now());
+    AI_STRACE_AT(14, 0, strace_now());
 }
 
 template <int DT, int ACC>
@@ -387,11 +422,38 @@ int launch_stream_dt(ai_ctx *ctx, const CUtensorMap &map, const StreamFirstDescs
 }  // namespace
 
 #ifdef AI_PIPE_TRACE
-extern "C" int ai_debug_set_stream_trace(void *dev_buffer)
+extern "C" int ai_debug_set_stream_trace(void *dev_buffer, int div)
 {
+    cudaMemcpyToSymbol(g_strace_div, &div, sizeof(int));
     return (int)cudaMemcpyToSymbol(g_strace, &dev_buffer, sizeof(void *));
 }
 #endif
+
+// shared-memory plan: [tile stages][barriers + descriptors][blob stages]; false if fewer than two stages fit
+static bool stream_plan(const ai_ctx *ctx, int grid, StreamParams *p)
+{
+    const TiledLayout &tl = ctx->tl;
+    p->img_stage_bytes = tl.tile_h * kTileW * 4;
+    p->mat_stage_bytes = ai_align_up(tl.max_blob_bytes + 1024, 1024);     // slack: the look-ahead reads past a blob's end
+    p->items_max = (tl.ntiles + grid - 1) / grid;
+    p->hdr_bytes = ai_align_up(kStreamBarBytes + 16 * p->items_max, 1024);
+    int stages = (kPipeSmemBudget - p->hdr_bytes) / (p->img_stage_bytes + p->mat_stage_bytes);
+    if (stages > kStreamMaxStages) stages = kStreamMaxStages;
+    if (ctx->tune.stream_stages > 0 && stages > ctx->tune.stream_stages) stages = ctx->tune.stream_stages;
+    while (stages * p->img_stage_bytes > 0xf000) --stages;    // tile buffers stay inside the first 64 KB (packed rebase)
+    p->stages = stages;
+    return stages >= 2;
+}
+
+int ai_stream_stages(const ai_ctx *ctx)
+{
+    const TiledLayout &tl = ctx->tl;
+    if (tl.ntiles < 1 || !tl.blob) return 0;
+    const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
+    const int grid = tl.ntiles < sms ? tl.ntiles : sms;
+    StreamParams p{};
+    return grid <= kStreamMaxGrid && stream_plan(ctx, grid, &p) ? p.stages : 0;
+}
 
 // Launches the single-frame fast path when it applies (*handled = true): one frame of 32-bit pixels, no correction
 // arrays, rows on 16-byte boundaries, and at least two (tile + blob) stages fitting the shared memory of an SM.
@@ -410,22 +472,17 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStr
     if (grid > kStreamMaxGrid) return AI_OK;
 
     StreamParams p{};
-    p.img_stage_bytes = tl.tile_h * kTileW * 4;
-    p.mat_stage_bytes = ai_align_up(tl.max_blob_bytes + 1024, 1024);      // slack: the look-ahead reads past a blob's end
-    p.items_max = (tl.ntiles + grid - 1) / grid;
-    p.hdr_bytes = ai_align_up(kStreamBarBytes + 16 * p.items_max, 1024);
-    int stages = (kPipeSmemBudget - p.hdr_bytes) / (p.img_stage_bytes + p.mat_stage_bytes);
-    if (stages > kStreamMaxStages) stages = kStreamMaxStages;
-    if (ctx->tune.stream_stages > 0 && stages > ctx->tune.stream_stages) stages = ctx->tune.stream_stages;
-    while (stages * p.img_stage_bytes > 0xf000) --stages;     // tile buffers stay inside the first 64 KB (packed rebase)
-    if (stages < 2) return AI_OK;
-    p.stages = stages;
+    if (!stream_plan(ctx, grid, &p)) return AI_OK;
+    const int stages = p.stages;
     p.blob_desc = tl.blob_desc;
     p.blob = tl.blob;
     p.tile_h = tl.tile_h;
     p.ntiles = tl.ntiles;
     p.nslot = tl.nslot;
     p.partials = ctx->partials;
+    p.prefetch_tiles = ctx->tune.prefetch_tiles;
+    static unsigned launches = 0;                  // development trace only: which of 8 trace buffers the launch writes
+    p.launch_index = launches++ & 7;
     p.grid_sync = ctx->grid_sync;
     p.bin_slot_ptr = tl.bin_slot_ptr;
     p.range = ctx->d_range;

@@ -54,62 +54,74 @@ __device__ __forceinline__ void store_partial(void *partials, int64_t slot, cons
     }
 }
 
-// ---- H5: one warp adds the partials [beg, end) of one bin in a fixed order (lane-strided, then a shuffle tree) and
-// writes the three outputs (ratio, unweighted histogram, weighted histogram).  `part_f` = the frame's
-// partial records; loads bypass L1 (the records were written by other SMs).
-constexpr int kFinishUnroll = 4;      // 128-bit loads in flight per lane: 128 partials of a bin per trip
+// ---- H5: one warp adds the partials of a bin in a fixed order (lane-strided, then a shuffle tree) and writes the
+// three outputs (ratio, unweighted histogram, weighted histogram).  `part_f` = the frame's partial
+// records; loads bypass L1 (the records were written by other SMs).  Two bins are summed side by side so that their
+// loads overlap (the records may have to come from HBM); results do not depend on the pairing.
+constexpr int kFinishUnroll = 4;      // 128-bit loads in flight per lane and bin
+
+// one partial record as (signal, count) in the arithmetic the final sum is carried in
+template <int ACC> struct FinishT { using T = double; };
+template <> struct FinishT<AI_ACC_F32_PLAIN> { using T = float; };
+
+template <int ACC>
+__device__ __forceinline__ void finish_load(const void *part_f, int k, bool on, typename FinishT<ACC>::T &s,
+                                            typename FinishT<ACC>::T &c)
+{
+    if constexpr (ACC == AI_ACC_F64) {
+        const double2 v = on ? __ldcg(reinterpret_cast<const double2 *>(part_f) + k) : make_double2(0, 0);
+        s = v.x; c = v.y;
+    } else {
+        const float4 v = on ? __ldcg(reinterpret_cast<const float4 *>(part_f) + k) : make_float4(0, 0, 0, 0);
+        if constexpr (ACC == AI_ACC_F32_PLAIN) { s = v.x; c = v.z; }
+        else { s = (double)v.x + (double)v.y; c = (double)v.z + (double)v.w; }
+    }
+}
+
+template <int ACC>
+__device__ __forceinline__ void finish_write(typename FinishT<ACC>::T S, typename FinishT<ACC>::T C, int lane,
+                                             float empty, float *intensity, float *sum_signal, float *count)
+{
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        S += __shfl_xor_sync(AI_FULL_MASK, S, d);
+        C += __shfl_xor_sync(AI_FULL_MASK, C, d);
+    }
+    if (lane == 0) {
+        if constexpr (ACC == AI_ACC_F32_PLAIN) write_bin_f32(0, S, C, empty, intensity, sum_signal, count);
+        else write_bin(0, S, C, empty, intensity, sum_signal, count);
+    }
+}
+
+// bins b0 (slots [beg0, end0)) and, if two, b1 (slots [beg1, end1)); out_* point at element 0 of the frame's outputs
+template <int ACC>
+__device__ __forceinline__ void finish_bins(const void *part_f, int b0, int beg0, int end0, bool two, int b1, int beg1,
+                                            int end1, int lane, float empty, float *intensity, float *sum_signal,
+                                            float *count)
+{
+    using T = typename FinishT<ACC>::T;
+    T S0 = 0, C0 = 0, S1 = 0, C1 = 0;
+    if (!two) beg1 = end1 = 0;
+    const int n0 = end0 - beg0, n1 = end1 - beg1;
+    for (int k0 = lane; k0 < n0 || k0 < n1; k0 += 32 * kFinishUnroll) {
+        T s0[kFinishUnroll], c0[kFinishUnroll], s1[kFinishUnroll], c1[kFinishUnroll];
+#pragma unroll
+        for (int i = 0; i < kFinishUnroll; ++i) {
+            finish_load<ACC>(part_f, beg0 + k0 + 32 * i, k0 + 32 * i < n0, s0[i], c0[i]);
+            finish_load<ACC>(part_f, beg1 + k0 + 32 * i, k0 + 32 * i < n1, s1[i], c1[i]);
+        }
+#pragma unroll
+        for (int i = 0; i < kFinishUnroll; ++i) { S0 += s0[i]; C0 += c0[i]; S1 += s1[i]; C1 += c1[i]; }
+    }
+    finish_write<ACC>(S0, C0, lane, empty, intensity + b0, sum_signal + b0, count + b0);
+    if (two) finish_write<ACC>(S1, C1, lane, empty, intensity + b1, sum_signal + b1, count + b1);
+}
 
 template <int ACC>
 __device__ __forceinline__ void finish_bin(const void *part_f, int beg, int end, int lane, float empty, float *intensity,
                                            float *sum_signal, float *count)
 {
-    if constexpr (ACC == AI_ACC_F32_PLAIN) {
-        const float4 *p = reinterpret_cast<const float4 *>(part_f);
-        float S = 0.f, C = 0.f;
-        for (int k0 = beg + lane; k0 < end; k0 += 32 * kFinishUnroll) {
-            float4 v[kFinishUnroll];
-#pragma unroll
-            for (int i = 0; i < kFinishUnroll; ++i) v[i] = k0 + 32 * i < end ? __ldcg(p + k0 + 32 * i) : make_float4(0, 0, 0, 0);
-#pragma unroll
-            for (int i = 0; i < kFinishUnroll; ++i) { S += v[i].x; C += v[i].z; }
-        }
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            S += __shfl_xor_sync(AI_FULL_MASK, S, d);
-            C += __shfl_xor_sync(AI_FULL_MASK, C, d);
-        }
-        if (lane == 0) write_bin_f32(0, S, C, empty, intensity, sum_signal, count);
-    } else {
-        double S = 0.0, C = 0.0;
-        if constexpr (ACC == AI_ACC_F64) {
-            const double2 *p = reinterpret_cast<const double2 *>(part_f);
-            for (int k0 = beg + lane; k0 < end; k0 += 32 * kFinishUnroll) {
-                double2 v[kFinishUnroll];
-#pragma unroll
-                for (int i = 0; i < kFinishUnroll; ++i) v[i] = k0 + 32 * i < end ? __ldcg(p + k0 + 32 * i) : make_double2(0, 0);
-#pragma unroll
-                for (int i = 0; i < kFinishUnroll; ++i) { S += v[i].x; C += v[i].y; }
-            }
-        } else {
-            const float4 *p = reinterpret_cast<const float4 *>(part_f);
-            for (int k0 = beg + lane; k0 < end; k0 += 32 * kFinishUnroll) {
-                float4 v[kFinishUnroll];
-#pragma unroll
-                for (int i = 0; i < kFinishUnroll; ++i) v[i] = k0 + 32 * i < end ? __ldcg(p + k0 + 32 * i) : make_float4(0, 0, 0, 0);
-#pragma unroll
-                for (int i = 0; i < kFinishUnroll; ++i) {
-                    S += (double)v[i].x + (double)v[i].y;
-                    C += (double)v[i].z + (double)v[i].w;
-                }
-            }
-        }
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            S += __shfl_xor_sync(AI_FULL_MASK, S, d);
-            C += __shfl_xor_sync(AI_FULL_MASK, C, d);
-        }
-        if (lane == 0) write_bin(0, S, C, empty, intensity, sum_signal, count);
-    }
+    finish_bins<ACC>(part_f, 0, beg, end, false, 0, 0, 0, lane, empty, intensity, sum_signal, count);
 }
 
 // value of the pixel whose position in the tile buffer is stored as a byte offset
