@@ -132,6 +132,18 @@ int ai_integrate1d_host(ai_ctx *ctx, const void *image_host, ai_dtype dtype, con
                         const float *solidangle, const float *polarization, const uint8_t *mask,
                         float *intensity_host, float *sum_signal_host, float *count_host, void *cuda_stream);
 
+/* A stream of frames that live in HOST memory (the transfer is more than
+ * half of the paper's per-frame time): like ai_integrate1d_host for each of the `nframes` frames, with the upload of
+ * frame k+1 overlapping the kernels and downloads of frame k (two device staging buffers, a library-owned copy stream).
+ *   frames_host         HOST pointer (pinned memory for the overlap to happen), frame k at k * frame_stride_elems elements
+ *   dark ... mask       DEVICE pointers or NULL, shared by all frames
+ *   *_host outputs      HOST pointers, [nframes][npt] row-major
+ * Synchronises `cuda_stream` before returning.  Errors as ai_integrate1d. */
+int ai_integrate1d_host_frames(ai_ctx *ctx, const void *frames_host, ai_dtype dtype, int nframes,
+                               int64_t frame_stride_elems, const float *dark, const float *flat,
+                               const float *solidangle, const float *polarization, const uint8_t *mask,
+                               float *intensity_host, float *sum_signal_host, float *count_host, void *cuda_stream);
+
 /* Sizes of the TILED execution layout, for byte accounting in benchmarks.  info (HOST pointer)
  * receives 8 values: {tile height in rows, number of tiles, number of (tile, bin) segments, padded number of entries,
  * total bytes of the sliced matrix (all blobs), largest blob in bytes, partial records per frame, (tile + blob) stages

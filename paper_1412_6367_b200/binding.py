@@ -21,7 +21,7 @@ AI_ACC_F32_KAHAN, AI_ACC_F32_PLAIN, AI_ACC_F64 = range(3)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["ai_setup", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
-           "ai_integrate1d_host", "ai_get_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
+           "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_get_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
 class ai_geometry(C.Structure):
@@ -56,6 +56,7 @@ def lib():
     L.ai_integrate1d.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
     L.ai_integrate1d_batch.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_integrate1d_host.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, vp]
+    L.ai_integrate1d_host_frames.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_get_layout_info.argtypes = [vp, C.POINTER(C.c_int64)]
     L.ai_last_launch_count.argtypes = [vp]
     L.ai_profile_enable.argtypes = [vp, C.c_int]
@@ -158,6 +159,14 @@ def ai_integrate1d_host(ctx, image_host, dark, flat, solidangle, polarization, m
                                      _ptr(dark), _ptr(flat), _ptr(solidangle), _ptr(polarization), _ptr(mask),
                                      _ptr(intensity_host), _ptr(sum_signal_host), _ptr(count_host), _stream(stream)),
            ctx)
+
+
+def ai_integrate1d_host_frames(ctx, frames_host, nframes, frame_stride_elems, dark, flat, solidangle, polarization,
+                               mask, intensity_host, sum_signal_host, count_host, stream=None, dtype=None):
+    _check(lib().ai_integrate1d_host_frames(ctx, _ptr(frames_host), dtype_code(frames_host) if dtype is None else dtype,
+                                            nframes, frame_stride_elems, _ptr(dark), _ptr(flat), _ptr(solidangle),
+                                            _ptr(polarization), _ptr(mask), _ptr(intensity_host),
+                                            _ptr(sum_signal_host), _ptr(count_host), _stream(stream)), ctx)
 
 
 def ai_get_layout_info(ctx) -> dict:

@@ -104,6 +104,8 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
     }
     const char *e = getenv("AZINT_NO_TMA");
     ctx->no_tma = e && e[0] == '1';
+    e = getenv("AZINT_NO_PREPASS");
+    ctx->no_prepass = e && e[0] == '1';
     e = getenv("AZINT_NO_STREAM");
     ctx->no_stream = e && e[0] == '1';
     if ((e = getenv("AZINT_TUNE")) != nullptr) {        // experiments only: "th:32,ms:6,is:8,bms:2,bis:8,fl:2"
@@ -256,9 +258,71 @@ int ai_integrate1d_host(ai_ctx *ctx, const void *image_host, ai_dtype dtype, con
     return AI_OK;
 }
 
+int ai_integrate1d_host_frames(ai_ctx *ctx, const void *frames_host, ai_dtype dtype, int nframes,
+                               int64_t frame_stride_elems, const float *dark, const float *flat,
+                               const float *solidangle, const float *polarization, const uint8_t *mask,
+                               float *intensity_host, float *sum_signal_host, float *count_host, void *cuda_stream)
+{
+    if (!ctx) return AI_EINVAL;
+    if (!ctx->built) return ai_fail(ctx, AI_ENOTBUILT, "ai_build_csr has not been called");
+    if (!frames_host || !intensity_host || !sum_signal_host || !count_host) return ai_fail(ctx, AI_EINVAL, "NULL frames or output");
+    if ((int)dtype < AI_F32 || (int)dtype > AI_U32) return ai_fail(ctx, AI_EINVAL, "bad dtype %d", (int)dtype);
+    if (nframes < 1) return ai_fail(ctx, AI_EINVAL, "nframes < 1");
+    const int64_t npix = (int64_t)ctx->height * ctx->width;
+    if (frame_stride_elems < npix) return ai_fail(ctx, AI_EINVAL, "frame stride < height*width");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t esz = (dtype == AI_U16 || dtype == AI_I16) ? 2 : 4;
+    const size_t bytes = (size_t)npix * esz, nb = (size_t)ctx->npt * sizeof(float);
+    if (!ctx->copy_stream) {
+        AI_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            AI_CUDA(ctx, cudaEventCreateWithFlags(&ctx->h2d_done[i], cudaEventDisableTiming));
+            AI_CUDA(ctx, cudaEventCreateWithFlags(&ctx->slot_free[i], cudaEventDisableTiming));
+            AI_CUDA(ctx, cudaMalloc(&ctx->out2[i], 3 * nb));
+        }
+    }
+    if (ctx->stage2_bytes < bytes) {
+        for (int i = 0; i < 2; ++i) {
+            if (ctx->stage2[i]) AI_CUDA(ctx, cudaFree(ctx->stage2[i]));
+            ctx->stage2[i] = nullptr;
+        }
+        ctx->stage2_bytes = 0;
+        for (int i = 0; i < 2; ++i) AI_CUDA(ctx, cudaMalloc(&ctx->stage2[i], bytes));
+        ctx->stage2_bytes = bytes;
+    }
+    // uploads must not overtake work already queued on the caller's stream that may still use the staging buffers
+    AI_CUDA(ctx, cudaEventRecord(ctx->slot_free[0], st));
+    AI_CUDA(ctx, cudaEventRecord(ctx->slot_free[1], st));
+    for (int k = 0; k < nframes; ++k) {
+        const int slot = k & 1;
+        const char *src = static_cast<const char *>(frames_host) + (size_t)k * frame_stride_elems * esz;
+        AI_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->slot_free[slot], 0));
+        AI_CUDA(ctx, cudaMemcpyAsync(ctx->stage2[slot], src, bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+        AI_CUDA(ctx, cudaEventRecord(ctx->h2d_done[slot], ctx->copy_stream));
+        AI_CUDA(ctx, cudaStreamWaitEvent(st, ctx->h2d_done[slot], 0));
+        float *o = ctx->out2[slot];
+        FrameArgs a{ctx->stage2[slot], dtype, dark, flat, solidangle, polarization, mask, nullptr, o, o + ctx->npt,
+                    o + 2 * ctx->npt, 1, npix};
+        int rc = integrate(ctx, a, st);
+        if (rc != AI_OK) return rc;
+        AI_CUDA(ctx, cudaEventRecord(ctx->slot_free[slot], st));
+        AI_CUDA(ctx, cudaMemcpyAsync(intensity_host + (size_t)k * ctx->npt, o, nb, cudaMemcpyDeviceToHost, st));
+        AI_CUDA(ctx, cudaMemcpyAsync(sum_signal_host + (size_t)k * ctx->npt, o + ctx->npt, nb, cudaMemcpyDeviceToHost, st));
+        AI_CUDA(ctx, cudaMemcpyAsync(count_host + (size_t)k * ctx->npt, o + 2 * ctx->npt, nb, cudaMemcpyDeviceToHost, st));
+    }
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    return AI_OK;
+}
+
 void ai_destroy(ai_ctx *ctx)
 {
     if (!ctx) return;
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(ctx->stage2[i]); cudaFree(ctx->out2[i]);
+        if (ctx->h2d_done[i]) cudaEventDestroy(ctx->h2d_done[i]);
+        if (ctx->slot_free[i]) cudaEventDestroy(ctx->slot_free[i]);
+    }
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     cudaFree(ctx->indptr); cudaFree(ctx->indices); cudaFree(ctx->data); cudaFree(ctx->row_csum); cudaFree(ctx->d_range);
     cudaFree(ctx->lut_coef); cudaFree(ctx->lut_idx);
     TiledLayout &tl = ctx->tl;
@@ -266,7 +330,7 @@ void ai_destroy(ai_ctx *ctx)
     cudaFree(tl.tile_desc); cudaFree(tl.tile_order); cudaFree(tl.blob); cudaFree(tl.blob_desc);
     cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
     free(tl.h_first_desc);
-    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync);
+    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->corrected);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;

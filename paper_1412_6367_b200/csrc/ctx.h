@@ -144,11 +144,19 @@ struct ai_ctx {
     void *staging = nullptr;        // device copy of a host frame (ai_integrate1d_host)
     size_t staging_bytes = 0;
     float *out_dev = nullptr;       // [3*npt] device outputs of ai_integrate1d_host
+    // ai_integrate1d_host_frames: double-buffered upload
+    void *stage2[2] = {nullptr, nullptr};
+    size_t stage2_bytes = 0;
+    float *out2[2] = {nullptr, nullptr};
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t h2d_done[2] = {nullptr, nullptr}, slot_free[2] = {nullptr, nullptr};
+    float *corrected = nullptr;     // [height*width] corrected float32 frame (integrate_prep.cu), allocated on first use
     unsigned long long *grid_sync = nullptr;   // arrival counter of the fused single-frame kernel's grid barrier
 
     // measurement hook (ai_profile_enable): events around the dominant kernel of the last call
     PipeTune tune;
     bool no_tma = false;            // AZINT_NO_TMA=1: stage raw frames through registers even where TMA applies (testing)
+    bool no_prepass = false;        // AZINT_NO_PREPASS=1: corrected single frames take the general kernel (testing)
     bool no_stream = false;         // AZINT_NO_STREAM=1: single frames take the general pipelined kernel too (testing)
     bool profile = false, profile_valid = false;
     bool stage1_only = false;       // ai_profile_enable(ctx, 2): launch only the dominant kernel
@@ -197,4 +205,5 @@ struct FrameArgs {
 int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_csr(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_lut(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
+int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st);   // integrate_prep.cu
 int ai_stream_stages(const ai_ctx *ctx);      // integrate_stream.cu: (tile + blob) stages of the single-frame kernel, 0 = n/a

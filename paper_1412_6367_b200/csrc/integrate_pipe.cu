@@ -8,7 +8,7 @@
 //                                 (cp.async.bulk.tensor, SASS UTMALDG) into a ring of tile buffers, then the tile's
 //                                 blob of the matrix as one bulk copy (cp.async.bulk, SASS UBLKCP) into a ring of
 //                                 matrix stages.  No registers are held by data in flight.
-//   stagers   (kStageWarps warps) TMA mode (32-bit pixels, no correction arrays, aligned rows): turn the raw tile into
+//   stagers   (kStageGroups groups of kStageGroupWarps warps, alternate tiles) TMA mode (32-bit pixels, no correction arrays, aligned rows): turn the raw tile into
 //                                 float32 in place and look for non-finite pixels.  Otherwise: load the tile and the
 //                                 correction arrays with 128-bit loads, cast, correct and mask in registers
 //                                  and park the result in the tile buffer.
@@ -27,7 +27,10 @@
 
 namespace {
 
-constexpr int kStageWarps = 3;
+constexpr int kStageGroups = 1;                      // stager groups work on alternate tile images (two groups keep the
+constexpr int kStageGroupWarps = 3;                  // loads of two tiles in flight, but 23 warps cap the kernel at 80
+                                                     // registers and slow the consumers down: measured, one group kept)
+constexpr int kStageWarps = kStageGroups * kStageGroupWarps;
 constexpr int kConsWarps = 16;
 constexpr int kPipeThreads = 32 * (1 + kStageWarps + kConsWarps);
 static_assert((kConsWarps & (kConsWarps - 1)) == 0, "block dealing assumes a power of two");
@@ -236,7 +239,7 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
         }
         for (int s = 0; s < kPipeMaxImgStages; ++s) {
             mbar_init(raw_full + s, 1);
-            mbar_init(img_ready + s, kStageWarps);
+            mbar_init(img_ready + s, kStageGroupWarps);
             mbar_init(img_empty + s, kConsWarps);
             img_flag[s] = 0;
         }
@@ -312,7 +315,8 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
         }
 #endif
         if (direct) return;
-        const int sw = warp - 1, tid = sw * 32 + lane;
+        const int sw = warp - 1, group = sw / kStageGroupWarps, tid = (sw % kStageGroupWarps) * 32 + lane;
+        constexpr int kGroupThreads = kStageGroupWarps * 32;
         int ii = 0;
         for (int n = 0;; ++n) {
             const int w = item_at(n);
@@ -324,17 +328,21 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
             const int f1 = min(p.nframes, f0 + p.frames_per_item);
             const int ty = d.z >> 16, tx = d.z & 0xffff;
             for (int f = f0; f < f1; ++f, ++ii) {
+                if (ii % kStageGroups != group) {        // the other group's image
+                    ir.next(p.img_stages);
+                    continue;
+                }
                 float *tile = reinterpret_cast<float *>(img_base + (size_t)ir.stage * p.img_stage_bytes);
                 bool bad;
                 if (p.use_tma) {
                     if (tid == 0) AI_TRACE(ii, 5);
                     mbar_wait(raw_full + ir.stage, ir.parity);
                     if (tid == 0) AI_TRACE(ii, 6);
-                    bad = convert_tile_in_place<DT>(tile, p.tile_h * (kTileW / 4), tid, kStageWarps * 32);
+                    bad = convert_tile_in_place<DT>(tile, p.tile_h * (kTileW / 4), tid, kGroupThreads);
                     fence_proxy_async();               // generic-proxy writes before the next TMA write to the stage
                 } else {
                     const void *img = reinterpret_cast<const T *>(p.frames) + (int64_t)f * p.frame_stride;
-                    bad = stage_tile<DT, kStageWarps * 32, 8, 3>(tile, img, p.cor, ty, tx, p.tile_h, p.height, p.width,
+                    bad = stage_tile<DT, kGroupThreads, 8, 3>(tile, img, p.cor, ty, tx, p.tile_h, p.height, p.width,
                                                                   p.vec_ok, tid,
                                                                   [&] { mbar_wait(img_empty + ir.stage, ir.parity ^ 1u); });
                 }

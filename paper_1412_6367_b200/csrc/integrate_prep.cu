@@ -1,0 +1,77 @@
+// H1 + H2 as a streaming pre-pass for single frames that carry correction arrays, a mask or 16-bit pixels:
+// cast, dark, flat, solid angle, polarisation in one pass over the pixels, invalid pixels
+// (masked, zero / non-finite denominator, non-finite value: DESIGN.md reading 8) written as NaN.  The result is a
+// float32 image owned by the context that the single-frame kernel (integrate_stream.cu) consumes right away -- 16.8 MB
+// for a 2048 x 2048 frame, normally still in L2 when it is read back.  Chosen by measurement over staging the
+// corrections inside the gather kernel.
+#include "common.cuh"
+
+namespace {
+
+constexpr int kPrepThreads = 256;
+
+template <int DT>
+__global__ void __launch_bounds__(kPrepThreads) correct_frame_kernel(const void *__restrict__ img, Corrections cor,
+                                                                     int64_t npix, int vec_ok, float *__restrict__ out)
+{
+    // the single-frame kernel that follows may start its prologue (it reads `out` after its griddepcontrol.wait)
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const bool has_den = cor.flat || cor.solidangle || cor.polarization;
+    const int64_t stride = (int64_t)gridDim.x * kPrepThreads;
+    if (vec_ok) {
+        const float4 one4 = make_float4(1, 1, 1, 1), zero4 = make_float4(0, 0, 0, 0);
+        for (int64_t q = (int64_t)blockIdx.x * kPrepThreads + threadIdx.x; q < npix / 4; q += stride) {
+            const int64_t p = q * 4;
+            const float4 raw = load_raw4<DT>(img, p);
+            const float4 dk = cor.dark ? __ldg(reinterpret_cast<const float4 *>(cor.dark + p)) : zero4;
+            const float4 fl = cor.flat ? __ldg(reinterpret_cast<const float4 *>(cor.flat + p)) : one4;
+            const float4 sa = cor.solidangle ? __ldg(reinterpret_cast<const float4 *>(cor.solidangle + p)) : one4;
+            const float4 po = cor.polarization ? __ldg(reinterpret_cast<const float4 *>(cor.polarization + p)) : one4;
+            const uchar4 mk = cor.mask ? __ldg(reinterpret_cast<const uchar4 *>(cor.mask + p)) : make_uchar4(0, 0, 0, 0);
+            float4 v;
+            v.x = correct_value(raw.x, dk.x, fl.x, sa.x, po.x, mk.x != 0, has_den);
+            v.y = correct_value(raw.y, dk.y, fl.y, sa.y, po.y, mk.y != 0, has_den);
+            v.z = correct_value(raw.z, dk.z, fl.z, sa.z, po.z, mk.z != 0, has_den);
+            v.w = correct_value(raw.w, dk.w, fl.w, sa.w, po.w, mk.w != 0, has_den);
+            *reinterpret_cast<float4 *>(out + p) = v;
+        }
+    } else {
+        for (int64_t p = (int64_t)blockIdx.x * kPrepThreads + threadIdx.x; p < npix; p += stride)
+            out[p] = corrected_pixel<DT>(img, p, cor);
+    }
+}
+
+}  // namespace
+
+// Writes the corrected float32 image of frame 0 of `a` into ctx->corrected (allocated on first use).
+int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st)
+{
+    const int64_t npix = (int64_t)ctx->height * ctx->width;
+    if (!ctx->corrected) AI_CUDA(ctx, cudaMalloc(&ctx->corrected, (size_t)npix * sizeof(float)));
+    Corrections cor{a.dark, a.flat, a.solidangle, a.polarization, a.mask};
+    const int vec = vec_ok && npix % 4 == 0;
+    const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
+    int64_t blocks = ((vec ? npix / 4 : npix) + kPrepThreads - 1) / kPrepThreads;
+    if (blocks > (int64_t)sms * 8) blocks = (int64_t)sms * 8;        // grid-stride: 8 resident blocks per SM
+    if (blocks < 1) blocks = 1;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)blocks);
+    cfg.blockDim = dim3(kPrepThreads);
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+#define AI_PREP(DT) AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, correct_frame_kernel<DT>, a.image, cor, npix, vec, ctx->corrected))
+    switch (a.dtype) {
+    case AI_F32: AI_PREP(AI_F32); break;
+    case AI_I32: AI_PREP(AI_I32); break;
+    case AI_U16: AI_PREP(AI_U16); break;
+    case AI_I16: AI_PREP(AI_I16); break;
+    case AI_U32: AI_PREP(AI_U32); break;
+    }
+#undef AI_PREP
+    return AI_OK;
+}

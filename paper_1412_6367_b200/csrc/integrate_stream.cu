@@ -36,6 +36,7 @@ struct StreamParams {
     int stages, mat_stage_bytes, img_stage_bytes, hdr_bytes, items_max;
     int prefetch_tiles;          // tiles per block whose data is pulled into L2 before the grid dependency resolves
     int launch_index;            // launches of this context so far, modulo 8 (development trace only)
+    int track_all;               // float frames: every block skips non-finite pixels and accumulates count
     void *partials;
     // H5 fused behind a grid-wide barrier (every block is resident: one per SM, grid <= number of SMs)
     unsigned long long *grid_sync;     // arrivals of all launches of this context, never reset
@@ -159,7 +160,8 @@ __device__ __noinline__ bool stream_block(unsigned rebase, const unsigned char *
     return false;
 }
 
-// the same block with non-finite pixels skipped and count accumulated (float frames only; rare, kept simple)
+// the same block with non-finite pixels skipped and count accumulated (float frames: the pre-pass marks invalid
+// pixels with NaN, raw frames may carry NaN / Inf); same two-steps-per-trip pipeline
 template <int ACC>
 __device__ __noinline__ void stream_block_tracked(unsigned rebase, const unsigned char *blob, unsigned h, void *part_f,
                                                   int lane)
@@ -170,11 +172,16 @@ __device__ __noinline__ void stream_block_tracked(unsigned rebase, const unsigne
     const uint2 *xp = reinterpret_cast<const uint2 *>(blk + nsteps * 512) + lane;
     const int2 m = reinterpret_cast<const int2 *>(blk + nsteps * kBlkStepBytes)[lane];
     AccumQ<ACC> S2, C2;
+    float4 c0 = cp[0], c1 = cp[32];
+    uint2 x0 = xp[0], x1 = xp[32];
 #pragma unroll 1
-    for (int j = 0; j < nsteps; ++j) {
-        const float4 c = cp[j * 32];
-        const float4 v = stream_gather4<AI_F32>(xp[j * 32], rebase);
-        accumulate4<ACC, true>(c, v, S2, C2);
+    for (int j = 2; j <= nsteps; j += 2) {
+        const float4 n0 = cp[j * 32], n1 = cp[j * 32 + 32];
+        const uint2 y0 = xp[j * 32], y1 = xp[j * 32 + 32];
+        const float4 v0 = stream_gather4<AI_F32>(x0, rebase), v1 = stream_gather4<AI_F32>(x1, rebase);
+        accumulate4<ACC, true>(c0, v0, S2, C2);
+        accumulate4<ACC, true>(c1, v1, S2, C2);
+        c0 = n0; c1 = n1; x0 = y0; x1 = y1;
     }
     Accum<ACC> S = S2.total(), C = C2.total();
     stream_finish_block<ACC, true>(S, C, m, rounds, part_f);
@@ -309,8 +316,12 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
                 const unsigned rebase = (smem_u32(img_base + (size_t)r.stage * p.img_stage_bytes) & 0xffffu) * 0x10001u;
                 for (int b = firstb; b < d.w; b += kStreamCons) {
                     const unsigned h = bh[b];
-                    if (stream_block<DT, ACC>(rebase, blob, h, p.partials, lane)) {
-                        if constexpr (DT == AI_F32) stream_block_tracked<ACC>(rebase, blob, h, p.partials, lane);
+                    if constexpr (DT == AI_F32) {
+                        // track_all: the frame comes from the correction pre-pass and is expected to hold NaN marks
+                        if (p.track_all || stream_block<DT, ACC>(rebase, blob, h, p.partials, lane))
+                            stream_block_tracked<ACC>(rebase, blob, h, p.partials, lane);
+                    } else {
+                        stream_block<DT, ACC>(rebase, blob, h, p.partials, lane);
                     }
                 }
                 __syncwarp();
@@ -458,7 +469,7 @@ int ai_stream_stages(const ai_ctx *ctx)
 // Launches the single-frame fast path when it applies (*handled = true): one frame of 32-bit pixels, no correction
 // arrays, rows on 16-byte boundaries, and at least two (tile + blob) stages fitting the shared memory of an SM.
 // The kernel is the whole hot path of the frame: stage 1 and, behind a grid barrier, H5 (no second launch).
-int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled)
+int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int track_all, cudaStream_t st, bool *handled)
 {
     const TiledLayout &tl = ctx->tl;
     *handled = false;
@@ -481,6 +492,7 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStr
     p.nslot = tl.nslot;
     p.partials = ctx->partials;
     p.prefetch_tiles = ctx->tune.prefetch_tiles;
+    p.track_all = track_all;
     static unsigned launches = 0;                  // development trace only: which of 8 trace buffers the launch writes
     p.launch_index = launches++ & 7;
     p.grid_sync = ctx->grid_sync;

@@ -15,7 +15,7 @@
 #include "tiled_common.cuh"
 
 int ai_launch_pipe_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);
-int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);
+int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int track_all, cudaStream_t st, bool *handled);
 
 namespace {
 
@@ -212,11 +212,30 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
     bool handled = false;
     int rc = AI_OK;
     if (ctx->layout != AI_LAYOUT_TILED_DIRECT) {
-        rc = ai_launch_stream_stage1(ctx, a, vec_ok, st, &handled);           // one plain 32-bit frame: whole hot path
+        rc = ai_launch_stream_stage1(ctx, a, vec_ok, 0, st, &handled);        // one plain 32-bit frame: whole hot path
         if (rc != AI_OK) return rc;
         if (handled) {
             ctx->last_launches = 1;
             return AI_OK;
+        }
+        // one frame with correction arrays, a mask, 16-bit pixels or unaligned buffers: H1 + H2 as a streaming
+        // pre-pass into a float32 frame (invalid pixels as NaN), then the same single-frame kernel
+        if (a.nframes == 1 && !ctx->no_prepass && !ctx->no_stream && !ctx->no_tma && ctx->width % 4 == 0 &&
+            ai_stream_stages(ctx) >= 2) {
+            rc = ai_launch_correct(ctx, a, vec_ok, st);
+            if (rc != AI_OK) return rc;
+            FrameArgs b = a;
+            b.image = ctx->corrected;
+            b.dtype = AI_F32;
+            b.dark = b.flat = b.solidangle = b.polarization = nullptr;
+            b.mask = nullptr;
+            const int may_be_invalid = a.dark || a.flat || a.solidangle || a.polarization || a.mask || a.dtype == AI_F32;
+            rc = ai_launch_stream_stage1(ctx, b, 1, may_be_invalid, st, &handled);
+            if (rc != AI_OK) return rc;
+            if (handled) {
+                ctx->last_launches = 2;
+                return AI_OK;
+            }
         }
         rc = ai_launch_pipe_stage1(ctx, a, vec_ok, st, &handled);
     }

@@ -311,6 +311,42 @@ def test_single_frame_kernels(torch, B, oracle, workloads, monkeypatch, path, dt
     integ.close()
 
 
+@pytest.mark.parametrize("path", ["prepass", "pipe"])
+@pytest.mark.parametrize("dtype", ["float32", "uint16", "int32"])
+@pytest.mark.parametrize("shape", [(256, 256), (130, 200)])
+def test_corrected_frame_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, shape):
+    """One frame with every correction array and a mask: by default H1 + H2 run as a pre-pass and the single-frame
+    kernel consumes the corrected frame; AZINT_NO_PREPASS=1 stages the corrections inside the general kernel."""
+    if path == "pipe":
+        monkeypatch.setenv("AZINT_NO_PREPASS", "1")
+    h, w = shape
+    cfg = workloads.tiny_config(h, w, center_x=w * 0.3, center_y=h * 0.6, unit=workloads.TTH_DEG, npt=211,
+                                distance_m=0.03, name=f"corr_{h}x{w}")
+    rng = np.random.default_rng(h + 7 * w)
+    img = rng.poisson(300.0, size=(h, w)).astype(dtype)
+    fr = workloads.Frame(image=img, dark=rng.poisson(5.0, size=(h, w)).astype(np.float32),
+                         flat=rng.uniform(0.9, 1.1, size=(h, w)).astype(np.float32),
+                         solidangle=rng.uniform(0.7, 1.0, size=(h, w)).astype(np.float32),
+                         polarization=rng.uniform(0.95, 1.0, size=(h, w)).astype(np.float32),
+                         mask=(rng.random(size=(h, w)) < 0.05).astype(np.uint8))
+    fr.flat[3, 5] = 0.0                      # zero denominator: invalid pixel
+    integ = B.Integrator(cfg, empty_value=-2.0)
+    args = [_dev(torch, x) for x in (fr.dark, fr.flat, fr.solidangle, fr.polarization, fr.mask)]
+    if dtype == "uint16":
+        t, code = torch.from_numpy(img.view(np.int16)).cuda(), B.AI_U16
+    else:
+        t, code = torch.from_numpy(img).cuda(), None
+    for acc in ("kahan", "f64"):
+        integ.set_options(LAYOUTS["tiled"], ACCUMS[acc], -2.0)
+        i, s, c = integ.outputs()
+        B.ai_integrate1d(integ.ctx, t, *args, None, i, s, c, dtype=code)
+        torch.cuda.synchronize()
+        got = {"intensity": i.cpu().numpy(), "sum_signal": s.cpu().numpy(), "count": c.cpu().numpy()}
+        assert_profile(got, _oracle_profile(oracle, cfg, fr, empty=-2.0), what=f"{path}/{dtype}/{shape}/{acc}")
+    assert B.ai_last_launch_count(integ.ctx) == 2
+    integ.close()
+
+
 @pytest.mark.parametrize("path", ["stream", "pipe"])
 def test_non_finite_pixels_in_plain_float_frames(torch, B, oracle, workloads, monkeypatch, path):
     """No mask, no corrections: NaN / Inf pixels are found lazily (a non-finite lane sum repeats the block with the
@@ -383,6 +419,22 @@ def test_host_entry_point(torch, B, oracle, workloads):
     got = {"intensity": out[0].numpy(), "sum_signal": out[1].numpy(), "count": out[2].numpy()}
     assert_profile(got, _oracle_profile(oracle, cfg, fr), what="host entry")
     assert B.ai_last_launch_count(integ.ctx) >= 1
+    integ.close()
+
+
+def test_host_frames_entry_point(torch, B, oracle, workloads):
+    """ai_integrate1d_host_frames: pinned host frames in, host profiles out, uploads overlapping the kernels."""
+    cfg = workloads.CONFIGS["cfg1b"]
+    frames = np.stack([workloads.make_frame(cfg, frame_index=k).image for k in range(5)])
+    pinned = torch.from_numpy(frames).pin_memory()
+    outs = [torch.empty((5, cfg.npt), dtype=torch.float32).pin_memory() for _ in range(3)]
+    integ = B.Integrator(cfg)
+    for _ in range(2):       # second call reuses the staging buffers
+        B.ai_integrate1d_host_frames(integ.ctx, pinned.numpy(), 5, cfg.npix, None, None, None, None, None,
+                                     *[o.numpy() for o in outs])
+    for k in range(5):
+        got = {"intensity": outs[0][k].numpy(), "sum_signal": outs[1][k].numpy(), "count": outs[2][k].numpy()}
+        assert_profile(got, _oracle_profile(oracle, cfg, workloads.Frame(image=frames[k])), what=f"host frame {k}")
     integ.close()
 
 
