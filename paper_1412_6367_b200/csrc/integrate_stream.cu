@@ -92,20 +92,26 @@ __device__ __forceinline__ int lds_s32(unsigned addr)
     return v;
 }
 
-// pixel values of the four entries of one step; x holds four 16-bit byte offsets into the tile, rebase = low half-word
-// of the tile's shared address in both halves
-template <int DT>
-__device__ __forceinline__ float4 stream_gather4(const uint2 &x, unsigned rebase)
+// pixel values of the four entries of one step; x holds four 16-bit byte offsets into the tile.  PACKED: `base` = low
+// half-word of the tile's shared address in both halves (tile buffers inside the first 64 KB of the shared window: one
+// add rebases two positions); otherwise `base` = the tile's shared address.
+template <int DT, bool PACKED = true>
+__device__ __forceinline__ float4 stream_gather4(const uint2 &x, unsigned base)
 {
-    const unsigned p0 = x.x + rebase, p1 = x.y + rebase;
-    if constexpr (DT == AI_F32) {
-        return make_float4(lds_f32(p0 & 0xffffu), lds_f32(p0 >> 16), lds_f32(p1 & 0xffffu), lds_f32(p1 >> 16));
-    } else if constexpr (DT == AI_I32) {
-        return make_float4((float)lds_s32(p0 & 0xffffu), (float)lds_s32(p0 >> 16), (float)lds_s32(p1 & 0xffffu),
-                           (float)lds_s32(p1 >> 16));
+    unsigned a0, a1, a2, a3;
+    if constexpr (PACKED) {
+        const unsigned p0 = x.x + base, p1 = x.y + base;
+        a0 = p0 & 0xffffu; a1 = p0 >> 16; a2 = p1 & 0xffffu; a3 = p1 >> 16;
     } else {
-        return make_float4((float)(unsigned)lds_s32(p0 & 0xffffu), (float)(unsigned)lds_s32(p0 >> 16),
-                           (float)(unsigned)lds_s32(p1 & 0xffffu), (float)(unsigned)lds_s32(p1 >> 16));
+        a0 = base + (x.x & 0xffffu); a1 = base + (x.x >> 16); a2 = base + (x.y & 0xffffu); a3 = base + (x.y >> 16);
+    }
+    if constexpr (DT == AI_F32) {
+        return make_float4(lds_f32(a0), lds_f32(a1), lds_f32(a2), lds_f32(a3));
+    } else if constexpr (DT == AI_I32) {
+        return make_float4((float)lds_s32(a0), (float)lds_s32(a1), (float)lds_s32(a2), (float)lds_s32(a3));
+    } else {
+        return make_float4((float)(unsigned)lds_s32(a0), (float)(unsigned)lds_s32(a1), (float)(unsigned)lds_s32(a2),
+                           (float)(unsigned)lds_s32(a3));
     }
 }
 
@@ -132,7 +138,7 @@ __device__ __forceinline__ void stream_finish_block(Accum<ACC> &S, Accum<ACC> &C
 // stage has slack behind the blob, so the look-ahead needs no predicate.  Float frames are not screened: a
 // non-finite lane sum anywhere in the warp means a non-finite pixel may have been gathered; nothing is stored and
 // true is returned (the caller repeats the block with stream_block_tracked).
-template <int DT, int ACC>
+template <int DT, int ACC, bool PACKED = true>
 __device__ __noinline__ bool stream_block(unsigned rebase, const unsigned char *blob, unsigned h, void *part_f, int lane)
 {
     const int nsteps = h & 15, rounds = (h >> 4) & 7;
@@ -147,7 +153,7 @@ __device__ __noinline__ bool stream_block(unsigned rebase, const unsigned char *
     for (int j = 2; j <= nsteps; j += 2) {
         const float4 n0 = cp[j * 32], n1 = cp[j * 32 + 32];
         const uint2 y0 = xp[j * 32], y1 = xp[j * 32 + 32];
-        const float4 v0 = stream_gather4<DT>(x0, rebase), v1 = stream_gather4<DT>(x1, rebase);
+        const float4 v0 = stream_gather4<DT, PACKED>(x0, rebase), v1 = stream_gather4<DT, PACKED>(x1, rebase);
         accumulate4<ACC, false>(c0, v0, S2, C2);
         accumulate4<ACC, false>(c1, v1, S2, C2);
         c0 = n0; c1 = n1; x0 = y0; x1 = y1;
@@ -162,7 +168,7 @@ __device__ __noinline__ bool stream_block(unsigned rebase, const unsigned char *
 
 // the same block with non-finite pixels skipped and count accumulated (float frames: the pre-pass marks invalid
 // pixels with NaN, raw frames may carry NaN / Inf); same two-steps-per-trip pipeline
-template <int ACC>
+template <int ACC, bool PACKED = true>
 __device__ __noinline__ void stream_block_tracked(unsigned rebase, const unsigned char *blob, unsigned h, void *part_f,
                                                   int lane)
 {
@@ -178,13 +184,50 @@ __device__ __noinline__ void stream_block_tracked(unsigned rebase, const unsigne
     for (int j = 2; j <= nsteps; j += 2) {
         const float4 n0 = cp[j * 32], n1 = cp[j * 32 + 32];
         const uint2 y0 = xp[j * 32], y1 = xp[j * 32 + 32];
-        const float4 v0 = stream_gather4<AI_F32>(x0, rebase), v1 = stream_gather4<AI_F32>(x1, rebase);
+        const float4 v0 = stream_gather4<AI_F32, PACKED>(x0, rebase), v1 = stream_gather4<AI_F32, PACKED>(x1, rebase);
         accumulate4<ACC, true>(c0, v0, S2, C2);
         accumulate4<ACC, true>(c1, v1, S2, C2);
         c0 = n0; c1 = n1; x0 = y0; x1 = y1;
     }
     Accum<ACC> S = S2.total(), C = C2.total();
     stream_finish_block<ACC, true>(S, C, m, rounds, part_f);
+}
+
+// Batches (H6): the same block against the tiles of TWO frames at once.  Coefficients and positions are loaded and
+// unpacked once and serve both frames; the two sets of accumulators double the independent work per lane.  Returns
+// true (nothing stored) if a non-finite lane sum shows that either tile may hold a non-finite pixel.
+template <int DT, int ACC>
+__device__ __noinline__ bool stream_block2(unsigned tile_a, unsigned tile_b, const unsigned char *blob, unsigned h,
+                                           void *part_a, void *part_b, int lane)
+{
+    const int nsteps = h & 15, rounds = (h >> 4) & 7;
+    const unsigned char *blk = blob + (size_t)(h >> 8) * 16;
+    const float4 *cp = reinterpret_cast<const float4 *>(blk) + lane;
+    const uint2 *xp = reinterpret_cast<const uint2 *>(blk + nsteps * 512) + lane;
+    const int2 m = reinterpret_cast<const int2 *>(blk + nsteps * kBlkStepBytes)[lane];
+    AccumQ<ACC> SA, SB, C2;
+    float4 c0 = cp[0], c1 = cp[32];
+    uint2 x0 = xp[0], x1 = xp[32];
+#pragma unroll 1
+    for (int j = 2; j <= nsteps; j += 2) {
+        const float4 n0 = cp[j * 32], n1 = cp[j * 32 + 32];
+        const uint2 y0 = xp[j * 32], y1 = xp[j * 32 + 32];
+        const float4 a0 = stream_gather4<DT, false>(x0, tile_a), b0 = stream_gather4<DT, false>(x0, tile_b);
+        const float4 a1 = stream_gather4<DT, false>(x1, tile_a), b1 = stream_gather4<DT, false>(x1, tile_b);
+        accumulate4<ACC, false>(c0, a0, SA, C2);
+        accumulate4<ACC, false>(c0, b0, SB, C2);
+        accumulate4<ACC, false>(c1, a1, SA, C2);
+        accumulate4<ACC, false>(c1, b1, SB, C2);
+        c0 = n0; c1 = n1; x0 = y0; x1 = y1;
+    }
+    Accum<ACC> Sa = SA.total(), Sb = SB.total(), C = C2.total();
+    if constexpr (DT == AI_F32) {
+        if (__any_sync(AI_FULL_MASK, !finite_f((float)Sa.s) || !finite_f((float)Sb.s))) return true;
+    }
+    Accum<ACC> Ca = C;
+    stream_finish_block<ACC, false>(Sa, Ca, m, rounds, part_a);
+    stream_finish_block<ACC, false>(Sb, C, m, rounds, part_b);
+    return false;
 }
 
 template <int DT, int ACC>
@@ -393,6 +436,144 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
     AI_STRACE_AT(14, 0, strace_now());
 }
 
+// ---- batches (H6): tiled_bstream_kernel ---------------------------------------------------------------------------------
+// A work item = (tile, chunk of consecutive frames): the tile's blob is loaded ONCE into a matrix stage and serves
+// every frame of the chunk (the batched variant that amortises the matrix read across frames); the frames' tiles stream
+// through a ring of image stages and are consumed two frames at a time (stream_block2).  Writes one partial per run
+// and frame; tiled_stage2_kernel adds them up.
+constexpr int kBatchMaxImgStages = 8;
+constexpr int kBatchMaxMatStages = 2;
+
+struct BatchParams {
+    const int4 *blob_desc;
+    const unsigned char *blob;
+    int tile_h, ntiles, nslot;
+    int img_stages, mat_stages, img_stage_bytes, mat_stage_bytes, hdr_bytes;
+    int nframes, frames_per_item, nitems;
+    void *partials;
+};
+
+template <int DT, int ACC>
+__global__ void __launch_bounds__(kStreamThreads, 1) tiled_bstream_kernel(const __grid_constant__ CUtensorMap tmap,
+                                                                          const BatchParams p)
+{
+    // [image stages][barriers, item descriptors][matrix stages]
+    extern __shared__ __align__(1024) unsigned char smem[];
+    unsigned char *img_base = smem;
+    unsigned char *hdr = smem + (size_t)p.img_stages * p.img_stage_bytes;
+    uint64_t *img_full = reinterpret_cast<uint64_t *>(hdr);
+    uint64_t *img_empty = img_full + kBatchMaxImgStages;
+    uint64_t *mat_full = img_empty + kBatchMaxImgStages;
+    uint64_t *mat_empty = mat_full + kBatchMaxMatStages;
+    int4 *desc_s = reinterpret_cast<int4 *>(hdr + kStreamBarBytes);
+    unsigned char *mat_base = hdr + p.hdr_bytes;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    int nmine = 0;
+    while (stream_item_at(nmine) < p.nitems) ++nmine;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kBatchMaxImgStages; ++s) {
+            mbar_init(img_full + s, 1);
+            mbar_init(img_empty + s, kStreamCons);
+        }
+        for (int s = 0; s < kBatchMaxMatStages; ++s) {
+            mbar_init(mat_full + s, 1);
+            mbar_init(mat_empty + s, kStreamCons);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int k = threadIdx.x; k < nmine; k += kStreamThreads) {
+        const int w = stream_item_at(k);
+        int4 d = __ldg(p.blob_desc + w % p.ntiles);
+        d.x = d.w ? d.x : 0;
+        desc_s[k] = d;
+    }
+    asm volatile("griddepcontrol.launch_dependents;");       // stage 2 may be scheduled as SMs free up
+    __syncthreads();
+
+    Ring ir, mr;
+    if (warp == 0) {
+        // ===== producer: blob of the item, then the tiles of its frames ==================================================
+        int nblob = 0, nimg = 0;
+        for (int n = 0; n < nmine; ++n) {
+            const int4 d = desc_s[n];
+            if (d.w == 0) continue;
+            const int chunk = stream_item_at(n) / p.ntiles;
+            const int f0 = chunk * p.frames_per_item, f1 = min(p.nframes, f0 + p.frames_per_item);
+            const int ty = d.z >> 16, tx = d.z & 0xffff;
+            if (nblob >= p.mat_stages) mbar_wait(mat_empty + mr.stage, mr.parity ^ 1u);
+            if (lane == 0) {
+                mbar_arrive_expect_tx(mat_full + mr.stage, (uint32_t)d.y);
+                bulk_g2s(mat_base + (size_t)mr.stage * p.mat_stage_bytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y,
+                         mat_full + mr.stage);
+            }
+            ++nblob;
+            mr.next(p.mat_stages);
+            for (int f = f0; f < f1; ++f) {
+                if (nimg >= p.img_stages) mbar_wait(img_empty + ir.stage, ir.parity ^ 1u);
+                if (lane == 0) {
+                    unsigned char *tile = img_base + (size_t)ir.stage * p.img_stage_bytes;
+                    mbar_arrive_expect_tx(img_full + ir.stage, (uint32_t)p.img_stage_bytes);
+                    tma_box(tile, &tmap, tx * kTileW, ty * p.tile_h, f, img_full + ir.stage);
+                    tma_box(tile + p.img_stage_bytes / 2, &tmap, tx * kTileW + 32, ty * p.tile_h, f, img_full + ir.stage);
+                }
+                ++nimg;
+                ir.next(p.img_stages);
+            }
+        }
+    } else {
+        // ===== consumers: blocks dealt round-robin to the warps, continuing across frame pairs and items ==================
+        const int cw = warp - 1;
+        int firstb = cw;
+        for (int n = 0; n < nmine; ++n) {
+            const int4 d = desc_s[n];
+            if (d.w == 0) continue;
+            const int chunk = stream_item_at(n) / p.ntiles;
+            const int f0 = chunk * p.frames_per_item, f1 = min(p.nframes, f0 + p.frames_per_item);
+            mbar_wait(mat_full + mr.stage, mr.parity);
+            const unsigned char *blob = mat_base + (size_t)mr.stage * p.mat_stage_bytes;
+            const unsigned *bh = reinterpret_cast<const unsigned *>(blob) + 1;
+            for (int f = f0; f < f1; f += 2) {
+                const bool two = f + 1 < f1;
+                const int sa = ir.stage;
+                mbar_wait(img_full + sa, ir.parity);
+                ir.next(p.img_stages);
+                const int sb = ir.stage;
+                if (two) {
+                    mbar_wait(img_full + sb, ir.parity);
+                    ir.next(p.img_stages);
+                }
+                if (firstb < d.w) {
+                    const unsigned ta = smem_u32(img_base + (size_t)sa * p.img_stage_bytes);
+                    const unsigned tb = smem_u32(img_base + (size_t)sb * p.img_stage_bytes);
+                    char *pa = reinterpret_cast<char *>(p.partials) + (int64_t)f * p.nslot * 16;
+                    char *pb = pa + (int64_t)p.nslot * 16;
+                    for (int b = firstb; b < d.w; b += kStreamCons) {
+                        const unsigned h = bh[b];
+                        if (two && !stream_block2<DT, ACC>(ta, tb, blob, h, pa, pb, lane)) continue;
+                        // one frame left, or a non-finite pixel somewhere: frame by frame
+                        if (stream_block<DT, ACC, false>(ta, blob, h, pa, lane)) {
+                            if constexpr (DT == AI_F32) stream_block_tracked<ACC, false>(ta, blob, h, pa, lane);
+                        }
+                        if (two && stream_block<DT, ACC, false>(tb, blob, h, pb, lane)) {
+                            if constexpr (DT == AI_F32) stream_block_tracked<ACC, false>(tb, blob, h, pb, lane);
+                        }
+                    }
+                    __syncwarp();
+                }
+                if (lane == 0) {
+                    mbar_arrive(img_empty + sa);
+                    if (two) mbar_arrive(img_empty + sb);
+                }
+                firstb -= d.w % kStreamCons;
+                if (firstb < 0) firstb += kStreamCons;
+            }
+            if (lane == 0) mbar_arrive(mat_empty + mr.stage);
+            mr.next(p.mat_stages);
+        }
+    }
+}
+
 template <int DT, int ACC>
 int launch_stream(ai_ctx *ctx, const CUtensorMap &map, const StreamFirstDescs &first, const StreamParams &p, size_t smem,
                   int grid, cudaStream_t st)
@@ -521,6 +702,90 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int tra
     case AI_F32: rc = launch_stream_dt<AI_F32>(ctx, map, first, p, smem, grid, st); break;
     case AI_I32: rc = launch_stream_dt<AI_I32>(ctx, map, first, p, smem, grid, st); break;
     case AI_U32: rc = launch_stream_dt<AI_U32>(ctx, map, first, p, smem, grid, st); break;
+    default: break;
+    }
+    if (rc == AI_OK) *handled = true;
+    return rc;
+}
+
+namespace {
+
+template <int DT, int ACC>
+int launch_bstream(ai_ctx *ctx, const CUtensorMap &map, const BatchParams &p, size_t smem, int grid, cudaStream_t st)
+{
+    static int configured_device = -1;
+    if (configured_device != ctx->device) {
+        AI_CUDA(ctx, cudaFuncSetAttribute(tiled_bstream_kernel<DT, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          kPipeSmemBudget));
+        configured_device = ctx->device;
+    }
+    ai_prof_begin(ctx, st);
+    tiled_bstream_kernel<DT, ACC><<<grid, kStreamThreads, smem, st>>>(map, p);
+    ai_prof_end(ctx, st);
+    AI_CUDA(ctx, cudaGetLastError());
+    return AI_OK;
+}
+
+template <int DT>
+int launch_bstream_dt(ai_ctx *ctx, const CUtensorMap &map, const BatchParams &p, size_t smem, int grid, cudaStream_t st)
+{
+    switch (ctx->accum) {
+    case AI_ACC_F32_KAHAN: return launch_bstream<DT, AI_ACC_F32_KAHAN>(ctx, map, p, smem, grid, st);
+    case AI_ACC_F32_PLAIN: return launch_bstream<DT, AI_ACC_F32_PLAIN>(ctx, map, p, smem, grid, st);
+    default: return launch_bstream<DT, AI_ACC_F64>(ctx, map, p, smem, grid, st);
+    }
+}
+
+}  // namespace
+
+// Stage 1 of a batch of plain 32-bit frames (*handled = true when it applies); the caller launches stage 2.
+int ai_launch_bstream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled)
+{
+    const TiledLayout &tl = ctx->tl;
+    *handled = false;
+    if (a.nframes < 2 || tl.ntiles < 1 || !tl.blob || ctx->no_tma || ctx->no_stream) return AI_OK;
+    const bool plain = !a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask;
+    const bool is32 = a.dtype == AI_F32 || a.dtype == AI_I32 || a.dtype == AI_U32;
+    if (!plain || !is32 || !vec_ok || (reinterpret_cast<uintptr_t>(a.image) % 16) != 0) return AI_OK;
+    const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
+
+    BatchParams p{};
+    // items: every tile once per chunk of frames; enough chunks that each block gets several items, even chunks
+    int nchunks = (8 * sms + tl.ntiles - 1) / tl.ntiles;
+    if (nchunks > a.nframes / 2) nchunks = a.nframes / 2;
+    if (nchunks < 1) nchunks = 1;
+    p.frames_per_item = (a.nframes + nchunks - 1) / nchunks;
+    p.frames_per_item += p.frames_per_item & 1;
+    nchunks = (a.nframes + p.frames_per_item - 1) / p.frames_per_item;
+    const int64_t nitems = (int64_t)tl.ntiles * nchunks;
+    if (nitems > 0x3fffffffLL) return AI_OK;
+    p.nitems = (int)nitems;
+    const int grid = p.nitems < sms ? p.nitems : sms;
+    const int items_max = (p.nitems + grid - 1) / grid;
+    p.img_stage_bytes = tl.tile_h * kTileW * 4;
+    p.mat_stage_bytes = ai_align_up(tl.max_blob_bytes + 1024, 1024);
+    p.hdr_bytes = ai_align_up(kStreamBarBytes + 16 * items_max, 1024);
+    const int room = kPipeSmemBudget - p.hdr_bytes;
+    p.mat_stages = (room - 2 * p.mat_stage_bytes) / p.img_stage_bytes >= 4 ? 2 : 1;
+    p.img_stages = (room - p.mat_stages * p.mat_stage_bytes) / p.img_stage_bytes;
+    if (p.img_stages > kBatchMaxImgStages) p.img_stages = kBatchMaxImgStages;
+    if (p.img_stages < 2) return AI_OK;
+    p.blob_desc = tl.blob_desc;
+    p.blob = tl.blob;
+    p.tile_h = tl.tile_h;
+    p.ntiles = tl.ntiles;
+    p.nslot = tl.nslot;
+    p.nframes = a.nframes;
+    p.partials = ctx->partials;
+    const size_t smem = (size_t)p.img_stages * p.img_stage_bytes + p.hdr_bytes + (size_t)p.mat_stages * p.mat_stage_bytes;
+    CUtensorMap map{};
+    int rc = ai_make_frame_map(ctx, a, tl.tile_h, &map);
+    if (rc != AI_OK) return rc;
+    rc = AI_EINVAL;
+    switch (a.dtype) {
+    case AI_F32: rc = launch_bstream_dt<AI_F32>(ctx, map, p, smem, grid, st); break;
+    case AI_I32: rc = launch_bstream_dt<AI_I32>(ctx, map, p, smem, grid, st); break;
+    case AI_U32: rc = launch_bstream_dt<AI_U32>(ctx, map, p, smem, grid, st); break;
     default: break;
     }
     if (rc == AI_OK) *handled = true;

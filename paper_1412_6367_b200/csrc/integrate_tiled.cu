@@ -16,6 +16,7 @@
 
 int ai_launch_pipe_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);
 int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int track_all, cudaStream_t st, bool *handled);
+int ai_launch_bstream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);
 
 namespace {
 
@@ -237,7 +238,8 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
                 return AI_OK;
             }
         }
-        rc = ai_launch_pipe_stage1(ctx, a, vec_ok, st, &handled);
+        rc = ai_launch_bstream_stage1(ctx, a, vec_ok, st, &handled);          // batch of plain 32-bit frames
+        if (rc == AI_OK && !handled) rc = ai_launch_pipe_stage1(ctx, a, vec_ok, st, &handled);
     }
     if (rc != AI_OK) return rc;
     if (!handled) {

@@ -384,6 +384,51 @@ def test_batch_matches_oracle_small(torch, B, oracle, workloads):
     integ.close()
 
 
+@pytest.mark.parametrize("path", ["bstream", "pipe"])
+@pytest.mark.parametrize("dtype,nframes", [("int32", 7), ("float32", 6), ("uint32", 2), ("float32", 33)])
+def test_batch_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, nframes):
+    """Batches of plain 32-bit frames take the two-frames-at-a-time stream kernel; AZINT_NO_STREAM=1 sends them
+    through the general pipelined kernel.  Odd counts leave a single last frame; float frames carry NaN / Inf."""
+    if path == "pipe":
+        monkeypatch.setenv("AZINT_NO_STREAM", "1")
+    cfg = workloads.tiny_config(200, 264, center_x=100.3, center_y=90.1, unit=workloads.Q_NM, npt=257,
+                                distance_m=0.02, name="batch_small")
+    rng = np.random.default_rng(nframes)
+    frames = rng.poisson(100.0, size=(nframes, cfg.height, cfg.width)).astype(dtype)
+    if dtype == "float32":
+        frames[1, 17, 33] = np.nan
+        frames[nframes - 1, 100, 200] = np.inf
+    if dtype == "uint32":
+        t, code = torch.from_numpy(frames.view(np.int32)).cuda(), B.AI_U32
+    else:
+        t, code = torch.from_numpy(frames).cuda(), None
+    integ = B.Integrator(cfg)
+    i, s, c = integ.outputs(nframes)
+    B.ai_integrate1d_batch(integ.ctx, t, nframes, cfg.npix, None, None, None, None, None, i, s, c, dtype=code)
+    torch.cuda.synchronize()
+    for f in range(nframes):
+        want = _oracle_profile(oracle, cfg, workloads.Frame(image=frames[f]))
+        got = {"intensity": i[f].cpu().numpy(), "sum_signal": s[f].cpu().numpy(), "count": c[f].cpu().numpy()}
+        assert_profile(got, want, what=f"{path}/{dtype}/frame {f} of {nframes}")
+    integ.close()
+
+
+def test_batch_with_mask_takes_the_general_kernel(torch, B, oracle, workloads):
+    cfg = workloads.tiny_config(130, 200, center_x=60.0, center_y=70.0, unit=workloads.TTH_DEG, npt=150,
+                                distance_m=0.03, name="batch_mask")
+    rng = np.random.default_rng(3)
+    frames = rng.poisson(50.0, size=(4, cfg.height, cfg.width)).astype(np.int32)
+    mask = (rng.random(size=(cfg.height, cfg.width)) < 0.1).astype(np.uint8)
+    integ = B.Integrator(cfg)
+    i, s, c = integ.integrate1d_batch(torch.from_numpy(frames).cuda(), mask=torch.from_numpy(mask).cuda())
+    torch.cuda.synchronize()
+    for f in range(4):
+        want = _oracle_profile(oracle, cfg, workloads.Frame(image=frames[f], mask=mask))
+        got = {"intensity": i[f].cpu().numpy(), "sum_signal": s[f].cpu().numpy(), "count": c[f].cpu().numpy()}
+        assert_profile(got, want, what=f"masked batch frame {f}")
+    integ.close()
+
+
 def test_batch_full_size_sampled(torch, B, oracle, workloads):
     """BASELINE.json configs[3] at full size: 1024 frames of 1024x1024 int32 in one call (the launch configuration
     bench.py times).  The frames cycle through a pool of 8 distinct seeded frames; sampled outputs are compared with
