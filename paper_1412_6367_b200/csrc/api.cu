@@ -120,7 +120,6 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
                 else if (!strcmp(key, "bis")) ctx->tune.batch_img_stages = val;
                 else if (!strcmp(key, "fl")) ctx->tune.inflight = val;
                 else if (!strcmp(key, "ss")) ctx->tune.stream_stages = val;
-                else if (!strcmp(key, "pf")) ctx->tune.prefetch_tiles = val;
             }
             q = strchr(q, ',');
             if (q) ++q;
@@ -143,8 +142,8 @@ int ai_build_csr(ai_ctx *ctx, void *cuda_stream)
     ai_free_spans(&spans);
     if (rc != AI_OK) return rc;
     AI_CUDA(ctx, cudaMalloc(&ctx->out_dev, 3 * (size_t)ctx->npt * sizeof(float)));
-    AI_CUDA(ctx, cudaMalloc(&ctx->grid_sync, sizeof(unsigned long long)));
-    AI_CUDA(ctx, cudaMemsetAsync(ctx->grid_sync, 0, sizeof(unsigned long long), st));
+    AI_CUDA(ctx, cudaMalloc(&ctx->grid_sync, 2 * sizeof(unsigned long long)));
+    AI_CUDA(ctx, cudaMemsetAsync(ctx->grid_sync, 0, 2 * sizeof(unsigned long long), st));
     AI_CUDA(ctx, cudaStreamSynchronize(st));
     ctx->built = true;
     return AI_OK;

@@ -58,7 +58,6 @@ struct PipeTune {
     int batch_mat_stages = 2, batch_img_stages = kPipeMaxImgStages;
     int inflight = 0;                          // 0 = as many as there are stages
     int stream_stages = 0;                     // cap on the (tile + blob) stages of the single-frame kernel, 0 = none
-    int prefetch_tiles = 0;                    // single-frame kernel: tiles per block prefetched into L2 in the prologue
 };
 inline PipePlan ai_pipe_plan(int max_blob_bytes, int tile_h, bool batch, const PipeTune &tune = PipeTune())
 {
@@ -151,7 +150,7 @@ struct ai_ctx {
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t h2d_done[2] = {nullptr, nullptr}, slot_free[2] = {nullptr, nullptr};
     float *corrected = nullptr;     // [height*width] corrected float32 frame (integrate_prep.cu), allocated on first use
-    unsigned long long *grid_sync = nullptr;   // arrival counter of the fused single-frame kernel's grid barrier
+    unsigned long long *grid_sync = nullptr;   // fused single-frame kernel: [0] arrivals at its barrier, [1] tile tickets
 
     // measurement hook (ai_profile_enable): events around the dominant kernel of the last call
     PipeTune tune;

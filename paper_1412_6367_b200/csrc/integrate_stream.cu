@@ -23,7 +23,8 @@ constexpr int kStreamThreads = 32 * (1 + kStreamCons);
 constexpr int kStreamFirst = 3;                      // descriptors per block passed by value
 constexpr int kStreamMaxGrid = 160;
 constexpr int kStreamMaxStages = 8;
-constexpr int kStreamBarBytes = 256;                 // full[8] + empty[8] + a few words of block-wide state
+constexpr int kStreamBarBytes = 512;                 // full[8] + empty[8], block-wide state, per-stage descriptors
+constexpr int kStreamDescOffset = 256;
 
 struct StreamFirstDescs {
     int4 d[kStreamFirst][kStreamMaxGrid];
@@ -34,12 +35,12 @@ struct StreamParams {
     const unsigned char *blob;
     int tile_h, ntiles, nslot;
     int stages, mat_stage_bytes, img_stage_bytes, hdr_bytes, items_max;
-    int prefetch_tiles;          // tiles per block whose data is pulled into L2 before the grid dependency resolves
+    int dyn_base;                // rank of the first tile handed out by ticket (the ones before are dealt statically)
     int launch_index;            // launches of this context so far, modulo 8 (development trace only)
     int track_all;               // float frames: every block skips non-finite pixels and accumulates count
     void *partials;
     // H5 fused behind a grid-wide barrier (every block is resident: one per SM, grid <= number of SMs)
-    unsigned long long *grid_sync;     // arrivals of all launches of this context, never reset
+    unsigned long long *grid_sync;     // [0] arrivals of all launches of this context, never reset; [1] tile tickets
     const int *bin_slot_ptr;
     const double *range;
     int npt;
@@ -235,27 +236,29 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
                                                                          const __grid_constant__ StreamFirstDescs first,
                                                                          const StreamParams p)
 {
-    // [tile stages][barriers, tile descriptors][matrix stages]
+    // [tile stages][barriers, per-stage tile descriptors][matrix stages]
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *img_base = smem;
     unsigned char *hdr = smem + (size_t)p.stages * p.img_stage_bytes;
     uint64_t *full = reinterpret_cast<uint64_t *>(hdr);              // tile + blob landed (complete_tx)
     uint64_t *empty = full + kStreamMaxStages;                        // every consumer warp is done with the stage
-    int4 *desc_s = reinterpret_cast<int4 *>(hdr + kStreamBarBytes);
+    int4 *stage_desc = reinterpret_cast<int4 *>(hdr + kStreamDescOffset);   // descriptor of the tile in each stage
     unsigned char *mat_base = hdr + p.hdr_bytes;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     AI_STRACE_AT(15, 0, strace_now());
 
-    // number of tiles of this block
-    int nmine = 0;
-    while (stream_item_at(nmine) < p.ntiles) ++nmine;
+    // Tiles, longest first: the first npre of every block are dealt statically (snake order; their descriptors came
+    // with the launch), the rest are handed out by a ticket counter to whichever block has a free stage -- the blocks
+    // do not finish their static shares at the same time (the memory system serves them unevenly).
+    int npre = 0;
+    while (npre < min(kStreamFirst, p.stages) && stream_item_at(npre) < p.ntiles) ++npre;
 
     // Launch chain (programmatic dependent launch): this grid may start while the previous kernel of the stream is
-    // still running (stage 2 of the previous frame triggers its dependents at once).  Nothing that kernel may still
-    // read or write is touched before griddepcontrol.wait: until then only the matrix (static since ai_build_csr) is
-    // fetched -- the blobs of the block's first tiles -- together with descriptors, barriers and the tensor map; the
-    // frame is read and the partials are written after it.
+    // still running.  Nothing that kernel may still read or write is touched before griddepcontrol.wait: until then
+    // only the matrix (static since ai_build_csr) is fetched -- the blobs of the block's first tiles -- together with
+    // barriers and the tensor map; the frame is read, tickets are drawn and the partials are written after it.
     auto issue_blob = [&](int stage, const int4 &d) {
+        stage_desc[stage] = d;
         mbar_arrive_expect_tx(full + stage, (uint32_t)(p.img_stage_bytes + d.y));
         bulk_g2s(mat_base + (size_t)stage * p.mat_stage_bytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y, full + stage);
     };
@@ -265,7 +268,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
         tma_box(tile, &tmap, tx * kTileW, ty * p.tile_h, 0, full + stage);
         tma_box(tile + p.img_stage_bytes / 2, &tmap, tx * kTileW + 32, ty * p.tile_h, 0, full + stage);
     };
-    const int npre = min(min(kStreamFirst, p.stages), nmine);         // tiles whose copies are issued by thread 0 here
 
     if (threadIdx.x == 0) {
         // the packed rebase needs every tile buffer inside the first 64 KB of the shared window
@@ -283,32 +285,14 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
             issue_blob(stage++, d);
         }
     }
-    for (int k = threadIdx.x; k < nmine; k += kStreamThreads)
-        desc_s[k] = k < kStreamFirst ? first.d[k][blockIdx.x] : __ldg(p.blob_desc + stream_item_at(k));
-    // H5 reads the slot ranges of the bins at the very end: pull them into L2 now (static data, 4 bytes per bin)
+    // static data read late in the kernel, pulled into L2 now: the descriptors of the ticketed tiles (each block its
+    // share of the array) and the slot ranges of the bins (H5)
+    for (int k = p.dyn_base + (blockIdx.x * kStreamThreads + threadIdx.x) * 8; k < p.ntiles; k += gridDim.x * kStreamThreads * 8)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(p.blob_desc + k));
     for (int k = threadIdx.x * 32; k <= p.npt; k += kStreamThreads * 32)
         asm volatile("prefetch.global.L2 [%0];" ::"l"(p.bin_slot_ptr + k));
     // the next kernel of the stream may be scheduled as SMs free up
     asm volatile("griddepcontrol.launch_dependents;");
-    __syncthreads();                                   // descriptors are in shared memory
-    // While the previous kernel of the stream drains, HBM would idle: pull this block's share of the frame and the
-    // rest of its matrix into L2 (prefetches return nothing to the SM, and L2 is the point of coherence: a frame
-    // that the previous kernel is still writing is read, after the wait below, as that kernel left it).
-    if (warp == 0) {
-        const int npf = min(nmine, p.prefetch_tiles);
-        for (int n = lane; n < npf; n += 32) {
-            const int4 d = desc_s[n];
-            if (d.w == 0) continue;
-            const int ty = d.z >> 16, tx = d.z & 0xffff;
-            asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
-                         ::"l"(&tmap), "r"(tx * kTileW), "r"(ty * p.tile_h), "r"(0) : "memory");
-            asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
-                         ::"l"(&tmap), "r"(tx * kTileW + 32), "r"(ty * p.tile_h), "r"(0) : "memory");
-            if (n >= npre)
-                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;"
-                             ::"l"(p.blob + (size_t)d.x * 16), "r"(d.y) : "memory");
-        }
-    }
     asm volatile("griddepcontrol.wait;" ::: "memory");
     AI_STRACE_AT(14, 1, strace_now());
     if (threadIdx.x == 0) {
@@ -326,33 +310,64 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
     if (warp == 0) {
         // ===== producer ================================================================================================
         int issued = 0;
-        for (int n = 0; n < nmine; ++n) {
-            const int4 d = desc_s[n];
-            if (d.w == 0) continue;                       // tile without entries: skipped by every role
-            if (n >= npre) {
-                AI_STRACE(n, 0, strace_now());
-                if (issued >= p.stages) mbar_wait(empty + r.stage, r.parity ^ 1u);
-                if (lane == 0) {
-                    issue_blob(r.stage, d);
-                    issue_tile(r.stage, d);
-                }
-                AI_STRACE(n, 1, strace_now());
-            }
+        for (int n = 0; n < npre; ++n) {                  // stages taken by the static tiles
+            if (first.d[n][blockIdx.x].w == 0) continue;
             ++issued;
             r.next(p.stages);
+        }
+        // Ticketed tiles, two draws ahead so that neither the atomic nor the descriptor load is waited for: in every
+        // trip lane 0 takes the descriptor loaded in the previous trip, loads the one for the ticket drawn in the
+        // previous trip and draws a new ticket; only the block count is shared with the warp (uniform control flow).
+        const unsigned long long nticket = p.dyn_base < p.ntiles ? (unsigned long long)(p.ntiles - p.dyn_base) : 0ULL;
+        auto fetch = [&](unsigned long long t) {
+            return t < nticket ? __ldg(p.blob_desc + p.dyn_base + (int)t) : make_int4(0, 0, 0, -1);
+        };
+        unsigned long long t_next = ~0ULL;
+        int4 d_next = make_int4(0, 0, 0, -1);
+        if (lane == 0 && nticket) {
+            const unsigned long long t0 = atomicAdd(p.grid_sync + 1, 1ULL);
+            t_next = atomicAdd(p.grid_sync + 1, 1ULL);
+            d_next = fetch(t0);
+        }
+        int n = npre;
+        while (true) {
+            const int4 d = d_next;
+            if (lane == 0 && nticket) {
+                d_next = fetch(t_next);
+                t_next = atomicAdd(p.grid_sync + 1, 1ULL);
+            }
+            const int nblk = __shfl_sync(AI_FULL_MASK, d.w, 0);
+            if (nblk < 0) break;
+            if (nblk == 0) continue;                      // tile without entries: never published
+            AI_STRACE(n, 0, strace_now());
+            if (issued >= p.stages) mbar_wait(empty + r.stage, r.parity ^ 1u);
+            if (lane == 0) {
+                issue_blob(r.stage, d);
+                issue_tile(r.stage, d);
+            }
+            AI_STRACE(n, 1, strace_now());
+            ++issued;
+            ++n;
+            r.next(p.stages);
+        }
+        // no tile left: a descriptor with a negative block count ends the consumers' loop
+        if (issued >= p.stages) mbar_wait(empty + r.stage, r.parity ^ 1u);
+        if (lane == 0) {
+            stage_desc[r.stage] = make_int4(0, 0, 0, -1);
+            mbar_arrive(full + r.stage);
         }
     } else {
         // ===== consumers: a tile's blocks are dealt round-robin to the warps, continuing across tiles ===================
         const int cw = warp - 1;
         int firstb = cw;
-        for (int n = 0; n < nmine; ++n) {
-            const int4 d = desc_s[n];
-            if (d.w == 0) continue;
+        for (int n = 0;; ++n) {
             // every warp waits on and arrives at every stage, also when it holds no block of the tile: no warp is
             // ever a whole phase away from a barrier
             AI_STRACE(n, 0, strace_now());
             mbar_wait(full + r.stage, r.parity);
             AI_STRACE(n, 1, strace_now());
+            const int4 d = stage_desc[r.stage];
+            if (d.w < 0) break;
             if (firstb < d.w) {
                 const unsigned char *blob = mat_base + (size_t)r.stage * p.mat_stage_bytes;
                 const unsigned *bh = reinterpret_cast<const unsigned *>(blob) + 1;
@@ -395,7 +410,10 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
         const unsigned long long old = atomicAdd(p.grid_sync, 1ULL);
         const int place = (int)(old % gridDim.x);
         target = (old / gridDim.x + 1ULL) * gridDim.x;
-        if (old + 1 == target) target = 0;                       // the last block to arrive has nothing to wait for
+        if (old + 1 == target) {                                 // the last block to arrive has nothing to wait for,
+            target = 0;
+            p.grid_sync[1] = 0ULL;                               // and every producer is done: tickets start over
+        }
         *fin_rank = place >= (int)gridDim.x - nfin ? place - ((int)gridDim.x - nfin) : -1;
     }
     __syncthreads();
@@ -628,7 +646,7 @@ static bool stream_plan(const ai_ctx *ctx, int grid, StreamParams *p)
     p->img_stage_bytes = tl.tile_h * kTileW * 4;
     p->mat_stage_bytes = ai_align_up(tl.max_blob_bytes + 1024, 1024);     // slack: the look-ahead reads past a blob's end
     p->items_max = (tl.ntiles + grid - 1) / grid;
-    p->hdr_bytes = ai_align_up(kStreamBarBytes + 16 * p->items_max, 1024);
+    p->hdr_bytes = ai_align_up(kStreamBarBytes, 1024);
     int stages = (kPipeSmemBudget - p->hdr_bytes) / (p->img_stage_bytes + p->mat_stage_bytes);
     if (stages > kStreamMaxStages) stages = kStreamMaxStages;
     if (ctx->tune.stream_stages > 0 && stages > ctx->tune.stream_stages) stages = ctx->tune.stream_stages;
@@ -672,7 +690,7 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int tra
     p.ntiles = tl.ntiles;
     p.nslot = tl.nslot;
     p.partials = ctx->partials;
-    p.prefetch_tiles = ctx->tune.prefetch_tiles;
+    p.dyn_base = (p.stages < kStreamFirst ? p.stages : kStreamFirst) * grid;
     p.track_all = track_all;
     static unsigned launches = 0;                  // development trace only: which of 8 trace buffers the launch writes
     p.launch_index = launches++ & 7;
