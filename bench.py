@@ -435,6 +435,23 @@ def run_extras(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args):
         for it in its:
             it.close()
         del corr, fdev
+    # context (SURVEY.md section 8(d) "T3"): the frame shape of the paper's Table 3 (Pilatus 1M, 981 x 1043 int32,
+    # PAPER.md:257) -- geometry is a reading (centre of the image, 172 um pixels, 0.1 m, 1000 bins in 2theta)
+    cp = W.tiny_config(981, 1043, center_x=521.5, center_y=490.5, unit=W.TTH_DEG, npt=1000, pixel_m=172e-6,
+                       distance_m=0.1, name="pilatus1m")
+    rngp = np.random.default_rng(14126367 + 9)
+    fp = [torch.from_numpy(rngp.poisson(30.0, size=(cp.height, cp.width)).astype(np.int32)).cuda() for _ in range(4)]
+    its = [B.Integrator(cp) for _ in range(6)]
+    tot, launches = timed_train(torch, B, its, fp, none5, 200, 10)
+    ex["pilatus1m_int32_table3_shape"] = {"frames_per_s": 200 / (tot * 1e-3), "ms_per_step": tot / 200,
+                                          "launches_per_step": launches / 200,
+                                          "paper_table3": "integrate kernel 0.384 ms, OpenCL total 1.445 ms, Python call "
+                                                          "2.030 ms on a GeForce Titan (PAPER.md:244-257): context, "
+                                                          "other hardware",
+                                          "note": "width 1043 is not a multiple of 4: rows are not 16-byte aligned, the "
+                                                  "general kernel with scalar staging runs"}
+    for it in its:
+        it.close()
     # configs[3]: 1024 int32 frames of 1024x1024 in one batched call
     c4 = W.CONFIGS["cfg4"]
     pool = torch.from_numpy(W.make_frames(c4, 8)).cuda()

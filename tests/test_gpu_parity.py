@@ -256,6 +256,34 @@ def test_results_are_bit_reproducible(torch, B, workloads):
     integ.close()
 
 
+@pytest.mark.parametrize("corrected", [False, True])
+def test_back_to_back_launches_do_not_interfere(torch, B, workloads, corrected):
+    """Launches chained by programmatic dependent launch overlap (the next kernel's prologue runs while the previous
+    one drains) and share the context's partial buffer, ticket counter and barrier counter: a train of calls on
+    rotating frames and two contexts must give, bit for bit, what the same calls give one at a time."""
+    cfg = workloads.CONFIGS["cfg2"]
+    rng = np.random.default_rng(11)
+    base = workloads.make_frame(cfg).image
+    frames = [torch.from_numpy(base * np.float32(s)).cuda() for s in (1.0, 0.5, 2.0, 3.0, 0.25)]
+    mask = torch.from_numpy((rng.random(base.shape) < 0.03).astype(np.uint8)).cuda() if corrected else None
+    integs = [B.Integrator(cfg), B.Integrator(cfg)]
+    ref = []
+    for k in range(len(frames)):
+        out = integs[0].integrate1d(frames[k], mask=mask)
+        torch.cuda.synchronize()
+        ref.append([o.clone() for o in out])
+    n = 60
+    outs = [[integs[j].outputs() for _ in range(n)] for j in range(2)]
+    for k in range(n):
+        integs[k % 2].integrate1d(frames[k % len(frames)], mask=mask, out=outs[k % 2][k])
+    torch.cuda.synchronize()
+    for k in range(n):
+        for a, b in zip(outs[k % 2][k], ref[k % len(frames)]):
+            assert torch.equal(a, b), f"call {k} differs from the same call run alone"
+    for it in integs:
+        it.close()
+
+
 def test_compensation_keeps_small_terms(torch, B, workloads):
     """Kahan summation lets single precision give accurate sums.  One bin, one pixel of 2^24 and
     65535 pixels of 1: the exact sum is 2^24 + 65535; every lane that holds the big value would drop the ones without
