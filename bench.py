@@ -448,8 +448,8 @@ def run_extras(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args):
                                           "paper_table3": "integrate kernel 0.384 ms, OpenCL total 1.445 ms, Python call "
                                                           "2.030 ms on a GeForce Titan (PAPER.md:244-257): context, "
                                                           "other hardware",
-                                          "note": "width 1043 is not a multiple of 4: rows are not 16-byte aligned, the "
-                                                  "general kernel with scalar staging runs"}
+                                          "note": "width 1043 is not a multiple of 4 (rows off 16-byte boundaries): the "
+                                                  "pre-pass casts and re-pitches the frame, then the single-frame kernel"}
     for it in its:
         it.close()
     # configs[3]: 1024 int32 frames of 1024x1024 in one batched call

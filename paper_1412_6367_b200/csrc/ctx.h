@@ -200,6 +200,7 @@ struct FrameArgs {
     float *radial, *intensity, *sum_signal, *count;
     int nframes;
     int64_t frame_stride;
+    int64_t row_pitch = 0;       // elements between rows of `image`; 0 = width (only the library's own corrected frame differs)
 };
 int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_csr(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);

@@ -431,7 +431,8 @@ int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *
     const CUtensorMapDataType dt = a.dtype == AI_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
                                  : a.dtype == AI_I32 ? CU_TENSOR_MAP_DATA_TYPE_INT32 : CU_TENSOR_MAP_DATA_TYPE_UINT32;
     const cuuint64_t dims[3] = {(cuuint64_t)ctx->width, (cuuint64_t)ctx->height, (cuuint64_t)a.nframes};
-    const cuuint64_t strides[2] = {(cuuint64_t)ctx->width * 4, (cuuint64_t)a.frame_stride * 4};
+    const cuuint64_t pitch = a.row_pitch ? (cuuint64_t)a.row_pitch : (cuuint64_t)ctx->width;
+    const cuuint64_t strides[2] = {pitch * 4, (cuuint64_t)a.frame_stride * 4};
     const cuuint32_t box[3] = {32, (cuuint32_t)tile_h, 1};
     const cuuint32_t estr[3] = {1, 1, 1};
     const CUresult r = enc(map, dt, 3, const_cast<void *>(a.image), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,

@@ -12,7 +12,8 @@ constexpr int kPrepThreads = 256;
 
 template <int DT>
 __global__ void __launch_bounds__(kPrepThreads) correct_frame_kernel(const void *__restrict__ img, Corrections cor,
-                                                                     int64_t npix, int vec_ok, float *__restrict__ out)
+                                                                     int64_t npix, int width, int pitch, int vec_ok,
+                                                                     float *__restrict__ out)
 {
     // the single-frame kernel that follows may start its prologue (it reads `out` after its griddepcontrol.wait)
     asm volatile("griddepcontrol.launch_dependents;");
@@ -37,20 +38,25 @@ __global__ void __launch_bounds__(kPrepThreads) correct_frame_kernel(const void 
             *reinterpret_cast<float4 *>(out + p) = v;
         }
     } else {
-        for (int64_t p = (int64_t)blockIdx.x * kPrepThreads + threadIdx.x; p < npix; p += stride)
-            out[p] = corrected_pixel<DT>(img, p, cor);
+        // rows of the output start on 16-byte boundaries (pitch = width rounded up to 4): what the tensor map needs
+        for (int64_t p = (int64_t)blockIdx.x * kPrepThreads + threadIdx.x; p < npix; p += stride) {
+            const int64_t y = p / width;
+            out[y * pitch + (p - y * width)] = corrected_pixel<DT>(img, p, cor);
+        }
     }
 }
 
 }  // namespace
 
-// Writes the corrected float32 image of frame 0 of `a` into ctx->corrected (allocated on first use).
+// Writes the corrected float32 image of frame 0 of `a` into ctx->corrected (allocated on first use; row pitch = width
+// rounded up to a multiple of 4, so that frames of any width reach the single-frame kernel through a tensor map).
 int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st)
 {
     const int64_t npix = (int64_t)ctx->height * ctx->width;
-    if (!ctx->corrected) AI_CUDA(ctx, cudaMalloc(&ctx->corrected, (size_t)npix * sizeof(float)));
+    const int pitch = (ctx->width + 3) / 4 * 4;
+    if (!ctx->corrected) AI_CUDA(ctx, cudaMalloc(&ctx->corrected, (size_t)ctx->height * pitch * sizeof(float)));
     Corrections cor{a.dark, a.flat, a.solidangle, a.polarization, a.mask};
-    const int vec = vec_ok && npix % 4 == 0;
+    const int vec = vec_ok && ctx->width % 4 == 0;
     const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
     int64_t blocks = ((vec ? npix / 4 : npix) + kPrepThreads - 1) / kPrepThreads;
     if (blocks > (int64_t)sms * 8) blocks = (int64_t)sms * 8;        // grid-stride: 8 resident blocks per SM
@@ -64,7 +70,8 @@ int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t 
     cfg.stream = st;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-#define AI_PREP(DT) AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, correct_frame_kernel<DT>, a.image, cor, npix, vec, ctx->corrected))
+#define AI_PREP(DT) \
+    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, correct_frame_kernel<DT>, a.image, cor, npix, ctx->width, pitch, vec, ctx->corrected))
     switch (a.dtype) {
     case AI_F32: AI_PREP(AI_F32); break;
     case AI_I32: AI_PREP(AI_I32); break;

@@ -219,15 +219,17 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
             ctx->last_launches = 1;
             return AI_OK;
         }
-        // one frame with correction arrays, a mask, 16-bit pixels or unaligned buffers: H1 + H2 as a streaming
-        // pre-pass into a float32 frame (invalid pixels as NaN), then the same single-frame kernel
-        if (a.nframes == 1 && !ctx->no_prepass && !ctx->no_stream && !ctx->no_tma && ctx->width % 4 == 0 &&
-            ai_stream_stages(ctx) >= 2) {
+        // one frame with correction arrays, a mask, 16-bit pixels, unaligned buffers or rows that do not start on
+        // 16-byte boundaries (width not a multiple of 4): H1 + H2 as a streaming pre-pass into a float32 frame with
+        // padded rows (invalid pixels as NaN), then the same single-frame kernel
+        if (a.nframes == 1 && !ctx->no_prepass && !ctx->no_stream && !ctx->no_tma && ai_stream_stages(ctx) >= 2) {
             rc = ai_launch_correct(ctx, a, vec_ok, st);
             if (rc != AI_OK) return rc;
             FrameArgs b = a;
             b.image = ctx->corrected;
             b.dtype = AI_F32;
+            b.row_pitch = (ctx->width + 3) / 4 * 4;
+            b.frame_stride = (int64_t)ctx->height * b.row_pitch;
             b.dark = b.flat = b.solidangle = b.polarization = nullptr;
             b.mask = nullptr;
             const int may_be_invalid = a.dark || a.flat || a.solidangle || a.polarization || a.mask || a.dtype == AI_F32;

@@ -321,9 +321,11 @@ def _run_raw(torch, B, integ, img, dtype):
 
 @pytest.mark.parametrize("path", ["stream", "pipe"])
 @pytest.mark.parametrize("dtype", ["float32", "int32", "uint32"])
-@pytest.mark.parametrize("shape", [(256, 256), (130, 200), (70, 1028)])
+@pytest.mark.parametrize("shape", [(256, 256), (130, 200), (70, 1028), (97, 131)])
 def test_single_frame_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, shape):
-    """AZINT_NO_STREAM=1 (read by ai_setup) sends single plain frames through the general pipelined kernel."""
+    """AZINT_NO_STREAM=1 (read by ai_setup) sends single plain frames through the general pipelined kernel.  A width
+    that is not a multiple of 4 (rows off 16-byte boundaries) reaches the single-frame kernel through the pre-pass,
+    which re-pitches the frame."""
     if path == "pipe":
         monkeypatch.setenv("AZINT_NO_STREAM", "1")
     h, w = shape
