@@ -1,17 +1,19 @@
-// TILED stage 1, single-frame fast path: the CSR SpMV of PAPER.md:174-188 for one frame of
-// 32-bit pixels without correction arrays -- the configuration the headline metric is quoted on.
+// The TMA-streamed kernels of the TILED layout -- the CSR SpMV of PAPER.md:174-188 on B200.
 //
-// Same sliced matrix layout and the same arithmetic as integrate_pipe.cu, with everything that kernel carries for
-// batches, corrections and 16-bit pixels stripped from the critical path:
-//   - one persistent block per SM, 1 producer warp + kStreamCons consumer warps, no stager warps: float frames are
-//     gathered straight from the TMA tile, integer frames are converted at gather time ("casted from
-//     integer to float");
+// tiled_stream_kernel: the whole hot path of ONE frame of 32-bit pixels in one launch (the configuration the headline
+// metric is quoted on; corrected frames come here through the pre-pass of integrate_prep.cu).
+//   - one persistent block per SM, 1 producer warp + kStreamCons consumer warps; float frames are gathered straight
+//     from the TMA tile, integer frames are converted at gather time ("casted from integer to float");
 //   - one ring whose stage holds a tile of the frame AND that tile's blob of the matrix, one full / empty mbarrier pair
-//     per stage: a consumer warp waits once and arrives once per tile;
-//   - the block's tile descriptors sit in shared memory (one LDS per tile and warp); the first kStreamFirst of every
-//     block travel in the kernel parameters, so the first copies are issued before any global load has returned;
+//     per stage; the descriptor of the tile in a stage sits next to the barriers;
+//   - tiles longest first: the first kStreamFirst of every block are dealt statically and travel in the kernel
+//     parameters (their copies leave before any global load has returned), the rest are drawn from a ticket counter;
 //   - pixel positions of two entries are rebased with one packed 16-bit add: the tile buffers live in the first 64 KB of
-//     the shared window, so a position's low half-word is its whole shared address.
+//     the shared window, so a position's low half-word is its whole shared address;
+//   - H5 fused: the last blocks to arrive at a counter add the partials up (fixed order) and write the three outputs;
+//   - programmatic dependent launch: the next launch's prologue and first blobs overlap this launch's tail.
+// tiled_bstream_kernel: batches of plain 32-bit frames, the blob of a tile loaded once per chunk of frames, two frames
+// consumed per pass.
 #include "pipe_common.cuh"
 #include "tiled_common.cuh"
 
@@ -34,7 +36,7 @@ struct StreamParams {
     const int4 *blob_desc;       // longest first: {blob offset / 16, blob bytes, tile row << 16 | column, blocks}
     const unsigned char *blob;
     int tile_h, ntiles, nslot;
-    int stages, mat_stage_bytes, img_stage_bytes, hdr_bytes, items_max;
+    int stages, mat_stage_bytes, img_stage_bytes, hdr_bytes;
     int dyn_base;                // rank of the first tile handed out by ticket (the ones before are dealt statically)
     int launch_index;            // launches of this context so far, modulo 8 (development trace only)
     int track_all;               // float frames: every block skips non-finite pixels and accumulates count
@@ -406,8 +408,10 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
     unsigned long long target = 0;
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence();
-        const unsigned long long old = atomicAdd(p.grid_sync, 1ULL);
+        // release: the block's partials (ordered before this thread by the barrier above) are visible to whoever
+        // observes the arrival; acquire: the last block to arrive sees everybody's
+        unsigned long long old;
+        asm volatile("atom.add.acq_rel.gpu.global.u64 %0, [%1], 1;" : "=l"(old) : "l"(p.grid_sync) : "memory");
         const int place = (int)(old % gridDim.x);
         target = (old / gridDim.x + 1ULL) * gridDim.x;
         if (old + 1 == target) {                                 // the last block to arrive has nothing to wait for,
@@ -645,7 +649,6 @@ static bool stream_plan(const ai_ctx *ctx, int grid, StreamParams *p)
     const TiledLayout &tl = ctx->tl;
     p->img_stage_bytes = tl.tile_h * kTileW * 4;
     p->mat_stage_bytes = ai_align_up(tl.max_blob_bytes + 1024, 1024);     // slack: the look-ahead reads past a blob's end
-    p->items_max = (tl.ntiles + grid - 1) / grid;
     p->hdr_bytes = ai_align_up(kStreamBarBytes, 1024);
     int stages = (kPipeSmemBudget - p->hdr_bytes) / (p->img_stage_bytes + p->mat_stage_bytes);
     if (stages > kStreamMaxStages) stages = kStreamMaxStages;
