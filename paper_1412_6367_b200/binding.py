@@ -210,6 +210,11 @@ class Integrator:
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1412_6367_b200 needs a CUDA device (no CPU fallback)")
         self.torch = torch
+        self._integrate1d = lib().ai_integrate1d
+        self._codes = {torch.float32: AI_F32, torch.int32: AI_I32, torch.int16: AI_I16}
+        for name, code in (("uint16", AI_U16), ("uint32", AI_U32)):
+            if hasattr(torch, name):
+                self._codes[getattr(torch, name)] = code
         self.device = torch.device(device)
         self.cfg = cfg
         self.npt = cfg.npt
@@ -239,10 +244,22 @@ class Integrator:
 
     def integrate1d(self, image, dark=None, flat=None, solidangle=None, polarization=None, mask=None, out=None,
                     radial=None):
-        """Returns (intensity, sum_signal, count) device tensors; enqueues on the current stream."""
+        """Returns (intensity, sum_signal, count) device tensors; enqueues on the current stream.  Same marshalling as
+        ai_integrate1d above with the per-call lookups (library handle, dtype code table) hoisted: at ~18 us of GPU
+        time per 2048 x 2048 frame the host has to enqueue a call in well under that."""
         intensity, sum_signal, count = out if out is not None else self.outputs()
-        ai_integrate1d(self.ctx, image, dark, flat, solidangle, polarization, mask, radial, intensity, sum_signal,
-                       count)
+        code = self._codes.get(image.dtype)
+        if code is None:
+            raise AzintError(AI_EINVAL, f"unsupported frame dtype {image.dtype}")
+        rc = self._integrate1d(self.ctx, image.data_ptr(), code,
+                               None if dark is None else dark.data_ptr(), None if flat is None else flat.data_ptr(),
+                               None if solidangle is None else solidangle.data_ptr(),
+                               None if polarization is None else polarization.data_ptr(),
+                               None if mask is None else mask.data_ptr(), None if radial is None else radial.data_ptr(),
+                               intensity.data_ptr(), sum_signal.data_ptr(), count.data_ptr(),
+                               self.torch.cuda.current_stream().cuda_stream)
+        if rc != AI_OK:
+            _check(rc, self.ctx)
         return intensity, sum_signal, count
 
     def integrate1d_batch(self, frames, dark=None, flat=None, solidangle=None, polarization=None, mask=None,
