@@ -19,8 +19,8 @@
 
 namespace {
 
-constexpr int kStreamCons = 20;                      // consumer warps (21 warps x 72 registers leave room for
-                                                     // a block of stage 2 next to this one: see the launch chain)
+constexpr int kStreamCons = 16;                      // consumer warps: the single-frame kernel is bound by the memory
+                                                     // system, 16 keep up with it and arrive at barriers sooner than 20 or 24
 constexpr int kStreamThreads = 32 * (1 + kStreamCons);
 constexpr int kStreamFirst = 3;                      // descriptors per block passed by value
 constexpr int kStreamMaxGrid = 160;
@@ -463,6 +463,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
 // every frame of the chunk (the batched variant that amortises the matrix read across frames); the frames' tiles stream
 // through a ring of image stages and are consumed two frames at a time (stream_block2).  Writes one partial per run
 // and frame; tiled_stage2_kernel adds them up.
+constexpr int kBatchCons = 20;                       // consumer warps: the batch kernel is bound by the consumers' issue rate
+constexpr int kBatchThreads = 32 * (1 + kBatchCons);
 constexpr int kBatchMaxImgStages = 8;
 constexpr int kBatchMaxMatStages = 2;
 
@@ -476,7 +478,7 @@ struct BatchParams {
 };
 
 template <int DT, int ACC>
-__global__ void __launch_bounds__(kStreamThreads, 1) tiled_bstream_kernel(const __grid_constant__ CUtensorMap tmap,
+__global__ void __launch_bounds__(kBatchThreads, 1) tiled_bstream_kernel(const __grid_constant__ CUtensorMap tmap,
                                                                           const BatchParams p)
 {
     // [image stages][barriers, item descriptors][matrix stages]
@@ -496,15 +498,15 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_bstream_kernel(const 
     if (threadIdx.x == 0) {
         for (int s = 0; s < kBatchMaxImgStages; ++s) {
             mbar_init(img_full + s, 1);
-            mbar_init(img_empty + s, kStreamCons);
+            mbar_init(img_empty + s, kBatchCons);
         }
         for (int s = 0; s < kBatchMaxMatStages; ++s) {
             mbar_init(mat_full + s, 1);
-            mbar_init(mat_empty + s, kStreamCons);
+            mbar_init(mat_empty + s, kBatchCons);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int k = threadIdx.x; k < nmine; k += kStreamThreads) {
+    for (int k = threadIdx.x; k < nmine; k += kBatchThreads) {
         const int w = stream_item_at(k);
         int4 d = __ldg(p.blob_desc + w % p.ntiles);
         d.x = d.w ? d.x : 0;
@@ -570,7 +572,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_bstream_kernel(const 
                     const unsigned tb = smem_u32(img_base + (size_t)sb * p.img_stage_bytes);
                     char *pa = reinterpret_cast<char *>(p.partials) + (int64_t)f * p.nslot * 16;
                     char *pb = pa + (int64_t)p.nslot * 16;
-                    for (int b = firstb; b < d.w; b += kStreamCons) {
+                    for (int b = firstb; b < d.w; b += kBatchCons) {
                         const unsigned h = bh[b];
                         if (two && !stream_block2<DT, ACC>(ta, tb, blob, h, pa, pb, lane)) continue;
                         // one frame left, or a non-finite pixel somewhere: frame by frame
@@ -587,8 +589,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_bstream_kernel(const 
                     mbar_arrive(img_empty + sa);
                     if (two) mbar_arrive(img_empty + sb);
                 }
-                firstb -= d.w % kStreamCons;
-                if (firstb < 0) firstb += kStreamCons;
+                firstb -= d.w % kBatchCons;
+                if (firstb < 0) firstb += kBatchCons;
             }
             if (lane == 0) mbar_arrive(mat_empty + mr.stage);
             mr.next(p.mat_stages);
@@ -741,7 +743,7 @@ int launch_bstream(ai_ctx *ctx, const CUtensorMap &map, const BatchParams &p, si
         configured_device = ctx->device;
     }
     ai_prof_begin(ctx, st);
-    tiled_bstream_kernel<DT, ACC><<<grid, kStreamThreads, smem, st>>>(map, p);
+    tiled_bstream_kernel<DT, ACC><<<grid, kBatchThreads, smem, st>>>(map, p);
     ai_prof_end(ctx, st);
     AI_CUDA(ctx, cudaGetLastError());
     return AI_OK;
