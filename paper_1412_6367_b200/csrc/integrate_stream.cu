@@ -136,6 +136,36 @@ __device__ __forceinline__ void stream_finish_block(Accum<ACC> &S, Accum<ACC> &C
     if (m.x < 0) store_partial<ACC>(part_f, m.x & kMetaSlotMask, S, C, TRACK, (double)__int_as_float(m.y));
 }
 
+// Kahan mode, cheaper epilogue: a lane's four compensated sums are carried over to ONE double (s - c is exact in
+// fp64), the lanes of a run are added in fp64 (exact to 2^-53: nothing the fp32 two-sum merge kept is lost) and the
+// run's total goes out as the same (hi, lo) float pair.  A third of the instructions of the fp32 merges.
+__device__ __forceinline__ double kahan_total_d(const AccumQ<AI_ACC_F32_KAHAN> &q)
+{
+    return (((double)q.a.s - (double)q.a.c) + ((double)q.b.s - (double)q.b.c)) +
+           (((double)q.c.s - (double)q.c.c) + ((double)q.d.s - (double)q.d.c));
+}
+template <bool TRACK>
+__device__ __forceinline__ void stream_finish_d(double S, double C, const int2 &m, int rounds, void *part_f)
+{
+    const int rem = (m.x >> 24) & 31;
+    for (int r = 0; r < rounds; ++r) {
+        const int d = 1 << r;
+        const double S_o = __shfl_down_sync(AI_FULL_MASK, S, d);
+        double C_o = 0.0;
+        if constexpr (TRACK) C_o = __shfl_down_sync(AI_FULL_MASK, C, d);
+        if (rem >= d) {
+            S += S_o;
+            if constexpr (TRACK) C += C_o;
+        }
+    }
+    if (m.x < 0) {
+        if constexpr (!TRACK) C = (double)__int_as_float(m.y);       // every pixel valid: the build-time coefficient sum
+        const float s_hi = (float)S, c_hi = (float)C;
+        reinterpret_cast<float4 *>(part_f)[m.x & kMetaSlotMask] =
+            make_float4(s_hi, (float)(S - (double)s_hi), c_hi, (float)(C - (double)c_hi));
+    }
+}
+
 // One block of 32 slices against the staged tile: lane = slice, two steps (8 entries) per trip, the loads of the next
 // trip issued before the current one is consumed.  Blocks hold an even number of steps (build_sliced.cu) and the
 // stage has slack behind the blob, so the look-ahead needs no predicate.  Float frames are not screened: a
@@ -161,11 +191,19 @@ __device__ __noinline__ bool stream_block(unsigned rebase, const unsigned char *
         accumulate4<ACC, false>(c1, v1, S2, C2);
         c0 = n0; c1 = n1; x0 = y0; x1 = y1;
     }
-    Accum<ACC> S = S2.total(), C = C2.total();
-    if constexpr (DT == AI_F32) {
-        if (__any_sync(AI_FULL_MASK, !finite_f((float)S.s))) return true;
+    if constexpr (ACC == AI_ACC_F32_KAHAN) {
+        const double S = kahan_total_d(S2);
+        if constexpr (DT == AI_F32) {
+            if (__any_sync(AI_FULL_MASK, !finite_f((float)S))) return true;
+        }
+        stream_finish_d<false>(S, 0.0, m, rounds, part_f);
+    } else {
+        Accum<ACC> S = S2.total(), C = C2.total();
+        if constexpr (DT == AI_F32) {
+            if (__any_sync(AI_FULL_MASK, !finite_f((float)S.s))) return true;
+        }
+        stream_finish_block<ACC, false>(S, C, m, rounds, part_f);
     }
-    stream_finish_block<ACC, false>(S, C, m, rounds, part_f);
     return false;
 }
 
@@ -192,8 +230,12 @@ __device__ __noinline__ void stream_block_tracked(unsigned rebase, const unsigne
         accumulate4<ACC, true>(c1, v1, S2, C2);
         c0 = n0; c1 = n1; x0 = y0; x1 = y1;
     }
-    Accum<ACC> S = S2.total(), C = C2.total();
-    stream_finish_block<ACC, true>(S, C, m, rounds, part_f);
+    if constexpr (ACC == AI_ACC_F32_KAHAN) {
+        stream_finish_d<true>(kahan_total_d(S2), kahan_total_d(C2), m, rounds, part_f);
+    } else {
+        Accum<ACC> S = S2.total(), C = C2.total();
+        stream_finish_block<ACC, true>(S, C, m, rounds, part_f);
+    }
 }
 
 // Batches (H6): the same block against the tiles of TWO frames at once.  Coefficients and positions are loaded and
@@ -223,13 +265,22 @@ __device__ __noinline__ bool stream_block2(unsigned tile_a, unsigned tile_b, con
         accumulate4<ACC, false>(c1, b1, SB, C2);
         c0 = n0; c1 = n1; x0 = y0; x1 = y1;
     }
-    Accum<ACC> Sa = SA.total(), Sb = SB.total(), C = C2.total();
-    if constexpr (DT == AI_F32) {
-        if (__any_sync(AI_FULL_MASK, !finite_f((float)Sa.s) || !finite_f((float)Sb.s))) return true;
+    if constexpr (ACC == AI_ACC_F32_KAHAN) {
+        const double Sa = kahan_total_d(SA), Sb = kahan_total_d(SB);
+        if constexpr (DT == AI_F32) {
+            if (__any_sync(AI_FULL_MASK, !finite_f((float)Sa) || !finite_f((float)Sb))) return true;
+        }
+        stream_finish_d<false>(Sa, 0.0, m, rounds, part_a);
+        stream_finish_d<false>(Sb, 0.0, m, rounds, part_b);
+    } else {
+        Accum<ACC> Sa = SA.total(), Sb = SB.total(), C = C2.total();
+        if constexpr (DT == AI_F32) {
+            if (__any_sync(AI_FULL_MASK, !finite_f((float)Sa.s) || !finite_f((float)Sb.s))) return true;
+        }
+        Accum<ACC> Ca = C;
+        stream_finish_block<ACC, false>(Sa, Ca, m, rounds, part_a);
+        stream_finish_block<ACC, false>(Sb, C, m, rounds, part_b);
     }
-    Accum<ACC> Ca = C;
-    stream_finish_block<ACC, false>(Sa, Ca, m, rounds, part_a);
-    stream_finish_block<ACC, false>(Sb, C, m, rounds, part_b);
     return false;
 }
 

@@ -443,6 +443,27 @@ def test_batch_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, nf
     integ.close()
 
 
+def test_batch_equals_single_frame_calls_bit_for_bit(torch, B, oracle, workloads):
+    """BASELINE.json configs[1] frames through ai_integrate1d_batch (the launch bench.py's `batch_cfg2_64_frames`
+    times): every frame's profiles equal, bit for bit, what ai_integrate1d gives for it (same accumulation order in
+    both kernels), and a sampled frame matches the oracle."""
+    cfg = workloads.CONFIGS["cfg2"]
+    base = workloads.make_frame(cfg).image
+    frames = np.stack([base * np.float32(s) for s in (1.0, 0.5, 2.0, 0.75, 3.0)])
+    dev = torch.from_numpy(frames).cuda()
+    integ = B.Integrator(cfg)
+    bi, bs, bc = integ.integrate1d_batch(dev)
+    torch.cuda.synchronize()
+    for f in range(frames.shape[0]):
+        i, s, c = integ.integrate1d(dev[f])
+        torch.cuda.synchronize()
+        assert torch.equal(bi[f], i) and torch.equal(bs[f], s) and torch.equal(bc[f], c), f"frame {f}"
+    want = _oracle_profile(oracle, cfg, workloads.Frame(image=frames[3]))
+    got = {"intensity": bi[3].cpu().numpy(), "sum_signal": bs[3].cpu().numpy(), "count": bc[3].cpu().numpy()}
+    assert_profile(got, want, what="cfg2 batch frame 3")
+    integ.close()
+
+
 def test_batch_with_mask_takes_the_general_kernel(torch, B, oracle, workloads):
     cfg = workloads.tiny_config(130, 200, center_x=60.0, center_y=70.0, unit=workloads.TTH_DEG, npt=150,
                                 distance_m=0.03, name="batch_mask")
