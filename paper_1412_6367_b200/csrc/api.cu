@@ -104,6 +104,8 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
     }
     const char *e = getenv("AZINT_NO_TMA");
     ctx->no_tma = e && e[0] == '1';
+    e = getenv("AZINT_NO_SCHEDULE");
+    ctx->no_schedule = e && e[0] == '1';
     e = getenv("AZINT_NO_PREPASS");
     ctx->no_prepass = e && e[0] == '1';
     e = getenv("AZINT_NO_STREAM");

@@ -184,6 +184,48 @@ __global__ void __launch_bounds__(256) slice_fill_kernel(const int *__restrict__
     }
 }
 
+// Bank scheduling: the ORDER in which a lane walks its entries is free (it only fixes the order of a compensated sum),
+// and the pixel positions are known here -- so choose, slot by slot (slot = step * 4 + entry of the 128-bit load), for
+// every lane of a block the not yet placed entry whose shared-memory bank the lanes before it use least in that slot.
+// Unscheduled, the 32 lanes of a gather read unrelated pixels and fall into banks at random (2.4 wavefronts per
+// gather, which makes the batched kernel shared-memory-bound).  One thread per block of the layout, greedy, one-time.
+__global__ void __launch_bounds__(64) slice_schedule_kernel(const long long *__restrict__ tile_blob_off,
+                                                            unsigned char *__restrict__ blob)
+{
+    unsigned char *tb = blob + tile_blob_off[blockIdx.x];
+    const unsigned *hdr = reinterpret_cast<const unsigned *>(tb);
+    const int nblk = (int)hdr[0];
+    for (int b = threadIdx.x; b < nblk; b += blockDim.x) {
+        const unsigned h = hdr[1 + b];
+        const int nsteps = h & 15, T = nsteps * 4;
+        unsigned char *blk = tb + (size_t)(h >> 8) * 16;
+        float *coef = reinterpret_cast<float *>(blk);                                   // [step][lane][4]
+        unsigned short *idx = reinterpret_cast<unsigned short *>(blk + (size_t)nsteps * 512);
+        for (int t = 0; t < T; ++t) {
+            unsigned char cnt[32];
+            for (int k = 0; k < 32; ++k) cnt[k] = 0;
+            for (int lane = 0; lane < 32; ++lane) {
+                int best = t, bestc = 1 << 30;
+                for (int k = t; k < T && bestc > 0; ++k) {
+                    const int at = ((k >> 2) * 32 + lane) * 4 + (k & 3);
+                    const unsigned off = idx[at];
+                    // a padding entry (coefficient 0 at position 0) reads the same address in every lane: no conflict
+                    const int c = (off == 0 && coef[at] == 0.0f) ? 0 : cnt[(off >> 2) & 31];
+                    if (c < bestc) { bestc = c; best = k; }
+                }
+                const int a = ((t >> 2) * 32 + lane) * 4 + (t & 3), z = ((best >> 2) * 32 + lane) * 4 + (best & 3);
+                const float cz = coef[z];
+                const unsigned short xz = idx[z];
+                if (best != t) {
+                    coef[z] = coef[a]; idx[z] = idx[a];
+                    coef[a] = cz; idx[a] = xz;
+                }
+                if (!(xz == 0 && cz == 0.0f)) cnt[(xz >> 2) & 31]++;
+            }
+        }
+    }
+}
+
 }  // namespace
 
 // Largest blob over all tiles for the segment lengths `seg_len` (padded): decides whether a tile height fits the
@@ -276,6 +318,10 @@ int ai_build_sliced_fill(ai_ctx *ctx, SliceScratch *sc, cudaStream_t st)
     slice_fill_kernel<<<nt, 256, 0, st>>>(sc->tile_slice_ptr, sc->tile_blob_off, sc->slice_seg, sc->slice_win,
                                           sc->slice_run, tl.seg_ptr, tl.seg_slot, tl.tcoef, tl.tidx, tl.blob);
     AI_CUDA(ctx, cudaGetLastError());
+    if (!ctx->no_schedule) {
+        slice_schedule_kernel<<<nt, 64, 0, st>>>(sc->tile_blob_off, tl.blob);
+        AI_CUDA(ctx, cudaGetLastError());
+    }
     // longest-processing-time-first order of the tiles (host sort of ntiles integers, one-time)
     std::vector<int> order(nt);
     for (int t = 0; t < nt; ++t) order[t] = t;

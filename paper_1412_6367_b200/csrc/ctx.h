@@ -155,6 +155,7 @@ struct ai_ctx {
     // measurement hook (ai_profile_enable): events around the dominant kernel of the last call
     PipeTune tune;
     bool no_tma = false;            // AZINT_NO_TMA=1: stage raw frames through registers even where TMA applies (testing)
+    bool no_schedule = false;       // AZINT_NO_SCHEDULE=1: skip the bank scheduling of the sliced layout (measurement)
     bool no_prepass = false;        // AZINT_NO_PREPASS=1: corrected single frames take the general kernel (testing)
     bool no_stream = false;         // AZINT_NO_STREAM=1: single frames take the general pipelined kernel too (testing)
     bool profile = false, profile_valid = false;
