@@ -108,7 +108,14 @@ int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_va
  *                              intensity_b = sum_signal_b / count_b (empty_value where count_b == 0), with
  *                              v = (I - dark) / (flat * solidangle * polarization); a pixel is invalid if masked or if
  *                              its denominator is 0 / non-finite or its numerator non-finite.
- * Enqueues on `cuda_stream`; does not synchronise.  Errors: AI_EINVAL, AI_ENOTBUILT, AI_ECUDA. */
+ * Enqueues on `cuda_stream`; does not synchronise.  Errors: AI_EINVAL, AI_ENOTBUILT, AI_ECUDA.
+ * With the default layout a plain 32-bit frame is one kernel launch; correction arrays, a mask, 16-bit pixels or rows
+ * off 16-byte boundaries add one streaming pre-pass.  These kernels are launched with programmatic stream
+ * serialisation: their prologue (barriers, descriptors, the first matrix tiles -- data that only ai_build_csr writes)
+ * may overlap the tail of whatever precedes them on the stream; the frame, the correction arrays and every buffer the
+ * call writes are touched only after that predecessor has completed (griddepcontrol.wait), so ordinary stream
+ * ordering is what the caller sees.  Between calls the context keeps a corrected copy of the frame, partial sums and
+ * two counters: one context, one stream at a time. */
 int ai_integrate1d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *dark, const float *flat,
                    const float *solidangle, const float *polarization, const uint8_t *mask, float *radial,
                    float *intensity, float *sum_signal, float *count, void *cuda_stream);
