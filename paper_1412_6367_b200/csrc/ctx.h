@@ -149,6 +149,8 @@ struct ai_ctx {
     float *out2[2] = {nullptr, nullptr};
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t h2d_done[2] = {nullptr, nullptr}, slot_free[2] = {nullptr, nullptr};
+    void *stream_first = nullptr;   // HOST: descriptors of every block's first tiles, as the single-frame kernel takes them
+    int stream_first_grid = 0;
     float *corrected = nullptr;     // [height*width] corrected float32 frame (integrate_prep.cu), allocated on first use
     unsigned long long *grid_sync = nullptr;   // fused single-frame kernel: [0] arrivals at its barrier, [1] tile tickets
 

@@ -14,6 +14,8 @@
 //   - programmatic dependent launch: the next launch's prologue and first blobs overlap this launch's tail.
 // tiled_bstream_kernel: batches of plain 32-bit frames, the blob of a tile loaded once per chunk of frames, two frames
 // consumed per pass.
+#include <stdlib.h>
+
 #include "pipe_common.cuh"
 #include "tiled_common.cuh"
 
@@ -761,13 +763,20 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int tra
     p.count = a.count;
     const size_t smem = (size_t)stages * (p.img_stage_bytes + p.mat_stage_bytes) + p.hdr_bytes;
 
-    // descriptors of the first tiles of every block (host copy kept by the builder)
-    StreamFirstDescs first{};
-    for (int n = 0; n < kStreamFirst; ++n)
-        for (int b = 0; b < grid; ++b) {
-            const int w = n * grid + ((n & 1) ? grid - 1 - b : b);
-            first.d[n][b] = w < tl.ntiles ? tl.h_first_desc[w] : make_int4(0, 0, 0, 0);
-        }
+    // descriptors of the first tiles of every block (host copy kept by the builder), assembled once per context
+    if (!ctx->stream_first || ctx->stream_first_grid != grid) {
+        free(ctx->stream_first);
+        ctx->stream_first = calloc(1, sizeof(StreamFirstDescs));
+        if (!ctx->stream_first) return ai_fail(ctx, AI_ENOMEM, "first-tile descriptors");
+        StreamFirstDescs *fd = static_cast<StreamFirstDescs *>(ctx->stream_first);
+        for (int n = 0; n < kStreamFirst; ++n)
+            for (int b = 0; b < grid; ++b) {
+                const int w = n * grid + ((n & 1) ? grid - 1 - b : b);
+                fd->d[n][b] = w < tl.ntiles ? tl.h_first_desc[w] : make_int4(0, 0, 0, 0);
+            }
+        ctx->stream_first_grid = grid;
+    }
+    const StreamFirstDescs &first = *static_cast<const StreamFirstDescs *>(ctx->stream_first);
     CUtensorMap map{};
     int rc = ai_make_frame_map(ctx, a, tl.tile_h, &map);
     if (rc != AI_OK) return rc;
