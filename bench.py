@@ -365,7 +365,8 @@ def run_ours(args):
                 "single_frame_synchronous_call_fps": e2e_single_fps},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak_gbs, "unit": "GB/s",
-                     "frac": achieved / peak_gbs, "traffic": NCU_TRAFFIC_BYTES, "kernel": "tiled_stream_kernel",
+                     "frac": achieved / peak_gbs, "traffic": NCU_TRAFFIC_BYTES,
+                     "traffic_GBps": NCU_TRAFFIC_BYTES / (k_ms * 1e-3) / 1e9, "kernel": "tiled_stream_kernel",
                      "kernel_time_steps": k_steps, "traffic_source": NCU_TRAFFIC_SOURCE,
                      "kernel_ms": k_ms, "kernel_timing": "one event pair around a train of stage-1-only launches "
                      "(ai_profile_enable(ctx, 2)) on the same rotation of inputs", "algorithmic_bytes": alg_bytes,
