@@ -534,6 +534,22 @@ def test_host_frames_entry_point(torch, B, oracle, workloads):
     integ.close()
 
 
+def test_layout_info(torch, B, workloads):
+    """ai_get_layout_info: sizes of the execution layout, consistent with the canonical CSR."""
+    cfg = workloads.CONFIGS["cfg2"]
+    integ = B.Integrator(cfg)
+    info = B.ai_get_layout_info(integ.ctx)
+    nnz = B.ai_get_csr(integ.ctx)[3]
+    assert info["tile_h"] in (8, 16, 32, 64)
+    assert info["ntiles"] == ((cfg.height + info["tile_h"] - 1) // info["tile_h"]) * ((cfg.width + 63) // 64)
+    assert nnz <= info["padded_entries"] <= nnz + 4 * info["nseg"]          # segments padded to multiples of 4
+    assert 6 * info["padded_entries"] <= info["blob_bytes"] <= 8 * info["padded_entries"]   # < the CSR's 8 B/entry
+    assert info["max_blob_bytes"] * info["ntiles"] >= info["blob_bytes"]
+    assert info["nseg"] <= info["nslot"] <= 4 * info["nseg"]
+    assert info["stream_stages"] >= 2
+    integ.close()
+
+
 def test_error_codes_on_device(torch, B, workloads):
     cfg = workloads.CONFIGS["cfg1"]
     integ = B.Integrator(cfg)
