@@ -332,6 +332,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
             mbar_init(empty + s, kStreamCons);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        // the tensor map is first used after the grid dependency has resolved: have the TMA unit fetch it now
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
         // first blobs, from descriptors that came with the launch: in flight before any global load returns
         int stage = 0;
         for (int n = 0; n < npre; ++n) {
