@@ -3,9 +3,8 @@
 // kSliceMax entries and packed, 32 slices of similar length at a time, into blocks that one warp consumes with one
 // lane per slice.  A tile's blocks form one blob moved to shared memory by a single bulk copy (ctx.h).
 //
-// Order of the slices of a tile: all full slices (kSliceMax entries) in (bin, position) order, then the last, shorter
-// slice of every segment by descending length, bins ascending among equals.  Adjacent lanes of a block that belong to
-// the same segment form a run; a run yields one partial sum per frame.
+// Order of the slices of a tile: by descending length, within equal length in (bin, position) order.  Adjacent lanes of
+// a block that belong to the same segment form a run; a run yields one partial sum per frame.
 #include <stdlib.h>
 
 #include <algorithm>
@@ -20,13 +19,31 @@ struct SegLens {                 // padded segment lengths either as an array or
     __device__ int operator()(int s) const { return len ? len[s] : ptr[s + 1] - ptr[s]; }
 };
 
-// steps (groups of 4 entries) of the slice at sorted position i of a tile with nfull full slices and cnt[r] last
-// slices of r steps
-__device__ __forceinline__ int slice_steps_at(int i, int nfull, const int *cnt)
+// A segment of n entries (n a multiple of 4) is cut into k = ceil(n / kSliceMax) slices of 2q or 2q + 2 steps (a step
+// = 4 entries; blocks hold an even number of steps), the first r of them the longer ones: slices of a segment differ
+// by at most two steps and only the last one carries padding (at most one step), so blocks of slices of equal length
+// have almost no empty slots (cutting off full slices and a remainder left 8-19 % of the slots empty).
+struct SegCut {
+    int k, q, r, n;
+    __device__ __forceinline__ int steps(int w) const { return 2 * (q + (w < r ? 1 : 0)); }
+    __device__ __forceinline__ int start(int w) const { return 8 * (w * q + min(w, r)); }    // first entry of slice w
+    __device__ __forceinline__ int len(int w) const { return min(4 * steps(w), n - start(w)); }   // real entries
+};
+__device__ __forceinline__ SegCut seg_cut(int n)
 {
-    if (i < nfull) return kSliceSteps;
-    i -= nfull;
-    for (int r = kSliceSteps - 1; r >= 1; --r) {
+    SegCut c{0, 0, 0, n};
+    if (n <= 0) return c;
+    const int pairs = (n / 4 + 1) / 2;
+    c.k = (n + kSliceMax - 1) / kSliceMax;
+    c.q = pairs / c.k;
+    c.r = pairs % c.k;
+    return c;
+}
+
+// steps of the slice at sorted position i of a tile with cnt[r] slices of r steps (longest first)
+__device__ __forceinline__ int slice_steps_at(int i, const int *cnt)
+{
+    for (int r = kSliceSteps; r >= 1; --r) {
         if (i < cnt[r]) return r;
         i -= cnt[r];
     }
@@ -35,21 +52,24 @@ __device__ __forceinline__ int slice_steps_at(int i, int nfull, const int *cnt)
 
 // steps of the block whose first slice sits at sorted position i: the longest of its slices, rounded up to an even
 // number (the stream kernel consumes two steps per trip without tail predicates; the extra step is zero padding)
-__device__ __forceinline__ int block_steps_at(int i, int nfull, const int *cnt)
+__device__ __forceinline__ int block_steps_at(int i, const int *cnt)
 {
-    return (slice_steps_at(i, nfull, cnt) + 1) & ~1;
+    return (slice_steps_at(i, cnt) + 1) & ~1;
 }
 
-__device__ __forceinline__ void tile_slice_counts(const SegLens &L, int s0, int s1, int *nfull, int *cnt)
+// cnt[1 .. kSliceSteps]: slices of the tile by number of steps; returns their total
+__device__ __forceinline__ int tile_slice_counts(const SegLens &L, int s0, int s1, int *cnt)
 {
-    *nfull = 0;
-    for (int r = 0; r < kSliceSteps; ++r) cnt[r] = 0;
+    for (int r = 0; r <= kSliceSteps; ++r) cnt[r] = 0;
+    int S = 0;
     for (int s = s0; s < s1; ++s) {
-        const int n = L(s);
-        *nfull += n / kSliceMax;
-        const int r = (n % kSliceMax) / 4;
-        if (r) cnt[r]++;
+        const SegCut c = seg_cut(L(s));
+        if (c.k == 0) continue;
+        if (c.r) cnt[2 * c.q + 2] += c.r;
+        cnt[2 * c.q] += c.k - c.r;
+        S += c.k;
     }
+    return S;
 }
 
 // per tile: number of slices, number of blocks, bytes of the blob
@@ -59,13 +79,11 @@ __global__ void __launch_bounds__(64) slice_plan_kernel(int ntiles, const int *_
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ntiles) return;
-    int nfull, cnt[kSliceSteps];
-    tile_slice_counts(L, tile_seg_ptr[t], tile_seg_ptr[t + 1], &nfull, cnt);
-    int S = nfull;
-    for (int r = 1; r < kSliceSteps; ++r) S += cnt[r];
+    int cnt[kSliceSteps + 1];
+    const int S = tile_slice_counts(L, tile_seg_ptr[t], tile_seg_ptr[t + 1], cnt);
     const int nblk = (S + 31) / 32;
     int bytes = (4 * (1 + nblk) + 15) / 16 * 16;
-    for (int b = 0; b < nblk; ++b) bytes += block_steps_at(32 * b, nfull, cnt) * kBlkStepBytes + kBlkMetaBytes;
+    for (int b = 0; b < nblk; ++b) bytes += block_steps_at(32 * b, cnt) * kBlkStepBytes + kBlkMetaBytes;
     tile_nslices[t] = S;
     tile_nblk[t] = nblk;
     tile_blob_bytes[t] = bytes;
@@ -82,16 +100,18 @@ __global__ void __launch_bounds__(64) slice_assign_kernel(int ntiles, const int 
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ntiles) return;
     const int s0 = tile_seg_ptr[t], s1 = tile_seg_ptr[t + 1];
-    int nfull, cnt[kSliceSteps], part_pos[kSliceSteps];
-    tile_slice_counts(L, s0, s1, &nfull, cnt);
-    int S = nfull;
-    for (int r = kSliceSteps - 1; r >= 1; --r) { part_pos[r] = S; S += cnt[r]; }
+    int cnt[kSliceSteps + 1], pos[kSliceSteps + 1];
+    tile_slice_counts(L, s0, s1, cnt);
+    int S = 0;
+    for (int r = kSliceSteps; r >= 1; --r) { pos[r] = S; S += cnt[r]; }
     const int g0 = tile_slice_ptr[t];
-    int full_pos = 0;
     for (int s = s0; s < s1; ++s) {
-        const int n = L(s), nf = n / kSliceMax, r = (n % kSliceMax) / 4;
-        for (int k = 0; k < nf; ++k, ++full_pos) { slice_seg[g0 + full_pos] = s; slice_win[g0 + full_pos] = k; }
-        if (r) { const int i = part_pos[r]++; slice_seg[g0 + i] = s; slice_win[g0 + i] = nf; }
+        const SegCut c = seg_cut(L(s));
+        for (int w = 0; w < c.k; ++w) {                  // slices of equal length: (bin, position) order
+            const int i = pos[c.steps(w)]++;
+            slice_seg[g0 + i] = s;
+            slice_win[g0 + i] = w;
+        }
         seg_nruns[s] = 0;
     }
     // runs: adjacent lanes of one block with the same segment; run index counted per segment in slice order
@@ -118,7 +138,7 @@ __global__ void __launch_bounds__(64) slice_assign_kernel(int ntiles, const int 
         }
         int rounds = 0;
         while ((1 << rounds) < maxrun) ++rounds;
-        const int nsteps = block_steps_at(lo, nfull, cnt);
+        const int nsteps = block_steps_at(lo, cnt);
         hdr[1 + b] = ((unsigned)(off / 16) << 8) | ((unsigned)rounds << 4) | (unsigned)nsteps;
         off += nsteps * kBlkStepBytes + kBlkMetaBytes;
     }
@@ -144,25 +164,25 @@ __global__ void __launch_bounds__(256) slice_fill_kernel(const int *__restrict__
         const int nsteps = h & 15;
         unsigned char *blk = tb + (size_t)(h >> 8) * 16;
         const int s = slice_seg[g0 + i], win = slice_win[g0 + i];
-        const int base = seg_ptr[s] + kSliceMax * win;
-        const int len = min(kSliceMax, seg_ptr[s + 1] - base);
-        // Adjacent lanes that hold full slices of the same segment (windows win0, win0 + 1, ... of its entries) share
+        const SegCut c = seg_cut(seg_ptr[s + 1] - seg_ptr[s]);
+        const int len = 4 * c.steps(win);
+        const int seg_end = seg_ptr[s + 1];
+        // Adjacent lanes that hold slices of equal length of the same segment (consecutive windows of its entries) share
         // them interleaved: at step j lane q of m reads the four entries 4 * (j * m + q) ... of the m windows, so that
         // the lanes of one segment gather neighbouring pixels in the same step (different rows and columns of the tile
-        // -> different shared-memory banks) instead of pixels 32 entries, i.e. a whole number of swizzle periods, apart.
-        int src = base + step * 4;
-        if (len == kSliceMax) {
-            int q = 0, m = 1;
-            while (q < lane && slice_seg[g0 + i - q - 1] == s && slice_win[g0 + i - q - 1] == win - q - 1) ++q;
-            while (lane - q + m < 32 && i - q + m < S && slice_seg[g0 + i - q + m] == s &&
-                   seg_ptr[s + 1] - (seg_ptr[s] + kSliceMax * slice_win[g0 + i - q + m]) >= kSliceMax)
-                ++m;
-            src = seg_ptr[s] + kSliceMax * (win - q) + 4 * (step * m + q);
-        }
-        if (step * 4 < len) {      // the rest of the block stays zero: coefficient 0 at pixel 0 of the tile
-            const float4 c = *reinterpret_cast<const float4 *>(tcoef + src);
+        // -> different shared-memory banks) instead of pixels a whole slice apart.
+        int q = 0, m = 1;
+        while (q < lane && slice_seg[g0 + i - q - 1] == s && slice_win[g0 + i - q - 1] == win - q - 1 &&
+               c.steps(win - q - 1) == c.steps(win))
+            ++q;
+        while (lane - q + m < 32 && i - q + m < S && slice_seg[g0 + i - q + m] == s &&
+               slice_win[g0 + i - q + m] == win - q + m && c.steps(win - q + m) == c.steps(win))
+            ++m;
+        const int src = seg_ptr[s] + c.start(win - q) + 4 * (step * m + q);
+        if (step * 4 < len && src + 4 <= seg_end) {   // the rest stays zero: coefficient 0 at pixel 0 of the tile
+            const float4 cf = *reinterpret_cast<const float4 *>(tcoef + src);
             const ushort4 x = *reinterpret_cast<const ushort4 *>(tidx + src);
-            reinterpret_cast<float4 *>(blk)[step * 32 + lane] = c;
+            reinterpret_cast<float4 *>(blk)[step * 32 + lane] = cf;
             reinterpret_cast<ushort4 *>(blk + (size_t)nsteps * 512)[step * 32 + lane] = x;
         }
         if (step == 0) {
@@ -172,8 +192,8 @@ __global__ void __launch_bounds__(256) slice_fill_kernel(const int *__restrict__
                 const int rem = (r >> 24) & 31;
                 double sum = 0.0;      // coefficient sum of the run, fixed order: `count` when every pixel is valid
                 for (int j = 0; j <= rem; ++j) {
-                    const int bj = seg_ptr[s] + kSliceMax * slice_win[g0 + i + j];
-                    const int lj = min(kSliceMax, seg_ptr[s + 1] - bj);
+                    const int wj = slice_win[g0 + i + j];
+                    const int bj = seg_ptr[s] + c.start(wj), lj = c.len(wj);
                     for (int e = 0; e < lj; ++e) sum += (double)tcoef[bj + e];
                 }
                 m.x |= (int)0x80000000 | (seg_slot[s] + (r & kMetaSlotMask));
