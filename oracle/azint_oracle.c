@@ -172,6 +172,7 @@ int aio_integrate1d_bounds(const double *u_min, const double *u_max, int64_t npi
     double *S = (double *)calloc((size_t)nthreads * npt, sizeof(double));
     double *C = (double *)calloc((size_t)nthreads * npt, sizeof(double));
     if (!S || !C) { free(S); free(C); return -2; }
+    int overflow = 0;      /* a pixel that spans more than AIO_MAX_SPLIT bins is an error here as in aio_csr (-3) */
 #ifdef _OPENMP
 #pragma omp parallel num_threads(nthreads)
 #endif
@@ -187,13 +188,20 @@ int aio_integrate1d_bounds(const double *u_min, const double *u_max, int64_t npi
             double v;
             if (!pixel_value(p, image, dark, flat, solidangle, polarization, mask, &v)) continue;
             int n = aio_split(u_min[p], u_max[p], u0, u1, npt, bins, coefs, AIO_MAX_SPLIT);
-            if (n > AIO_MAX_SPLIT) n = AIO_MAX_SPLIT;
+            if (n > AIO_MAX_SPLIT) {
+#ifdef _OPENMP
+#pragma omp atomic write
+#endif
+                overflow = 1;
+                continue;
+            }
             for (int k = 0; k < n; ++k) {
                 St[bins[k]] += coefs[k] * v;      /* weighted histogram   */
                 Ct[bins[k]] += coefs[k];          /* unweighted histogram */
             }
         }
     }
+    if (overflow) { free(S); free(C); return -3; }
     for (int t = 1; t < nthreads; ++t)
         for (int b = 0; b < npt; ++b) { S[b] += S[(size_t)t * npt + b]; C[b] += C[(size_t)t * npt + b]; }
     for (int b = 0; b < npt; ++b) {

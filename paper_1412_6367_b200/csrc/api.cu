@@ -122,6 +122,7 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
                 else if (!strcmp(key, "bis")) ctx->tune.batch_img_stages = val;
                 else if (!strcmp(key, "fl")) ctx->tune.inflight = val;
                 else if (!strcmp(key, "ss")) ctx->tune.stream_stages = val;
+                else if (!strcmp(key, "nov")) ctx->tune.no_overlap = val;
             }
             q = strchr(q, ',');
             if (q) ++q;
@@ -144,8 +145,9 @@ int ai_build_csr(ai_ctx *ctx, void *cuda_stream)
     ai_free_spans(&spans);
     if (rc != AI_OK) return rc;
     AI_CUDA(ctx, cudaMalloc(&ctx->out_dev, 3 * (size_t)ctx->npt * sizeof(float)));
-    AI_CUDA(ctx, cudaMalloc(&ctx->grid_sync, 2 * sizeof(unsigned long long)));
-    AI_CUDA(ctx, cudaMemsetAsync(ctx->grid_sync, 0, 2 * sizeof(unsigned long long), st));
+    AI_CUDA(ctx, cudaMalloc(&ctx->grid_sync, 3 * sizeof(unsigned long long)));
+    AI_CUDA(ctx, cudaMemsetAsync(ctx->grid_sync, 0, 3 * sizeof(unsigned long long), st));
+    AI_CUDA(ctx, cudaMalloc(&ctx->stream_partials, 2 * (size_t)(ctx->tl.nslot > 0 ? ctx->tl.nslot : 1) * 16));
     AI_CUDA(ctx, cudaStreamSynchronize(st));
     ctx->built = true;
     return AI_OK;
@@ -332,7 +334,7 @@ void ai_destroy(ai_ctx *ctx)
     cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
     free(tl.h_first_desc);
     free(ctx->stream_first);
-    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->corrected);
+    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->stream_partials); cudaFree(ctx->corrected);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;

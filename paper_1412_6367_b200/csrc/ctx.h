@@ -58,6 +58,7 @@ struct PipeTune {
     int batch_mat_stages = 2, batch_img_stages = kPipeMaxImgStages;
     int inflight = 0;                          // 0 = as many as there are stages
     int stream_stages = 0;                     // cap on the (tile + blob) stages of the single-frame kernel, 0 = none
+    int no_overlap = 0;                        // single-frame kernel: never stream ahead of the grid dependency
 };
 inline PipePlan ai_pipe_plan(int max_blob_bytes, int tile_h, bool batch, const PipeTune &tune = PipeTune())
 {
@@ -152,7 +153,19 @@ struct ai_ctx {
     void *stream_first = nullptr;   // HOST: descriptors of every block's first tiles, as the single-frame kernel takes them
     int stream_first_grid = 0;
     float *corrected = nullptr;     // [height*width] corrected float32 frame (integrate_prep.cu), allocated on first use
-    unsigned long long *grid_sync = nullptr;   // fused single-frame kernel: [0] arrivals at its barrier, [1] tile tickets
+    // single-frame kernel: tile-ticket counters and partial records in alternating sets (two launches of a context may
+    // be resident at a time, integrate_stream.cu)
+    unsigned long long *grid_sync = nullptr;   // [3] tile tickets, used in rotation
+    void *stream_partials = nullptr;           // [2][nslot] partial records
+    unsigned stream_launches = 0;              // single-frame launches of this context so far
+    uint64_t stream_shared_sm = 0;             // bit k: instantiation k of the kernel does NOT have an SM to itself
+    // tensor map of the last frame buffer seen by the TMA kernels (encoding one costs the host ~1-2 us per call)
+    alignas(64) unsigned char map_cache[128] = {0};
+    const void *map_image = nullptr;
+    int map_dtype = -1, map_tile_h = 0, map_nframes = 0;
+    int64_t map_pitch = 0, map_stride = 0;
+    uint64_t smem_opt_in = 0;       // bit k: kernel instantiation k was given its dynamic shared-memory size (per context:
+                                    // no function-local static state, two host threads may drive two contexts)
 
     // measurement hook (ai_profile_enable): events around the dominant kernel of the last call
     PipeTune tune;

@@ -21,6 +21,7 @@
 // With more than one frame per item the matrix stage is loaded once and reused for every frame of the item: that is
 // the batched variant that amortises the matrix read across frames.
 #include <cuda.h>
+#include <string.h>
 
 #include "pipe_common.cuh"
 #include "tiled_common.cuh"
@@ -423,22 +424,37 @@ EncodeTiledFn encode_tiled_fn()
 
 }  // namespace
 
-// (x, y, frame) view of the frames, boxes of 32 pixels x tile_h rows x 1 frame, 128-byte swizzle, zeros outside
+// (x, y, frame) view of the frames, boxes of 32 pixels x tile_h rows x 1 frame, 128-byte swizzle, zeros outside.
+// The map of the last buffer is kept in the context: a stream of calls on one buffer (or a ring of a few) pays for
+// cuTensorMapEncodeTiled once, not per call.
 int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *map)
 {
+    static_assert(sizeof(CUtensorMap) <= sizeof(ctx->map_cache), "tensor map cache too small");
+    const int64_t pitch_el = a.row_pitch ? a.row_pitch : (int64_t)ctx->width;
+    if (ctx->map_image == a.image && ctx->map_dtype == (int)a.dtype && ctx->map_tile_h == tile_h &&
+        ctx->map_nframes == a.nframes && ctx->map_pitch == pitch_el && ctx->map_stride == a.frame_stride) {
+        memcpy(map, ctx->map_cache, sizeof(CUtensorMap));
+        return AI_OK;
+    }
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return ai_fail(ctx, AI_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
     const CUtensorMapDataType dt = a.dtype == AI_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
                                  : a.dtype == AI_I32 ? CU_TENSOR_MAP_DATA_TYPE_INT32 : CU_TENSOR_MAP_DATA_TYPE_UINT32;
     const cuuint64_t dims[3] = {(cuuint64_t)ctx->width, (cuuint64_t)ctx->height, (cuuint64_t)a.nframes};
-    const cuuint64_t pitch = a.row_pitch ? (cuuint64_t)a.row_pitch : (cuuint64_t)ctx->width;
-    const cuuint64_t strides[2] = {pitch * 4, (cuuint64_t)a.frame_stride * 4};
+    const cuuint64_t strides[2] = {(cuuint64_t)pitch_el * 4, (cuuint64_t)a.frame_stride * 4};
     const cuuint32_t box[3] = {32, (cuuint32_t)tile_h, 1};
     const cuuint32_t estr[3] = {1, 1, 1};
     const CUresult r = enc(map, dt, 3, const_cast<void *>(a.image), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return ai_fail(ctx, AI_ECUDA, "cuTensorMapEncodeTiled failed with %d", (int)r);
+    memcpy(ctx->map_cache, map, sizeof(CUtensorMap));
+    ctx->map_image = a.image;
+    ctx->map_dtype = (int)a.dtype;
+    ctx->map_tile_h = tile_h;
+    ctx->map_nframes = a.nframes;
+    ctx->map_pitch = pitch_el;
+    ctx->map_stride = a.frame_stride;
     return AI_OK;
 }
 
@@ -447,11 +463,11 @@ namespace {
 template <int DT, int ACC>
 int launch_pipe(ai_ctx *ctx, const CUtensorMap &map, const PipeParams &p, size_t smem, int grid, cudaStream_t st)
 {
-    static int configured_device = -1;            // per instantiation: opt in to the large dynamic shared memory once
-    if (configured_device != ctx->device) {
+    const uint64_t bit = 1ULL << (30 + DT * 3 + ACC);      // per context and instantiation: opt in to the large
+    if (!(ctx->smem_opt_in & bit)) {                       // dynamic shared memory once
         AI_CUDA(ctx, cudaFuncSetAttribute(tiled_pipe_kernel<DT, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           kPipeSmemBudget));
-        configured_device = ctx->device;
+        ctx->smem_opt_in |= bit;
     }
     ai_prof_begin(ctx, st);
     tiled_pipe_kernel<DT, ACC><<<grid, kPipeThreads, smem, st>>>(map, p);

@@ -1,7 +1,7 @@
 // The TMA-streamed kernels of the TILED layout -- the CSR SpMV of PAPER.md:174-188 on B200.
 //
-// tiled_stream_kernel: the whole hot path of ONE frame of 32-bit pixels in one launch (the configuration the headline
-// metric is quoted on; corrected frames come here through the pre-pass of integrate_prep.cu).
+// tiled_stream_kernel: H1 + H4 of ONE frame of 32-bit pixels (the configuration the headline metric is quoted on;
+// corrected frames come here through the pre-pass of integrate_prep.cu); H5 is tiled_stage2_kernel (integrate_tiled.cu).
 //   - one persistent block per SM, 1 producer warp + kStreamCons consumer warps; float frames are gathered straight
 //     from the TMA tile, integer frames are converted at gather time ("casted from integer to float");
 //   - one ring whose stage holds a tile of the frame AND that tile's blob of the matrix, one full / empty mbarrier pair
@@ -10,8 +10,9 @@
 //     parameters (their copies leave before any global load has returned), the rest are drawn from a ticket counter;
 //   - pixel positions of two entries are rebased with one packed 16-bit add: the tile buffers live in the first 64 KB of
 //     the shared window, so a position's low half-word is its whole shared address;
-//   - H5 fused: the last blocks to arrive at a counter add the partials up (fixed order) and write the three outputs;
-//   - programmatic dependent launch: the next launch's prologue and first blobs overlap this launch's tail.
+//   - one partial record per run of the sliced layout, in the set of partials of this launch's parity;
+//   - programmatic dependent launch: along a stream of calls the next call's kernel streams while this one drains and
+//     the small finish kernel in between adds up this one's partials (see the kernel).
 // tiled_bstream_kernel: batches of plain 32-bit frames, the blob of a tile loaded once per chunk of frames, two frames
 // consumed per pass.
 #include <stdlib.h>
@@ -27,8 +28,9 @@ constexpr int kStreamThreads = 32 * (1 + kStreamCons);
 constexpr int kStreamFirst = 3;                      // descriptors per block passed by value
 constexpr int kStreamMaxGrid = 160;
 constexpr int kStreamMaxStages = 8;
-constexpr int kStreamBarBytes = 512;                 // full[8] + empty[8], block-wide state, per-stage descriptors
+constexpr int kStreamBarBytes = 512;                 // full[8] + empty[8], per-stage descriptors
 constexpr int kStreamDescOffset = 256;
+constexpr int kBatchBarBytes = 512;                  // tiled_bstream_kernel: barriers, then the item descriptors
 
 struct StreamFirstDescs {
     int4 d[kStreamFirst][kStreamMaxGrid];
@@ -43,39 +45,36 @@ struct StreamParams {
     int launch_index;            // launches of this context so far, modulo 8 (development trace only)
     int track_all;               // float frames: every block skips non-finite pixels and accumulates count
     void *partials;
-    // H5 fused behind a grid-wide barrier (every block is resident: one per SM, grid <= number of SMs)
-    unsigned long long *grid_sync;     // [0] arrivals of all launches of this context, never reset; [1] tile tickets
-    const int *bin_slot_ptr;
-    const double *range;
-    int npt;
-    float empty;
-    float *radial, *intensity, *sum_signal, *count;
+    unsigned long long *tickets;       // tile tickets of this launch (zero at its start)
+    unsigned long long *tickets_reset; // the counter the context's next launch uses: zeroed by this one
+    int full_grid;                     // one block on every SM: a block of this launch runs where the previous
+                                       // launch's block has left, so the launch before that one is complete
+    int overlap;                       // stream before the grid dependency is resolved (see the kernel)
 };
 
-// ---- development aid (-DAI_PIPE_TRACE): per (block, tile, warp) globaltimer stamps ------------------------------------
-#ifdef AI_PIPE_TRACE
-__device__ long long *g_strace = nullptr;          // [grid][16 tiles][32 warps][4]
-__device__ int g_strace_div = 1;                   // trace every g_strace_div-th tile
-__device__ __forceinline__ long long strace_now()
-{
-    long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-#define AI_STRACE_AT(row, slot, val)                                                                            \
-    do {                                                                                                        \
-        if (g_strace && (threadIdx.x & 31) == 0)                                                                \
-            g_strace[(((((size_t)p.launch_index * gridDim.x + blockIdx.x) * 16 + (row)) * 32) + (threadIdx.x >> 5)) * 4 + (slot)] = (val); \
-    } while (0)
-// tiles: every g_strace_div-th one, rows 0..13; rows 14 and 15 hold the kernel-level stamps
-#define AI_STRACE(item, slot, val)                                                                              \
-    do {                                                                                                        \
-        if ((item) % g_strace_div == 0 && (item) / g_strace_div < 14) AI_STRACE_AT((item) / g_strace_div, slot, val); \
-    } while (0)
+// ---- development aid (-DAI_STREAM_TRACE): every warp of the single-frame kernel logs (globaltimer, code) events ----------
+#ifdef AI_STREAM_TRACE
+constexpr int kTraceWarps = 32, kTraceEvents = 64;
+__device__ long long *g_strace = nullptr;          // [8 launches][grid][kTraceWarps][kTraceEvents][2]
+struct WarpTrace {
+    long long *log;
+    int n;
+    __device__ void ev(long long code)
+    {
+        if (log && (threadIdx.x & 31) == 0 && n < kTraceEvents) {
+            log[2 * n] = (long long)globaltimer_ns();
+            log[2 * n + 1] = code;
+            ++n;
+        }
+    }
+};
+#define AI_TRACE_DECL(launch_index)                                                                                   \
+    WarpTrace wtrace{g_strace ? g_strace + ((((size_t)(launch_index) * gridDim.x + blockIdx.x) * kTraceWarps +          \
+                                              (threadIdx.x >> 5)) * kTraceEvents) * 2 : nullptr, 0}
+#define AI_TRACE(code) wtrace.ev(code)
 #else
-#define AI_STRACE(item, slot, val) do { } while (0)
-#define AI_STRACE_AT(row, slot, val) do { } while (0)
-#define strace_now() 0
+#define AI_TRACE_DECL(launch_index) do { } while (0)
+#define AI_TRACE(code) do { } while (0)
 #endif
 
 // n-th tile of this block: tiles (longest first) are dealt to the blocks in snake order
@@ -300,7 +299,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
     int4 *stage_desc = reinterpret_cast<int4 *>(hdr + kStreamDescOffset);   // descriptor of the tile in each stage
     unsigned char *mat_base = hdr + p.hdr_bytes;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    AI_STRACE_AT(15, 0, strace_now());
+    AI_TRACE_DECL(p.launch_index);
+    AI_TRACE(1);
 
     // Tiles, longest first: the first npre of every block are dealt statically (snake order; their descriptors came
     // with the launch), the rest are handed out by a ticket counter to whichever block has a free stage -- the blocks
@@ -308,10 +308,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
     int npre = 0;
     while (npre < min(kStreamFirst, p.stages) && stream_item_at(npre) < p.ntiles) ++npre;
 
-    // Launch chain (programmatic dependent launch): this grid may start while the previous kernel of the stream is
-    // still running.  Nothing that kernel may still read or write is touched before griddepcontrol.wait: until then
-    // only the matrix (static since ai_build_csr) is fetched -- the blobs of the block's first tiles -- together with
-    // barriers and the tensor map; the frame is read, tickets are drawn and the partials are written after it.
     auto issue_blob = [&](int stage, const int4 &d) {
         stage_desc[stage] = d;
         mbar_arrive_expect_tx(full + stage, (uint32_t)(p.img_stage_bytes + d.y));
@@ -324,6 +320,17 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
         tma_box(tile + p.img_stage_bytes / 2, &tmap, tx * kTileW + 32, ty * p.tile_h, 0, full + stage);
     };
 
+    // Launch chain (programmatic dependent launch).  A call is two launches, this kernel (S) and the finish kernel (F,
+    // tiled_stage2_kernel: it waits for S, adds the partials of every bin up and writes the caller's outputs); both
+    // let their dependents start at once, so along a stream of calls S_k, F_k, S_k+1, F_k+1 ... the blocks of S_k+1 take
+    // the SMs as the blocks of S_k leave them (one S block per SM: registers), while F_k, a few small blocks that fit
+    // beside them, waits for the last block of S_k.
+    //   p.overlap (the grid fills the GPU and the frame is not written by the kernel right before this one): S runs
+    //     WITHOUT waiting for its predecessors.  It reads the matrix and the frame and writes only this launch's set
+    //     of partial sums and tickets (alternating sets).  Before it leaves, every block waits for the grid dependency
+    //     (free by then): S_k completes after F_k-1, so a block of S_k+1 -- resident only where a block of S_k has
+    //     left -- finds the set of partials it shares with S_k-1 read out and S_k-1's ticket counter idle.
+    //   otherwise nothing but static data (barriers, tensor map, first blobs) is touched before griddepcontrol.wait.
     if (threadIdx.x == 0) {
         // the packed rebase needs every tile buffer inside the first 64 KB of the shared window
         if (smem_u32(img_base) + (unsigned)(p.stages * p.img_stage_bytes) > 0x10000u) __trap();
@@ -332,36 +339,42 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
             mbar_init(empty + s, kStreamCons);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        // the tensor map is first used after the grid dependency has resolved: have the TMA unit fetch it now
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
-        // first blobs, from descriptors that came with the launch: in flight before any global load returns
+        if (p.full_grid && blockIdx.x == 0) {
+            // tickets of the context's next launch (last used by the launch before the previous one, complete: see
+            // above): zero before any block of that launch can exist, i.e. before this block lets dependents start
+            *p.tickets_reset = 0ULL;
+            fence_acq_rel_gpu();
+        }
+        // first blobs (and tiles), from descriptors that came with the launch: in flight before any global load returns
         int stage = 0;
         for (int n = 0; n < npre; ++n) {
             const int4 d = first.d[n][blockIdx.x];
             if (d.w == 0) continue;
-            issue_blob(stage++, d);
+            issue_blob(stage, d);
+            if (p.overlap) issue_tile(stage, d);
+            ++stage;
         }
     }
-    // static data read late in the kernel, pulled into L2 now: the descriptors of the ticketed tiles (each block its
-    // share of the array) and the slot ranges of the bins (H5)
+    // the descriptors of the ticketed tiles (each block its share of the array), pulled into L2 now
     for (int k = p.dyn_base + (blockIdx.x * kStreamThreads + threadIdx.x) * 8; k < p.ntiles; k += gridDim.x * kStreamThreads * 8)
         asm volatile("prefetch.global.L2 [%0];" ::"l"(p.blob_desc + k));
-    for (int k = threadIdx.x * 32; k <= p.npt; k += kStreamThreads * 32)
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(p.bin_slot_ptr + k));
+    __syncthreads();
     // the next kernel of the stream may be scheduled as SMs free up
     asm volatile("griddepcontrol.launch_dependents;");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    AI_STRACE_AT(14, 1, strace_now());
-    if (threadIdx.x == 0) {
-        int stage = 0;
-        for (int n = 0; n < npre; ++n) {
-            const int4 d = first.d[n][blockIdx.x];
-            if (d.w == 0) continue;
-            issue_tile(stage++, d);
+    if (!p.overlap) {
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+        if (threadIdx.x == 0) {
+            int stage = 0;
+            for (int n = 0; n < npre; ++n) {
+                const int4 d = first.d[n][blockIdx.x];
+                if (d.w == 0) continue;
+                issue_tile(stage++, d);
+            }
+            if (!p.full_grid && blockIdx.x == 0) *p.tickets_reset = 0ULL;     // everything before this launch is complete
         }
     }
-    __syncthreads();
-    AI_STRACE_AT(15, 1, strace_now());
+    AI_TRACE(2);
 
     Ring r;
     if (warp == 0) {
@@ -382,29 +395,26 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
         unsigned long long t_next = ~0ULL;
         int4 d_next = make_int4(0, 0, 0, -1);
         if (lane == 0 && nticket) {
-            const unsigned long long t0 = atomicAdd(p.grid_sync + 1, 1ULL);
-            t_next = atomicAdd(p.grid_sync + 1, 1ULL);
+            const unsigned long long t0 = atomicAdd(p.tickets, 1ULL);
+            t_next = atomicAdd(p.tickets, 1ULL);
             d_next = fetch(t0);
         }
-        int n = npre;
         while (true) {
             const int4 d = d_next;
             if (lane == 0 && nticket) {
                 d_next = fetch(t_next);
-                t_next = atomicAdd(p.grid_sync + 1, 1ULL);
+                t_next = atomicAdd(p.tickets, 1ULL);
             }
             const int nblk = __shfl_sync(AI_FULL_MASK, d.w, 0);
             if (nblk < 0) break;
             if (nblk == 0) continue;                      // tile without entries: never published
-            AI_STRACE(n, 0, strace_now());
             if (issued >= p.stages) mbar_wait(empty + r.stage, r.parity ^ 1u);
             if (lane == 0) {
                 issue_blob(r.stage, d);
                 issue_tile(r.stage, d);
             }
-            AI_STRACE(n, 1, strace_now());
+            AI_TRACE(100 + issued);
             ++issued;
-            ++n;
             r.next(p.stages);
         }
         // no tile left: a descriptor with a negative block count ends the consumers' loop
@@ -413,6 +423,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
             stage_desc[r.stage] = make_int4(0, 0, 0, -1);
             mbar_arrive(full + r.stage);
         }
+        // overlap: the block (hence the grid) completes after everything before it in the stream
+        if (p.overlap) asm volatile("griddepcontrol.wait;" ::: "memory");
     } else {
         // ===== consumers: a tile's blocks are dealt round-robin to the warps, continuing across tiles ===================
         const int cw = warp - 1;
@@ -420,9 +432,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
         for (int n = 0;; ++n) {
             // every warp waits on and arrives at every stage, also when it holds no block of the tile: no warp is
             // ever a whole phase away from a barrier
-            AI_STRACE(n, 0, strace_now());
             mbar_wait(full + r.stage, r.parity);
-            AI_STRACE(n, 1, strace_now());
+            AI_TRACE(100 + n);
             const int4 d = stage_desc[r.stage];
             if (d.w < 0) break;
             if (firstb < d.w) {
@@ -440,77 +451,15 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
                     }
                 }
                 __syncwarp();
-                AI_STRACE(n, 2, strace_now());
-                AI_STRACE(n, 3, (long long)((d.w - firstb + kStreamCons - 1) / kStreamCons));
             }
+            AI_TRACE(200 + n);
             if (lane == 0) mbar_arrive(empty + r.stage);
             firstb -= d.w % kStreamCons;
             if (firstb < 0) firstb += kStreamCons;
             r.next(p.stages);
         }
     }
-    AI_STRACE_AT(15, 2, strace_now());
-
-    // ===== H5: the last blocks to finish add up the partials ===========================================================
-    // Every block publishes its partials (block barrier, then one thread: fence + atomic arrival).  A launch adds
-    // exactly gridDim.x arrivals to the context's counter, so old / gridDim.x is the launch's generation and
-    // old % gridDim.x the block's place in the order of arrival.  All but the last `nfin` blocks to arrive leave at once
-    // -- their SMs go to the next kernel of the stream; the last ones wait for the stragglers among themselves (all
-    // blocks of the grid are resident: one per SM), then share the bins: one warp per bin, fixed summation order.
-    volatile int *fin_rank = reinterpret_cast<volatile int *>(empty + kStreamMaxStages);   // spare bytes of the header
-    const int nwarps = kStreamThreads / 32;
-    const int nfin = min((int)gridDim.x, max(1, (p.npt + nwarps - 1) / nwarps));           // one bin per warp if possible
-    unsigned long long target = 0;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        // release: the block's partials (ordered before this thread by the barrier above) are visible to whoever
-        // observes the arrival; acquire: the last block to arrive sees everybody's
-        unsigned long long old;
-        asm volatile("atom.add.acq_rel.gpu.global.u64 %0, [%1], 1;" : "=l"(old) : "l"(p.grid_sync) : "memory");
-        const int place = (int)(old % gridDim.x);
-        target = (old / gridDim.x + 1ULL) * gridDim.x;
-        if (old + 1 == target) {                                 // the last block to arrive has nothing to wait for,
-            target = 0;
-            p.grid_sync[1] = 0ULL;                               // and every producer is done: tickets start over
-        }
-        *fin_rank = place >= (int)gridDim.x - nfin ? place - ((int)gridDim.x - nfin) : -1;
-    }
-    __syncthreads();
-    const int rank = *fin_rank;
-    if (rank < 0) return;
-    // the slot ranges of the warp's first two bins are fetched while thread 0 waits for the stragglers
-    const int stride = nfin * nwarps;
-    int b = rank + nfin * warp;
-    int beg0 = 0, end0 = 0, beg1 = 0, end1 = 0;
-    if (b < p.npt) { beg0 = __ldg(p.bin_slot_ptr + b); end0 = __ldg(p.bin_slot_ptr + b + 1); }
-    if (b + stride < p.npt) { beg1 = __ldg(p.bin_slot_ptr + b + stride); end1 = __ldg(p.bin_slot_ptr + b + stride + 1); }
-    if (threadIdx.x == 0 && target) {
-        unsigned spin = 0;
-        while (true) {
-            unsigned long long now;
-            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(now) : "l"(p.grid_sync) : "memory");
-            if (now >= target) break;
-            if (++spin > (1u << 24)) __trap();               // a lost block traps instead of hanging the device
-        }
-    }
-    __syncthreads();
-    AI_STRACE_AT(15, 3, strace_now());
-    while (b < p.npt) {
-        const bool two = b + stride < p.npt;
-        const int bn = b + 2 * stride;
-        int nb0 = 0, ne0 = 0, nb1 = 0, ne1 = 0;
-        if (bn < p.npt) { nb0 = __ldg(p.bin_slot_ptr + bn); ne0 = __ldg(p.bin_slot_ptr + bn + 1); }
-        if (bn + stride < p.npt) { nb1 = __ldg(p.bin_slot_ptr + bn + stride); ne1 = __ldg(p.bin_slot_ptr + bn + stride + 1); }
-        finish_bins<ACC>(p.partials, b, beg0, end0, two, b + stride, beg1, end1, lane, p.empty, p.intensity, p.sum_signal,
-                         p.count);
-        if (lane == 0 && p.radial) {
-            const double u0 = p.range[0], delta = (p.range[1] - p.range[0]) / (double)p.npt;
-            p.radial[b] = (float)(u0 + ((double)b + 0.5) * delta);
-            if (two) p.radial[b + stride] = (float)(u0 + ((double)(b + stride) + 0.5) * delta);
-        }
-        b = bn; beg0 = nb0; end0 = ne0; beg1 = nb1; end1 = ne1;
-    }
-    AI_STRACE_AT(14, 0, strace_now());
+    AI_TRACE(9);
 }
 
 // ---- batches (H6): tiled_bstream_kernel ---------------------------------------------------------------------------------
@@ -544,7 +493,7 @@ __global__ void __launch_bounds__(kBatchThreads, 1) tiled_bstream_kernel(const _
     uint64_t *img_empty = img_full + kBatchMaxImgStages;
     uint64_t *mat_full = img_empty + kBatchMaxImgStages;
     uint64_t *mat_empty = mat_full + kBatchMaxMatStages;
-    int4 *desc_s = reinterpret_cast<int4 *>(hdr + kStreamBarBytes);
+    int4 *desc_s = reinterpret_cast<int4 *>(hdr + kBatchBarBytes);
     unsigned char *mat_base = hdr + p.hdr_bytes;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -654,15 +603,20 @@ __global__ void __launch_bounds__(kBatchThreads, 1) tiled_bstream_kernel(const _
 }
 
 template <int DT, int ACC>
-int launch_stream(ai_ctx *ctx, const CUtensorMap &map, const StreamFirstDescs &first, const StreamParams &p, size_t smem,
+int launch_stream(ai_ctx *ctx, const CUtensorMap &map, const StreamFirstDescs &first, StreamParams p, size_t smem,
                   int grid, cudaStream_t st)
 {
-    static int configured_device = -1;            // per instantiation: opt in to the large dynamic shared memory once
-    if (configured_device != ctx->device) {
+    const uint64_t bit = 1ULL << (DT * 3 + ACC);          // per context and instantiation: opt in to the large
+    if (!(ctx->smem_opt_in & bit)) {                      // dynamic shared memory once
         AI_CUDA(ctx, cudaFuncSetAttribute(tiled_stream_kernel<DT, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           kPipeSmemBudget));
-        configured_device = ctx->device;
+        // the launch chain (see the kernel) relies on ONE block of this kernel per SM
+        int per_sm = 0;
+        AI_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tiled_stream_kernel<DT, ACC>, kStreamThreads, smem));
+        if (per_sm != 1) ctx->stream_shared_sm |= bit;
+        ctx->smem_opt_in |= bit;
     }
+    if (ctx->stream_shared_sm & bit) p.full_grid = p.overlap = 0;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
@@ -692,10 +646,10 @@ int launch_stream_dt(ai_ctx *ctx, const CUtensorMap &map, const StreamFirstDescs
 
 }  // namespace
 
-#ifdef AI_PIPE_TRACE
-extern "C" int ai_debug_set_stream_trace(void *dev_buffer, int div)
+
+#ifdef AI_STREAM_TRACE
+extern "C" int ai_debug_set_stream_trace(void *dev_buffer)
 {
-    cudaMemcpyToSymbol(g_strace_div, &div, sizeof(int));
     return (int)cudaMemcpyToSymbol(g_strace, &dev_buffer, sizeof(void *));
 }
 #endif
@@ -727,12 +681,15 @@ int ai_stream_stages(const ai_ctx *ctx)
 
 // Launches the single-frame fast path when it applies (*handled = true): one frame of 32-bit pixels, no correction
 // arrays, rows on 16-byte boundaries, and at least two (tile + blob) stages fitting the shared memory of an SM.
-// The kernel is the whole hot path of the frame: stage 1 and, behind a grid barrier, H5 (no second launch).
-int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int track_all, cudaStream_t st, bool *handled)
+// Stage 1 of the frame (H1 + H4); the caller launches stage 2 (H5) on *partials_used.
+// image_dep: the frame is written by the kernel launched right before this one (the correction pre-pass).
+int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int track_all, int image_dep, cudaStream_t st,
+                            bool *handled, const void **partials_used)
 {
     const TiledLayout &tl = ctx->tl;
     *handled = false;
-    if (a.nframes != 1 || tl.ntiles < 1 || !tl.blob || !tl.h_first_desc || !ctx->grid_sync || ctx->no_tma || ctx->no_stream)
+    if (a.nframes != 1 || tl.ntiles < 1 || !tl.blob || !tl.h_first_desc || !ctx->grid_sync || !ctx->stream_partials ||
+        ctx->no_tma || ctx->no_stream)
         return AI_OK;
     const bool plain = !a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask;
     const bool is32 = a.dtype == AI_F32 || a.dtype == AI_I32 || a.dtype == AI_U32;
@@ -749,20 +706,16 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int tra
     p.tile_h = tl.tile_h;
     p.ntiles = tl.ntiles;
     p.nslot = tl.nslot;
-    p.partials = ctx->partials;
+    // alternating sets of partial sums, three ticket counters in rotation: see the kernel
+    const unsigned seq = ctx->stream_launches;
+    p.partials = static_cast<char *>(ctx->stream_partials) + (size_t)(seq & 1) * (size_t)(tl.nslot > 0 ? tl.nslot : 1) * 16;
     p.dyn_base = (p.stages < kStreamFirst ? p.stages : kStreamFirst) * grid;
     p.track_all = track_all;
-    static unsigned launches = 0;                  // development trace only: which of 8 trace buffers the launch writes
-    p.launch_index = launches++ & 7;
-    p.grid_sync = ctx->grid_sync;
-    p.bin_slot_ptr = tl.bin_slot_ptr;
-    p.range = ctx->d_range;
-    p.npt = ctx->npt;
-    p.empty = ctx->empty_value;
-    p.radial = a.radial;
-    p.intensity = a.intensity;
-    p.sum_signal = a.sum_signal;
-    p.count = a.count;
+    p.launch_index = (int)(ctx->stream_launches & 7);   // development trace only: which of 8 trace buffers the launch writes
+    p.tickets = ctx->grid_sync + seq % 3;
+    p.tickets_reset = ctx->grid_sync + (seq + 1) % 3;
+    p.full_grid = grid == sms;
+    p.overlap = p.full_grid && !image_dep && !ctx->tune.no_overlap;
     const size_t smem = (size_t)stages * (p.img_stage_bytes + p.mat_stage_bytes) + p.hdr_bytes;
 
     // descriptors of the first tiles of every block (host copy kept by the builder), assembled once per context
@@ -789,7 +742,11 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int tra
     case AI_U32: rc = launch_stream_dt<AI_U32>(ctx, map, first, p, smem, grid, st); break;
     default: break;
     }
-    if (rc == AI_OK) *handled = true;
+    if (rc == AI_OK) {
+        *handled = true;
+        *partials_used = p.partials;
+        ++ctx->stream_launches;
+    }
     return rc;
 }
 
@@ -798,11 +755,11 @@ namespace {
 template <int DT, int ACC>
 int launch_bstream(ai_ctx *ctx, const CUtensorMap &map, const BatchParams &p, size_t smem, int grid, cudaStream_t st)
 {
-    static int configured_device = -1;
-    if (configured_device != ctx->device) {
+    const uint64_t bit = 1ULL << (15 + DT * 3 + ACC);
+    if (!(ctx->smem_opt_in & bit)) {
         AI_CUDA(ctx, cudaFuncSetAttribute(tiled_bstream_kernel<DT, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           kPipeSmemBudget));
-        configured_device = ctx->device;
+        ctx->smem_opt_in |= bit;
     }
     ai_prof_begin(ctx, st);
     tiled_bstream_kernel<DT, ACC><<<grid, kBatchThreads, smem, st>>>(map, p);
@@ -849,7 +806,7 @@ int ai_launch_bstream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaSt
     const int items_max = (p.nitems + grid - 1) / grid;
     p.img_stage_bytes = tl.tile_h * kTileW * 4;
     p.mat_stage_bytes = ai_align_up(tl.max_blob_bytes + 1024, 1024);
-    p.hdr_bytes = ai_align_up(kStreamBarBytes + 16 * items_max, 1024);
+    p.hdr_bytes = ai_align_up(kBatchBarBytes + 16 * items_max, 1024);
     const int room = kPipeSmemBudget - p.hdr_bytes;
     p.mat_stages = (room - 2 * p.mat_stage_bytes) / p.img_stage_bytes >= 4 ? 2 : 1;
     p.img_stages = (room - p.mat_stages * p.mat_stage_bytes) / p.img_stage_bytes;

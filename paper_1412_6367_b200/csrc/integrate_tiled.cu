@@ -15,7 +15,8 @@
 #include "tiled_common.cuh"
 
 int ai_launch_pipe_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);
-int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int track_all, cudaStream_t st, bool *handled);
+int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int track_all, int image_dep, cudaStream_t st,
+                            bool *handled, const void **partials_used);
 int ai_launch_bstream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);
 
 namespace {
@@ -127,6 +128,43 @@ __global__ void __launch_bounds__(256) tiled_stage2_kernel(const int *__restrict
                     intensity + o, sum_signal + o, count + o);
 }
 
+// H5 of the single-frame kernel (integrate_stream.cu): the same sums in the same order, shaped for the launch chain --
+// at most one small block per SM (4 warps, registers capped so that it fits beside a block of the stream kernel), every
+// warp taking bins in a grid-wide stride.  All its blocks become resident and let their dependents go while the stream
+// kernel before them is still running; they wait for it, add up, and leave.
+constexpr int kFinishThreads = 128;
+template <int ACC>
+__global__ void __launch_bounds__(kFinishThreads, 10) tiled_finish_kernel(const int *__restrict__ bin_slot_ptr, int npt,
+                                                                           const void *partials,
+                                                                           const double *__restrict__ range, float empty,
+                                                                           float *__restrict__ radial,
+                                                                           float *__restrict__ intensity,
+                                                                           float *__restrict__ sum_signal,
+                                                                           float *__restrict__ count)
+{
+    const int lane = threadIdx.x & 31, nw = gridDim.x * (kFinishThreads / 32);
+    int b = blockIdx.x * (kFinishThreads / 32) + (threadIdx.x >> 5);
+    int beg = 0, end = 0;
+    if (b < npt) {
+        beg = __ldg(bin_slot_ptr + b);
+        end = __ldg(bin_slot_ptr + b + 1);
+    }
+    const double u0 = radial ? range[0] : 0.0, delta = radial ? (range[1] - range[0]) / (double)npt : 0.0;
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    while (b < npt) {
+        const int bn = b + nw;
+        int nbeg = 0, nend = 0;
+        if (bn < npt) {
+            nbeg = __ldg(bin_slot_ptr + bn);
+            nend = __ldg(bin_slot_ptr + bn + 1);
+        }
+        finish_bin<ACC>(partials, beg, end, lane, empty, intensity + b, sum_signal + b, count + b);
+        if (lane == 0 && radial) radial[b] = (float)(u0 + ((double)b + 0.5) * delta);
+        b = bn; beg = nbeg; end = nend;
+    }
+}
+
 template <int DT, int ACC>
 int launch_simple(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st)
 {
@@ -190,6 +228,36 @@ int launch_stage2(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
     return AI_OK;
 }
 
+int launch_finish(ai_ctx *ctx, const FrameArgs &a, const void *partials, cudaStream_t st)
+{
+    const TiledLayout &tl = ctx->tl;
+    const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
+    const int wpb = kFinishThreads / 32;
+    int grid = (ctx->npt + wpb - 1) / wpb;
+    if (grid > sms) grid = sms;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kFinishThreads);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+#define AI_FIN(ACC)                                                                                                   \
+    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, tiled_finish_kernel<ACC>, (const int *)tl.bin_slot_ptr, ctx->npt, partials,  \
+                                    (const double *)ctx->d_range, ctx->empty_value, a.radial, a.intensity,           \
+                                    a.sum_signal, a.count))
+    switch (ctx->accum) {
+    case AI_ACC_F32_KAHAN: AI_FIN(AI_ACC_F32_KAHAN); break;
+    case AI_ACC_F32_PLAIN: AI_FIN(AI_ACC_F32_PLAIN); break;
+    default: AI_FIN(AI_ACC_F64); break;
+    }
+#undef AI_FIN
+    return AI_OK;
+}
+
 bool aligned(const void *p, size_t a) { return p == nullptr || (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
 }  // namespace
@@ -198,13 +266,17 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 {
     const TiledLayout &tl = ctx->tl;
     const size_t need = (size_t)(tl.nslot > 0 ? tl.nslot : 1) * 16 * a.nframes;
-    if (ctx->partials_bytes < need) {
+    // partial records of the two-launch paths (the single-frame kernel has its own): grown on demand, which
+    // synchronises the device -- ai_reserve_batch sizes it ahead of time
+    auto ensure_partials = [&]() -> int {
+        if (ctx->partials_bytes >= need) return AI_OK;
         if (ctx->partials) AI_CUDA(ctx, cudaFree(ctx->partials));
         ctx->partials = nullptr;
         ctx->partials_bytes = 0;
         AI_CUDA(ctx, cudaMalloc(&ctx->partials, need));
         ctx->partials_bytes = need;
-    }
+        return AI_OK;
+    };
     const size_t esz = (a.dtype == AI_U16 || a.dtype == AI_I16) ? 2 : 4;
     // 128-bit path: rows of 4 pixels never straddle the image edge and every array is aligned for 4-pixel vectors
     const int vec_ok = ctx->width % 4 == 0 && a.frame_stride % 4 == 0 && aligned(a.image, 4 * esz) &&
@@ -213,11 +285,14 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
     bool handled = false;
     int rc = AI_OK;
     if (ctx->layout != AI_LAYOUT_TILED_DIRECT) {
-        rc = ai_launch_stream_stage1(ctx, a, vec_ok, 0, st, &handled);        // one plain 32-bit frame: whole hot path
+        const void *used = nullptr;
+        rc = ai_launch_stream_stage1(ctx, a, vec_ok, 0, 0, st, &handled, &used);     // one plain 32-bit frame
         if (rc != AI_OK) return rc;
         if (handled) {
             ctx->last_launches = 1;
-            return AI_OK;
+            if (ctx->stage1_only) return AI_OK;
+            ctx->last_launches = 2;
+            return launch_finish(ctx, a, used, st);
         }
         // one frame with correction arrays, a mask, 16-bit pixels, unaligned buffers or rows that do not start on
         // 16-byte boundaries (width not a multiple of 4): H1 + H2 as a streaming pre-pass into a float32 frame with
@@ -233,18 +308,24 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
             b.dark = b.flat = b.solidangle = b.polarization = nullptr;
             b.mask = nullptr;
             const int may_be_invalid = a.dark || a.flat || a.solidangle || a.polarization || a.mask || a.dtype == AI_F32;
-            rc = ai_launch_stream_stage1(ctx, b, 1, may_be_invalid, st, &handled);
+            rc = ai_launch_stream_stage1(ctx, b, 1, may_be_invalid, 1, st, &handled, &used);
             if (rc != AI_OK) return rc;
             if (handled) {
                 ctx->last_launches = 2;
-                return AI_OK;
+                if (ctx->stage1_only) return AI_OK;
+                ctx->last_launches = 3;
+                return launch_finish(ctx, a, used, st);
             }
         }
+        rc = ensure_partials();
+        if (rc != AI_OK) return rc;
         rc = ai_launch_bstream_stage1(ctx, a, vec_ok, st, &handled);          // batch of plain 32-bit frames
         if (rc == AI_OK && !handled) rc = ai_launch_pipe_stage1(ctx, a, vec_ok, st, &handled);
     }
     if (rc != AI_OK) return rc;
     if (!handled) {
+        rc = ensure_partials();
+        if (rc != AI_OK) return rc;
         // this kernel writes one partial per segment, into the first of the segment's slots (one per run of the
         // sliced layout): the others must read as zero
         AI_CUDA(ctx, cudaMemsetAsync(ctx->partials, 0, need, st));

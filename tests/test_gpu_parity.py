@@ -411,7 +411,7 @@ def test_corrected_frame_kernels(torch, B, oracle, workloads, monkeypatch, path,
         torch.cuda.synchronize()
         got = {"intensity": i.cpu().numpy(), "sum_signal": s.cpu().numpy(), "count": c.cpu().numpy()}
         assert_profile(got, _oracle_profile(oracle, cfg, fr, empty=-2.0), what=f"{path}/{dtype}/{shape}/{acc}")
-    assert B.ai_last_launch_count(integ.ctx) == 2
+    assert B.ai_last_launch_count(integ.ctx) == (3 if path == "prepass" else 2)
     integ.close()
 
 

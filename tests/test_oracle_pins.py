@@ -197,7 +197,7 @@ def _csr_indptr_only(oracle, umin, umax, cfg, u0, u1):
     return indptr, None, None
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg4"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
 def test_bins_per_pixel_histogram(oracle, workloads, name):
     cfg = workloads.CONFIGS[name]
     ref = gold("survey_table_8a.json")[name]["bins_per_pixel"]
