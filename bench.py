@@ -1,17 +1,21 @@
 #!/usr/bin/env python
 """bench.py -- frames/s of the 1D azimuthal-integration hot path on B200 (BASELINE.json metric, configs[1]).
 
-A step is one pass of the whole per-frame hot path (cast + corrections + SpMV + ratio)
-through the C ABI (`ai_integrate1d`) on one synthetic 2048x2048 float32 gold-ring frame, 1000 bins in r (mm).
-Everything is resident in HBM when the timed region starts.  Matrix + frame (70 MB) would stay in the 126 MB L2
-from one step to the next, so the timed steps cycle through REPLICAS contexts (each owns its own copy of the matrix)
-and POOL frames: ~700 MB of inputs, five times the L2, touched round-robin -- every step reads its matrix and its
-frame from HBM.  The K steps are enqueued back to back on one stream and timed as a whole with one pair of CUDA
-events (a pair of events around a single 20 us step costs ~6 us by itself on this box; `extras` reports that
-protocol, with an explicit L2 flush before every step, next to the headline).  With N > 1 every rank runs an
-independent replica (frames are independent) and the job time is the max over ranks.
+A step is one pass of the whole per-frame hot path (cast + SpMV + ratio) through the
+C ABI (`ai_integrate1d`) on one synthetic 2048x2048 float32 gold-ring frame, 1000 bins in r (mm).  Everything is
+resident in HBM when the timed region starts.  Matrix + frame (70 MB) would stay in the 126 MB L2 from one step to
+the next, so the timed steps cycle through REPLICAS contexts (each owns its own copy of the matrix) and POOL frames:
+~590 MB of inputs, touched round-robin -- every step reads its matrix and its frame from HBM.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W]                 our arm
+Protocol: the K steps of a train are enqueued back to back on one stream and timed as a whole
+with one pair of CUDA events.  Warm-up: trains of K steps until at least max(W, SPIN_UP) steps have run and three
+trains in a row agree to 3 % -- a fresh process enqueues its first ~300 calls at half its later speed (20 us instead of
+10 us per call, whatever the GPU is doing), and there the host, not the GPU, sets the pace; that first train is
+reported as `extras.first_train_of_the_process`.  Then TRAINS trains of exactly K steps are timed and the MEDIAN train
+is the headline.  With N > 1 every rank runs an independent replica (frames are independent,
+PAPER.md:190) on its own GPU and the job time is the max over ranks.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W]                 our arm (N > 1 re-executes itself under torchrun)
     python bench.py --impl reference [--steps K] [--warmup W]          the CPU oracle, timed on the host cores
 
 Prints ONE JSON line (rank 0).  See DESIGN.md section 7 for every field.
@@ -21,6 +25,7 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import socket
 import statistics
 import subprocess
 import sys
@@ -39,9 +44,10 @@ WORKLOAD = "cfg2: 2048x2048 float32 gold-ring frame, pixel 1e-4 m, D 0.1 m, cent
 L2_FLUSH_BYTES = 256 << 20
 POOL = 16                      # distinct frames rotated through the steps
 REPLICAS = 6                   # contexts (matrix copies) rotated through the steps: working set >> L2
-# dram__bytes_read.sum + dram__bytes_write.sum of one stage-1 launch on this workload, from the committed capture
-NCU_TRAFFIC_BYTES = 72323328
-NCU_TRAFFIC_SOURCE = "profiles/r01_v9_ncu_full_stream_cfg2.txt (ncu --set full, one launch: 71.27 MB read + 1.05 MB written)"
+TRAINS = 9                     # timed trains of K steps; the median one is reported
+SPIN_UP = 600                  # calls a fresh process makes before its enqueue rate has settled (measured: ~300)
+# ncu's dram__bytes of one launch of the dominant kernel: written by the profiling run (profiles/r02_README.md)
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json")
 
 
 def measured_peaks():
@@ -50,6 +56,18 @@ def measured_peaks():
         with open(path) as f:
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def ncu_traffic(kernel, workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture, or None."""
+    try:
+        with open(TRAFFIC_FILE) as f:
+            for e in json.load(f)["captures"]:
+                if e["kernel"] == kernel and e["workload"] == workload:
+                    return int(e["dram_bytes_read"]) + int(e["dram_bytes_write"]), e.get("source", TRAFFIC_FILE)
+    except (OSError, KeyError, ValueError):
+        pass
+    return None, None
 
 
 def algorithmic_bytes(cfg, nnz, corrections=False):
@@ -108,17 +126,13 @@ class ClockSampler:
 # ----------------------------------------------------------------------------------------------------------------------
 # CPU oracle legs
 # ----------------------------------------------------------------------------------------------------------------------
-def time_oracle(cfg, image, budget_s=12.0, rows=None):
-    """Per-frame integrate of the oracle (O4-O7 forward scatter over precomputed bounds) on the host cores.
-    Returns dict(value frames/s, cores, single_thread, ms_per_frame, sample)."""
+def time_oracle(cfg, image, budget_s=12.0):
+    """Per-frame integrate of the oracle (O4-O7 forward scatter over precomputed bounds) on the host cores, whole
+    frame.  Returns dict(value frames/s, cores, ms_per_frame, sample)."""
     from oracle import oracle as O
     umin, umax = O.pixel_bounds(cfg)
     u0, u1 = O.auto_range(umin, umax)
     img = np.ascontiguousarray(image, dtype=np.float64).ravel()
-    if rows is not None:
-        n = rows * cfg.width
-        umin, umax, img = umin[:n].copy(), umax[:n].copy(), img[:n].copy()
-    frac = 1.0 if rows is None else rows / cfg.height
     ncores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else O.num_threads_available()
     res = {}
     for nt in sorted({1, ncores}):
@@ -130,11 +144,26 @@ def time_oracle(cfg, image, budget_s=12.0, rows=None):
             ts.append(time.perf_counter() - t0)
         res[nt] = statistics.median(ts)
     best = min(res, key=res.get)
-    return {"value": frac / res[best], "unit": "frames/s", "cores": best, "kind": "oracle",
-            "sample": (f"median of >=5 per-frame integrate calls (O4-O7 over precomputed bounds) on "
-                       f"{'the whole frame' if rows is None else f'{rows} of {cfg.height} image rows'} of {cfg.name}; "
-                       f"threads tried: {sorted(res)}"),
-            "ms_per_frame": {str(k): v * 1e3 / frac for k, v in res.items()}, "host_cores": ncores}
+    out = {"value": 1.0 / res[best], "unit": "frames/s", "cores": best, "kind": "oracle",
+           "sample": (f"median of >=5 per-frame integrate calls (O4-O7 over precomputed bounds) on the whole frame "
+                      f"of {cfg.name}; threads tried: {sorted(res)}"),
+           "ms_per_frame": {str(k): v * 1e3 for k, v in res.items()}, "host_cores": ncores}
+    # context: the paper's own CPU hot path is the precomputed CSR product, not the forward scatter; the
+    # same oracle matrix applied by scipy's csr_matvec (one thread) -- not the baseline, not tuned
+    try:
+        import scipy.sparse as sp
+        indptr, indices, data = O.csr(umin, umax, cfg.npt, u0, u1)
+        m = sp.csr_matrix((data, indices, indptr), shape=(cfg.npt, cfg.npix))
+        m @ img
+        ts = []
+        for _ in range(5):
+            t0 = time.perf_counter()
+            m @ img
+            ts.append(time.perf_counter() - t0)
+        out["also_scipy_csr_matvec_fps_1_thread"] = 1.0 / statistics.median(ts)
+    except Exception as e:                                     # context only
+        out["also_scipy_csr_matvec_fps_1_thread"] = f"unavailable: {e}"
+    return out
 
 
 def run_reference(args):
@@ -158,8 +187,11 @@ def run_reference(args):
     nt = min(t, key=t.get)
     total = args.steps + args.warmup
     rows = int(min(cfg.height, max(8, cfg.height * 120.0 / max(total * t[nt], 1e-9))))
-    n = rows * cfg.width
-    a, b, c = umin[:n].copy(), umax[:n].copy(), img[:n].copy()
+    # image rows strided over the whole frame (the first rows alone are a detector corner)
+    pick = np.unique(np.linspace(0, cfg.height - 1, rows).astype(np.int64))
+    rows = int(pick.size)
+    sel = (pick[:, None] * cfg.width + np.arange(cfg.width)[None, :]).ravel()
+    a, b, c = umin[sel].copy(), umax[sel].copy(), img[sel].copy()
     for _ in range(args.warmup):
         O.integrate1d_bounds(a, b, cfg.npt, u0, u1, c, nthreads=nt)
     t0 = time.perf_counter()
@@ -167,7 +199,8 @@ def run_reference(args):
         O.integrate1d_bounds(a, b, cfg.npt, u0, u1, c, nthreads=nt)
     dt = time.perf_counter() - t0
     fps = args.steps * (rows / cfg.height) / dt
-    sample = f"each step = the first {rows} of {cfg.height} image rows of one cfg2 frame (O4-O7 over precomputed bounds), {nt} thread(s)"
+    sample = (f"each step = {rows} of {cfg.height} image rows, evenly strided over one cfg2 frame (O4-O7 over precomputed "
+              f"bounds), {nt} thread(s)")
     line = {"impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -224,29 +257,54 @@ def timed_steps(torch, B, integ, frames_dev, corr, steps, warmup, flush, profile
     return total, kernel_ms, launches
 
 
-def timed_train(torch, B, integs, frames_dev, corr, steps, warmup, stage1_only=False):
+class Train:
     """K steps enqueued back to back, step k on context k % len(integs) and frame k % len(frames_dev); one event pair
-    around the whole train.  Returns (total_ms, launches).  stage1_only: only the dominant kernel of every step."""
-    outs = [it.outputs() for it in integs]
-    for it in integs:
-        B.ai_profile_enable(it.ctx, 2 if stage1_only else 0)
-    launches = 0
-    # every context runs at least twice before the timed region (its first call allocates its scratch buffers)
-    warmup = max(warmup, 2 * len(integs))
-    for k in range(warmup):
-        integs[k % len(integs)].integrate1d(frames_dev[k % len(frames_dev)], *corr, out=outs[k % len(integs)])
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for k in range(steps):
-        j = (k + warmup) % len(integs)
-        integs[j].integrate1d(frames_dev[(k + warmup) % len(frames_dev)], *corr, out=outs[j])
-        launches += B.ai_last_launch_count(integs[j].ctx)
-    e1.record()
-    torch.cuda.synchronize()
-    for it in integs:
-        B.ai_profile_enable(it.ctx, 0)
-    return e0.elapsed_time(e1), launches
+    around the whole train.  stage1_only: only the dominant kernel of every step is launched."""
+
+    def __init__(self, torch, B, integs, frames_dev, corr):
+        self.torch, self.B, self.integs, self.frames, self.corr = torch, B, integs, frames_dev, corr
+        self.outs = [it.outputs() for it in integs]
+        self.k = 0                          # position in the rotation, carried from train to train
+
+    def run(self, steps, stage1_only=False, count=False):
+        torch, B = self.torch, self.B
+        for it in self.integs:
+            B.ai_profile_enable(it.ctx, 2 if stage1_only else 0)
+        ni, nf = len(self.integs), len(self.frames)
+        launches = 0
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            j = self.k % ni
+            self.integs[j].integrate1d(self.frames[self.k % nf], *self.corr, out=self.outs[j])
+            if count:
+                launches += B.ai_last_launch_count(self.integs[j].ctx)
+            self.k += 1
+        e1.record()
+        torch.cuda.synchronize()
+        for it in self.integs:
+            B.ai_profile_enable(it.ctx, 0)
+        return e0.elapsed_time(e1), launches
+
+    def warm_up(self, steps, min_steps, stage1_only=False, max_trains=60):
+        """Warm-up trains until three in a row agree to 3 % (and at least min_steps steps have run).  Returns
+        (steps run, ms of the very first train)."""
+        done, hist, first = 0, [], None
+        for _ in range(max_trains):
+            ms, _ = self.run(steps, stage1_only)
+            first = ms if first is None else first
+            done += steps
+            hist.append(ms)
+            if done >= min_steps and len(hist) >= 3 and max(hist[-3:]) <= 1.03 * min(hist[-3:]):
+                break
+        return done, first
+
+    def measure(self, steps, trains, stage1_only=False):
+        """`trains` trains of exactly `steps` steps: (median ms, all ms, launches of the median-sized train)."""
+        res = [self.run(steps, stage1_only, count=True) for _ in range(trains)]
+        ms = sorted(r[0] for r in res)
+        return statistics.median(ms), [r[0] for r in res], res[0][1]
 
 
 def back_to_back(torch, integ, frames_dev, corr, calls, warmup=20):
@@ -264,14 +322,32 @@ def back_to_back(torch, integ, frames_dev, corr, calls, warmup=20):
     return e0.elapsed_time(e1)
 
 
+def free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` started by hand: run N ranks, one per GPU, under torchrun on this node."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__), *sys.argv[1:]]
+    os.execv(sys.executable, cmd)
+
+
 def run_ours(args):
     import torch
     from paper_1412_6367_b200 import binding as B
 
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        respawn_under_torchrun(args)
     rank, local_rank, world = dist.init()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    torch.cuda.set_device(local_rank % torch.cuda.device_count())
+    if world > torch.cuda.device_count():
+        raise SystemExit(f"{world} ranks but {torch.cuda.device_count()} GPU(s): one process per GPU, replicas do not share one")
+    torch.cuda.set_device(local_rank)
+    device = f"cuda:{local_rank}"
     if rank == 0:
         from paper_1412_6367_b200 import build as cuda_build
         cuda_build.build()                       # no-op when libazint.so is newer than its sources
@@ -283,27 +359,31 @@ def run_ours(args):
     # ---- inputs: POOL distinct seeded frames per rank, generated on the host, resident in HBM before timing -----------
     host_frames = [W.make_frame(cfg, frame_index=(0 if (rank == 0 and k == 0) else 100 * rank + k)).image
                    for k in range(POOL)]
-    frames_dev = [torch.from_numpy(f).cuda() for f in host_frames]
+    frames_dev = [torch.from_numpy(f).to(device) for f in host_frames]
     none5 = (None, None, None, None, None)
-    integs = [B.Integrator(cfg) for _ in range(REPLICAS)]
+    t0 = time.perf_counter()
+    integs = [B.Integrator(cfg, device=device) for _ in range(REPLICAS)]
+    torch.cuda.synchronize()
+    build_ms = (time.perf_counter() - t0) * 1e3 / REPLICAS
     integ = integs[0]
     nnz = B.ai_get_csr(integ.ctx)[3]
     alg_bytes = algorithmic_bytes(cfg, nnz)
-    flush = Flusher(torch)
 
     sampler = ClockSampler(torch.cuda.current_device()) if rank == 0 else None
     dist.barrier()
     torch.cuda.synchronize()
-    # headline: a train of K whole steps (stage 1 + stage 2), every step on inputs that are not in L2
-    total_ms, launches = timed_train(torch, B, integs, frames_dev, none5, args.steps, args.warmup)
-    torch.cuda.synchronize()
+    # headline: TRAINS trains of K whole steps, every step on inputs that are not in L2; median train
+    tr = Train(torch, B, integs, frames_dev, none5)
+    warm_steps, first_ms = tr.warm_up(args.steps, max(args.warmup, SPIN_UP))
     dist.barrier()
-    fps, job_ms = dist.aggregate_throughput(args.steps, total_ms)
+    med_ms, all_ms, launches = tr.measure(args.steps, TRAINS)
+    dist.barrier()
+    fps, job_ms = dist.aggregate_throughput(args.steps, med_ms)
     ms_per_step = job_ms / args.steps
-    # roofline: the same train with only the dominant kernel (stage 1, the SpMV) launched
-    k_total_ms, _ = timed_train(torch, B, integs, frames_dev, none5, args.steps, args.warmup, stage1_only=True)
-    kernel_ms = [k_total_ms / args.steps]
-    k_steps = args.steps
+    # roofline: the same trains with only the dominant kernel (the SpMV) launched
+    tr.warm_up(args.steps, 2 * REPLICAS, stage1_only=True, max_trains=10)
+    k_med_ms, k_all_ms, _ = tr.measure(args.steps, TRAINS, stage1_only=True)
+    k_ms = k_med_ms / args.steps
     # ---- end to end through the host entry point for a stream of frames: every frame is copied from pinned host
     # memory inside the timed region (the upload of frame k+1 overlaps the kernel of frame k) and its three profiles
     # are copied back to the host
@@ -336,26 +416,37 @@ def run_ours(args):
 
     extras = {}
     if world == 1 and not args.no_extras:
-        extras = run_extras(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args)
+        import bench_extras
+        extras = bench_extras.run(torch, B, integ, cfg, frames_dev, Flusher(torch), peak_gbs, args, device)
     clocks = sampler.stop() if sampler else None
 
     if rank != 0:
         dist.finalize()
         return 0
 
-    k_ms = statistics.mean(kernel_ms)
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
+    traffic, traffic_src = ncu_traffic("tiled_stream_kernel", "cfg2")
+    extras["first_train_of_the_process"] = {
+        "ms_per_step": first_ms / args.steps, "steps": args.steps,
+        "note": "the first K-step train of this process, before the warm-up trains: the host enqueues its first ~300 "
+                "calls at about half its later speed and sets the pace there, not the GPU"}
+    extras["build"] = {"ai_setup_plus_ai_build_csr_ms_per_context": build_ms,
+                       "note": f"wall time of building {REPLICAS} cfg2 contexts one after the other / {REPLICAS} "
+                               "(B1-B6: bounds, range, count, scan, fill, tiled + sliced layouts); see extras.build_vs_oracle"}
     line = {
         "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD, "layout": "tiled", "accum": "f32_kahan", "frames_in_rotation": POOL,
                    "matrix_replicas_in_rotation": REPLICAS,
-                   "warmup_steps_run": max(args.warmup, 2 * REPLICAS),
+                   "warmup_steps_run": warm_steps, "timed_trains": TRAINS,
+                   "train_ms": all_ms,
+                   "protocol": f"warm-up trains of K steps until >= {SPIN_UP} steps have run and three in a row agree to 3 % ({warm_steps} steps here), then "
+                               f"{TRAINS} trains of exactly K = {args.steps} steps, each enqueued back to back and timed "
+                               "with one CUDA event pair; value = K / median train",
                    "l2": f"inputs larger than L2: {REPLICAS} copies of the matrix and {POOL} frames "
-                         f"({(REPLICAS * 53.6 + POOL * 16.8):.0f} MB) touched round-robin, no flush kernels; steps "
-                         "enqueued back to back, one event pair around the K steps",
-                   "parallelism": f"{world} independent replica(s)"},
+                         f"({(REPLICAS * 54.4 + POOL * 16.8):.0f} MB) touched round-robin, no flush kernels",
+                   "parallelism": f"{world} independent replica(s), one process per GPU"},
         "mpix_per_s": fps * cfg.npix / 1e6,
         "clocks": clocks,
         "e2e": {"value": e2e_fps, "unit": "frames/s", "h2d_bytes_per_step": cfg.npix * 4,
@@ -365,158 +456,33 @@ def run_ours(args):
                 "single_frame_synchronous_call_fps": e2e_single_fps},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak_gbs, "unit": "GB/s",
-                     "frac": achieved / peak_gbs, "traffic": NCU_TRAFFIC_BYTES,
-                     "traffic_GBps": NCU_TRAFFIC_BYTES / (k_ms * 1e-3) / 1e9, "kernel": "tiled_stream_kernel",
-                     "kernel_time_steps": k_steps, "traffic_source": NCU_TRAFFIC_SOURCE,
-                     "kernel_ms": k_ms, "kernel_timing": "one event pair around a train of stage-1-only launches "
-                     "(ai_profile_enable(ctx, 2)) on the same rotation of inputs", "algorithmic_bytes": alg_bytes,
-                     "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
-                     "whole_step_achieved": alg_bytes / (ms_per_step * 1e-3) / 1e9},
+                     "frac": achieved / peak_gbs, "traffic": traffic,
+                     "traffic_GBps": None if traffic is None else traffic / (k_ms * 1e-3) / 1e9,
+                     "kernel": "tiled_stream_kernel", "traffic_source": traffic_src,
+                     "kernel_ms": k_ms, "kernel_train_ms": k_all_ms,
+                     "kernel_timing": f"median of {TRAINS} trains of K launches of the kernel alone "
+                                      "(ai_profile_enable(ctx, 2): no finish kernel) on the same rotation of inputs, one "
+                                      "event pair per train; consecutive launches overlap (programmatic dependent "
+                                      "launch), so this is the kernel's share of a streamed step, not its isolated latency",
+                     "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
+                     "frac_of_8TBs_nominal": achieved / 8000.0,
+                     "whole_step_achieved": alg_bytes / (ms_per_step * 1e-3) / 1e9,
+                     "whole_step_frac": alg_bytes / (ms_per_step * 1e-3) / 1e9 / peak_gbs},
     }
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = time_oracle(cfg, host_frames[0], budget_s=args.cpu_budget)
     else:
         line["cpu_baseline"] = None
-    if extras:
-        line["extras"] = extras
+    line["extras"] = extras
     print(json.dumps(line))
     dist.finalize()
     return 0
 
 
-def run_extras(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args):
-    """Context numbers beside the headline (N = 1 only): steady-state streaming, latency, the paper's own layouts, the
-    accumulator choices, the corrected and the batched paths.  Each is small; none feeds `value`."""
-    none5 = (None, None, None, None, None)
-    ex = {}
-    nnz = B.ai_get_csr(integ.ctx)[3]
-    ab = algorithmic_bytes(cfg, nnz)
-    n = max(50, min(args.steps, 500))
-    # steady state: matrix stays in L2, frames rotate
-    ms = back_to_back(torch, integ, frames_dev, none5, 2000)
-    ex["warm_back_to_back"] = {"frames_per_s": 2000 / (ms * 1e-3), "algorithmic_GBps": ab * 2000 / (ms * 1e-3) / 1e9,
-                               "note": "no L2 flush, 16 frames rotating, matrix L2-resident"}
-    # the other protocol: L2 flushed before every step, one event pair per step (and the library's events around
-    # stage 1); the cost of an event pair around a trivial kernel after the same flush is reported beside it
-    tot, _, _ = timed_steps(torch, B, integ, frames_dev, none5, n, 3, flush, profile=False)
-    x = torch.zeros(32, device="cuda")
-    ov = []
-    for _ in range(30):
-        flush()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(); x.add_(1); e1.record()
-        torch.cuda.synchronize()
-        ov.append(e0.elapsed_time(e1))
-    ex["flushed_per_step_events"] = {"frames_per_s": n / (tot * 1e-3), "ms_per_step": tot / n,
-                                     "event_pair_around_trivial_kernel_ms": statistics.median(ov),
-                                     "note": "256 MiB written + 256 MiB read before every step; events around each step"}
-    # the paper's own layouts and the other accumulators, cold (same flushed protocol, library events around the kernel)
-    for lname, layout in (("tiled", B.AI_LAYOUT_TILED), ("csr", B.AI_LAYOUT_CSR), ("lut", B.AI_LAYOUT_LUT)):
-        for aname, acc in (("kahan", B.AI_ACC_F32_KAHAN), ("f64", B.AI_ACC_F64), ("plain", B.AI_ACC_F32_PLAIN)):
-            if lname != "tiled" and aname != "kahan":
-                continue
-            integ.set_options(layout, acc)
-            steps = n if lname != "lut" else 20
-            tot, kms, _ = timed_steps(torch, B, integ, frames_dev, none5, steps, 3, flush)
-            k = statistics.mean(kms)
-            ex[f"cold_{lname}_{aname}"] = {"frames_per_s": steps / (tot * 1e-3), "kernel_ms": k,
-                                           "algorithmic_GBps": ab / (k * 1e-3) / 1e9,
-                                           "frac_of_peak": ab / (k * 1e-3) / 1e9 / peak_gbs}
-    integ.set_options()
-    # configs[2] (full preprocessing, q, 3000 bins) and configs[4] (4096^2, 5000 bins): the same train protocol as the
-    # headline -- 3 contexts and 4 frames in rotation (> L2), one event pair around the train, whole steps
-    for name in ("cfg3", "cfg5"):
-        c = W.CONFIGS[name]
-        fr = W.make_frame(c)
-        its = [B.Integrator(c) for _ in range(3)]
-        fdev = [torch.from_numpy(fr.image).cuda() for _ in range(4)]
-        corr = tuple(None if a is None else torch.from_numpy(a).cuda()
-                     for a in (fr.dark, fr.flat, fr.solidangle, fr.polarization, fr.mask))
-        ab_c = algorithmic_bytes(c, B.ai_get_csr(its[0].ctx)[3], corrections=c.corrections)
-        steps = max(20, n // 2)
-        tot, launches = timed_train(torch, B, its, fdev, corr, steps, 6)
-        ms = tot / steps
-        ex[f"train_{name}_tiled_kahan"] = {"frames_per_s": 1e3 / ms, "ms_per_step": ms, "launches_per_step": launches / steps,
-                                           "algorithmic_bytes": ab_c, "algorithmic_GBps": ab_c / (ms * 1e-3) / 1e9,
-                                           "frac_of_peak": ab_c / (ms * 1e-3) / 1e9 / peak_gbs,
-                                           "layout": B.ai_get_layout_info(its[0].ctx)}
-        for it in its:
-            it.close()
-        del corr, fdev
-    # context (SURVEY.md section 8(d) "T3"): the frame shape of the paper's Table 3 (Pilatus 1M, 981 x 1043 int32,
-    # PAPER.md:257) -- geometry is a reading (centre of the image, 172 um pixels, 0.1 m, 1000 bins in 2theta)
-    cp = W.tiny_config(981, 1043, center_x=521.5, center_y=490.5, unit=W.TTH_DEG, npt=1000, pixel_m=172e-6,
-                       distance_m=0.1, name="pilatus1m")
-    rngp = np.random.default_rng(14126367 + 9)
-    fp = [torch.from_numpy(rngp.poisson(30.0, size=(cp.height, cp.width)).astype(np.int32)).cuda() for _ in range(4)]
-    its = [B.Integrator(cp) for _ in range(6)]
-    tot, launches = timed_train(torch, B, its, fp, none5, 200, 10)
-    ex["pilatus1m_int32_table3_shape"] = {"frames_per_s": 200 / (tot * 1e-3), "ms_per_step": tot / 200,
-                                          "launches_per_step": launches / 200,
-                                          "paper_table3": "integrate kernel 0.384 ms, OpenCL total 1.445 ms, Python call "
-                                                          "2.030 ms on a GeForce Titan (PAPER.md:244-257): context, "
-                                                          "other hardware",
-                                          "note": "width 1043 is not a multiple of 4 (rows off 16-byte boundaries): the "
-                                                  "pre-pass casts and re-pitches the frame, then the single-frame kernel"}
-    for it in its:
-        it.close()
-    # the headline workload through the batched entry point: 64 frames of cfg2 (1.07 GB > L2) in one call, the
-    # matrix read once per chunk of frames (north_star: "batched path reported the same way")
-    nb = 64
-    fb = torch.stack([frames_dev[k % len(frames_dev)] for k in range(nb)])
-    outb = integ.outputs(nb)
-    for _ in range(2):
-        integ.integrate1d_batch(fb, out=outb)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(5):
-        integ.integrate1d_batch(fb, out=outb)
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / 5
-    abb = nb * cfg.npix * 4 + nnz * 8 + (cfg.npt + 1) * 4 + nb * 3 * cfg.npt * 4
-    ex["batch_cfg2_64_frames"] = {"frames_per_s": nb / (ms * 1e-3), "ms_per_batch": ms, "us_per_frame": ms * 1e3 / nb,
-                                  "mpix_per_s": nb * cfg.npix / (ms * 1e-3) / 1e6,
-                                  "algorithmic_bytes": abb, "algorithmic_GBps": abb / (ms * 1e-3) / 1e9,
-                                  "frac_of_peak": abb / (ms * 1e-3) / 1e9 / peak_gbs,
-                                  "kernel": "tiled_bstream_kernel (two frames per pass) + tiled_stage2_kernel",
-                                  "note": "ai_integrate1d_batch on 64 device-resident cfg2 frames; results are bit-identical "
-                                          "to the single-frame kernel's"}
-    del fb, outb
-    # configs[3]: 1024 int32 frames of 1024x1024 in one batched call
-    c4 = W.CONFIGS["cfg4"]
-    pool = torch.from_numpy(W.make_frames(c4, 8)).cuda()
-    frames = pool.repeat(c4.nframes // 8, 1, 1)
-    it = B.Integrator(c4)
-    out = it.outputs(c4.nframes)
-    for _ in range(2):
-        it.integrate1d_batch(frames, out=out)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    reps = 5
-    e0.record()
-    for _ in range(reps):
-        it.integrate1d_batch(frames, out=out)
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / reps
-    nnz4 = B.ai_get_csr(it.ctx)[3]
-    ab4 = c4.nframes * c4.npix * 4 + nnz4 * 8 + (c4.npt + 1) * 4 + c4.nframes * 3 * c4.npt * 4
-    ex["batch_cfg4_1024_frames"] = {"frames_per_s": c4.nframes / (ms * 1e-3), "ms_per_batch": ms,
-                                    "algorithmic_bytes": ab4, "algorithmic_GBps": ab4 / (ms * 1e-3) / 1e9,
-                                    "frac_of_peak": ab4 / (ms * 1e-3) / 1e9 / peak_gbs,
-                                    "vs_3000_fps_detector": c4.nframes / (ms * 1e-3) / 3000.0,
-                                    "kernel": "tiled_bstream_kernel (two frames per pass) + tiled_stage2_kernel",
-                                    "note": "4.3 GB of frames > L2; 8 distinct frames repeated"}
-    it.close()
-    return ex
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-extras", action="store_true")
@@ -526,8 +492,6 @@ def main():
     if args.warmup < 3:
         args.warmup = 3
     if args.impl == "reference":
-        if args.steps > 200:
-            args.steps = args.steps          # the per-step sample shrinks instead (run_reference)
         return run_reference(args)
     return run_ours(args)
 

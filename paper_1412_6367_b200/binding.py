@@ -204,11 +204,13 @@ class Integrator:
     cfg: object with height, width, pixel_m, distance_m, wavelength_m, center_x_px, center_y_px, unit, npt
     (e.g. workloads.Config).  Outputs are torch float32 CUDA tensors allocated here for convenience."""
 
-    def __init__(self, cfg, radial_range=None, device="cuda:0", layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN,
+    def __init__(self, cfg, radial_range=None, device=None, layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN,
                  empty_value=0.0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1412_6367_b200 needs a CUDA device (no CPU fallback)")
+        if device is None:                      # the matrix lives on the device that is current now; calls must be
+            device = f"cuda:{torch.cuda.current_device()}"      # made with the same device current (AI_EINVAL otherwise)
         self.torch = torch
         self._integrate1d = lib().ai_integrate1d
         self._codes = {torch.float32: AI_F32, torch.int32: AI_I32, torch.int16: AI_I16}

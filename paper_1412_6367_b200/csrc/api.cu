@@ -199,6 +199,10 @@ static int integrate(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
     if (!a.image || !a.intensity || !a.sum_signal || !a.count) return ai_fail(ctx, AI_EINVAL, "NULL image or output");
     if ((int)a.dtype < AI_F32 || (int)a.dtype > AI_U32) return ai_fail(ctx, AI_EINVAL, "bad dtype %d", (int)a.dtype);
     if (a.nframes < 1) return ai_fail(ctx, AI_EINVAL, "nframes < 1");
+    int dev = -1;
+    AI_CUDA(ctx, cudaGetDevice(&dev));
+    if (dev != ctx->device)
+        return ai_fail(ctx, AI_EINVAL, "the matrix was built on device %d, the current device is %d", ctx->device, dev);
     if (a.frame_stride < (int64_t)ctx->height * ctx->width) return ai_fail(ctx, AI_EINVAL, "frame stride < height*width");
     switch (ctx->layout) {
     case AI_LAYOUT_TILED:
@@ -334,7 +338,7 @@ void ai_destroy(ai_ctx *ctx)
     cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
     free(tl.h_first_desc);
     free(ctx->stream_first);
-    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->stream_partials); cudaFree(ctx->corrected);
+    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->stream_partials); cudaFree(ctx->corrected[0]); cudaFree(ctx->corrected[1]);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;

@@ -152,7 +152,8 @@ struct ai_ctx {
     cudaEvent_t h2d_done[2] = {nullptr, nullptr}, slot_free[2] = {nullptr, nullptr};
     void *stream_first = nullptr;   // HOST: descriptors of every block's first tiles, as the single-frame kernel takes them
     int stream_first_grid = 0;
-    float *corrected = nullptr;     // [height*width] corrected float32 frame (integrate_prep.cu), allocated on first use
+    float *corrected[2] = {nullptr, nullptr};   // corrected float32 frames (integrate_prep.cu), alternating, allocated on first use
+    unsigned prep_launches = 0;
     // single-frame kernel: tile-ticket counters and partial records in alternating sets (two launches of a context may
     // be resident at a time, integrate_stream.cu)
     unsigned long long *grid_sync = nullptr;   // [3] tile tickets, used in rotation
@@ -160,10 +161,13 @@ struct ai_ctx {
     unsigned stream_launches = 0;              // single-frame launches of this context so far
     uint64_t stream_shared_sm = 0;             // bit k: instantiation k of the kernel does NOT have an SM to itself
     // tensor map of the last frame buffer seen by the TMA kernels (encoding one costs the host ~1-2 us per call)
-    alignas(64) unsigned char map_cache[128] = {0};
-    const void *map_image = nullptr;
-    int map_dtype = -1, map_tile_h = 0, map_nframes = 0;
-    int64_t map_pitch = 0, map_stride = 0;
+    struct MapEntry {
+        alignas(64) unsigned char map[128];
+        const void *image = nullptr;
+        int dtype = -1, tile_h = 0, nframes = 0;
+        int64_t pitch = 0, stride = 0;
+    } map_cache[8];
+    unsigned map_next = 0;          // entry replaced next (round robin)
     uint64_t smem_opt_in = 0;       // bit k: kernel instantiation k was given its dynamic shared-memory size (per context:
                                     // no function-local static state, two host threads may drive two contexts)
 
@@ -221,5 +225,6 @@ struct FrameArgs {
 int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_csr(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_lut(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
-int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st);   // integrate_prep.cu
+int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, cudaStream_t st, float **out);   // integrate_prep.cu
+int ai_stream_full_grid(const ai_ctx *ctx);   // integrate_stream.cu: 1 if the single-frame kernel puts one block on every SM
 int ai_stream_stages(const ai_ctx *ctx);      // integrate_stream.cu: (tile + blob) stages of the single-frame kernel, 0 = n/a

@@ -425,17 +425,18 @@ EncodeTiledFn encode_tiled_fn()
 }  // namespace
 
 // (x, y, frame) view of the frames, boxes of 32 pixels x tile_h rows x 1 frame, 128-byte swizzle, zeros outside.
-// The map of the last buffer is kept in the context: a stream of calls on one buffer (or a ring of a few) pays for
-// cuTensorMapEncodeTiled once, not per call.
+// The maps of the last eight buffers are kept in the context: a stream of calls on a ring of buffers pays for
+// cuTensorMapEncodeTiled once per buffer, not per call.
 int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *map)
 {
-    static_assert(sizeof(CUtensorMap) <= sizeof(ctx->map_cache), "tensor map cache too small");
+    static_assert(sizeof(CUtensorMap) <= sizeof(ctx->map_cache[0].map), "tensor map cache too small");
     const int64_t pitch_el = a.row_pitch ? a.row_pitch : (int64_t)ctx->width;
-    if (ctx->map_image == a.image && ctx->map_dtype == (int)a.dtype && ctx->map_tile_h == tile_h &&
-        ctx->map_nframes == a.nframes && ctx->map_pitch == pitch_el && ctx->map_stride == a.frame_stride) {
-        memcpy(map, ctx->map_cache, sizeof(CUtensorMap));
-        return AI_OK;
-    }
+    for (auto &e : ctx->map_cache)
+        if (e.image == a.image && e.dtype == (int)a.dtype && e.tile_h == tile_h && e.nframes == a.nframes &&
+            e.pitch == pitch_el && e.stride == a.frame_stride) {
+            memcpy(map, e.map, sizeof(CUtensorMap));
+            return AI_OK;
+        }
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return ai_fail(ctx, AI_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
     const CUtensorMapDataType dt = a.dtype == AI_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
@@ -448,13 +449,14 @@ int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *
                            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return ai_fail(ctx, AI_ECUDA, "cuTensorMapEncodeTiled failed with %d", (int)r);
-    memcpy(ctx->map_cache, map, sizeof(CUtensorMap));
-    ctx->map_image = a.image;
-    ctx->map_dtype = (int)a.dtype;
-    ctx->map_tile_h = tile_h;
-    ctx->map_nframes = a.nframes;
-    ctx->map_pitch = pitch_el;
-    ctx->map_stride = a.frame_stride;
+    auto &e = ctx->map_cache[ctx->map_next++ % (sizeof(ctx->map_cache) / sizeof(ctx->map_cache[0]))];
+    memcpy(e.map, map, sizeof(CUtensorMap));
+    e.image = a.image;
+    e.dtype = (int)a.dtype;
+    e.tile_h = tile_h;
+    e.nframes = a.nframes;
+    e.pitch = pitch_el;
+    e.stride = a.frame_stride;
     return AI_OK;
 }
 

@@ -13,11 +13,15 @@ constexpr int kPrepThreads = 256;
 template <int DT>
 __global__ void __launch_bounds__(kPrepThreads) correct_frame_kernel(const void *__restrict__ img, Corrections cor,
                                                                      int64_t npix, int width, int pitch, int vec_ok,
-                                                                     float *__restrict__ out)
+                                                                     int overlap, float *__restrict__ out)
 {
-    // the single-frame kernel that follows may start its prologue (it reads `out` after its griddepcontrol.wait)
+    // Launch chain (integrate_stream.cu): the single-frame kernel that follows may start its prologue (it reads `out`
+    // after its griddepcontrol.wait).  overlap: this pass itself runs beside the stream kernel of the PREVIOUS call --
+    // it reads the caller's inputs and writes the corrected frame of its own parity, which the call before the
+    // previous one has finished reading (its stream kernel has left every SM) -- and waits for the grid dependency
+    // only before it leaves, so that completion stays transitive along the stream.
     asm volatile("griddepcontrol.launch_dependents;");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (!overlap) asm volatile("griddepcontrol.wait;" ::: "memory");
     const bool has_den = cor.flat || cor.solidangle || cor.polarization;
     const int64_t stride = (int64_t)gridDim.x * kPrepThreads;
     if (vec_ok) {
@@ -44,17 +48,21 @@ __global__ void __launch_bounds__(kPrepThreads) correct_frame_kernel(const void 
             out[y * pitch + (p - y * width)] = corrected_pixel<DT>(img, p, cor);
         }
     }
+    if (overlap) asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 }  // namespace
 
-// Writes the corrected float32 image of frame 0 of `a` into ctx->corrected (allocated on first use; row pitch = width
-// rounded up to a multiple of 4, so that frames of any width reach the single-frame kernel through a tensor map).
-int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st)
+// Writes the corrected float32 image of frame 0 of `a` into one of the context's two corrected frames (*out; they
+// alternate from call to call and are allocated on first use; row pitch = width rounded up to a multiple of 4, so that
+// frames of any width reach the single-frame kernel through a tensor map).
+int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, cudaStream_t st, float **out)
 {
     const int64_t npix = (int64_t)ctx->height * ctx->width;
     const int pitch = (ctx->width + 3) / 4 * 4;
-    if (!ctx->corrected) AI_CUDA(ctx, cudaMalloc(&ctx->corrected, (size_t)ctx->height * pitch * sizeof(float)));
+    for (int i = 0; i < 2; ++i)
+        if (!ctx->corrected[i]) AI_CUDA(ctx, cudaMalloc(&ctx->corrected[i], (size_t)ctx->height * pitch * sizeof(float)));
+    float *dst = ctx->corrected[ctx->prep_launches & 1];
     Corrections cor{a.dark, a.flat, a.solidangle, a.polarization, a.mask};
     const int vec = vec_ok && ctx->width % 4 == 0;
     const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
@@ -71,7 +79,7 @@ int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t 
     cfg.attrs = attr;
     cfg.numAttrs = 1;
 #define AI_PREP(DT) \
-    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, correct_frame_kernel<DT>, a.image, cor, npix, ctx->width, pitch, vec, ctx->corrected))
+    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, correct_frame_kernel<DT>, a.image, cor, npix, ctx->width, pitch, vec, overlap, dst))
     switch (a.dtype) {
     case AI_F32: AI_PREP(AI_F32); break;
     case AI_I32: AI_PREP(AI_I32); break;
@@ -80,5 +88,7 @@ int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t 
     case AI_U32: AI_PREP(AI_U32); break;
     }
 #undef AI_PREP
+    ++ctx->prep_launches;
+    *out = dst;
     return AI_OK;
 }

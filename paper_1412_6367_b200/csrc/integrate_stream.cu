@@ -679,6 +679,12 @@ int ai_stream_stages(const ai_ctx *ctx)
     return grid <= kStreamMaxGrid && stream_plan(ctx, grid, &p) ? p.stages : 0;
 }
 
+int ai_stream_full_grid(const ai_ctx *ctx)
+{
+    const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
+    return ai_stream_stages(ctx) >= 2 && ctx->tl.ntiles >= sms && !ctx->stream_shared_sm;
+}
+
 // Launches the single-frame fast path when it applies (*handled = true): one frame of 32-bit pixels, no correction
 // arrays, rows on 16-byte boundaries, and at least two (tile + blob) stages fitting the shared memory of an SM.
 // Stage 1 of the frame (H1 + H4); the caller launches stage 2 (H5) on *partials_used.

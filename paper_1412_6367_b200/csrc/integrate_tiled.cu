@@ -298,10 +298,11 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
         // 16-byte boundaries (width not a multiple of 4): H1 + H2 as a streaming pre-pass into a float32 frame with
         // padded rows (invalid pixels as NaN), then the same single-frame kernel
         if (a.nframes == 1 && !ctx->no_prepass && !ctx->no_stream && !ctx->no_tma && ai_stream_stages(ctx) >= 2) {
-            rc = ai_launch_correct(ctx, a, vec_ok, st);
+            float *corrected = nullptr;
+            rc = ai_launch_correct(ctx, a, vec_ok, ai_stream_full_grid(ctx) && !ctx->tune.no_overlap, st, &corrected);
             if (rc != AI_OK) return rc;
             FrameArgs b = a;
-            b.image = ctx->corrected;
+            b.image = corrected;
             b.dtype = AI_F32;
             b.row_pitch = (ctx->width + 3) / 4 * 4;
             b.frame_stride = (int64_t)ctx->height * b.row_pitch;

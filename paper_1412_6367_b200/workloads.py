@@ -70,7 +70,7 @@ CONFIGS = {
     # configs[4]: off-image beam centre, rings are arcs
     "cfg5": Config("cfg5", 4096, 4096, 75e-6, 0.2, 1e-10, -200.0, 2048.0, Q_NM, 5000, seed_index=5),
     # Pilatus-1M shape of PAPER.md:257 (Table 3); pixel size is a reading
-    "t3": Config("t3", 1043, 981, 172e-6, 0.1, 1e-10, 490.5, 521.5, TTH_DEG, 1000,
+    "t3": Config("t3", 981, 1043, 172e-6, 0.1, 1e-10, 521.5, 490.5, TTH_DEG, 1000,
                  dtype="int32", seed_index=6),
 }
 
