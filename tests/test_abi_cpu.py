@@ -10,9 +10,8 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 @pytest.fixture(scope="module")
-def B():
-    from paper_1412_6367_b200 import binding, build
-    build.build()
+def B(cuda_lib):
+    from paper_1412_6367_b200 import binding
     binding.lib()
     return binding
 

@@ -23,7 +23,7 @@ def torch():
 
 
 @pytest.fixture(scope="module")
-def B():
+def B(cuda_lib):
     from paper_1412_6367_b200 import binding
     binding.lib()
     return binding
@@ -78,9 +78,9 @@ def _ragged_cases(W):
     ]
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg1b", "cfg2", "cfg4", "ragged0", "ragged1", "ragged2", "ragged3",
-                                  "ragged4", "ragged5"])
-def test_csr_matches_oracle(torch, B, oracle, workloads, name):
+@pytest.mark.parametrize("name", ["cfg1", "cfg1b", "cfg2", "cfg3", "cfg4", "cfg5", "ragged0", "ragged1", "ragged2",
+                                  "ragged3", "ragged4", "ragged5"])
+def test_csr_matches_oracle(torch, B, oracle, workloads, parity_report, name):
     cfg = _ragged_cases(workloads)[int(name[-1])] if name.startswith("ragged") else workloads.CONFIGS[name]
     integ = B.Integrator(cfg)
     gi, gx, gd, (u0, u1) = integ.csr()
@@ -89,6 +89,8 @@ def test_csr_matches_oracle(torch, B, oracle, workloads, name):
     ora = oracle.csr(umin, umax, cfg.npt, o0, o1)
     rep = compare_csr((gi, gx, gd), ora, cfg.npix)
     print(name, rep)
+    parity_report.setdefault("csr_vs_oracle", {})[cfg.name] = dict(rep, unit=workloads.UNIT_NAMES[cfg.unit], npt=cfg.npt,
+                                                                   shape=[cfg.height, cfg.width])
     if cfg.unit == workloads.R_MM:
         # sqrt, multiply and divide are correctly rounded on both sides: the r-unit matrix must match structurally
         assert rep["ties"] == 0
@@ -116,32 +118,37 @@ def test_csr_with_explicit_range(torch, B, oracle, workloads):
 # H1-H5: one frame, every layout and accumulator
 # ----------------------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("layout", ["tiled", "direct", "csr", "lut"])
-@pytest.mark.parametrize("accum", ["kahan", "f64"])
+@pytest.mark.parametrize("accum", ["kahan", "f64", "plain"])
 @pytest.mark.parametrize("name", ["cfg1", "cfg1b", "cfg2"])
-def test_profile_parity(torch, B, oracle, workloads, name, layout, accum):
+def test_profile_parity(torch, B, oracle, workloads, parity_report, name, layout, accum):
     cfg = workloads.CONFIGS[name]
     fr = workloads.make_frame(cfg)
     integ = B.Integrator(cfg, layout=LAYOUTS[layout], accum=ACCUMS[accum])
     got = _run(torch, integ, fr, radial=True)
     want = _oracle_profile(oracle, cfg, fr)
-    worst = assert_profile(got, want, what=f"{name}/{layout}/{accum}")
+    # uncompensated fp32 is reported, not held to 1e-6 (north_star: "and reported without it")
+    worst = assert_profile(got, want, tol=1e-3 if accum == "plain" else 1e-6, what=f"{name}/{layout}/{accum}")
     assert np.allclose(got["radial"], want["radial"], rtol=2e-7)
     print(name, layout, accum, worst)
+    parity_report.setdefault("max_per_bin_relative_error", {})[f"{name}/{layout}/{accum}"] = worst
     integ.close()
 
 
 @pytest.mark.parametrize("layout", ["tiled", "direct", "csr"])
-def test_profile_parity_full_corrections_cfg3(torch, B, oracle, workloads, layout):
+@pytest.mark.parametrize("accum", ["kahan", "plain"])
+def test_profile_parity_full_corrections_cfg3(torch, B, oracle, workloads, parity_report, layout, accum):
     cfg = workloads.CONFIGS["cfg3"]
     fr = workloads.make_frame(cfg)
-    integ = B.Integrator(cfg, layout=LAYOUTS[layout])
+    integ = B.Integrator(cfg, layout=LAYOUTS[layout], accum=ACCUMS[accum])
     got = _run(torch, integ, fr)
     want = _oracle_profile(oracle, cfg, fr)
-    print("cfg3", layout, assert_profile(got, want, what=f"cfg3/{layout}"))
+    worst = assert_profile(got, want, tol=1e-3 if accum == "plain" else 1e-6, what=f"cfg3/{layout}/{accum}")
+    print("cfg3", layout, accum, worst)
+    parity_report.setdefault("max_per_bin_relative_error", {})[f"cfg3/{layout}/{accum}"] = worst
     integ.close()
 
 
-def test_profile_parity_cfg5_layouts_and_accumulators(torch, B, oracle, workloads):
+def test_profile_parity_cfg5_layouts_and_accumulators(torch, B, oracle, workloads, parity_report):
     """BASELINE.json configs[4]: compensated vs uncompensated fp32 and LUT vs CSR against the fp64 oracle."""
     cfg = workloads.CONFIGS["cfg5"]
     fr = workloads.make_frame(cfg)
@@ -152,13 +159,10 @@ def test_profile_parity_cfg5_layouts_and_accumulators(torch, B, oracle, workload
         for accum in ("kahan", "f64", "plain"):
             integ.set_options(LAYOUTS[layout], ACCUMS[accum])
             got = _run(torch, integ, fr)
-            if accum == "plain":
-                # uncompensated fp32 is reported, not held to 1e-6 (north_star: "and reported without it")
-                e = rel_err(got["intensity"], want["intensity"])
-                report[(layout, accum)] = float(e.max())
-                assert e.max() < 1e-3
-            else:
-                report[(layout, accum)] = assert_profile(got, want, what=f"cfg5/{layout}/{accum}")["intensity"]
+            # uncompensated fp32 is reported, not held to 1e-6 (north_star: "and reported without it")
+            worst = assert_profile(got, want, tol=1e-3 if accum == "plain" else 1e-6, what=f"cfg5/{layout}/{accum}")
+            report[(layout, accum)] = worst["intensity"]
+            parity_report.setdefault("max_per_bin_relative_error", {})[f"cfg5/{layout}/{accum}"] = worst
     print("cfg5 max per-bin relative error on intensity:", report)
     # the thread-per-bin LUT sums sequentially: without compensation it is the worst of the lot
     assert report[("lut", "plain")] >= report[("lut", "kahan")]

@@ -388,3 +388,20 @@ def test_threaded_variant_agrees_with_single_thread(oracle, workloads):
     r4 = oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, fr.image, nthreads=4)
     assert np.allclose(r1["sum_signal"], r4["sum_signal"], rtol=1e-13)
     assert np.allclose(r1["count"], r4["count"], rtol=1e-13)
+
+
+def test_a_pixel_spanning_more_bins_than_the_oracle_buffers_is_an_error_not_a_clamp(oracle, workloads):
+    # one pixel over 5000 bins: both the scatter and the CSR routine refuse (-3) instead of dropping contributions
+    W = workloads
+    cfg = W.tiny_config(1, 1, center_x=0.5, center_y=0.5, unit=W.R_MM, npt=5000)
+    umin, umax = oracle.pixel_bounds(cfg)
+    u0, u1 = oracle.auto_range(umin, umax)
+    with pytest.raises(ValueError, match="-3"):
+        oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, np.ones(1))
+    with pytest.raises(ValueError, match="-3"):
+        oracle.csr(umin, umax, cfg.npt, u0, u1)
+    # 4096 bins is still fine, and the pixel is spread evenly: every coefficient 1 / 4096
+    cfg = W.scaled(cfg, npt=4096)
+    r = oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, np.full(1, 3.0))
+    assert r["count"] == pytest.approx(np.full(4096, 1.0 / 4096), rel=1e-9)
+    assert r["intensity"] == pytest.approx(np.full(4096, 3.0), rel=1e-12)
