@@ -23,7 +23,10 @@
  * Parity pins (tests/test_oracle_pins.py): hand-worked split, the 2x2 worked example, mpmath brute force of every
  * coefficient on tiny images, closed-form ranges, conservation of signal and of pixel count, uniform
  * image, npt = 1 mean, scipy CSR product, Bragg ring positions, the nnz / row-length statistics of
- * SURVEY.md section 8(a).  Unpinned: behaviour for non-finite inputs and <= 1 ulp bin-edge ties (reported, not asserted).
+ * SURVEY.md section 8(a).  The bidimensional routines at the end of the file are pinned in tests/test_oracle_pins_2d.py:
+ * the sum over the azimuthal bins equals the (pinned) 1D result bin by bin, per-pixel weights sum to 1, conservation,
+ * a hand-worked 2x2 image, 4-fold symmetry, mpmath brute force of the azimuthal extents (seam, centre inside / on an
+ * edge / on a corner).  Unpinned: behaviour for non-finite inputs and <= 1 ulp bin-edge ties (reported, not asserted).
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).  No fast-math; IEEE double throughout.
  */
@@ -271,6 +274,184 @@ int64_t aio_csr(const double *u_min, const double *u_max, int64_t npix, int npt,
     }
     free(len);
     return nnz;
+}
+
+/* ==================================================================================================================
+ * Bidimensional ("cake") integration: bins = azimuthal x radial ("mono- and bidimensional integration";
+ * PAPER.md:114-116, Fig. 3: pixel splitting matters most "when the number of pixels falling into each bin is small like
+ * for example for 2D integration").  The paper gives the azimuthal coordinate chi = atan(y/x) and the
+ * bounding-box scheme; it says nothing more about the 2D case.  Readings:
+ *   - the bounding box is taken in (u, chi): the pixel's extent along each axis, split independently, so that the weight
+ *     of pixel p in bin (a, r) is  overlap_chi(a) / w_chi  *  overlap_u(r) / w_u  -- the area of the box segment over
+ *     the area of the box ("we use the area of the bounding box segment");
+ *   - chi = atan2(y, x) in (-pi, pi]; the azimuthal axis is periodic: a pixel that crosses the negative x axis is
+ *     split across the seam, a pixel that holds the beam centre strictly inside covers the full circle;
+ *   - default azimuthal range = the full circle [-pi, pi], last bin closed, bins half-open as on the radial axis;
+ *   - output layout [npt_azim][npt_rad] (row = azimuthal bin).
+ * ================================================================================================================== */
+
+/* Azimuthal extent of pixel (i, j): start chi_lo in [-pi, pi) and width w in [0, 2 pi]; the pixel covers
+ * [chi_lo, chi_lo + w], which may run past +pi (the seam).  The extent of a convex region that does not hold the origin
+ * is reached at its corners; each corner's angle is measured from the direction of the pixel centre (signed angle
+ * atan2(cross, dot)), which keeps the seam out of the way. */
+static void pixel_chi_extent(const aio_geometry *g, int i, int j, double *chi_lo, double *chi_w)
+{
+    const double pi = 3.14159265358979323846;
+    double x_lo = ((double)j - g->center_x_px) * g->pixel_x_m;
+    double x_hi = ((double)(j + 1) - g->center_x_px) * g->pixel_x_m;
+    double y_lo = ((double)i - g->center_y_px) * g->pixel_y_m;
+    double y_hi = ((double)(i + 1) - g->center_y_px) * g->pixel_y_m;
+    if (x_lo < 0.0 && x_hi > 0.0 && y_lo < 0.0 && y_hi > 0.0) {     /* beam centre strictly inside: every direction */
+        *chi_lo = -pi; *chi_w = 2.0 * pi;
+        return;
+    }
+    double xc = 0.5 * (x_lo + x_hi), yc = 0.5 * (y_lo + y_hi);
+    double chi_c = atan2(yc, xc);
+    double xs[4] = {x_lo, x_hi, x_lo, x_hi}, ys[4] = {y_lo, y_lo, y_hi, y_hi};
+    double d_min = 0.0, d_max = 0.0;
+    for (int k = 0; k < 4; ++k) {
+        if (xs[k] == 0.0 && ys[k] == 0.0) continue;       /* a corner on the beam centre has no direction */
+        double d = atan2(xc * ys[k] - yc * xs[k], xc * xs[k] + yc * ys[k]);
+        if (d < d_min) d_min = d;
+        if (d > d_max) d_max = d;
+    }
+    double lo = chi_c + d_min;
+    if (lo < -pi) lo += 2.0 * pi;
+    if (lo >= pi) lo -= 2.0 * pi;
+    *chi_lo = lo;
+    *chi_w = d_max - d_min;
+}
+
+int aio_pixel_chi_bounds(const aio_geometry *g, int height, int width, double *chi_lo, double *chi_w)
+{
+    if (!g || height < 1 || width < 1) return -1;
+    for (int i = 0; i < height; ++i)
+        for (int j = 0; j < width; ++j)
+            pixel_chi_extent(g, i, j, &chi_lo[(int64_t)i * width + j], &chi_w[(int64_t)i * width + j]);
+    return 0;
+}
+
+/* Split of the periodic interval [chi_lo, chi_lo + w] over npt bins on [c0, c1] (c1 - c0 <= 2 pi): the interval and its
+ * images shifted by -2 pi and +2 pi are each split like a radial interval (aio_split's overlap / width, the width being
+ * the pixel's whole w), and what lands in the same bin is added.  Bins come out ascending.  Returns the number of bins. */
+int aio_split_azim(double chi_lo, double w, double c0, double c1, int npt, int *bins, double *coefs, int cap)
+{
+    const double two_pi = 2.0 * 3.14159265358979323846;
+    double delta = (c1 - c0) / (double)npt;
+    int n = 0;
+    if (!(w > 0.0)) {                                   /* degenerate: a direction */
+        for (int k = -1; k <= 1; ++k) {
+            double f = (chi_lo + two_pi * k - c0) / delta;
+            if (f >= 0.0 && f <= (double)npt) {
+                int b = (int)floor(f);
+                if (b > npt - 1) b = npt - 1;
+                if (cap > 0) { bins[0] = b; coefs[0] = 1.0; }
+                return 1;
+            }
+        }
+        return 0;
+    }
+    for (int k = -1; k <= 1; ++k) {
+        double f_min = (chi_lo + two_pi * k - c0) / delta;
+        double f_max = (chi_lo + w + two_pi * k - c0) / delta;
+        double wf = f_max - f_min;                      /* as on the radial axis: width from the two bounds */
+        if (!(f_max > 0.0) || !(f_min < (double)npt)) continue;
+        double a = max2(f_min, 0.0), z = min2(f_max, (double)npt);
+        int b_first = (int)floor(a), b_last = (int)floor(z);
+        if (b_last > npt - 1) b_last = npt - 1;
+        for (int b = b_first; b <= b_last; ++b) {
+            double ov = min2(z, (double)(b + 1)) - max2(a, (double)b);
+            if (!(ov > 0.0)) continue;
+            int at = -1;
+            for (int q = 0; q < n && q < cap; ++q) if (bins[q] == b) at = q;
+            if (at >= 0) coefs[at] += ov / wf;
+            else {
+                if (n < cap) { bins[n] = b; coefs[n] = ov / wf; }
+                ++n;
+            }
+        }
+    }
+    /* ascending bins (insertion sort: a handful of entries) */
+    int m = n < cap ? n : cap;
+    for (int q = 1; q < m; ++q) {
+        int b = bins[q]; double c = coefs[q]; int t = q - 1;
+        while (t >= 0 && bins[t] > b) { bins[t + 1] = bins[t]; coefs[t + 1] = coefs[t]; --t; }
+        bins[t + 1] = b; coefs[t + 1] = c;
+    }
+    return n;
+}
+
+/* Forward scatter into azimuthal x radial bins: the 1D loop of aio_integrate1d_bounds with the weight of PAPER.md:120
+ * taken on both axes.  Outputs are [npt_azim][npt_rad]. */
+int aio_integrate2d_bounds(const double *u_min, const double *u_max, const double *chi_lo, const double *chi_w,
+                           int64_t npix, int npt_rad, double u0, double u1, int npt_azim, double c0, double c1,
+                           const double *image, const double *dark, const double *flat, const double *solidangle,
+                           const double *polarization, const uint8_t *mask, double empty_value,
+                           double *intensity, double *sum_signal, double *count)
+{
+    if (npix < 1 || npt_rad < 1 || npt_azim < 1 || !(u1 > u0) || !(c1 > c0) || !image) return -1;
+    int64_t nb = (int64_t)npt_rad * npt_azim;
+    int *br = (int *)malloc(AIO_MAX_SPLIT * sizeof(int)), *ba = (int *)malloc(AIO_MAX_SPLIT * sizeof(int));
+    double *cr = (double *)malloc(AIO_MAX_SPLIT * sizeof(double)), *ca = (double *)malloc(AIO_MAX_SPLIT * sizeof(double));
+    if (!br || !ba || !cr || !ca) { free(br); free(ba); free(cr); free(ca); return -2; }
+    for (int64_t b = 0; b < nb; ++b) { sum_signal[b] = 0.0; count[b] = 0.0; }
+    int rc = 0;
+    for (int64_t p = 0; p < npix && rc == 0; ++p) {
+        double v;
+        if (!pixel_value(p, image, dark, flat, solidangle, polarization, mask, &v)) continue;
+        int nr = aio_split(u_min[p], u_max[p], u0, u1, npt_rad, br, cr, AIO_MAX_SPLIT);
+        int na = aio_split_azim(chi_lo[p], chi_w[p], c0, c1, npt_azim, ba, ca, AIO_MAX_SPLIT);
+        if (nr > AIO_MAX_SPLIT || na > AIO_MAX_SPLIT) { rc = -3; break; }
+        for (int a = 0; a < na; ++a)
+            for (int r = 0; r < nr; ++r) {
+                int64_t b = (int64_t)ba[a] * npt_rad + br[r];
+                sum_signal[b] += ca[a] * cr[r] * v;      /* weighted histogram   */
+                count[b] += ca[a] * cr[r];               /* unweighted histogram */
+            }
+    }
+    if (rc == 0)
+        for (int64_t b = 0; b < nb; ++b) intensity[b] = count[b] > 0.0 ? sum_signal[b] / count[b] : empty_value;
+    free(br); free(ba); free(cr); free(ca);
+    return rc;
+}
+
+/* The 2D matrix in CSR form: row = a * npt_rad + r, columns (pixels) ascending.  Two calls as aio_csr. */
+int64_t aio_csr2d(const double *u_min, const double *u_max, const double *chi_lo, const double *chi_w, int64_t npix,
+                  int npt_rad, double u0, double u1, int npt_azim, double c0, double c1,
+                  int64_t *indptr, int32_t *indices, double *data)
+{
+    int64_t nb = (int64_t)npt_rad * npt_azim;
+    int *br = (int *)malloc(AIO_MAX_SPLIT * sizeof(int)), *ba = (int *)malloc(AIO_MAX_SPLIT * sizeof(int));
+    double *cr = (double *)malloc(AIO_MAX_SPLIT * sizeof(double)), *ca = (double *)malloc(AIO_MAX_SPLIT * sizeof(double));
+    int64_t *len = (int64_t *)calloc((size_t)nb + 1, sizeof(int64_t));
+    if (!br || !ba || !cr || !ca || !len) { free(br); free(ba); free(cr); free(ca); free(len); return -2; }
+    int64_t rc = 0;
+    for (int pass = 0; pass < 2 && rc == 0; ++pass) {
+        if (pass == 1) {
+            indptr[0] = 0;
+            for (int64_t b = 0; b < nb; ++b) indptr[b + 1] = indptr[b] + len[b];
+            if (!indices || !data) break;
+            for (int64_t b = 0; b < nb; ++b) len[b] = indptr[b];      /* running cursors */
+        }
+        for (int64_t p = 0; p < npix; ++p) {
+            int nr = aio_split(u_min[p], u_max[p], u0, u1, npt_rad, br, cr, AIO_MAX_SPLIT);
+            int na = aio_split_azim(chi_lo[p], chi_w[p], c0, c1, npt_azim, ba, ca, AIO_MAX_SPLIT);
+            if (nr > AIO_MAX_SPLIT || na > AIO_MAX_SPLIT) { rc = -3; break; }
+            for (int a = 0; a < na; ++a)
+                for (int r = 0; r < nr; ++r) {
+                    int64_t b = (int64_t)ba[a] * npt_rad + br[r];
+                    if (pass == 0) len[b]++;
+                    else {
+                        int64_t pos = len[b]++;
+                        indices[pos] = (int32_t)p;
+                        data[pos] = ca[a] * cr[r];
+                    }
+                }
+        }
+    }
+    if (rc == 0) rc = indptr[nb];
+    free(br); free(ba); free(cr); free(ca); free(len);
+    return rc;
 }
 
 int aio_num_threads_available(void)

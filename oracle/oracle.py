@@ -36,6 +36,13 @@ def lib():
         L.aio_csr.argtypes = [dp, dp, C.c_int64, C.c_int, C.c_double, C.c_double,
                               C.POINTER(C.c_int64), C.POINTER(C.c_int32), dp]
         L.aio_csr.restype = C.c_int64
+        L.aio_pixel_chi_bounds.argtypes = [C.POINTER(Geometry), C.c_int, C.c_int, dp, dp]
+        L.aio_split_azim.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, ip, dp, C.c_int]
+        L.aio_integrate2d_bounds.argtypes = [dp, dp, dp, dp, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int,
+                                             C.c_double, C.c_double, dp, dp, dp, dp, dp, u8p, C.c_double, dp, dp, dp]
+        L.aio_csr2d.argtypes = [dp, dp, dp, dp, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int, C.c_double,
+                                C.c_double, C.POINTER(C.c_int64), C.POINTER(C.c_int32), dp]
+        L.aio_csr2d.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -129,6 +136,75 @@ def csr(umin, umax, npt, u0, u1):
     data = np.empty(nnz, dtype=np.float64)
     lib().aio_csr(keep[0][1], keep[1][1], keep[0][0].size, npt, u0, u1, pi,
                   indices.ctypes.data_as(C.POINTER(C.c_int32)), data.ctypes.data_as(C.POINTER(C.c_double)))
+    return indptr, indices, data
+
+
+# ---- bidimensional integration (azimuthal x radial bins) ----------------------------------------------------------------
+FULL_CIRCLE = (-np.pi, np.pi)
+
+
+def pixel_chi_bounds(cfg):
+    """(chi_lo, chi_w): every pixel covers [chi_lo, chi_lo + chi_w] on the periodic azimuthal axis, radians."""
+    n = cfg.height * cfg.width
+    lo, w = np.empty(n), np.empty(n)
+    g = geometry(cfg)
+    rc = lib().aio_pixel_chi_bounds(C.byref(g), cfg.height, cfg.width, lo.ctypes.data_as(C.POINTER(C.c_double)),
+                                    w.ctypes.data_as(C.POINTER(C.c_double)))
+    if rc:
+        raise ValueError(f"aio_pixel_chi_bounds: {rc}")
+    return lo, w
+
+
+def split_azim(chi_lo, w, c0, c1, npt, cap=4096):
+    bins = (C.c_int * cap)()
+    coefs = (C.c_double * cap)()
+    n = lib().aio_split_azim(chi_lo, w, c0, c1, npt, bins, coefs, cap)
+    return list(bins[:n]), list(coefs[:n])
+
+
+def integrate2d_bounds(umin, umax, chi_lo, chi_w, npt_rad, u0, u1, npt_azim, c0, c1, image, dark=None, flat=None,
+                       solidangle=None, polarization=None, mask=None, empty=0.0):
+    """Forward scatter into [npt_azim][npt_rad] bins; dict(radial, azimuthal, intensity, sum_signal, count)."""
+    keep = [_d(umin), _d(umax), _d(chi_lo), _d(chi_w), _d(image), _d(dark), _d(flat), _d(solidangle),
+            _d(polarization), _m(mask)]
+    out = {k: np.empty((npt_azim, npt_rad)) for k in ("intensity", "sum_signal", "count")}
+    po = [out[k].ctypes.data_as(C.POINTER(C.c_double)) for k in ("intensity", "sum_signal", "count")]
+    rc = lib().aio_integrate2d_bounds(keep[0][1], keep[1][1], keep[2][1], keep[3][1], keep[0][0].size, npt_rad, u0, u1,
+                                      npt_azim, c0, c1, *[k[1] for k in keep[4:]], empty, *po)
+    if rc:
+        raise ValueError(f"aio_integrate2d_bounds: {rc}")
+    out["radial"] = u0 + (np.arange(npt_rad) + 0.5) * (u1 - u0) / npt_rad
+    out["azimuthal"] = c0 + (np.arange(npt_azim) + 0.5) * (c1 - c0) / npt_azim
+    return out
+
+
+def integrate2d(cfg, frame, radial_range=None, azim_range=None, empty=0.0):
+    """O1-O7 on both axes for a workloads.Config-like `cfg` with npt (radial) and npt_azim bins."""
+    umin, umax = pixel_bounds(cfg)
+    u0, u1 = auto_range(umin, umax) if radial_range is None else radial_range
+    c0, c1 = FULL_CIRCLE if azim_range is None else azim_range
+    lo, w = pixel_chi_bounds(cfg)
+    out = integrate2d_bounds(umin, umax, lo, w, cfg.npt, u0, u1, cfg.npt_azim, c0, c1, frame.image, frame.dark,
+                             frame.flat, frame.solidangle, frame.polarization, frame.mask, empty=empty)
+    out["range"] = (u0, u1)
+    out["azim_range"] = (c0, c1)
+    return out
+
+
+def csr2d(umin, umax, chi_lo, chi_w, npt_rad, u0, u1, npt_azim, c0, c1):
+    """Oracle CSR of the 2D matrix, row = a * npt_rad + r: (indptr int64, indices int32, data float64)."""
+    keep = [_d(umin), _d(umax), _d(chi_lo), _d(chi_w)]
+    nb = npt_rad * npt_azim
+    indptr = np.zeros(nb + 1, dtype=np.int64)
+    pi = indptr.ctypes.data_as(C.POINTER(C.c_int64))
+    a = [k[1] for k in keep]
+    nnz = lib().aio_csr2d(*a, keep[0][0].size, npt_rad, u0, u1, npt_azim, c0, c1, pi, None, None)
+    if nnz < 0:
+        raise ValueError(f"aio_csr2d: {nnz}")
+    indices = np.empty(nnz, dtype=np.int32)
+    data = np.empty(nnz, dtype=np.float64)
+    lib().aio_csr2d(*a, keep[0][0].size, npt_rad, u0, u1, npt_azim, c0, c1, pi,
+                    indices.ctypes.data_as(C.POINTER(C.c_int32)), data.ctypes.data_as(C.POINTER(C.c_double)))
     return indptr, indices, data
 
 

@@ -48,6 +48,7 @@ class Config:
     corrections: bool = False   # dark / flat / solid angle / polarisation / mask
     seed_index: int = 0
     note: str = ""
+    npt_azim: int = 0           # > 0: bidimensional integration, azimuthal x radial bins (npt = radial bins)
 
     @property
     def npix(self) -> int:
@@ -69,6 +70,9 @@ CONFIGS = {
                    dtype="int32", nframes=1024, seed_index=4),
     # configs[4]: off-image beam centre, rings are arcs
     "cfg5": Config("cfg5", 4096, 4096, 75e-6, 0.2, 1e-10, -200.0, 2048.0, Q_NM, 5000, seed_index=5),
+    # bidimensional ("cake") integration of the headline frame (Fig. 3): 360 azimuthal x 500
+    # radial bins over the full circle
+    "cake2": Config("cake2", 2048, 2048, 1e-4, 0.1, 1e-10, 1024.0, 1024.0, R_MM, 500, seed_index=2, npt_azim=360),
     # Pilatus-1M shape of PAPER.md:257 (Table 3); pixel size is a reading
     "t3": Config("t3", 981, 1043, 172e-6, 0.1, 1e-10, 521.5, 490.5, TTH_DEG, 1000,
                  dtype="int32", seed_index=6),
