@@ -77,6 +77,19 @@ typedef struct {
 int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt, ai_unit unit,
              const double *range_or_null);
 
+/* Bidimensional ("cake") integration ("mono- and bidimensional integration"; Fig. 3): bins
+ * = npt_azim azimuthal x npt_rad radial.  The azimuthal coordinate is chi = atan2(y, x), y along the image
+ * rows and x along the columns, both from the beam centre; the axis is periodic (a pixel across the negative x axis is
+ * split over the seam).  The weight of a pixel in a bin is the bounding box of PAPER.md:120 taken on both axes: its
+ * overlap / width along the radial unit times its overlap / width along chi.
+ *   npt_rad, npt_azim    >= 1, npt_rad * npt_azim < 2^28
+ *   range_or_null        HOST {u0, u1} in `unit`, NULL = automatic (as ai_setup)
+ *   azim_range_or_null   HOST {chi0, chi1} in RADIANS, 0 < chi1 - chi0 <= 2 pi; NULL = the full circle [-pi, pi]
+ * Then ai_build_csr, ai_get_csr (rows = bins, row index a * npt_rad + r) and ai_integrate2d; ai_set_options applies
+ * (AI_LAYOUT_LUT is not offered in 2D).  Errors: AI_EINVAL, AI_ENOMEM. */
+int ai_setup2d(ai_ctx **out, const ai_geometry *g, int height, int width, int npt_rad, int npt_azim, ai_unit unit,
+               const double *range_or_null, const double *azim_range_or_null);
+
 /* Build the matrix on the device: bounds -> range -> count -> exclusive scan -> ordered fill (PAPER.md:120-122 for
  * the coefficients, :150 scan, :180 CSR), then the tiled execution layout.  Idempotent.  Synchronises `cuda_stream`.
  * Errors: AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED. */
@@ -119,6 +132,14 @@ int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_va
 int ai_integrate1d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *dark, const float *flat,
                    const float *solidangle, const float *polarization, const uint8_t *mask, float *radial,
                    float *intensity, float *sum_signal, float *count, void *cuda_stream);
+
+/* Integrate one frame into azimuthal x radial bins (a context made by ai_setup2d).  As ai_integrate1d, with
+ *   radial       float32[npt_rad] bin centres, may be NULL        azimuthal   float32[npt_azim] bin centres in radians, may be NULL
+ *   intensity, sum_signal, count   float32[npt_azim][npt_rad], row-major, required
+ * Errors as ai_integrate1d; AI_EINVAL on a 1D context, AI_EUNSUPPORTED with AI_LAYOUT_LUT. */
+int ai_integrate2d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *dark, const float *flat,
+                   const float *solidangle, const float *polarization, const uint8_t *mask, float *radial,
+                   float *azimuthal, float *intensity, float *sum_signal, float *count, void *cuda_stream);
 
 /* Integrate `nframes` frames that share one matrix and one set of correction arrays (a detector streaming frames,
  * PAPER.md:11); the matrix is read once per group of frames.  All pointers are DEVICE pointers.

@@ -20,7 +20,7 @@ AI_LAYOUT_TILED, AI_LAYOUT_CSR, AI_LAYOUT_LUT, AI_LAYOUT_TILED_DIRECT = range(4)
 AI_ACC_F32_KAHAN, AI_ACC_F32_PLAIN, AI_ACC_F64 = range(3)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ai_setup", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
+EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
            "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_get_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
@@ -49,6 +49,8 @@ def lib():
     L = C.CDLL(LIB_PATH)
     vp, dp, fp = C.c_void_p, C.POINTER(C.c_double), C.c_void_p
     L.ai_setup.argtypes = [C.POINTER(vp), C.POINTER(ai_geometry), C.c_int, C.c_int, C.c_int, C.c_int, dp]
+    L.ai_setup2d.argtypes = [C.POINTER(vp), C.POINTER(ai_geometry), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, dp, dp]
+    L.ai_integrate2d.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, fp, vp]
     L.ai_build_csr.argtypes = [vp, vp]
     L.ai_get_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int64), dp, dp]
     L.ai_copy_csr_to_host.argtypes = [vp, vp, vp, vp]
@@ -116,6 +118,23 @@ def ai_setup(distance_m, pixel_y_m, pixel_x_m, center_y_px, center_x_px, wavelen
     rng = None if radial_range is None else (C.c_double * 2)(*radial_range)
     _check(lib().ai_setup(C.byref(ctx), C.byref(g), height, width, npt, unit, rng))
     return ctx
+
+
+def ai_setup2d(distance_m, pixel_y_m, pixel_x_m, center_y_px, center_x_px, wavelength_m, height, width, npt_rad, npt_azim,
+               unit, radial_range=None, azim_range=None):
+    g = ai_geometry(distance_m, pixel_y_m, pixel_x_m, center_y_px, center_x_px, wavelength_m)
+    ctx = C.c_void_p()
+    rng = None if radial_range is None else (C.c_double * 2)(*radial_range)
+    arng = None if azim_range is None else (C.c_double * 2)(*azim_range)
+    _check(lib().ai_setup2d(C.byref(ctx), C.byref(g), height, width, npt_rad, npt_azim, unit, rng, arng))
+    return ctx
+
+
+def ai_integrate2d(ctx, image, dark, flat, solidangle, polarization, mask, radial, azimuthal, intensity, sum_signal, count,
+                   stream=None, dtype=None):
+    _check(lib().ai_integrate2d(ctx, _ptr(image), dtype_code(image) if dtype is None else dtype, _ptr(dark),
+                                _ptr(flat), _ptr(solidangle), _ptr(polarization), _ptr(mask), _ptr(radial),
+                                _ptr(azimuthal), _ptr(intensity), _ptr(sum_signal), _ptr(count), _stream(stream)), ctx)
 
 
 def ai_build_csr(ctx, stream=None):
@@ -205,7 +224,7 @@ class Integrator:
     (e.g. workloads.Config).  Outputs are torch float32 CUDA tensors allocated here for convenience."""
 
     def __init__(self, cfg, radial_range=None, device=None, layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN,
-                 empty_value=0.0):
+                 empty_value=0.0, azim_range=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1412_6367_b200 needs a CUDA device (no CPU fallback)")
@@ -220,8 +239,16 @@ class Integrator:
         self.device = torch.device(device)
         self.cfg = cfg
         self.npt = cfg.npt
-        self.ctx = ai_setup(cfg.distance_m, cfg.pixel_m, cfg.pixel_m, cfg.center_y_px, cfg.center_x_px,
-                            cfg.wavelength_m, cfg.height, cfg.width, cfg.npt, cfg.unit, radial_range)
+        self.npt_azim = int(getattr(cfg, "npt_azim", 0) or 0)
+        if self.npt_azim > 0:                   # bidimensional: npt counts all bins, outputs are [npt_azim][npt_rad]
+            self.npt_rad = cfg.npt
+            self.npt = cfg.npt * self.npt_azim
+            self.ctx = ai_setup2d(cfg.distance_m, cfg.pixel_m, cfg.pixel_m, cfg.center_y_px, cfg.center_x_px,
+                                  cfg.wavelength_m, cfg.height, cfg.width, cfg.npt, self.npt_azim, cfg.unit,
+                                  radial_range, azim_range)
+        else:
+            self.ctx = ai_setup(cfg.distance_m, cfg.pixel_m, cfg.pixel_m, cfg.center_y_px, cfg.center_x_px,
+                                cfg.wavelength_m, cfg.height, cfg.width, cfg.npt, cfg.unit, radial_range)
         with torch.cuda.device(self.device):
             ai_build_csr(self.ctx)
         ai_set_options(self.ctx, layout, accum, empty_value)
@@ -262,6 +289,17 @@ class Integrator:
                                self.torch.cuda.current_stream().cuda_stream)
         if rc != AI_OK:
             _check(rc, self.ctx)
+        return intensity, sum_signal, count
+
+    def integrate2d(self, image, dark=None, flat=None, solidangle=None, polarization=None, mask=None, out=None,
+                    radial=None, azimuthal=None):
+        """Bidimensional context: (intensity, sum_signal, count), each a (npt_azim, npt_rad) device tensor."""
+        t = self.torch
+        shape = (self.npt_azim, self.npt_rad)
+        intensity, sum_signal, count = out if out is not None else tuple(
+            t.empty(shape, dtype=t.float32, device=self.device) for _ in range(3))
+        ai_integrate2d(self.ctx, image, dark, flat, solidangle, polarization, mask, radial, azimuthal, intensity,
+                       sum_signal, count)
         return intensity, sum_signal, count
 
     def integrate1d_batch(self, frames, dark=None, flat=None, solidangle=None, polarization=None, mask=None,

@@ -76,8 +76,42 @@ int ai_profile_last(ai_ctx *ctx, float *kernel_ms)
     return AI_OK;
 }
 
+static int setup_common(ai_ctx **out, const ai_geometry *g, int height, int width, int npt, ai_unit unit,
+                        const double *range_or_null);
+
 int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt, ai_unit unit,
              const double *range_or_null)
+{
+    int rc = setup_common(out, g, height, width, npt, unit, range_or_null);
+    if (rc == AI_OK) (*out)->npt_rad = npt;
+    return rc;
+}
+
+int ai_setup2d(ai_ctx **out, const ai_geometry *g, int height, int width, int npt_rad, int npt_azim, ai_unit unit,
+               const double *range_or_null, const double *azim_range_or_null)
+{
+    if (!out) return AI_EINVAL;
+    *out = nullptr;
+    if (npt_rad < 1 || npt_azim < 1 || (int64_t)npt_rad * npt_azim > 0xfffffffLL) return AI_EINVAL;
+    const double two_pi = 2.0 * 3.14159265358979323846;
+    if (azim_range_or_null && !(azim_range_or_null[1] > azim_range_or_null[0] && isfinite(azim_range_or_null[0]) &&
+                                isfinite(azim_range_or_null[1]) &&
+                                azim_range_or_null[1] - azim_range_or_null[0] <= two_pi * (1.0 + 1e-15) &&
+                                azim_range_or_null[0] >= -two_pi && azim_range_or_null[1] <= 2.0 * two_pi))
+        return AI_EINVAL;
+    int rc = setup_common(out, g, height, width, npt_rad * npt_azim, unit, range_or_null);
+    if (rc != AI_OK) return rc;
+    (*out)->npt_rad = npt_rad;
+    (*out)->npt_azim = npt_azim;
+    if (azim_range_or_null) {
+        (*out)->azim_host[0] = azim_range_or_null[0];
+        (*out)->azim_host[1] = azim_range_or_null[1];
+    }
+    return AI_OK;
+}
+
+static int setup_common(ai_ctx **out, const ai_geometry *g, int height, int width, int npt, ai_unit unit,
+                        const double *range_or_null)
 {
     if (!out) return AI_EINVAL;
     *out = nullptr;
@@ -139,10 +173,29 @@ int ai_build_csr(ai_ctx *ctx, void *cuda_stream)
     cudaStream_t st = (cudaStream_t)cuda_stream;
     AI_CUDA(ctx, cudaGetDevice(&ctx->device));
     AI_CUDA(ctx, cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device));
-    PixelSpans spans;
-    int rc = ai_build_canonical(ctx, &spans, st);
-    if (rc == AI_OK) rc = ai_build_tiled(ctx, spans, st);
-    ai_free_spans(&spans);
+    int rc;
+    if (ctx->npt_azim > 0) {
+        rc = ai_build_2d(ctx, st);
+        if (rc == AI_OK) {
+            // bin centres of the two axes, copied out by ai_integrate2d
+            float *h = static_cast<float *>(malloc(((size_t)ctx->npt_rad + ctx->npt_azim) * sizeof(float)));
+            if (!h) return ai_fail(ctx, AI_ENOMEM, "axes");
+            const double du = (ctx->range_host[1] - ctx->range_host[0]) / ctx->npt_rad;
+            const double dc = (ctx->azim_host[1] - ctx->azim_host[0]) / ctx->npt_azim;
+            for (int r = 0; r < ctx->npt_rad; ++r) h[r] = (float)(ctx->range_host[0] + (r + 0.5) * du);
+            for (int a = 0; a < ctx->npt_azim; ++a) h[ctx->npt_rad + a] = (float)(ctx->azim_host[0] + (a + 0.5) * dc);
+            cudaError_t e = cudaMalloc(&ctx->axes2d, ((size_t)ctx->npt_rad + ctx->npt_azim) * sizeof(float));
+            if (e == cudaSuccess)
+                e = cudaMemcpy(ctx->axes2d, h, ((size_t)ctx->npt_rad + ctx->npt_azim) * sizeof(float), cudaMemcpyHostToDevice);
+            free(h);
+            AI_CUDA(ctx, e);
+        }
+    } else {
+        PixelSpans spans;
+        rc = ai_build_canonical(ctx, &spans, st);
+        if (rc == AI_OK) rc = ai_build_tiled(ctx, spans, st);
+        ai_free_spans(&spans);
+    }
     if (rc != AI_OK) return rc;
     AI_CUDA(ctx, cudaMalloc(&ctx->out_dev, 3 * (size_t)ctx->npt * sizeof(float)));
     AI_CUDA(ctx, cudaMalloc(&ctx->grid_sync, 3 * sizeof(unsigned long long)));
@@ -218,9 +271,30 @@ int ai_integrate1d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *
                    float *intensity, float *sum_signal, float *count, void *cuda_stream)
 {
     if (!ctx) return AI_EINVAL;
+    if (ctx->npt_azim > 0) return ai_fail(ctx, AI_EINVAL, "bidimensional context: use ai_integrate2d");
     FrameArgs a{image, dtype, dark, flat, solidangle, polarization, mask, radial, intensity, sum_signal, count, 1,
                 (int64_t)ctx->height * ctx->width};
     return integrate(ctx, a, (cudaStream_t)cuda_stream);
+}
+
+int ai_integrate2d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *dark, const float *flat,
+                   const float *solidangle, const float *polarization, const uint8_t *mask, float *radial,
+                   float *azimuthal, float *intensity, float *sum_signal, float *count, void *cuda_stream)
+{
+    if (!ctx) return AI_EINVAL;
+    if (ctx->npt_azim < 1) return ai_fail(ctx, AI_EINVAL, "not a bidimensional context (use ai_setup2d)");
+    if (ctx->layout == AI_LAYOUT_LUT) return ai_fail(ctx, AI_EUNSUPPORTED, "no padded LUT for the 2D matrix");
+    FrameArgs a{image, dtype, dark, flat, solidangle, polarization, mask, nullptr, intensity, sum_signal, count, 1,
+                (int64_t)ctx->height * ctx->width};
+    int rc = integrate(ctx, a, (cudaStream_t)cuda_stream);
+    if (rc != AI_OK) return rc;
+    if (radial)
+        AI_CUDA(ctx, cudaMemcpyAsync(radial, ctx->axes2d, (size_t)ctx->npt_rad * sizeof(float), cudaMemcpyDeviceToDevice,
+                                     (cudaStream_t)cuda_stream));
+    if (azimuthal)
+        AI_CUDA(ctx, cudaMemcpyAsync(azimuthal, ctx->axes2d + ctx->npt_rad, (size_t)ctx->npt_azim * sizeof(float),
+                                     cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    return AI_OK;
 }
 
 int ai_integrate1d_batch(ai_ctx *ctx, const void *frames, ai_dtype dtype, int nframes, int64_t frame_stride_elems,
@@ -338,7 +412,7 @@ void ai_destroy(ai_ctx *ctx)
     cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
     free(tl.h_first_desc);
     free(ctx->stream_first);
-    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->stream_partials); cudaFree(ctx->corrected[0]); cudaFree(ctx->corrected[1]);
+    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->stream_partials); cudaFree(ctx->axes2d); cudaFree(ctx->corrected[0]); cudaFree(ctx->corrected[1]);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;

@@ -271,9 +271,10 @@ void ai_free_spans(PixelSpans *s)
     *s = PixelSpans{};
 }
 
-int ai_build_canonical(ai_ctx *ctx, PixelSpans *sp, cudaStream_t st)
+// B1-B3a: bounds of every pixel on the radial axis, the range, and the pixel's first bin / number of bins for `npt` bins
+int ai_build_spans(ai_ctx *ctx, PixelSpans *sp, int npt, cudaStream_t st)
 {
-    const int H = ctx->height, W = ctx->width, npt = ctx->npt;
+    const int H = ctx->height, W = ctx->width;
     const int64_t n = (int64_t)H * W;
     AI_CUDA(ctx, cudaMalloc(&sp->fmin, n * sizeof(double)));
     AI_CUDA(ctx, cudaMalloc(&sp->fmax, n * sizeof(double)));
@@ -292,6 +293,17 @@ int ai_build_canonical(ai_ctx *ctx, PixelSpans *sp, cudaStream_t st)
     }
     span_kernel<<<nblk, 256, 0, st>>>(n, npt, ctx->d_range, sp->fmin, sp->fmax, sp->first, sp->nb);
     AI_CUDA(ctx, cudaGetLastError());
+    AI_CUDA(ctx, cudaMemcpyAsync(ctx->range_host, ctx->d_range, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    cudaFree(parts);
+    return AI_OK;
+}
+
+int ai_build_canonical(ai_ctx *ctx, PixelSpans *sp, cudaStream_t st)
+{
+    const int H = ctx->height, W = ctx->width, npt = ctx->npt;
+    int rc = ai_build_spans(ctx, sp, npt, st);
+    if (rc != AI_OK) return rc;
 
     int *cnt = nullptr;
     long long *row_len = nullptr;      // [npt] lengths, then [1] total
@@ -311,10 +323,9 @@ int ai_build_canonical(ai_ctx *ctx, PixelSpans *sp, cudaStream_t st)
 
     long long total = 0;
     AI_CUDA(ctx, cudaMemcpyAsync(&total, row_len + npt, sizeof(long long), cudaMemcpyDeviceToHost, st));
-    AI_CUDA(ctx, cudaMemcpyAsync(ctx->range_host, ctx->d_range, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-    AI_CUDA(ctx, cudaStreamSynchronize(st));      // the one host sync of the build: nnz sizes the matrix
+    AI_CUDA(ctx, cudaStreamSynchronize(st));      // nnz sizes the matrix
     if (total > 0x7fffffffLL) {
-        cudaFree(cnt); cudaFree(row_len); cudaFree(parts);
+        cudaFree(cnt); cudaFree(row_len);
         return ai_fail(ctx, AI_EUNSUPPORTED, "matrix has %lld entries, more than int32 row pointers can address", total);
     }
     ctx->nnz = total;
@@ -327,7 +338,7 @@ int ai_build_canonical(ai_ctx *ctx, PixelSpans *sp, cudaStream_t st)
     row_sum_kernel<<<(npt + 7) / 8, 256, 0, st>>>(npt, ctx->indptr, ctx->data, ctx->row_csum);
     AI_CUDA(ctx, cudaGetLastError());
     AI_CUDA(ctx, cudaStreamSynchronize(st));
-    cudaFree(cnt); cudaFree(row_len); cudaFree(parts);
+    cudaFree(cnt); cudaFree(row_len);
     return AI_OK;
 }
 

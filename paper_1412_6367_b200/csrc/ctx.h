@@ -110,7 +110,10 @@ struct TiledLayout {
 
 struct ai_ctx {
     ai_geometry geo{};
-    int height = 0, width = 0, npt = 0;
+    int height = 0, width = 0, npt = 0;   // npt = number of bins = rows of the matrix (2D: npt_azim * npt_rad)
+    int npt_rad = 0, npt_azim = 0;        // bidimensional integration (ai_setup2d): row = a * npt_rad + r; 1D: npt_azim = 0
+    double azim_host[2] = {-3.14159265358979323846, 3.14159265358979323846};   // azimuthal range, radians
+    float *axes2d = nullptr;              // [npt_rad + npt_azim] bin centres of the two axes (device)
     ai_unit unit = AI_R_MM;
     bool user_range = false;
     double range_host[2] = {0.0, 0.0};   // valid after build
@@ -208,6 +211,7 @@ struct PixelSpans {              // per-pixel result of the bounds pass, kept on
 };
 int ai_build_canonical(ai_ctx *ctx, PixelSpans *spans, cudaStream_t st);
 int ai_build_tiled(ai_ctx *ctx, const PixelSpans &spans, cudaStream_t st);
+int ai_build_2d(ai_ctx *ctx, cudaStream_t st);      // build_2d.cu: canonical CSR + tiled layout of the 2D matrix
 int ai_build_lut(ai_ctx *ctx, cudaStream_t st);
 void ai_free_spans(PixelSpans *s);
 

@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(256) tiled_stage2_kernel(const int *__restrict
 constexpr int kFinishThreads = 128;
 template <int ACC>
 __global__ void __launch_bounds__(kFinishThreads, 10) tiled_finish_kernel(const int *__restrict__ bin_slot_ptr, int npt,
-                                                                           const void *partials,
+                                                                           int serial, const void *partials,
                                                                            const double *__restrict__ range, float empty,
                                                                            float *__restrict__ radial,
                                                                            float *__restrict__ intensity,
@@ -152,6 +152,15 @@ __global__ void __launch_bounds__(kFinishThreads, 10) tiled_finish_kernel(const 
     const double u0 = radial ? range[0] : 0.0, delta = radial ? (range[1] - range[0]) / (double)npt : 0.0;
     asm volatile("griddepcontrol.launch_dependents;");
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (serial) {
+        // many bins of a few partials each (bidimensional integration): one thread per bin
+        for (int t = blockIdx.x * kFinishThreads + threadIdx.x; t < npt; t += gridDim.x * kFinishThreads) {
+            finish_bin_serial<ACC>(partials, __ldg(bin_slot_ptr + t), __ldg(bin_slot_ptr + t + 1), empty, intensity + t,
+                                   sum_signal + t, count + t);
+            if (radial) radial[t] = (float)(u0 + ((double)t + 0.5) * delta);
+        }
+        return;
+    }
     while (b < npt) {
         const int bn = b + nw;
         int nbeg = 0, nend = 0;
@@ -233,7 +242,8 @@ int launch_finish(ai_ctx *ctx, const FrameArgs &a, const void *partials, cudaStr
     const TiledLayout &tl = ctx->tl;
     const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
     const int wpb = kFinishThreads / 32;
-    int grid = (ctx->npt + wpb - 1) / wpb;
+    const int serial = (long long)tl.nslot < 8LL * ctx->npt;      // few partials per bin: one thread per bin
+    int grid = serial ? (ctx->npt + kFinishThreads - 1) / kFinishThreads : (ctx->npt + wpb - 1) / wpb;
     if (grid > sms) grid = sms;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -246,7 +256,7 @@ int launch_finish(ai_ctx *ctx, const FrameArgs &a, const void *partials, cudaStr
     cfg.attrs = attr;
     cfg.numAttrs = 1;
 #define AI_FIN(ACC)                                                                                                   \
-    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, tiled_finish_kernel<ACC>, (const int *)tl.bin_slot_ptr, ctx->npt, partials,  \
+    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, tiled_finish_kernel<ACC>, (const int *)tl.bin_slot_ptr, ctx->npt, serial, partials,  \
                                     (const double *)ctx->d_range, ctx->empty_value, a.radial, a.intensity,           \
                                     a.sum_signal, a.count))
     switch (ctx->accum) {

@@ -124,6 +124,23 @@ __device__ __forceinline__ void finish_bin(const void *part_f, int beg, int end,
     finish_bins<ACC>(part_f, 0, beg, end, false, 0, 0, 0, lane, empty, intensity, sum_signal, count);
 }
 
+// one THREAD adds the partials of a bin, in slot order: for matrices with many bins of a few partials each (2D)
+template <int ACC>
+__device__ __forceinline__ void finish_bin_serial(const void *part_f, int beg, int end, float empty, float *intensity,
+                                                  float *sum_signal, float *count)
+{
+    using T = typename FinishT<ACC>::T;
+    T S = 0, C = 0;
+    for (int k = beg; k < end; ++k) {
+        T s, c;
+        finish_load<ACC>(part_f, k, true, s, c);
+        S += s;
+        C += c;
+    }
+    if constexpr (ACC == AI_ACC_F32_PLAIN) write_bin_f32(0, S, C, empty, intensity, sum_signal, count);
+    else write_bin(0, S, C, empty, intensity, sum_signal, count);
+}
+
 // value of the pixel whose position in the tile buffer is stored as a byte offset
 __device__ __forceinline__ float tile_at(const float *tile, unsigned off)
 {
