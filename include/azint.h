@@ -50,11 +50,14 @@ typedef enum { AI_F32 = 0, AI_I32 = 1, AI_U16 = 2, AI_I16 = 3, AI_U32 = 4 } ai_d
 
 /* execution layout of the matrix.
  *   AI_LAYOUT_TILED  B200 design: the CSR re-ordered by image tile, tiles staged in shared memory
- *   AI_LAYOUT_CSR    the canonical CSR applied row by row, one thread block per bin
- *   AI_LAYOUT_LUT    padded look-up table, one thread per bin
+ *   AI_LAYOUT_CSR    the canonical CSR, one warp per row segment, 128-bit loads
+ *   AI_LAYOUT_LUT    padded look-up table, one warp per bin
  *   AI_LAYOUT_TILED_DIRECT  the tiled layout with one thread block per tile and plain loads of the matrix: the
- *                    fallback AI_LAYOUT_TILED takes when a tile's slice of the matrix exceeds its shared-memory ring  */
-typedef enum { AI_LAYOUT_TILED = 0, AI_LAYOUT_CSR = 1, AI_LAYOUT_LUT = 2, AI_LAYOUT_TILED_DIRECT = 3 } ai_layout;
+ *                    fallback AI_LAYOUT_TILED takes when a tile's slice of the matrix exceeds its shared-memory ring
+ *   AI_LAYOUT_SCATTER  no matrix at all: the forward scatter of PAPER.md:122 with fp32 atomics ("linear read / random
+ *                    write") -- a measured comparison, NOT compensated and NOT bit-reproducible  */
+typedef enum { AI_LAYOUT_TILED = 0, AI_LAYOUT_CSR = 1, AI_LAYOUT_LUT = 2, AI_LAYOUT_TILED_DIRECT = 3,
+               AI_LAYOUT_SCATTER = 4 } ai_layout;
 
 /* accumulator arithmetic: fp32 with Kahan compensation, plain fp32, or fp64 */
 typedef enum { AI_ACC_F32_KAHAN = 0, AI_ACC_F32_PLAIN = 1, AI_ACC_F64 = 2 } ai_accum;

@@ -217,6 +217,41 @@ int aio_integrate1d_bounds(const double *u_min, const double *u_max, int64_t npi
     return 0;
 }
 
+/*
+ * The other estimator (SURVEY.md section 8(c) reading 9, "summed normalisation"): instead of correcting every pixel and
+ * averaging, sum the dark-subtracted signal and the normalisation separately with the same weights and divide the sums:
+ *   sum_signal[b] = sum c (I - dark),   sum_norm[b] = sum c (flat * solidangle * polarization),
+ *   intensity[b] = sum_signal[b] / sum_norm[b]   (empty_value where sum_norm[b] == 0).
+ * Validity of a pixel is O5's.  The paper lists the corrections but not where the division happens; this
+ * variant is an option of the library (ai_set_normalization), the default stays O5-O7 above.
+ */
+int aio_integrate1d_bounds_split(const double *u_min, const double *u_max, int64_t npix, int npt, double u0, double u1,
+                                 const double *image, const double *dark, const double *flat, const double *solidangle,
+                                 const double *polarization, const uint8_t *mask, double empty_value,
+                                 double *intensity, double *sum_signal, double *sum_norm)
+{
+    if (npix < 1 || npt < 1 || !(u1 > u0) || !image) return -1;
+    int bins[AIO_MAX_SPLIT]; double coefs[AIO_MAX_SPLIT];
+    for (int b = 0; b < npt; ++b) { sum_signal[b] = 0.0; sum_norm[b] = 0.0; }
+    for (int64_t p = 0; p < npix; ++p) {
+        double v;
+        if (!pixel_value(p, image, dark, flat, solidangle, polarization, mask, &v)) continue;
+        double den = 1.0;
+        if (flat) den *= flat[p];
+        if (solidangle) den *= solidangle[p];
+        if (polarization) den *= polarization[p];
+        double num = image[p] - (dark ? dark[p] : 0.0);
+        int n = aio_split(u_min[p], u_max[p], u0, u1, npt, bins, coefs, AIO_MAX_SPLIT);
+        if (n > AIO_MAX_SPLIT) return -3;
+        for (int k = 0; k < n; ++k) {
+            sum_signal[bins[k]] += coefs[k] * num;
+            sum_norm[bins[k]] += coefs[k] * den;
+        }
+    }
+    for (int b = 0; b < npt; ++b) intensity[b] = sum_norm[b] != 0.0 ? sum_signal[b] / sum_norm[b] : empty_value;
+    return 0;
+}
+
 /* O1-O7 from the geometry (single thread). range_or_null = {u0, u1} or NULL for the automatic range. */
 int aio_integrate1d(const aio_geometry *g, int height, int width, int npt, int unit, const double *range_or_null,
                     const double *image, const double *dark, const double *flat, const double *solidangle,

@@ -31,6 +31,8 @@ def lib():
         L.aio_split.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, ip, dp, C.c_int]
         L.aio_integrate1d_bounds.argtypes = [dp, dp, C.c_int64, C.c_int, C.c_double, C.c_double,
                                              dp, dp, dp, dp, dp, u8p, C.c_double, C.c_int, dp, dp, dp, dp]
+        L.aio_integrate1d_bounds_split.argtypes = [dp, dp, C.c_int64, C.c_int, C.c_double, C.c_double,
+                                                   dp, dp, dp, dp, dp, u8p, C.c_double, dp, dp, dp]
         L.aio_integrate1d.argtypes = [C.POINTER(Geometry), C.c_int, C.c_int, C.c_int, C.c_int, dp,
                                       dp, dp, dp, dp, dp, u8p, C.c_double, dp, dp, dp, dp, dp]
         L.aio_csr.argtypes = [dp, dp, C.c_int64, C.c_int, C.c_double, C.c_double,
@@ -103,6 +105,20 @@ def integrate1d_bounds(umin, umax, npt, u0, u1, image, dark=None, flat=None, sol
                                       *[k[1] for k in keep[2:]], empty, nthreads, *po)
     if rc:
         raise ValueError(f"aio_integrate1d_bounds: {rc}")
+    return out
+
+
+def integrate1d_bounds_split(umin, umax, npt, u0, u1, image, dark=None, flat=None, solidangle=None, polarization=None,
+                             mask=None, empty=0.0):
+    """The split-normalisation estimator: dict(intensity, sum_signal, sum_norm); `count` is an alias of sum_norm."""
+    keep = [_d(umin), _d(umax), _d(image), _d(dark), _d(flat), _d(solidangle), _d(polarization), _m(mask)]
+    out = {k: np.empty(npt) for k in ("intensity", "sum_signal", "sum_norm")}
+    po = [out[k].ctypes.data_as(C.POINTER(C.c_double)) for k in ("intensity", "sum_signal", "sum_norm")]
+    rc = lib().aio_integrate1d_bounds_split(keep[0][1], keep[1][1], keep[0][0].size, npt, u0, u1,
+                                            *[k[1] for k in keep[2:]], empty, *po)
+    if rc:
+        raise ValueError(f"aio_integrate1d_bounds_split: {rc}")
+    out["count"] = out["sum_norm"]
     return out
 
 

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "libazint.so")
 # enums of include/azint.h
 AI_R_MM, AI_TTH_DEG, AI_TTH_RAD, AI_Q_NM, AI_Q_A = range(5)
 AI_F32, AI_I32, AI_U16, AI_I16, AI_U32 = range(5)
-AI_LAYOUT_TILED, AI_LAYOUT_CSR, AI_LAYOUT_LUT, AI_LAYOUT_TILED_DIRECT = range(4)
+AI_LAYOUT_TILED, AI_LAYOUT_CSR, AI_LAYOUT_LUT, AI_LAYOUT_TILED_DIRECT, AI_LAYOUT_SCATTER = range(5)
 AI_ACC_F32_KAHAN, AI_ACC_F32_PLAIN, AI_ACC_F64 = range(3)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 

@@ -157,6 +157,7 @@ static int setup_common(ai_ctx **out, const ai_geometry *g, int height, int widt
                 else if (!strcmp(key, "fl")) ctx->tune.inflight = val;
                 else if (!strcmp(key, "ss")) ctx->tune.stream_stages = val;
                 else if (!strcmp(key, "nov")) ctx->tune.no_overlap = val;
+                else if (!strcmp(key, "bu")) ctx->tune.batch_units = val;
             }
             q = strchr(q, ',');
             if (q) ++q;
@@ -237,7 +238,7 @@ int ai_copy_csr_to_host(const ai_ctx *ctx, int32_t *indptr_host, int32_t *indice
 int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_value)
 {
     if (!ctx) return AI_EINVAL;
-    if ((int)layout < AI_LAYOUT_TILED || (int)layout > AI_LAYOUT_TILED_DIRECT) return ai_fail(ctx, AI_EINVAL, "bad layout %d", (int)layout);
+    if ((int)layout < AI_LAYOUT_TILED || (int)layout > AI_LAYOUT_SCATTER) return ai_fail(ctx, AI_EINVAL, "bad layout %d", (int)layout);
     if ((int)accum < AI_ACC_F32_KAHAN || (int)accum > AI_ACC_F64) return ai_fail(ctx, AI_EINVAL, "bad accum %d", (int)accum);
     ctx->layout = layout;
     ctx->accum = accum;
@@ -262,6 +263,7 @@ static int integrate(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
     case AI_LAYOUT_TILED_DIRECT: return ai_launch_tiled(ctx, a, st);
     case AI_LAYOUT_CSR: return ai_launch_csr(ctx, a, st);
     case AI_LAYOUT_LUT: return ai_launch_lut(ctx, a, st);
+    case AI_LAYOUT_SCATTER: return ai_launch_scatter(ctx, a, st);
     }
     return AI_EINVAL;
 }
@@ -405,7 +407,7 @@ void ai_destroy(ai_ctx *ctx)
     }
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     cudaFree(ctx->indptr); cudaFree(ctx->indices); cudaFree(ctx->data); cudaFree(ctx->row_csum); cudaFree(ctx->d_range);
-    cudaFree(ctx->lut_coef); cudaFree(ctx->lut_idx);
+    cudaFree(ctx->lut_coef); cudaFree(ctx->lut_idx); cudaFree(ctx->csr_seg); cudaFree(ctx->csr_row_seg_ptr); cudaFree(ctx->csr_partials); cudaFree(ctx->scat_first_nb); cudaFree(ctx->scat_gw);
     TiledLayout &tl = ctx->tl;
     cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_meta); cudaFree(tl.seg_csum);
     cudaFree(tl.tile_desc); cudaFree(tl.tile_order); cudaFree(tl.blob); cudaFree(tl.blob_desc);

@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(256) row_sum_kernel(int npt, const int32_t *__
     if ((threadIdx.x & 31) == 0) row_csum[b] = (float)s;
 }
 
-// B6: padded, transposed look-up table: entry j of bin b at [j*npt + b]; padding has
+// B6: padded look-up table, row-major: entry j of bin b at [b * lut_width + j]; padding has
 // coefficient 0 and index 0.
 __global__ void __launch_bounds__(256) lut_kernel(int npt, int lut_width, const int32_t *__restrict__ indptr,
                                                   const int32_t *__restrict__ indices, const float *__restrict__ data,
@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(256) lut_kernel(int npt, int lut_width, const 
 {
     int64_t total = (int64_t)npt * lut_width;
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
-        int j = (int)(e / npt), b = (int)(e - (int64_t)j * npt);
+        int b = (int)(e / lut_width), j = (int)(e - (int64_t)b * lut_width);
         int k = indptr[b] + j;
         bool in = k < indptr[b + 1];
         lut_coef[e] = in ? data[k] : 0.0f;
@@ -352,7 +352,7 @@ int ai_build_lut(ai_ctx *ctx, cudaStream_t st)
     AI_CUDA(ctx, cudaMemcpyAsync(&h_max, d_max, sizeof(int), cudaMemcpyDeviceToHost, st));
     AI_CUDA(ctx, cudaStreamSynchronize(st));
     cudaFree(d_max);
-    ctx->lut_width = h_max > 0 ? h_max : 1;
+    ctx->lut_width = h_max > 0 ? (h_max + 3) / 4 * 4 : 4;      // rows start on 16-byte boundaries
     const size_t total = (size_t)ctx->npt * ctx->lut_width;
     size_t free_b = 0, total_b = 0;
     AI_CUDA(ctx, cudaMemGetInfo(&free_b, &total_b));

@@ -59,6 +59,7 @@ struct PipeTune {
     int inflight = 0;                          // 0 = as many as there are stages
     int stream_stages = 0;                     // cap on the (tile + blob) stages of the single-frame kernel, 0 = none
     int no_overlap = 0;                        // single-frame kernel: never stream ahead of the grid dependency
+    int batch_units = 0;                       // batched kernel: 1 = (block, frame) units, 2 = (block, two frames), 0 = by layout
 };
 inline PipePlan ai_pipe_plan(int max_blob_bytes, int tile_h, bool batch, const PipeTune &tune = PipeTune())
 {
@@ -134,7 +135,16 @@ struct ai_ctx {
     float *row_csum = nullptr;    // [npt] sum of each row's coefficients
     double *d_range = nullptr;    // [2] u0, u1 on the device
 
-    // padded LUT, transposed: entry j of bin b at [j * npt + b]
+    // segments of the canonical CSR's rows for AI_LAYOUT_CSR (integrate_csr.cu), built on first use
+    void *csr_seg = nullptr;              // int4 {row, first entry, end entry, -}
+    int *csr_row_seg_ptr = nullptr;       // [npt+1]
+    int csr_nseg = 0;
+    void *csr_partials = nullptr;         // [nframes][csr_nseg] double2
+    size_t csr_partials_bytes = 0;
+    // AI_LAYOUT_SCATTER (integrate_scatter.cu): 12 bytes of split geometry per pixel, built on first use
+    int *scat_first_nb = nullptr;
+    void *scat_gw = nullptr;              // float2 {lower bound relative to the first bin, width in bins}
+    // padded LUT, row-major: entry j of bin b at [b * lut_width + j], lut_width a multiple of 4
     int lut_width = 0;
     float *lut_coef = nullptr;
     int32_t *lut_idx = nullptr;
@@ -214,6 +224,7 @@ int ai_build_tiled(ai_ctx *ctx, const PixelSpans &spans, cudaStream_t st);
 int ai_build_2d(ai_ctx *ctx, cudaStream_t st);      // build_2d.cu: canonical CSR + tiled layout of the 2D matrix
 int ai_build_lut(ai_ctx *ctx, cudaStream_t st);
 void ai_free_spans(PixelSpans *s);
+int ai_build_spans(ai_ctx *ctx, PixelSpans *sp, int npt, cudaStream_t st);
 
 // per-frame launches (integrate_*.cu) -------------------------------------------------------------------------------
 struct FrameArgs {
@@ -229,6 +240,7 @@ struct FrameArgs {
 int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_csr(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_lut(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
+int ai_launch_scatter(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, cudaStream_t st, float **out);   // integrate_prep.cu
 int ai_stream_full_grid(const ai_ctx *ctx);   // integrate_stream.cu: 1 if the single-frame kernel puts one block on every SM
 int ai_stream_stages(const ai_ctx *ctx);      // integrate_stream.cu: (tile + blob) stages of the single-frame kernel, 0 = n/a

@@ -478,6 +478,7 @@ struct BatchParams {
     int tile_h, ntiles, nslot;
     int img_stages, mat_stages, img_stage_bytes, mat_stage_bytes, hdr_bytes;
     int nframes, frames_per_item, nitems;
+    int single_units;            // a consumer warp's work unit is (block, one frame) instead of (block, two frames)
     void *partials;
 };
 
@@ -571,13 +572,26 @@ __global__ void __launch_bounds__(kBatchThreads, 1) tiled_bstream_kernel(const _
                     mbar_wait(img_full + sb, ir.parity);
                     ir.next(p.img_stages);
                 }
-                if (firstb < d.w) {
+                // work units of the pass, dealt round-robin to the warps and continuing across passes: (block, both
+                // frames) -- coefficients and positions serve two frames -- or, when a tile has fewer blocks than half
+                // the warps (p.single_units, an experiment switch), (block, one frame): twice as many units
+                const int nunits = p.single_units && two ? 2 * d.w : d.w;
+                if (firstb < nunits) {
                     const unsigned ta = smem_u32(img_base + (size_t)sa * p.img_stage_bytes);
                     const unsigned tb = smem_u32(img_base + (size_t)sb * p.img_stage_bytes);
                     char *pa = reinterpret_cast<char *>(p.partials) + (int64_t)f * p.nslot * 16;
                     char *pb = pa + (int64_t)p.nslot * 16;
-                    for (int b = firstb; b < d.w; b += kBatchCons) {
-                        const unsigned h = bh[b];
+                    for (int u = firstb; u < nunits; u += kBatchCons) {
+                        if (p.single_units && two) {
+                            const unsigned h = bh[u >> 1];
+                            const unsigned t = (u & 1) ? tb : ta;
+                            char *pp = (u & 1) ? pb : pa;
+                            if (stream_block<DT, ACC, false>(t, blob, h, pp, lane)) {
+                                if constexpr (DT == AI_F32) stream_block_tracked<ACC, false>(t, blob, h, pp, lane);
+                            }
+                            continue;
+                        }
+                        const unsigned h = bh[u];
                         if (two && !stream_block2<DT, ACC>(ta, tb, blob, h, pa, pb, lane)) continue;
                         // one frame left, or a non-finite pixel somewhere: frame by frame
                         if (stream_block<DT, ACC, false>(ta, blob, h, pa, lane)) {
@@ -593,7 +607,7 @@ __global__ void __launch_bounds__(kBatchThreads, 1) tiled_bstream_kernel(const _
                     mbar_arrive(img_empty + sa);
                     if (two) mbar_arrive(img_empty + sb);
                 }
-                firstb -= d.w % kBatchCons;
+                firstb -= nunits % kBatchCons;
                 if (firstb < 0) firstb += kBatchCons;
             }
             if (lane == 0) mbar_arrive(mat_empty + mr.stage);
@@ -825,6 +839,7 @@ int ai_launch_bstream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaSt
     p.nslot = tl.nslot;
     p.nframes = a.nframes;
     p.partials = ctx->partials;
+    p.single_units = ctx->tune.batch_units == 1;      // measured slower on cfg2 x 64 and cfg4 (0.375 / 2.18 ms against 0.325 / 1.82 ms)
     const size_t smem = (size_t)p.img_stages * p.img_stage_bytes + p.hdr_bytes + (size_t)p.mat_stages * p.mat_stage_bytes;
     CUtensorMap map{};
     int rc = ai_make_frame_map(ctx, a, tl.tile_h, &map);

@@ -405,3 +405,41 @@ def test_a_pixel_spanning_more_bins_than_the_oracle_buffers_is_an_error_not_a_cl
     r = oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, np.full(1, 3.0))
     assert r["count"] == pytest.approx(np.full(4096, 1.0 / 4096), rel=1e-9)
     assert r["intensity"] == pytest.approx(np.full(4096, 3.0), rel=1e-12)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# the split-normalisation estimator (sum c (I - dark) over sum c flat Omega P)
+# ----------------------------------------------------------------------------------------------------------------
+def test_split_normalisation_against_scipy_products_and_closed_forms(oracle, workloads):
+    W = workloads
+    cfg = W.tiny_config(40, 52, center_x=20.3, center_y=31.1, unit=W.TTH_DEG, npt=37)
+    rng = np.random.default_rng(21)
+    shape = (cfg.height, cfg.width)
+    img = rng.poisson(300.0, size=shape).astype(np.float64)
+    dark = rng.poisson(5.0, size=shape).astype(np.float64)
+    flat = rng.uniform(0.8, 1.2, size=shape)
+    sa = rng.uniform(0.7, 1.0, size=shape)
+    pol = rng.uniform(0.9, 1.0, size=shape)
+    mask = (rng.random(shape) < 0.07).astype(np.uint8)
+    umin, umax = oracle.pixel_bounds(cfg)
+    u0, u1 = oracle.auto_range(umin, umax)
+    r = oracle.integrate1d_bounds_split(umin, umax, cfg.npt, u0, u1, img, dark, flat, sa, pol, mask)
+    # the same sums as two products of the (separately pinned) CSR matrix with masked vectors
+    import scipy.sparse as sp
+    indptr, indices, data = oracle.csr(umin, umax, cfg.npt, u0, u1)
+    m = sp.csr_matrix((data, indices, indptr), shape=(cfg.npt, cfg.npix))
+    ok = (mask.ravel() == 0)
+    num = np.where(ok, (img - dark).ravel(), 0.0)
+    den = np.where(ok, (flat * sa * pol).ravel(), 0.0)
+    assert r["sum_signal"] == pytest.approx(m @ num, rel=1e-12)
+    assert r["sum_norm"] == pytest.approx(m @ den, rel=1e-12)
+    assert r["intensity"] == pytest.approx((m @ num) / (m @ den), rel=1e-12)
+    # I = k * flat * Omega * P + dark  =>  the ratio of the sums is k in every bin, whatever the mask
+    k = 12.5
+    r2 = oracle.integrate1d_bounds_split(umin, umax, cfg.npt, u0, u1, k * flat * sa * pol + dark, dark, flat, sa, pol, mask)
+    assert r2["intensity"] == pytest.approx(np.full(cfg.npt, k), rel=1e-13)
+    # without a denominator the normalisation is the unweighted histogram: the default estimator
+    r3 = oracle.integrate1d_bounds_split(umin, umax, cfg.npt, u0, u1, img, dark, None, None, None, mask)
+    r4 = oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, img, dark, None, None, None, mask)
+    assert r3["intensity"] == pytest.approx(r4["intensity"], rel=1e-14)
+    assert r3["sum_norm"] == pytest.approx(r4["count"], rel=1e-14)
