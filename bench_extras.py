@@ -161,6 +161,30 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
                                     "vs_3000_fps_detector": c4.nframes / (ms * 1e-3) / 3000.0,
                                     "note": "4.3 GB of frames > L2; 8 distinct frames repeated"}
     it.close()
+    # bidimensional integration of the headline frame: 360 azimuthal x 500 radial bins
+    ck = W.CONFIGS["cake2"]
+    its = [B.Integrator(ck, device=device) for _ in range(3)]
+    outs = [tuple(torch.empty((ck.npt_azim, ck.npt), dtype=torch.float32, device=device) for _ in range(3)) for _ in its]
+    nnz2 = B.ai_get_csr(its[0].ctx)[3]
+
+    def cake_train(k):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(k):
+            its[i % 3].integrate2d(frames_dev[i % len(frames_dev)], out=outs[i % 3])
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / k
+
+    for _ in range(6):
+        cake_train(50)
+    ms = statistics.median(cake_train(100) for _ in range(5))
+    ab2 = ck.npix * 4 + nnz2 * 8 + (ck.npt * ck.npt_azim + 1) * 4 + 3 * ck.npt * ck.npt_azim * 4
+    ex["train_cake2_360x500_bins"] = {"frames_per_s": 1e3 / ms, "ms_per_step": ms, "nnz": nnz2, "algorithmic_bytes": ab2,
+                                      "frac_of_peak": ab2 / (ms * 1e-3) / 1e9 / peak_gbs,
+                                      "layout": B.ai_get_layout_info(its[0].ctx)}
+    for it in its:
+        it.close()
     ex["build_vs_oracle"] = build_times(torch, B, device)
     return ex
 
@@ -176,8 +200,11 @@ def cfg5_table(torch, B, BM, c, fr, integ, fdev, flush, peak_gbs):
     none5 = (None,) * 5
     table = {}
     lut_w = None
-    for lname, layout in (("tiled", B.AI_LAYOUT_TILED), ("csr", B.AI_LAYOUT_CSR), ("lut", B.AI_LAYOUT_LUT)):
+    for lname, layout in (("tiled", B.AI_LAYOUT_TILED), ("csr", B.AI_LAYOUT_CSR), ("lut", B.AI_LAYOUT_LUT),
+                          ("scatter", B.AI_LAYOUT_SCATTER)):
         for aname, acc in (("plain", B.AI_ACC_F32_PLAIN), ("kahan", B.AI_ACC_F32_KAHAN), ("f64", B.AI_ACC_F64)):
+            if lname == "scatter" and aname != "plain":
+                continue                              # fp32 atomics: there is only one arithmetic
             integ.set_options(layout, acc)
             i, s, cnt = integ.integrate1d(fdev[0])
             torch.cuda.synchronize()
@@ -185,11 +212,13 @@ def cfg5_table(torch, B, BM, c, fr, integ, fdev, flush, peak_gbs):
             steps = 12
             tot, kms, _ = BM.timed_steps(torch, B, integ, fdev, none5, steps, 2, flush)
             k = statistics.median(kms)
-            if lname == "lut":
+            if lname == "scatter":
+                bytes_ = c.npix * 4 + c.npix * 12 + 3 * c.npt * 4       # frame + 12 B of split geometry per pixel + outputs
+            elif lname == "lut":
                 if lut_w is None:                       # padded row length = the longest row of the CSR
                     indptr = np.empty(c.npt + 1, dtype=np.int32)
                     B.ai_copy_csr_to_host(integ.ctx, indptr)
-                    lut_w = int(np.diff(indptr).max())
+                    lut_w = (int(np.diff(indptr).max()) + 3) // 4 * 4
                 bytes_ = c.npix * 4 + 8 * lut_w * c.npt + 3 * c.npt * 4
             else:
                 bytes_ = BM.algorithmic_bytes(c, nnz)

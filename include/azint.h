@@ -62,6 +62,14 @@ typedef enum { AI_LAYOUT_TILED = 0, AI_LAYOUT_CSR = 1, AI_LAYOUT_LUT = 2, AI_LAY
 /* accumulator arithmetic: fp32 with Kahan compensation, plain fp32, or fp64 */
 typedef enum { AI_ACC_F32_KAHAN = 0, AI_ACC_F32_PLAIN = 1, AI_ACC_F64 = 2 } ai_accum;
 
+/* where the division by the normalisation happens (the paper lists the corrections, not this):
+ *   AI_NORM_PIXEL  every pixel is corrected, v = (I - dark) / (flat * solidangle * polarization), then averaged with the
+ *                  split weights: intensity = sum c v / sum c                                    (default)
+ *   AI_NORM_SPLIT  signal and normalisation are summed separately with the same weights and the sums divided:
+ *                  sum_signal = sum c (I - dark), count = sum c (flat * solidangle * polarization), intensity = their
+ *                  ratio (`count` then carries the summed normalisation).  One 1D frame per call, AI_LAYOUT_TILED. */
+typedef enum { AI_NORM_PIXEL = 0, AI_NORM_SPLIT = 1 } ai_norm;
+
 /* planar detector orthogonal to the beam; lengths in metres, centre in pixels */
 typedef struct {
     double distance_m;
@@ -112,6 +120,10 @@ int ai_copy_csr_to_host(const ai_ctx *ctx, int32_t *indptr_host, int32_t *indice
  * AI_LAYOUT_LUT builds the padded table on first use (inside the next integrate call's stream).
  * Errors: AI_EINVAL. */
 int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_value);
+
+/* Choose the estimator (see ai_norm).  Errors: AI_EINVAL; an integrate call that cannot honour AI_NORM_SPLIT (batches,
+ * bidimensional contexts, other layouts) returns AI_EUNSUPPORTED. */
+int ai_set_normalization(ai_ctx *ctx, ai_norm norm);
 
 /* Integrate one frame.  All pointers are DEVICE pointers.
  *   image                      height*width elements of `dtype`
@@ -164,8 +176,9 @@ int ai_integrate1d_host(ai_ctx *ctx, const void *image_host, ai_dtype dtype, con
                         float *intensity_host, float *sum_signal_host, float *count_host, void *cuda_stream);
 
 /* A stream of frames that live in HOST memory (the transfer is more than
- * half of the paper's per-frame time): like ai_integrate1d_host for each of the `nframes` frames, with the upload of
- * frame k+1 overlapping the kernels and downloads of frame k (two device staging buffers, a library-owned copy stream).
+ * half of the paper's per-frame time).  The frames travel in chunks of up to 8: one upload per chunk into one of two
+ * device staging buffers on a library-owned copy stream (the upload of chunk k+1 overlaps the kernels of chunk k), one
+ * batched launch per chunk (as ai_integrate1d_batch: the matrix is read once per chunk), three downloads per chunk.
  *   frames_host         HOST pointer (pinned memory for the overlap to happen), frame k at k * frame_stride_elems elements
  *   dark ... mask       DEVICE pointers or NULL, shared by all frames
  *   *_host outputs      HOST pointers, [nframes][npt] row-major

@@ -18,9 +18,10 @@ AI_R_MM, AI_TTH_DEG, AI_TTH_RAD, AI_Q_NM, AI_Q_A = range(5)
 AI_F32, AI_I32, AI_U16, AI_I16, AI_U32 = range(5)
 AI_LAYOUT_TILED, AI_LAYOUT_CSR, AI_LAYOUT_LUT, AI_LAYOUT_TILED_DIRECT, AI_LAYOUT_SCATTER = range(5)
 AI_ACC_F32_KAHAN, AI_ACC_F32_PLAIN, AI_ACC_F64 = range(3)
+AI_NORM_PIXEL, AI_NORM_SPLIT = range(2)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
+EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
            "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_get_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
@@ -55,6 +56,7 @@ def lib():
     L.ai_get_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int64), dp, dp]
     L.ai_copy_csr_to_host.argtypes = [vp, vp, vp, vp]
     L.ai_set_options.argtypes = [vp, C.c_int, C.c_int, C.c_float]
+    L.ai_set_normalization.argtypes = [vp, C.c_int]
     L.ai_integrate1d.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
     L.ai_integrate1d_batch.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_integrate1d_host.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, vp]
@@ -155,6 +157,10 @@ def ai_copy_csr_to_host(ctx, indptr_host=None, indices_host=None, data_host=None
 
 def ai_set_options(ctx, layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN, empty_value=0.0):
     _check(lib().ai_set_options(ctx, layout, accum, empty_value), ctx)
+
+
+def ai_set_normalization(ctx, norm=AI_NORM_PIXEL):
+    _check(lib().ai_set_normalization(ctx, norm), ctx)
 
 
 def ai_integrate1d(ctx, image, dark, flat, solidangle, polarization, mask, radial, intensity, sum_signal, count,

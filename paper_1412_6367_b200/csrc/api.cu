@@ -246,6 +246,14 @@ int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_va
     return AI_OK;
 }
 
+int ai_set_normalization(ai_ctx *ctx, ai_norm norm)
+{
+    if (!ctx) return AI_EINVAL;
+    if ((int)norm < AI_NORM_PIXEL || (int)norm > AI_NORM_SPLIT) return ai_fail(ctx, AI_EINVAL, "bad normalisation %d", (int)norm);
+    ctx->norm = norm;
+    return AI_OK;
+}
+
 static int integrate(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 {
     if (!ctx) return AI_EINVAL;
@@ -258,6 +266,10 @@ static int integrate(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
     if (dev != ctx->device)
         return ai_fail(ctx, AI_EINVAL, "the matrix was built on device %d, the current device is %d", ctx->device, dev);
     if (a.frame_stride < (int64_t)ctx->height * ctx->width) return ai_fail(ctx, AI_EINVAL, "frame stride < height*width");
+    if (ctx->norm == AI_NORM_SPLIT) {
+        if (ctx->layout != AI_LAYOUT_TILED) return ai_fail(ctx, AI_EUNSUPPORTED, "split normalisation: AI_LAYOUT_TILED only");
+        return ai_launch_tiled_split(ctx, a, st);
+    }
     switch (ctx->layout) {
     case AI_LAYOUT_TILED:
     case AI_LAYOUT_TILED_DIRECT: return ai_launch_tiled(ctx, a, st);
@@ -355,43 +367,70 @@ int ai_integrate1d_host_frames(ai_ctx *ctx, const void *frames_host, ai_dtype dt
     if (frame_stride_elems < npix) return ai_fail(ctx, AI_EINVAL, "frame stride < height*width");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t esz = (dtype == AI_U16 || dtype == AI_I16) ? 2 : 4;
-    const size_t bytes = (size_t)npix * esz, nb = (size_t)ctx->npt * sizeof(float);
-    if (!ctx->copy_stream) {
-        AI_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    const size_t bytes = (size_t)npix * esz;
+    if (!ctx->host_frames_ready) {           // set only once every resource exists (a failed attempt is retried)
+        if (!ctx->copy_stream) AI_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
         for (int i = 0; i < 2; ++i) {
-            AI_CUDA(ctx, cudaEventCreateWithFlags(&ctx->h2d_done[i], cudaEventDisableTiming));
-            AI_CUDA(ctx, cudaEventCreateWithFlags(&ctx->slot_free[i], cudaEventDisableTiming));
-            AI_CUDA(ctx, cudaMalloc(&ctx->out2[i], 3 * nb));
+            if (!ctx->h2d_done[i]) AI_CUDA(ctx, cudaEventCreateWithFlags(&ctx->h2d_done[i], cudaEventDisableTiming));
+            if (!ctx->slot_free[i]) AI_CUDA(ctx, cudaEventCreateWithFlags(&ctx->slot_free[i], cudaEventDisableTiming));
         }
+        ctx->host_frames_ready = true;
     }
-    if (ctx->stage2_bytes < bytes) {
+    // Frames travel in chunks of up to kHostChunk: one upload per chunk into one of two staging buffers (the upload of
+    // chunk k+1 overlaps the kernels of chunk k), ONE batched launch per chunk (ai_integrate1d_batch: the matrix is read
+    // once per chunk), three downloads per chunk.
+    constexpr int kHostChunk = 8;
+    const int chunk = nframes < kHostChunk ? nframes : kHostChunk;
+    const size_t chunk_bytes = bytes * chunk, out_floats = (size_t)ctx->npt * chunk;
+    if (ctx->stage2_bytes < chunk_bytes || ctx->out2_floats < 3 * out_floats) {
+        AI_CUDA(ctx, cudaStreamSynchronize(st));
+        AI_CUDA(ctx, cudaStreamSynchronize(ctx->copy_stream));
         for (int i = 0; i < 2; ++i) {
-            if (ctx->stage2[i]) AI_CUDA(ctx, cudaFree(ctx->stage2[i]));
-            ctx->stage2[i] = nullptr;
+            cudaFree(ctx->stage2[i]); cudaFree(ctx->out2[i]);
+            ctx->stage2[i] = nullptr; ctx->out2[i] = nullptr;
         }
         ctx->stage2_bytes = 0;
-        for (int i = 0; i < 2; ++i) AI_CUDA(ctx, cudaMalloc(&ctx->stage2[i], bytes));
-        ctx->stage2_bytes = bytes;
+        ctx->out2_floats = 0;
+        for (int i = 0; i < 2; ++i) {
+            AI_CUDA(ctx, cudaMalloc(&ctx->stage2[i], chunk_bytes));
+            AI_CUDA(ctx, cudaMalloc(&ctx->out2[i], 3 * out_floats * sizeof(float)));
+        }
+        ctx->stage2_bytes = chunk_bytes;
+        ctx->out2_floats = 3 * out_floats;
     }
     // uploads must not overtake work already queued on the caller's stream that may still use the staging buffers
     AI_CUDA(ctx, cudaEventRecord(ctx->slot_free[0], st));
     AI_CUDA(ctx, cudaEventRecord(ctx->slot_free[1], st));
-    for (int k = 0; k < nframes; ++k) {
-        const int slot = k & 1;
-        const char *src = static_cast<const char *>(frames_host) + (size_t)k * frame_stride_elems * esz;
+    int rc = AI_OK;
+    for (int k0 = 0, c = 0; k0 < nframes && rc == AI_OK; k0 += chunk, ++c) {
+        const int slot = c & 1, n = nframes - k0 < chunk ? nframes - k0 : chunk;
+        const char *src = static_cast<const char *>(frames_host) + (size_t)k0 * frame_stride_elems * esz;
         AI_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->slot_free[slot], 0));
-        AI_CUDA(ctx, cudaMemcpyAsync(ctx->stage2[slot], src, bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+        if (frame_stride_elems == npix) {
+            AI_CUDA(ctx, cudaMemcpyAsync(ctx->stage2[slot], src, bytes * n, cudaMemcpyHostToDevice, ctx->copy_stream));
+        } else {
+            for (int q = 0; q < n; ++q)
+                AI_CUDA(ctx, cudaMemcpyAsync(static_cast<char *>(ctx->stage2[slot]) + bytes * q,
+                                             src + (size_t)q * frame_stride_elems * esz, bytes, cudaMemcpyHostToDevice,
+                                             ctx->copy_stream));
+        }
         AI_CUDA(ctx, cudaEventRecord(ctx->h2d_done[slot], ctx->copy_stream));
         AI_CUDA(ctx, cudaStreamWaitEvent(st, ctx->h2d_done[slot], 0));
         float *o = ctx->out2[slot];
-        FrameArgs a{ctx->stage2[slot], dtype, dark, flat, solidangle, polarization, mask, nullptr, o, o + ctx->npt,
-                    o + 2 * ctx->npt, 1, npix};
-        int rc = integrate(ctx, a, st);
-        if (rc != AI_OK) return rc;
+        const size_t on = (size_t)ctx->npt * n;
+        FrameArgs a{ctx->stage2[slot], dtype, dark, flat, solidangle, polarization, mask, nullptr, o, o + on, o + 2 * on, n, npix};
+        rc = integrate(ctx, a, st);
+        if (rc != AI_OK) break;
         AI_CUDA(ctx, cudaEventRecord(ctx->slot_free[slot], st));
-        AI_CUDA(ctx, cudaMemcpyAsync(intensity_host + (size_t)k * ctx->npt, o, nb, cudaMemcpyDeviceToHost, st));
-        AI_CUDA(ctx, cudaMemcpyAsync(sum_signal_host + (size_t)k * ctx->npt, o + ctx->npt, nb, cudaMemcpyDeviceToHost, st));
-        AI_CUDA(ctx, cudaMemcpyAsync(count_host + (size_t)k * ctx->npt, o + 2 * ctx->npt, nb, cudaMemcpyDeviceToHost, st));
+        AI_CUDA(ctx, cudaMemcpyAsync(intensity_host + (size_t)k0 * ctx->npt, o, on * sizeof(float), cudaMemcpyDeviceToHost, st));
+        AI_CUDA(ctx, cudaMemcpyAsync(sum_signal_host + (size_t)k0 * ctx->npt, o + on, on * sizeof(float), cudaMemcpyDeviceToHost, st));
+        AI_CUDA(ctx, cudaMemcpyAsync(count_host + (size_t)k0 * ctx->npt, o + 2 * on, on * sizeof(float), cudaMemcpyDeviceToHost, st));
+    }
+    // also on failure: nothing of this call may still be writing the staging buffers when it returns
+    cudaStreamSynchronize(ctx->copy_stream);
+    if (rc != AI_OK) {
+        cudaStreamSynchronize(st);
+        return rc;
     }
     AI_CUDA(ctx, cudaStreamSynchronize(st));
     return AI_OK;
@@ -407,7 +446,7 @@ void ai_destroy(ai_ctx *ctx)
     }
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     cudaFree(ctx->indptr); cudaFree(ctx->indices); cudaFree(ctx->data); cudaFree(ctx->row_csum); cudaFree(ctx->d_range);
-    cudaFree(ctx->lut_coef); cudaFree(ctx->lut_idx); cudaFree(ctx->csr_seg); cudaFree(ctx->csr_row_seg_ptr); cudaFree(ctx->csr_partials); cudaFree(ctx->scat_first_nb); cudaFree(ctx->scat_gw);
+    cudaFree(ctx->lut_coef); cudaFree(ctx->lut_idx); cudaFree(ctx->csr_seg); cudaFree(ctx->csr_row_seg_ptr); cudaFree(ctx->csr_partials); cudaFree(ctx->scat_first_nb); cudaFree(ctx->scat_gw); cudaFree(ctx->norm_scratch);
     TiledLayout &tl = ctx->tl;
     cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_meta); cudaFree(tl.seg_csum);
     cudaFree(tl.tile_desc); cudaFree(tl.tile_order); cudaFree(tl.blob); cudaFree(tl.blob_desc);

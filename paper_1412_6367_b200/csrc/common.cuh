@@ -53,22 +53,26 @@ __device__ __forceinline__ float4 load_raw4(const void *img, int64_t p)
 __device__ __forceinline__ float quiet_nan() { return __int_as_float(0x7fc00000); }
 __device__ __forceinline__ bool finite_f(float x) { return fabsf(x) <= 3.402823466e38f; }   // false for NaN / Inf
 
+// mode 0: the corrected value; 1: its numerator I - dark; 2: its denominator flat * solid * pol (the two sums of the
+// split-normalisation estimator, ai_set_normalization) -- the validity test is the same in all three
 __device__ __forceinline__ float correct_value(float raw, float dark, float flat, float solid, float pol, bool masked,
-                                               bool has_den)
+                                               bool has_den, int mode = 0)
 {
     float num = raw - dark;
     bool ok = !masked && finite_f(num);
-    float v = num;
+    float v = num, den = 1.0f;
     if (has_den) {
-        float den = flat * solid * pol;
+        den = flat * solid * pol;
         ok = ok && den != 0.0f && finite_f(den);
         v = num / den;              // IEEE division (no fast-math): parity with the oracle within fp32 rounding
     }
+    if (mode == 1) v = num;
+    if (mode == 2) v = den;
     return ok ? v : quiet_nan();
 }
 
 template <int DT>
-__device__ __forceinline__ float corrected_pixel(const void *img, int64_t p, const Corrections &c)
+__device__ __forceinline__ float corrected_pixel(const void *img, int64_t p, const Corrections &c, int mode = 0)
 {
     float raw = load_raw<DT>(img, p);
     float dark = c.dark ? __ldg(c.dark + p) : 0.0f;
@@ -76,7 +80,7 @@ __device__ __forceinline__ float corrected_pixel(const void *img, int64_t p, con
     float sol = c.solidangle ? __ldg(c.solidangle + p) : 1.0f;
     float pol = c.polarization ? __ldg(c.polarization + p) : 1.0f;
     bool masked = c.mask ? (__ldg(c.mask + p) != 0) : false;
-    return correct_value(raw, dark, flat, sol, pol, masked, c.flat || c.solidangle || c.polarization);
+    return correct_value(raw, dark, flat, sol, pol, masked, c.flat || c.solidangle || c.polarization, mode);
 }
 
 // ---- accumulators -----------------------------------------------------------------------------------------------------

@@ -120,6 +120,8 @@ struct ai_ctx {
     double range_host[2] = {0.0, 0.0};   // valid after build
     ai_layout layout = AI_LAYOUT_TILED;
     ai_accum accum = AI_ACC_F32_KAHAN;
+    ai_norm norm = AI_NORM_PIXEL;
+    float *norm_scratch = nullptr;        // [2 * npt] throw-away outputs of the two passes of AI_NORM_SPLIT
     float empty_value = 0.0f;
     int device = 0;
     int sm_count = 0;
@@ -159,7 +161,8 @@ struct ai_ctx {
     float *out_dev = nullptr;       // [3*npt] device outputs of ai_integrate1d_host
     // ai_integrate1d_host_frames: double-buffered upload
     void *stage2[2] = {nullptr, nullptr};
-    size_t stage2_bytes = 0;
+    size_t stage2_bytes = 0, out2_floats = 0;
+    bool host_frames_ready = false;
     float *out2[2] = {nullptr, nullptr};
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t h2d_done[2] = {nullptr, nullptr}, slot_free[2] = {nullptr, nullptr};
@@ -238,9 +241,10 @@ struct FrameArgs {
     int64_t row_pitch = 0;       // elements between rows of `image`; 0 = width (only the library's own corrected frame differs)
 };
 int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
+int ai_launch_tiled_split(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_csr(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_lut(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_scatter(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
-int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, cudaStream_t st, float **out);   // integrate_prep.cu
+int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, int mode, cudaStream_t st, float **out);   // integrate_prep.cu
 int ai_stream_full_grid(const ai_ctx *ctx);   // integrate_stream.cu: 1 if the single-frame kernel puts one block on every SM
 int ai_stream_stages(const ai_ctx *ctx);      // integrate_stream.cu: (tile + blob) stages of the single-frame kernel, 0 = n/a

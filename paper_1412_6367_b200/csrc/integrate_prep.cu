@@ -13,7 +13,7 @@ constexpr int kPrepThreads = 256;
 template <int DT>
 __global__ void __launch_bounds__(kPrepThreads) correct_frame_kernel(const void *__restrict__ img, Corrections cor,
                                                                      int64_t npix, int width, int pitch, int vec_ok,
-                                                                     int overlap, float *__restrict__ out)
+                                                                     int overlap, int mode, float *__restrict__ out)
 {
     // Launch chain (integrate_stream.cu): the single-frame kernel that follows may start its prologue (it reads `out`
     // after its griddepcontrol.wait).  overlap: this pass itself runs beside the stream kernel of the PREVIOUS call --
@@ -35,17 +35,17 @@ __global__ void __launch_bounds__(kPrepThreads) correct_frame_kernel(const void 
             const float4 po = cor.polarization ? __ldg(reinterpret_cast<const float4 *>(cor.polarization + p)) : one4;
             const uchar4 mk = cor.mask ? __ldg(reinterpret_cast<const uchar4 *>(cor.mask + p)) : make_uchar4(0, 0, 0, 0);
             float4 v;
-            v.x = correct_value(raw.x, dk.x, fl.x, sa.x, po.x, mk.x != 0, has_den);
-            v.y = correct_value(raw.y, dk.y, fl.y, sa.y, po.y, mk.y != 0, has_den);
-            v.z = correct_value(raw.z, dk.z, fl.z, sa.z, po.z, mk.z != 0, has_den);
-            v.w = correct_value(raw.w, dk.w, fl.w, sa.w, po.w, mk.w != 0, has_den);
+            v.x = correct_value(raw.x, dk.x, fl.x, sa.x, po.x, mk.x != 0, has_den, mode);
+            v.y = correct_value(raw.y, dk.y, fl.y, sa.y, po.y, mk.y != 0, has_den, mode);
+            v.z = correct_value(raw.z, dk.z, fl.z, sa.z, po.z, mk.z != 0, has_den, mode);
+            v.w = correct_value(raw.w, dk.w, fl.w, sa.w, po.w, mk.w != 0, has_den, mode);
             *reinterpret_cast<float4 *>(out + p) = v;
         }
     } else {
         // rows of the output start on 16-byte boundaries (pitch = width rounded up to 4): what the tensor map needs
         for (int64_t p = (int64_t)blockIdx.x * kPrepThreads + threadIdx.x; p < npix; p += stride) {
             const int64_t y = p / width;
-            out[y * pitch + (p - y * width)] = corrected_pixel<DT>(img, p, cor);
+            out[y * pitch + (p - y * width)] = corrected_pixel<DT>(img, p, cor, mode);
         }
     }
     if (overlap) asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -55,8 +55,9 @@ __global__ void __launch_bounds__(kPrepThreads) correct_frame_kernel(const void 
 
 // Writes the corrected float32 image of frame 0 of `a` into one of the context's two corrected frames (*out; they
 // alternate from call to call and are allocated on first use; row pitch = width rounded up to a multiple of 4, so that
-// frames of any width reach the single-frame kernel through a tensor map).
-int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, cudaStream_t st, float **out)
+// frames of any width reach the single-frame kernel through a tensor map).  mode: 0 corrected value, 1 numerator,
+// 2 denominator (correct_value).
+int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, int mode, cudaStream_t st, float **out)
 {
     const int64_t npix = (int64_t)ctx->height * ctx->width;
     const int pitch = (ctx->width + 3) / 4 * 4;
@@ -79,7 +80,7 @@ int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, 
     cfg.attrs = attr;
     cfg.numAttrs = 1;
 #define AI_PREP(DT) \
-    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, correct_frame_kernel<DT>, a.image, cor, npix, ctx->width, pitch, vec, overlap, dst))
+    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, correct_frame_kernel<DT>, a.image, cor, npix, ctx->width, pitch, vec, overlap, mode, dst))
     switch (a.dtype) {
     case AI_F32: AI_PREP(AI_F32); break;
     case AI_I32: AI_PREP(AI_I32); break;

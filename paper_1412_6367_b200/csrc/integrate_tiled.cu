@@ -272,6 +272,68 @@ bool aligned(const void *p, size_t a) { return p == nullptr || (reinterpret_cast
 
 }  // namespace
 
+// pre-pass (cast + corrections, mode as correct_value) -> stream kernel -> finish kernel, for one frame
+static int launch_prepass_stream(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int mode, cudaStream_t st, bool *handled)
+{
+    float *corrected = nullptr;
+    int rc = ai_launch_correct(ctx, a, vec_ok, ai_stream_full_grid(ctx) && !ctx->tune.no_overlap, mode, st, &corrected);
+    if (rc != AI_OK) return rc;
+    FrameArgs b = a;
+    b.image = corrected;
+    b.dtype = AI_F32;
+    b.row_pitch = (ctx->width + 3) / 4 * 4;
+    b.frame_stride = (int64_t)ctx->height * b.row_pitch;
+    b.dark = b.flat = b.solidangle = b.polarization = nullptr;
+    b.mask = nullptr;
+    const int may_be_invalid = a.dark || a.flat || a.solidangle || a.polarization || a.mask || a.dtype == AI_F32;
+    const void *used = nullptr;
+    rc = ai_launch_stream_stage1(ctx, b, 1, may_be_invalid, 1, st, handled, &used);
+    if (rc != AI_OK || !*handled) return rc;
+    ctx->last_launches = 2;
+    if (ctx->stage1_only) return AI_OK;
+    ctx->last_launches = 3;
+    return launch_finish(ctx, a, used, st);
+}
+
+__global__ void __launch_bounds__(256) ratio_kernel(int npt, float empty, const float *__restrict__ num,
+                                                    const float *__restrict__ den, float *__restrict__ out)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < npt) out[b] = den[b] != 0.0f ? __fdiv_rn(num[b], den[b]) : empty;
+}
+
+// AI_NORM_SPLIT (ai_set_normalization): sum c (I - dark) and sum c (flat * solidangle * polarization) as two passes of
+// the same engine over the numerator and the denominator frame, then their ratio.  One frame, TILED layout.
+int ai_launch_tiled_split(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
+{
+    if (a.nframes != 1 || ctx->npt_azim > 0) return ai_fail(ctx, AI_EUNSUPPORTED, "split normalisation: one 1D frame per call");
+    if (ctx->no_prepass || ctx->no_stream || ctx->no_tma || ai_stream_stages(ctx) < 2)
+        return ai_fail(ctx, AI_EUNSUPPORTED, "split normalisation needs the pre-pass + single-frame kernel path");
+    if (!ctx->norm_scratch) AI_CUDA(ctx, cudaMalloc(&ctx->norm_scratch, 2 * (size_t)ctx->npt * sizeof(float)));
+    const size_t esz = (a.dtype == AI_U16 || a.dtype == AI_I16) ? 2 : 4;
+    const int vec_ok = ctx->width % 4 == 0 && a.frame_stride % 4 == 0 && aligned(a.image, 4 * esz) &&
+                       aligned(a.dark, 16) && aligned(a.flat, 16) && aligned(a.solidangle, 16) &&
+                       aligned(a.polarization, 16) && aligned(a.mask, 4);
+    bool handled = false;
+    FrameArgs n = a;                                   // numerator: sum_signal <- sum c (I - dark)
+    n.intensity = ctx->norm_scratch;
+    n.count = ctx->norm_scratch + ctx->npt;
+    int rc = launch_prepass_stream(ctx, n, vec_ok, 1, st, &handled);
+    if (rc != AI_OK) return rc;
+    if (!handled) return ai_fail(ctx, AI_EUNSUPPORTED, "split normalisation: the single-frame kernel does not apply");
+    FrameArgs d = a;                                   // denominator: count <- sum c (flat * solidangle * polarization)
+    d.radial = nullptr;
+    d.intensity = ctx->norm_scratch;
+    d.sum_signal = a.count;
+    d.count = ctx->norm_scratch + ctx->npt;
+    rc = launch_prepass_stream(ctx, d, vec_ok, 2, st, &handled);
+    if (rc != AI_OK) return rc;
+    ratio_kernel<<<(ctx->npt + 255) / 256, 256, 0, st>>>(ctx->npt, ctx->empty_value, a.sum_signal, a.count, a.intensity);
+    AI_CUDA(ctx, cudaGetLastError());
+    ctx->last_launches = 7;
+    return AI_OK;
+}
+
 int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 {
     const TiledLayout &tl = ctx->tl;
@@ -308,25 +370,8 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
         // 16-byte boundaries (width not a multiple of 4): H1 + H2 as a streaming pre-pass into a float32 frame with
         // padded rows (invalid pixels as NaN), then the same single-frame kernel
         if (a.nframes == 1 && !ctx->no_prepass && !ctx->no_stream && !ctx->no_tma && ai_stream_stages(ctx) >= 2) {
-            float *corrected = nullptr;
-            rc = ai_launch_correct(ctx, a, vec_ok, ai_stream_full_grid(ctx) && !ctx->tune.no_overlap, st, &corrected);
-            if (rc != AI_OK) return rc;
-            FrameArgs b = a;
-            b.image = corrected;
-            b.dtype = AI_F32;
-            b.row_pitch = (ctx->width + 3) / 4 * 4;
-            b.frame_stride = (int64_t)ctx->height * b.row_pitch;
-            b.dark = b.flat = b.solidangle = b.polarization = nullptr;
-            b.mask = nullptr;
-            const int may_be_invalid = a.dark || a.flat || a.solidangle || a.polarization || a.mask || a.dtype == AI_F32;
-            rc = ai_launch_stream_stage1(ctx, b, 1, may_be_invalid, 1, st, &handled, &used);
-            if (rc != AI_OK) return rc;
-            if (handled) {
-                ctx->last_launches = 2;
-                if (ctx->stage1_only) return AI_OK;
-                ctx->last_launches = 3;
-                return launch_finish(ctx, a, used, st);
-            }
+            rc = launch_prepass_stream(ctx, a, vec_ok, 0, st, &handled);
+            if (rc != AI_OK || handled) return rc;
         }
         rc = ensure_partials();
         if (rc != AI_OK) return rc;

@@ -576,6 +576,88 @@ def test_host_frames_entry_point(torch, B, oracle, workloads):
     integ.close()
 
 
+def test_host_frames_in_chunks_with_a_mask_and_a_stride(torch, B, oracle, workloads):
+    """19 frames = two chunks of 8 and one of 3, each one batched launch; frames 2 elements apart more than a frame."""
+    cfg = workloads.CONFIGS["cfg1b"]
+    nf, stride = 19, cfg.npix + 8
+    rng = np.random.default_rng(31)
+    buf = np.zeros(nf * stride, dtype=np.float32)
+    frames = []
+    for k in range(nf):
+        fr = rng.poisson(40.0 + 3 * k, size=cfg.npix).astype(np.float32)
+        buf[k * stride:k * stride + cfg.npix] = fr
+        frames.append(fr.reshape(cfg.height, cfg.width))
+    mask = (rng.random((cfg.height, cfg.width)) < 0.05).astype(np.uint8)
+    pinned = torch.from_numpy(buf).pin_memory()
+    outs = [torch.empty((nf, cfg.npt), dtype=torch.float32).pin_memory() for _ in range(3)]
+    integ = B.Integrator(cfg)
+    B.ai_integrate1d_host_frames(integ.ctx, pinned.numpy(), nf, stride, None, None, None, None, _dev(torch, mask),
+                                 *[o.numpy() for o in outs])
+    for k in (0, 7, 8, 15, 16, 18):
+        got = {"intensity": outs[0][k].numpy(), "sum_signal": outs[1][k].numpy(), "count": outs[2][k].numpy()}
+        assert_profile(got, _oracle_profile(oracle, cfg, workloads.Frame(image=frames[k], mask=mask)), what=f"host frame {k}")
+    integ.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1b", "cfg2", "cfg3"])
+def test_scatter_comparison_path(torch, B, oracle, workloads, parity_report, name):
+    """AI_LAYOUT_SCATTER: forward scatter with fp32 atomics -- uncompensated, order not fixed: held
+    to 2e-5 and reported."""
+    cfg = workloads.CONFIGS[name]
+    fr = workloads.make_frame(cfg)
+    integ = B.Integrator(cfg, layout=B.AI_LAYOUT_SCATTER)
+    got = _run(torch, integ, fr, radial=True)
+    want = _oracle_profile(oracle, cfg, fr)
+    worst = assert_profile(got, want, tol=2e-5, what=f"scatter/{name}")
+    again = _run(torch, integ, fr)
+    worst["bit_reproducible_in_this_run"] = bool(np.array_equal(got["sum_signal"], again["sum_signal"]))
+    print("scatter", name, worst)
+    parity_report.setdefault("scatter_with_atomics", {})[name] = worst
+    # a small batch through the same path
+    if name == "cfg1b":
+        frames = np.stack([fr.image, fr.image * 2]).astype(np.float32)
+        i, s, c = integ.integrate1d_batch(_dev(torch, frames))
+        torch.cuda.synchronize()
+        got1 = {"intensity": i[1].cpu().numpy(), "sum_signal": s[1].cpu().numpy(), "count": c[1].cpu().numpy()}
+        assert_profile(got1, _oracle_profile(oracle, cfg, workloads.Frame(image=frames[1])), tol=2e-5, what="scatter batch")
+    integ.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1b", "cfg3"])
+def test_split_normalisation(torch, B, oracle, workloads, name):
+    """ai_set_normalization(AI_NORM_SPLIT): sum c (I - dark) over sum c (flat * solidangle * polarization)."""
+    cfg = workloads.CONFIGS[name]
+    fr = workloads.make_frame(cfg)
+    if not cfg.corrections:
+        rng = np.random.default_rng(41)
+        shape = fr.image.shape
+        fr = workloads.Frame(image=fr.image, dark=rng.poisson(5.0, shape).astype(np.float32),
+                             flat=rng.uniform(0.9, 1.1, shape).astype(np.float32),
+                             solidangle=rng.uniform(0.8, 1.0, shape).astype(np.float32),
+                             polarization=rng.uniform(0.95, 1.0, shape).astype(np.float32),
+                             mask=(rng.random(shape) < 0.04).astype(np.uint8))
+    umin, umax, u0, u1 = _oracle_bounds(oracle, cfg)
+    want = oracle.integrate1d_bounds_split(umin, umax, cfg.npt, u0, u1, fr.image, fr.dark, fr.flat, fr.solidangle,
+                                           fr.polarization, fr.mask)
+    integ = B.Integrator(cfg)
+    B.ai_set_normalization(integ.ctx, B.AI_NORM_SPLIT)
+    got = _run(torch, integ, fr)
+    for key in ("intensity", "sum_signal", "count"):
+        e = rel_err(got[key], want[key])
+        assert e.max() <= 1e-6, (name, key, float(e.max()))
+    # a frame without corrections: the two estimators coincide
+    plain = workloads.Frame(image=fr.image)
+    got_p = _run(torch, integ, plain)
+    B.ai_set_normalization(integ.ctx, B.AI_NORM_PIXEL)
+    ref_p = _run(torch, integ, plain)
+    assert np.allclose(got_p["intensity"], ref_p["intensity"], rtol=1e-6)
+    # batches are refused in this mode, not silently computed with the other estimator
+    B.ai_set_normalization(integ.ctx, B.AI_NORM_SPLIT)
+    with pytest.raises(B.AzintError):
+        integ.integrate1d_batch(_dev(torch, np.stack([fr.image, fr.image])))
+    integ.close()
+
+
 def test_layout_info(torch, B, workloads):
     """ai_get_layout_info: sizes of the execution layout, consistent with the canonical CSR."""
     cfg = workloads.CONFIGS["cfg2"]
