@@ -489,6 +489,128 @@ int64_t aio_csr2d(const double *u_min, const double *u_max, const double *chi_lo
     return rc;
 }
 
+/* ==================================================================================================================
+ * Full pixel splitting (section 4.2): "no abstraction takes place and the pixel splitting works using
+ * the area of the actual pixel segments (assuming they are straight lines)".  The pixel is the quadrilateral spanned by
+ * its four corners in the (radial unit, chi) plane, sides taken as straight lines; the weight of the pixel in bin b is
+ * the area of the part of that quadrilateral between the bin's two edges over the area of the whole quadrilateral.
+ * As the paper describes it: "a function for each of the lines that make up the sides of the pixel is defined by
+ * calculating the slope and the point of intersection ... the algorithm loops over the bins that the pixel spans over
+ * and proceeds to integrate the four functions ... over the bounds of each bin.  Taking the absolute value of the sum of
+ * all these integrals will yield the area of the pixel segment".
+ * Readings: corner angles are measured from the direction of the pixel centre (no seam); a corner on the beam centre
+ * takes the centre direction; a pixel with the beam centre strictly inside, or whose corners are collinear in this plane
+ * (zero area), is split by its bounding box instead (section 4.1).
+ * ================================================================================================================== */
+
+/* corners (x_lo,y_lo) (x_hi,y_lo) (x_hi,y_hi) (x_lo,y_hi) of pixel (i, j) in the (u, chi) plane; returns 0 if the beam
+ * centre is strictly inside the pixel (no quadrilateral) */
+static int pixel_corners(const aio_geometry *g, int unit, int i, int j, double u[4], double chi[4])
+{
+    double x_lo = ((double)j - g->center_x_px) * g->pixel_x_m;
+    double x_hi = ((double)(j + 1) - g->center_x_px) * g->pixel_x_m;
+    double y_lo = ((double)i - g->center_y_px) * g->pixel_y_m;
+    double y_hi = ((double)(i + 1) - g->center_y_px) * g->pixel_y_m;
+    if (x_lo < 0.0 && x_hi > 0.0 && y_lo < 0.0 && y_hi > 0.0) return 0;
+    double xc = 0.5 * (x_lo + x_hi), yc = 0.5 * (y_lo + y_hi);
+    double chi_c = atan2(yc, xc);
+    double xs[4] = {x_lo, x_hi, x_hi, x_lo}, ys[4] = {y_lo, y_lo, y_hi, y_hi};
+    for (int k = 0; k < 4; ++k) {
+        u[k] = unit_of_r(sqrt(xs[k] * xs[k] + ys[k] * ys[k]), g, unit);
+        chi[k] = (xs[k] == 0.0 && ys[k] == 0.0) ? chi_c
+                                                : chi_c + atan2(xc * ys[k] - yc * xs[k], xc * xs[k] + yc * ys[k]);
+    }
+    return 1;
+}
+
+int aio_pixel_corners(const aio_geometry *g, int height, int width, int unit, double *u4, double *chi4, uint8_t *has_quad)
+{
+    if (!g || height < 1 || width < 1 || unit < 0 || unit > 4) return -1;
+    for (int i = 0; i < height; ++i)
+        for (int j = 0; j < width; ++j) {
+            int64_t p = (int64_t)i * width + j;
+            has_quad[p] = (uint8_t)pixel_corners(g, unit, i, j, u4 + 4 * p, chi4 + 4 * p);
+        }
+    return 0;
+}
+
+/* signed integral of the line through (f_a, c_a) and (f_b, c_b) over the part of [lo, hi] it spans, along its direction */
+static double edge_integral(double f_a, double c_a, double f_b, double c_b, double lo, double hi)
+{
+    if (f_a == f_b) return 0.0;                                  /* a side parallel to the chi axis sweeps no area */
+    double m = (c_b - c_a) / (f_b - f_a);                        /* slope; c_a - m f_a is the point of intersection */
+    double e_lo = max2(lo, min2(f_a, f_b)), e_hi = min2(hi, max2(f_a, f_b));
+    if (!(e_hi > e_lo)) return 0.0;
+    double v_lo = c_a + m * (e_lo - f_a), v_hi = c_a + m * (e_hi - f_a);
+    double area = 0.5 * (v_lo + v_hi) * (e_hi - e_lo);
+    return f_b > f_a ? area : -area;
+}
+
+/* full splitting of one quadrilateral; same conventions as aio_split (bins half-open, last closed, returns the count) */
+int aio_split_full(const double *u, const double *chi, double u0, double u1, int npt, int *bins, double *coefs, int cap)
+{
+    double delta = (u1 - u0) / (double)npt, f[4];
+    double f_min = 0.0, f_max = 0.0;
+    for (int k = 0; k < 4; ++k) {
+        f[k] = (u[k] - u0) / delta;
+        if (k == 0 || f[k] < f_min) f_min = f[k];
+        if (k == 0 || f[k] > f_max) f_max = f[k];
+    }
+    double total = 0.0;
+    for (int k = 0; k < 4; ++k) total += edge_integral(f[k], chi[k], f[(k + 1) & 3], chi[(k + 1) & 3], f_min, f_max);
+    total = fabs(total);
+    if (!(total > 0.0)) return aio_split(u0 + f_min * delta, u0 + f_max * delta, u0, u1, npt, bins, coefs, cap);
+    if (!(f_max > 0.0) || !(f_min < (double)npt)) return 0;
+    int b_first = (int)floor(max2(f_min, 0.0)), b_last = (int)floor(min2(f_max, (double)npt)), n = 0;
+    if (b_last > npt - 1) b_last = npt - 1;
+    for (int b = b_first; b <= b_last; ++b) {
+        double area = 0.0;
+        for (int k = 0; k < 4; ++k)
+            area += edge_integral(f[k], chi[k], f[(k + 1) & 3], chi[(k + 1) & 3], (double)b, (double)(b + 1));
+        area = fabs(area);
+        if (area > 0.0) {
+            if (n < cap) { bins[n] = b; coefs[n] = area / total; }
+            ++n;
+        }
+    }
+    return n;
+}
+
+/* CSR of the full-splitting matrix (two calls as aio_csr); u_min / u_max are the bounding-box bounds, used for the
+ * pixels that have no quadrilateral */
+int64_t aio_csr_full(const double *u4, const double *chi4, const uint8_t *has_quad, const double *u_min,
+                     const double *u_max, int64_t npix, int npt, double u0, double u1,
+                     int64_t *indptr, int32_t *indices, double *data)
+{
+    int bins[AIO_MAX_SPLIT]; double coefs[AIO_MAX_SPLIT];
+    int64_t *len = (int64_t *)calloc((size_t)npt + 1, sizeof(int64_t));
+    if (!len) return -2;
+    for (int pass = 0; pass < 2; ++pass) {
+        if (pass == 1) {
+            indptr[0] = 0;
+            for (int b = 0; b < npt; ++b) indptr[b + 1] = indptr[b] + len[b];
+            if (!indices || !data) break;
+            for (int b = 0; b < npt; ++b) len[b] = indptr[b];
+        }
+        for (int64_t p = 0; p < npix; ++p) {
+            int n = has_quad[p] ? aio_split_full(u4 + 4 * p, chi4 + 4 * p, u0, u1, npt, bins, coefs, AIO_MAX_SPLIT)
+                                : aio_split(u_min[p], u_max[p], u0, u1, npt, bins, coefs, AIO_MAX_SPLIT);
+            if (n > AIO_MAX_SPLIT) { free(len); return -3; }
+            for (int k = 0; k < n; ++k) {
+                if (pass == 0) len[bins[k]]++;
+                else {
+                    int64_t pos = len[bins[k]]++;
+                    indices[pos] = (int32_t)p;
+                    data[pos] = coefs[k];
+                }
+            }
+        }
+    }
+    int64_t nnz = indptr[npt];
+    free(len);
+    return nnz;
+}
+
 int aio_num_threads_available(void)
 {
 #ifdef _OPENMP

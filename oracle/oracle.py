@@ -45,6 +45,11 @@ def lib():
         L.aio_csr2d.argtypes = [dp, dp, dp, dp, C.c_int64, C.c_int, C.c_double, C.c_double, C.c_int, C.c_double,
                                 C.c_double, C.POINTER(C.c_int64), C.POINTER(C.c_int32), dp]
         L.aio_csr2d.restype = C.c_int64
+        L.aio_pixel_corners.argtypes = [C.POINTER(Geometry), C.c_int, C.c_int, C.c_int, dp, dp, u8p]
+        L.aio_split_full.argtypes = [dp, dp, C.c_double, C.c_double, C.c_int, ip, dp, C.c_int]
+        L.aio_csr_full.argtypes = [dp, dp, u8p, dp, dp, C.c_int64, C.c_int, C.c_double, C.c_double,
+                                   C.POINTER(C.c_int64), C.POINTER(C.c_int32), dp]
+        L.aio_csr_full.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -222,6 +227,70 @@ def csr2d(umin, umax, chi_lo, chi_w, npt_rad, u0, u1, npt_azim, c0, c1):
     lib().aio_csr2d(*a, keep[0][0].size, npt_rad, u0, u1, npt_azim, c0, c1, pi,
                     indices.ctypes.data_as(C.POINTER(C.c_int32)), data.ctypes.data_as(C.POINTER(C.c_double)))
     return indptr, indices, data
+
+
+# ---- full pixel splitting -------------------------------------------------------------------------------
+def pixel_corners(cfg):
+    """(u4 [npix][4], chi4 [npix][4], has_quad [npix]): the pixels' corners in the (radial unit, chi) plane."""
+    n = cfg.height * cfg.width
+    u4, c4, q = np.empty((n, 4)), np.empty((n, 4)), np.empty(n, dtype=np.uint8)
+    g = geometry(cfg)
+    dp = C.POINTER(C.c_double)
+    rc = lib().aio_pixel_corners(C.byref(g), cfg.height, cfg.width, cfg.unit, u4.ctypes.data_as(dp), c4.ctypes.data_as(dp),
+                                 q.ctypes.data_as(C.POINTER(C.c_uint8)))
+    if rc:
+        raise ValueError(f"aio_pixel_corners: {rc}")
+    return u4, c4, q
+
+
+def split_full(u4, chi4, u0, u1, npt, cap=4096):
+    bins = (C.c_int * cap)()
+    coefs = (C.c_double * cap)()
+    dp = C.POINTER(C.c_double)
+    a, b = np.ascontiguousarray(u4, dtype=np.float64), np.ascontiguousarray(chi4, dtype=np.float64)
+    n = lib().aio_split_full(a.ctypes.data_as(dp), b.ctypes.data_as(dp), u0, u1, npt, bins, coefs, cap)
+    return list(bins[:n]), list(coefs[:n])
+
+
+def csr_full(cfg, u0=None, u1=None):
+    """Oracle CSR of the full-splitting matrix (the range defaults to the bounding-box automatic range)."""
+    umin, umax = pixel_bounds(cfg)
+    if u0 is None:
+        u0, u1 = auto_range(umin, umax)
+    u4, c4, q = pixel_corners(cfg)
+    dp = C.POINTER(C.c_double)
+    indptr = np.zeros(cfg.npt + 1, dtype=np.int64)
+    pi = indptr.ctypes.data_as(C.POINTER(C.c_int64))
+    args = (u4.ctypes.data_as(dp), c4.ctypes.data_as(dp), q.ctypes.data_as(C.POINTER(C.c_uint8)),
+            umin.ctypes.data_as(dp), umax.ctypes.data_as(dp), umin.size, cfg.npt, u0, u1, pi)
+    nnz = lib().aio_csr_full(*args, None, None)
+    if nnz < 0:
+        raise ValueError(f"aio_csr_full: {nnz}")
+    indices = np.empty(nnz, dtype=np.int32)
+    data = np.empty(nnz, dtype=np.float64)
+    lib().aio_csr_full(*args, indices.ctypes.data_as(C.POINTER(C.c_int32)), data.ctypes.data_as(dp))
+    return indptr, indices, data, (u0, u1)
+
+
+def integrate1d_full(cfg, frame, empty=0.0):
+    """Full pixel splitting as matrix x corrected frame in float64: dict(radial, intensity, sum_signal, count)."""
+    import scipy.sparse as sp
+    indptr, indices, data, (u0, u1) = csr_full(cfg)
+    m = sp.csr_matrix((data, indices, indptr), shape=(cfg.npt, cfg.npix))
+    img = np.asarray(frame.image, dtype=np.float64).ravel()
+    num = img - (0.0 if frame.dark is None else np.asarray(frame.dark, dtype=np.float64).ravel())
+    den = np.ones_like(img)
+    for a in (frame.flat, frame.solidangle, frame.polarization):
+        if a is not None:
+            den = den * np.asarray(a, dtype=np.float64).ravel()
+    ok = np.isfinite(num) & np.isfinite(den) & (den != 0.0)
+    if frame.mask is not None:
+        ok &= np.asarray(frame.mask).ravel() == 0
+    v = np.where(ok, num / np.where(den != 0.0, den, 1.0), 0.0)
+    S, Cn = m @ v, m @ ok.astype(np.float64)
+    out = {"sum_signal": S, "count": Cn, "intensity": np.where(Cn > 0, S / np.where(Cn > 0, Cn, 1.0), empty),
+           "radial": u0 + (np.arange(cfg.npt) + 0.5) * (u1 - u0) / cfg.npt, "range": (u0, u1)}
+    return out
 
 
 def num_threads_available() -> int:
