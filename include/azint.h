@@ -70,6 +70,14 @@ typedef enum { AI_ACC_F32_KAHAN = 0, AI_ACC_F32_PLAIN = 1, AI_ACC_F64 = 2 } ai_a
  *                  ratio (`count` then carries the summed normalisation).  One 1D frame per call, AI_LAYOUT_TILED. */
 typedef enum { AI_NORM_PIXEL = 0, AI_NORM_SPLIT = 1 } ai_norm;
 
+/* pixel-splitting scheme of the matrix (section 4):
+ *   AI_SPLIT_BBOX  bounding box: the pixel's extent along the radial axis, split by overlap / width
+ *   AI_SPLIT_FULL  full pixel splitting: the quadrilateral of the pixel's four corners in the (radial
+ *                  unit, chi) plane with straight sides; weight = area between the bin's edges / area of the whole.  A
+ *                  pixel that holds the beam centre strictly inside, or has no area in that plane, keeps its bounding box.
+ *                  1D only.  The automatic range is the bounding-box one in both schemes. */
+typedef enum { AI_SPLIT_BBOX = 0, AI_SPLIT_FULL = 1 } ai_split;
+
 /* planar detector orthogonal to the beam; lengths in metres, centre in pixels */
 typedef struct {
     double distance_m;
@@ -100,6 +108,10 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
  * (AI_LAYOUT_LUT is not offered in 2D).  Errors: AI_EINVAL, AI_ENOMEM. */
 int ai_setup2d(ai_ctx **out, const ai_geometry *g, int height, int width, int npt_rad, int npt_azim, ai_unit unit,
                const double *range_or_null, const double *azim_range_or_null);
+
+/* Choose the pixel-splitting scheme; between ai_setup and ai_build_csr.  Errors: AI_EINVAL (unknown value, or the matrix
+ * is already built), AI_EUNSUPPORTED (AI_SPLIT_FULL on a bidimensional context). */
+int ai_set_splitting(ai_ctx *ctx, ai_split split);
 
 /* Build the matrix on the device: bounds -> range -> count -> exclusive scan -> ordered fill (PAPER.md:120-122 for
  * the coefficients, :150 scan, :180 CSR), then the tiled execution layout.  Idempotent.  Synchronises `cuda_stream`.

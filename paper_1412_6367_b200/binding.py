@@ -19,9 +19,10 @@ AI_F32, AI_I32, AI_U16, AI_I16, AI_U32 = range(5)
 AI_LAYOUT_TILED, AI_LAYOUT_CSR, AI_LAYOUT_LUT, AI_LAYOUT_TILED_DIRECT, AI_LAYOUT_SCATTER = range(5)
 AI_ACC_F32_KAHAN, AI_ACC_F32_PLAIN, AI_ACC_F64 = range(3)
 AI_NORM_PIXEL, AI_NORM_SPLIT = range(2)
+AI_SPLIT_BBOX, AI_SPLIT_FULL = range(2)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
+EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_set_splitting", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
            "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_get_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
@@ -57,6 +58,7 @@ def lib():
     L.ai_copy_csr_to_host.argtypes = [vp, vp, vp, vp]
     L.ai_set_options.argtypes = [vp, C.c_int, C.c_int, C.c_float]
     L.ai_set_normalization.argtypes = [vp, C.c_int]
+    L.ai_set_splitting.argtypes = [vp, C.c_int]
     L.ai_integrate1d.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
     L.ai_integrate1d_batch.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_integrate1d_host.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, vp]
@@ -159,6 +161,10 @@ def ai_set_options(ctx, layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN, empty_va
     _check(lib().ai_set_options(ctx, layout, accum, empty_value), ctx)
 
 
+def ai_set_splitting(ctx, split=AI_SPLIT_BBOX):
+    _check(lib().ai_set_splitting(ctx, split), ctx)
+
+
 def ai_set_normalization(ctx, norm=AI_NORM_PIXEL):
     _check(lib().ai_set_normalization(ctx, norm), ctx)
 
@@ -230,7 +236,7 @@ class Integrator:
     (e.g. workloads.Config).  Outputs are torch float32 CUDA tensors allocated here for convenience."""
 
     def __init__(self, cfg, radial_range=None, device=None, layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN,
-                 empty_value=0.0, azim_range=None):
+                 empty_value=0.0, azim_range=None, split=AI_SPLIT_BBOX):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1412_6367_b200 needs a CUDA device (no CPU fallback)")
@@ -255,6 +261,8 @@ class Integrator:
         else:
             self.ctx = ai_setup(cfg.distance_m, cfg.pixel_m, cfg.pixel_m, cfg.center_y_px, cfg.center_x_px,
                                 cfg.wavelength_m, cfg.height, cfg.width, cfg.npt, cfg.unit, radial_range)
+        if split != AI_SPLIT_BBOX:
+            ai_set_splitting(self.ctx, split)
         with torch.cuda.device(self.device):
             ai_build_csr(self.ctx)
         ai_set_options(self.ctx, layout, accum, empty_value)

@@ -191,6 +191,8 @@ int ai_build_csr(ai_ctx *ctx, void *cuda_stream)
             free(h);
             AI_CUDA(ctx, e);
         }
+    } else if (ctx->split == AI_SPLIT_FULL) {
+        rc = ai_build_full(ctx, st);
     } else {
         PixelSpans spans;
         rc = ai_build_canonical(ctx, &spans, st);
@@ -243,6 +245,16 @@ int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_va
     ctx->layout = layout;
     ctx->accum = accum;
     ctx->empty_value = empty_value;
+    return AI_OK;
+}
+
+int ai_set_splitting(ai_ctx *ctx, ai_split split)
+{
+    if (!ctx) return AI_EINVAL;
+    if ((int)split < AI_SPLIT_BBOX || (int)split > AI_SPLIT_FULL) return ai_fail(ctx, AI_EINVAL, "bad splitting %d", (int)split);
+    if (ctx->built) return ai_fail(ctx, AI_EINVAL, "the matrix is already built");
+    if (split == AI_SPLIT_FULL && ctx->npt_azim > 0) return ai_fail(ctx, AI_EUNSUPPORTED, "full pixel splitting is 1D only");
+    ctx->split = split;
     return AI_OK;
 }
 

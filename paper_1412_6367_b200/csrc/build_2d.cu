@@ -318,49 +318,18 @@ template <class T> struct DevBuf {       // freed on every return path
 
 }  // namespace
 
-int ai_build_2d(ai_ctx *ctx, cudaStream_t st)
+// From the unsorted entries (key = bin << 32 | pixel, coefficient) to the canonical CSR and the tiled + sliced execution
+// layout.  keys_a / vals_a hold the entries; keys_b / vals_b are work buffers of the same size.
+static int entries_to_layouts(ai_ctx *ctx, Scratch &scr, unsigned long long *keys_a_p, unsigned long long *keys_b_p,
+                              float *vals_a_p, float *vals_b_p, long long nnz, long long nbins, cudaStream_t st)
 {
-    const int H = ctx->height, W = ctx->width, npt_rad = ctx->npt_rad, npt_azim = ctx->npt_azim;
-    const int64_t npix = (int64_t)H * W;
-    const long long nbins = (long long)npt_rad * npt_azim;
-    if (nbins > 0xfffffffLL) return ai_fail(ctx, AI_EUNSUPPORTED, "%lld bins: more than 2^28", nbins);
+    const int H = ctx->height, W = ctx->width;
     TiledLayout &tl = ctx->tl;
     const int grid = 148 * 8;
-    Scratch scr;
-
-    // ---- per-pixel spans on both axes -------------------------------------------------------------------------------------
-    PixelSpans sp;
-    int rc = ai_build_spans(ctx, &sp, npt_rad, st);
-    if (rc != AI_OK) { ai_free_spans(&sp); return rc; }
-    struct SpanGuard { PixelSpans *s; ~SpanGuard() { ai_free_spans(s); } } span_guard{&sp};
-    const double c0 = ctx->azim_host[0], dchi = (ctx->azim_host[1] - ctx->azim_host[0]) / (double)npt_azim;
-    DevBuf<double> chi_lo, chi_w;
-    DevBuf<long long> cnt, off;
-    AI_CUDA(ctx, chi_lo.alloc(npix));
-    AI_CUDA(ctx, chi_w.alloc(npix));
-    AI_CUDA(ctx, cnt.alloc(npix + 1));
-    AI_CUDA(ctx, off.alloc(npix + 1));
-    chi_kernel<<<grid, 256, 0, st>>>(ctx->geo, H, W, chi_lo.p, chi_w.p);
-    AI_CUDA(ctx, cudaMemsetAsync(cnt.p + npix, 0, sizeof(long long), st));
-    count2d_kernel<<<grid, 256, 0, st>>>(npix, sp.nb, chi_lo.p, chi_w.p, c0, dchi, npt_azim, cnt.p);
-    AI_CUDA(ctx, cudaGetLastError());
-    AI_CUDA(ctx, exclusive_sum(scr, cnt.p, off.p, npix + 1, st));
-    long long nnz = 0;
-    AI_CUDA(ctx, cudaMemcpyAsync(&nnz, off.p + npix, sizeof(long long), cudaMemcpyDeviceToHost, st));
-    AI_CUDA(ctx, cudaStreamSynchronize(st));
-    if (nnz > 0x7fffffffLL) return ai_fail(ctx, AI_EUNSUPPORTED, "2D matrix has %lld entries", nnz);
-    ctx->nnz = nnz;
-
-    // ---- entries, sorted by (bin, pixel): the canonical CSR -----------------------------------------------------------------
-    DevBuf<unsigned long long> keys_a, keys_b;
-    DevBuf<float> vals_a, vals_b;
-    AI_CUDA(ctx, keys_a.alloc(nnz));
-    AI_CUDA(ctx, keys_b.alloc(nnz));
-    AI_CUDA(ctx, vals_a.alloc(nnz));
-    AI_CUDA(ctx, vals_b.alloc(nnz));
-    emit2d_kernel<<<grid, 256, 0, st>>>(npix, npt_rad, npt_azim, sp.fmin, sp.fmax, sp.first, sp.nb, chi_lo.p, chi_w.p, c0,
-                                        dchi, off.p, keys_a.p, vals_a.p);
-    AI_CUDA(ctx, cudaGetLastError());
+    int rc = AI_OK;
+    struct { unsigned long long *p; } keys_a{keys_a_p}, keys_b{keys_b_p};
+    struct { float *p; } vals_a{vals_a_p}, vals_b{vals_b_p};
+    (void)H;
     AI_CUDA(ctx, sort_pairs(scr, keys_a.p, keys_b.p, vals_a.p, vals_b.p, nnz, 32 + bits_for(nbins), st));
     const size_t nnz_alloc = nnz > 0 ? (size_t)nnz : 1;
     AI_CUDA(ctx, cudaMalloc(&ctx->indptr, ((size_t)nbins + 1) * sizeof(int32_t)));
@@ -482,4 +451,201 @@ int ai_build_2d(ai_ctx *ctx, cudaStream_t st)
     rc = ai_build_sliced_fill(ctx, sc, st);
     if (rc != AI_OK) return rc;
     return ai_tiled_finalize(ctx, st);
+}
+
+int ai_build_2d(ai_ctx *ctx, cudaStream_t st)
+{
+    const int H = ctx->height, W = ctx->width, npt_rad = ctx->npt_rad, npt_azim = ctx->npt_azim;
+    const int64_t npix = (int64_t)H * W;
+    const long long nbins = (long long)npt_rad * npt_azim;
+    if (nbins > 0xfffffffLL) return ai_fail(ctx, AI_EUNSUPPORTED, "%lld bins: more than 2^28", nbins);
+    TiledLayout &tl = ctx->tl;
+    const int grid = 148 * 8;
+    Scratch scr;
+
+    // ---- per-pixel spans on both axes -------------------------------------------------------------------------------------
+    PixelSpans sp;
+    int rc = ai_build_spans(ctx, &sp, npt_rad, st);
+    if (rc != AI_OK) { ai_free_spans(&sp); return rc; }
+    struct SpanGuard { PixelSpans *s; ~SpanGuard() { ai_free_spans(s); } } span_guard{&sp};
+    const double c0 = ctx->azim_host[0], dchi = (ctx->azim_host[1] - ctx->azim_host[0]) / (double)npt_azim;
+    DevBuf<double> chi_lo, chi_w;
+    DevBuf<long long> cnt, off;
+    AI_CUDA(ctx, chi_lo.alloc(npix));
+    AI_CUDA(ctx, chi_w.alloc(npix));
+    AI_CUDA(ctx, cnt.alloc(npix + 1));
+    AI_CUDA(ctx, off.alloc(npix + 1));
+    chi_kernel<<<grid, 256, 0, st>>>(ctx->geo, H, W, chi_lo.p, chi_w.p);
+    AI_CUDA(ctx, cudaMemsetAsync(cnt.p + npix, 0, sizeof(long long), st));
+    count2d_kernel<<<grid, 256, 0, st>>>(npix, sp.nb, chi_lo.p, chi_w.p, c0, dchi, npt_azim, cnt.p);
+    AI_CUDA(ctx, cudaGetLastError());
+    AI_CUDA(ctx, exclusive_sum(scr, cnt.p, off.p, npix + 1, st));
+    long long nnz = 0;
+    AI_CUDA(ctx, cudaMemcpyAsync(&nnz, off.p + npix, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    if (nnz > 0x7fffffffLL) return ai_fail(ctx, AI_EUNSUPPORTED, "2D matrix has %lld entries", nnz);
+    ctx->nnz = nnz;
+
+    // ---- entries, sorted by (bin, pixel): the canonical CSR -----------------------------------------------------------------
+    DevBuf<unsigned long long> keys_a, keys_b;
+    DevBuf<float> vals_a, vals_b;
+    AI_CUDA(ctx, keys_a.alloc(nnz));
+    AI_CUDA(ctx, keys_b.alloc(nnz));
+    AI_CUDA(ctx, vals_a.alloc(nnz));
+    AI_CUDA(ctx, vals_b.alloc(nnz));
+    emit2d_kernel<<<grid, 256, 0, st>>>(npix, npt_rad, npt_azim, sp.fmin, sp.fmax, sp.first, sp.nb, chi_lo.p, chi_w.p, c0,
+                                        dchi, off.p, keys_a.p, vals_a.p);
+    AI_CUDA(ctx, cudaGetLastError());
+    return entries_to_layouts(ctx, scr, keys_a.p, keys_b.p, vals_a.p, vals_b.p, nnz, nbins, st);
+}
+
+// ======================================================================================================================
+// Full pixel splitting (section 4.2): the pixel is the quadrilateral of its four corners in the (radial
+// unit, chi) plane, its sides straight lines; the weight in bin b is the area of the part of the quadrilateral between
+// the bin's edges -- "integrate the four functions ... over the bounds of each bin", absolute value of the sum -- over
+// the area of the whole.  A pixel with the beam centre strictly inside, or with zero area in this plane, is split by its
+// bounding box (section 4.1).  Same sort-based path to the layouts as the 2D matrix.
+// ======================================================================================================================
+namespace {
+
+// signed integral of the line through (f_a, c_a) and (f_b, c_b) over the part of [lo, hi] it spans, along its direction
+__device__ __forceinline__ double edge_integral(double f_a, double c_a, double f_b, double c_b, double lo, double hi)
+{
+    if (f_a == f_b) return 0.0;
+    const double m = __ddiv_rn(__dsub_rn(c_b, c_a), __dsub_rn(f_b, f_a));
+    const double e_lo = fmax(lo, fmin(f_a, f_b)), e_hi = fmin(hi, fmax(f_a, f_b));
+    if (!(e_hi > e_lo)) return 0.0;
+    const double v_lo = __dadd_rn(c_a, __dmul_rn(m, __dsub_rn(e_lo, f_a))), v_hi = __dadd_rn(c_a, __dmul_rn(m, __dsub_rn(e_hi, f_a)));
+    const double area = __dmul_rn(__dmul_rn(0.5, __dadd_rn(v_lo, v_hi)), __dsub_rn(e_hi, e_lo));
+    return f_b > f_a ? area : -area;
+}
+
+struct Quad {
+    double f[4], chi[4];
+    double f_min, f_max, total;       // total = 0: no quadrilateral (bounding-box split of [f_min, f_max])
+};
+
+__device__ __forceinline__ double quad_slice(const Quad &q, double lo, double hi)
+{
+    double a = 0.0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) a = __dadd_rn(a, edge_integral(q.f[k], q.chi[k], q.f[(k + 1) & 3], q.chi[(k + 1) & 3], lo, hi));
+    return fabs(a);
+}
+
+// corners (x_lo,y_lo) (x_hi,y_lo) (x_hi,y_hi) (x_lo,y_hi) of pixel (i, j) in bin units / radians; false if the beam
+// centre is strictly inside
+__device__ __forceinline__ bool pixel_quad(const ai_geometry &g, int unit, int i, int j, double u0, double delta, Quad *q)
+{
+    const double x_lo = __dmul_rn(__dsub_rn((double)j, g.center_x_px), g.pixel_x_m);
+    const double x_hi = __dmul_rn(__dsub_rn((double)(j + 1), g.center_x_px), g.pixel_x_m);
+    const double y_lo = __dmul_rn(__dsub_rn((double)i, g.center_y_px), g.pixel_y_m);
+    const double y_hi = __dmul_rn(__dsub_rn((double)(i + 1), g.center_y_px), g.pixel_y_m);
+    if (x_lo < 0.0 && x_hi > 0.0 && y_lo < 0.0 && y_hi > 0.0) return false;
+    const double xc = __dmul_rn(0.5, __dadd_rn(x_lo, x_hi)), yc = __dmul_rn(0.5, __dadd_rn(y_lo, y_hi));
+    const double chi_c = atan2(yc, xc);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const double x = (k == 1 || k == 2) ? x_hi : x_lo, y = (k >= 2) ? y_hi : y_lo;
+        const double r = __dsqrt_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)));
+        q->f[k] = __ddiv_rn(__dsub_rn(unit_of_r(r, g.distance_m, g.wavelength_m, unit), u0), delta);
+        q->chi[k] = (x == 0.0 && y == 0.0)
+                        ? chi_c
+                        : __dadd_rn(chi_c, atan2(__dsub_rn(__dmul_rn(xc, y), __dmul_rn(yc, x)),
+                                                 __dadd_rn(__dmul_rn(xc, x), __dmul_rn(yc, y))));
+    }
+    q->f_min = fmin(fmin(q->f[0], q->f[1]), fmin(q->f[2], q->f[3]));
+    q->f_max = fmax(fmax(q->f[0], q->f[1]), fmax(q->f[2], q->f[3]));
+    q->total = quad_slice(*q, q->f_min, q->f_max);
+    return true;
+}
+
+// COUNT = true: number of entries of every pixel; false: the entries themselves at offset[p]
+template <bool COUNT>
+__global__ void __launch_bounds__(256) full_split_kernel(ai_geometry g, int unit, int height, int width, int npt,
+                                                         const double *__restrict__ range,
+                                                         const double *__restrict__ fmin_a, const double *__restrict__ fmax_a,
+                                                         const int *__restrict__ first_a, const int *__restrict__ nb_a,
+                                                         long long *__restrict__ cnt, const long long *__restrict__ offset,
+                                                         unsigned long long *__restrict__ keys, float *__restrict__ vals)
+{
+    const int64_t n = (int64_t)height * width;
+    const double u0 = range[0], delta = __ddiv_rn(__dsub_rn(range[1], range[0]), (double)npt);
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(p / width), j = (int)(p - (int64_t)i * width);
+        Quad q;
+        long long at = COUNT ? 0 : offset[p];
+        int count = 0;
+        const bool quad = pixel_quad(g, unit, i, j, u0, delta, &q);
+        if (quad && q.total > 0.0) {
+            if (q.f_max > 0.0 && q.f_min < (double)npt) {
+                const int b0 = (int)floor(fmax(q.f_min, 0.0)), b1 = min((int)floor(fmin(q.f_max, (double)npt)), npt - 1);
+                for (int b = b0; b <= b1; ++b) {
+                    const double area = quad_slice(q, (double)b, (double)(b + 1));
+                    if (!(area > 0.0)) continue;
+                    if (!COUNT) {
+                        keys[at] = ((unsigned long long)b << 32) | (unsigned long long)p;
+                        vals[at] = (float)__ddiv_rn(area, q.total);
+                        ++at;
+                    }
+                    ++count;
+                }
+            }
+        } else {
+            // bounding box: of the pixel rectangle (beam centre inside), or of the degenerate quadrilateral's corners
+            double f_lo = fmin_a[p], f_hi = fmax_a[p];
+            int first = first_a[p], nb = nb_a[p];
+            if (quad) {
+                f_lo = q.f_min;
+                f_hi = q.f_max;
+                split_span(f_lo, f_hi, npt, &first, &nb);
+            }
+            for (int b = first; b < first + nb; ++b) {
+                if (!COUNT) {
+                    keys[at] = ((unsigned long long)b << 32) | (unsigned long long)p;
+                    vals[at] = (float)split_coefficient(f_lo, f_hi, b, npt);
+                    ++at;
+                }
+                ++count;
+            }
+        }
+        if (COUNT) cnt[p] = count;
+    }
+}
+
+}  // namespace
+
+int ai_build_full(ai_ctx *ctx, cudaStream_t st)
+{
+    const int H = ctx->height, W = ctx->width, npt = ctx->npt;
+    const int64_t npix = (int64_t)H * W;
+    const int grid = 148 * 8;
+    Scratch scr;
+    PixelSpans sp;                       // bounding-box spans: the automatic range, and the pixels without a quadrilateral
+    int rc = ai_build_spans(ctx, &sp, npt, st);
+    if (rc != AI_OK) { ai_free_spans(&sp); return rc; }
+    struct SpanGuard { PixelSpans *s; ~SpanGuard() { ai_free_spans(s); } } span_guard{&sp};
+    DevBuf<long long> cnt, off;
+    AI_CUDA(ctx, cnt.alloc(npix + 1));
+    AI_CUDA(ctx, off.alloc(npix + 1));
+    AI_CUDA(ctx, cudaMemsetAsync(cnt.p + npix, 0, sizeof(long long), st));
+    full_split_kernel<true><<<grid, 256, 0, st>>>(ctx->geo, (int)ctx->unit, H, W, npt, ctx->d_range, sp.fmin, sp.fmax,
+                                                  sp.first, sp.nb, cnt.p, nullptr, nullptr, nullptr);
+    AI_CUDA(ctx, cudaGetLastError());
+    AI_CUDA(ctx, exclusive_sum(scr, cnt.p, off.p, npix + 1, st));
+    long long nnz = 0;
+    AI_CUDA(ctx, cudaMemcpyAsync(&nnz, off.p + npix, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    if (nnz > 0x7fffffffLL) return ai_fail(ctx, AI_EUNSUPPORTED, "matrix has %lld entries", nnz);
+    ctx->nnz = nnz;
+    DevBuf<unsigned long long> keys_a, keys_b;
+    DevBuf<float> vals_a, vals_b;
+    AI_CUDA(ctx, keys_a.alloc(nnz));
+    AI_CUDA(ctx, keys_b.alloc(nnz));
+    AI_CUDA(ctx, vals_a.alloc(nnz));
+    AI_CUDA(ctx, vals_b.alloc(nnz));
+    full_split_kernel<false><<<grid, 256, 0, st>>>(ctx->geo, (int)ctx->unit, H, W, npt, ctx->d_range, sp.fmin, sp.fmax,
+                                                   sp.first, sp.nb, nullptr, off.p, keys_a.p, vals_a.p);
+    AI_CUDA(ctx, cudaGetLastError());
+    return entries_to_layouts(ctx, scr, keys_a.p, keys_b.p, vals_a.p, vals_b.p, nnz, npt, st);
 }

@@ -4,6 +4,25 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "../../include/azint.h"
+
+constexpr double kBuildPi = 3.14159265358979323846;
+
+// B1 (map): radial coordinate of a radius r in the requested unit, fp64, every operation
+// rounded once.
+__device__ __forceinline__ double unit_of_r(double r, double dist, double lambda, int unit)
+{
+    switch (unit) {
+    case AI_R_MM: return __dmul_rn(1e3, r);
+    case AI_TTH_RAD: return atan(__ddiv_rn(r, dist));
+    case AI_TTH_DEG: return __ddiv_rn(__dmul_rn(atan(__ddiv_rn(r, dist)), 180.0), kBuildPi);
+    case AI_Q_NM:
+        return __dmul_rn(1e-9, __ddiv_rn(__dmul_rn(4.0 * kBuildPi, sin(__ddiv_rn(atan(__ddiv_rn(r, dist)), 2.0))), lambda));
+    default:
+        return __dmul_rn(1e-10, __ddiv_rn(__dmul_rn(4.0 * kBuildPi, sin(__ddiv_rn(atan(__ddiv_rn(r, dist)), 2.0))), lambda));
+    }
+}
+
 // Overlap of pixel [f_lo, f_hi] (bin units) with bin b, over the pixel's width ("proportional to the
 // area of the pixel segment that falls into that bin"; PAPER.md:122 outermost bins first, the rest evenly).
 // Plain fp64 operations, each rounded once (no FMA contraction).

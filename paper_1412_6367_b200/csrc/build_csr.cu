@@ -9,23 +9,6 @@
 
 namespace {
 
-constexpr double kPi = 3.14159265358979323846;
-
-// B1 (map): radial coordinate of a radius r in the requested unit, fp64, every operation
-// rounded once.
-__device__ __forceinline__ double unit_of_r(double r, double dist, double lambda, int unit)
-{
-    switch (unit) {
-    case AI_R_MM: return __dmul_rn(1e3, r);
-    case AI_TTH_RAD: return atan(__ddiv_rn(r, dist));
-    case AI_TTH_DEG: return __ddiv_rn(__dmul_rn(atan(__ddiv_rn(r, dist)), 180.0), kPi);
-    case AI_Q_NM:
-        return __dmul_rn(1e-9, __ddiv_rn(__dmul_rn(4.0 * kPi, sin(__ddiv_rn(atan(__ddiv_rn(r, dist)), 2.0))), lambda));
-    default:
-        return __dmul_rn(1e-10, __ddiv_rn(__dmul_rn(4.0 * kPi, sin(__ddiv_rn(atan(__ddiv_rn(r, dist)), 2.0))), lambda));
-    }
-}
-
 // B1: bounds of every pixel's bounding box along the radial axis (PAPER.md:50 r = sqrt((x-xc)^2 + (y-yc)^2);
 // PAPER.md:120 "rectangular box circumscribing the actual pixel") + block partials of the automatic range (B2).
 __global__ void __launch_bounds__(256) bounds_kernel(ai_geometry g, int height, int width, int unit,

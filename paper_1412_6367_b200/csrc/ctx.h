@@ -121,6 +121,7 @@ struct ai_ctx {
     ai_layout layout = AI_LAYOUT_TILED;
     ai_accum accum = AI_ACC_F32_KAHAN;
     ai_norm norm = AI_NORM_PIXEL;
+    ai_split split = AI_SPLIT_BBOX;
     float *norm_scratch = nullptr;        // [2 * npt] throw-away outputs of the two passes of AI_NORM_SPLIT
     float empty_value = 0.0f;
     int device = 0;
@@ -224,7 +225,8 @@ struct PixelSpans {              // per-pixel result of the bounds pass, kept on
 };
 int ai_build_canonical(ai_ctx *ctx, PixelSpans *spans, cudaStream_t st);
 int ai_build_tiled(ai_ctx *ctx, const PixelSpans &spans, cudaStream_t st);
-int ai_build_2d(ai_ctx *ctx, cudaStream_t st);      // build_2d.cu: canonical CSR + tiled layout of the 2D matrix
+int ai_build_2d(ai_ctx *ctx, cudaStream_t st);
+int ai_build_full(ai_ctx *ctx, cudaStream_t st);    // build_2d.cu: full pixel splitting, 1D      // build_2d.cu: canonical CSR + tiled layout of the 2D matrix
 int ai_build_lut(ai_ctx *ctx, cudaStream_t st);
 void ai_free_spans(PixelSpans *s);
 int ai_build_spans(ai_ctx *ctx, PixelSpans *sp, int npt, cudaStream_t st);
