@@ -301,10 +301,11 @@ class Train:
         return done, first
 
     def measure(self, steps, trains, stage1_only=False):
-        """`trains` trains of exactly `steps` steps: (median ms, all ms, launches of the median-sized train)."""
-        res = [self.run(steps, stage1_only, count=True) for _ in range(trains)]
-        ms = sorted(r[0] for r in res)
-        return statistics.median(ms), [r[0] for r in res], res[0][1]
+        """`trains` trains of exactly `steps` steps: (median ms, all ms, kernel launches of one train).  The launches are
+        counted on one extra, untimed train (asking the library after every call costs the host a microsecond)."""
+        res = [self.run(steps, stage1_only)[0] for _ in range(trains)]
+        _, launches = self.run(steps, stage1_only, count=True)
+        return statistics.median(res), res, launches
 
 
 def back_to_back(torch, integ, frames_dev, corr, calls, warmup=20):

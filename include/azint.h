@@ -149,13 +149,18 @@ int ai_set_normalization(ai_ctx *ctx, ai_norm norm);
  *                              v = (I - dark) / (flat * solidangle * polarization); a pixel is invalid if masked or if
  *                              its denominator is 0 / non-finite or its numerator non-finite.
  * Enqueues on `cuda_stream`; does not synchronise.  Errors: AI_EINVAL, AI_ENOTBUILT, AI_ECUDA.
- * With the default layout a plain 32-bit frame is one kernel launch; correction arrays, a mask, 16-bit pixels or rows
- * off 16-byte boundaries add one streaming pre-pass.  These kernels are launched with programmatic stream
- * serialisation: their prologue (barriers, descriptors, the first matrix tiles -- data that only ai_build_csr writes)
- * may overlap the tail of whatever precedes them on the stream; the frame, the correction arrays and every buffer the
- * call writes are touched only after that predecessor has completed (griddepcontrol.wait), so ordinary stream
- * ordering is what the caller sees.  Between calls the context keeps a corrected copy of the frame, partial sums and
- * two counters: one context, one stream at a time. */
+ * With the default layout a plain 32-bit frame is two kernel launches (the streaming product and a small finish
+ * kernel); correction arrays, a mask, 16-bit pixels or rows off 16-byte boundaries add one streaming pre-pass.  The
+ * kernels are launched with programmatic stream serialisation so that consecutive calls overlap:
+ *   - everything a call WRITES (outputs, the context's scratch) is written in stream order, after all earlier work;
+ *   - what a call READS -- the frame and the correction arrays -- may be read as soon as the kernel enqueued right
+ *     before it on the stream has completed OR has executed griddepcontrol.launch_dependents
+ *     (cudaTriggerProgrammaticLaunchCompletion).  Memory copies, memsets and kernels that never trigger early -- every
+ *     ordinary kernel -- give plain stream ordering.  A producer kernel that does trigger early must be followed by
+ *     any ordinary stream operation before the call (or set AZINT_TUNE=nov:1, which makes every kernel wait).
+ * Between calls the context keeps corrected copies of the frame, partial sums and ticket counters: one context is used
+ * by one host thread and on one stream at a time (different contexts are independent), on the device it was built on
+ * (AI_EINVAL otherwise). */
 int ai_integrate1d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *dark, const float *flat,
                    const float *solidangle, const float *polarization, const uint8_t *mask, float *radial,
                    float *intensity, float *sum_signal, float *count, void *cuda_stream);

@@ -249,6 +249,11 @@ class Integrator:
             if hasattr(torch, name):
                 self._codes[getattr(torch, name)] = code
         self.device = torch.device(device)
+        self._dev_index = self.device.index if self.device.index is not None else torch.cuda.current_device()
+        # the raw cudaStream_t of torch's current stream on the device, without building a Stream object per call
+        raw = getattr(torch._C, "_cuda_getCurrentRawStream", None)
+        self._raw_stream = raw if raw is not None else (lambda i: torch.cuda.current_stream(i).cuda_stream)
+        self._out_seen, self._out_ptrs = None, None
         self.cfg = cfg
         self.npt = cfg.npt
         self.npt_azim = int(getattr(cfg, "npt_azim", 0) or 0)
@@ -288,22 +293,27 @@ class Integrator:
     def integrate1d(self, image, dark=None, flat=None, solidangle=None, polarization=None, mask=None, out=None,
                     radial=None):
         """Returns (intensity, sum_signal, count) device tensors; enqueues on the current stream.  Same marshalling as
-        ai_integrate1d above with the per-call lookups (library handle, dtype code table) hoisted: at ~18 us of GPU
-        time per 2048 x 2048 frame the host has to enqueue a call in well under that."""
-        intensity, sum_signal, count = out if out is not None else self.outputs()
+        ai_integrate1d above with the per-call lookups hoisted (library handle, dtype table, the raw handle of the
+        current stream, the addresses of an `out` tuple that is passed again): at ~13 us of GPU time per 2048 x 2048
+        frame the host has to enqueue a call in well under that."""
+        if out is None:
+            out = self.outputs()
+        if out is not self._out_seen:
+            self._out_ptrs = (out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr())
+            self._out_seen = out
         code = self._codes.get(image.dtype)
         if code is None:
             raise AzintError(AI_EINVAL, f"unsupported frame dtype {image.dtype}")
+        p = self._out_ptrs
         rc = self._integrate1d(self.ctx, image.data_ptr(), code,
                                None if dark is None else dark.data_ptr(), None if flat is None else flat.data_ptr(),
                                None if solidangle is None else solidangle.data_ptr(),
                                None if polarization is None else polarization.data_ptr(),
                                None if mask is None else mask.data_ptr(), None if radial is None else radial.data_ptr(),
-                               intensity.data_ptr(), sum_signal.data_ptr(), count.data_ptr(),
-                               self.torch.cuda.current_stream().cuda_stream)
+                               p[0], p[1], p[2], self._raw_stream(self._dev_index))
         if rc != AI_OK:
             _check(rc, self.ctx)
-        return intensity, sum_signal, count
+        return out
 
     def integrate2d(self, image, dark=None, flat=None, solidangle=None, polarization=None, mask=None, out=None,
                     radial=None, azimuthal=None):

@@ -338,8 +338,9 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 {
     const TiledLayout &tl = ctx->tl;
     const size_t need = (size_t)(tl.nslot > 0 ? tl.nslot : 1) * 16 * a.nframes;
-    // partial records of the two-launch paths (the single-frame kernel has its own): grown on demand, which
-    // synchronises the device -- ai_reserve_batch sizes it ahead of time
+    // partial records of the two-launch paths (the single-frame kernel has its own, sized at build time): grown on
+    // demand; cudaFree synchronises the device, so work in flight on the old buffer has finished.  A first call with
+    // the largest batch sizes it for good.
     auto ensure_partials = [&]() -> int {
         if (ctx->partials_bytes >= need) return AI_OK;
         if (ctx->partials) AI_CUDA(ctx, cudaFree(ctx->partials));
