@@ -144,6 +144,10 @@ static int setup_common(ai_ctx **out, const ai_geometry *g, int height, int widt
     ctx->no_prepass = e && e[0] == '1';
     e = getenv("AZINT_NO_STREAM");
     ctx->no_stream = e && e[0] == '1';
+    e = getenv("AZINT_NO_FL");
+    ctx->no_fl = e && e[0] == '1';
+    e = getenv("AZINT_FORCE_FL");
+    ctx->force_fl = e && e[0] == '1';
     if ((e = getenv("AZINT_TUNE")) != nullptr) {        // experiments only: "th:32,ms:6,is:8,bms:2,bis:8,fl:2"
         for (const char *q = e; q && *q;) {
             char key[8] = {0};
@@ -158,6 +162,10 @@ static int setup_common(ai_ctx **out, const ai_geometry *g, int height, int widt
                 else if (!strcmp(key, "ss")) ctx->tune.stream_stages = val;
                 else if (!strcmp(key, "nov")) ctx->tune.no_overlap = val;
                 else if (!strcmp(key, "bu")) ctx->tune.batch_units = val;
+                else if (!strcmp(key, "fls")) ctx->tune.fl_stages = val;
+                else if (!strcmp(key, "flc")) ctx->tune.fl_chunk = val;
+                else if (!strcmp(key, "flo")) ctx->tune.fl_owner = val;
+                else if (!strcmp(key, "flp")) ctx->tune.fl_prefetch = val;
             }
             q = strchr(q, ',');
             if (q) ++q;
@@ -465,6 +473,7 @@ void ai_destroy(ai_ctx *ctx)
     cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
     free(tl.h_first_desc);
     free(ctx->stream_first);
+    ai_free_fl(ctx->fl);
     cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->stream_partials); cudaFree(ctx->axes2d); cudaFree(ctx->corrected[0]); cudaFree(ctx->corrected[1]);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);

@@ -60,6 +60,10 @@ struct PipeTune {
     int stream_stages = 0;                     // cap on the (tile + blob) stages of the single-frame kernel, 0 = none
     int no_overlap = 0;                        // single-frame kernel: never stream ahead of the grid dependency
     int batch_units = 0;                       // batched kernel: 1 = (block, frame) units, 2 = (block, two frames), 0 = by layout
+    int fl_stages = 0;                         // frame-lane kernel: cap on the stages, 0 = none
+    int fl_prefetch = 0;                       // frame-lane kernel: tiles between the L2 prefetch and the loads, 0 = default
+    int fl_owner = 0;                          // frame-lane layout: 1 = bins dealt to the warps longest-first instead of round-robin
+    int fl_chunk = 0;                          // frame-lane layout: tiles per chunk, 0 = by the size of the first batch
 };
 inline PipePlan ai_pipe_plan(int max_blob_bytes, int tile_h, bool batch, const PipeTune &tune = PipeTune())
 {
@@ -109,6 +113,37 @@ struct TiledLayout {
     int nslot = 0;                 // number of partials per frame: one per run of the sliced layout
 };
 
+// ---- frame-lane layout (build_fl.cu, integrate_fl.cu): batches of plain 32-bit frames ----------
+// The batched kernel turns the problem by 90 degrees: a warp's 32 lanes are 32 PAIRS OF FRAMES, an entry (coefficient,
+// pixel) is warp-uniform and serves all 64 of them.  Tiles of kFlTileW x kFlTileH pixels of 64 frames are staged in
+// shared memory (the two frames of a lane interleaved pixel by pixel, lane l shifted by 2 l words: the 32 lanes of a
+// gather fall into 32 different bank pairs); tiles are taken in order of their lowest bin and cut into chunks whose
+// bins fit a window of kFlWindow shared-memory accumulators per frame, so that one partial per (chunk, bin, frame)
+// leaves the SM instead of one per (tile, bin, frame).
+constexpr int kFlTileW = 32, kFlTileH = 8;
+constexpr int kFlFrames = 64;       // frames per group = two per lane of a warp
+constexpr int kFlWindow = 128;      // bins a chunk may touch
+constexpr int kFlCons = 16;         // consumer warps; a bin of a chunk belongs to one of them
+constexpr int kFlChunkTilesMax = 64; // tiles per chunk at most (fewer where the window would overflow, or for small batches)
+struct FlLayout {
+    bool tried = false, ok = false;
+    int tiles_x = 0, tiles_y = 0;
+    int ntiles = 0;                 // tiles that hold entries
+    int nchunks = 0, nslot = 0;
+    int4 *tile_desc = nullptr;      // [ntiles] in chunk order: {blob offset / 16, blob bytes, tile row << 16 | column, pairs}
+    int4 *chunk_desc = nullptr;     // [nchunks] {first tile, tiles, first slot, lowest bin << 8 | bins in the window - 1}
+    uint8_t *chunk_owner = nullptr; // [nchunks][kFlWindow] consumer warp that owns bin (lowest bin of the chunk + k)
+    unsigned char *blob = nullptr;
+    int64_t blob_bytes = 0;
+    int max_blob_bytes = 0;
+    int *bin_slot_ptr = nullptr;    // [npt+1] H5: partial slots of bin b are bin_slots[bin_slot_ptr[b] .. bin_slot_ptr[b+1])
+    int *bin_slots = nullptr;       //         ascending chunk
+    double *bin_csum = nullptr;     // [npt] sum of the row's coefficients (count when every pixel is valid)
+    void *partials = nullptr;       // [nslot][frames rounded up to 64] float2 (sum, compensation), then, for float
+                                    // frames, [npt][frames rounded up] uint64: weight of the invalid pixels, 2^-40 units
+    size_t partials_bytes = 0;
+};
+
 struct ai_ctx {
     ai_geometry geo{};
     int height = 0, width = 0, npt = 0;   // npt = number of bins = rows of the matrix (2D: npt_azim * npt_rad)
@@ -153,6 +188,7 @@ struct ai_ctx {
     int32_t *lut_idx = nullptr;
 
     TiledLayout tl;
+    FlLayout fl;
 
     // per-call scratch
     void *partials = nullptr;       // tiled stage-1 output, bin-major
@@ -194,6 +230,8 @@ struct ai_ctx {
     bool no_schedule = false;       // AZINT_NO_SCHEDULE=1: skip the bank scheduling of the sliced layout (measurement)
     bool no_prepass = false;        // AZINT_NO_PREPASS=1: corrected single frames take the general kernel (testing)
     bool no_stream = false;         // AZINT_NO_STREAM=1: single frames take the general pipelined kernel too (testing)
+    bool force_fl = false;          // AZINT_FORCE_FL=1: every batch of plain 32-bit frames takes the frame-lane kernel (testing)
+    bool no_fl = false;             // AZINT_NO_FL=1: large batches stay on the slice-per-lane batched kernel (testing)
     bool profile = false, profile_valid = false;
     bool stage1_only = false;       // ai_profile_enable(ctx, 2): launch only the dominant kernel
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -247,6 +285,9 @@ int ai_launch_tiled_split(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_csr(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_lut(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_scatter(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
+int ai_build_fl(ai_ctx *ctx, int nframes, cudaStream_t st);                          // build_fl.cu: frame-lane layout from the canonical CSR
+void ai_free_fl(FlLayout &fl);
+int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);   // integrate_fl.cu
 int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, int mode, cudaStream_t st, float **out);   // integrate_prep.cu
 int ai_stream_full_grid(const ai_ctx *ctx);   // integrate_stream.cu: 1 if the single-frame kernel puts one block on every SM
 int ai_stream_stages(const ai_ctx *ctx);      // integrate_stream.cu: (tile + blob) stages of the single-frame kernel, 0 = n/a

@@ -1,0 +1,567 @@
+// Batches of plain 32-bit frames on the frame-lane layout (H6 of SURVEY.md section 8(a): "a batched multi-frame variant
+// that amortises the matrix read across frames"; PAPER.md:11 detectors streaming thousands of frames per second;
+// DESIGN.md section 5.4).
+//
+// fl_batch_kernel: lane = two frames.  A work item is (chunk of tiles, group of 64 frames); one persistent block per SM.
+//   - kFlLoad loader warps bring a tile (32 x 8 pixels) of the group's 64 frames in with 128-bit loads (the lines were
+//     pulled into L2 two tiles earlier by bulk prefetches), cast them (H1) and store the two frames of
+//     lane l interleaved pixel by pixel, lane l shifted by 2 l words (lane pitch = tile bytes + 8): the 32 lanes of a
+//     gather -- same pixel, 64 frames -- fall into 32 different bank pairs.  The tile's blob of the matrix arrives by one
+//     bulk copy.  One ring of (tile + blob) stages, one full / empty mbarrier pair per stage.
+//   - kFlCons consumer warps: every (tile, bin) segment belongs to the warp that owns the bin inside the chunk.  An
+//     entry pair {c0, c1, pixel 0, pixel 1} is one broadcast 128-bit shared load for the whole warp; each lane gathers
+//     its two frames' pixel with one 64-bit load and adds the two products with two Kahan recurrences
+//     carried in packed fp32x2 arithmetic (FFMA2 / FADD2, the coefficient a scalar operand).  The running (sum,
+//     compensation) of every (bin, frame) of the chunk lives in shared memory, touched by its owner warp only: fixed
+//     order of every sum, no atomics, bit-reproducible.
+//   - at the end of an item the owner warps write one (sum, compensation) pair per (chunk, bin, frame).
+// fl_finish_kernel (H5): adds a bin's partials over the chunks in fp64 and writes the three outputs.
+// Float frames: the loaders flag a tile that holds a non-finite pixel; its segments then take the variant that skips
+// such pixels and adds their weight -- in 2^-40 fixed point, so that the atomic sums do not depend on their order -- to
+// a (bin, frame) array which H5 subtracts from the row's coefficient sum.
+#include "common.cuh"
+#include "pipe_common.cuh"
+
+namespace {
+
+constexpr int kFlLoad = 8;                           // loader warps: warp w stages lanes 4w .. 4w+3 (frames 8w .. 8w+7 of the group)
+constexpr int kFlThreads = 32 * (kFlLoad + kFlCons);
+constexpr int kFlMaxStages = 4;
+constexpr int kFlBarBytes = 512;                     // full[8], empty[8], flags[kFlMaxStages][kFlLoad]
+constexpr int kFlFlagOffset = 128;
+constexpr int kFlHdrBytes = 48;                      // as build_fl.cu
+constexpr int kFlTilePix = kFlTileW * kFlTileH;
+constexpr int kFlLaneBytes = kFlTilePix * 8 + 8;     // a lane's two frames of the tile, and the shift
+constexpr int kFlImgBytes = 32 * kFlLaneBytes;
+constexpr int kFlPassRows = 4;                       // rows of the tile a loader holds in registers at a time
+constexpr int kFlPrefetchAhead = 3;                  // tiles between the L2 prefetch and the loads
+constexpr int kFlMinFrames = 96;
+constexpr float kFlFix = 1099511627776.0f;           // 2^40: weights of invalid pixels as integers
+
+struct FlParams {
+    const int4 *tile_desc, *chunk_desc;
+    const uint8_t *chunk_owner;
+    const unsigned char *blob;
+    const unsigned char *frames;
+    int64_t frame_stride_bytes;
+    int height, width;
+    int nframes, ngroups, nitems;
+    int stages, stage_bytes, prefetch_ahead;
+    float2 *part_s;
+    unsigned long long *part_d;                      // float frames only
+    int64_t nfp;                                     // frames rounded up to a multiple of kFlFrames
+};
+
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
+{
+    return (unsigned long long)__float_as_uint(lo) | ((unsigned long long)__float_as_uint(hi) << 32);
+}
+__device__ __forceinline__ float lo_of(unsigned long long v) { return __uint_as_float((unsigned)v); }
+__device__ __forceinline__ float hi_of(unsigned long long v) { return __uint_as_float((unsigned)(v >> 32)); }
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ unsigned long long add2(unsigned long long a, unsigned long long b)
+{
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ unsigned long long sub2(unsigned long long a, unsigned long long b)
+{
+    unsigned long long d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ unsigned long long lds_u64(unsigned addr)
+{
+    unsigned long long v;
+    asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint4 lds_v4(unsigned addr)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts_v4(unsigned addr, const uint4 &v)
+{
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void sts_f2(unsigned addr, float a, float b)
+{
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
+}
+__device__ __forceinline__ void prefetch_l2(const void *p, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+// Waits of the frame-lane kernel: try_wait with a long suspend-time hint -- the warp sleeps in the barrier unit until
+// the phase completes instead of polling, so waiting warps leave the issue slots to the warps that work.  Bounded
+// (20 s of wall time) like mbar_wait.
+__device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity)
+{
+    unsigned long long t0 = 0;
+    for (uint32_t spin = 1;; ++spin) {
+        uint32_t ok;
+        asm volatile("{\n\t.reg .pred p;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity), "r"(100000u) : "memory");
+        if (ok) return;
+        if ((spin & 0xffu) == 0) {
+            const unsigned long long now = globaltimer_ns();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 20000000000ULL) __trap();
+        }
+    }
+}
+
+// One Kahan step for the two frames of a lane, the compensation carried as e = -(running error):
+// the carried value is s + e.  c2 = the coefficient in both halves.
+__device__ __forceinline__ void kahan2(unsigned long long &s, unsigned long long &e, unsigned long long c2,
+                                       unsigned long long v)
+{
+    const unsigned long long y = fma2(c2, v, e);
+#ifndef AI_FL_MIXED_KAHAN
+    const unsigned long long t = add2(s, y);
+    e = add2(sub2(s, t), y);
+    s = t;
+#else
+    // FFMA2 / FADD2 run on one of the SM's two fp32 pipes only (measured: ~4 cycles per warp instruction): the two middle
+    // steps go as scalar adds so that the other pipe takes its share
+    const float tx = __fadd_rn(lo_of(s), lo_of(y)), ty = __fadd_rn(hi_of(s), hi_of(y));
+    const float ux = __fsub_rn(lo_of(s), tx), uy = __fsub_rn(hi_of(s), ty);
+    e = add2(pack2(ux, uy), y);
+    s = pack2(tx, ty);
+#endif
+}
+
+// position in the sequence of (item, tile) this block walks: items blockIdx.x, + gridDim.x, ...; an item is a chunk of
+// tiles for one group of frames, chunk-major so that neighbouring blocks share the chunk's blobs in L2
+struct FlWalk {
+    int item, r, r_end, group, chunk;
+    bool done;
+};
+__device__ __forceinline__ void fl_enter(FlWalk &w, const FlParams &p)
+{
+    w.done = w.item >= p.nitems;
+    if (w.done) return;
+    w.chunk = w.item / p.ngroups;
+    w.group = w.item - w.chunk * p.ngroups;
+    const int4 cd = __ldg(p.chunk_desc + w.chunk);
+    w.r = cd.x;
+    w.r_end = cd.x + cd.y;
+}
+__device__ __forceinline__ void fl_next(FlWalk &w, const FlParams &p)
+{
+    if (++w.r < w.r_end) return;
+    w.item += gridDim.x;
+    fl_enter(w, p);
+}
+
+template <int DT>
+__device__ __forceinline__ float fl_cast(unsigned v)
+{
+    if constexpr (DT == AI_F32) return __uint_as_float(v);
+    else if constexpr (DT == AI_I32) return (float)(int)v;
+    else return (float)v;
+}
+
+template <int DT>
+__global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_constant__ CUtensorMap tmap, const FlParams p)
+{
+    constexpr bool TRACK = DT == AI_F32;
+    // [accumulators][barriers, flags][stages: tile of 64 frames, blob]
+    extern __shared__ __align__(1024) unsigned char smem[];
+    unsigned char *bar = smem + kFlWindow * 32 * 16;
+    uint64_t *full = reinterpret_cast<uint64_t *>(bar);
+    uint64_t *empty = full + 8;
+    int *flags = reinterpret_cast<int *>(bar + kFlFlagOffset);
+    unsigned char *stage0 = bar + kFlBarBytes;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < 8; ++s) {
+            mbar_init(full + s, kFlLoad + 1);
+            mbar_init(empty + s, kFlCons);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    Ring ring;
+    FlWalk cur;
+    cur.item = blockIdx.x;
+    fl_enter(cur, p);
+    if (warp < kFlLoad) {
+        // ===== loaders =================================================================================================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");          // two passes of 128-bit loads in registers
+        // lane = (lane of the consumers, 16-byte piece of a tile row): lanes 4 lw .. 4 lw + 3 x pieces 0..7, so that the
+        // 8 lanes of a 128-bit load phase read one 128-byte line.  Stores are 64-bit (one pixel of the lane's two
+        // frames); pieces 4..7 store their pixels in the order 2, 3, 0, 1, which puts the 16 lanes of a store phase into
+        // 16 different bank pairs.
+        const int lw = warp, piece = lane & 7, cl = lw * 4 + (lane >> 3);
+        const bool swap = piece >= 4;
+        const int d2 = swap ? -16 : 16;
+        const unsigned dst_lane = (unsigned)cl * kFlLaneBytes + (unsigned)piece * 32 + (swap ? 16u : 0u);
+        const int64_t row_bytes = (int64_t)p.width * 4;
+        const int tid = threadIdx.x;                                   // 0 .. 255 among the loaders
+        if (tid == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
+        // L2 prefetch of a tile: ONE instruction (a tensor-map box of 32 pixels x 8 rows x 64 frames) by one thread
+        auto prefetch_tile = [&](const FlWalk &w) {
+            if (tid != 0) return;
+            const int4 d = __ldg(p.tile_desc + w.r);
+            asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
+                         ::"l"(&tmap), "r"((d.z & 0xffff) * kFlTileW), "r"((d.z >> 16) * kFlTileH), "r"(w.group * kFlFrames) : "memory");
+        };
+        FlWalk ahead = cur;
+        for (int k = 0; k < p.prefetch_ahead && !ahead.done; ++k) {
+            prefetch_tile(ahead);
+            fl_next(ahead, p);
+        }
+        // 128-bit loads of rows 4 h .. 4 h + 3 of the tile for the lane's two frames
+        auto issue = [&](const FlWalk &w, int h, uint4 (&a)[kFlPassRows], uint4 (&b)[kFlPassRows], int4 &d) {
+            d = __ldg(p.tile_desc + w.r);
+            const int x = (d.z & 0xffff) * kFlTileW + piece * 4, y0 = (d.z >> 16) * kFlTileH + h * kFlPassRows;
+            const int fa = w.group * kFlFrames + 2 * cl;
+            const unsigned char *src = p.frames + (int64_t)fa * p.frame_stride_bytes + ((int64_t)y0 * p.width + x) * 4;
+            const bool in_a = fa < p.nframes && x < p.width, in_b = fa + 1 < p.nframes && x < p.width;
+#pragma unroll
+            for (int u = 0; u < kFlPassRows; ++u) {
+                const unsigned char *q = src + u * row_bytes;
+                a[u] = b[u] = make_uint4(0, 0, 0, 0);
+                if (in_a && y0 + u < p.height) a[u] = __ldcs(reinterpret_cast<const uint4 *>(q));
+                if (in_b && y0 + u < p.height) b[u] = __ldcs(reinterpret_cast<const uint4 *>(q + p.frame_stride_bytes));
+            }
+        };
+        int issued = 0;
+        bool bad = false;
+        auto store = [&](int h, const uint4 (&a)[kFlPassRows], const uint4 (&b)[kFlPassRows], const int4 &d) {
+            unsigned char *stage = stage0 + (size_t)ring.stage * p.stage_bytes;
+            if (h == 0) {
+                if (issued >= p.stages) mbar_wait_relaxed(empty + ring.stage, ring.parity ^ 1u);
+                if (lw == 0 && lane == 0) {
+                    mbar_arrive_expect_tx(full + ring.stage, (uint32_t)d.y);
+                    bulk_g2s(stage + kFlImgBytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y, full + ring.stage);
+                }
+                bad = false;
+            }
+            const unsigned dst = smem_u32(stage) + dst_lane + (unsigned)(h * kFlPassRows * kFlTileW * 8);
+#pragma unroll
+            for (int u = 0; u < kFlPassRows; ++u) {
+                const unsigned o = dst + (unsigned)(u * kFlTileW * 8);
+                const float a0 = fl_cast<DT>(a[u].x), a1 = fl_cast<DT>(a[u].y), a2 = fl_cast<DT>(a[u].z), a3 = fl_cast<DT>(a[u].w);
+                const float b0 = fl_cast<DT>(b[u].x), b1 = fl_cast<DT>(b[u].y), b2 = fl_cast<DT>(b[u].z), b3 = fl_cast<DT>(b[u].w);
+                if constexpr (TRACK)
+                    bad = bad || !finite_f(a0) || !finite_f(a1) || !finite_f(a2) || !finite_f(a3) || !finite_f(b0) ||
+                          !finite_f(b1) || !finite_f(b2) || !finite_f(b3);
+                sts_f2(o, swap ? a2 : a0, swap ? b2 : b0);
+                sts_f2(o + 8, swap ? a3 : a1, swap ? b3 : b1);
+                sts_f2(o + d2, swap ? a0 : a2, swap ? b0 : b2);
+                sts_f2(o + d2 + 8, swap ? a1 : a3, swap ? b1 : b3);
+            }
+            if (h == kFlTileH / kFlPassRows - 1) {
+                if constexpr (TRACK) {
+                    const bool any = __any_sync(AI_FULL_MASK, bad);
+                    if (lane == 0) flags[ring.stage * kFlLoad + lw] = any ? 1 : 0;
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(full + ring.stage);
+                ++issued;
+                ring.next(p.stages);
+            }
+        };
+        // the loads of the next pass are in flight while the current one is cast and stored
+        uint4 a0[kFlPassRows], b0[kFlPassRows], a1[kFlPassRows], b1[kFlPassRows];
+        int4 d0 = make_int4(0, 0, 0, 0), d1 = d0;
+        int h = 0;
+        if (!cur.done) issue(cur, 0, a0, b0, d0);
+        while (!cur.done) {
+            FlWalk nxt = cur;
+            int hn = h + 1;
+            if (hn == kFlTileH / kFlPassRows) {
+                hn = 0;
+                fl_next(nxt, p);
+                if (!ahead.done) {
+                    prefetch_tile(ahead);
+                    fl_next(ahead, p);
+                }
+            }
+            if (!nxt.done) issue(nxt, hn, a1, b1, d1);
+            store(h, a0, b0, d0);
+#pragma unroll
+            for (int u = 0; u < kFlPassRows; ++u) { a0[u] = a1[u]; b0[u] = b1[u]; }
+            d0 = d1;
+            cur = nxt;
+            h = hn;
+        }
+    } else {
+        // ===== consumers ===============================================================================================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
+        const int cw = warp - kFlLoad;
+        const unsigned acc = smem_u32(smem) + (unsigned)lane * 16;     // + bin * 512: {s of the two frames, e of the two}
+        while (!cur.done) {
+            // bins of this chunk's window that this warp owns
+            const int4 cd = __ldg(p.chunk_desc + cur.chunk);
+            const int nb = (cd.w & 0xff) + 1, bin_lo = cd.w >> 8;
+            unsigned own[kFlWindow / 32];
+#pragma unroll
+            for (int k = 0; k < kFlWindow / 32; ++k) {
+                const int bl = 32 * k + lane;
+                own[k] = __ballot_sync(AI_FULL_MASK, bl < nb && __ldg(p.chunk_owner + (size_t)cur.chunk * kFlWindow + bl) == cw);
+            }
+#pragma unroll
+            for (int k = 0; k < kFlWindow / 32; ++k)
+                for (unsigned m = own[k]; m; m &= m - 1) sts_v4(acc + (unsigned)(32 * k + __ffs(m) - 1) * 512, make_uint4(0, 0, 0, 0));
+            const int item = cur.item, group = cur.group;
+            const int fa = group * kFlFrames + 2 * lane;
+            while (!cur.done && cur.item == item) {
+                mbar_wait_relaxed(full + ring.stage, ring.parity);
+                const unsigned char *stage = stage0 + (size_t)ring.stage * p.stage_bytes;
+                const unsigned char *blob = stage + kFlImgBytes;
+                const unsigned short *wptr = reinterpret_cast<const unsigned short *>(blob);
+                const int s0 = wptr[cw], s1 = wptr[cw + 1], nrec = wptr[kFlCons];
+                const unsigned recs = smem_u32(blob) + kFlHdrBytes;
+                const unsigned pairs = smem_u32(blob) + (unsigned)((kFlHdrBytes + 4 * nrec + 15) & ~15);
+                const unsigned img = smem_u32(stage) + (unsigned)lane * kFlLaneBytes;
+                bool tracked = false;
+                if constexpr (TRACK) {
+                    const int4 *fp = reinterpret_cast<const int4 *>(flags + ring.stage * kFlLoad);
+                    const int4 f0 = fp[0], f1 = fp[1];
+                    tracked = (f0.x | f0.y | f0.z | f0.w | f1.x | f1.y | f1.z | f1.w) != 0;
+                }
+                if (s0 < s1 && !tracked) {
+                    // the warp's segments are contiguous in the blob: the look-ahead (entry pair two ahead, pixels one
+                    // ahead) runs on across segment boundaries; two zero pairs stand behind the last one
+                    unsigned rec = 0;
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(rec) : "r"(recs + 4 * s0));
+                    unsigned q = pairs + (rec & 16383u) * 16;
+                    uint4 w0 = lds_v4(q), w1 = lds_v4(q + 16);
+                    unsigned long long v0 = lds_u64(img + w0.z), v1 = lds_u64(img + w0.w);
+                    for (int s = s0; s < s1; ++s) {
+                        const int np = (rec >> 14) & 1023;
+                        const unsigned a_addr = acc + (rec >> 24) * 512;
+                        unsigned rec_n = 0;
+                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(rec_n) : "r"(recs + 4 * s + 4));   // (one past the end: an entry pair)
+                        const uint4 a = lds_v4(a_addr);
+                        unsigned long long s2 = (unsigned long long)a.x | ((unsigned long long)a.y << 32);
+                        unsigned long long e2 = (unsigned long long)a.z | ((unsigned long long)a.w << 32);
+#pragma unroll 2
+                        for (int k = 0; k < np; ++k) {
+                            const uint4 w2 = lds_v4(q + 32);
+                            const unsigned long long n0 = lds_u64(img + w1.z), n1 = lds_u64(img + w1.w);
+                            kahan2(s2, e2, pack2(__uint_as_float(w0.x), __uint_as_float(w0.x)), v0);
+                            kahan2(s2, e2, pack2(__uint_as_float(w0.y), __uint_as_float(w0.y)), v1);
+                            w0 = w1; w1 = w2; v0 = n0; v1 = n1;
+                            q += 16;
+                        }
+                        sts_v4(a_addr, make_uint4((unsigned)s2, (unsigned)(s2 >> 32), (unsigned)e2, (unsigned)(e2 >> 32)));
+                        rec = rec_n;
+                    }
+                } else if (s0 < s1) {
+                    if constexpr (TRACK) {
+                        for (int s = s0; s < s1; ++s) {
+                            unsigned rec;
+                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(rec) : "r"(recs + 4 * s));
+                            const int np = (rec >> 14) & 1023, bl = rec >> 24;
+                            const unsigned q = pairs + (rec & 16383u) * 16, a_addr = acc + bl * 512;
+                            const uint4 a = lds_v4(a_addr);
+                            unsigned long long s2 = (unsigned long long)a.x | ((unsigned long long)a.y << 32);
+                            unsigned long long e2 = (unsigned long long)a.z | ((unsigned long long)a.w << 32);
+                            unsigned long long *dd = p.part_d + (int64_t)(bin_lo + bl) * p.nfp + fa;
+                            for (int k = 0; k < 2 * np; ++k) {
+                                const uint4 w = lds_v4(q + 16 * (k >> 1));
+                                const float c = __uint_as_float((k & 1) ? w.y : w.x);
+                                const unsigned long long v = lds_u64(img + ((k & 1) ? w.w : w.z));
+                                const bool oka = finite_f(lo_of(v)), okb = finite_f(hi_of(v));
+                                kahan2(s2, e2, pack2(c, c), pack2(oka ? lo_of(v) : 0.f, okb ? hi_of(v) : 0.f));
+                                if (c != 0.f) {
+                                    const unsigned long long fix = __float2ull_rn(c * kFlFix);
+                                    if (!oka && fa < p.nframes) atomicAdd(dd, fix);
+                                    if (!okb && fa + 1 < p.nframes) atomicAdd(dd + 1, fix);
+                                }
+                            }
+                            sts_v4(a_addr, make_uint4((unsigned)s2, (unsigned)(s2 >> 32), (unsigned)e2, (unsigned)(e2 >> 32)));
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + ring.stage);
+                ring.next(p.stages);
+                fl_next(cur, p);
+            }
+            // one partial per (chunk, bin, frame), written by the bin's owner: {s, e} of frame 2 lane, {s, e} of the next
+#pragma unroll
+            for (int k = 0; k < kFlWindow / 32; ++k)
+                for (unsigned m = own[k]; m; m &= m - 1) {
+                    const int bl = 32 * k + __ffs(m) - 1;
+                    const uint4 a = lds_v4(acc + (unsigned)bl * 512);
+                    if (fa < p.nframes)
+                        *reinterpret_cast<uint4 *>(p.part_s + (int64_t)(cd.z + bl) * p.nfp + fa) = make_uint4(a.x, a.z, a.y, a.w);
+                }
+            // the next item deals the window's accumulators to the warps afresh: every warp must be done with this one
+            asm volatile("bar.sync 1, %0;" ::"n"(32 * kFlCons) : "memory");
+        }
+    }
+}
+
+// H5: block = 32 bins x 32 frames; lane = frame while the partials are added (coalesced over frames), lane = bin when
+// the outputs are written ([frame][bin] rows)
+template <bool TRACK>
+__global__ void __launch_bounds__(256) fl_finish_kernel(const int *__restrict__ bin_slot_ptr,
+                                                        const int *__restrict__ bin_slots,
+                                                        const double *__restrict__ bin_csum, int npt, int nframes,
+                                                        int64_t nfp, const float2 *__restrict__ part_s,
+                                                        const unsigned long long *__restrict__ part_d, float empty,
+                                                        float *__restrict__ intensity, float *__restrict__ sum_signal,
+                                                        float *__restrict__ count)
+{
+    __shared__ float t_i[32][33], t_s[32][33], t_c[32][33];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int b0 = blockIdx.x * 32, f0 = blockIdx.y * 32;
+    for (int i = w; i < 32; i += 8) {
+        const int b = b0 + i, f = f0 + lane;
+        double S = 0.0, C = 0.0;
+        if (b < npt && f < nframes) {
+            const int beg = __ldg(bin_slot_ptr + b), end = __ldg(bin_slot_ptr + b + 1);
+            for (int k = beg; k < end; ++k) {
+                const float2 v = __ldcg(part_s + (int64_t)__ldg(bin_slots + k) * nfp + f);
+                S += (double)v.x + (double)v.y;
+            }
+            const double csum = __ldg(bin_csum + b);
+            C = csum;
+            if constexpr (TRACK) {
+                C = csum - (double)__ldcg(part_d + (int64_t)b * nfp + f) * (1.0 / (double)kFlFix);
+                // all of a bin's pixels invalid: the two sums of the same coefficients differ by rounding only
+                if (fabs(C) <= 1e-10 * csum) C = 0.0;
+            }
+        }
+        t_s[i][lane] = (float)S;
+        t_c[i][lane] = (float)C;
+        t_i[i][lane] = C > 0.0 ? (float)(S / C) : empty;
+    }
+    __syncthreads();
+    for (int j = w; j < 32; j += 8) {
+        const int f = f0 + j, b = b0 + lane;
+        if (f < nframes && b < npt) {
+            const int64_t o = (int64_t)f * npt + b;
+            intensity[o] = t_i[lane][j];
+            sum_signal[o] = t_s[lane][j];
+            count[o] = t_c[lane][j];
+        }
+    }
+}
+
+template <int DT>
+int launch_fl(ai_ctx *ctx, const CUtensorMap &map, const FlParams &p, size_t smem, int grid, cudaStream_t st)
+{
+    const uint64_t bit = 1ULL << (40 + DT);
+    if (!(ctx->smem_opt_in & bit)) {
+        AI_CUDA(ctx, cudaFuncSetAttribute(fl_batch_kernel<DT>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPipeSmemBudget));
+        ctx->smem_opt_in |= bit;
+    }
+    ai_prof_begin(ctx, st);
+    fl_batch_kernel<DT><<<grid, kFlThreads, smem, st>>>(map, p);
+    ai_prof_end(ctx, st);
+    AI_CUDA(ctx, cudaGetLastError());
+    return AI_OK;
+}
+
+}  // namespace
+
+// Batches of at least kFlMinFrames plain 32-bit frames, Kahan accumulation, 1D: *handled = true when the frame-lane
+// kernel took the call (both launches).  The first such call of a context builds the layout (one-time; synchronises
+// `st`).
+int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled)
+{
+    *handled = false;
+    if (a.nframes < 2 || ctx->no_fl || ctx->no_tma || ctx->no_stream || ctx->npt_azim > 0 ||
+        ctx->accum != AI_ACC_F32_KAHAN || ctx->layout != AI_LAYOUT_TILED)
+        return AI_OK;
+    // Where it pays (measured): batches of two groups of frames or more on matrices with more than
+    // ~2.2 entries per pixel -- below that the per-pixel cost of staging the frames outweighs the cheaper entries and
+    // the slice-per-lane kernel is as fast.  AZINT_FORCE_FL=1 takes every batch (testing).
+    if (!ctx->force_fl && (a.nframes < kFlMinFrames || (double)ctx->nnz < 2.2 * (double)ctx->height * ctx->width)) return AI_OK;
+    const bool plain = !a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask;
+    const bool is32 = a.dtype == AI_F32 || a.dtype == AI_I32 || a.dtype == AI_U32;
+    if (!plain || !is32 || !vec_ok || (reinterpret_cast<uintptr_t>(a.image) % 16) != 0) return AI_OK;
+    if (a.row_pitch != 0 && a.row_pitch != ctx->width) return AI_OK;
+    FlLayout &fl = ctx->fl;
+    if (!fl.tried) {
+        int rc = ai_build_fl(ctx, a.nframes, st);
+        if (rc != AI_OK) return rc;
+    }
+    if (!fl.ok) return AI_OK;
+    const bool track = a.dtype == AI_F32;
+    const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
+
+    FlParams p{};
+    p.stage_bytes = kFlImgBytes + ai_align_up(fl.max_blob_bytes, 16);
+    const int acc_bytes = kFlWindow * 32 * 16;
+    int stages = (kPipeSmemBudget - acc_bytes - kFlBarBytes) / p.stage_bytes;
+    if (stages > kFlMaxStages) stages = kFlMaxStages;
+    if (ctx->tune.fl_stages > 0 && stages > ctx->tune.fl_stages) stages = ctx->tune.fl_stages;
+    if (stages < 2) return AI_OK;
+    p.stages = stages;
+    p.prefetch_ahead = ctx->tune.fl_prefetch > 0 ? ctx->tune.fl_prefetch : kFlPrefetchAhead;
+    p.ngroups = (a.nframes + kFlFrames - 1) / kFlFrames;
+    const int64_t nitems = (int64_t)fl.nchunks * p.ngroups;
+    if (nitems > 0x3fffffffLL) return AI_OK;
+    p.nitems = (int)nitems;
+    p.nfp = (int64_t)p.ngroups * kFlFrames;
+    const size_t part_bytes = (size_t)fl.nslot * (size_t)p.nfp * sizeof(float2);
+    const size_t d_bytes = track ? (size_t)ctx->npt * (size_t)p.nfp * sizeof(unsigned long long) : 0;
+    const size_t need = part_bytes + d_bytes;
+    if (fl.partials_bytes < need) {
+        // grown on demand; cudaFree synchronises the device, so work in flight on the old buffer has finished
+        if (fl.partials) AI_CUDA(ctx, cudaFree(fl.partials));
+        fl.partials = nullptr;
+        fl.partials_bytes = 0;
+        AI_CUDA(ctx, cudaMalloc(&fl.partials, need));
+        fl.partials_bytes = need;
+    }
+    p.part_s = static_cast<float2 *>(fl.partials);
+    p.part_d = track ? reinterpret_cast<unsigned long long *>(static_cast<char *>(fl.partials) + part_bytes) : nullptr;
+    if (track) AI_CUDA(ctx, cudaMemsetAsync(p.part_d, 0, d_bytes, st));
+    p.tile_desc = fl.tile_desc;
+    p.chunk_desc = fl.chunk_desc;
+    p.chunk_owner = fl.chunk_owner;
+    p.blob = fl.blob;
+    p.frames = static_cast<const unsigned char *>(a.image);
+    p.frame_stride_bytes = a.frame_stride * 4;
+    p.height = ctx->height;
+    p.width = ctx->width;
+    p.nframes = a.nframes;
+    const int grid = p.nitems < sms ? p.nitems : sms;
+    const size_t smem = (size_t)acc_bytes + kFlBarBytes + (size_t)stages * p.stage_bytes;
+    CUtensorMap map{};
+    int rc = ai_make_frame_map(ctx, a, kFlTileH, &map, kFlFrames);      // boxes of 64 frames: the L2 prefetch of a tile
+    if (rc != AI_OK) return rc;
+    rc = AI_EINVAL;
+    switch (a.dtype) {
+    case AI_F32: rc = launch_fl<AI_F32>(ctx, map, p, smem, grid, st); break;
+    case AI_I32: rc = launch_fl<AI_I32>(ctx, map, p, smem, grid, st); break;
+    case AI_U32: rc = launch_fl<AI_U32>(ctx, map, p, smem, grid, st); break;
+    default: break;
+    }
+    if (rc != AI_OK) return rc;
+    *handled = true;
+    ctx->last_launches = 1;
+    if (ctx->stage1_only) return AI_OK;
+    const dim3 g2((ctx->npt + 31) / 32, (a.nframes + 31) / 32);
+    if (track)
+        fl_finish_kernel<true><<<g2, 256, 0, st>>>(fl.bin_slot_ptr, fl.bin_slots, fl.bin_csum, ctx->npt, a.nframes, p.nfp,
+                                                   p.part_s, p.part_d, ctx->empty_value, a.intensity, a.sum_signal, a.count);
+    else
+        fl_finish_kernel<false><<<g2, 256, 0, st>>>(fl.bin_slot_ptr, fl.bin_slots, fl.bin_csum, ctx->npt, a.nframes, p.nfp,
+                                                    p.part_s, p.part_d, ctx->empty_value, a.intensity, a.sum_signal, a.count);
+    AI_CUDA(ctx, cudaGetLastError());
+    ctx->last_launches = 2;
+    return AI_OK;
+}

@@ -427,12 +427,12 @@ EncodeTiledFn encode_tiled_fn()
 // (x, y, frame) view of the frames, boxes of 32 pixels x tile_h rows x 1 frame, 128-byte swizzle, zeros outside.
 // The maps of the last eight buffers are kept in the context: a stream of calls on a ring of buffers pays for
 // cuTensorMapEncodeTiled once per buffer, not per call.
-int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *map)
+int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *map, int box_frames)
 {
     static_assert(sizeof(CUtensorMap) <= sizeof(ctx->map_cache[0].map), "tensor map cache too small");
     const int64_t pitch_el = a.row_pitch ? a.row_pitch : (int64_t)ctx->width;
     for (auto &e : ctx->map_cache)
-        if (e.image == a.image && e.dtype == (int)a.dtype && e.tile_h == tile_h && e.nframes == a.nframes &&
+        if (e.image == a.image && e.dtype == (int)a.dtype && e.tile_h == tile_h + 1024 * box_frames && e.nframes == a.nframes &&
             e.pitch == pitch_el && e.stride == a.frame_stride) {
             memcpy(map, e.map, sizeof(CUtensorMap));
             return AI_OK;
@@ -443,7 +443,7 @@ int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *
                                  : a.dtype == AI_I32 ? CU_TENSOR_MAP_DATA_TYPE_INT32 : CU_TENSOR_MAP_DATA_TYPE_UINT32;
     const cuuint64_t dims[3] = {(cuuint64_t)ctx->width, (cuuint64_t)ctx->height, (cuuint64_t)a.nframes};
     const cuuint64_t strides[2] = {(cuuint64_t)pitch_el * 4, (cuuint64_t)a.frame_stride * 4};
-    const cuuint32_t box[3] = {32, (cuuint32_t)tile_h, 1};
+    const cuuint32_t box[3] = {32, (cuuint32_t)tile_h, (cuuint32_t)box_frames};
     const cuuint32_t estr[3] = {1, 1, 1};
     const CUresult r = enc(map, dt, 3, const_cast<void *>(a.image), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -453,7 +453,7 @@ int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *
     memcpy(e.map, map, sizeof(CUtensorMap));
     e.image = a.image;
     e.dtype = (int)a.dtype;
-    e.tile_h = tile_h;
+    e.tile_h = tile_h + 1024 * box_frames;
     e.nframes = a.nframes;
     e.pitch = pitch_el;
     e.stride = a.frame_stride;

@@ -374,6 +374,9 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
             rc = launch_prepass_stream(ctx, a, vec_ok, 0, st, &handled);
             if (rc != AI_OK || handled) return rc;
         }
+        // 32 or more plain 32-bit frames: the frame-lane kernel (integrate_fl.cu), both launches
+        rc = ai_launch_fl(ctx, a, vec_ok, st, &handled);
+        if (rc != AI_OK || handled) return rc;
         rc = ensure_partials();
         if (rc != AI_OK) return rc;
         rc = ai_launch_bstream_stage1(ctx, a, vec_ok, st, &handled);          // batch of plain 32-bit frames

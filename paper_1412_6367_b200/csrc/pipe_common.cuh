@@ -7,7 +7,7 @@
 #include "ctx.h"
 
 // host: tensor map of the frames for the TMA image path (integrate_pipe.cu)
-int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *map);
+int ai_make_frame_map(ai_ctx *ctx, const FrameArgs &a, int tile_h, CUtensorMap *map, int box_frames = 1);
 
 // ---- mbarrier / bulk-copy primitives (PTX, sm_90+) ---------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }

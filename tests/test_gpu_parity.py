@@ -456,13 +456,16 @@ def test_batch_matches_oracle_small(torch, B, oracle, workloads):
     integ.close()
 
 
-@pytest.mark.parametrize("path", ["bstream", "pipe"])
+@pytest.mark.parametrize("path", ["bstream", "pipe", "fl"])
 @pytest.mark.parametrize("dtype,nframes", [("int32", 7), ("float32", 6), ("uint32", 2), ("float32", 33)])
 def test_batch_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, nframes):
     """Batches of plain 32-bit frames take the two-frames-at-a-time stream kernel; AZINT_NO_STREAM=1 sends them
-    through the general pipelined kernel.  Odd counts leave a single last frame; float frames carry NaN / Inf."""
+    through the general pipelined kernel, AZINT_FORCE_FL=1 through the frame-lane kernel (tests/test_gpu_parity_fl.py has
+    more of those).  Odd counts leave a single last frame; float frames carry NaN / Inf."""
     if path == "pipe":
         monkeypatch.setenv("AZINT_NO_STREAM", "1")
+    if path == "fl":
+        monkeypatch.setenv("AZINT_FORCE_FL", "1")
     cfg = workloads.tiny_config(200, 264, center_x=100.3, center_y=90.1, unit=workloads.Q_NM, npt=257,
                                 distance_m=0.02, name="batch_small")
     rng = np.random.default_rng(nframes)

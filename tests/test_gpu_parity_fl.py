@@ -1,0 +1,171 @@
+"""Parity of the frame-lane batched kernel (integrate_fl.cu: lane = two frames) against the CPU
+oracle through the C ABI.  Large batches on matrices with more than ~2.2 entries per pixel take it by themselves
+(BASELINE.json configs[3]: test_gpu_parity.py::test_batch_full_size_sampled); AZINT_FORCE_FL=1 sends every batch of plain
+32-bit frames through it, AZINT_TUNE="flc:N,fls:N" cuts the chunks short / caps the stages so that small cases cover
+several work items per block and ring wrap-arounds.
+"""
+import numpy as np
+import pytest
+
+from parity import assert_profile
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B(cuda_lib):
+    from paper_1412_6367_b200 import binding
+    binding.lib()
+    return binding
+
+
+_bounds = {}
+
+
+def _want(oracle, cfg, image, empty=0.0):
+    if cfg not in _bounds:
+        umin, umax = oracle.pixel_bounds(cfg)
+        _bounds.clear()
+        _bounds[cfg] = (umin, umax) + tuple(oracle.auto_range(umin, umax))
+    umin, umax, u0, u1 = _bounds[cfg]
+    return oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, image, None, None, None, None, None, empty=empty)
+
+
+def _batch(torch, B, integ, frames, stride=None):
+    n = frames.shape[0]
+    if frames.dtype == np.uint32:
+        t, code = torch.from_numpy(frames.view(np.int32)).cuda(), B.AI_U32
+    else:
+        t, code = torch.from_numpy(frames).cuda(), None
+    i, s, c = integ.outputs(n)
+    B.ai_integrate1d_batch(integ.ctx, t, n, stride or frames[0].size, None, None, None, None, None, i, s, c, dtype=code)
+    torch.cuda.synchronize()
+    assert B.ai_last_launch_count(integ.ctx) == 2
+    return i, s, c
+
+
+def _row(i, s, c, f):
+    return {"intensity": i[f].cpu().numpy(), "sum_signal": s[f].cpu().numpy(), "count": c[f].cpu().numpy()}
+
+
+SMALL = dict(center_x=100.3, center_y=90.1, npt=257, distance_m=0.02)
+
+
+@pytest.mark.parametrize("tune", [None, "flc:2", "flc:1,fls:2", "flo:1"])
+@pytest.mark.parametrize("dtype,nframes", [("int32", 7), ("int32", 64), ("uint32", 65), ("float32", 130)])
+def test_fl_batches_match_the_oracle(torch, B, oracle, workloads, monkeypatch, tune, dtype, nframes):
+    """Every frame of a forced frame-lane batch against the oracle: one frame short of / one beyond a group of 64, a
+    ragged image (264 = 8 tiles of 32 + 8 columns, 200 = 25 tiles of 8 rows), float frames with NaN and +-Inf."""
+    monkeypatch.setenv("AZINT_FORCE_FL", "1")
+    if tune:
+        monkeypatch.setenv("AZINT_TUNE", tune)
+    cfg = workloads.tiny_config(200, 264, unit=workloads.Q_NM, name="fl_small", **SMALL)
+    rng = np.random.default_rng(nframes)
+    frames = rng.poisson(100.0, size=(nframes, cfg.height, cfg.width)).astype(dtype)
+    if dtype == "float32":
+        frames[1, 17, 33] = np.nan
+        frames[nframes - 1, 100, 200] = np.inf
+        frames[64, 199, 263] = -np.inf
+        frames[3, 0, 0] = np.nan
+        frames[70, 40:60, :] = np.nan            # whole bins of one frame without a valid pixel
+    integ = B.Integrator(cfg)
+    i, s, c = _batch(torch, B, integ, frames)
+    step = 1 if nframes <= 16 else 9
+    for f in sorted(set(range(0, nframes, step)) | {1, 3, 64, 70, nframes - 1} & set(range(nframes))):
+        assert_profile(_row(i, s, c, f), _want(oracle, cfg, frames[f]), what=f"fl/{dtype}/{tune}/frame {f} of {nframes}")
+    integ.close()
+
+
+def test_fl_bins_without_a_valid_pixel_are_empty(torch, B, oracle, workloads, monkeypatch):
+    """A float frame whose centre region is NaN: the bins that only see that region have count exactly 0 and
+    intensity = empty_value (the invalid weight is subtracted from the row's coefficient sum in fixed point)."""
+    monkeypatch.setenv("AZINT_FORCE_FL", "1")
+    cfg = workloads.tiny_config(128, 128, center_x=64.0, center_y=64.0, unit=workloads.R_MM, npt=90, name="fl_hole")
+    rng = np.random.default_rng(5)
+    frames = rng.poisson(30.0, size=(66, cfg.height, cfg.width)).astype(np.float32)
+    yy, xx = np.mgrid[0:128, 0:128]
+    hole = (yy - 63.5) ** 2 + (xx - 63.5) ** 2 < 30.0 ** 2
+    frames[5][hole] = np.nan
+    frames[65][:] = np.nan
+    integ = B.Integrator(cfg, empty_value=-7.0)
+    i, s, c = _batch(torch, B, integ, frames)
+    for f in (0, 5, 65):
+        want = _want(oracle, cfg, frames[f], empty=-7.0)
+        got = _row(i, s, c, f)
+        assert (want["count"] <= 0).sum() > (10 if f == 5 else (89 if f == 65 else -1))
+        assert_profile(got, want, what=f"hole frame {f}")
+        assert np.array_equal(got["intensity"][want["count"] <= 0], np.full((want["count"] <= 0).sum(), -7.0, np.float32))
+    integ.close()
+
+
+def test_fl_rows_do_not_depend_on_the_batch(torch, B, workloads, monkeypatch):
+    """A frame's profiles are the same bits wherever it sits in a batch (which lane, which half of the lane, which
+    group), whatever the other frames are, and from run to run: every sum has a fixed order."""
+    monkeypatch.setenv("AZINT_FORCE_FL", "1")
+    monkeypatch.setenv("AZINT_TUNE", "flc:3")
+    cfg = workloads.tiny_config(200, 264, unit=workloads.TTH_DEG, name="fl_repro", **SMALL)
+    rng = np.random.default_rng(11)
+    pool = rng.poisson(200.0, size=(5, cfg.height, cfg.width)).astype(np.int32)
+    order = rng.integers(0, 5, size=150)
+    frames = pool[order]
+    integ = B.Integrator(cfg)
+    i, s, c = _batch(torch, B, integ, frames)
+    i2, s2, c2 = _batch(torch, B, integ, np.ascontiguousarray(frames[::-1]))
+    for k in range(5):
+        rows = np.nonzero(order == k)[0]
+        for r in rows[1:]:
+            assert torch.equal(i[r], i[rows[0]]) and torch.equal(s[r], s[rows[0]]) and torch.equal(c[r], c[rows[0]])
+        assert torch.equal(i2[149 - rows[0]], i[rows[0]]) and torch.equal(s2[149 - rows[0]], s[rows[0]])
+    integ.close()
+
+
+def test_fl_compensation_keeps_small_terms(torch, B, workloads, monkeypatch):
+    """PAPER.md:186-188 in the batched kernel: one pixel of 2^24 and 65535 pixels of 1 in one bin -- the per-product
+    Kahan recurrence keeps every 1 (plain fp32 accumulation would lose those added after the big value)."""
+    monkeypatch.setenv("AZINT_FORCE_FL", "1")
+    cfg = workloads.scaled(workloads.CONFIGS["cfg1"], npt=1)
+    img = np.ones((cfg.height, cfg.width), dtype=np.float32)
+    img[0, 0] = 2.0 ** 24
+    exact = 2.0 ** 24 + cfg.npix - 1
+    frames = np.stack([img, img[::-1].copy(), img * np.float32(0.5)] * 22)
+    integ = B.Integrator(cfg)
+    i, s, c = _batch(torch, B, integ, frames)
+    got = s.cpu().numpy()[:, 0]
+    assert np.all(np.abs(got[0::3] - exact) <= 1.0) and np.all(np.abs(got[1::3] - exact) <= 1.0)      # fp32 output spacing is 2
+    assert np.all(np.abs(got[2::3] - exact / 2) <= 0.5)
+    integ.close()
+
+
+def test_fl_frame_stride_and_the_other_kernels_agree(torch, B, oracle, workloads, monkeypatch):
+    """Frames 12 elements apart more than a frame; the slice-per-lane batched kernel (AZINT_NO_FL=1) gives the same
+    profiles within the tolerance (different, equally fixed, summation orders)."""
+    cfg = workloads.tiny_config(200, 264, unit=workloads.R_MM, name="fl_stride", **SMALL)
+    rng = np.random.default_rng(3)
+    n, stride = 67, cfg.npix + 12
+    buf = rng.poisson(50.0, size=(n, stride)).astype(np.int32)
+    t = torch.from_numpy(buf).cuda()
+    out = {}
+    for name, env in (("fl", "AZINT_FORCE_FL"), ("slices", "AZINT_NO_FL")):
+        monkeypatch.setenv(env, "1")
+        integ = B.Integrator(cfg)
+        i, s, c = integ.outputs(n)
+        B.ai_integrate1d_batch(integ.ctx, t, n, stride, None, None, None, None, None, i, s, c)
+        torch.cuda.synchronize()
+        out[name] = (i.cpu().numpy(), s.cpu().numpy(), c.cpu().numpy())
+        monkeypatch.delenv(env)
+        integ.close()
+    for f in (0, 33, 66):
+        img = buf[f, :cfg.npix].reshape(cfg.height, cfg.width)
+        want = _want(oracle, cfg, img)
+        for name in out:
+            got = {"intensity": out[name][0][f], "sum_signal": out[name][1][f], "count": out[name][2][f]}
+            assert_profile(got, want, what=f"{name} frame {f}")
+    assert np.allclose(out["fl"][1], out["slices"][1], rtol=1e-6, atol=0)
