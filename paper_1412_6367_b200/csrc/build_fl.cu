@@ -223,12 +223,18 @@ int ai_build_fl(ai_ctx *ctx, int nframes, cudaStream_t st)
         if (bmax[t] >= 0) order.push_back(t);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return bmin[a] < bmin[b]; });
     const int ntiles = (int)order.size();
-    // tiles per chunk: as many as possible (fewer flushes and barriers) while the batch this layout is built for still
-    // gives every SM about eight items
+    // tiles per chunk: large chunks mean fewer flushes and barriers, but the items (chunk x group of frames) are dealt to
+    // the SMs in rounds: of the sizes 8 .. kFlChunkTilesMax take the one whose last round is fullest for the batch this
+    // layout is built for (ties: the larger)
     int chunk_tiles = ctx->tune.fl_chunk;
     if (chunk_tiles <= 0) {
         const int64_t ngroups = (nframes + kFlFrames - 1) / kFlFrames, sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
-        chunk_tiles = (int)std::min<int64_t>(kFlChunkTilesMax, std::max<int64_t>(8, (int64_t)ntiles * ngroups / (8 * sms)));
+        double best = -1.0;
+        for (int ct = kFlChunkTilesMax; ct >= 8; --ct) {
+            const int64_t items = (int64_t)((ntiles + ct - 1) / ct) * ngroups, rounds = (items + sms - 1) / sms;
+            const double eff = (double)items / (double)(rounds * sms) - (rounds < 4 ? 0.05 * (4 - rounds) : 0.0);
+            if (eff > best + 1e-9) { best = eff; chunk_tiles = ct; }
+        }
     }
     std::vector<int4> chunk_desc;
     std::vector<int> chunk_lo;

@@ -225,37 +225,38 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
             prefetch_tile(ahead);
             fl_next(ahead, p);
         }
-        // 128-bit loads of rows 4 h .. 4 h + 3 of the tile for the lane's two frames
-        auto issue = [&](const FlWalk &w, int h, uint4 (&a)[kFlPassRows], uint4 (&b)[kFlPassRows], int4 &d) {
+        // 128-bit loads of rows 4 h .. 4 h + 3 of a tile for the lane's two frames; `src` = the lane's piece of row 0
+        struct Src {
+            const unsigned char *p;
+            int rows;                    // rows of the tile inside the image
+            bool in_a, in_b;
+        };
+        auto locate = [&](const FlWalk &w, int4 &d) {
             d = __ldg(p.tile_desc + w.r);
-            const int x = (d.z & 0xffff) * kFlTileW + piece * 4, y0 = (d.z >> 16) * kFlTileH + h * kFlPassRows;
+            const int x = (d.z & 0xffff) * kFlTileW + piece * 4, y0 = (d.z >> 16) * kFlTileH;
             const int fa = w.group * kFlFrames + 2 * cl;
-            const unsigned char *src = p.frames + (int64_t)fa * p.frame_stride_bytes + ((int64_t)y0 * p.width + x) * 4;
-            const bool in_a = fa < p.nframes && x < p.width, in_b = fa + 1 < p.nframes && x < p.width;
+            Src s;
+            s.p = p.frames + (int64_t)fa * p.frame_stride_bytes + ((int64_t)y0 * p.width + x) * 4;
+            s.rows = p.height - y0;
+            s.in_a = fa < p.nframes && x < p.width;
+            s.in_b = fa + 1 < p.nframes && x < p.width;
+            return s;
+        };
+        auto issue = [&](const Src &s, int h, uint4 (&a)[kFlPassRows], uint4 (&b)[kFlPassRows]) {
 #pragma unroll
             for (int u = 0; u < kFlPassRows; ++u) {
-                const unsigned char *q = src + u * row_bytes;
+                const int row = h * kFlPassRows + u;
+                const unsigned char *q = s.p + row * row_bytes;
                 a[u] = b[u] = make_uint4(0, 0, 0, 0);
-                if (in_a && y0 + u < p.height) a[u] = __ldcs(reinterpret_cast<const uint4 *>(q));
-                if (in_b && y0 + u < p.height) b[u] = __ldcs(reinterpret_cast<const uint4 *>(q + p.frame_stride_bytes));
+                if (s.in_a && row < s.rows) a[u] = __ldcs(reinterpret_cast<const uint4 *>(q));
+                if (s.in_b && row < s.rows) b[u] = __ldcs(reinterpret_cast<const uint4 *>(q + p.frame_stride_bytes));
             }
         };
-        int issued = 0;
         bool bad = false;
-        auto store = [&](int h, const uint4 (&a)[kFlPassRows], const uint4 (&b)[kFlPassRows], const int4 &d) {
-            unsigned char *stage = stage0 + (size_t)ring.stage * p.stage_bytes;
-            if (h == 0) {
-                if (issued >= p.stages) mbar_wait_relaxed(empty + ring.stage, ring.parity ^ 1u);
-                if (lw == 0 && lane == 0) {
-                    mbar_arrive_expect_tx(full + ring.stage, (uint32_t)d.y);
-                    bulk_g2s(stage + kFlImgBytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y, full + ring.stage);
-                }
-                bad = false;
-            }
-            const unsigned dst = smem_u32(stage) + dst_lane + (unsigned)(h * kFlPassRows * kFlTileW * 8);
+        auto store = [&](unsigned dst, int h, const uint4 (&a)[kFlPassRows], const uint4 (&b)[kFlPassRows]) {
 #pragma unroll
             for (int u = 0; u < kFlPassRows; ++u) {
-                const unsigned o = dst + (unsigned)(u * kFlTileW * 8);
+                const unsigned o = dst + (unsigned)((h * kFlPassRows + u) * kFlTileW * 8);
                 const float a0 = fl_cast<DT>(a[u].x), a1 = fl_cast<DT>(a[u].y), a2 = fl_cast<DT>(a[u].z), a3 = fl_cast<DT>(a[u].w);
                 const float b0 = fl_cast<DT>(b[u].x), b1 = fl_cast<DT>(b[u].y), b2 = fl_cast<DT>(b[u].z), b3 = fl_cast<DT>(b[u].w);
                 if constexpr (TRACK)
@@ -266,40 +267,49 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
                 sts_f2(o + d2, swap ? a0 : a2, swap ? b0 : b2);
                 sts_f2(o + d2 + 8, swap ? a1 : a3, swap ? b1 : b3);
             }
-            if (h == kFlTileH / kFlPassRows - 1) {
-                if constexpr (TRACK) {
-                    const bool any = __any_sync(AI_FULL_MASK, bad);
-                    if (lane == 0) flags[ring.stage * kFlLoad + lw] = any ? 1 : 0;
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(full + ring.stage);
-                ++issued;
-                ring.next(p.stages);
-            }
         };
-        // the loads of the next pass are in flight while the current one is cast and stored
+        // Steady state: both halves of the next tile are loaded (two register sets) while the current tile is cast and
+        // stored, and the loader then waits for the stage of the next tile with its loads in flight.
+        static_assert(kFlTileH == 2 * kFlPassRows, "a tile is two loader passes");
         uint4 a0[kFlPassRows], b0[kFlPassRows], a1[kFlPassRows], b1[kFlPassRows];
-        int4 d0 = make_int4(0, 0, 0, 0), d1 = d0;
-        int h = 0;
-        if (!cur.done) issue(cur, 0, a0, b0, d0);
+        int4 d = make_int4(0, 0, 0, 0), dn = d;
+        int issued = 0;
+        if (!cur.done) {
+            const Src s = locate(cur, d);
+            issue(s, 0, a0, b0);
+            issue(s, 1, a1, b1);
+        }
         while (!cur.done) {
             FlWalk nxt = cur;
-            int hn = h + 1;
-            if (hn == kFlTileH / kFlPassRows) {
-                hn = 0;
-                fl_next(nxt, p);
-                if (!ahead.done) {
-                    prefetch_tile(ahead);
-                    fl_next(ahead, p);
-                }
+            fl_next(nxt, p);
+            if (!ahead.done) {
+                prefetch_tile(ahead);
+                fl_next(ahead, p);
             }
-            if (!nxt.done) issue(nxt, hn, a1, b1, d1);
-            store(h, a0, b0, d0);
-#pragma unroll
-            for (int u = 0; u < kFlPassRows; ++u) { a0[u] = a1[u]; b0[u] = b1[u]; }
-            d0 = d1;
+            Src sn{};
+            if (!nxt.done) sn = locate(nxt, dn);
+            unsigned char *stage = stage0 + (size_t)ring.stage * p.stage_bytes;
+            if (issued >= p.stages) mbar_wait_relaxed(empty + ring.stage, ring.parity ^ 1u);
+            if (lw == 0 && lane == 0) {
+                mbar_arrive_expect_tx(full + ring.stage, (uint32_t)d.y);
+                bulk_g2s(stage + kFlImgBytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y, full + ring.stage);
+            }
+            const unsigned dst = smem_u32(stage) + dst_lane;
+            bad = false;
+            store(dst, 0, a0, b0);
+            if (!nxt.done) issue(sn, 0, a0, b0);
+            store(dst, 1, a1, b1);
+            if (!nxt.done) issue(sn, 1, a1, b1);
+            if constexpr (TRACK) {
+                const bool any = __any_sync(AI_FULL_MASK, bad);
+                if (lane == 0) flags[ring.stage * kFlLoad + lw] = any ? 1 : 0;
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(full + ring.stage);
+            ++issued;
+            ring.next(p.stages);
+            d = dn;
             cur = nxt;
-            h = hn;
         }
     } else {
         // ===== consumers ===============================================================================================
