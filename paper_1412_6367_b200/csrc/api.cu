@@ -161,6 +161,8 @@ static int setup_common(ai_ctx **out, const ai_geometry *g, int height, int widt
                 else if (!strcmp(key, "fl")) ctx->tune.inflight = val;
                 else if (!strcmp(key, "ss")) ctx->tune.stream_stages = val;
                 else if (!strcmp(key, "nov")) ctx->tune.no_overlap = val;
+                else if (!strcmp(key, "fbs")) ctx->tune.fin_blocks_per_sm = val;
+                else if (!strcmp(key, "ncg")) ctx->tune.no_chain_guard = val;
                 else if (!strcmp(key, "bu")) ctx->tune.batch_units = val;
                 else if (!strcmp(key, "fls")) ctx->tune.fl_stages = val;
                 else if (!strcmp(key, "flc")) ctx->tune.fl_chunk = val;
@@ -210,6 +212,8 @@ int ai_build_csr(ai_ctx *ctx, void *cuda_stream)
     if (rc != AI_OK) return rc;
     AI_CUDA(ctx, cudaMalloc(&ctx->out_dev, 3 * (size_t)ctx->npt * sizeof(float)));
     AI_CUDA(ctx, cudaMalloc(&ctx->grid_sync, 3 * sizeof(unsigned long long)));
+    AI_CUDA(ctx, cudaMalloc(&ctx->chain_done, sizeof(unsigned long long)));
+    AI_CUDA(ctx, cudaMemsetAsync(ctx->chain_done, 0, sizeof(unsigned long long), st));
     AI_CUDA(ctx, cudaMemsetAsync(ctx->grid_sync, 0, 3 * sizeof(unsigned long long), st));
     AI_CUDA(ctx, cudaMalloc(&ctx->stream_partials, 2 * (size_t)(ctx->tl.nslot > 0 ? ctx->tl.nslot : 1) * 16));
     AI_CUDA(ctx, cudaStreamSynchronize(st));
@@ -474,7 +478,7 @@ void ai_destroy(ai_ctx *ctx)
     free(tl.h_first_desc);
     free(ctx->stream_first);
     ai_free_fl(ctx->fl);
-    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->stream_partials); cudaFree(ctx->axes2d); cudaFree(ctx->corrected[0]); cudaFree(ctx->corrected[1]);
+    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->chain_done); cudaFree(ctx->stream_partials); cudaFree(ctx->axes2d); cudaFree(ctx->corrected[0]); cudaFree(ctx->corrected[1]);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;

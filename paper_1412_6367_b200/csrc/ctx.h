@@ -58,6 +58,8 @@ struct PipeTune {
     int batch_mat_stages = 2, batch_img_stages = kPipeMaxImgStages;
     int inflight = 0;                          // 0 = as many as there are stages
     int stream_stages = 0;                     // cap on the (tile + blob) stages of the single-frame kernel, 0 = none
+    int no_chain_guard = 0;                    // measurement: the stream kernel does not wait for the count of ended finish blocks
+    int fin_blocks_per_sm = 0;                 // finish kernel of the single-frame chain: blocks per SM at most, 0 = default
     int no_overlap = 0;                        // single-frame kernel: never stream ahead of the grid dependency
     int batch_units = 0;                       // batched kernel: 1 = (block, frame) units, 2 = (block, two frames), 0 = by layout
     int fl_stages = 0;                         // frame-lane kernel: cap on the stages, 0 = none
@@ -212,6 +214,12 @@ struct ai_ctx {
     unsigned long long *grid_sync = nullptr;   // [3] tile tickets, used in rotation
     void *stream_partials = nullptr;           // [2][nslot] partial records
     unsigned stream_launches = 0;              // single-frame launches of this context so far
+    // Blocks of finish kernels of this context that have ended, ever increasing.  The launch chain re-uses a set of
+    // partial sums (and a corrected frame) every second call on the argument that a block of the stream kernel only
+    // becomes resident where a block of the previous launch has left; another tenant of the GPU (a second context on a
+    // second stream) frees SMs out of turn, so the kernels that re-use check this count as well (normally long reached).
+    unsigned long long *chain_done = nullptr;  // device
+    unsigned long long fin_cum = 0, fin_cum_prev = 0;   // the count after every finish kernel launched so far / all but the last
     uint64_t stream_shared_sm = 0;             // bit k: instantiation k of the kernel does NOT have an SM to itself
     // tensor map of the last frame buffer seen by the TMA kernels (encoding one costs the host ~1-2 us per call)
     struct MapEntry {

@@ -5,6 +5,7 @@
 // for a 2048 x 2048 frame, normally still in L2 when it is read back.  Chosen by measurement over staging the
 // corrections inside the gather kernel.
 #include "common.cuh"
+#include "pipe_common.cuh"
 
 namespace {
 
@@ -13,7 +14,9 @@ constexpr int kPrepThreads = 256;
 template <int DT>
 __global__ void __launch_bounds__(kPrepThreads) correct_frame_kernel(const void *__restrict__ img, Corrections cor,
                                                                      int64_t npix, int width, int pitch, int vec_ok,
-                                                                     int overlap, int mode, float *__restrict__ out)
+                                                                     int overlap, int mode, float *__restrict__ out,
+                                                                     const unsigned long long *chain_done,
+                                                                     unsigned long long chain_target)
 {
     // Launch chain (integrate_stream.cu): the single-frame kernel that follows may start its prologue (it reads `out`
     // after its griddepcontrol.wait).  overlap: this pass itself runs beside the stream kernel of the PREVIOUS call --
@@ -22,6 +25,13 @@ __global__ void __launch_bounds__(kPrepThreads) correct_frame_kernel(const void 
     // only before it leaves, so that completion stays transitive along the stream.
     asm volatile("griddepcontrol.launch_dependents;");
     if (!overlap) asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (overlap) {
+        // the corrected frame this pass overwrites was read by the stream kernel of the call before the previous one: it
+        // has ended if the finish kernel behind it has (checked for the case of another tenant on the GPU, integrate_stream.cu)
+        if (threadIdx.x == 0) wait_count_at_least(chain_done, chain_target);
+        __syncthreads();
+    }
+
     const bool has_den = cor.flat || cor.solidangle || cor.polarization;
     const int64_t stride = (int64_t)gridDim.x * kPrepThreads;
     if (vec_ok) {
@@ -80,7 +90,8 @@ int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, 
     cfg.attrs = attr;
     cfg.numAttrs = 1;
 #define AI_PREP(DT) \
-    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, correct_frame_kernel<DT>, a.image, cor, npix, ctx->width, pitch, vec, overlap, mode, dst))
+    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, correct_frame_kernel<DT>, a.image, cor, npix, ctx->width, pitch, vec, overlap, mode, dst, \
+                                    (const unsigned long long *)ctx->chain_done, ctx->fin_cum_prev))
     switch (a.dtype) {
     case AI_F32: AI_PREP(AI_F32); break;
     case AI_I32: AI_PREP(AI_I32); break;

@@ -50,6 +50,8 @@ struct StreamParams {
     int full_grid;                     // one block on every SM: a block of this launch runs where the previous
                                        // launch's block has left, so the launch before that one is complete
     int overlap;                       // stream before the grid dependency is resolved (see the kernel)
+    const unsigned long long *chain_done;   // overlap: the finish kernel that read this launch's set of partials last has
+    unsigned long long chain_target;        // ended when *chain_done >= chain_target
 };
 
 // ---- development aid (-DAI_STREAM_TRACE): every warp of the single-frame kernel logs (globaltimer, code) events ----------
@@ -356,6 +358,10 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
             ++stage;
         }
     }
+    // overlap: nothing of this block writes partial sums before the finish kernel of the call before the previous one
+    // has read the set they share.  With the GPU to itself the chain guarantees it (see below); checked because another
+    // tenant may have let this block in out of turn.  One thread of a consumer warp, while thread 0 sets the block up.
+    if (threadIdx.x == 32 && p.overlap) wait_count_at_least(p.chain_done, p.chain_target);
     // the descriptors of the ticketed tiles (each block its share of the array), pulled into L2 now
     for (int k = p.dyn_base + (blockIdx.x * kStreamThreads + threadIdx.x) * 8; k < p.ntiles; k += gridDim.x * kStreamThreads * 8)
         asm volatile("prefetch.global.L2 [%0];" ::"l"(p.blob_desc + k));
@@ -736,6 +742,9 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int tra
     p.tickets_reset = ctx->grid_sync + (seq + 1) % 3;
     p.full_grid = grid == sms;
     p.overlap = p.full_grid && !image_dep && !ctx->tune.no_overlap;
+    p.chain_done = ctx->chain_done;
+    p.chain_target = ctx->tune.no_chain_guard ? 0ULL : ctx->fin_cum_prev;
+
     const size_t smem = (size_t)stages * (p.img_stage_bytes + p.mat_stage_bytes) + p.hdr_bytes;
 
     // descriptors of the first tiles of every block (host copy kept by the builder), assembled once per context

@@ -12,6 +12,7 @@
 //   stage 2  one warp per (bin, frame): adds the bin's partials in a fixed order and writes the three outputs
 //            (ratio, unweighted histogram, weighted histogram).  No atomics anywhere, so results are
 //            bit-reproducible; every bin is written exactly once, so the paper's memset disappears.
+#include "pipe_common.cuh"
 #include "tiled_common.cuh"
 
 int ai_launch_pipe_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);
@@ -140,8 +141,18 @@ __global__ void __launch_bounds__(kFinishThreads, 10) tiled_finish_kernel(const 
                                                                            float *__restrict__ radial,
                                                                            float *__restrict__ intensity,
                                                                            float *__restrict__ sum_signal,
-                                                                           float *__restrict__ count)
+                                                                           float *__restrict__ count,
+                                                                           unsigned long long *chain_done)
 {
+    // every block counts itself out (release) when it has read its partials: what the kernels that reuse them check
+    struct Done {
+        unsigned long long *c;
+        __device__ ~Done()
+        {
+            __syncthreads();
+            if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(c), "l"(1ULL) : "memory");
+        }
+    } done{chain_done};
     const int lane = threadIdx.x & 31, nw = gridDim.x * (kFinishThreads / 32);
     int b = blockIdx.x * (kFinishThreads / 32) + (threadIdx.x >> 5);
     int beg = 0, end = 0;
@@ -243,8 +254,12 @@ int launch_finish(ai_ctx *ctx, const FrameArgs &a, const void *partials, cudaStr
     const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
     const int wpb = kFinishThreads / 32;
     const int serial = (long long)tl.nslot < 8LL * ctx->npt;      // few partials per bin: one thread per bin
+    // up to fin_blocks_per_sm small blocks per SM (they fit beside a block of the stream kernel): the kernel is a chain of
+    // memory latencies per bin, so fewer bins per warp end it sooner -- and the stream kernel of the NEXT call cannot
+    // leave before this one has ended
+    const int per_sm = ctx->tune.fin_blocks_per_sm > 0 ? ctx->tune.fin_blocks_per_sm : 3;
     int grid = serial ? (ctx->npt + kFinishThreads - 1) / kFinishThreads : (ctx->npt + wpb - 1) / wpb;
-    if (grid > sms) grid = sms;
+    if (grid > per_sm * sms) grid = per_sm * sms;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
@@ -258,13 +273,15 @@ int launch_finish(ai_ctx *ctx, const FrameArgs &a, const void *partials, cudaStr
 #define AI_FIN(ACC)                                                                                                   \
     AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, tiled_finish_kernel<ACC>, (const int *)tl.bin_slot_ptr, ctx->npt, serial, partials,  \
                                     (const double *)ctx->d_range, ctx->empty_value, a.radial, a.intensity,           \
-                                    a.sum_signal, a.count))
+                                    a.sum_signal, a.count, ctx->chain_done))
     switch (ctx->accum) {
     case AI_ACC_F32_KAHAN: AI_FIN(AI_ACC_F32_KAHAN); break;
     case AI_ACC_F32_PLAIN: AI_FIN(AI_ACC_F32_PLAIN); break;
     default: AI_FIN(AI_ACC_F64); break;
     }
 #undef AI_FIN
+    ctx->fin_cum_prev = ctx->fin_cum;
+    ctx->fin_cum += (unsigned long long)grid;
     return AI_OK;
 }
 

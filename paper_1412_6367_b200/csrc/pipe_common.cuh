@@ -74,6 +74,21 @@ __device__ __forceinline__ void tma_box(void *dst_smem, const CUtensorMap *map, 
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
                  ::"r"(smem_u32(dst_smem)), "l"(map), "r"(x), "r"(y), "r"(f), "r"(smem_u32(bar)) : "memory");
 }
+// waits until *counter >= target (acquire); bounded like mbar_wait
+__device__ __forceinline__ void wait_count_at_least(const unsigned long long *counter, unsigned long long target)
+{
+    unsigned long long t0 = 0;
+    for (unsigned spin = 1;; ++spin) {
+        unsigned long long seen;
+        asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(counter) : "memory");
+        if (seen >= target) return;
+        if ((spin & 0x3ffu) == 0) {
+            const unsigned long long now = globaltimer_ns();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 20000000000ULL) __trap();
+        }
+    }
+}
 // acquire-release fences (lighter than __threadfence / __threadfence_block, which are sequentially consistent fences)
 __device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
 __device__ __forceinline__ void fence_acq_rel_cta() { asm volatile("fence.acq_rel.cta;" ::: "memory"); }

@@ -326,6 +326,51 @@ def test_mixed_call_sequence_is_bit_reproducible(torch, B, workloads):
         it.close()
 
 
+@pytest.mark.parametrize("masked", [False, True])
+def test_two_contexts_on_two_streams(torch, B, workloads, masked):
+    """Two contexts driven from two streams at once (another tenant on the GPU): blocks of either context's stream kernel
+    become resident out of turn, so the launch chain's "one block per SM" argument for re-using a set of partial sums
+    (and a corrected frame) every second call does not hold by itself -- the kernels check the count of ended finish
+    kernels.  3000 bins (BASELINE.json configs[2]'s shape), a few hundred calls per context, every call's result compared
+    with the context's isolated result for that frame, bit for bit."""
+    cfg = workloads.CONFIGS["cfg3"]
+    base = workloads.make_frame(cfg)
+    rng = np.random.default_rng(42)
+    frames = [torch.from_numpy(base.image * np.float32(s)).cuda() for s in (1.0, 0.5, 2.0)]
+    mask = torch.from_numpy(base.mask).cuda() if masked else None
+    ctxs = [B.Integrator(cfg), B.Integrator(cfg)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ref = []
+    for it in ctxs:                                  # isolated results, one call at a time
+        r = []
+        for f in frames:
+            o = it.integrate1d(f, mask=mask)
+            torch.cuda.synchronize()
+            r.append(tuple(t.clone() for t in o))
+        ref.append(r)
+    ncalls = 240
+    outs = [[tuple(torch.empty(cfg.npt, dtype=torch.float32, device="cuda") for _ in range(3)) for _ in range(ncalls)]
+            for _ in ctxs]
+    order = rng.integers(0, 3, size=(2, ncalls))
+    torch.cuda.synchronize()
+    k = [0, 0]
+    while k[0] < ncalls or k[1] < ncalls:            # enqueue in uneven bursts so that the two chains drift past each other
+        j = int(rng.integers(0, 2))
+        for _ in range(int(rng.integers(1, 9))):
+            if k[j] < ncalls:
+                with torch.cuda.stream(streams[j]):
+                    ctxs[j].integrate1d(frames[order[j, k[j]]], mask=mask, out=outs[j][k[j]])
+                k[j] += 1
+    torch.cuda.synchronize()
+    for j in range(2):
+        for n in range(ncalls):
+            want = ref[j][order[j, n]]
+            got = outs[j][n]
+            assert torch.equal(got[0], want[0]) and torch.equal(got[1], want[1]) and torch.equal(got[2], want[2]), (j, n)
+    for it in ctxs:
+        it.close()
+
+
 def test_compensation_keeps_small_terms(torch, B, workloads):
     """Kahan summation lets single precision give accurate sums.  One bin, one pixel of 2^24 and
     65535 pixels of 1: the exact sum is 2^24 + 65535; every lane that holds the big value would drop the ones without
