@@ -130,6 +130,8 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
                                   "frac_of_peak": abb / (ms * 1e-3) / 1e9 / peak_gbs,
                                   "extra_bytes_not_in_the_algorithmic_count":
                                       {"partial_records_written_and_read_back": 2 * 16 * info["nslot"] * nb},
+                                  "kernel": "tiled_bstream_kernel (slices per lane; 64 frames and 1.9 entries per pixel are below "
+                                            "what the frame-lane kernel takes)",
                                   "note": "ai_integrate1d_batch on 64 device-resident cfg2 frames; results are bit-identical "
                                           "to the single-frame kernel's"}
     del fb, outb
@@ -137,30 +139,56 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
     c4 = W.CONFIGS["cfg4"]
     pool = torch.from_numpy(W.make_frames(c4, 8)).to(device)
     frames = pool.repeat(c4.nframes // 8, 1, 1)
-    it = B.Integrator(c4, device=device)
-    out = it.outputs(c4.nframes)
-    for _ in range(2):
-        it.integrate1d_batch(frames, out=out)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    reps = 5
-    e0.record()
-    for _ in range(reps):
-        it.integrate1d_batch(frames, out=out)
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / reps
+    import os
+
+    def time_cfg4(env):
+        """ms per 1024-frame call (5 calls back to back after 2 warm-up calls) and the context, still open"""
+        for k, v in env.items():
+            os.environ[k] = v
+        it4 = B.Integrator(c4, device=device)
+        for k in env:
+            del os.environ[k]
+        out4 = it4.outputs(c4.nframes)
+        for _ in range(2):
+            it4.integrate1d_batch(frames, out=out4)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 5
+        e0.record()
+        for _ in range(reps):
+            it4.integrate1d_batch(frames, out=out4)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps, it4, out4
+
+    ms, it, out = time_cfg4({})
     nnz4 = B.ai_get_csr(it.ctx)[3]
     ab4 = c4.nframes * c4.npix * 4 + nnz4 * 8 + (c4.npt + 1) * 4 + c4.nframes * 3 * c4.npt * 4
+    fl4 = B.ai_get_batch_layout_info(it.ctx)
+    res_fl = [o.clone() for o in out]
+    it.close()
+    # the same call through the slice-per-lane batched kernel (AZINT_NO_FL=1): what the frame-lane kernel replaced here
+    ms_sl, it, out = time_cfg4({"AZINT_NO_FL": "1"})
     info4 = B.ai_get_layout_info(it.ctx)
+    dmax = max(float(((a - b).abs() / b.abs().clamp_min(1e-30)).max()) for a, b in zip(res_fl[:2], out[:2]))
+    it.close()
     ex["batch_cfg4_1024_frames"] = {"frames_per_s": c4.nframes / (ms * 1e-3), "ms_per_batch": ms,
+                                    "kernel": "fl_batch_kernel (frame-lane: lane = two frames, DESIGN.md 5.4)" if fl4["built"]
+                                              else "tiled_bstream_kernel",
                                     "algorithmic_bytes": ab4, "algorithmic_GBps": ab4 / (ms * 1e-3) / 1e9,
                                     "frac_of_peak": ab4 / (ms * 1e-3) / 1e9 / peak_gbs,
                                     "extra_bytes_not_in_the_algorithmic_count":
+                                        {"partial_sums_written_and_read_back": 2 * 8 * fl4["nslot"] * c4.nframes,
+                                         "matrix_blobs_read_once_per_group_of_64_frames_mostly_from_L2":
+                                             fl4["blob_bytes"] * (c4.nframes // 64)} if fl4["built"] else
                                         {"partial_records_written_and_read_back": 2 * 16 * info4["nslot"] * c4.nframes},
+                                    "layout": fl4,
                                     "vs_3000_fps_detector": c4.nframes / (ms * 1e-3) / 3000.0,
+                                    "slice_per_lane_kernel_AZINT_NO_FL": {
+                                        "ms_per_batch": ms_sl, "frac_of_peak": ab4 / (ms_sl * 1e-3) / 1e9 / peak_gbs,
+                                        "partial_records_written_and_read_back": 2 * 16 * info4["nslot"] * c4.nframes,
+                                        "max_rel_diff_of_the_two_kernels_profiles": dmax},
                                     "note": "4.3 GB of frames > L2; 8 distinct frames repeated"}
-    it.close()
     # bidimensional integration of the headline frame: 360 azimuthal x 500 radial bins (PAPER.md:29, :114-116)
     ck = W.CONFIGS["cake2"]
     its = [B.Integrator(ck, device=device) for _ in range(3)]

@@ -178,7 +178,12 @@ int ai_integrate2d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *
  *   frames                     frame f starts at element f * frame_stride_elems (>= height*width)
  *   intensity, sum_signal,
  *   count                      float32[nframes][npt], row-major
- * Enqueues on `cuda_stream`; does not synchronise.  Errors as ai_integrate1d. */
+ * Enqueues on `cuda_stream`; does not synchronise -- with one exception: the first batch of 96 or more plain 32-bit
+ * frames on a 1D context whose matrix has more than ~2.2 entries per pixel builds the frame-lane layout of the matrix
+ * (one-time, synchronises `cuda_stream`; see ai_get_batch_layout_info), and a larger batch than any
+ * before re-allocates scratch (cudaFree synchronises the device).  A frame's profiles do not depend on where it sits in
+ * a batch, but they are not bit-identical between the kernels a batch may take (different fixed summation orders).
+ * Errors as ai_integrate1d. */
 int ai_integrate1d_batch(ai_ctx *ctx, const void *frames, ai_dtype dtype, int nframes, int64_t frame_stride_elems,
                          const float *dark, const float *flat, const float *solidangle, const float *polarization,
                          const uint8_t *mask, float *intensity, float *sum_signal, float *count, void *cuda_stream);
@@ -210,6 +215,13 @@ int ai_integrate1d_host_frames(ai_ctx *ctx, const void *frames_host, ai_dtype dt
  * total bytes of the sliced matrix (all blobs), largest blob in bytes, partial records per frame, (tile + blob) stages
  * the single-frame kernel would use (0 = it does not apply)}.  Errors: AI_EINVAL, AI_ENOTBUILT. */
 int ai_get_layout_info(const ai_ctx *ctx, int64_t info[8]);
+
+/* Sizes of the frame-lane layout used by large batches.  info (HOST pointer) receives 8 values:
+ * {1 if the layout is built (0: not yet, or it does not apply -- the rest is 0 then), tile height in rows (tiles are 32
+ * pixels wide), tiles that hold entries, chunks of tiles (a work item = chunk x group of 64 frames), partial sums per
+ * frame (one per chunk and bin of the chunk's window), total bytes of the blobs, largest blob in bytes, frames per
+ * group}.  Errors: AI_EINVAL, AI_ENOTBUILT. */
+int ai_get_batch_layout_info(const ai_ctx *ctx, int64_t info[8]);
 
 /* Number of kernels the last ai_integrate1d* call launched (for accounting in benchmarks). */
 int ai_last_launch_count(const ai_ctx *ctx);

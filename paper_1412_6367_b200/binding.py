@@ -23,7 +23,7 @@ AI_SPLIT_BBOX, AI_SPLIT_FULL = range(2)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_set_splitting", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
-           "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_get_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
+           "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_get_layout_info", "ai_get_batch_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
 class ai_geometry(C.Structure):
@@ -64,6 +64,7 @@ def lib():
     L.ai_integrate1d_host.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_integrate1d_host_frames.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_get_layout_info.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.ai_get_batch_layout_info.argtypes = [vp, C.POINTER(C.c_int64)]
     L.ai_last_launch_count.argtypes = [vp]
     L.ai_profile_enable.argtypes = [vp, C.c_int]
     L.ai_profile_last.argtypes = [vp, C.POINTER(C.c_float)]
@@ -205,6 +206,14 @@ def ai_get_layout_info(ctx) -> dict:
     a = (C.c_int64 * 8)()
     _check(lib().ai_get_layout_info(ctx, a), ctx)
     keys = ("tile_h", "ntiles", "nseg", "padded_entries", "blob_bytes", "max_blob_bytes", "nslot", "stream_stages")
+    return dict(zip(keys, [int(x) for x in a]))
+
+
+def ai_get_batch_layout_info(ctx) -> dict:
+    """Sizes of the frame-lane layout large batches use (see include/azint.h); built=0 before the first such batch."""
+    a = (C.c_int64 * 8)()
+    _check(lib().ai_get_batch_layout_info(ctx, a), ctx)
+    keys = ("built", "tile_h", "ntiles", "nchunks", "nslot", "blob_bytes", "max_blob_bytes", "frames_per_group")
     return dict(zip(keys, [int(x) for x in a]))
 
 

@@ -54,6 +54,24 @@ int ai_get_layout_info(const ai_ctx *ctx, int64_t info[8])
     return AI_OK;
 }
 
+int ai_get_batch_layout_info(const ai_ctx *ctx, int64_t info[8])
+{
+    if (!ctx || !info) return AI_EINVAL;
+    if (!ctx->built) return AI_ENOTBUILT;
+    const FlLayout &fl = ctx->fl;
+    for (int k = 0; k < 8; ++k) info[k] = 0;
+    if (!fl.ok) return AI_OK;
+    info[0] = 1;
+    info[1] = kFlTileH;
+    info[2] = fl.ntiles;
+    info[3] = fl.nchunks;
+    info[4] = fl.nslot;
+    info[5] = fl.blob_bytes;
+    info[6] = fl.max_blob_bytes;
+    info[7] = kFlFrames;
+    return AI_OK;
+}
+
 int ai_profile_enable(ai_ctx *ctx, int on)
 {
     if (!ctx) return AI_EINVAL;
