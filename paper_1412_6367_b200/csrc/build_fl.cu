@@ -1,14 +1,16 @@
 // Frame-lane layout of the matrix (SURVEY.md section 8(a) B6 "derived layouts", H6): the
 // bounding-box coefficients of the canonical CSR, re-ordered for the batched kernel of
-// integrate_fl.cu, in which the 32 lanes of a warp are 32 frames and every matrix entry is warp-uniform.
-//   - the image is cut into tiles of kFlTileW x tile_h pixels; a tile's entries are grouped by bin into segments;
-//   - tiles are ordered by their lowest bin and cut into chunks of <= kFlChunkTiles tiles whose bins fit a window of
-//     kFlWindow bins: the kernel keeps one shared-memory accumulator per (bin of the window, frame) and writes one
+// integrate_fl.cu, in which the 32 lanes of a warp are 32 pairs of frames and every matrix entry is warp-uniform.
+//   - the image is cut into tiles of kFlTileW x kFlTileH pixels; a tile's entries are grouped by bin into segments;
+//   - tiles are ordered by their lowest bin and cut into chunks of at most kFlChunkTilesMax tiles whose bins fit a window
+//     of kFlWindow bins: the kernel keeps one shared-memory accumulator per (bin of the window, frame) and writes one
 //     partial per (chunk, bin, frame);
-//   - inside a chunk every bin belongs to ONE consumer warp (longest-processing-time-first over the chunk's entries per
-//     bin), so accumulators are never shared between warps and every sum has a fixed order;
+//   - inside a chunk every bin belongs to ONE consumer warp (dealt round-robin: a tile's bins are a contiguous range, so
+//     every warp gets an even sample of its short and long segments), so accumulators are never shared between warps and
+//     every sum has a fixed order;
 //   - a tile's blob = header {first record of each warp} + records {bin - chunk's lowest bin, pairs, first pair} +
-//     entry pairs {c0, c1, byte offset of pixel 0, byte offset of pixel 1} (one 128-bit broadcast load per pair).
+//     entry pairs {c0, c1, byte offset of pixel 0, byte offset of pixel 1} (one 128-bit broadcast load per pair), a
+//     warp's segments one after the other.
 // Built from the canonical CSR on the device (count, fill: one warp per row, entries keep the row's ascending pixel
 // order, no atomics on the data path); the plan in between (chunks, owners, offsets) is host work over the segment
 // lengths.

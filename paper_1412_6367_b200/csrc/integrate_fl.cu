@@ -4,7 +4,7 @@
 //
 // fl_batch_kernel: lane = two frames.  A work item is (chunk of tiles, group of 64 frames); one persistent block per SM.
 //   - kFlLoad loader warps bring a tile (32 x 8 pixels) of the group's 64 frames in with 128-bit loads (the lines were
-//     pulled into L2 two tiles earlier by bulk prefetches), cast them (H1) and store the two frames of
+//     pulled into L2 three tiles earlier by one tensor-map prefetch per tile), cast them (H1) and store the two frames of
 //     lane l interleaved pixel by pixel, lane l shifted by 2 l words (lane pitch = tile bytes + 8): the 32 lanes of a
 //     gather -- same pixel, 64 frames -- fall into 32 different bank pairs.  The tile's blob of the matrix arrives by one
 //     bulk copy.  One ring of (tile + blob) stages, one full / empty mbarrier pair per stage.
@@ -96,11 +96,6 @@ __device__ __forceinline__ void sts_f2(unsigned addr, float a, float b)
 {
     asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
 }
-__device__ __forceinline__ void prefetch_l2(const void *p, unsigned bytes)
-{
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
-}
-
 // Waits of the frame-lane kernel: try_wait with a long suspend-time hint -- the warp sleeps in the barrier unit until
 // the phase completes instead of polling, so waiting warps leave the issue slots to the warps that work.  Bounded
 // (20 s of wall time) like mbar_wait.
@@ -128,18 +123,11 @@ __device__ __forceinline__ void kahan2(unsigned long long &s, unsigned long long
                                        unsigned long long v)
 {
     const unsigned long long y = fma2(c2, v, e);
-#ifndef AI_FL_MIXED_KAHAN
+    // (FFMA2 / FADD2 run on one of the SM's two fp32 pipes, ~4 cycles per warp instruction; doing the two middle steps as
+    // scalar adds for the other pipe was measured no faster: the kernel is bound by shared-memory wavefronts)
     const unsigned long long t = add2(s, y);
     e = add2(sub2(s, t), y);
     s = t;
-#else
-    // FFMA2 / FADD2 run on one of the SM's two fp32 pipes only (measured: ~4 cycles per warp instruction): the two middle
-    // steps go as scalar adds so that the other pipe takes its share
-    const float tx = __fadd_rn(lo_of(s), lo_of(y)), ty = __fadd_rn(hi_of(s), hi_of(y));
-    const float ux = __fsub_rn(lo_of(s), tx), uy = __fsub_rn(hi_of(s), ty);
-    e = add2(pack2(ux, uy), y);
-    s = pack2(tx, ty);
-#endif
 }
 
 // position in the sequence of (item, tile) this block walks: items blockIdx.x, + gridDim.x, ...; an item is a chunk of
