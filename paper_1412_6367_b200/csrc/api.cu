@@ -94,6 +94,7 @@ int ai_profile_last(ai_ctx *ctx, float *kernel_ms)
     return AI_OK;
 }
 
+static void release_matrix_and_scratch(ai_ctx *ctx);
 static int setup_common(ai_ctx **out, const ai_geometry *g, int height, int width, int npt, ai_unit unit,
                         const double *range_or_null);
 
@@ -199,6 +200,7 @@ int ai_build_csr(ai_ctx *ctx, void *cuda_stream)
 {
     if (!ctx) return AI_EINVAL;
     if (ctx->built) return AI_OK;
+    release_matrix_and_scratch(ctx);          // whatever an earlier, failed build left
     cudaStream_t st = (cudaStream_t)cuda_stream;
     AI_CUDA(ctx, cudaGetDevice(&ctx->device));
     AI_CUDA(ctx, cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device));
@@ -478,6 +480,33 @@ int ai_integrate1d_host_frames(ai_ctx *ctx, const void *frames_host, ai_dtype dt
     return AI_OK;
 }
 
+// everything ai_build_csr and the integrate calls allocate on the device (and the host copies that go with it), freed and
+// reset: ai_destroy, and ai_build_csr before it builds (a build that failed half-way leaves nothing behind)
+static void release_matrix_and_scratch(ai_ctx *ctx)
+{
+    auto drop = [](auto *&p) { cudaFree(p); p = nullptr; };
+    drop(ctx->indptr); drop(ctx->indices); drop(ctx->data); drop(ctx->row_csum); drop(ctx->d_range);
+    drop(ctx->lut_coef); drop(ctx->lut_idx); drop(ctx->csr_seg); drop(ctx->csr_row_seg_ptr); drop(ctx->csr_partials);
+    drop(ctx->scat_first_nb); drop(ctx->scat_gw); drop(ctx->norm_scratch);
+    ctx->csr_partials_bytes = 0;
+    ctx->csr_nseg = 0;
+    ctx->lut_width = 0;
+    TiledLayout &tl = ctx->tl;
+    cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_meta); cudaFree(tl.seg_csum);
+    cudaFree(tl.tile_desc); cudaFree(tl.tile_order); cudaFree(tl.blob); cudaFree(tl.blob_desc);
+    cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
+    free(tl.h_first_desc);
+    tl = TiledLayout{};
+    free(ctx->stream_first);
+    ctx->stream_first = nullptr;
+    ctx->stream_first_grid = 0;
+    ai_free_fl(ctx->fl);
+    drop(ctx->partials); drop(ctx->staging); drop(ctx->out_dev); drop(ctx->grid_sync); drop(ctx->chain_done);
+    drop(ctx->stream_partials); drop(ctx->axes2d); drop(ctx->corrected[0]); drop(ctx->corrected[1]);
+    ctx->partials_bytes = ctx->staging_bytes = 0;
+    ctx->nnz = 0;
+}
+
 void ai_destroy(ai_ctx *ctx)
 {
     if (!ctx) return;
@@ -487,16 +516,7 @@ void ai_destroy(ai_ctx *ctx)
         if (ctx->slot_free[i]) cudaEventDestroy(ctx->slot_free[i]);
     }
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
-    cudaFree(ctx->indptr); cudaFree(ctx->indices); cudaFree(ctx->data); cudaFree(ctx->row_csum); cudaFree(ctx->d_range);
-    cudaFree(ctx->lut_coef); cudaFree(ctx->lut_idx); cudaFree(ctx->csr_seg); cudaFree(ctx->csr_row_seg_ptr); cudaFree(ctx->csr_partials); cudaFree(ctx->scat_first_nb); cudaFree(ctx->scat_gw); cudaFree(ctx->norm_scratch);
-    TiledLayout &tl = ctx->tl;
-    cudaFree(tl.tile_seg_ptr); cudaFree(tl.seg_ptr); cudaFree(tl.seg_slot); cudaFree(tl.seg_meta); cudaFree(tl.seg_csum);
-    cudaFree(tl.tile_desc); cudaFree(tl.tile_order); cudaFree(tl.blob); cudaFree(tl.blob_desc);
-    cudaFree(tl.tcoef); cudaFree(tl.tidx); cudaFree(tl.bin_slot_ptr);
-    free(tl.h_first_desc);
-    free(ctx->stream_first);
-    ai_free_fl(ctx->fl);
-    cudaFree(ctx->partials); cudaFree(ctx->staging); cudaFree(ctx->out_dev); cudaFree(ctx->grid_sync); cudaFree(ctx->chain_done); cudaFree(ctx->stream_partials); cudaFree(ctx->axes2d); cudaFree(ctx->corrected[0]); cudaFree(ctx->corrected[1]);
+    release_matrix_and_scratch(ctx);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;

@@ -47,7 +47,9 @@ def test_full_splitting_matrix_and_profiles(torch, B, oracle, workloads, parity_
     assert u0 == pytest.approx(o0, rel=1e-15, abs=1e-300) and u1 == pytest.approx(o1, rel=4e-16)
     # a corner exactly on a bin edge gives a zero-area slice on one side and none on the other: counted as ties
     rep = compare_csr((gi, gx, gd), (oi, ox, od), cfg.npix, max_ties=4 * (cfg.height + cfg.width))
-    bbox_nnz = int(B.ai_get_csr(B.Integrator(cfg).ctx)[3])
+    bbox = B.Integrator(cfg)                               # (kept alive while its context is read)
+    bbox_nnz = int(B.ai_get_csr(bbox.ctx)[3])
+    bbox.close()
     rep["nnz_bounding_box"] = bbox_nnz
     print(name, rep)
     assert rep["nnz_gpu"] <= bbox_nnz                      # the quadrilateral lies inside its bounding box
