@@ -169,3 +169,24 @@ def test_fl_frame_stride_and_the_other_kernels_agree(torch, B, oracle, workloads
             got = {"intensity": out[name][0][f], "sum_signal": out[name][1][f], "count": out[name][2][f]}
             assert_profile(got, want, what=f"{name} frame {f}")
     assert np.allclose(out["fl"][1], out["slices"][1], rtol=1e-6, atol=0)
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg5"])
+def test_fl_full_size_geometries_sampled(torch, B, oracle, workloads, name):
+    """The frame-lane kernel on the two large q-unit matrices at full size (BASELINE.json configs[2] and configs[4]
+    geometries: 3000 / 5000 bins, 3.5 / 2.3 entries per pixel, the latter with the beam centre off the image), taken by
+    itself (no environment switch) on 96 plain float frames from a pool of two; sampled frames against the oracle."""
+    cfg = workloads.CONFIGS[name]
+    base = workloads.make_frame(cfg).image
+    pool = np.stack([base, base[::-1].copy() * np.float32(0.5)])
+    dev = torch.from_numpy(pool).cuda()
+    frames = dev.repeat(48, 1, 1)
+    integ = B.Integrator(cfg)
+    i, s, c = integ.integrate1d_batch(frames)
+    torch.cuda.synchronize()
+    assert B.ai_get_batch_layout_info(integ.ctx)["built"] == 1, "the frame-lane kernel did not take the batch"
+    for f in (0, 95):
+        want = _want(oracle, cfg, pool[f % 2])
+        assert_profile(_row(i, s, c, f), want, what=f"{name} frame {f}")
+    assert torch.equal(i[0], i[94]) and torch.equal(s[1], s[95]) and torch.equal(c[0], c[64])
+    integ.close()
