@@ -141,6 +141,8 @@ struct FlLayout {
     int *bin_slot_ptr = nullptr;    // [npt+1] H5: partial slots of bin b are bin_slots[bin_slot_ptr[b] .. bin_slot_ptr[b+1])
     int *bin_slots = nullptr;       //         ascending chunk
     double *bin_csum = nullptr;     // [npt] sum of the row's coefficients (count when every pixel is valid)
+    double *call_csum = nullptr;    // [npt] corrected batches: the same without the pixels invalid for every frame, per call
+    uint8_t *gone = nullptr;        // [npix] corrected batches: 1 = the pixel is invalid for every frame of the call
     void *partials = nullptr;       // [nslot][frames rounded up to 64] float2 (sum, compensation), then, for float
                                     // frames, [npt][frames rounded up] uint64: weight of the invalid pixels, 2^-40 units
     size_t partials_bytes = 0;

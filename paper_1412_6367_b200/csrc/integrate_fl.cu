@@ -36,6 +36,8 @@ constexpr int kFlImgBytes = 32 * kFlLaneBytes;
 constexpr int kFlPassRows = 4;                       // rows of the tile a loader holds in registers at a time
 constexpr int kFlPrefetchAhead = 3;                  // tiles between the L2 prefetch and the loads
 constexpr int kFlMinFrames = 96;
+constexpr int kFlCorBytes = 4 * kFlTilePix * 4 + kFlTilePix;     // corrected variant, per stage: dark, flat, solid angle,
+                                                                 // polarisation (float) and mask (bytes) of the tile
 constexpr float kFlFix = 1099511627776.0f;           // 2^40: weights of invalid pixels as integers
 
 struct FlParams {
@@ -47,8 +49,9 @@ struct FlParams {
     int height, width;
     int nframes, ngroups, nitems;
     int stages, stage_bytes, prefetch_ahead;
+    Corrections cor;                                 // corrected variant: per-pixel arrays shared by all frames
     float2 *part_s;
-    unsigned long long *part_d;                      // float frames only
+    unsigned long long *part_d;                      // float frames and corrected batches only
     int64_t nfp;                                     // frames rounded up to a multiple of kFlFrames
 };
 
@@ -96,26 +99,9 @@ __device__ __forceinline__ void sts_f2(unsigned addr, float a, float b)
 {
     asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
 }
-// Waits of the frame-lane kernel: try_wait with a long suspend-time hint -- the warp sleeps in the barrier unit until
-// the phase completes instead of polling, so waiting warps leave the issue slots to the warps that work.  Bounded
-// (20 s of wall time) like mbar_wait.
-__device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity)
-{
-    unsigned long long t0 = 0;
-    for (uint32_t spin = 1;; ++spin) {
-        uint32_t ok;
-        asm volatile("{\n\t.reg .pred p;\n\t"
-                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
-                     "selp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity), "r"(100000u) : "memory");
-        if (ok) return;
-        if ((spin & 0xffu) == 0) {
-            const unsigned long long now = globaltimer_ns();
-            if (t0 == 0) t0 = now;
-            else if (now - t0 > 20000000000ULL) __trap();
-        }
-    }
-}
+// Waits of the frame-lane kernel: bounded (20 s of wall time) like mbar_wait.  (A try_wait with a long suspend-time hint
+// was measured to oversleep by microseconds once the waiting side is the faster one: plain try_wait.)
+__device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity) { mbar_wait(bar, parity); }
 
 // One Kahan step for the two frames of a lane, the compensation carried as e = -(running error):
 // the carried value is s + e.  c2 = the coefficient in both halves.
@@ -161,10 +147,14 @@ __device__ __forceinline__ float fl_cast(unsigned v)
     else return (float)v;
 }
 
-template <int DT>
+// COR: the batch carries correction arrays and / or a mask (one set for all frames).  The loaders apply them
+// as they stage a tile (H2): a pixel that is invalid for every frame -- masked, or with a zero / non-finite denominator --
+// is stored as 0 and its weight is taken off the bins' counts once per call (fl_static_count_kernel); a pixel whose
+// corrected value is not finite is stored as NaN and handled per frame like a non-finite pixel of a float frame.
+template <int DT, bool COR>
 __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_constant__ CUtensorMap tmap, const FlParams p)
 {
-    constexpr bool TRACK = DT == AI_F32;
+    constexpr bool TRACK = DT == AI_F32 || COR;
     // [accumulators][barriers, flags][stages: tile of 64 frames, blob]
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *bar = smem + kFlWindow * 32 * 16;
@@ -216,8 +206,9 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
         // 128-bit loads of rows 4 h .. 4 h + 3 of a tile for the lane's two frames; `src` = the lane's piece of row 0
         struct Src {
             const unsigned char *p;
+            int64_t pix;                 // index of the lane's first pixel of row 0 (corrections)
             int rows;                    // rows of the tile inside the image
-            bool in_a, in_b;
+            bool in_a, in_b, in_x;
         };
         auto locate = [&](const FlWalk &w, int4 &d) {
             d = __ldg(p.tile_desc + w.r);
@@ -225,9 +216,11 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
             const int fa = w.group * kFlFrames + 2 * cl;
             Src s;
             s.p = p.frames + (int64_t)fa * p.frame_stride_bytes + ((int64_t)y0 * p.width + x) * 4;
+            s.pix = (int64_t)y0 * p.width + x;
             s.rows = p.height - y0;
-            s.in_a = fa < p.nframes && x < p.width;
-            s.in_b = fa + 1 < p.nframes && x < p.width;
+            s.in_x = x < p.width;
+            s.in_a = fa < p.nframes && s.in_x;
+            s.in_b = fa + 1 < p.nframes && s.in_x;
             return s;
         };
         auto issue = [&](const Src &s, int h, uint4 (&a)[kFlPassRows], uint4 (&b)[kFlPassRows]) {
@@ -240,13 +233,83 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
                 if (s.in_b && row < s.rows) b[u] = __ldcs(reinterpret_cast<const uint4 *>(q + p.frame_stride_bytes));
             }
         };
+        // corrected variant: the tile's correction values travel like the frames -- loaded into registers one tile ahead,
+        // one 16-byte chunk per loader thread (4 arrays x 64 chunks) and the mask's 16 chunks by the first 16 threads,
+        // stored into the stage when it is free; absent arrays and chunks outside the image read as 0 (dark, mask) / 1
+        const bool has_den = COR && (p.cor.flat || p.cor.solidangle || p.cor.polarization);
+        uint4 cq = make_uint4(0, 0, 0, 0), mq = cq;
+        auto issue_cor = [&](const FlWalk &w) {
+            if constexpr (COR) {
+                const int4 dd = __ldg(p.tile_desc + w.r);
+                const int x0 = (dd.z & 0xffff) * kFlTileW, y0 = (dd.z >> 16) * kFlTileH;
+                const int arr = tid >> 6, k = tid & 63, y = y0 + (k >> 3), x = x0 + (k & 7) * 4;
+                const float *src = arr == 0 ? p.cor.dark : arr == 1 ? p.cor.flat : arr == 2 ? p.cor.solidangle : p.cor.polarization;
+                const unsigned dflt = arr == 0 ? 0u : 0x3f800000u;
+                cq = make_uint4(dflt, dflt, dflt, dflt);
+                if (src && y < p.height && x < p.width) cq = __ldg(reinterpret_cast<const uint4 *>(src + (int64_t)y * p.width + x));
+                mq = make_uint4(0, 0, 0, 0);
+                if (tid < 16 && p.cor.mask) {
+                    // 16 mask bytes = 4 chunks of 4 pixels: half a tile row
+                    const int my = y0 + (tid >> 1), mx = x0 + (tid & 1) * 16;
+                    if (my < p.height && mx < p.width) {
+                        const uint8_t *mp = p.cor.mask + (int64_t)my * p.width + mx;
+                        if (mx + 16 <= p.width) {
+                            const uint32_t *m32 = reinterpret_cast<const uint32_t *>(mp);
+                            mq = make_uint4(__ldg(m32), __ldg(m32 + 1), __ldg(m32 + 2), __ldg(m32 + 3));
+                        } else {
+                            unsigned v[4] = {0, 0, 0, 0};
+                            for (int j = 0; mx + j < p.width; j += 4) v[j >> 2] = __ldg(reinterpret_cast<const uint32_t *>(mp + j));
+                            mq = make_uint4(v[0], v[1], v[2], v[3]);
+                        }
+                    }
+                }
+            }
+        };
+        auto store_cor = [&](unsigned cor_s) {
+            if constexpr (COR) {
+                sts_v4(cor_s + (unsigned)tid * 16, cq);
+                if (tid < 16) sts_v4(cor_s + 4 * kFlTilePix * 4 + (unsigned)tid * 16, mq);
+                asm volatile("bar.sync 2, %0;" ::"n"(32 * kFlLoad) : "memory");
+                // one pixel per loader thread: the scale, over the flat values (the other two factors are not read again)
+                static_assert(32 * kFlLoad == kFlTilePix, "one pixel of the tile per loader thread");
+                float fl_v, sa_v, po_v;
+                unsigned mbyte;
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(fl_v) : "r"(cor_s + (unsigned)(kFlTilePix + tid) * 4));
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(sa_v) : "r"(cor_s + (unsigned)(2 * kFlTilePix + tid) * 4));
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(po_v) : "r"(cor_s + (unsigned)(3 * kFlTilePix + tid) * 4));
+                asm volatile("ld.shared.u8 %0, [%1];" : "=r"(mbyte) : "r"(cor_s + (unsigned)(4 * kFlTilePix * 4 + tid)));
+                const float den = fl_v * sa_v * po_v;
+                const bool gone = mbyte != 0 || (has_den && (den == 0.f || !finite_f(den)));
+                const float scale = gone ? 0.f : (has_den ? __frcp_rn(den) : 1.0f);
+                asm volatile("st.shared.f32 [%0], %1;" ::"r"(cor_s + (unsigned)(kFlTilePix + tid) * 4), "f"(scale) : "memory");
+                asm volatile("bar.sync 2, %0;" ::"n"(32 * kFlLoad) : "memory");      // every loader reads what the others staged
+            }
+        };
         bool bad = false;
-        auto store = [&](unsigned dst, int h, const uint4 (&a)[kFlPassRows], const uint4 (&b)[kFlPassRows]) {
+        // corrected value of one pixel of one frame: (raw - dark) * scale, scale = the rounded reciprocal of flat * solid
+        // angle * polarisation (one rounding more than the division of the single-frame path: 6e-8 relative), or 0 for a
+        // pixel that is invalid for every frame (stored as 0, its weight leaves the counts once per call); otherwise a
+        // non-finite result becomes NaN (this frame only)
+        auto corr = [&](float raw, float dk, float scale) {
+            const float v = __fmul_rn(__fsub_rn(raw, dk), scale);
+            return scale == 0.f ? 0.f : (finite_f(v) ? v : quiet_nan());
+        };
+        auto store = [&](unsigned dst, int h, const uint4 (&a)[kFlPassRows], const uint4 (&b)[kFlPassRows], unsigned cor_s) {
 #pragma unroll
             for (int u = 0; u < kFlPassRows; ++u) {
                 const unsigned o = dst + (unsigned)((h * kFlPassRows + u) * kFlTileW * 8);
-                const float a0 = fl_cast<DT>(a[u].x), a1 = fl_cast<DT>(a[u].y), a2 = fl_cast<DT>(a[u].z), a3 = fl_cast<DT>(a[u].w);
-                const float b0 = fl_cast<DT>(b[u].x), b1 = fl_cast<DT>(b[u].y), b2 = fl_cast<DT>(b[u].z), b3 = fl_cast<DT>(b[u].w);
+                float a0 = fl_cast<DT>(a[u].x), a1 = fl_cast<DT>(a[u].y), a2 = fl_cast<DT>(a[u].z), a3 = fl_cast<DT>(a[u].w);
+                float b0 = fl_cast<DT>(b[u].x), b1 = fl_cast<DT>(b[u].y), b2 = fl_cast<DT>(b[u].z), b3 = fl_cast<DT>(b[u].w);
+                if constexpr (COR) {
+                    // the tile's dark current and scale (1 / denominator, 0 for a pixel that is invalid for every frame),
+                    // staged by the loaders themselves (below): the lane's four pixels of the row
+                    const unsigned q = cor_s + (unsigned)((h * kFlPassRows + u) * kFlTileW + piece * 4) * 4;
+                    const uint4 dku = lds_v4(q), scu = lds_v4(q + kFlTilePix * 4);
+                    a0 = corr(a0, __uint_as_float(dku.x), __uint_as_float(scu.x)); b0 = corr(b0, __uint_as_float(dku.x), __uint_as_float(scu.x));
+                    a1 = corr(a1, __uint_as_float(dku.y), __uint_as_float(scu.y)); b1 = corr(b1, __uint_as_float(dku.y), __uint_as_float(scu.y));
+                    a2 = corr(a2, __uint_as_float(dku.z), __uint_as_float(scu.z)); b2 = corr(b2, __uint_as_float(dku.z), __uint_as_float(scu.z));
+                    a3 = corr(a3, __uint_as_float(dku.w), __uint_as_float(scu.w)); b3 = corr(b3, __uint_as_float(dku.w), __uint_as_float(scu.w));
+                }
                 if constexpr (TRACK)
                     bad = bad || !finite_f(a0) || !finite_f(a1) || !finite_f(a2) || !finite_f(a3) || !finite_f(b0) ||
                           !finite_f(b1) || !finite_f(b2) || !finite_f(b3);
@@ -266,6 +329,7 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
             const Src s = locate(cur, d);
             issue(s, 0, a0, b0);
             issue(s, 1, a1, b1);
+            issue_cor(cur);
         }
         while (!cur.done) {
             FlWalk nxt = cur;
@@ -284,9 +348,12 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
             }
             const unsigned dst = smem_u32(stage) + dst_lane;
             bad = false;
-            store(dst, 0, a0, b0);
+            const unsigned cor_s = smem_u32(stage) + (unsigned)(p.stage_bytes - kFlCorBytes);
+            store_cor(cor_s);
+            if (!nxt.done) issue_cor(nxt);            // (its registers are free again: a whole tile of time to arrive)
+            store(dst, 0, a0, b0, cor_s);
             if (!nxt.done) issue(sn, 0, a0, b0);
-            store(dst, 1, a1, b1);
+            store(dst, 1, a1, b1, cor_s);
             if (!nxt.done) issue(sn, 1, a1, b1);
             if constexpr (TRACK) {
                 const bool any = __any_sync(AI_FULL_MASK, bad);
@@ -409,6 +476,42 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
     }
 }
 
+// Corrected batches: the count every frame of the call starts from -- the sum of a row's coefficients over the pixels that
+// are not invalid for every frame (masked, zero / non-finite denominator: the same test as the loaders').  First a byte
+// per pixel, then one block per row (fp64, fixed order; a row with nothing but such pixels gives exactly 0).
+__global__ void __launch_bounds__(256) fl_gone_kernel(int64_t npix, Corrections cor, uint8_t *__restrict__ gone)
+{
+    const bool has_den = cor.flat || cor.solidangle || cor.polarization;
+    for (int64_t px = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; px < npix; px += (int64_t)gridDim.x * blockDim.x) {
+        bool g = cor.mask && __ldg(cor.mask + px) != 0;
+        if (has_den) {
+            float den = cor.flat ? __ldg(cor.flat + px) : 1.0f;
+            den *= cor.solidangle ? __ldg(cor.solidangle + px) : 1.0f;
+            den *= cor.polarization ? __ldg(cor.polarization + px) : 1.0f;
+            g = g || den == 0.f || !finite_f(den);
+        }
+        gone[px] = g ? 1 : 0;
+    }
+}
+
+__global__ void __launch_bounds__(128) fl_static_count_kernel(int npt, const int *__restrict__ indptr,
+                                                              const int *__restrict__ indices,
+                                                              const float *__restrict__ data,
+                                                              const uint8_t *__restrict__ gone,
+                                                              double *__restrict__ call_csum)
+{
+    __shared__ double part[4];
+    const int b = blockIdx.x, lane = threadIdx.x & 31;
+    double a = 0.0;
+    for (int e = __ldg(indptr + b) + threadIdx.x, end = __ldg(indptr + b + 1); e < end; e += 128)
+        a += __ldg(gone + __ldg(indices + e)) ? 0.0 : (double)__ldg(data + e);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    if (lane == 0) part[threadIdx.x >> 5] = a;
+    __syncthreads();
+    if (threadIdx.x == 0) call_csum[b] = (part[0] + part[1]) + (part[2] + part[3]);
+}
+
 // H5: block = 32 bins x 32 frames; lane = frame while the partials are added (coalesced over frames), lane = bin when
 // the outputs are written ([frame][bin] rows)
 template <bool TRACK>
@@ -456,16 +559,16 @@ __global__ void __launch_bounds__(256) fl_finish_kernel(const int *__restrict__ 
     }
 }
 
-template <int DT>
+template <int DT, bool COR>
 int launch_fl(ai_ctx *ctx, const CUtensorMap &map, const FlParams &p, size_t smem, int grid, cudaStream_t st)
 {
-    const uint64_t bit = 1ULL << (40 + DT);
+    const uint64_t bit = 1ULL << (50 + DT + (COR ? 5 : 0));     // (bits 0..44: the other kernels' instantiations)
     if (!(ctx->smem_opt_in & bit)) {
-        AI_CUDA(ctx, cudaFuncSetAttribute(fl_batch_kernel<DT>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPipeSmemBudget));
+        AI_CUDA(ctx, cudaFuncSetAttribute(fl_batch_kernel<DT, COR>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPipeSmemBudget));
         ctx->smem_opt_in |= bit;
     }
     ai_prof_begin(ctx, st);
-    fl_batch_kernel<DT><<<grid, kFlThreads, smem, st>>>(map, p);
+    fl_batch_kernel<DT, COR><<<grid, kFlThreads, smem, st>>>(map, p);
     ai_prof_end(ctx, st);
     AI_CUDA(ctx, cudaGetLastError());
     return AI_OK;
@@ -485,10 +588,13 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
     // Where it pays (measured): batches of two groups of frames or more on matrices with more than
     // ~2.2 entries per pixel -- below that the per-pixel cost of staging the frames outweighs the cheaper entries and
     // the slice-per-lane kernel is as fast.  AZINT_FORCE_FL=1 takes every batch (testing).
-    if (!ctx->force_fl && (a.nframes < kFlMinFrames || (double)ctx->nnz < 2.2 * (double)ctx->height * ctx->width)) return AI_OK;
     const bool plain = !a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask;
+    // (batches with correction arrays: whatever the matrix -- the alternative is the general pipelined kernel)
+    if (!ctx->force_fl && (a.nframes < kFlMinFrames || (plain && (double)ctx->nnz < 2.2 * (double)ctx->height * ctx->width)))
+        return AI_OK;
     const bool is32 = a.dtype == AI_F32 || a.dtype == AI_I32 || a.dtype == AI_U32;
-    if (!plain || !is32 || !vec_ok || (reinterpret_cast<uintptr_t>(a.image) % 16) != 0) return AI_OK;
+    // (vec_ok: every array, the correction arrays and the mask included, on its 4-pixel vector boundary)
+    if (!is32 || !vec_ok || (reinterpret_cast<uintptr_t>(a.image) % 16) != 0) return AI_OK;
     if (a.row_pitch != 0 && a.row_pitch != ctx->width) return AI_OK;
     FlLayout &fl = ctx->fl;
     if (!fl.tried) {
@@ -496,11 +602,11 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
         if (rc != AI_OK) return rc;
     }
     if (!fl.ok) return AI_OK;
-    const bool track = a.dtype == AI_F32;
+    const bool track = a.dtype == AI_F32 || !plain;
     const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
 
     FlParams p{};
-    p.stage_bytes = kFlImgBytes + ai_align_up(fl.max_blob_bytes, 16);
+    p.stage_bytes = kFlImgBytes + ai_align_up(fl.max_blob_bytes, 16) + (plain ? 0 : ai_align_up(kFlCorBytes, 16));
     const int acc_bytes = kFlWindow * 32 * 16;
     int stages = (kPipeSmemBudget - acc_bytes - kFlBarBytes) / p.stage_bytes;
     if (stages > kFlMaxStages) stages = kFlMaxStages;
@@ -531,6 +637,7 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
     p.chunk_desc = fl.chunk_desc;
     p.chunk_owner = fl.chunk_owner;
     p.blob = fl.blob;
+    p.cor = Corrections{a.dark, a.flat, a.solidangle, a.polarization, a.mask};
     p.frames = static_cast<const unsigned char *>(a.image);
     p.frame_stride_bytes = a.frame_stride * 4;
     p.height = ctx->height;
@@ -541,25 +648,38 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
     CUtensorMap map{};
     int rc = ai_make_frame_map(ctx, a, kFlTileH, &map, kFlFrames);      // boxes of 64 frames: the L2 prefetch of a tile
     if (rc != AI_OK) return rc;
+    // corrected batches: the count all frames share, without the pixels that are invalid for every frame
+    const double *csum = fl.bin_csum;
+    int launches = 0;
+    if (!plain) {
+        const int64_t npix = (int64_t)ctx->height * ctx->width;
+        if (!fl.call_csum) AI_CUDA(ctx, cudaMalloc(&fl.call_csum, (size_t)ctx->npt * sizeof(double)));
+        if (!fl.gone) AI_CUDA(ctx, cudaMalloc(&fl.gone, (size_t)npix));
+        fl_gone_kernel<<<sms * 8, 256, 0, st>>>(npix, p.cor, fl.gone);
+        fl_static_count_kernel<<<ctx->npt, 128, 0, st>>>(ctx->npt, ctx->indptr, ctx->indices, ctx->data, fl.gone, fl.call_csum);
+        AI_CUDA(ctx, cudaGetLastError());
+        csum = fl.call_csum;
+        launches = 2;
+    }
     rc = AI_EINVAL;
     switch (a.dtype) {
-    case AI_F32: rc = launch_fl<AI_F32>(ctx, map, p, smem, grid, st); break;
-    case AI_I32: rc = launch_fl<AI_I32>(ctx, map, p, smem, grid, st); break;
-    case AI_U32: rc = launch_fl<AI_U32>(ctx, map, p, smem, grid, st); break;
+    case AI_F32: rc = plain ? launch_fl<AI_F32, false>(ctx, map, p, smem, grid, st) : launch_fl<AI_F32, true>(ctx, map, p, smem, grid, st); break;
+    case AI_I32: rc = plain ? launch_fl<AI_I32, false>(ctx, map, p, smem, grid, st) : launch_fl<AI_I32, true>(ctx, map, p, smem, grid, st); break;
+    case AI_U32: rc = plain ? launch_fl<AI_U32, false>(ctx, map, p, smem, grid, st) : launch_fl<AI_U32, true>(ctx, map, p, smem, grid, st); break;
     default: break;
     }
     if (rc != AI_OK) return rc;
     *handled = true;
-    ctx->last_launches = 1;
+    ctx->last_launches = launches + 1;
     if (ctx->stage1_only) return AI_OK;
     const dim3 g2((ctx->npt + 31) / 32, (a.nframes + 31) / 32);
     if (track)
-        fl_finish_kernel<true><<<g2, 256, 0, st>>>(fl.bin_slot_ptr, fl.bin_slots, fl.bin_csum, ctx->npt, a.nframes, p.nfp,
+        fl_finish_kernel<true><<<g2, 256, 0, st>>>(fl.bin_slot_ptr, fl.bin_slots, csum, ctx->npt, a.nframes, p.nfp,
                                                    p.part_s, p.part_d, ctx->empty_value, a.intensity, a.sum_signal, a.count);
     else
         fl_finish_kernel<false><<<g2, 256, 0, st>>>(fl.bin_slot_ptr, fl.bin_slots, fl.bin_csum, ctx->npt, a.nframes, p.nfp,
                                                     p.part_s, p.part_d, ctx->empty_value, a.intensity, a.sum_signal, a.count);
     AI_CUDA(ctx, cudaGetLastError());
-    ctx->last_launches = 2;
+    ctx->last_launches = launches + 2;
     return AI_OK;
 }

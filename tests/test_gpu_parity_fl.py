@@ -190,3 +190,46 @@ def test_fl_full_size_geometries_sampled(torch, B, oracle, workloads, name):
         assert_profile(_row(i, s, c, f), want, what=f"{name} frame {f}")
     assert torch.equal(i[0], i[94]) and torch.equal(s[1], s[95]) and torch.equal(c[0], c[64])
     integ.close()
+
+
+@pytest.mark.parametrize("dtype,nframes,tune", [("int32", 7, None), ("float32", 100, "flc:2"), ("uint32", 66, None)])
+def test_fl_corrected_batches(torch, B, oracle, workloads, monkeypatch, dtype, nframes, tune):
+    """Batches with every correction array and a mask (one set for all frames) through the frame-lane
+    kernel: the loaders correct the tiles as they stage them.  Pixels invalid for every frame (masked, flat = 0, a whole
+    masked band that empties bins) leave the counts once per call; non-finite raw pixels per frame."""
+    monkeypatch.setenv("AZINT_FORCE_FL", "1")
+    if tune:
+        monkeypatch.setenv("AZINT_TUNE", tune)
+    cfg = workloads.tiny_config(200, 264, unit=workloads.TTH_DEG, name="fl_corr", **SMALL)
+    rng = np.random.default_rng(17 + nframes)
+    shape = (cfg.height, cfg.width)
+    frames = rng.poisson(80.0, size=(nframes,) + shape).astype(dtype)
+    dark = rng.poisson(5.0, shape).astype(np.float32)
+    flat = rng.uniform(0.9, 1.1, shape).astype(np.float32)
+    solid = rng.uniform(0.7, 1.0, shape).astype(np.float32)
+    pol = rng.uniform(0.95, 1.0, shape).astype(np.float32)
+    mask = (rng.random(shape) < 0.04).astype(np.uint8)
+    mask[80:100, 90:112] = 1                      # around the beam centre: the innermost bins lose every pixel
+    flat[10, 10] = 0.0
+    flat[150, 200] = np.inf
+    if dtype == "float32":
+        frames[2, 33, 44] = np.nan
+        frames[nframes - 1, 120, 7] = np.inf
+    integ = B.Integrator(cfg)
+    n = frames.shape[0]
+    if dtype == "uint32":
+        t, code = torch.from_numpy(frames.view(np.int32)).cuda(), B.AI_U32
+    else:
+        t, code = torch.from_numpy(frames).cuda(), None
+    cor = [torch.from_numpy(x).cuda() for x in (dark, flat, solid, pol, mask)]
+    i, s, c = integ.outputs(n)
+    B.ai_integrate1d_batch(integ.ctx, t, n, cfg.npix, *cor, i, s, c, dtype=code)
+    torch.cuda.synchronize()
+    assert B.ai_last_launch_count(integ.ctx) == 4 and B.ai_get_batch_layout_info(integ.ctx)["built"] == 1
+    umin, umax = oracle.pixel_bounds(cfg)
+    u0, u1 = oracle.auto_range(umin, umax)
+    for f in sorted({0, 2, n // 2, n - 1}):
+        want = oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, frames[f], dark, flat, solid, pol, mask)
+        assert (want["count"] <= 0).sum() >= 3
+        assert_profile(_row(i, s, c, f), want, what=f"corrected fl/{dtype}/frame {f} of {n}")
+    integ.close()
