@@ -189,6 +189,36 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
                                         "partial_records_written_and_read_back": 2 * 16 * info4["nslot"] * c4.nframes,
                                         "max_rel_diff_of_the_two_kernels_profiles": dmax},
                                     "note": "4.3 GB of frames > L2; 8 distinct frames repeated"}
+    # configs[2] as a stream: 256 frames with every correction array and the mask in ONE batched call (PAPER.md:240-254:
+    # the corrections are per-detector constants, only the image changes from frame to frame)
+    c3 = W.CONFIGS["cfg3"]
+    fr3 = W.make_frame(c3)
+    b3 = torch.from_numpy(fr3.image).to(device)
+    fb3 = torch.stack([b3, b3 * 0.5]).repeat(128, 1, 1)
+    cor3 = tuple(None if a is None else torch.from_numpy(a).to(device)
+                 for a in (fr3.dark, fr3.flat, fr3.solidangle, fr3.polarization, fr3.mask))
+    it = B.Integrator(c3, device=device)
+    out3 = it.outputs(256)
+    for _ in range(2):
+        it.integrate1d_batch(fb3, *cor3, out=out3)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(3):
+        it.integrate1d_batch(fb3, *cor3, out=out3)
+    e1.record()
+    torch.cuda.synchronize()
+    ms3 = e0.elapsed_time(e1) / 3
+    ab3 = 256 * c3.npix * 4 + 17 * c3.npix + B.ai_get_csr(it.ctx)[3] * 8 + (c3.npt + 1) * 4 + 256 * 3 * c3.npt * 4
+    ex["batch_cfg3_256_frames_all_corrections"] = {
+        "frames_per_s": 256 / (ms3 * 1e-3), "ms_per_batch": ms3, "us_per_frame": ms3 * 1e3 / 256,
+        "launches_per_call": B.ai_last_launch_count(it.ctx), "algorithmic_bytes": ab3,
+        "frac_of_peak": ab3 / (ms3 * 1e-3) / 1e9 / peak_gbs,
+        "kernel": "fl_batch_kernel, corrected variant (the loaders apply dark / flat / solid angle / polarisation / mask as "
+                  "they stage a tile)",
+        "note": "the same frames one by one (extras.train_cfg3_tiled_kahan) take 45 us each"}
+    it.close()
+    del fb3, out3, cor3
     # bidimensional integration of the headline frame: 360 azimuthal x 500 radial bins
     ck = W.CONFIGS["cake2"]
     its = [B.Integrator(ck, device=device) for _ in range(3)]

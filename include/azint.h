@@ -178,10 +178,12 @@ int ai_integrate2d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *
  *   frames                     frame f starts at element f * frame_stride_elems (>= height*width)
  *   intensity, sum_signal,
  *   count                      float32[nframes][npt], row-major
- * Enqueues on `cuda_stream`; does not synchronise -- with one exception: the first batch of 96 or more plain 32-bit
- * frames on a 1D context whose matrix has more than ~2.2 entries per pixel builds the frame-lane layout of the matrix
- * (one-time, synchronises `cuda_stream`; see ai_get_batch_layout_info), and a larger batch than any
- * before re-allocates scratch (cudaFree synchronises the device).  A frame's profiles do not depend on where it sits in
+ * Enqueues on `cuda_stream`; does not synchronise -- with one exception: the first batch of 96 or more 32-bit frames
+ * that the frame-lane kernel takes (1D context, Kahan accumulation, every array on a 16-byte boundary,
+ * and either correction arrays / a mask or a matrix with more than ~2.2 entries per pixel) builds the frame-lane layout
+ * of the matrix (one-time, synchronises `cuda_stream`; see ai_get_batch_layout_info), and a larger batch than any before
+ * re-allocates scratch (cudaFree synchronises the device).  In that kernel a corrected value is (I - dark) times the
+ * rounded reciprocal of flat * solidangle * polarization (one rounding more than the division of the other paths).  A frame's profiles do not depend on where it sits in
  * a batch, but they are not bit-identical between the kernels a batch may take (different fixed summation orders).
  * Errors as ai_integrate1d. */
 int ai_integrate1d_batch(ai_ctx *ctx, const void *frames, ai_dtype dtype, int nframes, int64_t frame_stride_elems,
