@@ -145,7 +145,7 @@ int upload(ai_ctx *ctx, T **dev, const std::vector<T> &h, cudaStream_t st)
 void ai_free_fl(FlLayout &fl)
 {
     cudaFree(fl.tile_desc); cudaFree(fl.chunk_desc); cudaFree(fl.chunk_owner); cudaFree(fl.blob);
-    cudaFree(fl.bin_slot_ptr); cudaFree(fl.bin_slots); cudaFree(fl.bin_csum); cudaFree(fl.call_csum); cudaFree(fl.gone); cudaFree(fl.partials);
+    cudaFree(fl.bin_slot_ptr); cudaFree(fl.bin_slots); cudaFree(fl.bin_csum); cudaFree(fl.call_csum); cudaFree(fl.gone); cudaFree(fl.scale); cudaFree(fl.blob_call); cudaFree(fl.partials);
     fl = FlLayout{};
 }
 

@@ -143,6 +143,9 @@ struct FlLayout {
     double *bin_csum = nullptr;     // [npt] sum of the row's coefficients (count when every pixel is valid)
     double *call_csum = nullptr;    // [npt] corrected batches: the same without the pixels invalid for every frame, per call
     uint8_t *gone = nullptr;        // [npix] corrected batches: 1 = the pixel is invalid for every frame of the call
+    float *scale = nullptr;         // [3][npix] corrected batches, per call: 1 / (flat x solid angle x polarisation) (0 where
+                                    // gone), dark current (0 where gone), keep word (0 where gone, else all ones)
+    unsigned char *blob_call = nullptr;   // corrected batches: blob with the coefficients times scale, rewritten per call
     void *partials = nullptr;       // [nslot][frames rounded up to 64] float2 (sum, compensation), then, for float
                                     // frames, [npt][frames rounded up] uint64: weight of the invalid pixels, 2^-40 units
     size_t partials_bytes = 0;

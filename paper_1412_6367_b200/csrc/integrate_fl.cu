@@ -36,20 +36,22 @@ constexpr int kFlImgBytes = 32 * kFlLaneBytes;
 constexpr int kFlPassRows = 4;                       // rows of the tile a loader holds in registers at a time
 constexpr int kFlPrefetchAhead = 3;                  // tiles between the L2 prefetch and the loads
 constexpr int kFlMinFrames = 96;
-constexpr int kFlCorBytes = 4 * kFlTilePix * 4 + kFlTilePix;     // corrected variant, per stage: dark, flat, solid angle,
-                                                                 // polarisation (float) and mask (bytes) of the tile
+constexpr int kFlCorBytes = 2 * kFlTilePix * 4;                  // corrected variant, per stage: the tile's dark current
+                                                                 // (float) and keep words (float frames)
 constexpr float kFlFix = 1099511627776.0f;           // 2^40: weights of invalid pixels as integers
 
 struct FlParams {
     const int4 *tile_desc, *chunk_desc;
     const uint8_t *chunk_owner;
-    const unsigned char *blob;
+    const unsigned char *blob;                       // (corrected variant: the copy with the coefficients scaled for this call)
+    const unsigned char *blob_orig;                  // the layout's own blobs
     const unsigned char *frames;
     int64_t frame_stride_bytes;
     int height, width;
     int nframes, ngroups, nitems;
     int stages, stage_bytes, prefetch_ahead;
-    Corrections cor;                                 // corrected variant: per-pixel arrays shared by all frames
+    const float *dark;                               // corrected variant: the call's dark current and keep words, per pixel
+    const uint32_t *keep;                            // (fl_prep_kernel)
     float2 *part_s;
     unsigned long long *part_d;                      // float frames and corrected batches only
     int64_t nfp;                                     // frames rounded up to a multiple of kFlFrames
@@ -99,9 +101,29 @@ __device__ __forceinline__ void sts_f2(unsigned addr, float a, float b)
 {
     asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
 }
-// Waits of the frame-lane kernel: bounded (20 s of wall time) like mbar_wait.  (A try_wait with a long suspend-time hint
-// was measured to oversleep by microseconds once the waiting side is the faster one: plain try_wait.)
-__device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity) { mbar_wait(bar, parity); }
+// Waits of the frame-lane kernel: bounded (20 s of wall time) like mbar_wait.  EXIT (the corrected variant): a timed-out
+// wait raises its error with a store to address 0 followed by exit instead of trap: with a trap instruction in a branch, ptxas keeps that
+// branch at the launch-time register count and ignores its setmaxnreg (measured: the loaders spilled their in-flight
+// loads to local memory at 80 registers and stalled on them every tile; without the trap they use up to 108, no spills).
+// (A try_wait with a long suspend-time hint was measured to oversleep by microseconds once the waiting side is the
+// faster one: plain try_wait.)
+template <bool EXIT>
+__device__ __forceinline__ void mbar_wait_fl(uint64_t *bar, uint32_t parity)
+{
+    if constexpr (!EXIT) {
+        mbar_wait(bar, parity);
+        return;
+    }
+    unsigned long long t0 = 0;
+    for (uint32_t spin = 1; !mbar_try_wait(bar, parity); ++spin) {
+        if ((spin & 0xfffu) == 0) {
+            const unsigned long long now = globaltimer_ns();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 20000000000ULL)
+                asm volatile("st.global.u32 [%0], %1;\n\texit;" ::"l"(0ULL), "r"(spin) : "memory");
+        }
+    }
+}
 
 // One Kahan step for the two frames of a lane, the compensation carried as e = -(running error):
 // the carried value is s + e.  c2 = the coefficient in both halves.
@@ -147,14 +169,16 @@ __device__ __forceinline__ float fl_cast(unsigned v)
     else return (float)v;
 }
 
-// COR: the batch carries correction arrays and / or a mask (one set for all frames).  The loaders apply them
-// as they stage a tile (H2): a pixel that is invalid for every frame -- masked, or with a zero / non-finite denominator --
-// is stored as 0 and its weight is taken off the bins' counts once per call (fl_static_count_kernel); a pixel whose
-// corrected value is not finite is stored as NaN and handled per frame like a non-finite pixel of a float frame.
+// COR: the batch carries correction arrays and / or a mask (one set for all frames).  sum c (I - dark) / den
+// is computed as sum (c / den) (I - dark): the division is folded into a per-call copy of the coefficients
+// (fl_scale_blob_kernel), the loaders subtract the dark current as they stage a tile.  A pixel that is invalid for every
+// frame -- masked, or with a zero / non-finite denominator -- is stored as 0 (its scaled coefficients are 0 too) and its
+// weight is taken off the bins' counts once per call (fl_static_count_kernel); a pixel whose I - dark is not finite is
+// stored as NaN and handled per frame like a non-finite pixel of a float frame.
 template <int DT, bool COR>
 __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_constant__ CUtensorMap tmap, const FlParams p)
 {
-    constexpr bool TRACK = DT == AI_F32 || COR;
+    constexpr bool TRACK = DT == AI_F32;      // (integer frames minus a finite dark current are finite)
     // [accumulators][barriers, flags][stages: tile of 64 frames, blob]
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *bar = smem + kFlWindow * 32 * 16;
@@ -179,7 +203,11 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
     fl_enter(cur, p);
     if (warp < kFlLoad) {
         // ===== loaders =================================================================================================
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");          // two passes of 128-bit loads in registers
+        // two passes of 128-bit loads in registers.  (ptxas follows setmaxnreg only in the corrected variant, whose waits
+        // carry no trap -- see mbar_wait_fl; the plain variant's loaders fit the launch-time 80 registers but for one
+        // 4-byte spill, and were measured 5-10 % slower when given more: 80 / 88 / 96 / 104 / 112 -> 1.17 / 1.25 / 1.23 /
+        // 1.25 / 1.28 ms per 1024 frames of configs[3].)
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
         // lane = (lane of the consumers, 16-byte piece of a tile row): lanes 4 lw .. 4 lw + 3 x pieces 0..7, so that the
         // 8 lanes of a 128-bit load phase read one 128-byte line.  Stores are 64-bit (one pixel of the lane's two
         // frames); pieces 4..7 store their pixels in the order 2, 3, 0, 1, which puts the 16 lanes of a store phase into
@@ -233,82 +261,55 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
                 if (s.in_b && row < s.rows) b[u] = __ldcs(reinterpret_cast<const uint4 *>(q + p.frame_stride_bytes));
             }
         };
-        // corrected variant: the tile's correction values travel like the frames -- loaded into registers one tile ahead,
-        // one 16-byte chunk per loader thread (4 arrays x 64 chunks) and the mask's 16 chunks by the first 16 threads,
-        // stored into the stage when it is free; absent arrays and chunks outside the image read as 0 (dark, mask) / 1
-        const bool has_den = COR && (p.cor.flat || p.cor.solidangle || p.cor.polarization);
-        uint4 cq = make_uint4(0, 0, 0, 0), mq = cq;
+        // corrected variant: the tile's dark current (0 for a pixel that is invalid for every frame: fl_prep_kernel) and,
+        // for float frames, its keep words (0 for such a pixel, else all ones) travel like the frames -- loaded into
+        // registers one tile ahead (one 16-byte chunk per thread: 64 threads the dark current, 64 the keep words), stored
+        // into the stage when it is free; chunks outside the image read as 0
+        constexpr int kCorThreads = DT == AI_F32 ? 128 : 64;
+        uint4 cq = make_uint4(0, 0, 0, 0);
         auto issue_cor = [&](const FlWalk &w) {
             if constexpr (COR) {
-                const int4 dd = __ldg(p.tile_desc + w.r);
-                const int x0 = (dd.z & 0xffff) * kFlTileW, y0 = (dd.z >> 16) * kFlTileH;
-                const int arr = tid >> 6, k = tid & 63, y = y0 + (k >> 3), x = x0 + (k & 7) * 4;
-                const float *src = arr == 0 ? p.cor.dark : arr == 1 ? p.cor.flat : arr == 2 ? p.cor.solidangle : p.cor.polarization;
-                const unsigned dflt = arr == 0 ? 0u : 0x3f800000u;
-                cq = make_uint4(dflt, dflt, dflt, dflt);
-                if (src && y < p.height && x < p.width) cq = __ldg(reinterpret_cast<const uint4 *>(src + (int64_t)y * p.width + x));
-                mq = make_uint4(0, 0, 0, 0);
-                if (tid < 16 && p.cor.mask) {
-                    // 16 mask bytes = 4 chunks of 4 pixels: half a tile row
-                    const int my = y0 + (tid >> 1), mx = x0 + (tid & 1) * 16;
-                    if (my < p.height && mx < p.width) {
-                        const uint8_t *mp = p.cor.mask + (int64_t)my * p.width + mx;
-                        if (mx + 16 <= p.width) {
-                            const uint32_t *m32 = reinterpret_cast<const uint32_t *>(mp);
-                            mq = make_uint4(__ldg(m32), __ldg(m32 + 1), __ldg(m32 + 2), __ldg(m32 + 3));
-                        } else {
-                            unsigned v[4] = {0, 0, 0, 0};
-                            for (int j = 0; mx + j < p.width; j += 4) v[j >> 2] = __ldg(reinterpret_cast<const uint32_t *>(mp + j));
-                            mq = make_uint4(v[0], v[1], v[2], v[3]);
-                        }
-                    }
+                cq = make_uint4(0, 0, 0, 0);
+                if (tid < kCorThreads) {
+                    const int4 dd = __ldg(p.tile_desc + w.r);
+                    const int k = tid & 63;
+                    const int y = (dd.z >> 16) * kFlTileH + (k >> 3), x = (dd.z & 0xffff) * kFlTileW + (k & 7) * 4;
+                    const float *src = tid < 64 ? p.dark : reinterpret_cast<const float *>(p.keep);
+                    if (y < p.height && x < p.width) cq = __ldg(reinterpret_cast<const uint4 *>(src + (int64_t)y * p.width + x));
                 }
             }
         };
         auto store_cor = [&](unsigned cor_s) {
             if constexpr (COR) {
-                sts_v4(cor_s + (unsigned)tid * 16, cq);
-                if (tid < 16) sts_v4(cor_s + 4 * kFlTilePix * 4 + (unsigned)tid * 16, mq);
-                asm volatile("bar.sync 2, %0;" ::"n"(32 * kFlLoad) : "memory");
-                // one pixel per loader thread: the scale, over the flat values (the other two factors are not read again)
-                static_assert(32 * kFlLoad == kFlTilePix, "one pixel of the tile per loader thread");
-                float fl_v, sa_v, po_v;
-                unsigned mbyte;
-                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(fl_v) : "r"(cor_s + (unsigned)(kFlTilePix + tid) * 4));
-                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(sa_v) : "r"(cor_s + (unsigned)(2 * kFlTilePix + tid) * 4));
-                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(po_v) : "r"(cor_s + (unsigned)(3 * kFlTilePix + tid) * 4));
-                asm volatile("ld.shared.u8 %0, [%1];" : "=r"(mbyte) : "r"(cor_s + (unsigned)(4 * kFlTilePix * 4 + tid)));
-                const float den = fl_v * sa_v * po_v;
-                const bool gone = mbyte != 0 || (has_den && (den == 0.f || !finite_f(den)));
-                const float scale = gone ? 0.f : (has_den ? __frcp_rn(den) : 1.0f);
-                asm volatile("st.shared.f32 [%0], %1;" ::"r"(cor_s + (unsigned)(kFlTilePix + tid) * 4), "f"(scale) : "memory");
-                asm volatile("bar.sync 2, %0;" ::"n"(32 * kFlLoad) : "memory");      // every loader reads what the others staged
+                if (tid < kCorThreads) sts_v4(cor_s + (unsigned)tid * 16, cq);
+                asm volatile("bar.sync 2, %0;" ::"n"(32 * kFlLoad) : "memory");      // every loader reads what these staged
             }
         };
         bool bad = false;
-        // corrected value of one pixel of one frame: (raw - dark) * scale, scale = the rounded reciprocal of flat * solid
-        // angle * polarisation (one rounding more than the division of the single-frame path: 6e-8 relative), or 0 for a
-        // pixel that is invalid for every frame (stored as 0, its weight leaves the counts once per call); otherwise a
-        // non-finite result becomes NaN (this frame only)
-        auto corr = [&](float raw, float dk, float scale) {
-            const float v = __fmul_rn(__fsub_rn(raw, dk), scale);
-            return scale == 0.f ? 0.f : (finite_f(v) ? v : quiet_nan());
-        };
         auto store = [&](unsigned dst, int h, const uint4 (&a)[kFlPassRows], const uint4 (&b)[kFlPassRows], unsigned cor_s) {
 #pragma unroll
             for (int u = 0; u < kFlPassRows; ++u) {
                 const unsigned o = dst + (unsigned)((h * kFlPassRows + u) * kFlTileW * 8);
-                float a0 = fl_cast<DT>(a[u].x), a1 = fl_cast<DT>(a[u].y), a2 = fl_cast<DT>(a[u].z), a3 = fl_cast<DT>(a[u].w);
-                float b0 = fl_cast<DT>(b[u].x), b1 = fl_cast<DT>(b[u].y), b2 = fl_cast<DT>(b[u].z), b3 = fl_cast<DT>(b[u].w);
+                float a0, a1, a2, a3, b0, b1, b2, b3;
                 if constexpr (COR) {
-                    // the tile's dark current and scale (1 / denominator, 0 for a pixel that is invalid for every frame),
-                    // staged by the loaders themselves (below): the lane's four pixels of the row
-                    const unsigned q = cor_s + (unsigned)((h * kFlPassRows + u) * kFlTileW + piece * 4) * 4;
-                    const uint4 dku = lds_v4(q), scu = lds_v4(q + kFlTilePix * 4);
-                    a0 = corr(a0, __uint_as_float(dku.x), __uint_as_float(scu.x)); b0 = corr(b0, __uint_as_float(dku.x), __uint_as_float(scu.x));
-                    a1 = corr(a1, __uint_as_float(dku.y), __uint_as_float(scu.y)); b1 = corr(b1, __uint_as_float(dku.y), __uint_as_float(scu.y));
-                    a2 = corr(a2, __uint_as_float(dku.z), __uint_as_float(scu.z)); b2 = corr(b2, __uint_as_float(dku.z), __uint_as_float(scu.z));
-                    a3 = corr(a3, __uint_as_float(dku.w), __uint_as_float(scu.w)); b3 = corr(b3, __uint_as_float(dku.w), __uint_as_float(scu.w));
+                    // I - dark of the lane's four pixels of the row (the division is in the call's coefficients).  A pixel
+                    // that is invalid for every frame gives 0 - 0 (float frames: its bits are cleared first, integer
+                    // frames are finite anyway); a difference that is not finite invalidates the pixel for this frame
+                    const unsigned pix = (unsigned)((h * kFlPassRows + u) * kFlTileW + piece * 4);
+                    const uint4 dku = lds_v4(cor_s + pix * 4);
+                    uint4 ka = a[u], kb = b[u];
+                    if constexpr (DT == AI_F32) {
+                        const uint4 keep = lds_v4(cor_s + kFlTilePix * 4 + pix * 4);
+                        ka = make_uint4(ka.x & keep.x, ka.y & keep.y, ka.z & keep.z, ka.w & keep.w);
+                        kb = make_uint4(kb.x & keep.x, kb.y & keep.y, kb.z & keep.z, kb.w & keep.w);
+                    }
+                    a0 = __fsub_rn(fl_cast<DT>(ka.x), __uint_as_float(dku.x)); b0 = __fsub_rn(fl_cast<DT>(kb.x), __uint_as_float(dku.x));
+                    a1 = __fsub_rn(fl_cast<DT>(ka.y), __uint_as_float(dku.y)); b1 = __fsub_rn(fl_cast<DT>(kb.y), __uint_as_float(dku.y));
+                    a2 = __fsub_rn(fl_cast<DT>(ka.z), __uint_as_float(dku.z)); b2 = __fsub_rn(fl_cast<DT>(kb.z), __uint_as_float(dku.z));
+                    a3 = __fsub_rn(fl_cast<DT>(ka.w), __uint_as_float(dku.w)); b3 = __fsub_rn(fl_cast<DT>(kb.w), __uint_as_float(dku.w));
+                } else {
+                    a0 = fl_cast<DT>(a[u].x); a1 = fl_cast<DT>(a[u].y); a2 = fl_cast<DT>(a[u].z); a3 = fl_cast<DT>(a[u].w);
+                    b0 = fl_cast<DT>(b[u].x); b1 = fl_cast<DT>(b[u].y); b2 = fl_cast<DT>(b[u].z); b3 = fl_cast<DT>(b[u].w);
                 }
                 if constexpr (TRACK)
                     bad = bad || !finite_f(a0) || !finite_f(a1) || !finite_f(a2) || !finite_f(a3) || !finite_f(b0) ||
@@ -341,7 +342,7 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
             Src sn{};
             if (!nxt.done) sn = locate(nxt, dn);
             unsigned char *stage = stage0 + (size_t)ring.stage * p.stage_bytes;
-            if (issued >= p.stages) mbar_wait_relaxed(empty + ring.stage, ring.parity ^ 1u);
+            if (issued >= p.stages) mbar_wait_fl<COR>(empty + ring.stage, ring.parity ^ 1u);
             if (lw == 0 && lane == 0) {
                 mbar_arrive_expect_tx(full + ring.stage, (uint32_t)d.y);
                 bulk_g2s(stage + kFlImgBytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y, full + ring.stage);
@@ -387,7 +388,7 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
             const int item = cur.item, group = cur.group;
             const int fa = group * kFlFrames + 2 * lane;
             while (!cur.done && cur.item == item) {
-                mbar_wait_relaxed(full + ring.stage, ring.parity);
+                mbar_wait_fl<COR>(full + ring.stage, ring.parity);
                 const unsigned char *stage = stage0 + (size_t)ring.stage * p.stage_bytes;
                 const unsigned char *blob = stage + kFlImgBytes;
                 const unsigned short *wptr = reinterpret_cast<const unsigned short *>(blob);
@@ -440,14 +441,19 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
                             unsigned long long s2 = (unsigned long long)a.x | ((unsigned long long)a.y << 32);
                             unsigned long long e2 = (unsigned long long)a.z | ((unsigned long long)a.w << 32);
                             unsigned long long *dd = p.part_d + (int64_t)(bin_lo + bl) * p.nfp + fa;
+                            // (corrected variant: the weight that leaves the count is the matrix coefficient, not the
+                            // scaled one of the stage: read from the layout's own blob)
+                            const float *c_orig = reinterpret_cast<const float *>(
+                                p.blob_orig + (size_t)__ldg(p.tile_desc + cur.r).x * 16 + (q - smem_u32(blob)));
                             for (int k = 0; k < 2 * np; ++k) {
                                 const uint4 w = lds_v4(q + 16 * (k >> 1));
                                 const float c = __uint_as_float((k & 1) ? w.y : w.x);
                                 const unsigned long long v = lds_u64(img + ((k & 1) ? w.w : w.z));
                                 const bool oka = finite_f(lo_of(v)), okb = finite_f(hi_of(v));
                                 kahan2(s2, e2, pack2(c, c), pack2(oka ? lo_of(v) : 0.f, okb ? hi_of(v) : 0.f));
-                                if (c != 0.f) {
-                                    const unsigned long long fix = __float2ull_rn(c * kFlFix);
+                                if (c != 0.f && !(oka && okb)) {
+                                    const float cw = COR ? __ldg(c_orig + 4 * (k >> 1) + (k & 1)) : c;
+                                    const unsigned long long fix = __float2ull_rn(cw * kFlFix);
                                     if (!oka && fa < p.nframes) atomicAdd(dd, fix);
                                     if (!okb && fa + 1 < p.nframes) atomicAdd(dd + 1, fix);
                                 }
@@ -476,21 +482,60 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
     }
 }
 
-// Corrected batches: the count every frame of the call starts from -- the sum of a row's coefficients over the pixels that
-// are not invalid for every frame (masked, zero / non-finite denominator: the same test as the loaders').  First a byte
-// per pixel, then one block per row (fp64, fixed order; a row with nothing but such pixels gives exactly 0).
-__global__ void __launch_bounds__(256) fl_gone_kernel(int64_t npix, Corrections cor, uint8_t *__restrict__ gone)
+// Corrected batches, once per call.  (1) fl_prep_kernel: per pixel, the byte "invalid for every frame" (masked, zero /
+// non-finite denominator or reciprocal, non-finite dark current), the factor its coefficients take (the reciprocal of
+// flat x solid angle x polarisation, 0 for an invalid pixel), the dark current the loaders subtract (0 for an invalid
+// pixel) and the keep word they AND float frames with (0 for an invalid pixel, else all ones).  (2) fl_scale_blob_kernel:
+// the call's copy of the tile blobs with every coefficient multiplied by its pixel's factor.  (3)
+// fl_static_count_kernel: the count every frame of the call starts from -- the sum of a row's coefficients over the
+// pixels that are not invalid for every frame; one block per row (fp64, fixed order; a row with nothing but such pixels
+// gives exactly 0).
+__global__ void __launch_bounds__(256) fl_prep_kernel(int64_t npix, Corrections cor, uint8_t *__restrict__ gone,
+                                                      float *__restrict__ scale, float *__restrict__ dark_call,
+                                                      uint32_t *__restrict__ keep)
 {
     const bool has_den = cor.flat || cor.solidangle || cor.polarization;
     for (int64_t px = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; px < npix; px += (int64_t)gridDim.x * blockDim.x) {
         bool g = cor.mask && __ldg(cor.mask + px) != 0;
+        float sc = 1.0f;
         if (has_den) {
             float den = cor.flat ? __ldg(cor.flat + px) : 1.0f;
             den *= cor.solidangle ? __ldg(cor.solidangle + px) : 1.0f;
             den *= cor.polarization ? __ldg(cor.polarization + px) : 1.0f;
-            g = g || den == 0.f || !finite_f(den);
+            sc = __frcp_rn(den);
+            g = g || den == 0.f || !finite_f(den) || !finite_f(sc);
         }
+        const float dk = cor.dark ? __ldg(cor.dark + px) : 0.f;
+        g = g || !finite_f(dk);
         gone[px] = g ? 1 : 0;
+        scale[px] = g ? 0.f : sc;
+        dark_call[px] = g ? 0.f : dk;
+        keep[px] = g ? 0u : 0xffffffffu;
+    }
+}
+
+// one block per tile: header and records copied, pairs {c0, c1, pos0, pos1} scaled (pos = 8 x pixel within the tile)
+__global__ void __launch_bounds__(128) fl_scale_blob_kernel(const int4 *__restrict__ tile_desc,
+                                                            const unsigned char *__restrict__ blob,
+                                                            const float *__restrict__ scale, int width, int height,
+                                                            unsigned char *__restrict__ blob_call)
+{
+    const int4 d = __ldg(tile_desc + blockIdx.x);
+    const uint4 *src = reinterpret_cast<const uint4 *>(blob) + d.x;
+    uint4 *dst = reinterpret_cast<uint4 *>(blob_call) + d.x;
+    const int nq = d.y >> 4, first_pair = nq - 2 - d.w;
+    const int x0 = (d.z & 0xffff) * kFlTileW, y0 = (d.z >> 16) * kFlTileH;
+    auto factor = [&](unsigned pos) {
+        const int pix = (int)(pos >> 3), y = y0 + pix / kFlTileW, x = x0 + pix % kFlTileW;
+        return (y < height && x < width) ? __ldg(scale + (int64_t)y * width + x) : 0.f;
+    };
+    for (int i = threadIdx.x; i < nq; i += blockDim.x) {
+        uint4 q = __ldg(src + i);
+        if (i >= first_pair && i < nq - 2) {
+            q.x = __float_as_uint(__fmul_rn(__uint_as_float(q.x), factor(q.z)));
+            q.y = __float_as_uint(__fmul_rn(__uint_as_float(q.y), factor(q.w)));
+        }
+        dst[i] = q;
     }
 }
 
@@ -602,7 +647,7 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
         if (rc != AI_OK) return rc;
     }
     if (!fl.ok) return AI_OK;
-    const bool track = a.dtype == AI_F32 || !plain;
+    const bool track = a.dtype == AI_F32;
     const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
 
     FlParams p{};
@@ -637,7 +682,7 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
     p.chunk_desc = fl.chunk_desc;
     p.chunk_owner = fl.chunk_owner;
     p.blob = fl.blob;
-    p.cor = Corrections{a.dark, a.flat, a.solidangle, a.polarization, a.mask};
+    p.blob_orig = fl.blob;
     p.frames = static_cast<const unsigned char *>(a.image);
     p.frame_stride_bytes = a.frame_stride * 4;
     p.height = ctx->height;
@@ -655,11 +700,20 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
         const int64_t npix = (int64_t)ctx->height * ctx->width;
         if (!fl.call_csum) AI_CUDA(ctx, cudaMalloc(&fl.call_csum, (size_t)ctx->npt * sizeof(double)));
         if (!fl.gone) AI_CUDA(ctx, cudaMalloc(&fl.gone, (size_t)npix));
-        fl_gone_kernel<<<sms * 8, 256, 0, st>>>(npix, p.cor, fl.gone);
+        if (!fl.scale) AI_CUDA(ctx, cudaMalloc(&fl.scale, 3 * (size_t)npix * sizeof(float)));
+        float *dark_call = fl.scale + npix;
+        uint32_t *keep = reinterpret_cast<uint32_t *>(fl.scale + 2 * npix);
+        if (!fl.blob_call) AI_CUDA(ctx, cudaMalloc(&fl.blob_call, (size_t)fl.blob_bytes));
+        const Corrections cor{a.dark, a.flat, a.solidangle, a.polarization, a.mask};
+        fl_prep_kernel<<<sms * 8, 256, 0, st>>>(npix, cor, fl.gone, fl.scale, dark_call, keep);
+        fl_scale_blob_kernel<<<fl.ntiles, 128, 0, st>>>(fl.tile_desc, fl.blob, fl.scale, ctx->width, ctx->height, fl.blob_call);
         fl_static_count_kernel<<<ctx->npt, 128, 0, st>>>(ctx->npt, ctx->indptr, ctx->indices, ctx->data, fl.gone, fl.call_csum);
         AI_CUDA(ctx, cudaGetLastError());
         csum = fl.call_csum;
-        launches = 2;
+        p.blob = fl.blob_call;
+        p.dark = dark_call;
+        p.keep = keep;
+        launches = 3;
     }
     rc = AI_EINVAL;
     switch (a.dtype) {
@@ -677,7 +731,7 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
         fl_finish_kernel<true><<<g2, 256, 0, st>>>(fl.bin_slot_ptr, fl.bin_slots, csum, ctx->npt, a.nframes, p.nfp,
                                                    p.part_s, p.part_d, ctx->empty_value, a.intensity, a.sum_signal, a.count);
     else
-        fl_finish_kernel<false><<<g2, 256, 0, st>>>(fl.bin_slot_ptr, fl.bin_slots, fl.bin_csum, ctx->npt, a.nframes, p.nfp,
+        fl_finish_kernel<false><<<g2, 256, 0, st>>>(fl.bin_slot_ptr, fl.bin_slots, csum, ctx->npt, a.nframes, p.nfp,
                                                     p.part_s, p.part_d, ctx->empty_value, a.intensity, a.sum_signal, a.count);
     AI_CUDA(ctx, cudaGetLastError());
     ctx->last_launches = launches + 2;

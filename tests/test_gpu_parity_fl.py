@@ -195,8 +195,9 @@ def test_fl_full_size_geometries_sampled(torch, B, oracle, workloads, name):
 @pytest.mark.parametrize("dtype,nframes,tune", [("int32", 7, None), ("float32", 100, "flc:2"), ("uint32", 66, None)])
 def test_fl_corrected_batches(torch, B, oracle, workloads, monkeypatch, dtype, nframes, tune):
     """Batches with every correction array and a mask (one set for all frames) through the frame-lane
-    kernel: the loaders correct the tiles as they stage them.  Pixels invalid for every frame (masked, flat = 0, a whole
-    masked band that empties bins) leave the counts once per call; non-finite raw pixels per frame."""
+    kernel: the division is folded into a per-call copy of the coefficients, the loaders subtract the dark current as
+    they stage the tiles.  Pixels invalid for every frame (masked, flat = 0 or not finite, a dark current that is not
+    finite, a whole masked band that empties bins) leave the counts once per call; non-finite raw pixels per frame."""
     monkeypatch.setenv("AZINT_FORCE_FL", "1")
     if tune:
         monkeypatch.setenv("AZINT_TUNE", tune)
@@ -212,8 +213,11 @@ def test_fl_corrected_batches(torch, B, oracle, workloads, monkeypatch, dtype, n
     mask[80:100, 90:112] = 1                      # around the beam centre: the innermost bins lose every pixel
     flat[10, 10] = 0.0
     flat[150, 200] = np.inf
+    dark[60, 70] = np.nan                         # a dark current that is not finite: invalid for every frame, any dtype
+    dark[61, 170] = np.inf
     if dtype == "float32":
         frames[2, 33, 44] = np.nan
+        frames[0, 85, 95] = np.nan                # under the mask: must not touch anything
         frames[nframes - 1, 120, 7] = np.inf
     integ = B.Integrator(cfg)
     n = frames.shape[0]
@@ -225,7 +229,7 @@ def test_fl_corrected_batches(torch, B, oracle, workloads, monkeypatch, dtype, n
     i, s, c = integ.outputs(n)
     B.ai_integrate1d_batch(integ.ctx, t, n, cfg.npix, *cor, i, s, c, dtype=code)
     torch.cuda.synchronize()
-    assert B.ai_last_launch_count(integ.ctx) == 4 and B.ai_get_batch_layout_info(integ.ctx)["built"] == 1
+    assert B.ai_last_launch_count(integ.ctx) == 5 and B.ai_get_batch_layout_info(integ.ctx)["built"] == 1
     umin, umax = oracle.pixel_bounds(cfg)
     u0, u1 = oracle.auto_range(umin, umax)
     for f in sorted({0, 2, n // 2, n - 1}):
