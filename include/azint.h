@@ -225,6 +225,29 @@ int ai_get_layout_info(const ai_ctx *ctx, int64_t info[8]);
  * group}.  Errors: AI_EINVAL, AI_ENOTBUILT. */
 int ai_get_batch_layout_info(const ai_ctx *ctx, int64_t info[8]);
 
+/* Holds a set of correction arrays for the calls that follow (dark current, flat field, solid angle and
+ * polarisation are per-experiment constants; in PAPER.md:248-254 only the image crosses the bus per frame).  DEVICE
+ * pointers to height*width elements each, any of them NULL; all five NULL drops the held set.  The arrays are read by
+ * kernels this call enqueues on `cuda_stream` and not referenced afterwards: they may be freed or changed once the
+ * stream has passed this point (changing them has no effect until they are held again).  Every later ai_integrate1d /
+ * ai_integrate1d_batch / ai_integrate1d_host* / ai_integrate2d call on this context that passes NO correction array and
+ * no mask of its own integrates frames corrected with the held set; a call that passes any array uses its own
+ * arguments only, as before.  ai_build_csr drops the held set.
+ *
+ * What holding buys: sum c (I - dark) / den = sum (c / den) (I - dark), so the division and the mask are
+ * folded into a copy of the matrix once -- a pixel that is invalid for every frame (masked, zero or non-finite
+ * denominator or reciprocal, non-finite dark current) gets zero coefficients and leaves the counts -- and a frame is
+ * corrected inside the integration kernel: AI_LAYOUT_TILED with AI_ACC_F32_KAHAN, one 32-bit frame per call, takes the
+ * single-frame kernel with the dark tile loaded beside the frame tile (2 launches instead of 3, one pass over frame,
+ * dark current and matrix), and corrected frame-lane batches skip their per-call preparation.  Everywhere else the held
+ * set acts as a (dark, flat = product of the three, 0 where invalid) pair.  A corrected value is (I - dark) times the
+ * rounded reciprocal of the denominator here (one rounding more than the division of the per-call path).
+ * Costs 17 bytes per pixel plus a copy of the layout's blobs.  Call it with the context idle or on the stream the
+ * integrate calls use (the derived arrays are rewritten in place).
+ * Errors: AI_EINVAL, AI_ENOTBUILT, AI_ENOMEM, AI_ECUDA. */
+int ai_hold_corrections(ai_ctx *ctx, const float *dark, const float *flat, const float *solidangle,
+                        const float *polarization, const uint8_t *mask, void *cuda_stream);
+
 /* Number of kernels the last ai_integrate1d* call launched (for accounting in benchmarks). */
 int ai_last_launch_count(const ai_ctx *ctx);
 

@@ -23,7 +23,7 @@ AI_SPLIT_BBOX, AI_SPLIT_FULL = range(2)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_set_splitting", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
-           "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_get_layout_info", "ai_get_batch_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
+           "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_hold_corrections", "ai_get_layout_info", "ai_get_batch_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
 class ai_geometry(C.Structure):
@@ -53,6 +53,7 @@ def lib():
     L.ai_setup.argtypes = [C.POINTER(vp), C.POINTER(ai_geometry), C.c_int, C.c_int, C.c_int, C.c_int, dp]
     L.ai_setup2d.argtypes = [C.POINTER(vp), C.POINTER(ai_geometry), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, dp, dp]
     L.ai_integrate2d.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, fp, vp]
+    L.ai_hold_corrections.argtypes = [vp, fp, fp, fp, fp, vp, vp]
     L.ai_build_csr.argtypes = [vp, vp]
     L.ai_get_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_int64), dp, dp]
     L.ai_copy_csr_to_host.argtypes = [vp, vp, vp, vp]
@@ -183,6 +184,12 @@ def ai_integrate1d_batch(ctx, frames, nframes, frame_stride_elems, dark, flat, s
                                       frame_stride_elems, _ptr(dark), _ptr(flat), _ptr(solidangle),
                                       _ptr(polarization), _ptr(mask), _ptr(intensity), _ptr(sum_signal), _ptr(count),
                                       _stream(stream)), ctx)
+
+
+def ai_hold_corrections(ctx, dark, flat, solidangle, polarization, mask, stream=None):
+    """Holds the correction arrays (device tensors or None) for the calls that pass none; all None drops them."""
+    _check(lib().ai_hold_corrections(ctx, _ptr(dark), _ptr(flat), _ptr(solidangle), _ptr(polarization), _ptr(mask),
+                                     _stream(stream)), ctx)
 
 
 def ai_integrate1d_host(ctx, image_host, dark, flat, solidangle, polarization, mask, intensity_host, sum_signal_host,
@@ -342,6 +349,9 @@ class Integrator:
         ai_integrate1d_batch(self.ctx, frames, nframes, frames.stride(0), dark, flat, solidangle, polarization, mask,
                              intensity, sum_signal, count)
         return intensity, sum_signal, count
+
+    def hold_corrections(self, dark=None, flat=None, solidangle=None, polarization=None, mask=None):
+        ai_hold_corrections(self.ctx, dark, flat, solidangle, polarization, mask)
 
     def close(self):
         if self.ctx is not None:

@@ -298,10 +298,18 @@ int ai_set_normalization(ai_ctx *ctx, ai_norm norm)
     return AI_OK;
 }
 
-static int integrate(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
+static int integrate(ai_ctx *ctx, const FrameArgs &args, cudaStream_t st)
 {
     if (!ctx) return AI_EINVAL;
     if (!ctx->built) return ai_fail(ctx, AI_ENOTBUILT, "ai_build_csr has not been called");
+    // held corrections (ai_hold_corrections) serve the calls that pass no correction array of their own: to every kernel
+    // but the ones that know better (hold.cu) they are a dark current and a denominator, 0 where the pixel is invalid
+    FrameArgs a = args;
+    if (ctx->held.on && !a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask) {
+        a.held = true;
+        a.dark = ctx->held.dark;
+        if (ctx->held.has_den) a.flat = ctx->held.den;
+    }
     if (!a.image || !a.intensity || !a.sum_signal || !a.count) return ai_fail(ctx, AI_EINVAL, "NULL image or output");
     if ((int)a.dtype < AI_F32 || (int)a.dtype > AI_U32) return ai_fail(ctx, AI_EINVAL, "bad dtype %d", (int)a.dtype);
     if (a.nframes < 1) return ai_fail(ctx, AI_EINVAL, "nframes < 1");
@@ -333,6 +341,23 @@ int ai_integrate1d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *
     FrameArgs a{image, dtype, dark, flat, solidangle, polarization, mask, radial, intensity, sum_signal, count, 1,
                 (int64_t)ctx->height * ctx->width};
     return integrate(ctx, a, (cudaStream_t)cuda_stream);
+}
+
+int ai_hold_corrections(ai_ctx *ctx, const float *dark, const float *flat, const float *solidangle,
+                        const float *polarization, const uint8_t *mask, void *cuda_stream)
+{
+    if (!ctx) return AI_EINVAL;
+    if (!ctx->built) return ai_fail(ctx, AI_ENOTBUILT, "ai_build_csr has not been called");
+    int dev = -1;
+    AI_CUDA(ctx, cudaGetDevice(&dev));
+    if (dev != ctx->device)
+        return ai_fail(ctx, AI_EINVAL, "the matrix was built on device %d, the current device is %d", ctx->device, dev);
+    if (!dark && !flat && !solidangle && !polarization && !mask) {
+        // scratch of calls in flight on other streams is the caller's to wait for, as with ai_destroy
+        ai_release_held(ctx);
+        return AI_OK;
+    }
+    return ai_hold_build(ctx, dark, flat, solidangle, polarization, mask, (cudaStream_t)cuda_stream);
 }
 
 int ai_integrate2d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *dark, const float *flat,
@@ -501,6 +526,7 @@ static void release_matrix_and_scratch(ai_ctx *ctx)
     ctx->stream_first = nullptr;
     ctx->stream_first_grid = 0;
     ai_free_fl(ctx->fl);
+    ai_release_held(ctx);
     drop(ctx->partials); drop(ctx->staging); drop(ctx->out_dev); drop(ctx->grid_sync); drop(ctx->chain_done);
     drop(ctx->stream_partials); drop(ctx->axes2d); drop(ctx->corrected[0]); drop(ctx->corrected[1]);
     ctx->partials_bytes = ctx->staging_bytes = 0;

@@ -151,6 +151,22 @@ struct FlLayout {
     size_t partials_bytes = 0;
 };
 
+// ---- held corrections (hold.cu) ----------------------------------------------------------------------------------------
+struct HeldCorrections {
+    bool on = false;
+    bool has_den = false;           // the set holds a denominator array or a mask (else only a dark current)
+    uint8_t *gone = nullptr;        // [npix] 1 = invalid for every frame
+    float *scale = nullptr;         // [4][npix], one allocation: 1 / den (0 where gone), then
+    float *dark = nullptr;          //   the dark current (0 where gone),
+    uint32_t *keep = nullptr;       //   the keep word (all ones, 0 where gone),
+    float *den = nullptr;           //   the denominator (0 where gone)
+    unsigned char *tl_blob = nullptr;   // tiled blobs: coefficients x scale, run sums without the gone pixels
+    bool tl_ready = false;
+    unsigned char *fl_blob = nullptr;   // frame-lane blobs, coefficients x scale (built with the first frame-lane batch)
+    double *fl_csum = nullptr;          // [npt] the frame-lane finish kernel's count without the gone pixels
+    bool fl_ready = false;
+};
+
 struct ai_ctx {
     ai_geometry geo{};
     int height = 0, width = 0, npt = 0;   // npt = number of bins = rows of the matrix (2D: npt_azim * npt_rad)
@@ -196,6 +212,7 @@ struct ai_ctx {
 
     TiledLayout tl;
     FlLayout fl;
+    HeldCorrections held;
 
     // per-call scratch
     void *partials = nullptr;       // tiled stage-1 output, bin-major
@@ -292,6 +309,7 @@ struct FrameArgs {
     int nframes;
     int64_t frame_stride;
     int64_t row_pitch = 0;       // elements between rows of `image`; 0 = width (only the library's own corrected frame differs)
+    bool held = false;           // the call uses the context's held corrections (dark / flat point at their derived arrays)
 };
 int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_tiled_split(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
@@ -301,6 +319,9 @@ int ai_launch_scatter(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_build_fl(ai_ctx *ctx, int nframes, cudaStream_t st);                          // build_fl.cu: frame-lane layout from the canonical CSR
 void ai_free_fl(FlLayout &fl);
 int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled);   // integrate_fl.cu
+void ai_release_held(ai_ctx *ctx);                                                     // hold.cu
+int ai_hold_build(ai_ctx *ctx, const float *dark, const float *flat, const float *solidangle, const float *polarization,
+                  const uint8_t *mask, cudaStream_t st);
 int ai_launch_correct(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int overlap, int mode, cudaStream_t st, float **out);   // integrate_prep.cu
 int ai_stream_full_grid(const ai_ctx *ctx);   // integrate_stream.cu: 1 if the single-frame kernel puts one block on every SM
 int ai_stream_stages(const ai_ctx *ctx);      // integrate_stream.cu: (tile + blob) stages of the single-frame kernel, 0 = n/a

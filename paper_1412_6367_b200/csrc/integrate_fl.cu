@@ -696,7 +696,24 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
     // corrected batches: the count all frames share, without the pixels that are invalid for every frame
     const double *csum = fl.bin_csum;
     int launches = 0;
-    if (!plain) {
+    if (!plain && a.held && ctx->held.on) {
+        // held corrections (hold.cu): the per-pixel arrays exist; the scaled blobs and the static count are made with the
+        // first batch after ai_hold_corrections and kept
+        HeldCorrections &h = ctx->held;
+        if (!h.fl_ready) {
+            if (!h.fl_csum) AI_CUDA(ctx, cudaMalloc(&h.fl_csum, (size_t)ctx->npt * sizeof(double)));
+            if (!h.fl_blob) AI_CUDA(ctx, cudaMalloc(&h.fl_blob, (size_t)fl.blob_bytes));
+            fl_scale_blob_kernel<<<fl.ntiles, 128, 0, st>>>(fl.tile_desc, fl.blob, h.scale, ctx->width, ctx->height, h.fl_blob);
+            fl_static_count_kernel<<<ctx->npt, 128, 0, st>>>(ctx->npt, ctx->indptr, ctx->indices, ctx->data, h.gone, h.fl_csum);
+            AI_CUDA(ctx, cudaGetLastError());
+            h.fl_ready = true;
+            launches = 2;
+        }
+        csum = h.fl_csum;
+        p.blob = h.fl_blob;
+        p.dark = h.dark;
+        p.keep = h.keep;
+    } else if (!plain) {
         const int64_t npix = (int64_t)ctx->height * ctx->width;
         if (!fl.call_csum) AI_CUDA(ctx, cudaMalloc(&fl.call_csum, (size_t)ctx->npt * sizeof(double)));
         if (!fl.gone) AI_CUDA(ctx, cudaMalloc(&fl.gone, (size_t)npix));

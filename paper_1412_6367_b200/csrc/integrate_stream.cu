@@ -39,8 +39,12 @@ struct StreamFirstDescs {
 struct StreamParams {
     const int4 *blob_desc;       // longest first: {blob offset / 16, blob bytes, tile row << 16 | column, blocks}
     const unsigned char *blob;
+    const unsigned char *blob_orig;   // held corrections: `blob` is the held copy, this one the matrix's own
     int tile_h, ntiles, nslot;
     int stages, mat_stage_bytes, img_stage_bytes, hdr_bytes;
+    int tile_bytes;              // bytes of a frame tile (= img_stage_bytes without held corrections)
+    int dk;                      // held corrections: the dark tile lies dk bytes behind the frame tile (a multiple of
+                                 // 1024: same 128-byte swizzle phase), img_stage_bytes = 2 dk
     int dyn_base;                // rank of the first tile handed out by ticket (the ones before are dealt statically)
     int launch_index;            // launches of this context so far, modulo 8 (development trace only)
     int track_all;               // float frames: every block skips non-finite pixels and accumulates count
@@ -121,6 +125,25 @@ __device__ __forceinline__ float4 stream_gather4(const uint2 &x, unsigned base)
     }
 }
 
+// held corrections: the pixel minus the held dark current, whose tile lies `dk` bytes behind the frame's
+template <int DT>
+__device__ __forceinline__ float4 stream_gather4_held(const uint2 &x, unsigned base, unsigned dk)
+{
+    const unsigned p0 = x.x + base, p1 = x.y + base;
+    const unsigned a0 = p0 & 0xffffu, a1 = p0 >> 16, a2 = p1 & 0xffffu, a3 = p1 >> 16;
+    float4 v;
+    if constexpr (DT == AI_F32) {
+        v = make_float4(lds_f32(a0), lds_f32(a1), lds_f32(a2), lds_f32(a3));
+    } else if constexpr (DT == AI_I32) {
+        v = make_float4((float)lds_s32(a0), (float)lds_s32(a1), (float)lds_s32(a2), (float)lds_s32(a3));
+    } else {
+        v = make_float4((float)(unsigned)lds_s32(a0), (float)(unsigned)lds_s32(a1), (float)(unsigned)lds_s32(a2),
+                        (float)(unsigned)lds_s32(a3));
+    }
+    return make_float4(__fsub_rn(v.x, lds_f32(a0 + dk)), __fsub_rn(v.y, lds_f32(a1 + dk)), __fsub_rn(v.z, lds_f32(a2 + dk)),
+                       __fsub_rn(v.w, lds_f32(a3 + dk)));
+}
+
 // lanes of a run are adjacent: suffix sums by doubling, the head of the run ends with the run's total
 template <int ACC, bool TRACK>
 __device__ __forceinline__ void stream_finish_block(Accum<ACC> &S, Accum<ACC> &C, const int2 &m, int rounds, void *part_f)
@@ -174,8 +197,9 @@ __device__ __forceinline__ void stream_finish_d(double S, double C, const int2 &
 // stage has slack behind the blob, so the look-ahead needs no predicate.  Float frames are not screened: a
 // non-finite lane sum anywhere in the warp means a non-finite pixel may have been gathered; nothing is stored and
 // true is returned (the caller repeats the block with stream_block_tracked).
-template <int DT, int ACC, bool PACKED = true>
-__device__ __noinline__ bool stream_block(unsigned rebase, const unsigned char *blob, unsigned h, void *part_f, int lane)
+template <int DT, int ACC, bool PACKED = true, bool HELD = false>
+__device__ __noinline__ bool stream_block(unsigned rebase, const unsigned char *blob, unsigned h, void *part_f, int lane,
+                                          unsigned dk = 0)
 {
     const int nsteps = h & 15, rounds = (h >> 4) & 7;
     const unsigned char *blk = blob + (size_t)(h >> 8) * 16;
@@ -189,7 +213,14 @@ __device__ __noinline__ bool stream_block(unsigned rebase, const unsigned char *
     for (int j = 2; j <= nsteps; j += 2) {
         const float4 n0 = cp[j * 32], n1 = cp[j * 32 + 32];
         const uint2 y0 = xp[j * 32], y1 = xp[j * 32 + 32];
-        const float4 v0 = stream_gather4<DT, PACKED>(x0, rebase), v1 = stream_gather4<DT, PACKED>(x1, rebase);
+        float4 v0, v1;
+        if constexpr (HELD) {
+            v0 = stream_gather4_held<DT>(x0, rebase, dk);
+            v1 = stream_gather4_held<DT>(x1, rebase, dk);
+        } else {
+            v0 = stream_gather4<DT, PACKED>(x0, rebase);
+            v1 = stream_gather4<DT, PACKED>(x1, rebase);
+        }
         accumulate4<ACC, false>(c0, v0, S2, C2);
         accumulate4<ACC, false>(c1, v1, S2, C2);
         c0 = n0; c1 = n1; x0 = y0; x1 = y1;
@@ -241,6 +272,38 @@ __device__ __noinline__ void stream_block_tracked(unsigned rebase, const unsigne
     }
 }
 
+// Held corrections (hold.cu), a block that met a non-finite I - dark (a non-finite pixel of a float frame): the staged
+// coefficients carry 1 / den, so the weight a valid pixel adds to count is read from the matrix's own blob (`orig`, global
+// memory, same offsets).  A pixel that is invalid for every frame has a zero staged coefficient and adds nothing: its
+// weight is not in the run sums of the held blob either.
+template <int DT>
+__device__ __noinline__ void stream_block_tracked_held(unsigned rebase, const unsigned char *blob, const unsigned char *orig,
+                                                       unsigned h, void *part_f, int lane, unsigned dk)
+{
+    const int nsteps = h & 15, rounds = (h >> 4) & 7;
+    const unsigned char *blk = blob + (size_t)(h >> 8) * 16;
+    const float4 *cp = reinterpret_cast<const float4 *>(blk) + lane;
+    const float4 *op = reinterpret_cast<const float4 *>(orig + (size_t)(h >> 8) * 16) + lane;
+    const uint2 *xp = reinterpret_cast<const uint2 *>(blk + nsteps * 512) + lane;
+    const int2 m = reinterpret_cast<const int2 *>(blk + nsteps * kBlkStepBytes)[lane];
+    AccumQ<AI_ACC_F32_KAHAN> S2, C2;
+#pragma unroll 1
+    for (int j = 0; j < nsteps; ++j) {
+        const float4 c = cp[j * 32], o = __ldg(op + j * 32);
+        const float4 v = stream_gather4_held<DT>(xp[j * 32], rebase, dk);
+        const bool k0 = finite_f(v.x), k1 = finite_f(v.y), k2 = finite_f(v.z), k3 = finite_f(v.w);
+        S2.a.add(c.x, k0 ? v.x : 0.0f);
+        S2.b.add(c.y, k1 ? v.y : 0.0f);
+        S2.c.add(c.z, k2 ? v.z : 0.0f);
+        S2.d.add(c.w, k3 ? v.w : 0.0f);
+        C2.a.add1(k0 && c.x != 0.0f ? o.x : 0.0f);
+        C2.b.add1(k1 && c.y != 0.0f ? o.y : 0.0f);
+        C2.c.add1(k2 && c.z != 0.0f ? o.z : 0.0f);
+        C2.d.add1(k3 && c.w != 0.0f ? o.w : 0.0f);
+    }
+    stream_finish_d<true>(kahan_total_d(S2), kahan_total_d(C2), m, rounds, part_f);
+}
+
 // Batches (H6): the same block against the tiles of TWO frames at once.  Coefficients and positions are loaded and
 // unpacked once and serve both frames; the two sets of accumulators double the independent work per lane.  Returns
 // true (nothing stored) if a non-finite lane sum shows that either tile may hold a non-finite pixel.
@@ -287,8 +350,9 @@ __device__ __noinline__ bool stream_block2(unsigned tile_a, unsigned tile_b, con
     return false;
 }
 
-template <int DT, int ACC>
+template <int DT, int ACC, bool HELD = false>
 __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const __grid_constant__ CUtensorMap tmap,
+                                                                         const __grid_constant__ CUtensorMap dmap,
                                                                          const __grid_constant__ StreamFirstDescs first,
                                                                          const StreamParams p)
 {
@@ -312,14 +376,19 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
 
     auto issue_blob = [&](int stage, const int4 &d) {
         stage_desc[stage] = d;
-        mbar_arrive_expect_tx(full + stage, (uint32_t)(p.img_stage_bytes + d.y));
+        mbar_arrive_expect_tx(full + stage, (uint32_t)((HELD ? 2 : 1) * p.tile_bytes + d.y));
         bulk_g2s(mat_base + (size_t)stage * p.mat_stage_bytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y, full + stage);
     };
     auto issue_tile = [&](int stage, const int4 &d) {
         unsigned char *tile = img_base + (size_t)stage * p.img_stage_bytes;
         const int ty = d.z >> 16, tx = d.z & 0xffff;
         tma_box(tile, &tmap, tx * kTileW, ty * p.tile_h, 0, full + stage);
-        tma_box(tile + p.img_stage_bytes / 2, &tmap, tx * kTileW + 32, ty * p.tile_h, 0, full + stage);
+        tma_box(tile + p.tile_bytes / 2, &tmap, tx * kTileW + 32, ty * p.tile_h, 0, full + stage);
+        if constexpr (HELD) {
+            // the held dark current of the same pixels, behind the frame tile
+            tma_box(tile + p.dk, &dmap, tx * kTileW, ty * p.tile_h, 0, full + stage);
+            tma_box(tile + p.dk + p.tile_bytes / 2, &dmap, tx * kTileW + 32, ty * p.tile_h, 0, full + stage);
+        }
     };
 
     // Launch chain (programmatic dependent launch).  A call is two launches, this kernel (S) and the finish kernel (F,
@@ -342,6 +411,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
+        if constexpr (HELD) asm volatile("prefetch.tensormap [%0];" ::"l"(&dmap) : "memory");
         if (p.full_grid && blockIdx.x == 0) {
             // tickets of the context's next launch (last used by the launch before the previous one, complete: see
             // above): zero before any block of that launch can exist, i.e. before this block lets dependents start
@@ -448,7 +518,11 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
                 const unsigned rebase = (smem_u32(img_base + (size_t)r.stage * p.img_stage_bytes) & 0xffffu) * 0x10001u;
                 for (int b = firstb; b < d.w; b += kStreamCons) {
                     const unsigned h = bh[b];
-                    if constexpr (DT == AI_F32) {
+                    if constexpr (HELD) {
+                        if (stream_block<DT, ACC, true, true>(rebase, blob, h, p.partials, lane, (unsigned)p.dk))
+                            stream_block_tracked_held<DT>(rebase, blob, p.blob_orig + (size_t)d.x * 16, h, p.partials, lane,
+                                                          (unsigned)p.dk);
+                    } else if constexpr (DT == AI_F32) {
                         // track_all: the frame comes from the correction pre-pass and is expected to hold NaN marks
                         if (p.track_all || stream_block<DT, ACC>(rebase, blob, h, p.partials, lane))
                             stream_block_tracked<ACC>(rebase, blob, h, p.partials, lane);
@@ -622,17 +696,17 @@ __global__ void __launch_bounds__(kBatchThreads, 1) tiled_bstream_kernel(const _
     }
 }
 
-template <int DT, int ACC>
-int launch_stream(ai_ctx *ctx, const CUtensorMap &map, const StreamFirstDescs &first, StreamParams p, size_t smem,
-                  int grid, cudaStream_t st)
+template <int DT, int ACC, bool HELD = false>
+int launch_stream(ai_ctx *ctx, const CUtensorMap &map, const CUtensorMap &dmap, const StreamFirstDescs &first, StreamParams p,
+                  size_t smem, int grid, cudaStream_t st)
 {
-    const uint64_t bit = 1ULL << (DT * 3 + ACC);          // per context and instantiation: opt in to the large
+    const uint64_t bit = 1ULL << (HELD ? 45 + (DT == AI_F32 ? 0 : DT == AI_I32 ? 1 : 2) : DT * 3 + ACC);      // per context and instantiation: opt in to the large
     if (!(ctx->smem_opt_in & bit)) {                      // dynamic shared memory once
-        AI_CUDA(ctx, cudaFuncSetAttribute(tiled_stream_kernel<DT, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        AI_CUDA(ctx, cudaFuncSetAttribute(tiled_stream_kernel<DT, ACC, HELD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           kPipeSmemBudget));
         // the launch chain (see the kernel) relies on ONE block of this kernel per SM
         int per_sm = 0;
-        AI_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tiled_stream_kernel<DT, ACC>, kStreamThreads, smem));
+        AI_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tiled_stream_kernel<DT, ACC, HELD>, kStreamThreads, smem));
         if (per_sm != 1) ctx->stream_shared_sm |= bit;
         ctx->smem_opt_in |= bit;
     }
@@ -648,19 +722,20 @@ int launch_stream(ai_ctx *ctx, const CUtensorMap &map, const StreamFirstDescs &f
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     ai_prof_begin(ctx, st);
-    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, tiled_stream_kernel<DT, ACC>, map, first, p));
+    AI_CUDA(ctx, cudaLaunchKernelEx(&cfg, tiled_stream_kernel<DT, ACC, HELD>, map, dmap, first, p));
     ai_prof_end(ctx, st);
     return AI_OK;
 }
 
 template <int DT>
-int launch_stream_dt(ai_ctx *ctx, const CUtensorMap &map, const StreamFirstDescs &first, const StreamParams &p,
-                     size_t smem, int grid, cudaStream_t st)
+int launch_stream_dt(ai_ctx *ctx, const CUtensorMap &map, const CUtensorMap *dmap, const StreamFirstDescs &first,
+                     const StreamParams &p, size_t smem, int grid, cudaStream_t st)
 {
+    if (dmap) return launch_stream<DT, AI_ACC_F32_KAHAN, true>(ctx, map, *dmap, first, p, smem, grid, st);
     switch (ctx->accum) {
-    case AI_ACC_F32_KAHAN: return launch_stream<DT, AI_ACC_F32_KAHAN>(ctx, map, first, p, smem, grid, st);
-    case AI_ACC_F32_PLAIN: return launch_stream<DT, AI_ACC_F32_PLAIN>(ctx, map, first, p, smem, grid, st);
-    default: return launch_stream<DT, AI_ACC_F64>(ctx, map, first, p, smem, grid, st);
+    case AI_ACC_F32_KAHAN: return launch_stream<DT, AI_ACC_F32_KAHAN>(ctx, map, map, first, p, smem, grid, st);
+    case AI_ACC_F32_PLAIN: return launch_stream<DT, AI_ACC_F32_PLAIN>(ctx, map, map, first, p, smem, grid, st);
+    default: return launch_stream<DT, AI_ACC_F64>(ctx, map, map, first, p, smem, grid, st);
     }
 }
 
@@ -675,10 +750,12 @@ extern "C" int ai_debug_set_stream_trace(void *dev_buffer)
 #endif
 
 // shared-memory plan: [tile stages][barriers + descriptors][blob stages]; false if fewer than two stages fit
-static bool stream_plan(const ai_ctx *ctx, int grid, StreamParams *p)
+static bool stream_plan(const ai_ctx *ctx, int grid, StreamParams *p, bool held = false)
 {
     const TiledLayout &tl = ctx->tl;
-    p->img_stage_bytes = tl.tile_h * kTileW * 4;
+    p->tile_bytes = tl.tile_h * kTileW * 4;
+    p->dk = held ? ai_align_up(p->tile_bytes, 1024) : 0;
+    p->img_stage_bytes = held ? 2 * p->dk : p->tile_bytes;
     p->mat_stage_bytes = ai_align_up(tl.max_blob_bytes + 1024, 1024);     // slack: the look-ahead reads past a blob's end
     p->hdr_bytes = ai_align_up(kStreamBarBytes, 1024);
     int stages = (kPipeSmemBudget - p->hdr_bytes) / (p->img_stage_bytes + p->mat_stage_bytes);
@@ -714,10 +791,13 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int tra
 {
     const TiledLayout &tl = ctx->tl;
     *handled = false;
+    // held corrections (hold.cu): the held copy of the blobs, the dark tile behind every frame tile
+    const bool held = a.held;
+    if (held && (!ctx->held.on || !ctx->held.tl_ready || ctx->accum != AI_ACC_F32_KAHAN || ctx->width % 4 != 0)) return AI_OK;
     if (a.nframes != 1 || tl.ntiles < 1 || !tl.blob || !tl.h_first_desc || !ctx->grid_sync || !ctx->stream_partials ||
         ctx->no_tma || ctx->no_stream)
         return AI_OK;
-    const bool plain = !a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask;
+    const bool plain = held || (!a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask);
     const bool is32 = a.dtype == AI_F32 || a.dtype == AI_I32 || a.dtype == AI_U32;
     if (!plain || !is32 || !vec_ok || (reinterpret_cast<uintptr_t>(a.image) % 16) != 0) return AI_OK;
     const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
@@ -725,10 +805,11 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int tra
     if (grid > kStreamMaxGrid) return AI_OK;
 
     StreamParams p{};
-    if (!stream_plan(ctx, grid, &p)) return AI_OK;
+    if (!stream_plan(ctx, grid, &p, held)) return AI_OK;
     const int stages = p.stages;
     p.blob_desc = tl.blob_desc;
-    p.blob = tl.blob;
+    p.blob = held ? ctx->held.tl_blob : tl.blob;
+    p.blob_orig = tl.blob;
     p.tile_h = tl.tile_h;
     p.ntiles = tl.ntiles;
     p.nslot = tl.nslot;
@@ -761,14 +842,24 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int tra
         ctx->stream_first_grid = grid;
     }
     const StreamFirstDescs &first = *static_cast<const StreamFirstDescs *>(ctx->stream_first);
-    CUtensorMap map{};
+    CUtensorMap map{}, dmap{};
     int rc = ai_make_frame_map(ctx, a, tl.tile_h, &map);
     if (rc != AI_OK) return rc;
+    if (held) {
+        FrameArgs dk{};
+        dk.image = ctx->held.dark;
+        dk.dtype = AI_F32;
+        dk.nframes = 1;
+        dk.frame_stride = (int64_t)ctx->height * ctx->width;
+        rc = ai_make_frame_map(ctx, dk, tl.tile_h, &dmap);
+        if (rc != AI_OK) return rc;
+    }
+    const CUtensorMap *dm = held ? &dmap : nullptr;
     rc = AI_EINVAL;
     switch (a.dtype) {
-    case AI_F32: rc = launch_stream_dt<AI_F32>(ctx, map, first, p, smem, grid, st); break;
-    case AI_I32: rc = launch_stream_dt<AI_I32>(ctx, map, first, p, smem, grid, st); break;
-    case AI_U32: rc = launch_stream_dt<AI_U32>(ctx, map, first, p, smem, grid, st); break;
+    case AI_F32: rc = launch_stream_dt<AI_F32>(ctx, map, dm, first, p, smem, grid, st); break;
+    case AI_I32: rc = launch_stream_dt<AI_I32>(ctx, map, dm, first, p, smem, grid, st); break;
+    case AI_U32: rc = launch_stream_dt<AI_U32>(ctx, map, dm, first, p, smem, grid, st); break;
     default: break;
     }
     if (rc == AI_OK) {
