@@ -43,8 +43,9 @@ struct StreamParams {
     int tile_h, ntiles, nslot;
     int stages, mat_stage_bytes, img_stage_bytes, hdr_bytes;
     int tile_bytes;              // bytes of a frame tile (= img_stage_bytes without held corrections)
-    int dk;                      // held corrections: the dark tile lies dk bytes behind the frame tile (a multiple of
-                                 // 1024: same 128-byte swizzle phase), img_stage_bytes = 2 dk
+    int dk;                      // held corrections: the dark tiles of all stages follow the frame tiles of all stages; a
+                                 // stage's dark tile lies dk = stages x tile_bytes behind its frame tile (a multiple of 1024:
+                                 // same 128-byte swizzle phase); img_stage_bytes = 2 tile_bytes
     int dyn_base;                // rank of the first tile handed out by ticket (the ones before are dealt statically)
     int launch_index;            // launches of this context so far, modulo 8 (development trace only)
     int track_all;               // float frames: every block skips non-finite pixels and accumulates count
@@ -356,7 +357,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
                                                                          const __grid_constant__ StreamFirstDescs first,
                                                                          const StreamParams p)
 {
-    // [tile stages][barriers, per-stage tile descriptors][matrix stages]
+    // [frame tile stages (, HELD: dark tile stages)][barriers, per-stage tile descriptors][matrix stages]
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *img_base = smem;
     unsigned char *hdr = smem + (size_t)p.stages * p.img_stage_bytes;
@@ -380,7 +381,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
         bulk_g2s(mat_base + (size_t)stage * p.mat_stage_bytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y, full + stage);
     };
     auto issue_tile = [&](int stage, const int4 &d) {
-        unsigned char *tile = img_base + (size_t)stage * p.img_stage_bytes;
+        unsigned char *tile = img_base + (size_t)stage * p.tile_bytes;
         const int ty = d.z >> 16, tx = d.z & 0xffff;
         tma_box(tile, &tmap, tx * kTileW, ty * p.tile_h, 0, full + stage);
         tma_box(tile + p.tile_bytes / 2, &tmap, tx * kTileW + 32, ty * p.tile_h, 0, full + stage);
@@ -404,7 +405,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
     //   otherwise nothing but static data (barriers, tensor map, first blobs) is touched before griddepcontrol.wait.
     if (threadIdx.x == 0) {
         // the packed rebase needs every tile buffer inside the first 64 KB of the shared window
-        if (smem_u32(img_base) + (unsigned)(p.stages * p.img_stage_bytes) > 0x10000u) __trap();
+        if (smem_u32(img_base) + (unsigned)(p.stages * p.tile_bytes) > 0x10000u) __trap();
         for (int s = 0; s < kStreamMaxStages; ++s) {
             mbar_init(full + s, 1);
             mbar_init(empty + s, kStreamCons);
@@ -515,7 +516,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
             if (firstb < d.w) {
                 const unsigned char *blob = mat_base + (size_t)r.stage * p.mat_stage_bytes;
                 const unsigned *bh = reinterpret_cast<const unsigned *>(blob) + 1;
-                const unsigned rebase = (smem_u32(img_base + (size_t)r.stage * p.img_stage_bytes) & 0xffffu) * 0x10001u;
+                const unsigned rebase = (smem_u32(img_base + (size_t)r.stage * p.tile_bytes) & 0xffffu) * 0x10001u;
                 for (int b = firstb; b < d.w; b += kStreamCons) {
                     const unsigned h = bh[b];
                     if constexpr (HELD) {
@@ -754,15 +755,16 @@ static bool stream_plan(const ai_ctx *ctx, int grid, StreamParams *p, bool held 
 {
     const TiledLayout &tl = ctx->tl;
     p->tile_bytes = tl.tile_h * kTileW * 4;
-    p->dk = held ? ai_align_up(p->tile_bytes, 1024) : 0;
-    p->img_stage_bytes = held ? 2 * p->dk : p->tile_bytes;
+    p->img_stage_bytes = held ? 2 * p->tile_bytes : p->tile_bytes;
     p->mat_stage_bytes = ai_align_up(tl.max_blob_bytes + 1024, 1024);     // slack: the look-ahead reads past a blob's end
     p->hdr_bytes = ai_align_up(kStreamBarBytes, 1024);
     int stages = (kPipeSmemBudget - p->hdr_bytes) / (p->img_stage_bytes + p->mat_stage_bytes);
     if (stages > kStreamMaxStages) stages = kStreamMaxStages;
     if (ctx->tune.stream_stages > 0 && stages > ctx->tune.stream_stages) stages = ctx->tune.stream_stages;
-    while (stages * p->img_stage_bytes > 0xf000) --stages;    // tile buffers stay inside the first 64 KB (packed rebase)
+    while (stages * p->tile_bytes > 0xf000) --stages;    // frame tile buffers stay inside the first 64 KB (packed rebase)
     p->stages = stages;
+    p->dk = held ? stages * p->tile_bytes : 0;
+    if (held && p->tile_bytes % 1024 != 0) return false;
     return stages >= 2;
 }
 

@@ -302,6 +302,7 @@ static int launch_prepass_stream(ai_ctx *ctx, const FrameArgs &a, int vec_ok, in
     b.frame_stride = (int64_t)ctx->height * b.row_pitch;
     b.dark = b.flat = b.solidangle = b.polarization = nullptr;
     b.mask = nullptr;
+    b.held = false;              // (a held set reached this pass as a dark current and a denominator)
     const int may_be_invalid = a.dark || a.flat || a.solidangle || a.polarization || a.mask || a.dtype == AI_F32;
     const void *used = nullptr;
     rc = ai_launch_stream_stage1(ctx, b, 1, may_be_invalid, 1, st, handled, &used);
