@@ -84,6 +84,24 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
                                                if c.corrections else
                                                {"partial_records_written_and_read_back": 2 * 16 * info["nslot"]}),
                                            "layout": info}
+        if name == "cfg3":
+            # the same frames against HELD corrections (ai_hold_corrections): the division and the mask are folded into a
+            # copy of the matrix once, the single-frame kernel loads the dark tile beside the frame tile -- no pre-pass
+            for it in its:
+                it.hold_corrections(*corr)
+            trh = BM.Train(torch, B, its, fdev, (None,) * 5)
+            trh.warm_up(steps, 3 * steps, max_trains=12)
+            medh, _, launches_h = trh.measure(steps, 5)
+            msh = medh / steps
+            ab_h = c.npix * 4 + c.npix * 4 + B.ai_get_csr(its[0].ctx)[3] * 8 + (c.npt + 1) * 4 + 3 * c.npt * 4
+            ex["train_cfg3_held_corrections"] = {
+                "frames_per_s": 1e3 / msh, "ms_per_step": msh, "launches_per_step": launches_h / steps,
+                "algorithmic_bytes_of_the_per_call_path": ab_c, "frac_of_peak_on_those": ab_c / (msh * 1e-3) / 1e9 / peak_gbs,
+                "bytes_this_path_needs": ab_h, "frac_of_peak_on_its_own_bytes": ab_h / (msh * 1e-3) / 1e9 / peak_gbs,
+                "note": "frame + held dark current (4 B per pixel each) + matrix + outputs; flat, solid angle, polarisation "
+                        "and mask are not read per frame"}
+            for it in its:
+                it.hold_corrections()
         if name == "cfg5":
             ex["cfg5_layouts_and_accumulators"] = cfg5_table(torch, B, BM, c, fr, its[0], fdev, flush, peak_gbs)
         for it in its:
@@ -214,9 +232,23 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
         "frames_per_s": 256 / (ms3 * 1e-3), "ms_per_batch": ms3, "us_per_frame": ms3 * 1e3 / 256,
         "launches_per_call": B.ai_last_launch_count(it.ctx), "algorithmic_bytes": ab3,
         "frac_of_peak": ab3 / (ms3 * 1e-3) / 1e9 / peak_gbs,
-        "kernel": "fl_batch_kernel, corrected variant (the loaders apply dark / flat / solid angle / polarisation / mask as "
-                  "they stage a tile)",
+        "kernel": "fl_batch_kernel, corrected variant (per call: validity, scale and dark per pixel, the blobs with the "
+                  "coefficients scaled, the static count; the loaders subtract the dark current as they stage a tile)",
         "note": "the same frames one by one (extras.train_cfg3_tiled_kahan) take 45 us each"}
+    it.hold_corrections(*cor3)
+    for _ in range(2):
+        it.integrate1d_batch(fb3, out=out3)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(3):
+        it.integrate1d_batch(fb3, out=out3)
+    e1.record()
+    torch.cuda.synchronize()
+    ms3h = e0.elapsed_time(e1) / 3
+    ex["batch_cfg3_256_frames_held_corrections"] = {
+        "frames_per_s": 256 / (ms3h * 1e-3), "ms_per_batch": ms3h, "us_per_frame": ms3h * 1e3 / 256,
+        "launches_per_call": B.ai_last_launch_count(it.ctx),
+        "note": "ai_hold_corrections: the scaled blobs and the static count are kept from call to call"}
     it.close()
     del fb3, out3, cor3
     # bidimensional integration of the headline frame: 360 azimuthal x 500 radial bins

@@ -2,6 +2,7 @@
 
     python -m paper_1412_6367_b200.profile_cases cfg4_batch [--calls 3]      # BASELINE.json configs[3]: 1024 int32 frames per call
     python -m paper_1412_6367_b200.profile_cases cfg3 [--calls 12]           # configs[2]: every correction array + mask
+    python -m paper_1412_6367_b200.profile_cases cfg3_held [--calls 12]      # the same against held corrections (ai_hold_corrections)
     python -m paper_1412_6367_b200.profile_cases cfg2_batch64                # 64 frames of configs[1] per call
     python -m paper_1412_6367_b200.profile_cases cake2                       # 2048^2 into 360 x 500 bins
 
@@ -19,7 +20,7 @@ from . import workloads as W
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("case", choices=["cfg4_batch", "cfg3", "cfg2_batch64", "cake2"])
+    ap.add_argument("case", choices=["cfg4_batch", "cfg3", "cfg3_held", "cfg2_batch64", "cake2"])
     ap.add_argument("--calls", type=int, default=0)
     args = ap.parse_args()
     B.lib()
@@ -40,7 +41,7 @@ def main():
         out = it.outputs(64)
         for _ in range(args.calls or 3):
             it.integrate1d_batch(frames, out=out)
-    elif args.case == "cfg3":
+    elif args.case in ("cfg3", "cfg3_held"):
         c = W.CONFIGS["cfg3"]
         fr = W.make_frame(c)
         fdev = [torch.from_numpy(fr.image).to(dev) for _ in range(4)]
@@ -48,6 +49,10 @@ def main():
                      for a in (fr.dark, fr.flat, fr.solidangle, fr.polarization, fr.mask))
         its = [B.Integrator(c, device=dev) for _ in range(3)]
         outs = [it.outputs() for it in its]
+        if args.case == "cfg3_held":
+            for it in its:
+                it.hold_corrections(*corr)
+            corr = (None,) * 5
         for k in range(args.calls or 12):
             its[k % 3].integrate1d(fdev[k % 4], *corr, out=outs[k % 3])
     else:
