@@ -100,6 +100,19 @@ __global__ void __launch_bounds__(256) hold_scale_tiled_kernel(int ntiles, const
 
 }  // namespace
 
+// the derived per-pixel arrays of one set of correction arrays (den_out may be NULL)
+int ai_launch_corr_prep(ai_ctx *ctx, const float *dark, const float *flat, const float *solidangle, const float *polarization,
+                        const uint8_t *mask, uint8_t *gone, float *scale, float *dark_out, uint32_t *keep, float *den_out,
+                        cudaStream_t st)
+{
+    const int64_t npix = (int64_t)ctx->height * ctx->width;
+    const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
+    const Corrections cor{dark, flat, solidangle, polarization, mask};
+    hold_prep_kernel<<<sms * 8, 256, 0, st>>>(npix, cor, gone, scale, dark_out, keep, den_out);
+    AI_CUDA(ctx, cudaGetLastError());
+    return AI_OK;
+}
+
 void ai_release_held(ai_ctx *ctx)
 {
     HeldCorrections &h = ctx->held;
@@ -111,10 +124,8 @@ void ai_release_held(ai_ctx *ctx)
 int ai_hold_build(ai_ctx *ctx, const float *dark, const float *flat, const float *solidangle, const float *polarization,
                   const uint8_t *mask, cudaStream_t st)
 {
-    const Corrections cor{dark, flat, solidangle, polarization, mask};
     HeldCorrections &h = ctx->held;
     const int64_t npix = (int64_t)ctx->height * ctx->width;
-    const int sms = ctx->sm_count > 0 ? ctx->sm_count : 148;
     h.on = false;
     h.fl_ready = false;
     if (!h.gone) AI_CUDA(ctx, cudaMalloc(&h.gone, (size_t)npix));
@@ -124,9 +135,9 @@ int ai_hold_build(ai_ctx *ctx, const float *dark, const float *flat, const float
         h.keep = reinterpret_cast<uint32_t *>(h.scale + 2 * npix);
         h.den = h.scale + 3 * npix;
     }
-    hold_prep_kernel<<<sms * 8, 256, 0, st>>>(npix, cor, h.gone, h.scale, h.dark, h.keep, h.den);
-    AI_CUDA(ctx, cudaGetLastError());
-    h.has_den = cor.flat || cor.solidangle || cor.polarization || cor.mask;
+    int rc = ai_launch_corr_prep(ctx, dark, flat, solidangle, polarization, mask, h.gone, h.scale, h.dark, h.keep, h.den, st);
+    if (rc != AI_OK) return rc;
+    h.has_den = flat || solidangle || polarization || mask;
     const TiledLayout &tl = ctx->tl;
     h.tl_ready = false;
     if (ctx->npt_azim == 0 && tl.blob && tl.ntiles > 0 && tl.blob_bytes > 0) {      // (whatever ai_set_options says now)

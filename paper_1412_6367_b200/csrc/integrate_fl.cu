@@ -482,37 +482,14 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
     }
 }
 
-// Corrected batches, once per call.  (1) fl_prep_kernel: per pixel, the byte "invalid for every frame" (masked, zero /
-// non-finite denominator or reciprocal, non-finite dark current), the factor its coefficients take (the reciprocal of
-// flat x solid angle x polarisation, 0 for an invalid pixel), the dark current the loaders subtract (0 for an invalid
-// pixel) and the keep word they AND float frames with (0 for an invalid pixel, else all ones).  (2) fl_scale_blob_kernel:
-// the call's copy of the tile blobs with every coefficient multiplied by its pixel's factor.  (3)
-// fl_static_count_kernel: the count every frame of the call starts from -- the sum of a row's coefficients over the
+// Corrected batches, once per call.  (1) ai_launch_corr_prep (hold.cu): per pixel, the byte "invalid for every frame"
+// (masked, zero / non-finite denominator or reciprocal, non-finite dark current), the factor its coefficients take (the
+// reciprocal of flat x solid angle x polarisation, 0 for an invalid pixel), the dark current the loaders subtract (0 for
+// an invalid pixel) and the keep word they AND float frames with (0 for an invalid pixel, else all ones).
+// (2) fl_scale_blob_kernel: the call's copy of the tile blobs with every coefficient multiplied by its pixel's factor.
+// (3) fl_static_count_kernel: the count every frame of the call starts from -- the sum of a row's coefficients over the
 // pixels that are not invalid for every frame; one block per row (fp64, fixed order; a row with nothing but such pixels
-// gives exactly 0).
-__global__ void __launch_bounds__(256) fl_prep_kernel(int64_t npix, Corrections cor, uint8_t *__restrict__ gone,
-                                                      float *__restrict__ scale, float *__restrict__ dark_call,
-                                                      uint32_t *__restrict__ keep)
-{
-    const bool has_den = cor.flat || cor.solidangle || cor.polarization;
-    for (int64_t px = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; px < npix; px += (int64_t)gridDim.x * blockDim.x) {
-        bool g = cor.mask && __ldg(cor.mask + px) != 0;
-        float sc = 1.0f;
-        if (has_den) {
-            float den = cor.flat ? __ldg(cor.flat + px) : 1.0f;
-            den *= cor.solidangle ? __ldg(cor.solidangle + px) : 1.0f;
-            den *= cor.polarization ? __ldg(cor.polarization + px) : 1.0f;
-            sc = __frcp_rn(den);
-            g = g || den == 0.f || !finite_f(den) || !finite_f(sc);
-        }
-        const float dk = cor.dark ? __ldg(cor.dark + px) : 0.f;
-        g = g || !finite_f(dk);
-        gone[px] = g ? 1 : 0;
-        scale[px] = g ? 0.f : sc;
-        dark_call[px] = g ? 0.f : dk;
-        keep[px] = g ? 0u : 0xffffffffu;
-    }
-}
+// gives exactly 0).  With held corrections (ai_hold_corrections) all three are done once and kept.
 
 // one block per tile: header and records copied, pairs {c0, c1, pos0, pos1} scaled (pos = 8 x pixel within the tile)
 __global__ void __launch_bounds__(128) fl_scale_blob_kernel(const int4 *__restrict__ tile_desc,
@@ -721,8 +698,9 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
         float *dark_call = fl.scale + npix;
         uint32_t *keep = reinterpret_cast<uint32_t *>(fl.scale + 2 * npix);
         if (!fl.blob_call) AI_CUDA(ctx, cudaMalloc(&fl.blob_call, (size_t)fl.blob_bytes));
-        const Corrections cor{a.dark, a.flat, a.solidangle, a.polarization, a.mask};
-        fl_prep_kernel<<<sms * 8, 256, 0, st>>>(npix, cor, fl.gone, fl.scale, dark_call, keep);
+        rc = ai_launch_corr_prep(ctx, a.dark, a.flat, a.solidangle, a.polarization, a.mask, fl.gone, fl.scale, dark_call, keep,
+                                 nullptr, st);
+        if (rc != AI_OK) return rc;
         fl_scale_blob_kernel<<<fl.ntiles, 128, 0, st>>>(fl.tile_desc, fl.blob, fl.scale, ctx->width, ctx->height, fl.blob_call);
         fl_static_count_kernel<<<ctx->npt, 128, 0, st>>>(ctx->npt, ctx->indptr, ctx->indices, ctx->data, fl.gone, fl.call_csum);
         AI_CUDA(ctx, cudaGetLastError());
