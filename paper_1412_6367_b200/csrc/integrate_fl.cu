@@ -44,14 +44,17 @@ struct FlParams {
     const int4 *tile_desc, *chunk_desc;
     const uint8_t *chunk_owner;
     const unsigned char *blob;                       // (corrected variant: the copy with the coefficients scaled for this call)
-    const unsigned char *blob_orig;                  // the layout's own blobs
     const unsigned char *frames;
     int64_t frame_stride_bytes;
     int height, width;
     int nframes, ngroups, nitems;
     int stages, stage_bytes, prefetch_ahead;
     const float *dark;                               // corrected variant: the call's dark current and keep words, per pixel
-    const uint32_t *keep;                            // (fl_prep_kernel)
+    const uint32_t *keep;                            // (hold.cu: hold_prep_kernel)
+    const unsigned char *blob_orig;                  // the layout's own blobs
+    int64_t pad_;                                    // measured: with this struct at exactly 128 bytes ptxas 12.9 allocates the
+                                                     // plain variant's loader loop differently (a spill, 16 more instructions)
+                                                     // and 1024 cfg4 frames take 1.205 instead of 1.14 ms
     float2 *part_s;
     unsigned long long *part_d;                      // float frames and corrected batches only
     int64_t nfp;                                     // frames rounded up to a multiple of kFlFrames
@@ -234,7 +237,6 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
         // 128-bit loads of rows 4 h .. 4 h + 3 of a tile for the lane's two frames; `src` = the lane's piece of row 0
         struct Src {
             const unsigned char *p;
-            int64_t pix;                 // index of the lane's first pixel of row 0 (corrections)
             int rows;                    // rows of the tile inside the image
             bool in_a, in_b, in_x;
         };
@@ -244,7 +246,6 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
             const int fa = w.group * kFlFrames + 2 * cl;
             Src s;
             s.p = p.frames + (int64_t)fa * p.frame_stride_bytes + ((int64_t)y0 * p.width + x) * 4;
-            s.pix = (int64_t)y0 * p.width + x;
             s.rows = p.height - y0;
             s.in_x = x < p.width;
             s.in_a = fa < p.nframes && s.in_x;
