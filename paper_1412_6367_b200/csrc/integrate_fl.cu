@@ -104,19 +104,14 @@ __device__ __forceinline__ void sts_f2(unsigned addr, float a, float b)
 {
     asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
 }
-// Waits of the frame-lane kernel: bounded (20 s of wall time) like mbar_wait.  EXIT (the corrected variant): a timed-out
-// wait raises its error with a store to address 0 followed by exit instead of trap: with a trap instruction in a branch, ptxas keeps that
-// branch at the launch-time register count and ignores its setmaxnreg (measured: the loaders spilled their in-flight
-// loads to local memory at 80 registers and stalled on them every tile; without the trap they use up to 108, no spills).
-// (A try_wait with a long suspend-time hint was measured to oversleep by microseconds once the waiting side is the
-// faster one: plain try_wait.)
-template <bool EXIT>
+// Waits of the frame-lane kernel: bounded (20 s of wall time) like mbar_wait, but a timed-out wait raises its error with a
+// store to address 0 followed by exit instead of trap.  With a trap instruction in a branch, ptxas keeps that branch at
+// the launch-time register count and ignores its setmaxnreg (measured on the corrected variant: the loaders spilled their
+// in-flight 128-bit loads to local memory at 80 registers and stalled on them every tile, 12.2 us per cfg3 frame; without
+// the trap they use up to 108 registers, no spills, 8.6 us).  (A try_wait with a long suspend-time hint was measured to
+// oversleep by microseconds once the waiting side is the faster one: plain try_wait.)
 __device__ __forceinline__ void mbar_wait_fl(uint64_t *bar, uint32_t parity)
 {
-    if constexpr (!EXIT) {
-        mbar_wait(bar, parity);
-        return;
-    }
     unsigned long long t0 = 0;
     for (uint32_t spin = 1; !mbar_try_wait(bar, parity); ++spin) {
         if ((spin & 0xfffu) == 0) {
@@ -206,11 +201,11 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
     fl_enter(cur, p);
     if (warp < kFlLoad) {
         // ===== loaders =================================================================================================
-        // two passes of 128-bit loads in registers.  (ptxas follows setmaxnreg only in the corrected variant, whose waits
-        // carry no trap -- see mbar_wait_fl; the plain variant's loaders fit the launch-time 80 registers but for one
-        // 4-byte spill, and were measured 5-10 % slower when given more: 80 / 88 / 96 / 104 / 112 -> 1.17 / 1.25 / 1.23 /
-        // 1.25 / 1.28 ms per 1024 frames of configs[3].)
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
+        // two passes of 128-bit loads in registers.  The corrected variant takes what it needs (108); the plain one is held
+        // at 80: it was measured 5-10 % slower with more (80 / 88 / 96 / 104 / 112 registers: 1.17 / 1.25 / 1.23 / 1.25 / 1.28 ms per
+        // 1024 frames of configs[3] before the last round of changes; ptxas schedules the loads differently)
+        if constexpr (COR) asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
+        else asm volatile("setmaxnreg.inc.sync.aligned.u32 80;");
         // lane = (lane of the consumers, 16-byte piece of a tile row): lanes 4 lw .. 4 lw + 3 x pieces 0..7, so that the
         // 8 lanes of a 128-bit load phase read one 128-byte line.  Stores are 64-bit (one pixel of the lane's two
         // frames); pieces 4..7 store their pixels in the order 2, 3, 0, 1, which puts the 16 lanes of a store phase into
@@ -343,7 +338,7 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
             Src sn{};
             if (!nxt.done) sn = locate(nxt, dn);
             unsigned char *stage = stage0 + (size_t)ring.stage * p.stage_bytes;
-            if (issued >= p.stages) mbar_wait_fl<COR>(empty + ring.stage, ring.parity ^ 1u);
+            if (issued >= p.stages) mbar_wait_fl(empty + ring.stage, ring.parity ^ 1u);
             if (lw == 0 && lane == 0) {
                 mbar_arrive_expect_tx(full + ring.stage, (uint32_t)d.y);
                 bulk_g2s(stage + kFlImgBytes, p.blob + (size_t)d.x * 16, (uint32_t)d.y, full + ring.stage);
@@ -389,7 +384,7 @@ __global__ void __launch_bounds__(kFlThreads, 1) fl_batch_kernel(const __grid_co
             const int item = cur.item, group = cur.group;
             const int fa = group * kFlFrames + 2 * lane;
             while (!cur.done && cur.item == item) {
-                mbar_wait_fl<COR>(full + ring.stage, ring.parity);
+                mbar_wait_fl(full + ring.stage, ring.parity);
                 const unsigned char *stage = stage0 + (size_t)ring.stage * p.stage_bytes;
                 const unsigned char *blob = stage + kFlImgBytes;
                 const unsigned short *wptr = reinterpret_cast<const unsigned short *>(blob);
