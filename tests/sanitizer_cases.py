@@ -91,6 +91,16 @@ def run_cfg(cfg, switches):
                 torch.cuda.synchronize()
                 check("tiled/kahan/masked batch, frame 4", i[4].cpu().numpy(),
                       O.integrate1d(cfg, W.Frame(image=frames[4], mask=frc.mask)))
+                # the corrected frame again, against the same arrays held by the context (hold.cu): a chain of calls
+                integ.hold_corrections(*args[1:])
+                for _ in range(3):
+                    i, s, c = integ.integrate1d(args[0])
+                torch.cuda.synchronize()
+                check("tiled/kahan/held corrections", i.cpu().numpy(), wantc)
+                i, s, c = integ.integrate1d_batch(dev(np.stack([frc.image] * 4)))
+                torch.cuda.synchronize()
+                check("tiled/kahan/held corrections, batch of 4, frame 2", i[2].cpu().numpy(), wantc)
+                integ.hold_corrections()
             integ.close()
 
 
