@@ -273,6 +273,30 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
     ex["train_cake2_360x500_bins"] = {"frames_per_s": 1e3 / ms, "ms_per_step": ms, "nnz": nnz2, "algorithmic_bytes": ab2,
                                       "frac_of_peak": ab2 / (ms * 1e-3) / 1e9 / peak_gbs,
                                       "layout": B.ai_get_layout_info(its[0].ctx)}
+    # the same with the correction arrays of cfg3 (same detector size): per call, and held by the contexts
+    fr3c = W.make_frame(W.CONFIGS["cfg3"])
+    corc = tuple(torch.from_numpy(a).to(device) for a in (fr3c.dark, fr3c.flat, fr3c.solidangle, fr3c.polarization, fr3c.mask))
+
+    def cake_train_corrected(k, args):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(k):
+            its[i % 3].integrate2d(frames_dev[i % len(frames_dev)], *args, out=outs[i % 3])
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / k
+
+    for _ in range(4):
+        cake_train_corrected(50, corc)
+    ms_pc = statistics.median(cake_train_corrected(100, corc) for _ in range(5))
+    for it in its:
+        it.hold_corrections(*corc)
+    for _ in range(4):
+        cake_train_corrected(50, (None,) * 5)
+    ms_h = statistics.median(cake_train_corrected(100, (None,) * 5) for _ in range(5))
+    ex["train_cake2_all_corrections"] = {"per_call_arrays_ms_per_step": ms_pc, "held_corrections_ms_per_step": ms_h,
+                                         "held_launches_per_step": B.ai_last_launch_count(its[0].ctx)}
+    del corc
     for it in its:
         it.close()
     ex["build_vs_oracle"] = build_times(torch, B, device)

@@ -140,7 +140,7 @@ int ai_hold_build(ai_ctx *ctx, const float *dark, const float *flat, const float
     h.has_den = flat || solidangle || polarization || mask;
     const TiledLayout &tl = ctx->tl;
     h.tl_ready = false;
-    if (ctx->npt_azim == 0 && tl.blob && tl.ntiles > 0 && tl.blob_bytes > 0) {      // (whatever ai_set_options says now)
+    if (tl.blob && tl.ntiles > 0 && tl.blob_bytes > 0) {      // (1D and 2D; whatever ai_set_options says now)
         if (!h.tl_blob) AI_CUDA(ctx, cudaMalloc(&h.tl_blob, (size_t)tl.blob_bytes));
         hold_scale_tiled_kernel<<<tl.ntiles, 256, 0, st>>>(tl.ntiles, tl.blob_desc, tl.blob, h.scale, ctx->width, ctx->height,
                                                           tl.tile_h, h.tl_blob);

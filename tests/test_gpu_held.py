@@ -254,7 +254,7 @@ def test_held_full_size_and_reproducible(torch, B, oracle, workloads):
 
 
 def test_held_2d(torch, B, oracle, workloads):
-    """A bidimensional context with a held set (the general kernels, (dark, denominator) pair)."""
+    """A bidimensional context with a held set: the same single-frame kernel on the held copy of the 2D matrix."""
     import math
     W = workloads
     cfg = W.scaled(W.tiny_config(80, 112, center_x=40.4, center_y=61.7, unit=W.R_MM, npt=33, name="held2d"), npt_azim=48)
@@ -266,6 +266,7 @@ def test_held_2d(torch, B, oracle, workloads):
     integ.hold_corrections(*_dev(torch, (dark, flat, solid, pol, mask)))
     i, s, c = integ.integrate2d(torch.from_numpy(img).cuda())
     torch.cuda.synchronize()
+    assert B.ai_last_launch_count(integ.ctx) == 2
     umin, umax = oracle.pixel_bounds(cfg)
     u0, u1 = oracle.auto_range(umin, umax)
     lo, w = oracle.pixel_chi_bounds(cfg)
