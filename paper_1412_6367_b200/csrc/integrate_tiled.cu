@@ -395,6 +395,28 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
         // 32 or more plain 32-bit frames: the frame-lane kernel (integrate_fl.cu), both launches
         rc = ai_launch_fl(ctx, a, vec_ok, st, &handled);
         if (rc != AI_OK || handled) return rc;
+        // smaller batches with correction arrays, a mask or held corrections: frame by frame through the single-frame
+        // paths above -- measured 1.5 to 4 times faster than staging the corrections inside the general batched kernel
+        // (us per frame, 8 to 64 frames per call: cfg3 43 against 62-69, held 25 against 100; cfg2's matrix with cfg3's
+        // arrays 34 against 54-60, held 12.5 against 90)
+        if (a.nframes > 1 && (a.dark || a.flat || a.solidangle || a.polarization || a.mask) && !ctx->no_prepass &&
+            !ctx->no_stream && !ctx->no_tma && ai_stream_stages(ctx) >= 2) {
+            int launches = 0;
+            for (int f = 0; f < a.nframes; ++f) {
+                FrameArgs one = a;
+                one.nframes = 1;
+                one.image = static_cast<const char *>(a.image) + (size_t)f * (size_t)a.frame_stride * esz;
+                one.radial = nullptr;
+                one.intensity = a.intensity + (size_t)f * ctx->npt;
+                one.sum_signal = a.sum_signal + (size_t)f * ctx->npt;
+                one.count = a.count + (size_t)f * ctx->npt;
+                rc = ai_launch_tiled(ctx, one, st);
+                if (rc != AI_OK) return rc;
+                launches += ctx->last_launches;
+            }
+            ctx->last_launches = launches;
+            return AI_OK;
+        }
         rc = ensure_partials();
         if (rc != AI_OK) return rc;
         rc = ai_launch_bstream_stage1(ctx, a, vec_ok, st, &handled);          // batch of plain 32-bit frames

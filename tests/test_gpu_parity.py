@@ -554,7 +554,12 @@ def test_batch_equals_single_frame_calls_bit_for_bit(torch, B, oracle, workloads
     integ.close()
 
 
-def test_batch_with_mask_takes_the_general_kernel(torch, B, oracle, workloads):
+@pytest.mark.parametrize("path", ["frame by frame", "general kernel"])
+def test_small_batch_with_mask(torch, B, oracle, workloads, monkeypatch, path):
+    """A small batch with a mask: frame by frame through the pre-pass + single-frame kernel (3 launches per frame), or,
+    without the pre-pass (AZINT_NO_PREPASS=1), the general batched kernel that stages the corrections itself."""
+    if path == "general kernel":
+        monkeypatch.setenv("AZINT_NO_PREPASS", "1")
     cfg = workloads.tiny_config(130, 200, center_x=60.0, center_y=70.0, unit=workloads.TTH_DEG, npt=150,
                                 distance_m=0.03, name="batch_mask")
     rng = np.random.default_rng(3)
@@ -563,6 +568,7 @@ def test_batch_with_mask_takes_the_general_kernel(torch, B, oracle, workloads):
     integ = B.Integrator(cfg)
     i, s, c = integ.integrate1d_batch(torch.from_numpy(frames).cuda(), mask=torch.from_numpy(mask).cuda())
     torch.cuda.synchronize()
+    assert B.ai_last_launch_count(integ.ctx) == (12 if path == "frame by frame" else 2)
     for f in range(4):
         want = _oracle_profile(oracle, cfg, workloads.Frame(image=frames[f], mask=mask))
         got = {"intensity": i[f].cpu().numpy(), "sum_signal": s[f].cpu().numpy(), "count": c[f].cpu().numpy()}
