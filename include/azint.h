@@ -178,15 +178,18 @@ int ai_integrate2d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *
  *   frames                     frame f starts at element f * frame_stride_elems (>= height*width)
  *   intensity, sum_signal,
  *   count                      float32[nframes][npt], row-major
- * Enqueues on `cuda_stream`; does not synchronise -- with one exception: the first batch of 96 or more 32-bit frames
- * that the frame-lane kernel takes (1D context, Kahan accumulation, every array on a 16-byte boundary,
- * and either correction arrays / a mask or a matrix with more than ~2.2 entries per pixel) builds the frame-lane layout
- * of the matrix (one-time, synchronises `cuda_stream`; see ai_get_batch_layout_info), and a larger batch than any before
- * re-allocates scratch (cudaFree synchronises the device).  In that kernel a corrected value is (I - dark) times the
- * rounded reciprocal of flat * solidangle * polarization (one rounding more than the division of the other paths).  A frame's profiles do not depend on where it sits in
- * a batch, but they are not bit-identical between the kernels a batch may take (different fixed summation orders).
- * Batches of fewer than 96 frames that carry correction arrays or a mask (or use a held set) are integrated frame by
- * frame by the single-frame kernels (measured faster than correcting inside a batched kernel): 2 or 3 launches per frame.
+ * Enqueues on `cuda_stream`; does not synchronise -- with one exception: the first batch that sends 32 or more 32-bit
+ * frames to the frame-lane kernel (1D context, Kahan accumulation, every array on a 16-byte boundary)
+ * builds the frame-lane layout of the matrix (one-time, synchronises `cuda_stream`; see ai_get_batch_layout_info), and a
+ * larger batch than any before re-allocates scratch (cudaFree synchronises the device).
+ * Which kernels a batch takes is decided by measured cost: the frame-lane kernel takes the leading groups
+ * of 64 frames and the remaining frames if they are many enough (plain frames 44 or 60, frames with per-call correction
+ * arrays 14, with held corrections 24); the rest goes to the slice-per-lane batch kernel (plain 32-bit frames) or frame
+ * by frame through the single-frame kernels (correction arrays, a mask, held corrections, 16-bit pixels: 2 or 3 launches
+ * per frame, measured faster than correcting inside a batched kernel).  In the frame-lane kernel and with held
+ * corrections a corrected value is (I - dark) times the rounded reciprocal of flat * solidangle * polarization (one
+ * rounding more than the division of the other paths).  A frame's profiles do not depend on where it sits among the
+ * frames one kernel takes, but they are not bit-identical between the kernels (different fixed summation orders).
  * Errors as ai_integrate1d. */
 int ai_integrate1d_batch(ai_ctx *ctx, const void *frames, ai_dtype dtype, int nframes, int64_t frame_stride_elems,
                          const float *dark, const float *flat, const float *solidangle, const float *polarization,

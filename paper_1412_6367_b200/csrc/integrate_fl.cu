@@ -35,7 +35,7 @@ constexpr int kFlLaneBytes = kFlTilePix * 8 + 8;     // a lane's two frames of t
 constexpr int kFlImgBytes = 32 * kFlLaneBytes;
 constexpr int kFlPassRows = 4;                       // rows of the tile a loader holds in registers at a time
 constexpr int kFlPrefetchAhead = 3;                  // tiles between the L2 prefetch and the loads
-constexpr int kFlMinFrames = 96;
+constexpr int kFlMinFrames = 32;         // a context builds the layout for a batch that sends at least this many frames here
 constexpr int kFlCorBytes = 2 * kFlTilePix * 4;                  // corrected variant, per stage: the tile's dark current
                                                                  // (float) and keep words (float frames)
 constexpr float kFlFix = 1099511627776.0f;           // 2^40: weights of invalid pixels as integers
@@ -594,22 +594,37 @@ int launch_fl(ai_ctx *ctx, const CUtensorMap &map, const FlParams &p, size_t sme
 
 }  // namespace
 
-// Batches of at least kFlMinFrames plain 32-bit frames, Kahan accumulation, 1D: *handled = true when the frame-lane
-// kernel took the call (both launches).  The first such call of a context builds the layout (one-time; synchronises
-// `st`).
-int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, bool *handled)
+// Batches of 32-bit frames, Kahan accumulation, 1D: *taken = the number of leading frames of the batch the frame-lane
+// kernel took (both launches); the caller sends the rest through the other kernels.  The first call that takes frames
+// builds the layout (one-time; synchronises `st`).
+//
+// Which frames (measured, us per frame on B200).  The kernel works on groups of 64 frames and a group costs
+// nearly the same full or half empty (cfg3's matrix: 365 + 0.7 per frame; cfg2's: 225 + 1.3 per frame), so full groups
+// always go here and the frames behind the last full group only if there are enough of them to beat the alternative:
+//   plain frames, against the slice-per-lane batch kernel (cfg3 9.8, cfg2 5.1, cfg5 29 per frame): 44 frames on matrices
+//     with more than 2.2 entries per pixel, 60 below;
+//   frames with per-call correction arrays, against frame-by-frame calls (cfg3 43, cfg2's matrix 34): 14 frames;
+//   frames against held corrections, against frame-by-frame calls (cfg3 25, cfg2's matrix 12.5): 24 frames.
+// A context that has not built the layout yet builds it for 32 frames or more.  AZINT_FORCE_FL=1 takes every batch
+// (testing), AZINT_NO_FL=1 none.
+int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a0, int vec_ok, cudaStream_t st, int *taken)
 {
-    *handled = false;
-    if (a.nframes < 2 || ctx->no_fl || ctx->no_tma || ctx->no_stream || ctx->npt_azim > 0 ||
+    *taken = 0;
+    if (a0.nframes < 2 || ctx->no_fl || ctx->no_tma || ctx->no_stream || ctx->npt_azim > 0 ||
         ctx->accum != AI_ACC_F32_KAHAN || ctx->layout != AI_LAYOUT_TILED)
         return AI_OK;
-    // Where it pays (measured): batches of two groups of frames or more on matrices with more than
-    // ~2.2 entries per pixel -- below that the per-pixel cost of staging the frames outweighs the cheaper entries and
-    // the slice-per-lane kernel is as fast.  AZINT_FORCE_FL=1 takes every batch (testing).
-    const bool plain = !a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask;
-    // (batches with correction arrays: whatever the matrix -- the alternative is the general pipelined kernel)
-    if (!ctx->force_fl && (a.nframes < kFlMinFrames || (plain && (double)ctx->nnz < 2.2 * (double)ctx->height * ctx->width)))
-        return AI_OK;
+    const bool plain = !a0.dark && !a0.flat && !a0.solidangle && !a0.polarization && !a0.mask;
+    int take = a0.nframes;
+    if (!ctx->force_fl) {
+        const bool heavy = (double)ctx->nnz >= 2.2 * (double)ctx->height * ctx->width;
+        const int tail_min = !plain ? (a0.held ? 24 : 14) : (heavy ? 44 : 60);
+        const int full = a0.nframes / kFlFrames * kFlFrames, tail = a0.nframes - full;
+        take = full + (tail >= tail_min ? tail : 0);
+        if (!(ctx->fl.tried && ctx->fl.ok) && take < kFlMinFrames) take = 0;
+    }
+    if (take < 2) return AI_OK;
+    FrameArgs a = a0;
+    a.nframes = take;
     const bool is32 = a.dtype == AI_F32 || a.dtype == AI_I32 || a.dtype == AI_U32;
     // (vec_ok: every array, the correction arrays and the mask included, on its 4-pixel vector boundary)
     if (!is32 || !vec_ok || (reinterpret_cast<uintptr_t>(a.image) % 16) != 0) return AI_OK;
@@ -714,7 +729,7 @@ int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, b
     default: break;
     }
     if (rc != AI_OK) return rc;
-    *handled = true;
+    *taken = take;
     ctx->last_launches = launches + 1;
     if (ctx->stage1_only) return AI_OK;
     const dim3 g2((ctx->npt + 31) / 32, (a.nframes + 31) / 32);

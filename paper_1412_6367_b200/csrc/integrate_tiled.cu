@@ -392,15 +392,33 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
             rc = launch_prepass_stream(ctx, a, vec_ok, 0, st, &handled);
             if (rc != AI_OK || handled) return rc;
         }
-        // 32 or more plain 32-bit frames: the frame-lane kernel (integrate_fl.cu), both launches
-        rc = ai_launch_fl(ctx, a, vec_ok, st, &handled);
-        if (rc != AI_OK || handled) return rc;
-        // smaller batches with correction arrays, a mask or held corrections: frame by frame through the single-frame
-        // paths above -- measured 1.5 to 4 times faster than staging the corrections inside the general batched kernel
-        // (us per frame, 8 to 64 frames per call: cfg3 43 against 62-69, held 25 against 100; cfg2's matrix with cfg3's
-        // arrays 34 against 54-60, held 12.5 against 90)
-        if (a.nframes > 1 && (a.dark || a.flat || a.solidangle || a.polarization || a.mask) && !ctx->no_prepass &&
-            !ctx->no_stream && !ctx->no_tma && ai_stream_stages(ctx) >= 2) {
+        // batches of 32-bit frames: the frame-lane kernel (integrate_fl.cu) takes the groups of 64 frames it is faster on,
+        // the frames behind them continue below
+        int taken = 0;
+        rc = ai_launch_fl(ctx, a, vec_ok, st, &taken);
+        if (rc != AI_OK || taken == a.nframes) return rc;
+        if (taken > 0) {
+            const int launches = ctx->last_launches;
+            FrameArgs rest = a;
+            rest.nframes = a.nframes - taken;
+            rest.image = static_cast<const char *>(a.image) + (size_t)taken * (size_t)a.frame_stride * esz;
+            rest.intensity = a.intensity + (size_t)taken * ctx->npt;
+            rest.sum_signal = a.sum_signal + (size_t)taken * ctx->npt;
+            rest.count = a.count + (size_t)taken * ctx->npt;
+            rc = ai_launch_tiled(ctx, rest, st);
+            ctx->last_launches += launches;
+            return rc;
+        }
+        rc = ensure_partials();
+        if (rc != AI_OK) return rc;
+        rc = ai_launch_bstream_stage1(ctx, a, vec_ok, st, &handled);          // batch of plain 32-bit frames
+        // what is left of a batch -- frames with correction arrays, a mask or held corrections, 16-bit frames, buffers off
+        // the 16-byte boundaries: frame by frame through the single-frame paths above.  Measured 1.5 to 4 times faster
+        // than staging the corrections inside the general batched kernel (us per frame, 8 to 64 frames per call: cfg3 43
+        // against 62-69, held 25 against 100; cfg2's matrix with cfg3's arrays 34 against 54-60, held 12.5 against 90;
+        // plain uint16 frames 20 against 30-32)
+        if (rc == AI_OK && !handled && a.nframes > 1 && !ctx->no_prepass && !ctx->no_stream && !ctx->no_tma &&
+            ai_stream_stages(ctx) >= 2) {
             int launches = 0;
             for (int f = 0; f < a.nframes; ++f) {
                 FrameArgs one = a;
@@ -417,9 +435,6 @@ int ai_launch_tiled(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
             ctx->last_launches = launches;
             return AI_OK;
         }
-        rc = ensure_partials();
-        if (rc != AI_OK) return rc;
-        rc = ai_launch_bstream_stage1(ctx, a, vec_ok, st, &handled);          // batch of plain 32-bit frames
         if (rc == AI_OK && !handled) rc = ai_launch_pipe_stage1(ctx, a, vec_ok, st, &handled);
     }
     if (rc != AI_OK) return rc;

@@ -175,20 +175,29 @@ def test_fl_frame_stride_and_the_other_kernels_agree(torch, B, oracle, workloads
 def test_fl_full_size_geometries_sampled(torch, B, oracle, workloads, name):
     """The frame-lane kernel on the two large q-unit matrices at full size (BASELINE.json configs[2] and configs[4]
     geometries: 3000 / 5000 bins, 3.5 / 2.3 entries per pixel, the latter with the beam centre off the image), taken by
-    itself (no environment switch) on 96 plain float frames from a pool of two; sampled frames against the oracle."""
+    itself (no environment switch) on plain float frames from a pool of two; sampled frames against the oracle.
+    112 frames = a full group of 64 and a tail of 48, enough for the kernel to take the tail as well; with 96 frames the
+    tail of 32 goes to the slice-per-lane batch kernel (two more launches) -- same profiles, other summation order."""
     cfg = workloads.CONFIGS[name]
     base = workloads.make_frame(cfg).image
     pool = np.stack([base, base[::-1].copy() * np.float32(0.5)])
     dev = torch.from_numpy(pool).cuda()
-    frames = dev.repeat(48, 1, 1)
+    frames = dev.repeat(56, 1, 1)
     integ = B.Integrator(cfg)
     i, s, c = integ.integrate1d_batch(frames)
     torch.cuda.synchronize()
     assert B.ai_get_batch_layout_info(integ.ctx)["built"] == 1, "the frame-lane kernel did not take the batch"
-    for f in (0, 95):
+    assert B.ai_last_launch_count(integ.ctx) == 2
+    for f in (0, 111):
         want = _want(oracle, cfg, pool[f % 2])
         assert_profile(_row(i, s, c, f), want, what=f"{name} frame {f}")
-    assert torch.equal(i[0], i[94]) and torch.equal(s[1], s[95]) and torch.equal(c[0], c[64])
+    assert torch.equal(i[0], i[110]) and torch.equal(s[1], s[111]) and torch.equal(c[0], c[64])
+    i, s, c = integ.integrate1d_batch(frames[:96])
+    torch.cuda.synchronize()
+    assert B.ai_last_launch_count(integ.ctx) == 4           # frame-lane kernel + finish, slice-per-lane kernel + stage 2
+    for f in (63, 64, 95):
+        assert_profile(_row(i, s, c, f), _want(oracle, cfg, pool[f % 2]), what=f"{name} frame {f} of 96")
+    assert torch.equal(i[0], i[62]) and torch.equal(i[64], i[94]) and torch.equal(s[65], s[95])
     integ.close()
 
 
