@@ -130,34 +130,46 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
     nb = 64
     fb = torch.stack([frames_dev[k % len(frames_dev)] for k in range(nb)])
     outb = integ.outputs(nb)
-    for _ in range(2):
-        integ.integrate1d_batch(fb, out=outb)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(5):
-        integ.integrate1d_batch(fb, out=outb)
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / 5
+    import os
+
+    def time_batch64(it):
+        for _ in range(2):
+            it.integrate1d_batch(fb, out=outb)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(5):
+            it.integrate1d_batch(fb, out=outb)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / 5
+
+    ms = time_batch64(integ)                  # one full group of 64 frames: the frame-lane kernel
+    fl_info = B.ai_get_batch_layout_info(integ.ctx)
+    os.environ["AZINT_NO_FL"] = "1"
+    it_nofl = B.Integrator(cfg, device=device)
+    del os.environ["AZINT_NO_FL"]
+    ms_nofl = time_batch64(it_nofl)           # the slice-per-lane batch kernel on the same call
+    it_nofl.close()
     abb = nb * cfg.npix * 4 + nnz * 8 + (cfg.npt + 1) * 4 + nb * 3 * cfg.npt * 4
     info = B.ai_get_layout_info(integ.ctx)
     ex["batch_cfg2_64_frames"] = {"frames_per_s": nb / (ms * 1e-3), "ms_per_batch": ms, "us_per_frame": ms * 1e3 / nb,
                                   "mpix_per_s": nb * cfg.npix / (ms * 1e-3) / 1e6,
                                   "algorithmic_bytes": abb, "algorithmic_GBps": abb / (ms * 1e-3) / 1e9,
                                   "frac_of_peak": abb / (ms * 1e-3) / 1e9 / peak_gbs,
-                                  "extra_bytes_not_in_the_algorithmic_count":
-                                      {"partial_records_written_and_read_back": 2 * 16 * info["nslot"] * nb},
-                                  "kernel": "tiled_bstream_kernel (slices per lane; 64 frames and 1.9 entries per pixel are below "
-                                            "what the frame-lane kernel takes)",
-                                  "note": "ai_integrate1d_batch on 64 device-resident cfg2 frames; results are bit-identical "
-                                          "to the single-frame kernel's"}
+                                  "kernel": "fl_batch_kernel (one full group of 64 frames)" if fl_info.get("built") else
+                                            "tiled_bstream_kernel",
+                                  "slice_per_lane_kernel_AZINT_NO_FL": {
+                                      "ms_per_batch": ms_nofl, "us_per_frame": ms_nofl * 1e3 / nb,
+                                      "frac_of_peak": abb / (ms_nofl * 1e-3) / 1e9 / peak_gbs,
+                                      "partial_records_written_and_read_back": 2 * 16 * info["nslot"] * nb,
+                                      "note": "bit-identical to the single-frame kernel's results"},
+                                  "note": "ai_integrate1d_batch on 64 device-resident cfg2 frames"}
     del fb, outb
     # configs[3]: 1024 int32 frames of 1024x1024 in one batched call
     c4 = W.CONFIGS["cfg4"]
     pool = torch.from_numpy(W.make_frames(c4, 8)).to(device)
     frames = pool.repeat(c4.nframes // 8, 1, 1)
-    import os
 
     def time_cfg4(env):
         """ms per 1024-frame call (5 calls back to back after 2 warm-up calls) and the context, still open"""

@@ -534,9 +534,9 @@ def test_batch_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, nf
 
 
 def test_batch_equals_single_frame_calls_bit_for_bit(torch, B, oracle, workloads):
-    """BASELINE.json configs[1] frames through ai_integrate1d_batch (the launch bench.py's `batch_cfg2_64_frames`
-    times): every frame's profiles equal, bit for bit, what ai_integrate1d gives for it (same accumulation order in
-    both kernels), and a sampled frame matches the oracle."""
+    """BASELINE.json configs[1] frames through ai_integrate1d_batch in a small batch (the slice-per-lane batch kernel,
+    bench.py's `batch_cfg2_64_frames.slice_per_lane_kernel_AZINT_NO_FL`): every frame's profiles equal, bit for bit,
+    what ai_integrate1d gives for it (same accumulation order in both kernels), and a sampled frame matches the oracle."""
     cfg = workloads.CONFIGS["cfg2"]
     base = workloads.make_frame(cfg).image
     frames = np.stack([base * np.float32(s) for s in (1.0, 0.5, 2.0, 0.75, 3.0)])
