@@ -275,3 +275,20 @@ def test_held_2d(torch, B, oracle, workloads):
     got = {"intensity": i.cpu().numpy().ravel(), "sum_signal": s.cpu().numpy().ravel(), "count": c.cpu().numpy().ravel()}
     assert_profile(got, {k: np.asarray(want[k]).ravel() for k in got}, what="held 2d")
     integ.close()
+
+
+def test_held_with_split_normalisation(torch, B, oracle, workloads):
+    """ai_set_normalization(AI_NORM_SPLIT) against a held set: sum c (I - dark) over sum c (flat * solidangle *
+    polarization), the held set seen as a (dark, denominator) pair by the two passes."""
+    cfg = workloads.tiny_config(200, 264, unit=workloads.TTH_DEG, name="held5", **FITS)
+    rng = np.random.default_rng(61)
+    img = rng.poisson(90.0, size=(cfg.height, cfg.width)).astype(np.float32)
+    arrays = _arrays((cfg.height, cfg.width), 67)
+    umin, umax = oracle.pixel_bounds(cfg)
+    u0, u1 = oracle.auto_range(umin, umax)
+    want = oracle.integrate1d_bounds_split(umin, umax, cfg.npt, u0, u1, img, *arrays)
+    integ = B.Integrator(cfg)
+    integ.hold_corrections(*_dev(torch, arrays))
+    B.ai_set_normalization(integ.ctx, B.AI_NORM_SPLIT)
+    assert_profile(_got(*integ.integrate1d(torch.from_numpy(img).cuda())), want, what="held, split normalisation")
+    integ.close()
