@@ -70,6 +70,8 @@ def test_calls_before_build_are_refused(B):
     assert L.ai_integrate1d_host(ctx, dummy, B.AI_F32, None, None, None, None, None, dummy, dummy, dummy, None) \
         == B.AI_ENOTBUILT
     assert b"ai_build_csr" in L.ai_last_error(ctx)
+    assert L.ai_hold_corrections(ctx, dummy, None, None, None, None, None) == B.AI_ENOTBUILT
+    assert L.ai_hold_corrections(ctx, None, None, None, None, None, None) == B.AI_ENOTBUILT
     assert L.ai_set_options(ctx, B.AI_LAYOUT_LUT, B.AI_ACC_F64, 1.5) == B.AI_OK
     assert L.ai_set_options(ctx, 5, 0, 0.0) == B.AI_EINVAL
     assert L.ai_last_launch_count(ctx) == 0
@@ -80,6 +82,7 @@ def test_null_context_is_an_error_not_a_crash(B):
     L = B.lib()
     assert L.ai_build_csr(None, None) == B.AI_EINVAL
     assert L.ai_set_options(None, 0, 0, 0.0) == B.AI_EINVAL
+    assert L.ai_hold_corrections(None, None, None, None, None, None, None) == B.AI_EINVAL
     assert L.ai_integrate1d(None, None, 0, None, None, None, None, None, None, None, None, None, None) == B.AI_EINVAL
     assert L.ai_strerror(B.AI_ECUDA) == b"CUDA error" and L.ai_strerror(123) == b"unknown status"
     assert L.ai_last_error(None) == b""
