@@ -246,3 +246,52 @@ def test_fl_corrected_batches(torch, B, oracle, workloads, monkeypatch, dtype, n
         assert (want["count"] <= 0).sum() >= 3
         assert_profile(_row(i, s, c, f), want, what=f"corrected fl/{dtype}/frame {f} of {n}")
     integ.close()
+
+
+@pytest.mark.parametrize("mode", ["plain", "percall", "held"])
+def test_batch_sizes_around_the_kernel_thresholds(torch, B, oracle, workloads, mode):
+    """ai_integrate1d_batch splits a batch by measured cost: the frame-lane kernel takes the leading groups
+    of 64 frames and a tail that is long enough (plain 60 on this light matrix, per-call corrections 14, held 24), the rest
+    goes to the slice-per-lane kernel (plain) or frame by frame through the single-frame kernels (corrected).  Sizes on
+    both sides of every threshold, float frames with NaN / Inf pixels, sampled frames against the oracle, launch counts."""
+    cfg = workloads.tiny_config(200, 264, unit=workloads.TTH_DEG, name="thresholds", center_x=100.3, center_y=90.1,
+                                npt=120, distance_m=0.03)
+    rng = np.random.default_rng(5)
+    shape = (cfg.height, cfg.width)
+    dark = rng.poisson(5.0, shape).astype(np.float32)
+    flat = rng.uniform(0.9, 1.1, shape).astype(np.float32)
+    solid = rng.uniform(0.7, 1.0, shape).astype(np.float32)
+    pol = rng.uniform(0.95, 1.0, shape).astype(np.float32)
+    mask = (rng.random(shape) < 0.04).astype(np.uint8)
+    flat[10, 10] = 0.0
+    dark[60, 70] = np.nan
+    arrays = (dark, flat, solid, pol, mask) if mode != "plain" else (None,) * 5
+    dev = [None if a is None else torch.from_numpy(a).cuda() for a in arrays]
+    pool = rng.poisson(80.0, size=(5,) + shape).astype(np.float32)
+    pool[1, 33, 44] = np.nan
+    pool[3, 120, 7] = np.inf
+    umin, umax = oracle.pixel_bounds(cfg)
+    u0, u1 = oracle.auto_range(umin, umax)
+    want = [oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, pool[k], *arrays) for k in range(5)]
+    integ = B.Integrator(cfg)
+    if mode == "held":
+        integ.hold_corrections(*dev)
+    per_frame = {"percall": 3, "held": 2}          # launches of a frame that goes through the single-frame kernels
+    tail_min = {"plain": 60, "percall": 14, "held": 24}[mode]
+    first = True
+    for n in (32, 13, 14, 23, 24, 59, 60, 65, 77, 129):
+        frames = torch.from_numpy(pool[[k % 5 for k in range(n)]]).cuda()
+        i, s, c = integ.integrate1d_batch(frames, *(dev if mode == "percall" else [None] * 5))
+        torch.cuda.synchronize()
+        full, tail = n // 64 * 64, n % 64
+        taken = full + (tail if tail >= tail_min else 0)
+        expect = 0
+        if taken:
+            expect += 2 + (3 if mode == "percall" else 0) + (2 if mode == "held" and first else 0)
+            first = False
+        if n - taken:
+            expect += 2 if mode == "plain" and n - taken > 1 else (n - taken) * per_frame.get(mode, 2)
+        assert B.ai_last_launch_count(integ.ctx) == expect, (mode, n, taken)
+        for f in sorted({0, 1, n // 2, n - 2, n - 1}):
+            assert_profile(_row(i, s, c, f), want[f % 5], what=f"{mode} batch of {n}, frame {f}")
+    integ.close()
