@@ -165,6 +165,44 @@ int ai_integrate1d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *
                    const float *solidangle, const float *polarization, const uint8_t *mask, float *radial,
                    float *intensity, float *sum_signal, float *count, void *cuda_stream);
 
+/* ai_integrate1d for callers that must not allocate device memory once they are running.
+ *
+ * Why it exists: every other integrate entry may call cudaMalloc (and cudaFree, which waits for the whole device) the
+ * first time a call needs a library-owned buffer -- partial sums sized by the batch, a corrected copy of the frame, the
+ * padded table, the frame-lane layout.  That is no good for (a) a process where something else already owns all device
+ * memory (a framework's caching allocator, a fixed memory budget per tenant on a shared GPU): the library's own
+ * cudaMalloc fails there; (b) a real-time loop behind a detector: an allocation or a free in the middle of the run
+ * stalls every stream of the device, other people's too; (c) code that has to prove "nothing is allocated after
+ * start-up".  This entry calls no cudaMalloc, no cudaFree and no library routine that allocates, ever: its only scratch
+ * memory, the partial sums (16 bytes per record, `partial records per frame` of ai_get_layout_info), lives in a fixed
+ * array of AI_NOALLOC_SCRATCH_BYTES (8 MiB = 524 288 records) that is part of the library's device image -- every GPU
+ * that loads the library holds those 8 MiB until the process exits.  ai_setup / ai_build_csr still allocate the matrix:
+ * do them at start-up.
+ *
+ * Arguments, outputs and arithmetic as ai_integrate1d (all DEVICE pointers; AI_NORM_PIXEL; any ai_dtype; the accumulator
+ * of ai_set_options).  The layout option is ignored: the frame always takes the block-per-tile kernel pair of
+ * AI_LAYOUT_TILED_DIRECT (a memset of the records + 2 launches, plain stream ordering, no overlap between calls) and
+ * the profiles are bit-identical to that layout's -- slower than the default path (27.7 against 11.8 us per 2048 x 2048
+ * frame in a train of calls on a B200), which is the price of owning no per-context buffers.
+ *
+ * Limits and rules
+ *   - a matrix with more than AI_NOALLOC_SCRATCH_BYTES / 16 partial records is refused with AI_EUNSUPPORTED and a text
+ *     that names both sizes; nothing is launched.  For scale: 2048 x 2048 pixels with 1000 bins has 103 132 records, with
+ *     3000 bins in q 361 792 (both fit); 4096 x 4096 with 5000 bins has 851 154 (refused).  Bidimensional contexts,
+ *     AI_NORM_SPLIT and held corrections (pass the arrays instead) are refused likewise.
+ *   - the FIRST call made with a given device current asks the CUDA runtime where the array lives on that device (one
+ *     cudaGetSymbolAddress; the runtime may load the library's device code at that moment).  Make that first call during
+ *     start-up, outside any stream capture; later calls only enqueue.
+ *   - the array is shared by every context, stream and thread of the process on that device and keeps the last call's
+ *     records; each call clears what it needs first.  Two calls whose kernels can run on the GPU at the same time (two
+ *     streams, two host threads) therefore race on it and both results are garbage: keep all ai_integrate1d_noalloc
+ *     calls of a device on one stream, or order them with events.  Calls of the other entry points are not affected.
+ * Enqueues on `cuda_stream`; does not synchronise.  Errors: AI_EINVAL, AI_ENOTBUILT, AI_EUNSUPPORTED, AI_ECUDA. */
+#define AI_NOALLOC_SCRATCH_BYTES (8u << 20)
+int ai_integrate1d_noalloc(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *dark, const float *flat,
+                           const float *solidangle, const float *polarization, const uint8_t *mask, float *radial,
+                           float *intensity, float *sum_signal, float *count, void *cuda_stream);
+
 /* Integrate one frame into azimuthal x radial bins (a context made by ai_setup2d).  As ai_integrate1d, with
  *   radial       float32[npt_rad] bin centres, may be NULL        azimuthal   float32[npt_azim] bin centres in radians, may be NULL
  *   intensity, sum_signal, count   float32[npt_azim][npt_rad], row-major, required

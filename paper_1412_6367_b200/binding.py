@@ -22,7 +22,7 @@ AI_NORM_PIXEL, AI_NORM_SPLIT = range(2)
 AI_SPLIT_BBOX, AI_SPLIT_FULL = range(2)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_set_splitting", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_batch",
+EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_set_splitting", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_noalloc", "ai_integrate1d_batch",
            "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_hold_corrections", "ai_get_layout_info", "ai_get_batch_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
@@ -61,6 +61,7 @@ def lib():
     L.ai_set_normalization.argtypes = [vp, C.c_int]
     L.ai_set_splitting.argtypes = [vp, C.c_int]
     L.ai_integrate1d.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
+    L.ai_integrate1d_noalloc.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
     L.ai_integrate1d_batch.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_integrate1d_host.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_integrate1d_host_frames.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
@@ -176,6 +177,20 @@ def ai_integrate1d(ctx, image, dark, flat, solidangle, polarization, mask, radia
     _check(lib().ai_integrate1d(ctx, _ptr(image), dtype_code(image) if dtype is None else dtype, _ptr(dark),
                                 _ptr(flat), _ptr(solidangle), _ptr(polarization), _ptr(mask), _ptr(radial),
                                 _ptr(intensity), _ptr(sum_signal), _ptr(count), _stream(stream)), ctx)
+
+
+AI_NOALLOC_SCRATCH_BYTES = 8 << 20
+
+
+def ai_integrate1d_noalloc(ctx, image, dark, flat, solidangle, polarization, mask, radial, intensity, sum_signal, count,
+                           stream=None, dtype=None):
+    """ai_integrate1d for callers that must not allocate device memory while running (another component owns all of
+    it, or a cudaMalloc / cudaFree in mid-run would stall the device): the partial sums live in a fixed 8 MiB array
+    inside the library instead of a buffer the context allocates.  Same arguments; see include/azint.h for the limits
+    (matrix size, one stream per device, first call outside stream capture)."""
+    _check(lib().ai_integrate1d_noalloc(ctx, _ptr(image), dtype_code(image) if dtype is None else dtype, _ptr(dark),
+                                        _ptr(flat), _ptr(solidangle), _ptr(polarization), _ptr(mask), _ptr(radial),
+                                        _ptr(intensity), _ptr(sum_signal), _ptr(count), _stream(stream)), ctx)
 
 
 def ai_integrate1d_batch(ctx, frames, nframes, frame_stride_elems, dark, flat, solidangle, polarization, mask,
@@ -329,6 +344,16 @@ class Integrator:
                                p[0], p[1], p[2], self._raw_stream(self._dev_index))
         if rc != AI_OK:
             _check(rc, self.ctx)
+        return out
+
+    def integrate1d_noalloc(self, image, dark=None, flat=None, solidangle=None, polarization=None, mask=None, out=None,
+                            radial=None):
+        """integrate1d through ai_integrate1d_noalloc: no device allocation inside the library (scratch in the
+        library's fixed array).  Pass `out` to keep torch from allocating the outputs either."""
+        if out is None:
+            out = self.outputs()
+        ai_integrate1d_noalloc(self.ctx, image, dark, flat, solidangle, polarization, mask, radial, out[0], out[1],
+                               out[2], stream=self._raw_stream(self._dev_index), dtype=self._codes.get(image.dtype))
         return out
 
     def integrate2d(self, image, dark=None, flat=None, solidangle=None, polarization=None, mask=None, out=None,
