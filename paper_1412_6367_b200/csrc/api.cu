@@ -308,7 +308,9 @@ static int integrate(ai_ctx *ctx, const FrameArgs &args, cudaStream_t st)
     if (ctx->held.on && !a.dark && !a.flat && !a.solidangle && !a.polarization && !a.mask) {
         a.held = true;
         a.dark = ctx->held.dark;
-        if (ctx->held.has_den) a.flat = ctx->held.den;
+        // always with the denominator, also for a set that holds a dark current only: a pixel whose dark current is not
+        // finite is invalid for every frame, and the derived pair says so through den == 0 (its dark reads 0 there)
+        a.flat = ctx->held.den;
     }
     if (!a.image || !a.intensity || !a.sum_signal || !a.count) return ai_fail(ctx, AI_EINVAL, "NULL image or output");
     if ((int)a.dtype < AI_F32 || (int)a.dtype > AI_U32) return ai_fail(ctx, AI_EINVAL, "bad dtype %d", (int)a.dtype);

@@ -154,7 +154,6 @@ struct FlLayout {
 // ---- held corrections (hold.cu) ----------------------------------------------------------------------------------------
 struct HeldCorrections {
     bool on = false;
-    bool has_den = false;           // the set holds a denominator array or a mask (else only a dark current)
     uint8_t *gone = nullptr;        // [npix] 1 = invalid for every frame
     float *scale = nullptr;         // [4][npix], one allocation: 1 / den (0 where gone), then
     float *dark = nullptr;          //   the dark current (0 where gone),

@@ -137,7 +137,6 @@ int ai_hold_build(ai_ctx *ctx, const float *dark, const float *flat, const float
     }
     int rc = ai_launch_corr_prep(ctx, dark, flat, solidangle, polarization, mask, h.gone, h.scale, h.dark, h.keep, h.den, st);
     if (rc != AI_OK) return rc;
-    h.has_den = flat || solidangle || polarization || mask;
     const TiledLayout &tl = ctx->tl;
     h.tl_ready = false;
     if (tl.blob && tl.ntiles > 0 && tl.blob_bytes > 0) {      // (1D and 2D; whatever ai_set_options says now)

@@ -110,6 +110,39 @@ def test_held_subsets(torch, B, oracle, workloads, which):
     integ.close()
 
 
+@pytest.mark.parametrize("layout", ["tiled", "direct", "csr", "lut"])
+def test_held_dark_only_with_non_finite_pixels(torch, B, oracle, workloads, layout):
+    """A held set of a dark current alone whose NaN / Inf pixels are invalid for every frame (include/azint.h): the same
+    profiles on the held-aware kernel, on the kernels that see the set as a (dark, denominator) pair -- other layouts,
+    fp64 accumulation, 16-bit frames -- and with the array passed per call."""
+    cfg = workloads.tiny_config(130, 200, unit=workloads.Q_NM, name="held_dark", center_x=60.2, center_y=70.7, npt=150,
+                                distance_m=0.03)
+    rng = np.random.default_rng(31)
+    img = rng.poisson(200.0, size=(cfg.height, cfg.width)).astype(np.float32)
+    img16 = rng.poisson(300.0, size=(cfg.height, cfg.width)).astype(np.uint16)
+    dark = rng.poisson(5.0, size=img.shape).astype(np.float32)
+    dark[60, 70] = np.nan
+    dark[61, 170] = np.inf
+    dark[0, 0] = -np.inf
+    dark[100:104, 20:90] = np.nan                 # enough weight to move several bins far beyond the tolerance
+    arrays = (dark, None, None, None, None)
+    want = _oracle(oracle, cfg, img, arrays)
+    want16 = _oracle(oracle, cfg, img16, arrays)
+    integ = B.Integrator(cfg)
+    d_dark = torch.from_numpy(dark).cuda()
+    t, t16 = torch.from_numpy(img).cuda(), torch.from_numpy(img16.view(np.int16)).cuda()
+    assert_profile(_got(*integ.integrate1d(t, dark=d_dark)), want, what="dark per call")
+    integ.hold_corrections(dark=d_dark)
+    for accum in ("kahan", "f64"):
+        integ.set_options(LAYOUTS[layout], ACCUMS[accum], 0.0)
+        assert_profile(_got(*integ.integrate1d(t)), want, what=f"held dark only via {layout}/{accum}")
+        i, s, c = integ.outputs()
+        B.ai_integrate1d(integ.ctx, t16, None, None, None, None, None, None, i, s, c, dtype=B.AI_U16)
+        torch.cuda.synchronize()
+        assert_profile(_got(i, s, c), want16, what=f"held dark only, uint16 via {layout}/{accum}")
+    integ.close()
+
+
 def test_held_replaced_dropped_and_overridden(torch, B, oracle, workloads):
     """A second ai_hold_corrections replaces the set, all-NULL drops it, and a call with arrays of its own ignores it."""
     cfg = workloads.tiny_config(200, 264, unit=workloads.R_MM, name="held2", **SMALL)
