@@ -163,13 +163,25 @@ int ensure_segments(ai_ctx *ctx, cudaStream_t st)
         }
     }
     ptr[ctx->npt] = (int)seg.size();
-    ctx->csr_nseg = (int)seg.size();
+    // built into local pointers and published together once both copies have arrived: a failure half-way leaves the
+    // context without a table (the next call tries again), never with half of one
     const size_t n = seg.empty() ? 1 : seg.size();
-    AI_CUDA(ctx, cudaMalloc(&ctx->csr_seg, n * sizeof(int4)));
-    AI_CUDA(ctx, cudaMalloc(&ctx->csr_row_seg_ptr, ptr.size() * sizeof(int)));
-    AI_CUDA(ctx, cudaMemcpyAsync(ctx->csr_seg, seg.data(), seg.size() * sizeof(int4), cudaMemcpyHostToDevice, st));
-    AI_CUDA(ctx, cudaMemcpyAsync(ctx->csr_row_seg_ptr, ptr.data(), ptr.size() * sizeof(int), cudaMemcpyHostToDevice, st));
-    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    void *d_seg = nullptr;
+    int *d_ptr = nullptr;
+    cudaError_t e = cudaMalloc(&d_seg, n * sizeof(int4));
+    if (e == cudaSuccess) e = cudaMalloc(&d_ptr, ptr.size() * sizeof(int));
+    if (e == cudaSuccess && !seg.empty())
+        e = cudaMemcpyAsync(d_seg, seg.data(), seg.size() * sizeof(int4), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_ptr, ptr.data(), ptr.size() * sizeof(int), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+        cudaFree(d_seg);
+        cudaFree(d_ptr);
+        AI_CUDA(ctx, e);
+    }
+    ctx->csr_row_seg_ptr = d_ptr;
+    ctx->csr_nseg = (int)seg.size();
+    ctx->csr_seg = d_seg;
     return AI_OK;
 }
 
@@ -244,15 +256,25 @@ int dispatch_acc(Tag tag, ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 
 }  // namespace
 
+// frames ride on gridDim.y in these comparison layouts
+static int frames_fit_grid(ai_ctx *ctx, const FrameArgs &a)
+{
+    if (a.nframes > 65535) return ai_fail(ctx, AI_EUNSUPPORTED, "this layout takes at most 65535 frames per call (%d given)", a.nframes);
+    return AI_OK;
+}
+
 int ai_launch_csr(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 {
+    if (int rc = frames_fit_grid(ctx, a)) return rc;
     AI_DISPATCH(csr, ctx, a, st)
     return ai_fail(ctx, AI_EINVAL, "unknown dtype %d", (int)a.dtype);
 }
 
 int ai_launch_lut(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 {
-    int rc = ai_build_lut(ctx, st);
+    int rc = frames_fit_grid(ctx, a);
+    if (rc != AI_OK) return rc;
+    rc = ai_build_lut(ctx, st);
     if (rc != AI_OK) return rc;
     AI_DISPATCH(lut, ctx, a, st)
     return ai_fail(ctx, AI_EINVAL, "unknown dtype %d", (int)a.dtype);

@@ -135,6 +135,10 @@ __global__ void __launch_bounds__(256) scatter_finish_kernel(int npt, const doub
 int ai_launch_scatter(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st)
 {
     if (ctx->npt_azim > 0) return ai_fail(ctx, AI_EUNSUPPORTED, "the scatter comparison path is 1D only");
+    // the per-pixel geometry below is the bounding box's; with full pixel splitting it would disagree with the matrix
+    if (ctx->split == AI_SPLIT_FULL)
+        return ai_fail(ctx, AI_EUNSUPPORTED, "the scatter comparison path splits by bounding box only (context built with AI_SPLIT_FULL)");
+    if (a.nframes > 65535) return ai_fail(ctx, AI_EUNSUPPORTED, "this layout takes at most 65535 frames per call (%d given)", a.nframes);
     const int64_t n = (int64_t)ctx->height * ctx->width;
     if (!ctx->scat_first_nb) {
         // split geometry per pixel, from the same bounds as the matrix (one-time, synchronises)

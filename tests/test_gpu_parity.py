@@ -739,3 +739,21 @@ def test_error_codes_on_device(torch, B, workloads):
         B.ai_set_options(integ.ctx, 9, 0, 0.0)
     assert e.value.code == B.AI_EINVAL
     integ.close()
+
+
+@pytest.mark.parametrize("layout", ["csr", "lut", "scatter"])
+def test_comparison_layouts_refuse_more_frames_than_the_grid_holds(torch, B, workloads, layout):
+    """Frames ride on gridDim.y (<= 65535) in the comparison layouts: a larger batch is refused, not mis-launched."""
+    W = workloads
+    cfg = W.tiny_config(4, 4, center_x=2.0, center_y=2.0, unit=W.R_MM, npt=3, name="many_frames")
+    code = {"csr": B.AI_LAYOUT_CSR, "lut": B.AI_LAYOUT_LUT, "scatter": B.AI_LAYOUT_SCATTER}[layout]
+    integ = B.Integrator(cfg, layout=code)
+    n = 65536
+    frames = torch.ones((n, 4, 4), dtype=torch.float32, device="cuda")
+    with pytest.raises(B.AzintError) as e:
+        integ.integrate1d_batch(frames)
+    assert e.value.code == B.AI_EUNSUPPORTED and "65535" in str(e.value)
+    i, s, c = integ.integrate1d_batch(frames[:65535])
+    torch.cuda.synchronize()
+    assert torch.allclose(i, torch.ones_like(i), rtol=1e-6)
+    integ.close()

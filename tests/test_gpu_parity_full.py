@@ -79,3 +79,20 @@ def test_splitting_is_fixed_once_built(torch, B, workloads):
     with pytest.raises(B.AzintError):
         B.ai_set_splitting(integ.ctx, B.AI_SPLIT_FULL)
     integ.close()
+
+
+def test_scatter_layout_is_refused_with_full_splitting(torch, B, workloads):
+    """AI_LAYOUT_SCATTER splits by bounding box on the fly: on a context whose matrix was built with full pixel splitting
+    it would silently disagree with every other layout, so the call is refused."""
+    cfg = _cases(workloads)["centred"]
+    integ = B.Integrator(cfg, split=B.AI_SPLIT_FULL)
+    img = torch.ones((cfg.height, cfg.width), dtype=torch.float32, device="cuda")
+    integ.set_options(layout=B.AI_LAYOUT_SCATTER)
+    with pytest.raises(B.AzintError) as e:
+        integ.integrate1d(img)
+    assert e.value.code == B.AI_EUNSUPPORTED and "AI_SPLIT_FULL" in str(e.value)
+    integ.set_options()
+    i, s, c = integ.integrate1d(img)
+    torch.cuda.synchronize()
+    assert np.allclose(i.cpu().numpy()[c.cpu().numpy() > 0], 1.0, rtol=1e-6)
+    integ.close()
