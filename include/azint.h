@@ -103,7 +103,8 @@ int ai_setup(ai_ctx **out, const ai_geometry *g, int height, int width, int npt,
  * overlap / width along the radial unit times its overlap / width along chi.
  *   npt_rad, npt_azim    >= 1, npt_rad * npt_azim < 2^28
  *   range_or_null        HOST {u0, u1} in `unit`, NULL = automatic (as ai_setup)
- *   azim_range_or_null   HOST {chi0, chi1} in RADIANS, 0 < chi1 - chi0 <= 2 pi; NULL = the full circle [-pi, pi]
+ *   azim_range_or_null   HOST {chi0, chi1} in RADIANS, 0 < chi1 - chi0 <= 2 pi, -2 pi <= chi0, chi1 <= 3 pi; NULL = the
+ *                        full circle [-pi, pi]
  * Then ai_build_csr, ai_get_csr (rows = bins, row index a * npt_rad + r) and ai_integrate2d; ai_set_options applies
  * (AI_LAYOUT_LUT is not offered in 2D).  Errors: AI_EINVAL, AI_ENOMEM. */
 int ai_setup2d(ai_ctx **out, const ai_geometry *g, int height, int width, int npt_rad, int npt_azim, ai_unit unit,

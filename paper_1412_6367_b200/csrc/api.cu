@@ -116,8 +116,9 @@ int ai_setup2d(ai_ctx **out, const ai_geometry *g, int height, int width, int np
     if (azim_range_or_null && !(azim_range_or_null[1] > azim_range_or_null[0] && isfinite(azim_range_or_null[0]) &&
                                 isfinite(azim_range_or_null[1]) &&
                                 azim_range_or_null[1] - azim_range_or_null[0] <= two_pi * (1.0 + 1e-15) &&
-                                azim_range_or_null[0] >= -two_pi && azim_range_or_null[1] <= 2.0 * two_pi))
-        return AI_EINVAL;
+                                azim_range_or_null[0] >= -two_pi && azim_range_or_null[1] <= 1.5 * two_pi))
+        return AI_EINVAL;       // (a pixel's chi interval starts in [-pi, pi); its images shifted by -2 pi, 0 and +2 pi
+                                //  are what the builder looks at: together they cover [-3 pi, 3 pi])
     int rc = setup_common(out, g, height, width, npt_rad * npt_azim, unit, range_or_null);
     if (rc != AI_OK) return rc;
     (*out)->npt_rad = npt_rad;

@@ -94,6 +94,19 @@ __device__ __forceinline__ void azim_pieces(double lo, double w, double c0, doub
             out->f_lo[q] = f_lo; out->f_hi[q] = f_hi; out->first[q] = first; out->nb[q] = nb;
         }
     }
+    // One azimuthal bin over the full circle: the two images of a pixel across the seam fall into the same bin and would
+    // be two entries with one (bin, pixel) key.  They become one piece with the overlap of both: [ov - w, ov] in bin units
+    // has overlap ov (<= w) with bin 0 and width w.  With two bins or more the images land in different bins.
+    if (npt == 1 && out->n > 1) {
+        const double wf = __dsub_rn(out->f_hi[0], out->f_lo[0]);
+        double ov = 0.0;
+        for (int q = 0; q < out->n; ++q) ov = __dadd_rn(ov, split_overlap(out->f_lo[q], out->f_hi[q], 0, 1));
+        out->f_hi[0] = ov;
+        out->f_lo[0] = __dsub_rn(ov, wf);
+        out->first[0] = 0;
+        out->nb[0] = 1;
+        out->n = 1;
+    }
 }
 
 __global__ void __launch_bounds__(256) chi_kernel(ai_geometry g, int height, int width, double *__restrict__ chi_lo,

@@ -99,3 +99,19 @@ def test_no_cpu_fallback_without_a_gpu(B):
     from paper_1412_6367_b200 import workloads
     with pytest.raises(RuntimeError):
         B.Integrator(workloads.CONFIGS["cfg1"])
+
+
+def test_setup2d_azimuthal_range_limits(B):
+    """0 < chi1 - chi0 <= 2 pi inside [-2 pi, 3 pi] (include/azint.h): beyond 3 pi the builder's three images of a pixel
+    (shifted by -2 pi, 0, +2 pi) would leave bins silently empty, so such a range is refused at set-up."""
+    import math
+
+    def setup(rng):
+        return B.ai_setup2d(0.1, 1e-4, 1e-4, 8.0, 8.0, 1e-10, 16, 16, 5, 6, B.AI_R_MM, None, rng)
+    for ok in ((-math.pi, math.pi), (0.0, 2 * math.pi), (-2 * math.pi, 0.0), (math.pi, 3 * math.pi), (0.5, 1.5)):
+        B.ai_destroy(setup(ok))
+    for bad in ((1.5 * math.pi, 3.5 * math.pi), (2 * math.pi, 4 * math.pi), (-2.5 * math.pi, -1.0), (0.0, 7.0),
+                (1.0, 1.0), (2.0, 1.0), (0.0, float("nan"))):
+        with pytest.raises(B.AzintError) as e:
+            setup(bad)
+        assert e.value.code == B.AI_EINVAL, bad

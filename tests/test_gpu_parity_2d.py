@@ -41,6 +41,7 @@ def _cases(W):
         "seam_only": c("seam_only", 70, 130, 150.5, 33.3, 50, 90, W.Q_NM),   # beam right of the image: all chi near +-pi
         "off_image": c("off_image", 67, 259, -12.5, 300.0, 41, 180, W.TTH_DEG),
         "many_bins": c("many_bins", 48, 48, 24.0, 24.0, 64, 360),            # more bins than pixels near the centre
+        "one_azim_bin": c("one_azim_bin", 60, 72, 30.3, 29.6, 45, 1),        # pixels across the seam: both images in bin 0
     }
 
 
@@ -70,7 +71,8 @@ def _flat(want):
     return {k: np.asarray(want[k]).ravel() for k in ("intensity", "sum_signal", "count")}
 
 
-@pytest.mark.parametrize("name", ["centred", "inside_a_pixel", "on_an_edge", "seam_only", "off_image", "many_bins"])
+@pytest.mark.parametrize("name", ["centred", "inside_a_pixel", "on_an_edge", "seam_only", "off_image", "many_bins",
+                                  "one_azim_bin"])
 def test_csr2d_matches_oracle(torch, B, oracle, workloads, parity_report, name):
     cfg = _cases(workloads)[name]
     integ = B.Integrator(cfg)
@@ -89,7 +91,8 @@ def test_csr2d_matches_oracle(torch, B, oracle, workloads, parity_report, name):
 
 
 @pytest.mark.parametrize("layout", ["tiled", "direct", "csr"])
-@pytest.mark.parametrize("name", ["centred", "inside_a_pixel", "on_an_edge", "seam_only", "off_image", "many_bins"])
+@pytest.mark.parametrize("name", ["centred", "inside_a_pixel", "on_an_edge", "seam_only", "off_image", "many_bins",
+                                  "one_azim_bin"])
 def test_profile2d_parity_small(torch, B, oracle, workloads, name, layout):
     cfg = _cases(workloads)[name]
     rng = np.random.default_rng(11)
