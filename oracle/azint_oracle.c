@@ -26,7 +26,9 @@
  * SURVEY.md section 8(a).  The bidimensional routines at the end of the file are pinned in tests/test_oracle_pins_2d.py:
  * the sum over the azimuthal bins equals the (pinned) 1D result bin by bin, per-pixel weights sum to 1, conservation,
  * a hand-worked 2x2 image, 4-fold symmetry, mpmath brute force of the azimuthal extents (seam, centre inside / on an
- * edge / on a corner).  Unpinned: behaviour for non-finite inputs and <= 1 ulp bin-edge ties (reported, not asserted).
+ * edge / on a corner).  Non-finite inputs (a NaN / Inf pixel, dark current or denominator = an invalid pixel, DESIGN.md
+ * reading 8) are pinned as "exactly the result of masking that pixel" (tests/test_oracle_pins.py); <= 1 ulp bin-edge ties
+ * are reported, not asserted.
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).  No fast-math; IEEE double throughout.
  */
@@ -609,6 +611,46 @@ int64_t aio_csr_full(const double *u4, const double *chi4, const uint8_t *has_qu
     int64_t nnz = indptr[npt];
     free(len);
     return nnz;
+}
+
+/*
+ * Full pixel splitting, one frame, as the paper states it (section 4.2): a loop over the PIXELS; for each
+ * pixel "loops over the bins that the pixel spans", the slice areas give the pixel's contribution to each of those bins
+ * (aio_split_full above; the bounding box of aio_split for a pixel without a quadrilateral), and "contributions to the
+ * histograms are calculated using these areas": the weighted histogram gets c v, the unweighted one c,
+ * v and the pixel's validity from O5 (pixel_value).  Then O7.  A forward scatter like aio_integrate1d_bounds, single
+ * thread, plain double sums in pixel order.
+ * Pins (tests/test_oracle_pins_full.py): uniform image -> constant profile; sum of sum_signal = sum of v and sum of count
+ * = number of valid pixels when the range holds every pixel; npt = 1 -> the mean; masked / invalid pixels
+ * leave both histograms; equal to (pinned aio_csr_full matrix) x v; equal to aio_integrate1d_bounds when no pixel has a
+ * quadrilateral.
+ */
+int aio_integrate1d_full(const double *u4, const double *chi4, const uint8_t *has_quad, const double *u_min,
+                         const double *u_max, int64_t npix, int npt, double u0, double u1,
+                         const double *image, const double *dark, const double *flat, const double *solidangle,
+                         const double *polarization, const uint8_t *mask, double empty_value,
+                         double *radial, double *intensity, double *sum_signal, double *count)
+{
+    if (npix < 1 || npt < 1 || !(u1 > u0) || !image) return -1;
+    int bins[AIO_MAX_SPLIT]; double coefs[AIO_MAX_SPLIT];
+    double delta = (u1 - u0) / (double)npt;
+    for (int b = 0; b < npt; ++b) sum_signal[b] = count[b] = 0.0;
+    for (int64_t p = 0; p < npix; ++p) {
+        double v;
+        if (!pixel_value(p, image, dark, flat, solidangle, polarization, mask, &v)) continue;
+        int n = has_quad[p] ? aio_split_full(u4 + 4 * p, chi4 + 4 * p, u0, u1, npt, bins, coefs, AIO_MAX_SPLIT)
+                            : aio_split(u_min[p], u_max[p], u0, u1, npt, bins, coefs, AIO_MAX_SPLIT);
+        if (n > AIO_MAX_SPLIT) return -3;
+        for (int k = 0; k < n; ++k) {
+            sum_signal[bins[k]] += coefs[k] * v;      /* weighted histogram   */
+            count[bins[k]] += coefs[k];               /* unweighted histogram */
+        }
+    }
+    for (int b = 0; b < npt; ++b) {
+        if (radial) radial[b] = u0 + ((double)b + 0.5) * delta;
+        intensity[b] = count[b] > 0.0 ? sum_signal[b] / count[b] : empty_value;
+    }
+    return 0;
 }
 
 int aio_num_threads_available(void)

@@ -50,6 +50,8 @@ def lib():
         L.aio_csr_full.argtypes = [dp, dp, u8p, dp, dp, C.c_int64, C.c_int, C.c_double, C.c_double,
                                    C.POINTER(C.c_int64), C.POINTER(C.c_int32), dp]
         L.aio_csr_full.restype = C.c_int64
+        L.aio_integrate1d_full.argtypes = [dp, dp, u8p, dp, dp, C.c_int64, C.c_int, C.c_double, C.c_double,
+                                           dp, dp, dp, dp, dp, u8p, C.c_double, dp, dp, dp, dp]
         _lib = L
     return _lib
 
@@ -273,23 +275,26 @@ def csr_full(cfg, u0=None, u1=None):
 
 
 def integrate1d_full(cfg, frame, empty=0.0):
-    """Full pixel splitting as matrix x corrected frame in float64: dict(radial, intensity, sum_signal, count)."""
-    import scipy.sparse as sp
-    indptr, indices, data, (u0, u1) = csr_full(cfg)
-    m = sp.csr_matrix((data, indices, indptr), shape=(cfg.npt, cfg.npix))
-    img = np.asarray(frame.image, dtype=np.float64).ravel()
-    num = img - (0.0 if frame.dark is None else np.asarray(frame.dark, dtype=np.float64).ravel())
-    den = np.ones_like(img)
-    for a in (frame.flat, frame.solidangle, frame.polarization):
-        if a is not None:
-            den = den * np.asarray(a, dtype=np.float64).ravel()
-    ok = np.isfinite(num) & np.isfinite(den) & (den != 0.0)
-    if frame.mask is not None:
-        ok &= np.asarray(frame.mask).ravel() == 0
-    v = np.where(ok, num / np.where(den != 0.0, den, 1.0), 0.0)
-    S, Cn = m @ v, m @ ok.astype(np.float64)
-    out = {"sum_signal": S, "count": Cn, "intensity": np.where(Cn > 0, S / np.where(Cn > 0, Cn, 1.0), empty),
-           "radial": u0 + (np.arange(cfg.npt) + 0.5) * (u1 - u0) / cfg.npt, "range": (u0, u1)}
+    """Full pixel splitting of one frame (aio_integrate1d_full: the per-pixel forward scatter of PAPER.md:126-130) over
+    the bounding-box automatic range: dict(radial, intensity, sum_signal, count).  Marshalling only."""
+    umin, umax = pixel_bounds(cfg)
+    u0, u1 = auto_range(umin, umax)
+    u4, c4, q = pixel_corners(cfg)
+    return integrate1d_full_corners(u4, c4, q, umin, umax, cfg.npt, u0, u1, frame.image, frame.dark, frame.flat,
+                                    frame.solidangle, frame.polarization, frame.mask, empty=empty)
+
+
+def integrate1d_full_corners(u4, c4, has_quad, umin, umax, npt, u0, u1, image, dark=None, flat=None, solidangle=None,
+                             polarization=None, mask=None, empty=0.0):
+    keep = [_d(u4), _d(c4), _m(has_quad), _d(umin), _d(umax), _d(image), _d(dark), _d(flat), _d(solidangle),
+            _d(polarization), _m(mask)]
+    out = {k: np.empty(npt) for k in ("radial", "intensity", "sum_signal", "count")}
+    po = [out[k].ctypes.data_as(C.POINTER(C.c_double)) for k in ("radial", "intensity", "sum_signal", "count")]
+    rc = lib().aio_integrate1d_full(keep[0][1], keep[1][1], keep[2][1], keep[3][1], keep[4][1], keep[3][0].size, npt,
+                                    u0, u1, *[k[1] for k in keep[5:]], empty, *po)
+    if rc:
+        raise ValueError(f"aio_integrate1d_full: {rc}")
+    out["range"] = (u0, u1)
     return out
 
 

@@ -443,3 +443,49 @@ def test_split_normalisation_against_scipy_products_and_closed_forms(oracle, wor
     r4 = oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, img, dark, None, None, None, mask)
     assert r3["intensity"] == pytest.approx(r4["intensity"], rel=1e-14)
     assert r3["sum_norm"] == pytest.approx(r4["count"], rel=1e-14)
+
+
+def test_non_finite_inputs_are_exactly_a_masked_pixel(oracle, workloads):
+    """DESIGN.md reading 8 of PAPER.md:240: a pixel whose numerator I - dark or whose denominator flat x solid angle x
+    polarisation is not finite (or whose denominator is 0) is an invalid pixel.  Hand case: each of a NaN pixel, an Inf
+    pixel, an Inf / NaN dark current, an Inf / NaN / zero flat, solid angle or polarisation gives bit for bit the profile of
+    the clean inputs with that one pixel masked -- also in count, which would keep the pixel's weight if only the signal
+    were dropped."""
+    W = workloads
+    cfg = W.tiny_config(12, 15, center_x=4.2, center_y=6.9, unit=W.TTH_DEG, npt=9)
+    rng = np.random.default_rng(77)
+    shape = (cfg.height, cfg.width)
+    clean = dict(image=rng.poisson(100.0, size=shape).astype(np.float64), dark=rng.poisson(5.0, size=shape).astype(np.float64),
+                 flat=rng.uniform(0.9, 1.1, size=shape), solidangle=rng.uniform(0.7, 1.0, size=shape),
+                 polarization=rng.uniform(0.95, 1.0, size=shape))
+    base_mask = (rng.random(shape) < 0.1).astype(np.uint8)
+    umin, umax = oracle.pixel_bounds(cfg)
+    u0, u1 = oracle.auto_range(umin, umax)
+
+    def run(arrays, mask):
+        return oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, arrays["image"], arrays["dark"], arrays["flat"],
+                                         arrays["solidangle"], arrays["polarization"], mask, empty=-1.0)
+    spot = (5, 7)
+    assert base_mask[spot] == 0
+    masked = base_mask.copy()
+    masked[spot] = 1
+    want = run(clean, masked)
+    unmasked = run(clean, base_mask)
+    assert np.abs(want["count"] - unmasked["count"]).max() > 0.1          # the pixel matters
+    cases = [("image", np.nan), ("image", np.inf), ("image", -np.inf), ("dark", np.inf), ("dark", np.nan),
+             ("flat", np.inf), ("flat", np.nan), ("flat", 0.0), ("solidangle", np.nan), ("solidangle", 0.0),
+             ("polarization", -np.inf), ("polarization", 0.0)]
+    for name, bad in cases:
+        arrays = {k: v.copy() for k, v in clean.items()}
+        arrays[name][spot] = bad
+        got = run(arrays, base_mask)
+        for k in ("sum_signal", "count", "intensity"):
+            assert np.array_equal(got[k], want[k]), (name, bad, k)
+    # Inf - Inf in the numerator, and a non-finite value under the mask (must stay harmless)
+    arrays = {k: v.copy() for k, v in clean.items()}
+    arrays["image"][spot] = np.inf
+    arrays["dark"][spot] = np.inf
+    arrays["image"][np.nonzero(base_mask)[0][0], np.nonzero(base_mask)[1][0]] = np.nan
+    got = run(arrays, base_mask)
+    for k in ("sum_signal", "count", "intensity"):
+        assert np.array_equal(got[k], want[k]), k

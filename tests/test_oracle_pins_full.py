@@ -117,3 +117,94 @@ def test_corner_geometry(oracle, workloads):
     assert q.tolist() == [1, 1, 1, 1, 0, 1, 1, 1, 1]
     # the pixel left of the centre crosses the seam: its corner angles stay within half a turn of one another
     assert np.ptp(c4[3]) < math.pi
+
+
+# ---- aio_integrate1d_full: the per-pixel forward scatter of PAPER.md:126-130 ------------------------------------------------
+def _full_cases(W):
+    return {"centred": W.tiny_config(16, 16, center_x=8.0, center_y=8.0, unit=W.R_MM, npt=23),
+            "offcentre_q": W.tiny_config(14, 18, center_x=5.3, center_y=9.6, unit=W.Q_NM, npt=31),
+            "offimage_tth": W.tiny_config(12, 20, center_x=-6.5, center_y=30.0, unit=W.TTH_DEG, npt=40)}
+
+
+def _corrected_frame(W, cfg, seed):
+    rng = np.random.default_rng(seed)
+    shape = (cfg.height, cfg.width)
+    return W.Frame(image=rng.poisson(300.0, size=shape).astype(np.float64),
+                   dark=rng.poisson(5.0, size=shape).astype(np.float64),
+                   flat=rng.uniform(0.9, 1.1, size=shape), solidangle=rng.uniform(0.7, 1.0, size=shape),
+                   polarization=rng.uniform(0.95, 1.0, size=shape), mask=(rng.random(shape) < 0.1).astype(np.uint8))
+
+
+def _value_and_validity(fr):
+    """O5 written out once more, for the pins only: v = (I - dark) / (flat solid pol), valid = unmasked."""
+    v = (fr.image - fr.dark) / (fr.flat * fr.solidangle * fr.polarization)
+    ok = fr.mask == 0
+    return np.where(ok, v, 0.0).ravel(), ok.ravel()
+
+
+@pytest.mark.parametrize("case", ["centred", "offcentre_q", "offimage_tth"])
+def test_full_profile_uniform_image_and_conservation(oracle, workloads, case):
+    """the splitting conserves the signal and the pixels.  Over the automatic range every pixel lies inside
+    the range, so sum_b sum_signal = sum_p v_p and sum_b count = number of valid pixels; a uniform image gives a constant
+    profile wherever a bin holds any pixel."""
+    W = workloads
+    cfg = _full_cases(W)[case]
+    fr = _corrected_frame(W, cfg, 3)
+    v, ok = _value_and_validity(fr)
+    out = oracle.integrate1d_full(cfg, fr)
+    assert out["sum_signal"].sum() == pytest.approx(v.sum(), rel=1e-12)
+    assert out["count"].sum() == pytest.approx(ok.sum(), rel=1e-12)
+    uni = oracle.integrate1d_full(cfg, W.Frame(image=np.full((cfg.height, cfg.width), 7.25)))
+    filled = uni["count"] > 0
+    assert filled.sum() >= cfg.npt // 2
+    assert uni["intensity"][filled] == pytest.approx(7.25, rel=1e-13)
+    assert np.all(uni["intensity"][~filled] == 0.0)
+    assert uni["count"].sum() == pytest.approx(cfg.npix, rel=1e-12)
+    u0, u1 = out["range"]
+    assert out["radial"] == pytest.approx(u0 + (np.arange(cfg.npt) + 0.5) * (u1 - u0) / cfg.npt, rel=1e-15)
+
+
+@pytest.mark.parametrize("case", ["centred", "offcentre_q", "offimage_tth"])
+def test_full_profile_equals_pinned_matrix_times_frame(oracle, workloads, case):
+    """The scatter and the (clipper-pinned) matrix of aio_csr_full are two routes to the same sums: S = M v, C = M valid.
+    A dropped validity test, a swapped mask polarity or a missing dark current in the scatter shows here."""
+    W = workloads
+    cfg = _full_cases(W)[case]
+    fr = _corrected_frame(W, cfg, 9)
+    v, ok = _value_and_validity(fr)
+    indptr, indices, data, _ = oracle.csr_full(cfg)
+    out = oracle.integrate1d_full(cfg, fr, empty=-3.0)
+    for b in range(cfg.npt):
+        cols, c = indices[indptr[b]:indptr[b + 1]], data[indptr[b]:indptr[b + 1]]
+        S, Cn = float(np.dot(c, v[cols])), float(np.dot(c, ok[cols].astype(np.float64)))
+        assert out["sum_signal"][b] == pytest.approx(S, rel=1e-12, abs=1e-12)
+        assert out["count"][b] == pytest.approx(Cn, rel=1e-12, abs=1e-12)
+        assert out["intensity"][b] == (pytest.approx(S / Cn, rel=1e-12) if Cn > 0 else -3.0)
+    # every pixel masked: both histograms empty, intensity = the empty value
+    dead = W.Frame(image=fr.image, mask=np.ones_like(fr.mask))
+    out = oracle.integrate1d_full(cfg, dead, empty=-3.0)
+    assert np.all(out["count"] == 0.0) and np.all(out["sum_signal"] == 0.0) and np.all(out["intensity"] == -3.0)
+
+
+def test_full_profile_one_bin_is_the_mean_and_no_quadrilateral_is_the_bounding_box(oracle, workloads):
+    W = workloads
+    cfg = W.tiny_config(14, 18, center_x=5.3, center_y=9.6, unit=W.TTH_DEG, npt=1)
+    fr = _corrected_frame(W, cfg, 21)
+    v, ok = _value_and_validity(fr)
+    out = oracle.integrate1d_full(cfg, fr)
+    assert out["count"][0] == pytest.approx(ok.sum(), rel=1e-13)
+    assert out["intensity"][0] == pytest.approx(v.sum() / ok.sum(), rel=1e-12)
+    # with no pixel given a quadrilateral the routine is bounding-box splitting: equal to the pinned 1D oracle
+    cfg = _full_cases(W)["offcentre_q"]
+    fr = _corrected_frame(W, cfg, 22)
+    umin, umax = oracle.pixel_bounds(cfg)
+    u0, u1 = oracle.auto_range(umin, umax)
+    u4, c4, q = oracle.pixel_corners(cfg)
+    args = (fr.image, fr.dark, fr.flat, fr.solidangle, fr.polarization, fr.mask)
+    got = oracle.integrate1d_full_corners(u4, c4, np.zeros_like(q), umin, umax, cfg.npt, u0, u1, *args)
+    want = oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, *args)
+    for k in ("sum_signal", "count", "intensity"):
+        assert np.array_equal(got[k], want[k]), k
+    # ... and with the quadrilaterals it is not (the pin above would be empty otherwise)
+    full = oracle.integrate1d_full_corners(u4, c4, q, umin, umax, cfg.npt, u0, u1, *args)
+    assert np.abs(full["count"] - want["count"]).max() > 1e-3
