@@ -757,3 +757,53 @@ def test_comparison_layouts_refuse_more_frames_than_the_grid_holds(torch, B, wor
     torch.cuda.synchronize()
     assert torch.allclose(i, torch.ones_like(i), rtol=1e-6)
     integ.close()
+
+
+def test_train_with_a_producer_kernel_before_every_call(torch, B, workloads):
+    """include/azint.h (ai_integrate1d, reading 25 of DESIGN.md 3.2): consecutive calls overlap on the GPU, and a call may
+    read its frame as soon as the kernel enqueued right before it has completed or triggered its dependents early; an
+    ordinary kernel never triggers early, so it gives plain stream ordering.  The everyday pipeline "a kernel writes the
+    frame (decompression, a cast), then integrate": 200 calls on one buffer that an elementwise torch kernel rewrites
+    immediately before every call with one of two contents -- every profile bit-equal to the isolated call's."""
+    W = workloads
+    cfg = W.CONFIGS["cfg2"]
+    integ = B.Integrator(cfg)
+    src = [torch.from_numpy(W.make_frame(cfg, k).image).cuda() for k in range(2)]
+    ref = []
+    for k in range(2):
+        out = integ.integrate1d(src[k], out=integ.outputs())
+        torch.cuda.synchronize()
+        ref.append(out)
+    assert not torch.equal(ref[0][1], ref[1][1])
+    buf = torch.empty_like(src[0])
+    n = 200
+    outs = integ.outputs(n)
+    for k in range(n):
+        torch.mul(src[k % 2], 1.0, out=buf)                 # an ordinary kernel, same stream, no synchronisation
+        integ.integrate1d(buf, out=(outs[0][k], outs[1][k], outs[2][k]))
+    torch.cuda.synchronize()
+    assert B.ai_last_launch_count(integ.ctx) == 2           # the single-frame kernel chain, not a fallback
+    for k in range(n):
+        for q in range(3):
+            assert torch.equal(outs[q][k], ref[k % 2][q]), (k, q)
+    # the same with corrections: the library's own pre-pass sits between the producer and the stream kernel
+    cfg3 = W.CONFIGS["cfg3"]
+    fr = [W.make_frame(cfg3, k) for k in range(2)]
+    cor = [_dev(torch, x) for x in (fr[0].dark, fr[0].flat, fr[0].solidangle, fr[0].polarization, fr[0].mask)]
+    integ3 = B.Integrator(cfg3)
+    src = [_dev(torch, f.image) for f in fr]
+    ref = []
+    for k in range(2):
+        out = integ3.integrate1d(src[k], *cor, out=integ3.outputs())
+        torch.cuda.synchronize()
+        ref.append(out)
+    outs = integ3.outputs(n)
+    for k in range(n):
+        torch.mul(src[k % 2], 1.0, out=buf)
+        integ3.integrate1d(buf, *cor, out=(outs[0][k], outs[1][k], outs[2][k]))
+    torch.cuda.synchronize()
+    for k in range(n):
+        for q in range(3):
+            assert torch.equal(outs[q][k], ref[k % 2][q]), ("corrected", k, q)
+    integ.close()
+    integ3.close()

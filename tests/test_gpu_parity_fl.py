@@ -295,3 +295,41 @@ def test_batch_sizes_around_the_kernel_thresholds(torch, B, oracle, workloads, m
         for f in sorted({0, 1, n // 2, n - 2, n - 1}):
             assert_profile(_row(i, s, c, f), want[f % 5], what=f"{mode} batch of {n}, frame {f}")
     integ.close()
+
+
+@pytest.mark.parametrize("mode", ["percall", "held"])
+def test_corrected_batches_at_full_size(torch, B, oracle, workloads, mode):
+    """The configuration bench_extras times as batch_cfg3_*_frames_all_corrections: BASELINE.json configs[2] (2048 x 2048,
+    3000 bins in q, dark / flat / solid angle / polarisation / mask) in one ai_integrate1d_batch call of 128 frames, with
+    the arrays passed per call and held by the context.  14.6 M entries: the scaled copy of the frame-lane blobs, the
+    static count of the pixels that are invalid for every frame and the finish kernel at full size; sampled frames
+    against the oracle (PAPER.md:240 corrections, :122 sums)."""
+    W = workloads
+    cfg = W.CONFIGS["cfg3"]
+    pool = [W.make_frame(cfg, k) for k in range(3)]
+    arrays = (pool[0].dark, pool[0].flat, pool[0].solidangle, pool[0].polarization, pool[0].mask)
+    n = 128
+    frames = torch.empty((n, cfg.height, cfg.width), dtype=torch.float32, device="cuda")
+    dev_pool = [torch.from_numpy(p.image).cuda() for p in pool]
+    for f in range(n):
+        frames[f].copy_(dev_pool[f % 3])
+    frames[5, 700, 900] = float("nan")             # a frame's own invalid pixels on top of the static ones
+    frames[127, 12, 2040] = float("inf")
+    cor = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in arrays]
+    integ = B.Integrator(cfg)
+    if mode == "held":
+        integ.hold_corrections(*cor)
+        i, s, c = integ.integrate1d_batch(frames)
+    else:
+        i, s, c = integ.integrate1d_batch(frames, *cor)
+    torch.cuda.synchronize()
+    assert B.ai_get_batch_layout_info(integ.ctx)["built"] == 1          # the frame-lane kernel took the batch
+    umin, umax = oracle.pixel_bounds(cfg)
+    u0, u1 = oracle.auto_range(umin, umax)
+    for f in (0, 5, 64, 127):
+        img = frames[f].cpu().numpy()
+        want = oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, img, *arrays, nthreads=8)
+        assert_profile(_row(i, s, c, f), want, what=f"cfg3 x {n} {mode}, frame {f}")
+    # frames with the same content give the same bits wherever they sit in the batch
+    assert torch.equal(i[0], i[63]) and torch.equal(s[1], s[124]) and torch.equal(c[2], c[125])
+    integ.close()
