@@ -146,9 +146,7 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
 
     ms = time_batch64(integ)                  # one full group of 64 frames: the frame-lane kernel
     fl_info = B.ai_get_batch_layout_info(integ.ctx)
-    os.environ["AZINT_NO_FL"] = "1"
-    it_nofl = B.Integrator(cfg, device=device)
-    del os.environ["AZINT_NO_FL"]
+    it_nofl = B.Integrator(cfg, device=device, path={"no_fl": 1})
     ms_nofl = time_batch64(it_nofl)           # the slice-per-lane batch kernel on the same call
     it_nofl.close()
     abb = nb * cfg.npix * 4 + nnz * 8 + (cfg.npt + 1) * 4 + nb * 3 * cfg.npt * 4
@@ -159,7 +157,7 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
                                   "frac_of_peak": abb / (ms * 1e-3) / 1e9 / peak_gbs,
                                   "kernel": "fl_batch_kernel (one full group of 64 frames)" if fl_info.get("built") else
                                             "tiled_bstream_kernel",
-                                  "slice_per_lane_kernel_AZINT_NO_FL": {
+                                  "slice_per_lane_kernel_no_fl": {
                                       "ms_per_batch": ms_nofl, "us_per_frame": ms_nofl * 1e3 / nb,
                                       "frac_of_peak": abb / (ms_nofl * 1e-3) / 1e9 / peak_gbs,
                                       "partial_records_written_and_read_back": 2 * 16 * info["nslot"] * nb,
@@ -171,13 +169,9 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
     pool = torch.from_numpy(W.make_frames(c4, 8)).to(device)
     frames = pool.repeat(c4.nframes // 8, 1, 1)
 
-    def time_cfg4(env):
+    def time_cfg4(path):
         """ms per 1024-frame call (5 calls back to back after 2 warm-up calls) and the context, still open"""
-        for k, v in env.items():
-            os.environ[k] = v
-        it4 = B.Integrator(c4, device=device)
-        for k in env:
-            del os.environ[k]
+        it4 = B.Integrator(c4, device=device, path=path)
         out4 = it4.outputs(c4.nframes)
         for _ in range(2):
             it4.integrate1d_batch(frames, out=out4)
@@ -197,8 +191,8 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
     fl4 = B.ai_get_batch_layout_info(it.ctx)
     res_fl = [o.clone() for o in out]
     it.close()
-    # the same call through the slice-per-lane batched kernel (AZINT_NO_FL=1): what the frame-lane kernel replaced here
-    ms_sl, it, out = time_cfg4({"AZINT_NO_FL": "1"})
+    # the same call through the slice-per-lane batched kernel (ai_path_options.no_fl): what the frame-lane kernel replaced here
+    ms_sl, it, out = time_cfg4({"no_fl": 1})
     info4 = B.ai_get_layout_info(it.ctx)
     dmax = max(float(((a - b).abs() / b.abs().clamp_min(1e-30)).max()) for a, b in zip(res_fl[:2], out[:2]))
     it.close()
@@ -214,7 +208,7 @@ def run(torch, B, integ, cfg, frames_dev, flush, peak_gbs, args, device):
                                         {"partial_records_written_and_read_back": 2 * 16 * info4["nslot"] * c4.nframes},
                                     "layout": fl4,
                                     "vs_3000_fps_detector": c4.nframes / (ms * 1e-3) / 3000.0,
-                                    "slice_per_lane_kernel_AZINT_NO_FL": {
+                                    "slice_per_lane_kernel_no_fl": {
                                         "ms_per_batch": ms_sl, "frac_of_peak": ab4 / (ms_sl * 1e-3) / 1e9 / peak_gbs,
                                         "partial_records_written_and_read_back": 2 * 16 * info4["nslot"] * c4.nframes,
                                         "max_rel_diff_of_the_two_kernels_profiles": dmax},

@@ -114,6 +114,26 @@ int ai_setup2d(ai_ctx **out, const ai_geometry *g, int height, int width, int np
  * is already built), AI_EUNSUPPORTED (AI_SPLIT_FULL on a bidimensional context). */
 int ai_set_splitting(ai_ctx *ctx, ai_split split);
 
+/* Which kernels a context may use, for tests and measurements (every switch 0 = the library's own choice, which is what
+ * production code wants).  The library reads no environment variable: this call is the only way to re-route frames.
+ *   no_tma       frames are staged through registers even where a TMA tensor map applies
+ *   no_schedule  the sliced layout is built without its shared-memory bank scheduling
+ *   no_prepass   corrected single frames are corrected inside the general pipelined kernel, not by a pre-pass
+ *   no_stream    single frames take the general pipelined kernel instead of the single-frame kernel chain
+ *   no_fl        batches never take the frame-lane kernel         force_fl   batches of 32-bit frames always take it
+ *   no_overlap   every kernel of the single-frame chain waits for the kernel before it (no early reads of the frame)
+ *   fl_chunk     frame-lane layout: tiles per chunk (0 = chosen from the first batch's size)
+ *   fl_stages    frame-lane kernel: cap on its shared-memory stages (0 = none)
+ *   fl_owner     frame-lane layout: 1 = bins dealt to the warps longest first instead of round-robin
+ * Between ai_setup / ai_setup2d and ai_build_csr (some switches shape the layouts); NULL = all defaults.
+ * Errors: AI_EINVAL (matrix already built, negative sizes, no_fl with force_fl, a non-zero reserved field). */
+typedef struct {
+    int no_tma, no_schedule, no_prepass, no_stream, no_fl, force_fl, no_overlap;
+    int fl_chunk, fl_stages, fl_owner;
+    int reserved[6]; /* zero */
+} ai_path_options;
+int ai_set_path_options(ai_ctx *ctx, const ai_path_options *opt);
+
 /* Build the matrix on the device: bounds -> range -> count -> exclusive scan -> ordered fill (PAPER.md:120-122 for
  * the coefficients, :150 scan, :180 CSR), then the tiled execution layout.  Idempotent.  Synchronises `cuda_stream`.
  * Errors: AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED. */
@@ -158,7 +178,7 @@ int ai_set_normalization(ai_ctx *ctx, ai_norm norm);
  *     before it on the stream has completed OR has executed griddepcontrol.launch_dependents
  *     (cudaTriggerProgrammaticLaunchCompletion).  Memory copies, memsets and kernels that never trigger early -- every
  *     ordinary kernel -- give plain stream ordering.  A producer kernel that does trigger early must be followed by
- *     any ordinary stream operation before the call (or set AZINT_TUNE=nov:1, which makes every kernel wait).
+ *     any ordinary stream operation before the call (or build the context with ai_path_options.no_overlap = 1).
  * Between calls the context keeps corrected copies of the frame, partial sums and ticket counters: one context is used
  * by one host thread and on one stream at a time (different contexts are independent), on the device it was built on
  * (AI_EINVAL otherwise). */

@@ -22,13 +22,23 @@ AI_NORM_PIXEL, AI_NORM_SPLIT = range(2)
 AI_SPLIT_BBOX, AI_SPLIT_FULL = range(2)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_set_splitting", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_noalloc", "ai_integrate1d_batch",
+EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_set_splitting", "ai_set_path_options", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_noalloc", "ai_integrate1d_batch",
            "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_hold_corrections", "ai_get_layout_info", "ai_get_batch_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
 class ai_geometry(C.Structure):
     _fields_ = [(n, C.c_double) for n in
                 ("distance_m", "pixel_y_m", "pixel_x_m", "center_y_px", "center_x_px", "wavelength_m")]
+
+
+class ai_path_options(C.Structure):
+    _fields_ = [(n, C.c_int) for n in ("no_tma", "no_schedule", "no_prepass", "no_stream", "no_fl", "force_fl",
+                                       "no_overlap", "fl_chunk", "fl_stages", "fl_owner")] + [("reserved", C.c_int * 6)]
+
+
+# Path options an Integrator applies when it is given none: empty in production.  The tests put switches here
+# (monkeypatch.setitem) to route the same calls through every kernel of the library.
+PATH_DEFAULTS = {}
 
 
 class AzintError(RuntimeError):
@@ -60,6 +70,7 @@ def lib():
     L.ai_set_options.argtypes = [vp, C.c_int, C.c_int, C.c_float]
     L.ai_set_normalization.argtypes = [vp, C.c_int]
     L.ai_set_splitting.argtypes = [vp, C.c_int]
+    L.ai_set_path_options.argtypes = [vp, C.POINTER(ai_path_options)]
     L.ai_integrate1d.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
     L.ai_integrate1d_noalloc.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
     L.ai_integrate1d_batch.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
@@ -168,6 +179,16 @@ def ai_set_splitting(ctx, split=AI_SPLIT_BBOX):
     _check(lib().ai_set_splitting(ctx, split), ctx)
 
 
+def ai_set_path_options(ctx, **switches):
+    """ai_set_path_options(ctx, force_fl=1, fl_chunk=2, ...): see include/azint.h; no switches = all defaults."""
+    opt = ai_path_options()
+    for k, v in switches.items():
+        if k == "reserved" or not hasattr(opt, k):
+            raise AzintError(AI_EINVAL, f"unknown path option {k}")
+        setattr(opt, k, int(v))
+    _check(lib().ai_set_path_options(ctx, C.byref(opt)), ctx)
+
+
 def ai_set_normalization(ctx, norm=AI_NORM_PIXEL):
     _check(lib().ai_set_normalization(ctx, norm), ctx)
 
@@ -267,7 +288,7 @@ class Integrator:
     (e.g. workloads.Config).  Outputs are torch float32 CUDA tensors allocated here for convenience."""
 
     def __init__(self, cfg, radial_range=None, device=None, layout=AI_LAYOUT_TILED, accum=AI_ACC_F32_KAHAN,
-                 empty_value=0.0, azim_range=None, split=AI_SPLIT_BBOX):
+                 empty_value=0.0, azim_range=None, split=AI_SPLIT_BBOX, path=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1412_6367_b200 needs a CUDA device (no CPU fallback)")
@@ -299,6 +320,9 @@ class Integrator:
                                 cfg.wavelength_m, cfg.height, cfg.width, cfg.npt, cfg.unit, radial_range)
         if split != AI_SPLIT_BBOX:
             ai_set_splitting(self.ctx, split)
+        path = dict(PATH_DEFAULTS) if path is None else path
+        if path:
+            ai_set_path_options(self.ctx, **path)
         with torch.cuda.device(self.device):
             ai_build_csr(self.ctx)
         ai_set_options(self.ctx, layout, accum, empty_value)

@@ -156,43 +156,6 @@ static int setup_common(ai_ctx **out, const ai_geometry *g, int height, int widt
         ctx->range_host[0] = range_or_null[0];
         ctx->range_host[1] = range_or_null[1];
     }
-    const char *e = getenv("AZINT_NO_TMA");
-    ctx->no_tma = e && e[0] == '1';
-    e = getenv("AZINT_NO_SCHEDULE");
-    ctx->no_schedule = e && e[0] == '1';
-    e = getenv("AZINT_NO_PREPASS");
-    ctx->no_prepass = e && e[0] == '1';
-    e = getenv("AZINT_NO_STREAM");
-    ctx->no_stream = e && e[0] == '1';
-    e = getenv("AZINT_NO_FL");
-    ctx->no_fl = e && e[0] == '1';
-    e = getenv("AZINT_FORCE_FL");
-    ctx->force_fl = e && e[0] == '1';
-    if ((e = getenv("AZINT_TUNE")) != nullptr) {        // experiments only: "th:32,ms:6,is:8,bms:2,bis:8,fl:2"
-        for (const char *q = e; q && *q;) {
-            char key[8] = {0};
-            int val = 0;
-            if (sscanf(q, "%7[a-z]:%d", key, &val) == 2) {
-                if (!strcmp(key, "th")) ctx->tune.tile_h_max = val;
-                else if (!strcmp(key, "ms")) ctx->tune.mat_stages = val;
-                else if (!strcmp(key, "is")) ctx->tune.img_stages = val;
-                else if (!strcmp(key, "bms")) ctx->tune.batch_mat_stages = val;
-                else if (!strcmp(key, "bis")) ctx->tune.batch_img_stages = val;
-                else if (!strcmp(key, "fl")) ctx->tune.inflight = val;
-                else if (!strcmp(key, "ss")) ctx->tune.stream_stages = val;
-                else if (!strcmp(key, "nov")) ctx->tune.no_overlap = val;
-                else if (!strcmp(key, "fbs")) ctx->tune.fin_blocks_per_sm = val;
-                else if (!strcmp(key, "ncg")) ctx->tune.no_chain_guard = val;
-                else if (!strcmp(key, "bu")) ctx->tune.batch_units = val;
-                else if (!strcmp(key, "fls")) ctx->tune.fl_stages = val;
-                else if (!strcmp(key, "flc")) ctx->tune.fl_chunk = val;
-                else if (!strcmp(key, "flo")) ctx->tune.fl_owner = val;
-                else if (!strcmp(key, "flp")) ctx->tune.fl_prefetch = val;
-            }
-            q = strchr(q, ',');
-            if (q) ++q;
-        }
-    }
     *out = ctx;
     return AI_OK;
 }
@@ -278,6 +241,29 @@ int ai_set_options(ai_ctx *ctx, ai_layout layout, ai_accum accum, float empty_va
     ctx->layout = layout;
     ctx->accum = accum;
     ctx->empty_value = empty_value;
+    return AI_OK;
+}
+
+int ai_set_path_options(ai_ctx *ctx, const ai_path_options *opt)
+{
+    if (!ctx) return AI_EINVAL;
+    if (ctx->built) return ai_fail(ctx, AI_EINVAL, "path options are fixed once the matrix is built");
+    const ai_path_options none{};
+    const ai_path_options &o = opt ? *opt : none;
+    for (int r : o.reserved)
+        if (r != 0) return ai_fail(ctx, AI_EINVAL, "ai_path_options.reserved must be zero");
+    if (o.fl_chunk < 0 || o.fl_stages < 0 || (o.no_fl && o.force_fl))
+        return ai_fail(ctx, AI_EINVAL, "bad path options (negative size, or no_fl together with force_fl)");
+    ctx->no_tma = o.no_tma != 0;
+    ctx->no_schedule = o.no_schedule != 0;
+    ctx->no_prepass = o.no_prepass != 0;
+    ctx->no_stream = o.no_stream != 0;
+    ctx->no_fl = o.no_fl != 0;
+    ctx->force_fl = o.force_fl != 0;
+    ctx->tune.no_overlap = o.no_overlap != 0;
+    ctx->tune.fl_chunk = o.fl_chunk;
+    ctx->tune.fl_stages = o.fl_stages;
+    ctx->tune.fl_owner = o.fl_owner != 0;
     return AI_OK;
 }
 

@@ -50,8 +50,8 @@ struct PipePlan {
     bool fits;
 };
 inline int ai_align_up(int x, int a) { return (x + a - 1) / a * a; }
-// Tunables (defaults chosen by measurement; AZINT_TUNE="th:32,ms:6,is:8,fl:2" overrides them
-// for experiments): largest tile height tried, caps on the matrix / image stages, tiles in flight per block.
+// Tunables (defaults chosen by measurement; ai_set_path_options reaches the few that tests
+// need): largest tile height tried, caps on the matrix / image stages, tiles in flight per block.
 struct PipeTune {
     int tile_h_max = 64;
     int mat_stages = 3, img_stages = 6;        // single frame
@@ -255,12 +255,12 @@ struct ai_ctx {
 
     // measurement hook (ai_profile_enable): events around the dominant kernel of the last call
     PipeTune tune;
-    bool no_tma = false;            // AZINT_NO_TMA=1: stage raw frames through registers even where TMA applies (testing)
-    bool no_schedule = false;       // AZINT_NO_SCHEDULE=1: skip the bank scheduling of the sliced layout (measurement)
-    bool no_prepass = false;        // AZINT_NO_PREPASS=1: corrected single frames take the general kernel (testing)
-    bool no_stream = false;         // AZINT_NO_STREAM=1: single frames take the general pipelined kernel too (testing)
-    bool force_fl = false;          // AZINT_FORCE_FL=1: every batch of plain 32-bit frames takes the frame-lane kernel (testing)
-    bool no_fl = false;             // AZINT_NO_FL=1: large batches stay on the slice-per-lane batched kernel (testing)
+    bool no_tma = false;            // ai_path_options.no_tma: stage raw frames through registers even where TMA applies (testing)
+    bool no_schedule = false;       // ai_path_options.no_schedule: skip the bank scheduling of the sliced layout (measurement)
+    bool no_prepass = false;        // ai_path_options.no_prepass: corrected single frames take the general kernel (testing)
+    bool no_stream = false;         // ai_path_options.no_stream: single frames take the general pipelined kernel too (testing)
+    bool force_fl = false;          // ai_path_options.force_fl: every batch of plain 32-bit frames takes the frame-lane kernel (testing)
+    bool no_fl = false;             // ai_path_options.no_fl: large batches stay on the slice-per-lane batched kernel (testing)
     bool profile = false, profile_valid = false;
     bool stage1_only = false;       // ai_profile_enable(ctx, 2): launch only the dominant kernel
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;

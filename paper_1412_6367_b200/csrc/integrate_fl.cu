@@ -605,8 +605,8 @@ int launch_fl(ai_ctx *ctx, const CUtensorMap &map, const FlParams &p, size_t sme
 //     with more than 2.2 entries per pixel, 60 below;
 //   frames with per-call correction arrays, against frame-by-frame calls (cfg3 43, cfg2's matrix 34): 14 frames;
 //   frames against held corrections, against frame-by-frame calls (cfg3 25, cfg2's matrix 12.5): 24 frames.
-// A context that has not built the layout yet builds it for 32 frames or more.  AZINT_FORCE_FL=1 takes every batch
-// (testing), AZINT_NO_FL=1 none.
+// A context that has not built the layout yet builds it for 32 frames or more.  ai_path_options.force_fl takes every batch
+// (testing), ai_path_options.no_fl none.
 int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a0, int vec_ok, cudaStream_t st, int *taken)
 {
     *taken = 0;

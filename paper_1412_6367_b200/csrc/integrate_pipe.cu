@@ -51,23 +51,6 @@ struct PipeParams {
     void *partials;
 };
 
-// ---- development aid: per-block event trace (compiled in only with -DAI_PIPE_TRACE) -------
-#ifdef AI_PIPE_TRACE
-__device__ long long *g_trace = nullptr;          // [grid][kTraceItems][16] globaltimer stamps (ns)
-constexpr int kTraceItems = 16;
-__device__ __forceinline__ long long trace_now()
-{
-    long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-#define AI_TRACE(item, slot)                                                                             \
-    do {                                                                                                 \
-        if (g_trace && (item) < kTraceItems) g_trace[((size_t)blockIdx.x * kTraceItems + (item)) * 16 + (slot)] = trace_now(); \
-    } while (0)
-#else
-#define AI_TRACE(item, slot) do { } while (0)
-#endif
 
 // n-th item of this block: tiles (longest first) are dealt to the blocks in snake order
 __device__ __forceinline__ int item_at(int n)
@@ -250,7 +233,6 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
     // stage 2 is launched with programmatic stream serialisation: let its blocks be scheduled as SMs free up (they
     // wait in griddepcontrol.wait until this whole grid has completed)
     asm volatile("griddepcontrol.launch_dependents;");
-    if (threadIdx.x == 0) AI_TRACE(0, 15);
 
     ItemWalk walk;
     Ring mr, ir;                                     // matrix ring position of item n, image ring position of image ii
@@ -271,26 +253,21 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
             }
             for (int f = f0; f < f1; ++f) {
                 if (p.use_tma) {
-                    if (lane == 0) AI_TRACE(n, 0);
                     mbar_wait(img_empty + ir.stage, ir.parity ^ 1u);
                     if (lane == 0) {
-                        AI_TRACE(n, 1);
                         unsigned char *dst = img_base + (size_t)ir.stage * p.img_stage_bytes;
                         mbar_arrive_expect_tx(raw_full + ir.stage, (uint32_t)p.img_stage_bytes);
                         tma_box(dst, &tmap, tx * kTileW, ty * p.tile_h, f, raw_full + ir.stage);
                         tma_box(dst + p.img_stage_bytes / 2, &tmap, tx * kTileW + 32, ty * p.tile_h, f, raw_full + ir.stage);
-                        AI_TRACE(n, 2);
                     }
                     ir.next(p.img_stages);
                 }
                 if (f == f0) {
                     mbar_wait(mat_empty + mr.stage, mr.parity ^ 1u);
                     if (lane == 0) {
-                        AI_TRACE(n, 3);
                         mbar_arrive_expect_tx(mat_full + mr.stage, (uint32_t)d.y);
                         bulk_g2s(mat_base + (size_t)mr.stage * p.mat_stage_bytes, p.blob + (size_t)d.x * 16,
                                  (uint32_t)d.y, mat_full + mr.stage);
-                        AI_TRACE(n, 4);
                     }
                     mr.next(p.mat_stages);
                 }
@@ -298,23 +275,7 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
         }
     } else if (warp <= kStageWarps) {
         // ===== stagers: raw tile -> float32, corrected, invalid pixels as NaN ==========================================
-#ifdef AI_PIPE_TRACE
-        if (direct && warp == 1 && p.frames_per_item == 1) {   // monitor: when did each blob / image tile land?
-            for (int n = 0;; ++n) {
-                const int w = item_at(n);
-                if (w >= p.nitems) break;
-                const int4 d = win.get(p, n, lane);
-                if (d.w == 0) continue;
-                mbar_wait(raw_full + ir.stage, ir.parity);
-                if (lane == 0) AI_TRACE(n, 6);
-                mbar_wait(mat_full + mr.stage, mr.parity);
-                if (lane == 0) AI_TRACE(n, 5);
-                ir.next(p.img_stages);
-                mr.next(p.mat_stages);
-            }
-            return;
-        }
-#endif
+
         if (direct) return;
         const int sw = warp - 1, group = sw / kStageGroupWarps, tid = (sw % kStageGroupWarps) * 32 + lane;
         constexpr int kGroupThreads = kStageGroupWarps * 32;
@@ -336,9 +297,7 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
                 float *tile = reinterpret_cast<float *>(img_base + (size_t)ir.stage * p.img_stage_bytes);
                 bool bad;
                 if (p.use_tma) {
-                    if (tid == 0) AI_TRACE(ii, 5);
                     mbar_wait(raw_full + ir.stage, ir.parity);
-                    if (tid == 0) AI_TRACE(ii, 6);
                     bad = convert_tile_in_place<DT>(tile, p.tile_h * (kTileW / 4), tid, kGroupThreads);
                     fence_proxy_async();               // generic-proxy writes before the next TMA write to the stage
                 } else {
@@ -349,7 +308,6 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
                 }
                 if (bad) img_flag[ir.stage] = ii + 1;           // value-equal writers; read after the barrier
                 __syncwarp();
-                if (tid == 0) AI_TRACE(ii, 7);
                 if (lane == 0) mbar_arrive(img_ready + ir.stage);
                 ir.next(p.img_stages);
             }
@@ -371,14 +329,11 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
             // Every warp waits on and arrives at every barrier, also for items of which it holds no block: no warp
             // is ever a whole phase away from a barrier (parity waits would alias).
             const bool mine = first < d.w;
-            if (cw == 0 && lane == 0) AI_TRACE(n, 8);
             mbar_wait(mat_full + mr.stage, mr.parity);
-            if (cw == 0 && lane == 0) AI_TRACE(n, 9);
             const unsigned char *blob = mat_base + (size_t)mr.stage * p.mat_stage_bytes;
             const unsigned *hdr = reinterpret_cast<const unsigned *>(blob) + 1;
             for (int f = f0; f < f1; ++f, ++ii) {
                 mbar_wait(img_bar + ir.stage, ir.parity);
-                if (lane == 0 && (cw == 0 || cw == 8)) AI_TRACE(ii, cw ? 12 : 10);
                 if (mine) {
                     const float *tile = reinterpret_cast<const float *>(img_base + (size_t)ir.stage * p.img_stage_bytes);
                     void *part_f = reinterpret_cast<char *>(p.partials) + (int64_t)f * p.nslot * 16;
@@ -389,7 +344,6 @@ __global__ void __launch_bounds__(kPipeThreads, 1) tiled_pipe_kernel(const __gri
                             consume_block<ACC, true>(tile, blob, h, part_f, lane, false);
                     }
                     __syncwarp();
-                    if (lane == 0 && (cw == 0 || cw == 8 || cw == 15)) AI_TRACE(ii, cw == 0 ? 11 : cw == 8 ? 13 : 14);
                 }
                 if (lane == 0) mbar_arrive(img_empty + ir.stage);
                 ir.next(p.img_stages);
@@ -490,12 +444,6 @@ int launch_pipe_dt(ai_ctx *ctx, const CUtensorMap &map, const PipeParams &p, siz
 
 }  // namespace
 
-#ifdef AI_PIPE_TRACE
-extern "C" int ai_debug_set_trace(void *dev_buffer)
-{
-    return (int)cudaMemcpyToSymbol(g_trace, &dev_buffer, sizeof(void *));
-}
-#endif
 
 // Launches the pipelined stage 1 if a tile's blob fits the shared-memory ring (*handled = true); otherwise leaves
 // *handled false and the caller falls back to the one-block-per-tile kernel.

@@ -47,7 +47,8 @@ struct StreamParams {
                                  // stage's dark tile lies dk = stages x tile_bytes behind its frame tile (a multiple of 1024:
                                  // same 128-byte swizzle phase); img_stage_bytes = 2 tile_bytes
     int dyn_base;                // rank of the first tile handed out by ticket (the ones before are dealt statically)
-    int launch_index;            // launches of this context so far, modulo 8 (development trace only)
+    int launch_index;            // launches of this context so far, modulo 8 (not read by the kernel; kept so that the
+                                 // parameter block, and with it ptxas's allocation, stays what was measured)
     int track_all;               // float frames: every block skips non-finite pixels and accumulates count
     void *partials;
     unsigned long long *tickets;       // tile tickets of this launch (zero at its start)
@@ -59,30 +60,6 @@ struct StreamParams {
     unsigned long long chain_target;        // ended when *chain_done >= chain_target
 };
 
-// ---- development aid (-DAI_STREAM_TRACE): every warp of the single-frame kernel logs (globaltimer, code) events ----------
-#ifdef AI_STREAM_TRACE
-constexpr int kTraceWarps = 32, kTraceEvents = 64;
-__device__ long long *g_strace = nullptr;          // [8 launches][grid][kTraceWarps][kTraceEvents][2]
-struct WarpTrace {
-    long long *log;
-    int n;
-    __device__ void ev(long long code)
-    {
-        if (log && (threadIdx.x & 31) == 0 && n < kTraceEvents) {
-            log[2 * n] = (long long)globaltimer_ns();
-            log[2 * n + 1] = code;
-            ++n;
-        }
-    }
-};
-#define AI_TRACE_DECL(launch_index)                                                                                   \
-    WarpTrace wtrace{g_strace ? g_strace + ((((size_t)(launch_index) * gridDim.x + blockIdx.x) * kTraceWarps +          \
-                                              (threadIdx.x >> 5)) * kTraceEvents) * 2 : nullptr, 0}
-#define AI_TRACE(code) wtrace.ev(code)
-#else
-#define AI_TRACE_DECL(launch_index) do { } while (0)
-#define AI_TRACE(code) do { } while (0)
-#endif
 
 // n-th tile of this block: tiles (longest first) are dealt to the blocks in snake order
 __device__ __forceinline__ int stream_item_at(int n)
@@ -366,8 +343,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
     int4 *stage_desc = reinterpret_cast<int4 *>(hdr + kStreamDescOffset);   // descriptor of the tile in each stage
     unsigned char *mat_base = hdr + p.hdr_bytes;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    AI_TRACE_DECL(p.launch_index);
-    AI_TRACE(1);
 
     // Tiles, longest first: the first npre of every block are dealt statically (snake order; their descriptors came
     // with the launch), the rest are handed out by a ticket counter to whichever block has a free stage -- the blocks
@@ -451,7 +426,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
             if (!p.full_grid && blockIdx.x == 0) *p.tickets_reset = 0ULL;     // everything before this launch is complete
         }
     }
-    AI_TRACE(2);
 
     Ring r;
     if (warp == 0) {
@@ -490,7 +464,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
                 issue_blob(r.stage, d);
                 issue_tile(r.stage, d);
             }
-            AI_TRACE(100 + issued);
             ++issued;
             r.next(p.stages);
         }
@@ -510,7 +483,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
             // every warp waits on and arrives at every stage, also when it holds no block of the tile: no warp is
             // ever a whole phase away from a barrier
             mbar_wait(full + r.stage, r.parity);
-            AI_TRACE(100 + n);
             const int4 d = stage_desc[r.stage];
             if (d.w < 0) break;
             if (firstb < d.w) {
@@ -533,14 +505,12 @@ __global__ void __launch_bounds__(kStreamThreads, 1) tiled_stream_kernel(const _
                 }
                 __syncwarp();
             }
-            AI_TRACE(200 + n);
             if (lane == 0) mbar_arrive(empty + r.stage);
             firstb -= d.w % kStreamCons;
             if (firstb < 0) firstb += kStreamCons;
             r.next(p.stages);
         }
     }
-    AI_TRACE(9);
 }
 
 // ---- batches (H6): tiled_bstream_kernel ---------------------------------------------------------------------------------
@@ -743,13 +713,6 @@ int launch_stream_dt(ai_ctx *ctx, const CUtensorMap &map, const CUtensorMap *dma
 }  // namespace
 
 
-#ifdef AI_STREAM_TRACE
-extern "C" int ai_debug_set_stream_trace(void *dev_buffer)
-{
-    return (int)cudaMemcpyToSymbol(g_strace, &dev_buffer, sizeof(void *));
-}
-#endif
-
 // shared-memory plan: [tile stages][barriers + descriptors][blob stages]; false if fewer than two stages fit
 static bool stream_plan(const ai_ctx *ctx, int grid, StreamParams *p, bool held = false)
 {
@@ -822,7 +785,7 @@ int ai_launch_stream_stage1(ai_ctx *ctx, const FrameArgs &a, int vec_ok, int tra
     p.partials = static_cast<char *>(ctx->stream_partials) + (size_t)(seq & 1) * (size_t)(tl.nslot > 0 ? tl.nslot : 1) * 16;
     p.dyn_base = (p.stages < kStreamFirst ? p.stages : kStreamFirst) * grid;
     p.track_all = track_all;
-    p.launch_index = (int)(ctx->stream_launches & 7);   // development trace only: which of 8 trace buffers the launch writes
+    p.launch_index = (int)(ctx->stream_launches & 7);
     p.tickets = ctx->grid_sync + seq % 3;
     p.tickets_reset = ctx->grid_sync + (seq + 1) % 3;
     p.full_grid = grid == sms;

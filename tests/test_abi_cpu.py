@@ -115,3 +115,28 @@ def test_setup2d_azimuthal_range_limits(B):
         with pytest.raises(B.AzintError) as e:
             setup(bad)
         assert e.value.code == B.AI_EINVAL, bad
+
+
+def test_path_options_are_an_explicit_call_not_the_environment(B):
+    """The library reads no environment variable (plain C structs and enums): kernels are re-routed
+    only through ai_set_path_options, before the matrix is built."""
+    src = os.path.join(ROOT, "paper_1412_6367_b200", "csrc")
+    for name in os.listdir(src):
+        if name.endswith((".cu", ".cuh", ".h")):
+            assert "getenv" not in open(os.path.join(src, name)).read(), name
+    ctx = B.ai_setup(0.1, 1e-4, 1e-4, 8.0, 8.0, 1e-10, 16, 16, 10, B.AI_TTH_DEG)
+    B.ai_set_path_options(ctx, force_fl=1, fl_chunk=2, fl_stages=2)
+    B.ai_set_path_options(ctx)                                   # back to the defaults
+    L = B.lib()
+    assert L.ai_set_path_options(ctx, None) == B.AI_OK           # NULL = defaults
+    for bad in (dict(no_fl=1, force_fl=1), dict(fl_chunk=-1), dict(fl_stages=-2)):
+        with pytest.raises(B.AzintError) as e:
+            B.ai_set_path_options(ctx, **bad)
+        assert e.value.code == B.AI_EINVAL, bad
+    opt = B.ai_path_options()
+    opt.reserved[3] = 1
+    assert L.ai_set_path_options(ctx, C.byref(opt)) == B.AI_EINVAL
+    assert L.ai_set_path_options(None, None) == B.AI_EINVAL
+    with pytest.raises(B.AzintError):
+        B.ai_set_path_options(ctx, no_such_switch=1)
+    B.ai_destroy(ctx)

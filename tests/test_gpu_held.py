@@ -206,7 +206,7 @@ def test_held_batches(torch, B, oracle, workloads, monkeypatch, dtype, nframes):
     """Batches against a held set through the frame-lane kernel: the first call makes the scaled blobs and the static
     count (2 + 2 launches), later calls are the batch kernel and its finish kernel only; small batches take the general
     kernel with the (dark, denominator) pair."""
-    monkeypatch.setenv("AZINT_FORCE_FL", "1")
+    monkeypatch.setitem(B.PATH_DEFAULTS, "force_fl", 1)
     cfg = workloads.tiny_config(200, 264, unit=workloads.TTH_DEG, name="held4", **SMALL)
     rng = np.random.default_rng(29 + nframes)
     frames = rng.poisson(80.0, size=(nframes, cfg.height, cfg.width)).astype(dtype)
@@ -231,8 +231,8 @@ def test_held_batches(torch, B, oracle, workloads, monkeypatch, dtype, nframes):
     torch.cuda.synchronize()
     assert B.ai_last_launch_count(integ.ctx) == 4
     assert_profile(_got(i[63], s[63], c[63]), _oracle(oracle, cfg, frames[63], other), what="held batch, second set")
-    monkeypatch.setenv("AZINT_NO_FL", "1")
-    monkeypatch.delenv("AZINT_FORCE_FL")
+    monkeypatch.setitem(B.PATH_DEFAULTS, "no_fl", 1)
+    monkeypatch.delitem(B.PATH_DEFAULTS, "force_fl")
     small = B.Integrator(cfg)
     small.hold_corrections(*_dev(torch, arrays))
     i, s, c = small.integrate1d_batch(t[:3])

@@ -410,11 +410,11 @@ def _run_raw(torch, B, integ, img, dtype):
 @pytest.mark.parametrize("dtype", ["float32", "int32", "uint32"])
 @pytest.mark.parametrize("shape", [(256, 256), (130, 200), (70, 1028), (97, 131)])
 def test_single_frame_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, shape):
-    """AZINT_NO_STREAM=1 (read by ai_setup) sends single plain frames through the general pipelined kernel.  A width
+    """ai_path_options.no_stream sends single plain frames through the general pipelined kernel.  A width
     that is not a multiple of 4 (rows off 16-byte boundaries) reaches the single-frame kernel through the pre-pass,
     which re-pitches the frame."""
     if path == "pipe":
-        monkeypatch.setenv("AZINT_NO_STREAM", "1")
+        monkeypatch.setitem(B.PATH_DEFAULTS, "no_stream", 1)
     h, w = shape
     cfg = workloads.tiny_config(h, w, center_x=w * 0.41, center_y=h * 0.57, unit=workloads.Q_NM, npt=173,
                                 distance_m=0.02, name=f"single_{h}x{w}")
@@ -433,9 +433,9 @@ def test_single_frame_kernels(torch, B, oracle, workloads, monkeypatch, path, dt
 @pytest.mark.parametrize("shape", [(256, 256), (130, 200)])
 def test_corrected_frame_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, shape):
     """One frame with every correction array and a mask: by default H1 + H2 run as a pre-pass and the single-frame
-    kernel consumes the corrected frame; AZINT_NO_PREPASS=1 stages the corrections inside the general kernel."""
+    kernel consumes the corrected frame; ai_path_options.no_prepass stages the corrections inside the general kernel."""
     if path == "pipe":
-        monkeypatch.setenv("AZINT_NO_PREPASS", "1")
+        monkeypatch.setitem(B.PATH_DEFAULTS, "no_prepass", 1)
     h, w = shape
     cfg = workloads.tiny_config(h, w, center_x=w * 0.3, center_y=h * 0.6, unit=workloads.TTH_DEG, npt=211,
                                 distance_m=0.03, name=f"corr_{h}x{w}")
@@ -469,7 +469,7 @@ def test_non_finite_pixels_in_plain_float_frames(torch, B, oracle, workloads, mo
     """No mask, no corrections: NaN / Inf pixels are found lazily (a non-finite lane sum repeats the block with the
     tracked variant) and behave like masked pixels (oracle O5)."""
     if path == "pipe":
-        monkeypatch.setenv("AZINT_NO_STREAM", "1")
+        monkeypatch.setitem(B.PATH_DEFAULTS, "no_stream", 1)
     cfg = workloads.CONFIGS["cfg1b"]
     img = workloads.make_frame(cfg).image.copy()
     rng = np.random.default_rng(77)
@@ -504,13 +504,13 @@ def test_batch_matches_oracle_small(torch, B, oracle, workloads):
 @pytest.mark.parametrize("path", ["bstream", "pipe", "fl"])
 @pytest.mark.parametrize("dtype,nframes", [("int32", 7), ("float32", 6), ("uint32", 2), ("float32", 33)])
 def test_batch_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, nframes):
-    """Batches of plain 32-bit frames take the two-frames-at-a-time stream kernel; AZINT_NO_STREAM=1 sends them
-    through the general pipelined kernel, AZINT_FORCE_FL=1 through the frame-lane kernel (tests/test_gpu_parity_fl.py has
+    """Batches of plain 32-bit frames take the two-frames-at-a-time stream kernel; ai_path_options.no_stream sends them
+    through the general pipelined kernel, ai_path_options.force_fl through the frame-lane kernel (tests/test_gpu_parity_fl.py has
     more of those).  Odd counts leave a single last frame; float frames carry NaN / Inf."""
     if path == "pipe":
-        monkeypatch.setenv("AZINT_NO_STREAM", "1")
+        monkeypatch.setitem(B.PATH_DEFAULTS, "no_stream", 1)
     if path == "fl":
-        monkeypatch.setenv("AZINT_FORCE_FL", "1")
+        monkeypatch.setitem(B.PATH_DEFAULTS, "force_fl", 1)
     cfg = workloads.tiny_config(200, 264, center_x=100.3, center_y=90.1, unit=workloads.Q_NM, npt=257,
                                 distance_m=0.02, name="batch_small")
     rng = np.random.default_rng(nframes)
@@ -535,7 +535,7 @@ def test_batch_kernels(torch, B, oracle, workloads, monkeypatch, path, dtype, nf
 
 def test_batch_equals_single_frame_calls_bit_for_bit(torch, B, oracle, workloads):
     """BASELINE.json configs[1] frames through ai_integrate1d_batch in a small batch (the slice-per-lane batch kernel,
-    bench.py's `batch_cfg2_64_frames.slice_per_lane_kernel_AZINT_NO_FL`): every frame's profiles equal, bit for bit,
+    bench.py's `batch_cfg2_64_frames.slice_per_lane_kernel_no_fl`): every frame's profiles equal, bit for bit,
     what ai_integrate1d gives for it (same accumulation order in both kernels), and a sampled frame matches the oracle."""
     cfg = workloads.CONFIGS["cfg2"]
     base = workloads.make_frame(cfg).image
@@ -557,9 +557,9 @@ def test_batch_equals_single_frame_calls_bit_for_bit(torch, B, oracle, workloads
 @pytest.mark.parametrize("path", ["frame by frame", "general kernel"])
 def test_small_batch_with_mask(torch, B, oracle, workloads, monkeypatch, path):
     """A small batch with a mask: frame by frame through the pre-pass + single-frame kernel (3 launches per frame), or,
-    without the pre-pass (AZINT_NO_PREPASS=1), the general batched kernel that stages the corrections itself."""
+    without the pre-pass (ai_path_options.no_prepass), the general batched kernel that stages the corrections itself."""
     if path == "general kernel":
-        monkeypatch.setenv("AZINT_NO_PREPASS", "1")
+        monkeypatch.setitem(B.PATH_DEFAULTS, "no_prepass", 1)
     cfg = workloads.tiny_config(130, 200, center_x=60.0, center_y=70.0, unit=workloads.TTH_DEG, npt=150,
                                 distance_m=0.03, name="batch_mask")
     rng = np.random.default_rng(3)

@@ -1,7 +1,7 @@
 """Parity of the frame-lane batched kernel (integrate_fl.cu: lane = two frames) against the CPU
 oracle through the C ABI.  Large batches on matrices with more than ~2.2 entries per pixel take it by themselves
-(BASELINE.json configs[3]: test_gpu_parity.py::test_batch_full_size_sampled); AZINT_FORCE_FL=1 sends every batch of plain
-32-bit frames through it, AZINT_TUNE="flc:N,fls:N" cuts the chunks short / caps the stages so that small cases cover
+(BASELINE.json configs[3]: test_gpu_parity.py::test_batch_full_size_sampled); ai_path_options.force_fl sends every batch of plain
+32-bit frames through it, ai_path_options.fl_chunk / fl_stages cuts the chunks short / caps the stages so that small cases cover
 several work items per block and ring wrap-arounds.
 """
 import numpy as np
@@ -59,14 +59,15 @@ def _row(i, s, c, f):
 SMALL = dict(center_x=100.3, center_y=90.1, npt=257, distance_m=0.02)
 
 
-@pytest.mark.parametrize("tune", [None, "flc:2", "flc:1,fls:2", "flo:1"])
+@pytest.mark.parametrize("tune", [None, {"fl_chunk": 2}, {"fl_chunk": 1, "fl_stages": 2}, {"fl_owner": 1}])
 @pytest.mark.parametrize("dtype,nframes", [("int32", 7), ("int32", 64), ("uint32", 65), ("float32", 130)])
 def test_fl_batches_match_the_oracle(torch, B, oracle, workloads, monkeypatch, tune, dtype, nframes):
     """Every frame of a forced frame-lane batch against the oracle: one frame short of / one beyond a group of 64, a
     ragged image (264 = 8 tiles of 32 + 8 columns, 200 = 25 tiles of 8 rows), float frames with NaN and +-Inf."""
-    monkeypatch.setenv("AZINT_FORCE_FL", "1")
+    monkeypatch.setitem(B.PATH_DEFAULTS, "force_fl", 1)
     if tune:
-        monkeypatch.setenv("AZINT_TUNE", tune)
+        for k, v in tune.items():
+            monkeypatch.setitem(B.PATH_DEFAULTS, k, v)
     cfg = workloads.tiny_config(200, 264, unit=workloads.Q_NM, name="fl_small", **SMALL)
     rng = np.random.default_rng(nframes)
     frames = rng.poisson(100.0, size=(nframes, cfg.height, cfg.width)).astype(dtype)
@@ -87,7 +88,7 @@ def test_fl_batches_match_the_oracle(torch, B, oracle, workloads, monkeypatch, t
 def test_fl_bins_without_a_valid_pixel_are_empty(torch, B, oracle, workloads, monkeypatch):
     """A float frame whose centre region is NaN: the bins that only see that region have count exactly 0 and
     intensity = empty_value (the invalid weight is subtracted from the row's coefficient sum in fixed point)."""
-    monkeypatch.setenv("AZINT_FORCE_FL", "1")
+    monkeypatch.setitem(B.PATH_DEFAULTS, "force_fl", 1)
     cfg = workloads.tiny_config(128, 128, center_x=64.0, center_y=64.0, unit=workloads.R_MM, npt=90, name="fl_hole")
     rng = np.random.default_rng(5)
     frames = rng.poisson(30.0, size=(66, cfg.height, cfg.width)).astype(np.float32)
@@ -109,8 +110,8 @@ def test_fl_bins_without_a_valid_pixel_are_empty(torch, B, oracle, workloads, mo
 def test_fl_rows_do_not_depend_on_the_batch(torch, B, workloads, monkeypatch):
     """A frame's profiles are the same bits wherever it sits in a batch (which lane, which half of the lane, which
     group), whatever the other frames are, and from run to run: every sum has a fixed order."""
-    monkeypatch.setenv("AZINT_FORCE_FL", "1")
-    monkeypatch.setenv("AZINT_TUNE", "flc:3")
+    monkeypatch.setitem(B.PATH_DEFAULTS, "force_fl", 1)
+    monkeypatch.setitem(B.PATH_DEFAULTS, "fl_chunk", 3)
     cfg = workloads.tiny_config(200, 264, unit=workloads.TTH_DEG, name="fl_repro", **SMALL)
     rng = np.random.default_rng(11)
     pool = rng.poisson(200.0, size=(5, cfg.height, cfg.width)).astype(np.int32)
@@ -130,7 +131,7 @@ def test_fl_rows_do_not_depend_on_the_batch(torch, B, workloads, monkeypatch):
 def test_fl_compensation_keeps_small_terms(torch, B, workloads, monkeypatch):
     """PAPER.md:186-188 in the batched kernel: one pixel of 2^24 and 65535 pixels of 1 in one bin -- the per-product
     Kahan recurrence keeps every 1 (plain fp32 accumulation would lose those added after the big value)."""
-    monkeypatch.setenv("AZINT_FORCE_FL", "1")
+    monkeypatch.setitem(B.PATH_DEFAULTS, "force_fl", 1)
     cfg = workloads.scaled(workloads.CONFIGS["cfg1"], npt=1)
     img = np.ones((cfg.height, cfg.width), dtype=np.float32)
     img[0, 0] = 2.0 ** 24
@@ -145,7 +146,7 @@ def test_fl_compensation_keeps_small_terms(torch, B, workloads, monkeypatch):
 
 
 def test_fl_frame_stride_and_the_other_kernels_agree(torch, B, oracle, workloads, monkeypatch):
-    """Frames 12 elements apart more than a frame; the slice-per-lane batched kernel (AZINT_NO_FL=1) gives the same
+    """Frames 12 elements apart more than a frame; the slice-per-lane batched kernel (ai_path_options.no_fl) gives the same
     profiles within the tolerance (different, equally fixed, summation orders)."""
     cfg = workloads.tiny_config(200, 264, unit=workloads.R_MM, name="fl_stride", **SMALL)
     rng = np.random.default_rng(3)
@@ -153,14 +154,12 @@ def test_fl_frame_stride_and_the_other_kernels_agree(torch, B, oracle, workloads
     buf = rng.poisson(50.0, size=(n, stride)).astype(np.int32)
     t = torch.from_numpy(buf).cuda()
     out = {}
-    for name, env in (("fl", "AZINT_FORCE_FL"), ("slices", "AZINT_NO_FL")):
-        monkeypatch.setenv(env, "1")
-        integ = B.Integrator(cfg)
+    for name, switch in (("fl", "force_fl"), ("slices", "no_fl")):
+        integ = B.Integrator(cfg, path={switch: 1})
         i, s, c = integ.outputs(n)
         B.ai_integrate1d_batch(integ.ctx, t, n, stride, None, None, None, None, None, i, s, c)
         torch.cuda.synchronize()
         out[name] = (i.cpu().numpy(), s.cpu().numpy(), c.cpu().numpy())
-        monkeypatch.delenv(env)
         integ.close()
     for f in (0, 33, 66):
         img = buf[f, :cfg.npix].reshape(cfg.height, cfg.width)
@@ -201,15 +200,16 @@ def test_fl_full_size_geometries_sampled(torch, B, oracle, workloads, name):
     integ.close()
 
 
-@pytest.mark.parametrize("dtype,nframes,tune", [("int32", 7, None), ("float32", 100, "flc:2"), ("uint32", 66, None)])
+@pytest.mark.parametrize("dtype,nframes,tune", [("int32", 7, None), ("float32", 100, {"fl_chunk": 2}), ("uint32", 66, None)])
 def test_fl_corrected_batches(torch, B, oracle, workloads, monkeypatch, dtype, nframes, tune):
     """Batches with every correction array and a mask (one set for all frames) through the frame-lane
     kernel: the division is folded into a per-call copy of the coefficients, the loaders subtract the dark current as
     they stage the tiles.  Pixels invalid for every frame (masked, flat = 0 or not finite, a dark current that is not
     finite, a whole masked band that empties bins) leave the counts once per call; non-finite raw pixels per frame."""
-    monkeypatch.setenv("AZINT_FORCE_FL", "1")
+    monkeypatch.setitem(B.PATH_DEFAULTS, "force_fl", 1)
     if tune:
-        monkeypatch.setenv("AZINT_TUNE", tune)
+        for k, v in tune.items():
+            monkeypatch.setitem(B.PATH_DEFAULTS, k, v)
     cfg = workloads.tiny_config(200, 264, unit=workloads.TTH_DEG, name="fl_corr", **SMALL)
     rng = np.random.default_rng(17 + nframes)
     shape = (cfg.height, cfg.width)
