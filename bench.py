@@ -48,6 +48,8 @@ TRAINS = 9                     # timed trains of K steps; the median one is repo
 SPIN_UP = 600                  # calls a fresh process makes before its enqueue rate has settled (measured: ~300)
 # ncu's dram__bytes of one launch of the dominant kernel: written by the profiling run (profiles/r02_README.md)
 TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json")
+# dram bytes per call measured over back-to-back trains (ncu --replay-mode app-range, profiles/r03_README.md)
+IN_SITU_FILE = os.path.join(ROOT, "profiles", "r03_traffic_in_situ.json")
 
 
 def measured_peaks():
@@ -68,6 +70,15 @@ def ncu_traffic(kernel, workload):
     except (OSError, KeyError, ValueError):
         pass
     return None, None
+
+
+def in_situ_traffic(case):
+    """DRAM bytes per call of a whole step, measured by ncu over a train in which the calls overlap, or None."""
+    try:
+        with open(IN_SITU_FILE) as f:
+            return int(json.load(f)["cases"][case]["dram_bytes_per_call_in_situ"])
+    except (OSError, KeyError, ValueError):
+        return None
 
 
 def algorithmic_bytes(cfg, nnz, corrections=False):
@@ -427,6 +438,7 @@ def run_ours(args):
 
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
     traffic, traffic_src = ncu_traffic("tiled_stream_kernel", "cfg2")
+    step_traffic = in_situ_traffic("cfg2")
     extras["first_train_of_the_process"] = {
         "ms_per_step": first_ms / args.steps, "steps": args.steps,
         "note": "the first K-step train of this process, before the warm-up trains: the host enqueues its first ~300 "
@@ -459,6 +471,15 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak_gbs, "unit": "GB/s",
                      "frac": achieved / peak_gbs, "traffic": traffic,
                      "traffic_GBps": None if traffic is None else traffic / (k_ms * 1e-3) / 1e9,
+                     "traffic_frac": None if traffic is None else traffic / (k_ms * 1e-3) / 1e9 / peak_gbs,
+                     "frac_is": "ALGORITHMIC bytes (north_star's count: image + CSR coef/index/indptr + output, 8 B per "
+                                "entry) / kernel time / peak; the sliced layout stores 6.8 B per entry, so the bytes that "
+                                "really cross HBM are fewer: traffic_frac and whole_step_traffic_frac are that version",
+                     "whole_step_traffic_in_situ": step_traffic,
+                     "whole_step_traffic_frac": None if step_traffic is None
+                     else step_traffic / (ms_per_step * 1e-3) / 1e9 / peak_gbs,
+                     "whole_step_traffic_source": "profiles/r03_traffic_in_situ.json: dram__bytes over ncu app-range "
+                                                  "replays of 60- and 20-call trains, difference / 40",
                      "kernel": "tiled_stream_kernel", "traffic_source": traffic_src,
                      "kernel_ms": k_ms, "kernel_train_ms": k_all_ms,
                      "kernel_timing": f"median of {TRAINS} trains of K launches of the kernel alone "
