@@ -254,6 +254,16 @@ int ai_integrate1d_batch(ai_ctx *ctx, const void *frames, ai_dtype dtype, int nf
                          const float *dark, const float *flat, const float *solidangle, const float *polarization,
                          const uint8_t *mask, float *intensity, float *sum_signal, float *count, void *cuda_stream);
 
+/* Does now, at start-up, what ai_integrate1d_batch (and ai_integrate1d with correction arrays) would otherwise do inside the
+ * first call that needs it: builds the frame-lane layout for batches of up to `max_frames` frames (where it applies) and
+ * allocates the library-owned scratch of every kernel a batch of that size can take -- partial sums, the per-call arrays of
+ * corrected batches, the corrected frames of the pre-pass, the scaled blobs of a held set (call it after
+ * ai_hold_corrections then).  After it, calls with at most `max_frames` frames only enqueue: no cudaMalloc, no cudaFree,
+ * no host synchronisation (tests/test_gpu_parity_fl.py checks the device's free memory across such calls).  Optional: without
+ * it, or for a larger batch later, the lazy behaviour described above remains.  ai_set_options / ai_set_path_options should
+ * be final before the call.  Synchronises `cuda_stream`.  Errors: AI_EINVAL, AI_ENOTBUILT, AI_ENOMEM, AI_ECUDA. */
+int ai_prepare_batch(ai_ctx *ctx, int max_frames, void *cuda_stream);
+
 /* End-to-end variant: `image_host` and the three outputs are HOST pointers (pinned memory makes the copies
  * asynchronous); correction arrays and mask stay DEVICE pointers (they are per-detector constants, uploaded once, as in
  * PAPER.md:240-254 where only the image crosses the bus per frame).  Copies the frame host->device, integrates, copies

@@ -22,7 +22,7 @@ AI_NORM_PIXEL, AI_NORM_SPLIT = range(2)
 AI_SPLIT_BBOX, AI_SPLIT_FULL = range(2)
 AI_OK, AI_EINVAL, AI_ENOTBUILT, AI_ECUDA, AI_ENOMEM, AI_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_set_splitting", "ai_set_path_options", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_noalloc", "ai_integrate1d_batch",
+EXPORTS = ["ai_setup", "ai_setup2d", "ai_integrate2d", "ai_set_normalization", "ai_set_splitting", "ai_set_path_options", "ai_build_csr", "ai_get_csr", "ai_copy_csr_to_host", "ai_set_options", "ai_integrate1d", "ai_integrate1d_noalloc", "ai_integrate1d_batch", "ai_prepare_batch",
            "ai_integrate1d_host", "ai_integrate1d_host_frames", "ai_hold_corrections", "ai_get_layout_info", "ai_get_batch_layout_info", "ai_last_launch_count", "ai_profile_enable", "ai_profile_last", "ai_destroy", "ai_strerror", "ai_last_error"]
 
 
@@ -74,6 +74,7 @@ def lib():
     L.ai_integrate1d.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
     L.ai_integrate1d_noalloc.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, fp, vp]
     L.ai_integrate1d_batch.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
+    L.ai_prepare_batch.argtypes = [vp, C.c_int, vp]
     L.ai_integrate1d_host.argtypes = [vp, vp, C.c_int, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_integrate1d_host_frames.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int64, fp, fp, fp, fp, vp, fp, fp, fp, vp]
     L.ai_get_layout_info.argtypes = [vp, C.POINTER(C.c_int64)]
@@ -220,6 +221,12 @@ def ai_integrate1d_batch(ctx, frames, nframes, frame_stride_elems, dark, flat, s
                                       frame_stride_elems, _ptr(dark), _ptr(flat), _ptr(solidangle),
                                       _ptr(polarization), _ptr(mask), _ptr(intensity), _ptr(sum_signal), _ptr(count),
                                       _stream(stream)), ctx)
+
+
+def ai_prepare_batch(ctx, max_frames, stream=None):
+    """Builds the batch layout and allocates every scratch buffer for batches of up to max_frames frames now, so that the
+    batched calls that follow only enqueue (no allocation, no synchronisation)."""
+    _check(lib().ai_prepare_batch(ctx, max_frames, _stream(stream)), ctx)
 
 
 def ai_hold_corrections(ctx, dark, flat, solidangle, polarization, mask, stream=None):

@@ -379,6 +379,35 @@ int ai_integrate1d_batch(ai_ctx *ctx, const void *frames, ai_dtype dtype, int nf
     return integrate(ctx, a, (cudaStream_t)cuda_stream);
 }
 
+int ai_prepare_batch(ai_ctx *ctx, int max_frames, void *cuda_stream)
+{
+    if (!ctx) return AI_EINVAL;
+    if (!ctx->built) return ai_fail(ctx, AI_ENOTBUILT, "ai_build_csr has not been called");
+    if (max_frames < 1) return ai_fail(ctx, AI_EINVAL, "max_frames < 1");
+    int dev = -1;
+    AI_CUDA(ctx, cudaGetDevice(&dev));
+    if (dev != ctx->device)
+        return ai_fail(ctx, AI_EINVAL, "the matrix was built on device %d, the current device is %d", ctx->device, dev);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // partial records of the two-launch kernels (slice-per-lane batches, the general pipelined kernel)
+    const size_t need = (size_t)(ctx->tl.nslot > 0 ? ctx->tl.nslot : 1) * 16 * (size_t)max_frames;
+    if (ctx->partials_bytes < need) {
+        if (ctx->partials) AI_CUDA(ctx, cudaFree(ctx->partials));
+        ctx->partials = nullptr;
+        ctx->partials_bytes = 0;
+        AI_CUDA(ctx, cudaMalloc(&ctx->partials, need));
+        ctx->partials_bytes = need;
+    }
+    // the two corrected frames of the pre-pass (frames of a batch that go one by one)
+    const int pitch = (ctx->width + 3) / 4 * 4;
+    for (int i = 0; i < 2; ++i)
+        if (!ctx->corrected[i]) AI_CUDA(ctx, cudaMalloc(&ctx->corrected[i], (size_t)ctx->height * pitch * sizeof(float)));
+    int rc = ai_prepare_fl(ctx, max_frames, st);
+    if (rc != AI_OK) return rc;
+    AI_CUDA(ctx, cudaStreamSynchronize(st));
+    return AI_OK;
+}
+
 int ai_integrate1d_host(ai_ctx *ctx, const void *image_host, ai_dtype dtype, const float *dark, const float *flat,
                         const float *solidangle, const float *polarization, const uint8_t *mask,
                         float *intensity_host, float *sum_signal_host, float *count_host, void *cuda_stream)

@@ -317,6 +317,7 @@ int ai_launch_lut(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_launch_scatter(ai_ctx *ctx, const FrameArgs &a, cudaStream_t st);
 int ai_build_fl(ai_ctx *ctx, int nframes, cudaStream_t st);                          // build_fl.cu: frame-lane layout from the canonical CSR
 void ai_free_fl(FlLayout &fl);
+int ai_prepare_fl(ai_ctx *ctx, int max_frames, cudaStream_t st);                         // integrate_fl.cu
 int ai_launch_fl(ai_ctx *ctx, const FrameArgs &a, int vec_ok, cudaStream_t st, int *taken);   // integrate_fl.cu
 int ai_launch_corr_prep(ai_ctx *ctx, const float *dark, const float *flat, const float *solidangle, const float *polarization,
                         const uint8_t *mask, uint8_t *gone, float *scale, float *dark_out, uint32_t *keep, float *den_out,

@@ -594,6 +594,43 @@ int launch_fl(ai_ctx *ctx, const CUtensorMap &map, const FlParams &p, size_t sme
 
 }  // namespace
 
+// ai_prepare_batch (include/azint.h), the frame-lane part: builds the layout now (for batches of up to `max_frames`) and
+// allocates everything ai_launch_fl would otherwise allocate on the call that first needs it -- the partial sums for the
+// largest batch (with the invalid-pixel weights of float frames), the per-call arrays of corrected batches, the scaled
+// blobs of a held set.  Nothing here is needed for correctness: a later, larger batch still grows the buffers.
+int ai_prepare_fl(ai_ctx *ctx, int max_frames, cudaStream_t st)
+{
+    if (max_frames < 2 || ctx->no_fl || ctx->no_tma || ctx->no_stream || ctx->npt_azim > 0 ||
+        ctx->accum != AI_ACC_F32_KAHAN || ctx->layout != AI_LAYOUT_TILED)
+        return AI_OK;
+    if (!ctx->force_fl && max_frames < kFlMinFrames) return AI_OK;
+    FlLayout &fl = ctx->fl;
+    if (!fl.tried) {
+        int rc = ai_build_fl(ctx, max_frames, st);
+        if (rc != AI_OK) return rc;
+    }
+    if (!fl.ok) return AI_OK;
+    const size_t nfp = (size_t)((max_frames + kFlFrames - 1) / kFlFrames) * kFlFrames;
+    const size_t need = (size_t)fl.nslot * nfp * sizeof(float2) + (size_t)ctx->npt * nfp * sizeof(unsigned long long);
+    if (fl.partials_bytes < need) {
+        if (fl.partials) AI_CUDA(ctx, cudaFree(fl.partials));
+        fl.partials = nullptr;
+        fl.partials_bytes = 0;
+        AI_CUDA(ctx, cudaMalloc(&fl.partials, need));
+        fl.partials_bytes = need;
+    }
+    const int64_t npix = (int64_t)ctx->height * ctx->width;
+    if (!fl.call_csum) AI_CUDA(ctx, cudaMalloc(&fl.call_csum, (size_t)ctx->npt * sizeof(double)));
+    if (!fl.gone) AI_CUDA(ctx, cudaMalloc(&fl.gone, (size_t)npix));
+    if (!fl.scale) AI_CUDA(ctx, cudaMalloc(&fl.scale, 3 * (size_t)npix * sizeof(float)));
+    if (!fl.blob_call) AI_CUDA(ctx, cudaMalloc(&fl.blob_call, (size_t)fl.blob_bytes));
+    if (ctx->held.on) {
+        if (!ctx->held.fl_csum) AI_CUDA(ctx, cudaMalloc(&ctx->held.fl_csum, (size_t)ctx->npt * sizeof(double)));
+        if (!ctx->held.fl_blob) AI_CUDA(ctx, cudaMalloc(&ctx->held.fl_blob, (size_t)fl.blob_bytes));
+    }
+    return AI_OK;
+}
+
 // Batches of 32-bit frames, Kahan accumulation, 1D: *taken = the number of leading frames of the batch the frame-lane
 // kernel took (both launches); the caller sends the rest through the other kernels.  The first call that takes frames
 // builds the layout (one-time; synchronises `st`).

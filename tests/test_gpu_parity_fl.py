@@ -333,3 +333,46 @@ def test_corrected_batches_at_full_size(torch, B, oracle, workloads, mode):
     # frames with the same content give the same bits wherever they sit in the batch
     assert torch.equal(i[0], i[63]) and torch.equal(s[1], s[124]) and torch.equal(c[2], c[125])
     integ.close()
+
+
+@pytest.mark.parametrize("mode", ["plain", "percall", "held"])
+def test_prepared_batches_allocate_nothing(torch, B, oracle, workloads, mode):
+    """ai_prepare_batch (include/azint.h) moves the one-time work of the batched path to start-up: the frame-lane layout and
+    every scratch buffer a batch of up to max_frames frames can need.  After it the device's free memory does not move
+    across batches of any size up to that -- through the frame-lane kernel, the slice-per-lane kernel and the frame-by-frame
+    paths -- and the results are the oracle's."""
+    cfg = workloads.tiny_config(200, 264, unit=workloads.TTH_DEG, name="prepared", center_x=100.3, center_y=90.1,
+                                npt=120, distance_m=0.03)
+    rng = np.random.default_rng(11)
+    shape = (cfg.height, cfg.width)
+    arrays = (rng.poisson(5.0, shape).astype(np.float32), rng.uniform(0.9, 1.1, shape).astype(np.float32),
+              rng.uniform(0.7, 1.0, shape).astype(np.float32), rng.uniform(0.95, 1.0, shape).astype(np.float32),
+              (rng.random(shape) < 0.04).astype(np.uint8)) if mode != "plain" else (None,) * 5
+    dev = [None if a is None else torch.from_numpy(a).cuda() for a in arrays]
+    pool = rng.poisson(80.0, size=(4,) + shape).astype(np.float32)
+    pool[1, 33, 44] = np.nan
+    nmax = 130
+    frames = torch.from_numpy(pool[[k % 4 for k in range(nmax)]]).cuda()
+    integ = B.Integrator(cfg)
+    if mode == "held":
+        integ.hold_corrections(*dev)
+    call_arrays = dev if mode == "percall" else [None] * 5
+    outs = {n: integ.outputs(n) for n in (130, 64, 40, 5, 2)}
+    assert B.ai_get_batch_layout_info(integ.ctx)["built"] == 0
+    B.ai_prepare_batch(integ.ctx, nmax)
+    assert B.ai_get_batch_layout_info(integ.ctx)["built"] == 1
+    torch.cuda.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    for n in (130, 64, 40, 5, 2, 130):
+        integ.integrate1d_batch(frames[:n], *call_arrays, out=outs[n])
+    torch.cuda.synchronize()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free1 == free0, f"{mode}: {free0 - free1} bytes of device memory were allocated after ai_prepare_batch"
+    umin, umax = oracle.pixel_bounds(cfg)
+    u0, u1 = oracle.auto_range(umin, umax)
+    want = [oracle.integrate1d_bounds(umin, umax, cfg.npt, u0, u1, pool[k], *arrays) for k in range(4)]
+    for n in (130, 40, 5):
+        i, s, c = outs[n]
+        for f in sorted({0, 1, n // 2, n - 1}):
+            assert_profile(_row(i, s, c, f), want[f % 4], what=f"prepared {mode} batch of {n}, frame {f}")
+    integ.close()
