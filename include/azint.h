@@ -240,7 +240,8 @@ int ai_integrate2d(ai_ctx *ctx, const void *image, ai_dtype dtype, const float *
  * Enqueues on `cuda_stream`; does not synchronise -- with one exception: the first batch that sends 32 or more 32-bit
  * frames to the frame-lane kernel (1D context, Kahan accumulation, every array on a 16-byte boundary)
  * builds the frame-lane layout of the matrix (one-time, synchronises `cuda_stream`; see ai_get_batch_layout_info), and a
- * larger batch than any before re-allocates scratch (cudaFree synchronises the device).
+ * larger batch than any before re-allocates scratch (cudaFree synchronises the device).  ai_prepare_batch does both ahead
+ * of time: after it, batches of up to its max_frames only enqueue.
  * Which kernels a batch takes is decided by measured cost: the frame-lane kernel takes the leading groups
  * of 64 frames and the remaining frames if they are many enough (plain frames 44 or 60, frames with per-call correction
  * arrays 14, with held corrections 24); the rest goes to the slice-per-lane batch kernel (plain 32-bit frames) or frame
